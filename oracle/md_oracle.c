@@ -1,0 +1,567 @@
+/*
+ * md_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+ *
+ * A plain, slow, fp64 CPU statement of what the neighbor-list MD hot path of
+ * "JAX, M.D." (arXiv 1912.04232; /root/reference/PAPER.md) computes, written
+ * from the paper's definitions.  It shares no code, header, table or helper
+ * with the CUDA path (paper_1912_04232_b200/csrc) and neither includes the
+ * other.  Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline /
+ * --impl reference legs may load it.
+ *
+ * What each function follows (PAPER.md line, section):
+ *   orc_neighbor_list   L84 §3.2.3 "pairs (i,j) such that ||r_i - r_j|| < sigma";
+ *                       dense N x N_nbrs rows L74 §3.2.1; static capacity L47 §3.1
+ *   orc_cell_list       L84 "places them into cells where each cell has size sigma"
+ *   orc_energy_force    L78 §3.2.2  U = 1/2 sum_{i!=j} u(r_i - r_j),  m r'' = -grad U;
+ *                       L104 §3.3.2 Lennard-Jones, soft-sphere; force = -grad U;
+ *                       L301 App. A  sigma_AB = (sigma_A + sigma_B)/2
+ *   orc_needs_rebuild   L49 §3.1 "whenever a particle moves by more than the halo"
+ *   orc_nve_run         L100 §3.3.1 NVE (init, update);  L72 shift function mu
+ *   displacement        L72 §3.2.1 "displacement between a particle and the
+ *                       nearest image of the second particle"
+ * Readings of everything the paper leaves open (strict <, half-skin, truncated
+ * and shifted LJ, wrap convention, rounding of the inclusion predicate) are
+ * SURVEY.md §8c A1-A18, restated in DESIGN.md §3.
+ *
+ * Parity pins (tests/test_oracle_pins.py): every function here is pinned to
+ * something other than itself -- FCC shell counts and lattice sums, two-body
+ * closed forms, finite differences, Newton's third law, translation
+ * invariance, scipy's periodic cKDTree, NVE invariants, the harmonic
+ * oscillator's exact discrete frequency.  The one unpinned thing is a chaotic
+ * trajectory beyond ~100 steps ("parity unpinned" by design).
+ *
+ * Arithmetic: fp64 everywhere, except the canonical inclusion predicate
+ * (predicate = 0), which is evaluated in singly-rounded fp32 because it decides
+ * an integer (set membership) that the fp32 GPU path must reproduce to the
+ * bit.  Build with -ffp-contract=off (no implicit FMA).
+ *
+ * Positions are double[n*3] (z ignored in 2-D); box is double[3]; diameters
+ * double[n]; indices int32.  Rows of a neighbor list are ascending, padded
+ * with n.  OpenMP only splits the outer loop over particles; there is no
+ * blocking, fusion or reordering beyond the definitions.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+#define ORC_OK 0
+#define ORC_EINVAL (-1)
+#define ORC_ENOMEM (-2)
+
+#define KIND_LJ 0
+#define KIND_SOFT 1
+
+int orc_num_threads(void)
+{
+#ifdef _OPENMP
+    return omp_get_max_threads();
+#else
+    return 1;
+#endif
+}
+
+void orc_set_num_threads(int t)
+{
+#ifdef _OPENMP
+    if (t > 0) omp_set_num_threads(t);
+#else
+    (void)t;
+#endif
+}
+
+/* ---------------------------------------------------------------- space -- */
+
+/* fp64 nearest-image displacement a - b, one component. */
+static double disp64(double a, double b, double L)
+{
+    double d = a - b;
+    return d - L * round(d / L);
+}
+
+/* Canonical fp32 nearest-image displacement, one component:
+ * every operation singly rounded; the inner subtraction of L is exact. */
+static float disp32(float xi, float xj, float L)
+{
+    float h = L / 2.0f;
+    float d = xi - xj;
+    if (d > h) {
+        float t = xi - L;
+        d = t - xj;
+    } else if (d < -h) {
+        float t = xj - L;
+        d = xi - t;
+    }
+    return d;
+}
+
+/* Shift function mu(r, dr) folded into [0, L). */
+static double wrap64(double x, double L)
+{
+    x = x - L * floor(x / L);
+    if (x >= L) x = 0.0;
+    if (x < 0.0) x = 0.0;
+    return x;
+}
+
+/* fp32 list radius R = fl(fl32(r_cut) + fl32(skin)). */
+static float list_radius32(float r_cut, float skin)
+{
+    float R = r_cut + skin;
+    return R;
+}
+
+/* inclusion predicate P(i,j): canonical fp32 (0) or fp64 (1) */
+static int within(int predicate, int dim, const double *pi, const double *pj,
+                  const double *box, float R32)
+{
+    if (predicate == 0) {
+        float R2 = R32 * R32;
+        float dx = disp32((float)pi[0], (float)pj[0], (float)box[0]);
+        float dy = disp32((float)pi[1], (float)pj[1], (float)box[1]);
+        float r2 = fmaf(dy, dy, dx * dx);
+        if (dim == 3) {
+            float dz = disp32((float)pi[2], (float)pj[2], (float)box[2]);
+            r2 = fmaf(dz, dz, r2);
+        }
+        return r2 < R2;
+    } else {
+        double R = (double)R32;
+        double r2 = 0.0;
+        for (int k = 0; k < dim; ++k) {
+            double d = disp64(pi[k], pj[k], box[k]);
+            r2 += d * d;
+        }
+        return r2 < R * R;
+    }
+}
+
+/* ----------------------------------------------------------- cell list -- */
+
+/* Cells per side n_k = floor(L_k / R), evaluated in fp64. */
+static void cells_per_side(int dim, const double *box, float R32, int32_t *nc)
+{
+    nc[0] = nc[1] = nc[2] = 1;
+    for (int k = 0; k < dim; ++k) {
+        int v = (int)floor(box[k] / (double)R32);
+        nc[k] = v < 1 ? 1 : v;
+    }
+}
+
+/* Canonical cell coordinate: fp32 product, truncation, clamp. */
+static int cell_coord32(double x, double L, int nk)
+{
+    float inv = (float)nk / (float)L;
+    float t = (float)x * inv;
+    int c = (int)t;
+    if (c > nk - 1) c = nk - 1;
+    if (c < 0) c = 0;
+    return c;
+}
+
+/* The oracle's own binning for its cell-binned search: plain fp64. */
+static int cell_coord64(double x, double L, int nk)
+{
+    int c = (int)floor(x / L * (double)nk);
+    if (c > nk - 1) c = nk - 1;
+    if (c < 0) c = 0;
+    return c;
+}
+
+/*
+ * orc_cell_list: canonical cell index per particle, and the counting sort by
+ * cell with ascending particle ids inside each cell.
+ *   ncell[3]   out: cells per side (1 in unused dimensions)
+ *   cell_of    out: int32[n] linear cell index (cz*ny + cy)*nx + cx
+ *   cell_start out: int32[cells+1] (may be NULL)
+ *   members    out: int32[n] particle ids grouped by cell (may be NULL)
+ */
+int orc_cell_list(int n, int dim, const double *pos, const double *box,
+                  float r_cut, float skin, int32_t *ncell, int32_t *cell_of,
+                  int32_t *cell_start, int32_t *members)
+{
+    if (n <= 0 || (dim != 2 && dim != 3)) return ORC_EINVAL;
+    float R = list_radius32(r_cut, skin);
+    int32_t nc[3];
+    cells_per_side(dim, box, R, nc);
+    ncell[0] = nc[0]; ncell[1] = nc[1]; ncell[2] = nc[2];
+    int64_t cells = (int64_t)nc[0] * nc[1] * nc[2];
+    for (int i = 0; i < n; ++i) {
+        int c[3] = {0, 0, 0};
+        for (int k = 0; k < dim; ++k)
+            c[k] = cell_coord32(pos[3 * i + k], box[k], nc[k]);
+        cell_of[i] = (c[2] * nc[1] + c[1]) * nc[0] + c[0];
+    }
+    if (cell_start && members) {
+        for (int64_t c = 0; c <= cells; ++c) cell_start[c] = 0;
+        for (int i = 0; i < n; ++i) cell_start[cell_of[i] + 1] += 1;
+        for (int64_t c = 0; c < cells; ++c) cell_start[c + 1] += cell_start[c];
+        int32_t *fill = (int32_t *)calloc((size_t)cells, sizeof(int32_t));
+        if (!fill) return ORC_ENOMEM;
+        for (int i = 0; i < n; ++i) {   /* ascending i => ascending inside a cell */
+            int c = cell_of[i];
+            members[cell_start[c] + fill[c]++] = i;
+        }
+        free(fill);
+    }
+    return ORC_OK;
+}
+
+/* ------------------------------------------------------- neighbor list -- */
+
+static int cmp_i32(const void *a, const void *b)
+{
+    int32_t x = *(const int32_t *)a, y = *(const int32_t *)b;
+    return (x > y) - (x < y);
+}
+
+/*
+ * orc_neighbor_list: S_i = { j != i : P(i,j) } for every i,
+ * as dense rows of `capacity` int32, ascending, padded with n (L74).
+ *   predicate 0: canonical fp32 (bit-exact target of the GPU list)
+ *             1: fp64 (the definition)
+ *   method    0: O(N^2) brute force over all j
+ *             1: the oracle's own cell-binned search (fp64 binning into cells of
+ *                side >= R, 3^D stencil; any dimension with fewer than 3 cells
+ *                scans all of its cells once)
+ *   nbr_count  out: TRUE count per particle (may exceed capacity)
+ *   status[0]  out: 1 if any count > capacity (rows then hold the first
+ *                   `capacity` ascending entries); status[1]: max true count
+ */
+int orc_neighbor_list(int n, int dim, const double *pos, const double *box,
+                      float r_cut, float skin, int capacity, int predicate,
+                      int method, int32_t *nbr_idx, int32_t *nbr_count,
+                      int32_t *status)
+{
+    if (n <= 0 || (dim != 2 && dim != 3) || capacity <= 0) return ORC_EINVAL;
+    float R = list_radius32(r_cut, skin);
+    int32_t nc[3];
+    cells_per_side(dim, box, R, nc);
+    int64_t cells = (int64_t)nc[0] * nc[1] * nc[2];
+    int32_t *cstart = NULL, *cmem = NULL, *cof = NULL;
+    if (method == 1) {
+        cstart = (int32_t *)calloc((size_t)cells + 1, sizeof(int32_t));
+        cmem = (int32_t *)malloc((size_t)n * sizeof(int32_t));
+        cof = (int32_t *)malloc((size_t)n * sizeof(int32_t));
+        if (!cstart || !cmem || !cof) { free(cstart); free(cmem); free(cof); return ORC_ENOMEM; }
+        for (int i = 0; i < n; ++i) {
+            int c[3] = {0, 0, 0};
+            for (int k = 0; k < dim; ++k)
+                c[k] = cell_coord64(pos[3 * i + k], box[k], nc[k]);
+            cof[i] = (c[2] * nc[1] + c[1]) * nc[0] + c[0];
+            cstart[cof[i] + 1] += 1;
+        }
+        for (int64_t c = 0; c < cells; ++c) cstart[c + 1] += cstart[c];
+        int32_t *fill = (int32_t *)calloc((size_t)cells, sizeof(int32_t));
+        if (!fill) { free(cstart); free(cmem); free(cof); return ORC_ENOMEM; }
+        for (int i = 0; i < n; ++i) cmem[cstart[cof[i]] + fill[cof[i]]++] = i;
+        free(fill);
+    }
+    int max_count = 0;
+    int fail = 0;
+#pragma omp parallel
+    {
+        int cap_tmp = 256;
+        int32_t *tmp = (int32_t *)malloc((size_t)cap_tmp * sizeof(int32_t));
+        int local_max = 0;
+#pragma omp for schedule(dynamic, 64)
+        for (int i = 0; i < n; ++i) {
+            if (!tmp) { fail = 1; continue; }
+            int cnt = 0;
+            const double *pi = pos + 3 * (size_t)i;
+            if (method == 0) {
+                for (int j = 0; j < n; ++j) {
+                    if (j == i) continue;
+                    if (within(predicate, dim, pi, pos + 3 * (size_t)j, box, R)) {
+                        if (cnt == cap_tmp) {
+                            cap_tmp *= 2;
+                            tmp = (int32_t *)realloc(tmp, (size_t)cap_tmp * sizeof(int32_t));
+                            if (!tmp) { fail = 1; break; }
+                        }
+                        tmp[cnt++] = j;
+                    }
+                }
+            } else {
+                int ci[3] = {0, 0, 0}, lo[3] = {0, 0, 0}, hi[3] = {0, 0, 0};
+                int c = cof[i];
+                ci[0] = c % nc[0]; ci[1] = (c / nc[0]) % nc[1]; ci[2] = c / (nc[0] * nc[1]);
+                for (int k = 0; k < 3; ++k) {
+                    if (k >= dim) { lo[k] = hi[k] = 0; }
+                    else if (nc[k] < 3) { lo[k] = -ci[k]; hi[k] = nc[k] - 1 - ci[k]; }
+                    else { lo[k] = -1; hi[k] = 1; }
+                }
+                for (int oz = lo[2]; oz <= hi[2] && tmp; ++oz)
+                for (int oy = lo[1]; oy <= hi[1] && tmp; ++oy)
+                for (int ox = lo[0]; ox <= hi[0] && tmp; ++ox) {
+                    int cx = (ci[0] + ox + nc[0]) % nc[0];
+                    int cy = (ci[1] + oy + nc[1]) % nc[1];
+                    int cz = (ci[2] + oz + nc[2]) % nc[2];
+                    int cc = (cz * nc[1] + cy) * nc[0] + cx;
+                    for (int s = cstart[cc]; s < cstart[cc + 1]; ++s) {
+                        int j = cmem[s];
+                        if (j == i) continue;
+                        if (within(predicate, dim, pi, pos + 3 * (size_t)j, box, R)) {
+                            if (cnt == cap_tmp) {
+                                cap_tmp *= 2;
+                                tmp = (int32_t *)realloc(tmp, (size_t)cap_tmp * sizeof(int32_t));
+                                if (!tmp) { fail = 1; break; }
+                            }
+                            tmp[cnt++] = j;
+                        }
+                    }
+                }
+            }
+            if (!tmp) continue;
+            qsort(tmp, (size_t)cnt, sizeof(int32_t), cmp_i32);
+            nbr_count[i] = cnt;
+            if (cnt > local_max) local_max = cnt;
+            int32_t *row = nbr_idx + (size_t)i * capacity;
+            for (int k = 0; k < capacity; ++k) row[k] = k < cnt ? tmp[k] : n;
+        }
+        free(tmp);
+#pragma omp critical
+        { if (local_max > max_count) max_count = local_max; }
+    }
+    free(cstart); free(cmem); free(cof);
+    if (fail) return ORC_ENOMEM;
+    status[0] = max_count > capacity ? 1 : 0;
+    status[1] = max_count;
+    return ORC_OK;
+}
+
+/*
+ * orc_predicate_band: ties the canonical fp32 predicate to the paper's
+ * "within sigma".  Over all pairs (brute force, method 0)
+ * or all stencil pairs (method 1) it counts the pairs on which the fp32 and
+ * fp64 predicates differ, the largest |r64 - R|/R among those, and the smallest
+ * |r64 - R| over all pairs examined.
+ */
+int orc_predicate_band(int n, int dim, const double *pos, const double *box,
+                       float r_cut, float skin, int method,
+                       int64_t *n_disagree, double *max_rel_band, double *closest)
+{
+    if (n <= 0 || (dim != 2 && dim != 3)) return ORC_EINVAL;
+    float R = list_radius32(r_cut, skin);
+    int cap = 256;
+    int rc = ORC_OK;
+    int32_t *idx = NULL, *cnt = NULL, status[2];
+    /* candidate superset: fp64 list at radius R*(1+1e-3) from the chosen method */
+    float Rw = R * 1.001f;
+    idx = (int32_t *)malloc((size_t)n * cap * sizeof(int32_t));
+    cnt = (int32_t *)malloc((size_t)n * sizeof(int32_t));
+    if (!idx || !cnt) { free(idx); free(cnt); return ORC_ENOMEM; }
+    rc = orc_neighbor_list(n, dim, pos, box, Rw, 0.0f, cap, 1, method, idx, cnt, status);
+    if (rc != ORC_OK || status[0]) { free(idx); free(cnt); return rc ? rc : ORC_EINVAL; }
+    int64_t nd = 0; double band = 0.0, close = 1e300;
+    for (int i = 0; i < n; ++i) {
+        for (int k = 0; k < cnt[i]; ++k) {
+            int j = idx[(size_t)i * cap + k];
+            const double *pi = pos + 3 * (size_t)i, *pj = pos + 3 * (size_t)j;
+            int a = within(0, dim, pi, pj, box, R);
+            int b = within(1, dim, pi, pj, box, R);
+            double r2 = 0.0;
+            for (int q = 0; q < dim; ++q) { double d = disp64(pi[q], pj[q], box[q]); r2 += d * d; }
+            double gap = fabs(sqrt(r2) - (double)R);
+            if (gap < close) close = gap;
+            if (a != b) { nd++; if (gap / (double)R > band) band = gap / (double)R; }
+        }
+    }
+    free(idx); free(cnt);
+    *n_disagree = nd; *max_rel_band = band; *closest = close;
+    return ORC_OK;
+}
+
+/* ------------------------------------------------------- pair functions -- */
+
+/* Lennard-Jones u(r) (unshifted) and -u'(r)/r, from r^2 (PAPER.md:L104 [69]). */
+static void lj_pair(double r2, double eps, double sigma, double *u, double *fr)
+{
+    double s2 = sigma * sigma / r2;
+    double s6 = s2 * s2 * s2;
+    double s12 = s6 * s6;
+    *u = 4.0 * eps * (s12 - s6);
+    *fr = 24.0 * eps * (2.0 * s12 - s6) / r2;
+}
+
+static double lj_u_cut(double eps, double sigma, double r_cut)
+{
+    double u, fr;
+    lj_pair(r_cut * r_cut, eps, sigma, &u, &fr);
+    return u;
+}
+
+/*
+ * orc_energy_force: e_i = 1/2 sum_j u(r_ij), E = sum_i e_i,
+ * F_i = -grad_{r_i} E in closed form, r_ij = ||d(r_i, r_j)||, fp64.
+ *   kind 0 LJ:   u = 4 eps[(s/r)^12 - (s/r)^6] - shift*u(r_cut)  for r < r_cut
+ *   kind 1 SOFT: u = eps/2 (1 - r/d_ij)^2 for r < d_ij, d_ij = (d_i + d_j)/2
+ *                (PAPER.md:L301); r = 0 gives energy eps/2 and zero force
+ *   nbr_idx == NULL: all pairs j != i (the definition);
+ *   else: over the list rows (L80 smap.neighbors), entries >= n are padding.
+ *   force double[n*3] (z = 0 in 2-D), e_i double[n], *E double.
+ */
+int orc_energy_force(int n, int dim, const double *pos, const double *diam,
+                     const double *box, int kind, double eps, double sigma,
+                     double r_cut, int shift, const int32_t *nbr_idx,
+                     const int32_t *nbr_count, int capacity, double *force,
+                     double *e_i, double *E)
+{
+    if (n <= 0 || (dim != 2 && dim != 3)) return ORC_EINVAL;
+    if (kind != KIND_LJ && kind != KIND_SOFT) return ORC_EINVAL;
+    if (kind == KIND_SOFT && !diam) return ORC_EINVAL;
+    double u_c = (kind == KIND_LJ && shift) ? lj_u_cut(eps, sigma, r_cut) : 0.0;
+#pragma omp parallel for schedule(dynamic, 64)
+    for (int i = 0; i < n; ++i) {
+        double f[3] = {0.0, 0.0, 0.0}, e = 0.0;
+        int m = nbr_idx ? (nbr_count[i] < capacity ? nbr_count[i] : capacity) : n;
+        for (int k = 0; k < m; ++k) {
+            int j = nbr_idx ? nbr_idx[(size_t)i * capacity + k] : k;
+            if (j == i || j >= n || j < 0) continue;
+            double d[3] = {0.0, 0.0, 0.0}, r2 = 0.0;
+            for (int q = 0; q < dim; ++q) {
+                d[q] = disp64(pos[3 * (size_t)i + q], pos[3 * (size_t)j + q], box[q]);
+                r2 += d[q] * d[q];
+            }
+            if (kind == KIND_LJ) {
+                if (r2 < r_cut * r_cut) {
+                    double u, fr;
+                    lj_pair(r2, eps, sigma, &u, &fr);
+                    e += 0.5 * (u - u_c);
+                    for (int q = 0; q < dim; ++q) f[q] += fr * d[q];
+                }
+            } else {
+                double dij = 0.5 * (diam[i] + diam[j]);
+                double r = sqrt(r2);
+                if (r < dij) {
+                    double x = 1.0 - r / dij;
+                    e += 0.5 * (0.5 * eps * x * x);
+                    if (r > 0.0) {
+                        double fr = eps / dij * x / r;
+                        for (int q = 0; q < dim; ++q) f[q] += fr * d[q];
+                    }
+                }
+            }
+        }
+        force[3 * (size_t)i + 0] = f[0];
+        force[3 * (size_t)i + 1] = f[1];
+        force[3 * (size_t)i + 2] = f[2];
+        e_i[i] = e;
+    }
+    double tot = 0.0;
+    for (int i = 0; i < n; ++i) tot += e_i[i];
+    *E = tot;
+    return ORC_OK;
+}
+
+/* ---------------------------------------------------------- rebuild test -- */
+
+/*
+ * orc_needs_rebuild: flag = max_i ||d(r_i, ref_i)||^2 >
+ * (skin/2)^2, strict, nearest-image displacement, fp64.
+ */
+int orc_needs_rebuild(int n, int dim, const double *pos, const double *ref,
+                      const double *box, double skin, int32_t *flag,
+                      double *max_disp2)
+{
+    if (n <= 0 || (dim != 2 && dim != 3)) return ORC_EINVAL;
+    double m = 0.0;
+    for (int i = 0; i < n; ++i) {
+        double r2 = 0.0;
+        for (int q = 0; q < dim; ++q) {
+            double d = disp64(pos[3 * (size_t)i + q], ref[3 * (size_t)i + q], box[q]);
+            r2 += d * d;
+        }
+        if (r2 > m) m = r2;
+    }
+    *max_disp2 = m;
+    *flag = m > (0.5 * skin) * (0.5 * skin) ? 1 : 0;
+    return ORC_OK;
+}
+
+/* ------------------------------------------------------------------ NVE -- */
+
+/*
+ * orc_nve_run: nsteps of kick-drift-kick velocity
+ * Verlet in fp64 (PAPER.md:L100, L78 m r'' = -grad U, L72 shift function):
+ *     v <- v + (dt/2m) F;  r <- wrap(r + dt v);  F <- F(r);  v <- v + (dt/2m) F
+ * `force` must hold F(pos) on entry.
+ *   use_list 0: forces by brute force over all pairs (no list anywhere)
+ *            1: forces over the oracle's own fp64 cell-binned list of radius
+ *               r_cut + skin, rebuilt when orc_needs_rebuild fires after the
+ *               drift (this is the loop bench.py times as the CPU baseline)
+ *   energies  out (may be NULL): double[(nsteps+1)*2] = (KE, PE) at every step
+ *             boundary, entry 0 being the state on entry
+ *   stats     out int32[3]: rebuilds, overflow (0/1), max neighbor count seen
+ */
+int orc_nve_run(int n, int dim, double *pos, double *vel, double *force,
+                const double *diam, const double *box, int kind, double eps,
+                double sigma, double r_cut, int shift, double dt, double mass,
+                int nsteps, int use_list, float skin, int capacity,
+                double *energies, int32_t *stats)
+{
+    if (n <= 0 || (dim != 2 && dim != 3) || dt <= 0.0 || mass <= 0.0) return ORC_EINVAL;
+    int rc = ORC_OK;
+    double *e_i = (double *)malloc((size_t)n * sizeof(double));
+    double *ref = NULL;
+    int32_t *idx = NULL, *cnt = NULL;
+    int32_t st[2] = {0, 0};
+    int rebuilds = 0, overflow = 0, maxc = 0;
+    double E = 0.0;
+    if (!e_i) return ORC_ENOMEM;
+    if (use_list) {
+        ref = (double *)malloc((size_t)n * 3 * sizeof(double));
+        idx = (int32_t *)malloc((size_t)n * capacity * sizeof(int32_t));
+        cnt = (int32_t *)malloc((size_t)n * sizeof(int32_t));
+        if (!ref || !idx || !cnt) { rc = ORC_ENOMEM; goto done; }
+        rc = orc_neighbor_list(n, dim, pos, box, (float)r_cut, skin, capacity, 1, 1, idx, cnt, st);
+        if (rc) goto done;
+        memcpy(ref, pos, (size_t)n * 3 * sizeof(double));
+        overflow |= st[0]; if (st[1] > maxc) maxc = st[1];
+    }
+    if (energies) {
+        double ke = 0.0;
+        rc = orc_energy_force(n, dim, pos, diam, box, kind, eps, sigma, r_cut, shift,
+                              idx, cnt, capacity, force, e_i, &E);
+        if (rc) goto done;
+        for (int i = 0; i < n; ++i)
+            for (int q = 0; q < dim; ++q) ke += vel[3 * (size_t)i + q] * vel[3 * (size_t)i + q];
+        energies[0] = 0.5 * mass * ke; energies[1] = E;
+    }
+    double a = dt / (2.0 * mass);
+    for (int s = 0; s < nsteps; ++s) {
+        for (int i = 0; i < n; ++i)
+            for (int q = 0; q < dim; ++q) {
+                size_t t = 3 * (size_t)i + q;
+                vel[t] = vel[t] + a * force[t];
+                pos[t] = wrap64(pos[t] + dt * vel[t], box[q]);
+            }
+        if (use_list) {
+            int32_t flag; double md2;
+            orc_needs_rebuild(n, dim, pos, ref, box, (double)skin, &flag, &md2);
+            if (flag) {
+                rc = orc_neighbor_list(n, dim, pos, box, (float)r_cut, skin, capacity, 1, 1, idx, cnt, st);
+                if (rc) goto done;
+                memcpy(ref, pos, (size_t)n * 3 * sizeof(double));
+                rebuilds++; overflow |= st[0]; if (st[1] > maxc) maxc = st[1];
+            }
+        }
+        rc = orc_energy_force(n, dim, pos, diam, box, kind, eps, sigma, r_cut, shift,
+                              idx, cnt, capacity, force, e_i, &E);
+        if (rc) goto done;
+        double ke = 0.0;
+        for (int i = 0; i < n; ++i)
+            for (int q = 0; q < dim; ++q) {
+                size_t t = 3 * (size_t)i + q;
+                vel[t] = vel[t] + a * force[t];
+                ke += vel[t] * vel[t];
+            }
+        if (energies) { energies[2 * (s + 1)] = 0.5 * mass * ke; energies[2 * (s + 1) + 1] = E; }
+    }
+    if (stats) { stats[0] = rebuilds; stats[1] = overflow; stats[2] = maxc; }
+done:
+    free(e_i); free(ref); free(idx); free(cnt);
+    return rc;
+}

@@ -1,0 +1,154 @@
+"""ctypes loader for the fp64 CPU oracle ``md_oracle.c``.
+
+TEST INFRASTRUCTURE, NOT THE PRODUCT: only ``tests/``,
+``__graft_entry__.smoke()`` and ``bench.py``'s cpu_baseline / ``--impl
+reference`` legs may import this.  It imports nothing from the CUDA package.
+Argument marshalling only; every formula lives in ``md_oracle.c`` with its
+PAPER.md citation.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "md_oracle.c")
+_LIB = os.path.join(_HERE, "libmd_oracle.so")
+_lib = None
+
+
+def build(force: bool = False) -> str:
+    """Compile md_oracle.c with gcc (no implicit FMA, OpenMP over particles)."""
+    if force or not os.path.exists(_LIB) or os.path.getmtime(_LIB) < os.path.getmtime(_SRC):
+        cmd = ["gcc", "-O2", "-std=c99", "-fopenmp", "-ffp-contract=off", "-fno-fast-math",
+               "-shared", "-fPIC", "-o", _LIB, _SRC, "-lm"]
+        subprocess.run(cmd, check=True)
+    return _LIB
+
+
+def lib():
+    global _lib
+    if _lib is None:
+        _lib = C.CDLL(build())
+    return _lib
+
+
+def num_threads() -> int:
+    return int(lib().orc_num_threads())
+
+
+def set_num_threads(t: int) -> None:
+    lib().orc_set_num_threads(int(t))
+
+
+def _d(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _p(a, t):
+    return a.ctypes.data_as(C.POINTER(t))
+
+
+def _pd(a):
+    return _p(a, C.c_double) if a is not None else None
+
+
+def _pi(a):
+    return _p(a, C.c_int32) if a is not None else None
+
+
+def _check(rc, what):
+    if rc != 0:
+        raise RuntimeError(f"oracle {what} failed: {rc}")
+
+
+def pos3(pos) -> np.ndarray:
+    """float32[N,4] or any [N,>=3]/[N,2] array -> exact fp64 [N,3]."""
+    a = np.asarray(pos)
+    out = np.zeros((a.shape[0], 3), dtype=np.float64)
+    k = min(3, a.shape[1])
+    out[:, :k] = a[:, :k].astype(np.float64)
+    return out
+
+
+def cell_list(pos, box, dim, r_cut, skin):
+    p = _d(pos3(pos)); b = _d(box)
+    n = p.shape[0]
+    ncell = np.zeros(3, dtype=np.int32)
+    cell_of = np.zeros(n, dtype=np.int32)
+    # first call sizes the arrays
+    _check(lib().orc_cell_list(n, dim, _pd(p), _pd(b), C.c_float(r_cut), C.c_float(skin),
+                               _pi(ncell), _pi(cell_of), None, None), "cell_list")
+    cells = int(ncell[0]) * int(ncell[1]) * int(ncell[2])
+    cell_start = np.zeros(cells + 1, dtype=np.int32)
+    members = np.zeros(n, dtype=np.int32)
+    _check(lib().orc_cell_list(n, dim, _pd(p), _pd(b), C.c_float(r_cut), C.c_float(skin),
+                               _pi(ncell), _pi(cell_of), _pi(cell_start), _pi(members)), "cell_list")
+    return ncell, cell_of, cell_start, members
+
+
+def neighbor_list(pos, box, dim, r_cut, skin, capacity, predicate=0, method=0):
+    p = _d(pos3(pos)); b = _d(box)
+    n = p.shape[0]
+    idx = np.empty((n, capacity), dtype=np.int32)
+    cnt = np.empty(n, dtype=np.int32)
+    status = np.zeros(2, dtype=np.int32)
+    _check(lib().orc_neighbor_list(n, dim, _pd(p), _pd(b), C.c_float(r_cut), C.c_float(skin),
+                                   capacity, predicate, method, _pi(idx), _pi(cnt), _pi(status)),
+           "neighbor_list")
+    return idx, cnt, status
+
+
+def predicate_band(pos, box, dim, r_cut, skin, method=1):
+    p = _d(pos3(pos)); b = _d(box)
+    nd = C.c_int64(0); band = C.c_double(0); close = C.c_double(0)
+    _check(lib().orc_predicate_band(p.shape[0], dim, _pd(p), _pd(b), C.c_float(r_cut),
+                                    C.c_float(skin), method, C.byref(nd), C.byref(band),
+                                    C.byref(close)), "predicate_band")
+    return int(nd.value), float(band.value), float(close.value)
+
+
+def energy_force(pos, diam, box, dim, kind, eps, sigma, r_cut, shift,
+                 nbr_idx=None, nbr_count=None):
+    p = _d(pos3(pos)); b = _d(box)
+    n = p.shape[0]
+    dm = _d(diam) if diam is not None else None
+    f = np.zeros((n, 3), dtype=np.float64)
+    e_i = np.zeros(n, dtype=np.float64)
+    E = C.c_double(0)
+    cap = 0
+    if nbr_idx is not None:
+        nbr_idx = np.ascontiguousarray(nbr_idx, dtype=np.int32)
+        nbr_count = np.ascontiguousarray(nbr_count, dtype=np.int32)
+        cap = nbr_idx.shape[1]
+    _check(lib().orc_energy_force(n, dim, _pd(p), _pd(dm), _pd(b), kind, C.c_double(eps),
+                                  C.c_double(sigma), C.c_double(r_cut), shift, _pi(nbr_idx),
+                                  _pi(nbr_count), cap, _pd(f), _pd(e_i), C.byref(E)),
+           "energy_force")
+    return f, e_i, float(E.value)
+
+
+def needs_rebuild(pos, ref, box, dim, skin):
+    p = _d(pos3(pos)); r = _d(pos3(ref)); b = _d(box)
+    flag = C.c_int32(0); m = C.c_double(0)
+    _check(lib().orc_needs_rebuild(p.shape[0], dim, _pd(p), _pd(r), _pd(b), C.c_double(skin),
+                                   C.byref(flag), C.byref(m)), "needs_rebuild")
+    return int(flag.value), float(m.value)
+
+
+def nve_run(pos, vel, force, diam, box, dim, kind, eps, sigma, r_cut, shift, dt, mass,
+            nsteps, use_list=0, skin=0.0, capacity=128, want_energies=True):
+    """Returns (pos, vel, force, energies[(nsteps+1),2] or None, stats[3])."""
+    p = _d(pos3(pos)).copy(); v = _d(pos3(vel)).copy(); f = _d(pos3(force)).copy()
+    b = _d(box)
+    dm = _d(diam) if diam is not None else None
+    en = np.zeros((nsteps + 1, 2), dtype=np.float64) if want_energies else None
+    stats = np.zeros(3, dtype=np.int32)
+    _check(lib().orc_nve_run(p.shape[0], dim, _pd(p), _pd(v), _pd(f), _pd(dm), _pd(b), kind,
+                             C.c_double(eps), C.c_double(sigma), C.c_double(r_cut), shift,
+                             C.c_double(dt), C.c_double(mass), nsteps, use_list,
+                             C.c_float(skin), capacity, _pd(en), _pi(stats)), "nve_run")
+    return p, v, f, en, stats

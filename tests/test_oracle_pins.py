@@ -1,0 +1,459 @@
+"""Pins for the fp64 CPU oracle (oracle/md_oracle.c) -- CPU only.
+
+Each test ties one oracle function to something OTHER than itself: a value
+from tests/golden (cited), a textbook closed form, an invariant, a library
+routine for a special case, or brute force on tiny inputs (SURVEY.md §8c "P").
+A dropped term, wrong sign, wrong index or transposed operand in the oracle
+fails at least one of them.
+"""
+import math
+
+import numpy as np
+import pytest
+from scipy.spatial import cKDTree
+
+from conftest import golden
+
+LJ, SOFT = 0, 1
+RHO = 0.8442
+
+
+def fcc64(m):
+    """fp64 perfect FCC lattice at rho = 0.8442 and its fp64 box."""
+    from paper_1912_04232_b200.workloads import fcc_sites
+    n = 4 * m ** 3
+    L = (n / RHO) ** (1.0 / 3.0)
+    return fcc_sites(m, L / m), np.array([L, L, L])
+
+
+def rows_as_sets(idx, cnt, n):
+    return [set(int(j) for j in idx[i, : min(cnt[i], idx.shape[1])] if j < n) for i in range(len(cnt))]
+
+
+# ---------------------------------------------------------------- P2: FCC --
+
+def test_fcc_shell_counts_and_lattice_sum(orc):
+    g = golden("fcc_shells.txt")
+    pos, box = fcc64(5)                        # L = 8.4 > 2 * 2.8
+    n = pos.shape[0]
+    a = box[0] / 5
+    assert abs(a - g["lattice_constant"]) < 1e-9
+    for R, key in [(2.8, "neighbors_within_2p8"), (2.7, "neighbors_within_2p7"),
+                   (2.5, "neighbors_within_2p5")]:
+        for method in (0, 1):
+            idx, cnt, st = orc.neighbor_list(pos, box, 3, R, 0.0, 128, predicate=1, method=method)
+            assert cnt.min() == cnt.max() == int(g[key]), (R, method)
+            assert st[0] == 0 and st[1] == int(g[key])
+    # independent lattice sum from the textbook FCC shells (multiplicity, k)
+    shells = [(12, 1), (6, 2), (24, 3), (12, 4), (24, 5), (8, 6)]
+    for (mult, k) in shells:
+        assert abs(a * math.sqrt(k / 2) - g[f"shell_{k}_r"]) < 1e-6
+    u = lambda r: 4.0 * (r ** -12 - r ** -6)
+    uc = u(2.5)
+    assert abs(uc - g["lj_u_cut_2p5"]) < 1e-12
+    rs = [(mult, a * math.sqrt(k / 2)) for (mult, k) in shells if a * math.sqrt(k / 2) < 2.5]
+    pe_unshifted = 0.5 * sum(mult * u(r) for mult, r in rs)
+    pe_shifted = 0.5 * sum(mult * (u(r) - uc) for mult, r in rs)
+    assert abs(pe_unshifted - g["pe_per_particle_unshifted"]) < 1e-9
+    assert abs(pe_shifted - g["pe_per_particle_shifted"]) < 1e-9
+    for shift, want in [(1, g["pe_per_particle_shifted"]), (0, g["pe_per_particle_unshifted"])]:
+        f, e_i, E = orc.energy_force(pos, None, box, 3, LJ, 1.0, 1.0, 2.5, shift)
+        assert abs(E / n - want) < 1e-10
+        assert np.allclose(e_i, want, atol=1e-10)          # every site equivalent
+        assert np.abs(f).max() < 1e-11                      # symmetry: F_i = 0
+    # same over the list (smap.neighbors form)
+    idx, cnt, st = orc.neighbor_list(pos, box, 3, 2.5, 0.3, 128, predicate=1, method=1)
+    f, e_i, E = orc.energy_force(pos, None, box, 3, LJ, 1.0, 1.0, 2.5, 1, idx, cnt)
+    assert abs(E / n - g["pe_per_particle_shifted"]) < 1e-10
+
+
+# ------------------------------------------------- P3: two-body closed forms --
+
+def two_body(r, axis=0, dim=3, box=20.0, diam=(1.0, 1.0), origin=(3.0, 4.0, 5.0)):
+    pos = np.zeros((2, 3))
+    pos[0, :dim] = origin[:dim]
+    pos[1, :dim] = origin[:dim]
+    pos[1, axis] += r
+    return pos, np.array([box, box, box]), np.array(diam, dtype=np.float64)
+
+
+@pytest.mark.parametrize("axis", [0, 1, 2])
+def test_lj_two_body(orc, axis):
+    eps, sig, rc = 1.7, 0.9, 2.5 * 0.9
+    rmin = 2 ** (1 / 6) * sig
+    # u(sigma) = 0 unshifted; u(rmin) = -eps; F(rmin) = 0
+    pos, box, _ = two_body(sig, axis)
+    f, e_i, E = orc.energy_force(pos, None, box, 3, LJ, eps, sig, rc, 0)
+    assert abs(E) < 1e-12
+    # at r = sigma the force is repulsive with magnitude 24 eps / sigma
+    want = np.zeros(3); want[axis] = -24 * eps / sig      # particle 0 pushed to -axis
+    assert np.allclose(f[0], want, rtol=1e-12) and np.allclose(f[1], -want, rtol=1e-12)
+    pos, box, _ = two_body(rmin, axis)
+    f, e_i, E = orc.energy_force(pos, None, box, 3, LJ, eps, sig, rc, 0)
+    assert abs(E + eps) < 1e-12 and np.abs(f).max() < 1e-12
+    assert np.allclose(e_i, [-eps / 2, -eps / 2])         # U = 1/2 sum_{i != j}: half each
+    # general r: closed form, attractive beyond rmin (sign check)
+    r = 1.5 * sig
+    u = 4 * eps * ((sig / r) ** 12 - (sig / r) ** 6)
+    du = 4 * eps * (-12 * sig ** 12 / r ** 13 + 6 * sig ** 6 / r ** 7)
+    uc = 4 * eps * ((sig / rc) ** 12 - (sig / rc) ** 6)
+    pos, box, _ = two_body(r, axis)
+    f, e_i, E0 = orc.energy_force(pos, None, box, 3, LJ, eps, sig, rc, 0)
+    _, _, E1 = orc.energy_force(pos, None, box, 3, LJ, eps, sig, rc, 1)
+    assert abs(E0 - u) < 1e-13 and abs(E1 - (u - uc)) < 1e-13
+    # F_0 = -dU/dr_0; r = x_1 - x_0 so dU/dx_0 = -u'(r)  =>  F_0 = +u'(r) e_axis
+    assert abs(f[0, axis] - du) < 1e-12 and abs(f[1, axis] + du) < 1e-12
+    assert du > 0 and f[0, axis] > 0                       # attraction pulls 0 toward 1
+    # continuity at the cutoff when shifted; zero beyond
+    pos, box, _ = two_body(rc * (1 - 1e-9), axis)
+    _, _, E = orc.energy_force(pos, None, box, 3, LJ, eps, sig, rc, 1)
+    assert abs(E) < 1e-8
+    pos, box, _ = two_body(rc * (1 + 1e-9), axis)
+    f, _, E = orc.energy_force(pos, None, box, 3, LJ, eps, sig, rc, 1)
+    assert E == 0.0 and np.abs(f).max() == 0.0
+    _, _, E = orc.energy_force(pos, None, box, 3, LJ, eps, sig, rc, 0)
+    assert E == 0.0
+
+
+@pytest.mark.parametrize("dim", [2, 3])
+def test_soft_two_body(orc, dim):
+    eps = 1.3
+    # equal disks, r = d/2: u = eps/8, |F| = eps/(2d)
+    d = 1.4
+    pos, box, diam = two_body(d / 2, axis=1, dim=dim, diam=(d, d))
+    f, e_i, E = orc.energy_force(pos, diam, box, dim, SOFT, eps, 1.0, 1.4, 0)
+    assert abs(E - eps / 8) < 1e-14
+    assert abs(np.linalg.norm(f[0]) - eps / (2 * d)) < 1e-14
+    assert f[0, 1] < 0 < f[1, 1]                           # repulsive
+    # mixed pair: d_ij = (1.0 + 1.4)/2 = 1.2
+    pos, box, diam = two_body(1.19, axis=0, dim=dim, diam=(1.0, 1.4))
+    _, _, E = orc.energy_force(pos, diam, box, dim, SOFT, eps, 1.0, 1.4, 0)
+    assert abs(E - 0.5 * eps * (1 - 1.19 / 1.2) ** 2) < 1e-15
+    pos, box, diam = two_body(1.2000001, axis=0, dim=dim, diam=(1.0, 1.4))
+    f, _, E = orc.energy_force(pos, diam, box, dim, SOFT, eps, 1.0, 1.4, 0)
+    assert E == 0.0 and np.abs(f).max() == 0.0
+    # r = 0: energy eps/2, zero force
+    pos, box, diam = two_body(0.0, axis=0, dim=dim, diam=(1.0, 1.0))
+    f, _, E = orc.energy_force(pos, diam, box, dim, SOFT, eps, 1.0, 1.4, 0)
+    assert abs(E - eps / 2) < 1e-15 and np.abs(f).max() == 0.0
+
+
+def test_two_body_across_periodic_boundary(orc):
+    """Nearest image: a pair straddling x = 0 / x = L."""
+    L = 12.0
+    pos = np.array([[0.3, 5.0, 5.0], [L - 0.9, 5.0, 5.0]])   # separation 1.2 through the wall
+    box = np.array([L, L, L])
+    f, _, E = orc.energy_force(pos, None, box, 3, LJ, 1.0, 1.0, 2.5, 0)
+    r = 1.2
+    assert abs(E - 4 * (r ** -12 - r ** -6)) < 1e-13
+    du = 4 * (-12 / r ** 13 + 6 / r ** 7)                  # > 0: attraction
+    # particle 0 is at +1.2 from particle 1's image => pulled toward -x
+    assert abs(f[0, 0] + du) < 1e-12 and abs(f[1, 0] - du) < 1e-12
+    idx, cnt, _ = orc.neighbor_list(pos, box, 3, 2.5, 0.3, 8, predicate=0, method=0)
+    assert list(cnt) == [1, 1] and idx[0, 0] == 1 and idx[1, 0] == 0
+
+
+# -------------------------------------------------- P4: finite differences --
+
+@pytest.mark.parametrize("kind,dim", [(LJ, 3), (SOFT, 2), (SOFT, 3), (LJ, 2)])
+def test_force_is_minus_gradient(orc, W, kind, dim):
+    """force = -grad U by central differences of the oracle's E."""
+    rng = np.random.default_rng(5)
+    if kind == LJ:
+        # jittered lattice so that no pair sits on the repulsive wall
+        m = 3
+        if dim == 3:
+            w = W.lj_fcc(0, m, seed=11)
+            pos, box = w.pos[:, :3].astype(np.float64), w.box.astype(np.float64)
+        else:
+            g = np.arange(8.0)
+            pos = np.zeros((64, 3))
+            pos[:, :2] = np.stack(np.meshgrid(g, g, indexing="ij"), -1).reshape(-1, 2) * 1.15
+            pos[:, :2] += rng.normal(0, 0.05, (64, 2))
+            box = np.array([8 * 1.15, 8 * 1.15, 1.0])
+        diam = None
+        args = (kind, 1.0, 1.0, 2.5, 1)
+    else:
+        p4, box32 = W.random_box(3, 200, dim, [9.0] * dim, diam=(1.0, 1.4))
+        pos, box, diam = p4[:, :3].astype(np.float64), box32.astype(np.float64), p4[:, 3].astype(np.float64)
+        args = (kind, 1.0, 1.0, 1.4, 0)
+    f, _, _ = orc.energy_force(pos, diam, box, dim, *args)
+    h = 1e-5
+    worst = 0.0
+    for i in rng.choice(pos.shape[0], 12, replace=False):
+        for q in range(dim):
+            pp = pos.copy(); pp[i, q] += h
+            pm = pos.copy(); pm[i, q] -= h
+            Ep = orc.energy_force(pp, diam, box, dim, *args)[2]
+            Em = orc.energy_force(pm, diam, box, dim, *args)[2]
+            fd = -(Ep - Em) / (2 * h)
+            worst = max(worst, abs(fd - f[i, q]) / max(1.0, np.abs(f[i]).max()))
+    assert worst < 1e-6, worst
+    if dim == 2:
+        assert np.abs(f[:, 2]).max() == 0.0
+
+
+# ------------------------------------------- P5/P6: Newton 3, translations --
+
+def test_newton_third_law_and_translation_invariance(orc, W):
+    for w in (W.config(0), W.soft_disks(1, 2048)):
+        pos = w.pos[:, :3].astype(np.float64); box = w.box.astype(np.float64)
+        diam = w.pos[:, 3].astype(np.float64)
+        args = (w.dim, w.kind, w.epsilon, w.sigma, w.r_cut, w.shift)
+        f, e_i, E = orc.energy_force(pos, diam, box, *args)
+        assert np.abs(f.sum(0)).max() <= 1e-10 * np.linalg.norm(f, axis=1).sum()
+        t = np.array([0.37, -11.3, 4.21 if w.dim == 3 else 0.0])
+        pos_t = np.mod(pos + t, box)
+        if w.dim == 2:
+            pos_t[:, 2] = 0.0
+        f2, e2, E2 = orc.energy_force(pos_t, diam, box, *args)
+        assert abs(E2 - E) <= 1e-10 * abs(E)
+        assert np.abs(f2 - f).max() <= 1e-9 * np.abs(f).max()
+        # neighbor sets under the fp64 predicate are translation invariant
+        a = orc.neighbor_list(pos, box, w.dim, w.r_cut, w.skin, w.capacity, predicate=1, method=1)
+        b = orc.neighbor_list(pos_t, box, w.dim, w.r_cut, w.skin, w.capacity, predicate=1, method=1)
+        assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1])
+        # the list is symmetric: j in S_i <=> i in S_j  (full list)
+        sets = rows_as_sets(a[0], a[1], w.n)
+        for i in range(0, w.n, 37):
+            for j in sets[i]:
+                assert i in sets[j]
+        # list-based energy/force == all-pairs definition (PAPER.md:L78 vs L80)
+        f3, e3, E3 = orc.energy_force(pos, diam, box, *args, a[0], a[1])
+        assert abs(E3 - E) <= 1e-12 * abs(E) and np.abs(f3 - f).max() <= 1e-11 * np.abs(f).max()
+
+
+# -------------------------------------------------- P1: neighbor sets -------
+
+def edge_case_positions(W, seed, n, dim, box):
+    """Uniform random + particles on cell faces, at 0 and just below L."""
+    pos, box32 = W.random_box(seed, n, dim, box)
+    R = np.float32(np.float32(1.0) + np.float32(0.25))
+    for k in range(dim):
+        L = box32[k]
+        nk = int(math.floor(float(L) / float(R)))
+        below = np.nextafter(L, np.float32(0.0), dtype=np.float32)
+        specials = [np.float32(0.0), below]
+        for c in range(1, nk):
+            face = np.float32(c * float(L) / nk)
+            specials += [face, np.nextafter(face, np.float32(0), dtype=np.float32),
+                         np.nextafter(face, np.float32(1e9), dtype=np.float32)]
+        for s, x in enumerate(specials):
+            pos[(7 * s + 3 * k) % n, k] = x
+    return pos, box32
+
+
+@pytest.mark.parametrize("dim,box", [(3, [3.9, 5.2, 6.4]), (2, [3.8, 6.3]), (3, [5.01, 5.01, 5.01]),
+                                     (2, [13.0, 4.0]), (3, [2.6, 3.0, 4.4])])
+def test_neighbor_brute_vs_cells_vs_kdtree(orc, W, dim, box):
+    n = 500 if dim == 3 else 300
+    pos, box32 = edge_case_positions(W, 17 + dim, n, dim, box)
+    r_cut, skin, cap = 1.0, 0.25, 192
+    for predicate in (0, 1):
+        a = orc.neighbor_list(pos, box32, dim, r_cut, skin, cap, predicate=predicate, method=0)
+        b = orc.neighbor_list(pos, box32, dim, r_cut, skin, cap, predicate=predicate, method=1)
+        assert a[2][0] == 0
+        assert np.array_equal(a[0], b[0]) and np.array_equal(a[1], b[1]) and np.array_equal(a[2], b[2])
+        # rows ascending, padded with n
+        for i in range(n):
+            row = a[0][i]
+            assert np.all(np.diff(row[: a[1][i]]) > 0) and np.all(row[a[1][i]:] == n)
+    # library pin: scipy's periodic kd-tree, fp64 ball query
+    p64 = pos[:, :dim].astype(np.float64)
+    R = float(np.float32(np.float32(r_cut) + np.float32(skin)))
+    tree = cKDTree(p64, boxsize=box32[:dim].astype(np.float64))
+    pairs = tree.query_pairs(R, output_type="ndarray")
+    want = [set() for _ in range(n)]
+    for i, j in pairs:
+        want[i].add(int(j)); want[j].add(int(i))
+    got = rows_as_sets(*orc.neighbor_list(pos, box32, dim, r_cut, skin, cap, predicate=1, method=0)[:2], n)
+    # kd-tree uses <=; a pair at exactly R would differ -- none here
+    assert got == want
+    # canonical fp32 predicate differs from fp64 only inside a 4e-6 R band (P11)
+    nd, band, closest = orc.predicate_band(pos, box32, dim, r_cut, skin, method=0)
+    assert band < 4e-6
+    got32 = rows_as_sets(*orc.neighbor_list(pos, box32, dim, r_cut, skin, cap, predicate=0, method=0)[:2], n)
+    ndiff = sum(len(x ^ y) for x, y in zip(got, got32))
+    assert ndiff == nd
+
+
+def test_canonical_predicate_by_hand(orc):
+    """SURVEY §8c-A2/A3 retyped in NumPy fp32 on a tiny system (brute force)."""
+    rng = np.random.default_rng(3)
+    n, L = 60, np.float32(6.0)
+    x = (rng.uniform(0, 1, (n, 3)) * 6.0).astype(np.float32)
+    x[0] = [0.0, 0.0, 0.0]; x[1] = [np.nextafter(L, np.float32(0)), 0.1, 5.9]
+    r_cut, skin = np.float32(1.5), np.float32(0.3)
+    R = np.float32(r_cut + skin); R2 = np.float32(R * R); h = np.float32(L / np.float32(2))
+    want = []
+    for i in range(n):
+        s = []
+        for j in range(n):
+            if i == j:
+                continue
+            d = []
+            for k in range(3):
+                a, b = x[i, k], x[j, k]
+                dd = np.float32(a - b)
+                if dd > h:
+                    dd = np.float32(np.float32(a - L) - b)
+                elif dd < -h:
+                    dd = np.float32(a - np.float32(b - L))
+                d.append(dd)
+            r2 = np.float32(d[0] * d[0])
+            r2 = np.float32(np.float64(d[1]) * np.float64(d[1]) + np.float64(r2))   # fmaf: one rounding
+            r2 = np.float32(np.float64(d[2]) * np.float64(d[2]) + np.float64(r2))
+            if r2 < R2:
+                s.append(j)
+        want.append(s)
+    idx, cnt, st = orc.neighbor_list(x, np.array([L, L, L]), 3, 1.5, 0.3, 64, predicate=0, method=0)
+    for i in range(n):
+        assert list(idx[i, : cnt[i]]) == want[i]
+    assert st[1] == max(len(s) for s in want)
+
+
+def test_overflow_convention(orc, W):
+    """P10: capacity 64 on config 0 overflows (static shapes)."""
+    w = W.config(0)
+    idx, cnt, st = orc.neighbor_list(w.pos, w.box, 3, w.r_cut, w.skin, 64)
+    assert st[0] == 1 and st[1] == cnt.max() and 64 < st[1] < 128
+    idx2, cnt2, st2 = orc.neighbor_list(w.pos, w.box, 3, w.r_cut, w.skin, 128)
+    assert st2[0] == 0 and st2[1] == st[1] and np.array_equal(cnt, cnt2)
+    assert 70 <= cnt2.min() and cnt2.max() <= 90 and abs(cnt2.mean() - 77.9) < 0.3
+
+
+def test_predicate_band_on_configs(orc, W):
+    """P11: fp32 vs fp64 predicate on the configs' initial states."""
+    for w in (W.config(0), W.config(2)):
+        nd, band, closest = orc.predicate_band(w.pos, w.box, w.dim, w.r_cut, w.skin, method=1)
+        assert band < 4e-6
+        assert nd <= 2
+
+
+# ------------------------------------------------------- O2: cell list ------
+
+def test_cell_list(orc, W):
+    pos, box32 = edge_case_positions(W, 5, 400, 3, [3.9, 5.2, 6.4])
+    ncell, cell_of, cell_start, members = orc.cell_list(pos, box32, 3, 1.0, 0.25)
+    assert list(ncell) == [3, 4, 5]
+    cells = 60
+    assert cell_start[0] == 0 and cell_start[cells] == 400 and np.all(np.diff(cell_start) >= 0)
+    assert sorted(members.tolist()) == list(range(400))
+    for c in range(cells):
+        seg = members[cell_start[c]: cell_start[c + 1]]
+        assert np.all(cell_of[seg] == c) and np.all(np.diff(seg) > 0)
+    # geometric meaning: the particle lies inside its cell (up to one fp32 ulp)
+    side = box32.astype(np.float64) / ncell
+    cx = cell_of % 3; cy = (cell_of // 3) % 4; cz = cell_of // 12
+    for k, ck in enumerate((cx, cy, cz)):
+        x = pos[:, k].astype(np.float64)
+        assert np.all(x >= ck * side[k] - 1e-6) and np.all(x <= (ck + 1) * side[k] + 1e-6)
+    # hand cases: x = 0 -> cell 0; largest float below L -> last cell
+    p = np.zeros((2, 4), dtype=np.float32)
+    p[1, :3] = np.nextafter(box32, np.float32(0), dtype=np.float32)
+    _, cof, _, _ = orc.cell_list(p, box32, 3, 1.0, 0.25)
+    assert cof[0] == 0 and cof[1] == cells - 1
+    # 2-D: linear index cy*nx + cx
+    p2, b2 = W.random_box(9, 100, 2, [13.0, 4.0])
+    nc2, cof2, cs2, mem2 = orc.cell_list(p2, b2, 2, 1.0, 0.25)
+    assert list(nc2) == [10, 3, 1]
+    want = np.minimum((p2[:, 1] * np.float32(3 / 4.0)).astype(np.int32), 2) * 10 + \
+        np.minimum((p2[:, 0] * (np.float32(10) / np.float32(13.0))).astype(np.int32), 9)
+    assert np.array_equal(cof2, want)
+
+
+# --------------------------------------------------- P9: rebuild test -------
+
+def test_needs_rebuild_constructed(orc, W):
+    w = W.config(0)
+    ref = w.pos.copy()
+    half = w.skin / 2
+    u = np.array([1.0, 2.0, -2.0]) / 3.0
+    for scale, want in [(1 - 1e-3, 0), (1 + 1e-3, 1)]:
+        pos = ref.astype(np.float64).copy()
+        pos[100, :3] = np.mod(pos[100, :3] + u * half * scale, w.box)
+        flag, m = orc.needs_rebuild(pos, ref, w.box, 3, w.skin)
+        assert flag == want and abs(math.sqrt(m) - half * scale) < 1e-9
+    # crossing the periodic boundary by 0.01 is a 0.01 displacement, not ~L
+    ref2 = ref.astype(np.float64).copy(); ref2[5, 0] = 0.004
+    pos2 = ref2.copy(); pos2[5, 0] = float(w.box[0]) - 0.006
+    flag, m = orc.needs_rebuild(pos2, ref2, w.box, 3, w.skin)
+    assert flag == 0 and abs(math.sqrt(m) - 0.01) < 1e-6
+    # 2-D ignores z
+    p = np.zeros((4, 3)); r = np.zeros((4, 3)); r[:, 2] = 5.0
+    assert orc.needs_rebuild(p, r, np.array([10.0, 10.0, 1.0]), 2, 0.1)[0] == 0
+
+
+# --------------------------------------------------- P7/P8: integrator ------
+
+def test_nve_invariants_config0(orc, W):
+    w = W.config(0)
+    box = w.box.astype(np.float64)
+    args = (None, box, 3, LJ, 1.0, 1.0, 2.5, 1)
+    f0, _, E0 = orc.energy_force(w.pos, None, box, 3, LJ, 1.0, 1.0, 2.5, 1)
+    p, v, f, en, st = orc.nve_run(w.pos, w.vel, f0, *args, 0.005, 1.0, 100)
+    tot = en.sum(1)
+    drift = np.abs(tot / tot[0] - 1).max()
+    assert drift < 2e-4                                   # symplectic: bounded, small
+    assert abs(en[0, 1] - E0) < 1e-9
+    # temperature bookkeeping of the generator: KE = 3(N-1)/2 T
+    assert abs(en[0, 0] - 1.5 * (w.n - 1)) < 1e-3 * w.n
+    # total momentum conserved (Newton 3)
+    mom0 = w.vel[:, :3].astype(np.float64).sum(0)
+    assert np.abs(v.sum(0) - mom0).max() < 1e-10
+    # second order: halving dt shrinks the energy excursion ~4x
+    p2, v2, f2, en2, _ = orc.nve_run(w.pos, w.vel, f0, *args, 0.0025, 1.0, 200)
+    tot2 = en2.sum(1)
+    ratio = drift / np.abs(tot2 / tot2[0] - 1).max()
+    assert 3.0 < ratio < 5.5, ratio
+    # time reversal: negate v, run back, recover the start
+    pb, vb, fb, _, _ = orc.nve_run(p, -v, f, *args, 0.005, 1.0, 100, want_energies=False)
+    d = pb - w.pos[:, :3].astype(np.float64)
+    d -= box * np.round(d / box)
+    assert np.abs(d).max() < 1e-8
+    assert np.abs(vb + w.vel[:, :3].astype(np.float64)).max() < 1e-8
+    # list-based loop with half-skin rebuilds gives the same trajectory
+    # (a valid list changes nothing) and does rebuild
+    pl, vl, fl, enl, stl = orc.nve_run(w.pos, w.vel, f0, *args, 0.005, 1.0, 100, use_list=1,
+                                       skin=0.3, capacity=128)
+    assert np.abs(pl - p).max() < 1e-10 and 5 <= stl[0] <= 20 and stl[1] == 0
+    # positions stay in [0, L)
+    assert p.min() >= 0 and np.all(p < box)
+
+
+def test_velocity_verlet_harmonic_oscillator(orc):
+    """P8: two overlapping equal soft disks = harmonic oscillator in the
+    relative coordinate x = r - d with omega^2 = 2 eps / (m d^2); velocity
+    Verlet reproduces it with cos(omega' dt) = 1 - (omega dt)^2 / 2 exactly."""
+    eps, m, d, dt, nsteps = 1.0, 1.0, 1.0, 0.05, 20
+    x0 = -0.05                                           # overlap 0.05, at rest
+    box = np.array([10.0, 10.0, 1.0])
+    pos = np.array([[4.0, 5.0, 0.0], [4.0 + d + x0, 5.0, 0.0]])
+    vel = np.zeros((2, 3))
+    diam = np.array([d, d])
+    f0, _, _ = orc.energy_force(pos, diam, box, 2, SOFT, eps, 1.0, 1.4, 0)
+    omega = math.sqrt(2 * eps / (m * d * d))
+    omega_p = math.acos(1 - (omega * dt) ** 2 / 2) / dt
+    # the spring is one-sided (u = 0 for r >= d): stay inside the first quarter
+    # period pi/(2 omega) = 1.11 = 22 steps, while the disks still overlap
+    for k in (1, 5, 13, nsteps):
+        p, v, f, en, _ = orc.nve_run(pos, vel, f0, diam, box, 2, SOFT, eps, 1.0, 1.4, 0, dt, m, k)
+        x = (p[1, 0] - p[0, 0]) - d
+        assert x < 0
+        assert abs(x - x0 * math.cos(omega_p * k * dt)) < 1e-12
+        assert abs((p[0, 0] + p[1, 0]) - (pos[0, 0] + pos[1, 0])) < 1e-12   # centre of mass at rest
+    # the continuous-time frequency would be off by a visible phase: the test discriminates
+    assert abs(x0 * math.cos(omega * nsteps * dt) - x0 * math.cos(omega_p * nsteps * dt)) > 1e-6
+
+
+def test_wrap_convention(orc):
+    """mu(r, dr) keeps 0 <= x < L: free flight through the wall."""
+    box = np.array([5.0, 5.0, 5.0])
+    pos = np.array([[4.99, 0.01, 2.5], [1.0, 1.0, 1.0]])
+    vel = np.array([[1.0, -1.0, 0.0], [0.0, 0.0, 0.0]])
+    f0 = np.zeros((2, 3))
+    # sigma tiny => no interaction; 5 steps of dt = 0.01 moves by 0.05
+    p, v, f, _, _ = orc.nve_run(pos, vel, f0, None, box, 3, LJ, 1.0, 1e-3, 2.5e-3, 1, 0.01, 1.0, 5,
+                                want_energies=False)
+    assert np.allclose(p[0], [0.04, 4.96, 2.5], atol=1e-12)
+    assert np.all(p >= 0) and np.all(p < box)
