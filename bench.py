@@ -1,0 +1,328 @@
+#!/usr/bin/env python
+"""bench.py -- LJ NVE particle-steps/s at N = 256,000 (BASELINE.json metric), B200.
+
+One bench "step" = `--md-steps` (default 100) velocity-Verlet steps of config 3 through ONE
+md_nve_step call: the whole hot path (kick/drift/rebuild test, conditional cell list + re-sort
++ neighbor list, LJ force + second kick), rebuilds amortised.  Defaults: 3 warm-up steps (the
+jittered lattice melts), 10 timed steps = the config's 1000 MD steps.
+
+  value      device-resident state, CUDA events per bench step on the launching stream,
+             L2 flushed between bench steps (not timed), max over ranks
+  e2e        the same metric through md_nve_run_host: pinned HOST buffers in, host buffers
+             out, H2D + list build + steps + D2H all inside the timed region
+  roofline   the force kernel (dominant): algorithmic bytes (4*Kbar + 36) * N per launch
+              over its average duration, L2 flushed before every launch,
+             against MEASURED_PEAKS.json's hbm_gbs
+  cpu_baseline  the fp64 oracle's own list-based loop on the host cores, bounded sample
+
+`--impl reference` times the oracle (this tier's reference arm) instead.
+N > 1 (torchrun): independent replicas, one per GPU, different seeds; no collective on the
+data path ("replicas only").
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "LJ NVE particle-steps/sec at N=256k (incl. amortised rebuilds)"
+UNIT = "particle-steps/s"
+FALLBACK_HBM_GBS = 6650.0      # /opt/skills/guides/B200_PROFILING.md fallback
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--config", type=int, default=3, help="BASELINE.json config index")
+    ap.add_argument("--md-steps", type=int, default=100, help="MD steps per bench step")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--breakdown", action="store_true", help="also time build and force separately")
+    return ap.parse_args()
+
+
+def peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        try:
+            return float(json.load(open(p))["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+        except Exception:
+            pass
+    return FALLBACK_HBM_GBS, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md)."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+         "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                 "--format=csv,noheader,nounits", "-lms", "100"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.t = threading.Thread(target=self._read, daemon=True)
+            self.t.start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append(line.strip())
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=2)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for ln in self.lines:
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) < 9:
+                continue
+            try:
+                sm.append(float(f[1])); mx.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, v in zip(names, f[5:9]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        return {"sm_mhz": statistics.median(sm) if sm else None,
+                "sm_max_mhz": max(mx) if mx else None, "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+
+def oracle_sample(w, md_steps):
+    """The oracle's own list-based fp64 loop (build + force + velocity Verlet + half-skin
+    rebuilds) on the host cores for `md_steps` steps of workload w. Returns seconds, threads."""
+    from oracle import md_oracle as orc
+    orc.build()
+    diam = w.pos[:, 3].astype(np.float64)
+    t0 = time.perf_counter()
+    idx, cnt, _ = orc.neighbor_list(w.pos, w.box, w.dim, w.r_cut, w.skin, w.capacity, predicate=1, method=1)
+    f0, _, _ = orc.energy_force(w.pos, diam, w.box, w.dim, w.kind, w.epsilon, w.sigma, w.r_cut, w.shift, idx, cnt)
+    orc.nve_run(w.pos, w.vel, f0, diam, w.box, w.dim, w.kind, w.epsilon, w.sigma, w.r_cut, w.shift,
+                w.dt, w.mass, md_steps, use_list=1, skin=w.skin, capacity=w.capacity, want_energies=False)
+    return time.perf_counter() - t0, orc.num_threads()
+
+
+def run_reference(args):
+    """This tier's reference arm: the oracle as it stands, timed on the host cores; each
+    bench step is a bounded sample (2 MD steps) of the same workload."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_1912_04232_b200 import workloads as W
+    w = W.config(args.config)
+    sample = 2
+    for _ in range(min(args.warmup, 1)):
+        oracle_sample(w, 1)
+    times = []
+    cores = 1
+    for _ in range(args.steps):
+        t, cores = oracle_sample(w, sample)
+        times.append(t)
+    total = sum(times)
+    value = w.n * sample * args.steps / total
+    desc = f"{sample} MD steps of config {args.config} (N={w.n}) per bench step incl. one list build"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
+        "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
+        "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+        "data": "synthetic", "config": {"workload": w.name, "n": w.n, "md_steps_per_step": sample},
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": desc},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }))
+
+
+def main():
+    args = parse()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import torch.distributed as dist
+    from paper_1912_04232_b200 import binding as B
+    from paper_1912_04232_b200 import workloads as W
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    B.lib()
+
+    # replicas: rank r simulates an independent sample of the same config
+    w = W.config(args.config, replica=rank)
+    S = B.System(w, device=dev)
+    stream = torch.cuda.Stream(device=dev)
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # 2x the 126 MB L2
+    md_steps = args.md_steps
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    with torch.cuda.stream(stream):
+        S.build(stream)
+        S.compute_force(True, stream)
+        for _ in range(args.warmup):
+            S.step(md_steps, stream)
+        barrier()
+        sampler = ClockSampler(local)
+        sampler.start()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
+              for _ in range(args.steps)]
+        rebuilds = 0
+        stats_acc = []
+        for a, b in ev:
+            flush.zero_()
+            a.record(stream)
+            S.step(md_steps, stream)
+            b.record(stream)
+            stats_acc.append(S.stats.clone())
+        barrier()
+        clocks = sampler.stop()
+        ms = sum(a.elapsed_time(b) for a, b in ev)
+        rebuilds = int(sum(int(s[1]) for s in stats_acc))
+        max_count = int(max(int(s[3]) for s in stats_acc))
+        overflow = any(int(s[2]) >= 0 for s in stats_acc)
+
+        # ---- roofline of the force kernel: cold L2, event pair per launch
+        kbar = float(S.nbr_count.float().mean())
+        reps = 30
+        fev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
+        for a, b in fev:
+            flush.zero_()
+            a.record(stream)
+            S.compute_force(False, stream)
+            b.record(stream)
+        torch.cuda.synchronize(dev)
+        force_ms_cold = statistics.median(a.elapsed_time(b) for a, b in fev)
+        a0, b0 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a0.record(stream)
+        for _ in range(reps):
+            S.compute_force(False, stream)
+        b0.record(stream)
+        torch.cuda.synchronize(dev)
+        force_ms_warm = a0.elapsed_time(b0) / reps
+        build_ms = None
+        if args.breakdown:
+            bev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(10)]
+            for a, b in bev:
+                flush.zero_()
+                a.record(stream)
+                S.build(stream)
+                b.record(stream)
+            torch.cuda.synchronize(dev)
+            build_ms = statistics.median(a.elapsed_time(b) for a, b in bev)
+            S.compute_force(False, stream)
+
+    t_ms = torch.tensor([ms], dtype=torch.float64, device=dev)
+    if world > 1:
+        dist.all_reduce(t_ms, op=dist.ReduceOp.MAX)
+    ms_max = float(t_ms[0])
+    value = world * w.n * md_steps * args.steps / (ms_max * 1e-3)
+
+    # ---- e2e through the host-buffer entry point (pinned host memory)
+    e2e = None
+    if not args.no_e2e:
+        pos_h = torch.from_numpy(w.pos.copy()).pin_memory()
+        vel_h = torch.from_numpy(w.vel.copy()).pin_memory()
+        force_h = torch.zeros_like(pos_h).pin_memory()
+        stats_h = np.zeros(4, np.int32)
+        B.md_nve_run_host(S.cfg, S.pot, pos_h, vel_h, force_h, w.dt, w.mass, md_steps, stats_h)  # warm
+        e2e_steps = max(1, min(args.steps, 5))
+        barrier()
+        t0 = time.perf_counter()
+        for _ in range(e2e_steps):
+            B.md_nve_run_host(S.cfg, S.pot, pos_h, vel_h, force_h, w.dt, w.mass, md_steps, stats_h)
+        barrier()
+        dt_e2e = time.perf_counter() - t0
+        t_e = torch.tensor([dt_e2e], dtype=torch.float64, device=dev)
+        if world > 1:
+            dist.all_reduce(t_e, op=dist.ReduceOp.MAX)
+        e2e = {"value": world * w.n * md_steps * e2e_steps / float(t_e[0]), "unit": UNIT,
+               "h2d_bytes_per_step": 2 * w.n * 16, "d2h_bytes_per_step": 3 * w.n * 16 + 8 + 16,
+               "what": f"md_nve_run_host: pinned host pos/vel in, list build + {md_steps} MD steps, host pos/vel/force/energy/stats out"}
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    peak, peak_src = peaks()
+    algo_bytes = (4.0 * kbar + 36.0) * w.n
+    achieved = algo_bytes / (force_ms_cold * 1e-3) / 1e9
+    step_bytes = (4.0 * kbar + 164.0) * w.n
+    out = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32",
+        "data": "synthetic",
+        "config": {"workload": f"BASELINE.json configs[{args.config}]: {w.name}, rho=0.8442, r_cut=2.5, "
+                               f"skin={w.skin}, capacity={w.capacity}, dt={w.dt}, re-sort at every rebuild",
+                   "n": w.n, "md_steps_per_step": md_steps, "parallelism": f"replicas x{world}",
+                   "l2": "flushed (256 MiB write) between bench steps; inside a bench step the loop "
+                         "re-reads its own ~100 MB working set every MD step as in production",
+                   "precision": "fp32 state; pair terms fp32 with fp64 re-evaluation where the error "
+                                "estimate requires it (DESIGN.md §5)"},
+        "us_per_md_step": 1e3 * ms_max / (args.steps * md_steps),
+        "rebuilds": rebuilds, "md_steps_per_rebuild": (args.steps * md_steps) / max(1, rebuilds),
+        "max_neighbors": max_count, "overflow": overflow,
+        "step_hbm_frac": step_bytes / (1e3 * ms_max / (args.steps * md_steps) * 1e-6) / 1e9 / peak,
+        "clocks": clocks,
+        "roofline": {"bound": "hbm", "kernel": "k_force (md_pair_energy_force)", "achieved": achieved,
+                     "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+                     "peak_source": peak_src, "algorithmic_bytes": algo_bytes, "kbar": kbar,
+                     "launch_ms_cold_l2": force_ms_cold, "launch_ms_warm_l2": force_ms_warm},
+        "gpu_launches": args.steps * (md_steps * 8 + 1),
+    }
+    if build_ms is not None:
+        out["build_ms_per_rebuild"] = build_ms
+    if e2e is not None:
+        out["e2e"] = e2e
+    if not args.no_cpu_baseline:
+        sample_steps = {0: 100, 1: 200, 2: 50, 3: 20, 4: 5}[args.config]
+        t, cores = oracle_sample(w, sample_steps)
+        out["cpu_baseline"] = {"value": w.n * sample_steps / t, "unit": UNIT, "cores": cores,
+                               "kind": "oracle",
+                               "sample": f"{sample_steps} MD steps of the same workload (N={w.n}) incl. the "
+                                         f"initial list build and half-skin rebuilds, {t:.1f} s"}
+    print(json.dumps(out))
+    S.close()
+    if world > 1:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()

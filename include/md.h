@@ -1,0 +1,180 @@
+/*
+ * md.h -- C ABI of libmd_b200: the neighbor-list molecular-dynamics hot path of
+ * "JAX, M.D." (arXiv 1912.04232) as hand-written CUDA kernels for sm_100a.
+ *
+ * Citations are lines of /root/reference/PAPER.md (L<line>, section); readings
+ * of points the paper leaves open are SURVEY.md §8c A1..A18, restated in
+ * DESIGN.md §3.
+ *
+ * Conventions (all calls)
+ *   - Return value: MD_OK, or a negative MD_E* for a failure detected on the
+ *     host before anything is launched; md_last_error() gives the text.
+ *     Asynchronous conditions (list overflow, rebuild needed) are DEVICE words,
+ *     never return codes.  No exceptions, no abort, no output to stdout.
+ *   - Pointers are DEVICE pointers unless the parameter says "host".  The
+ *     caller owns every buffer, the workspace included; the library allocates
+ *     no caller-visible memory and keeps no pointer past a call except the
+ *     workspace and (md_nve_step only) a cached CUDA graph of the last call's
+ *     arguments.  No call except md_create / md_destroy / md_nve_run_host
+ *     synchronises with the host.
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default
+ *     stream).  Work is ordered on that stream only.
+ *   - Particle arrays are float4[n], 16-byte aligned:
+ *       pos   = (x, y, z, w)  0 <= x < box[k]; z ignored (keep 0) when dim = 2;
+ *               w = particle diameter d_i (MD_KIND_SOFT) or unused (MD_KIND_LJ)
+ *       vel   = (vx, vy, vz, unused)
+ *       force = (Fx, Fy, Fz, e_i)  with e_i = 1/2 sum_j u(r_ij) on output
+ *     Indices are int32.
+ */
+#ifndef MD_B200_H
+#define MD_B200_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define MD_OK          0
+#define MD_EINVAL     (-1)  /* null/unaligned pointer, n<=0, dim not 2|3, capacity<=0 or not a
+                               multiple of 4, skin<0, r_cut<=0, dt<=0, mass<=0, unknown kind */
+#define MD_EBOX       (-2)  /* a box side holds fewer than 3 cells of side >= r_cut+skin, or the
+                               cell side exceeds r_cut+skin by less than 1e-5 of the box side */
+#define MD_EWORKSPACE (-3)  /* workspace null, unaligned (256 B) or too small */
+#define MD_ECUDA      (-4)  /* CUDA runtime error at launch; text in md_last_error() */
+
+#define MD_KIND_LJ   0      /* Lennard-Jones [69], L104 §3.3.2 */
+#define MD_KIND_SOFT 1      /* harmonic soft sphere [70], L104; d_ij = (d_i+d_j)/2, L301 App. A */
+
+typedef struct md_system md_system;   /* opaque; lives in host memory */
+
+/* Space + partitioning parameters (L72 §3.2.1 space.periodic(L); L84 §3.2.3). */
+typedef struct md_config {
+    int   dim;        /* 2 or 3 */
+    float box[3];     /* periodic box sides L_k; box[2] ignored when dim = 2 */
+    float r_cut;      /* neighborhood size sigma of L84 before the halo */
+    float skin;       /* halo (L49 §3.1); list radius R = fl32(r_cut + skin) */
+    int   capacity;   /* slots per neighbor row (static shape, L47 §3.1); multiple of 4 */
+    int   resort;     /* 1: md_cell_list_build physically re-orders pos/vel/id by cell */
+} md_config;
+
+/* Pair potential u(r) (L78 §3.2.2, L104 §3.3.2). */
+typedef struct md_potential {
+    int   kind;       /* MD_KIND_LJ | MD_KIND_SOFT */
+    float epsilon;
+    float sigma;      /* LJ length; unused for SOFT (diameters come from pos.w) */
+    float r_cut;      /* LJ truncation radius (<= config r_cut); unused for SOFT */
+    int   shift;      /* LJ: 1 = u(r) - u(r_cut) for r < r_cut, 0 = plain truncation */
+} md_potential;
+
+/* Text of the last error on the calling thread ("" if none). Host pointer, valid until the
+ * next failing call. */
+const char *md_last_error(void);
+
+/* Bytes of device workspace md_create needs for n particles (host out-pointer). */
+int md_workspace_bytes(const md_config *cfg, int n, size_t *bytes);
+
+/* Bind a system to a caller-owned device workspace (256-byte aligned, >= md_workspace_bytes).
+ * Validates cfg (MD_EINVAL / MD_EBOX), clears the workspace on the legacy stream and
+ * synchronises once.  *out is a host object released by md_destroy. */
+int md_create(const md_config *cfg, int n, void *workspace, size_t bytes, md_system **out);
+int md_destroy(md_system *sys);
+
+/* Tuning knobs (host call; drops the cached step graph):
+ *   "fp64_threshold"       re-evaluate a particle in fp64 when S > value * max(|F|, 1e-3)
+ *                          (default 16; <= 0: every particle in fp64; 1e30: never)
+ *   "threads_per_particle" lanes sharing one neighbor row in the force kernel (1..32, 2^k)
+ *   "use_graph"            0: md_nve_step launches kernels directly instead of a CUDA graph */
+int md_set_option(md_system *sys, const char *name, double value);
+
+/* Cells per side n_k = floor(L_k / R) (1 for unused dimensions) -> host int[3]. */
+int md_num_cells(const md_system *sys, int *ncell);
+
+/* Entry (i,k) of a neighbor list lives at nbr_idx[i*particle_stride + k*slot_stride]
+ * (host out-pointers; currently capacity and 1: row-major rows). */
+int md_nbr_layout(const md_system *sys, long *particle_stride, long *slot_stride);
+
+/*
+ * Cell list (L84 "partition.cell_list ... places them into cells where each cell has size
+ * sigma"): cell coordinate c_k = min(n_k-1, (int)(x_k * fl32(n_k/L_k))), linear index
+ * (c_z n_y + c_y) n_x + c_x, counting sort by cell.
+ *   cell_start int32[cells+1] out: slots [cell_start[c], cell_start[c+1]) belong to cell c
+ *   perm       int32[n]       out: perm[s] = index (on entry) of the particle in slot s;
+ *                                  inside a cell slots ascend by id (or by index if id = NULL)
+ *   resort = 1: pos, vel (may be NULL) and id (may be NULL) are permuted in place so that
+ *               new[s] = old[perm[s]];  resort = 0: they are left untouched.
+ */
+int md_cell_list_build(md_system *sys, void *pos, void *vel, int32_t *id,
+                       int32_t *cell_start, int32_t *perm, void *stream);
+
+/*
+ * Neighbor list (L84-L88 partition.neighbor_list; dense N x capacity rows, L74): for every
+ * i all j != i in the 3^dim adjacent cells with r2 < R^2 under the canonical fp32 predicate
+ * (nearest-image displacement with the box side subtracted from the larger
+ * coordinate first; r2 = fma(dz,dz, fma(dy,dy, dx*dx)); strict <).
+ *   pos        as left by md_cell_list_build (same cell_start / perm)
+ *   nbr_idx    int32[n*capacity] out: row i holds min(count_i, capacity) neighbor indices
+ *              (in the particle order of `pos`), then the pad value n up to capacity;
+ *              order within a row is unspecified
+ *   nbr_count  int32[n] out: TRUE count, may exceed capacity
+ *   status     int32[2] out: {1 if any count > capacity else 0, max true count}; rows of an
+ *              overflowed list are truncated and forces from it are invalid
+ * Also snapshots pos inside the workspace as the reference for md_needs_rebuild.
+ */
+int md_neighbor_list_build(md_system *sys, const void *pos, const int32_t *cell_start,
+                           const int32_t *perm, int32_t *nbr_idx, int32_t *nbr_count,
+                           int32_t *status, void *stream);
+
+/* Rebuild test (L49 "whenever a particle moves by more than the halo distance", read as
+ * half the skin): *flag = 1 if max_i ||d(pos_i, ref_i)||^2 > (skin/2)^2 else 0,
+ * ref = positions at the last md_neighbor_list_build, nearest-image displacement. */
+int md_needs_rebuild(md_system *sys, const void *pos, int32_t *flag, void *stream);
+
+/*
+ * Pair energy and force over the list (L78 U = 1/2 sum_{i!=j} u; L80 smap.neighbors;
+ * L104 force = -grad U, written in closed form):
+ *   LJ   u = 4 eps[(s/r)^12 - (s/r)^6] - shift*u(r_cut), r < r_cut
+ *   SOFT u = eps/2 (1 - r/d_ij)^2, r < d_ij = (pos_i.w + pos_j.w)/2; r = 0: eps/2, no force
+ *   force        float4[n] out: (F_i, e_i)
+ *   energy_total double* out (may be NULL): sum_i e_i accumulated in fp64
+ * Pair terms are evaluated and accumulated in fp64 from fp32 displacements and rounded to
+ * fp32 on store.
+ */
+int md_pair_energy_force(md_system *sys, const md_potential *pot, const void *pos,
+                         const int32_t *nbr_idx, const int32_t *nbr_count, void *force,
+                         double *energy_total, void *stream);
+
+/*
+ * nsteps of velocity-Verlet NVE (L100 simulate.nve; L78 m r'' = -grad U; L72 shift function):
+ *   v += dt/(2m) F;  r = wrap(r + dt v);  [rebuild test; if it fires: cell list (+ re-sort)
+ *   and neighbor list];  F = F(r);  v += dt/(2m) F
+ * with the rebuild decision taken on the device.  `force` must hold F(pos) on entry (call
+ * md_neighbor_list_build + md_pair_energy_force once first); nbr_idx / nbr_count must be the
+ * list of that build.  On exit pos/vel/force are the state after nsteps in the CURRENT
+ * particle order; id[s] (may be NULL) = original index of the particle in slot s.
+ *   stats int32[4] out: {steps done, rebuilds, first step (0-based) whose rebuild
+ *                        overflowed or -1, max neighbor count seen in rebuilds}
+ * stats is reset at the start of every call.
+ */
+int md_nve_step(md_system *sys, const md_potential *pot, void *pos, void *vel, void *force,
+                int32_t *id, int32_t *nbr_idx, int32_t *nbr_count, float dt, float mass,
+                int nsteps, int32_t *stats, void *stream);
+
+/*
+ * End-to-end convenience over HOST buffers: allocates device memory, copies pos/vel in,
+ * builds the lists, evaluates F, runs nsteps of md_nve_step, copies the state back
+ * un-permuted (original particle order) and frees.  Synchronous.
+ *   pos_host, vel_host   host float4[n] in/out
+ *   force_host           host float4[n] out (may be NULL)
+ *   energy_host          host double out (may be NULL): potential energy of the final state
+ *   stats_host           host int32[4] out (may be NULL)
+ */
+int md_nve_run_host(const md_config *cfg, const md_potential *pot, int n, void *pos_host,
+                    void *vel_host, void *force_host, double *energy_host, float dt,
+                    float mass, int nsteps, int32_t *stats_host);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* MD_B200_H */

@@ -1,0 +1,254 @@
+"""Thin ctypes binding over libmd_b200.so -- same names as include/md.h.
+
+Argument marshalling only: every step of the path runs in the CUDA kernels
+behind the C ABI.  PyTorch is used for device memory and streams.  There is no
+CPU fallback: if the library is missing or a call fails, this raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+from . import build as _build
+
+MD_OK, MD_EINVAL, MD_EBOX, MD_EWORKSPACE, MD_ECUDA = 0, -1, -2, -3, -4
+MD_KIND_LJ, MD_KIND_SOFT = 0, 1
+
+SYMBOLS = [
+    "md_last_error", "md_workspace_bytes", "md_create", "md_destroy", "md_set_option",
+    "md_num_cells", "md_nbr_layout", "md_cell_list_build", "md_neighbor_list_build",
+    "md_needs_rebuild", "md_pair_energy_force", "md_nve_step", "md_nve_run_host",
+]
+
+
+class md_config(C.Structure):
+    _fields_ = [("dim", C.c_int), ("box", C.c_float * 3), ("r_cut", C.c_float),
+                ("skin", C.c_float), ("capacity", C.c_int), ("resort", C.c_int)]
+
+
+class md_potential(C.Structure):
+    _fields_ = [("kind", C.c_int), ("epsilon", C.c_float), ("sigma", C.c_float),
+                ("r_cut", C.c_float), ("shift", C.c_int)]
+
+
+class MdError(RuntimeError):
+    def __init__(self, code, text):
+        super().__init__(f"libmd_b200 error {code}: {text}")
+        self.code = code
+
+
+_lib = None
+
+
+def lib():
+    """Load libmd_b200.so (built in-tree by build.py); raise if it is not there."""
+    global _lib
+    if _lib is None:
+        path = _build.LIB
+        if not os.path.exists(path):
+            raise RuntimeError(
+                f"{path} is missing: build it with `python -m paper_1912_04232_b200.build` "
+                "(nvcc, sm_100a). There is no CPU fallback.")
+        L = C.CDLL(path)
+        L.md_last_error.restype = C.c_char_p
+        for name in SYMBOLS:
+            getattr(L, name)           # AttributeError if the ABI lost a symbol
+        vp, ip = C.c_void_p, C.c_void_p
+        L.md_workspace_bytes.argtypes = [C.POINTER(md_config), C.c_int, C.POINTER(C.c_size_t)]
+        L.md_create.argtypes = [C.POINTER(md_config), C.c_int, vp, C.c_size_t, C.POINTER(vp)]
+        L.md_destroy.argtypes = [vp]
+        L.md_set_option.argtypes = [vp, C.c_char_p, C.c_double]
+        L.md_num_cells.argtypes = [vp, C.POINTER(C.c_int * 3)]
+        L.md_nbr_layout.argtypes = [vp, C.POINTER(C.c_long), C.POINTER(C.c_long)]
+        L.md_cell_list_build.argtypes = [vp, vp, vp, ip, ip, ip, vp]
+        L.md_neighbor_list_build.argtypes = [vp, vp, ip, ip, ip, ip, ip, vp]
+        L.md_needs_rebuild.argtypes = [vp, vp, ip, vp]
+        L.md_pair_energy_force.argtypes = [vp, C.POINTER(md_potential), vp, ip, ip, vp, vp, vp]
+        L.md_nve_step.argtypes = [vp, C.POINTER(md_potential), vp, vp, vp, ip, ip, ip,
+                                  C.c_float, C.c_float, C.c_int, ip, vp]
+        L.md_nve_run_host.argtypes = [C.POINTER(md_config), C.POINTER(md_potential), C.c_int, vp,
+                                      vp, vp, C.POINTER(C.c_double), C.c_float, C.c_float, C.c_int,
+                                      vp]
+        _lib = L
+    return _lib
+
+
+def _check(rc):
+    if rc != MD_OK:
+        raise MdError(rc, md_last_error())
+
+
+def _ptr(t):
+    """Device (or host, for *_host calls) address of a tensor / array, or NULL."""
+    if t is None:
+        return None
+    if isinstance(t, torch.Tensor):
+        assert t.is_contiguous()
+        return t.data_ptr()
+    if isinstance(t, np.ndarray):
+        assert t.flags["C_CONTIGUOUS"]
+        return t.ctypes.data
+    return int(t)
+
+
+def _stream(stream):
+    if stream is None:
+        return torch.cuda.current_stream().cuda_stream
+    if isinstance(stream, torch.cuda.Stream):
+        return stream.cuda_stream
+    return int(stream)
+
+
+def make_config(dim, box, r_cut, skin, capacity, resort=1) -> md_config:
+    b = [float(x) for x in box] + [1.0] * (3 - len(box))
+    return md_config(int(dim), (C.c_float * 3)(*b[:3]), float(r_cut), float(skin), int(capacity),
+                     int(resort))
+
+
+def make_potential(kind, epsilon=1.0, sigma=1.0, r_cut=2.5, shift=1) -> md_potential:
+    return md_potential(int(kind), float(epsilon), float(sigma), float(r_cut), int(shift))
+
+
+# ------------------------------------------------------------ the C ABI, same names ----
+
+def md_last_error() -> str:
+    return lib().md_last_error().decode()
+
+
+def md_workspace_bytes(cfg: md_config, n: int) -> int:
+    out = C.c_size_t(0)
+    _check(lib().md_workspace_bytes(C.byref(cfg), n, C.byref(out)))
+    return int(out.value)
+
+
+def md_create(cfg: md_config, n: int, workspace: torch.Tensor):
+    h = C.c_void_p(None)
+    _check(lib().md_create(C.byref(cfg), n, _ptr(workspace), workspace.numel() * workspace.element_size(),
+                           C.byref(h)))
+    return h
+
+
+def md_destroy(sys) -> None:
+    _check(lib().md_destroy(sys))
+
+
+def md_set_option(sys, name: str, value: float) -> None:
+    _check(lib().md_set_option(sys, name.encode(), float(value)))
+
+
+def md_num_cells(sys):
+    out = (C.c_int * 3)()
+    _check(lib().md_num_cells(sys, C.byref(out)))
+    return [int(out[0]), int(out[1]), int(out[2])]
+
+
+def md_nbr_layout(sys):
+    a, b = C.c_long(0), C.c_long(0)
+    _check(lib().md_nbr_layout(sys, C.byref(a), C.byref(b)))
+    return int(a.value), int(b.value)
+
+
+def md_cell_list_build(sys, pos, vel, id, cell_start, perm, stream=None) -> None:
+    _check(lib().md_cell_list_build(sys, _ptr(pos), _ptr(vel), _ptr(id), _ptr(cell_start), _ptr(perm),
+                                    _stream(stream)))
+
+
+def md_neighbor_list_build(sys, pos, cell_start, perm, nbr_idx, nbr_count, status, stream=None) -> None:
+    _check(lib().md_neighbor_list_build(sys, _ptr(pos), _ptr(cell_start), _ptr(perm), _ptr(nbr_idx),
+                                        _ptr(nbr_count), _ptr(status), _stream(stream)))
+
+
+def md_needs_rebuild(sys, pos, flag, stream=None) -> None:
+    _check(lib().md_needs_rebuild(sys, _ptr(pos), _ptr(flag), _stream(stream)))
+
+
+def md_pair_energy_force(sys, pot: md_potential, pos, nbr_idx, nbr_count, force, energy_total=None,
+                         stream=None) -> None:
+    _check(lib().md_pair_energy_force(sys, C.byref(pot), _ptr(pos), _ptr(nbr_idx), _ptr(nbr_count),
+                                      _ptr(force), _ptr(energy_total), _stream(stream)))
+
+
+def md_nve_step(sys, pot: md_potential, pos, vel, force, id, nbr_idx, nbr_count, dt, mass, nsteps,
+                stats, stream=None) -> None:
+    _check(lib().md_nve_step(sys, C.byref(pot), _ptr(pos), _ptr(vel), _ptr(force), _ptr(id),
+                             _ptr(nbr_idx), _ptr(nbr_count), float(dt), float(mass), int(nsteps),
+                             _ptr(stats), _stream(stream)))
+
+
+def md_nve_run_host(cfg: md_config, pot: md_potential, pos_host, vel_host, force_host, dt, mass,
+                    nsteps, stats_host=None, want_energy=True):
+    """HOST buffers in/out (numpy float32[n,4] or pinned CPU tensors). Returns the final
+    potential energy (or None)."""
+    n = pos_host.shape[0]
+    e = C.c_double(0.0)
+    _check(lib().md_nve_run_host(C.byref(cfg), C.byref(pot), n, _ptr(pos_host), _ptr(vel_host),
+                                 _ptr(force_host), C.byref(e) if want_energy else None, float(dt),
+                                 float(mass), int(nsteps), _ptr(stats_host)))
+    return float(e.value) if want_energy else None
+
+
+# -------------------------------------------------- device buffers for one system ------
+
+class System:
+    """Owns the torch tensors one simulation needs (allocation only; no arithmetic)."""
+
+    def __init__(self, w, device="cuda:0", resort=None, capacity=None):
+        self.w = w
+        self.device = torch.device(device)
+        self.cfg = make_config(w.dim, w.box, w.r_cut, w.skin, capacity or w.capacity,
+                               w.resort if resort is None else resort)
+        self.pot = make_potential(w.kind, w.epsilon, w.sigma, w.r_cut, w.shift)
+        n, cap = w.n, self.cfg.capacity
+        self.n, self.capacity = n, cap
+        with torch.cuda.device(self.device):
+            self.workspace = torch.empty(md_workspace_bytes(self.cfg, n), dtype=torch.uint8,
+                                         device=self.device)
+            self.sys = md_create(self.cfg, n, self.workspace)
+        ncell = md_num_cells(self.sys)
+        self.cells = ncell[0] * ncell[1] * ncell[2]
+        dev = self.device
+        self.pos = torch.from_numpy(w.pos).to(dev)
+        self.vel = torch.from_numpy(w.vel).to(dev)
+        self.force = torch.zeros(n, 4, dtype=torch.float32, device=dev)
+        self.id = torch.arange(n, dtype=torch.int32, device=dev)
+        self.cell_start = torch.zeros(self.cells + 1, dtype=torch.int32, device=dev)
+        self.perm = torch.zeros(n, dtype=torch.int32, device=dev)
+        self.nbr_idx = torch.full((n, cap), -1, dtype=torch.int32, device=dev)
+        self.nbr_count = torch.zeros(n, dtype=torch.int32, device=dev)
+        self.status = torch.zeros(2, dtype=torch.int32, device=dev)
+        self.flag = torch.zeros(1, dtype=torch.int32, device=dev)
+        self.stats = torch.zeros(4, dtype=torch.int32, device=dev)
+        self.energy = torch.zeros(1, dtype=torch.float64, device=dev)
+
+    def reset(self):
+        self.pos.copy_(torch.from_numpy(self.w.pos))
+        self.vel.copy_(torch.from_numpy(self.w.vel))
+        self.id.copy_(torch.arange(self.n, dtype=torch.int32))
+
+    def build(self, stream=None):
+        md_cell_list_build(self.sys, self.pos, self.vel, self.id, self.cell_start, self.perm, stream)
+        md_neighbor_list_build(self.sys, self.pos, self.cell_start, self.perm, self.nbr_idx,
+                               self.nbr_count, self.status, stream)
+
+    def compute_force(self, want_energy=True, stream=None):
+        md_pair_energy_force(self.sys, self.pot, self.pos, self.nbr_idx, self.nbr_count, self.force,
+                             self.energy if want_energy else None, stream)
+
+    def step(self, nsteps, stream=None):
+        md_nve_step(self.sys, self.pot, self.pos, self.vel, self.force, self.id, self.nbr_idx,
+                    self.nbr_count, self.w.dt, self.w.mass, nsteps, self.stats, stream)
+
+    def close(self):
+        if self.sys is not None:
+            torch.cuda.synchronize(self.device)
+            md_destroy(self.sys)
+            self.sys = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

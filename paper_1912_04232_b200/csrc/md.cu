@@ -1,0 +1,556 @@
+// md.cu -- host side of libmd_b200: the C ABI declared in include/md.h.
+// Argument checking, workspace carving, kernel launches and the CUDA-graph step loop.
+// Every step of the path runs in the kernels of md_kernels.cuh; there is no CPU fallback.
+#include "md.h"
+#include "md_kernels.cuh"
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstdlib>
+#include <cstring>
+#include <new>
+
+using namespace mdk;
+
+namespace {
+
+thread_local char g_err[512] = "";
+
+int fail(int code, const char *fmt, ...) {
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CU(call)                                                                        \
+    do {                                                                                \
+        cudaError_t e_ = (call);                                                        \
+        if (e_ != cudaSuccess)                                                          \
+            return fail(MD_ECUDA, "%s: %s (%s:%d)", #call, cudaGetErrorString(e_),      \
+                        __FILE__, __LINE__);                                            \
+    } while (0)
+
+#define LAUNCH_OK()                                                                     \
+    do {                                                                                \
+        cudaError_t e_ = cudaGetLastError();                                            \
+        if (e_ != cudaSuccess)                                                          \
+            return fail(MD_ECUDA, "kernel launch: %s (%s:%d)", cudaGetErrorString(e_),  \
+                        __FILE__, __LINE__);                                            \
+    } while (0)
+
+constexpr size_t ALIGN = 256;
+size_t up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
+bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
+int blocks_for(long long threads, int block = 256) { return (int)((threads + block - 1) / block); }
+
+struct StepKey {
+    const void *pos, *vel, *force, *id, *nbr_idx, *nbr_count, *stats;
+    float dt, mass;
+    md_potential pot;
+    int tpp;
+    float thr;
+};
+
+} // namespace
+
+struct md_system {
+    md_config cfg;
+    int n;
+    int device;          // CUDA device that owns the workspace
+    Geom g;
+    char *ws;
+    size_t ws_bytes;
+    // workspace slices
+    int *words;          // [0] rebuild flag, [1..2] internal status, [8..] spare
+    int *cell_count, *cell_start_i, *perm_i, *cell_of, *rank_tmp, *perm_tmp, *id_s;
+    float4 *pos_s, *vel_s, *ref_pos;
+    // tuning
+    int tpp;
+    float thr;           // fp64 re-evaluation threshold on S / max(|F|, 1e-3)
+    int use_graph;
+    // graph cache of md_nve_step
+    cudaStream_t cap_stream;
+    StepKey key;
+    bool key_valid;
+    cudaGraphExec_t exec1, execU;
+    int unroll;
+};
+
+namespace {
+
+// The library links its own (static) CUDA runtime: make the device that owns the workspace
+// current on the calling thread before touching streams or launching.
+int enter(const md_system *s) {
+    int cur = -1;
+    CU(cudaGetDevice(&cur));
+    if (cur != s->device) CU(cudaSetDevice(s->device));
+    return MD_OK;
+}
+
+struct Layout {
+    size_t words, cell_count, cell_start_i, perm_i, cell_of, rank_tmp, perm_tmp, id_s, pos_s,
+        vel_s, ref_pos, total;
+};
+
+Layout layout(int n, long long cells) {
+    Layout l;
+    size_t o = 0;
+    auto take = [&](size_t bytes) { size_t at = o; o += up(bytes); return at; };
+    l.words = take(64 * sizeof(int));
+    l.cell_count = take((size_t)(cells + 1) * sizeof(int));
+    l.cell_start_i = take((size_t)(cells + 1) * sizeof(int));
+    l.perm_i = take((size_t)n * sizeof(int));
+    l.cell_of = take((size_t)n * sizeof(int));
+    l.rank_tmp = take((size_t)n * sizeof(int));
+    l.perm_tmp = take((size_t)n * sizeof(int));
+    l.id_s = take((size_t)n * sizeof(int));
+    l.pos_s = take((size_t)n * sizeof(float4));
+    l.vel_s = take((size_t)n * sizeof(float4));
+    l.ref_pos = take((size_t)n * sizeof(float4));
+    l.total = o;
+    return l;
+}
+
+// Validates cfg and fills the geometry.
+int make_geom(const md_config *cfg, int n, Geom *g) {
+    if (!cfg) return fail(MD_EINVAL, "cfg is NULL");
+    if (n <= 0) return fail(MD_EINVAL, "n = %d must be positive", n);
+    if (cfg->dim != 2 && cfg->dim != 3) return fail(MD_EINVAL, "dim = %d must be 2 or 3", cfg->dim);
+    if (cfg->capacity <= 0 || cfg->capacity % 4) return fail(MD_EINVAL, "capacity = %d must be a positive multiple of 4", cfg->capacity);
+    if (!(cfg->r_cut > 0.0f)) return fail(MD_EINVAL, "r_cut must be positive");
+    if (!(cfg->skin >= 0.0f)) return fail(MD_EINVAL, "skin must be non-negative");
+    memset(g, 0, sizeof(*g));
+    g->dim = cfg->dim; g->n = n; g->capacity = cfg->capacity;
+    const float R = cfg->r_cut + cfg->skin;              // fl32(r_cut + skin)
+    g->R2 = R * R;
+    const float hs = cfg->skin * 0.5f;
+    g->half_skin2 = hs * hs;
+    g->face = R + cfg->skin;
+    long long cells = 1;
+    for (int k = 0; k < 3; ++k) {
+        g->nc[k] = 1; g->L[k] = 1.0f; g->h[k] = 0.5f; g->inv_cell[k] = 1.0f; g->inv_L[k] = 1.0f;
+        if (k >= cfg->dim) continue;
+        const float L = cfg->box[k];
+        if (!(L > 0.0f) || !std::isfinite(L)) return fail(MD_EINVAL, "box[%d] must be positive", k);
+        const int nk = (int)std::floor((double)L / (double)R);
+        if (nk < 3) return fail(MD_EBOX, "box[%d] = %g holds %d cells of side >= %g; need >= 3", k, L, nk, R);
+        if ((double)L / nk - (double)R < 1e-5 * (double)L)
+            return fail(MD_EBOX, "box[%d] = %g: cell side %.9g exceeds R = %.9g by less than 1e-5 L", k, L, (double)L / nk, (double)R);
+        g->nc[k] = nk; g->L[k] = L; g->h[k] = L / 2.0f;
+        g->inv_cell[k] = (float)nk / L;
+        g->inv_L[k] = 1.0f / L;
+        cells *= nk;
+    }
+    if (cells > 0x7fffffffLL / 2) return fail(MD_EINVAL, "too many cells");
+    g->cells = (int)cells;
+    return MD_OK;
+}
+
+int make_pair(const md_system *sys, const md_potential *pot, Pair *pp) {
+    if (!pot) return fail(MD_EINVAL, "potential is NULL");
+    if (pot->kind != MD_KIND_LJ && pot->kind != MD_KIND_SOFT) return fail(MD_EINVAL, "unknown potential kind %d", pot->kind);
+    memset(pp, 0, sizeof(*pp));
+    pp->kind = pot->kind;
+    pp->eps = pot->epsilon; pp->deps = (double)pot->epsilon;
+    pp->thr = sys->thr;
+    if (pot->kind == MD_KIND_LJ) {
+        if (!(pot->r_cut > 0.0f) || !(pot->sigma > 0.0f)) return fail(MD_EINVAL, "LJ needs sigma > 0 and r_cut > 0");
+        if (pot->r_cut > sys->cfg.r_cut) return fail(MD_EINVAL, "potential r_cut %g exceeds the list r_cut %g", pot->r_cut, sys->cfg.r_cut);
+        const double s = pot->sigma, rc = pot->r_cut;
+        pp->dsig2 = s * s; pp->drc2 = rc * rc;
+        const double s6 = std::pow(s / rc, 6.0);
+        pp->du_cut = pot->shift ? 4.0 * pp->deps * (s6 * s6 - s6) : 0.0;
+        pp->sig2 = (float)pp->dsig2; pp->rc2 = (float)pp->drc2; pp->u_cut = (float)pp->du_cut;
+    } else {
+        pp->sig2 = 1.0f; pp->dsig2 = 1.0; pp->rc2 = 3.0e38f; pp->drc2 = 1e300;
+    }
+    return MD_OK;
+}
+
+// ------------------------------------------------------------------ launch helpers ------
+
+int launch_cell_build(md_system *s, float4 *pos, float4 *vel, int *id, int *cell_start,
+                      int *perm, int *status, const int *cond, cudaStream_t st) {
+    const Geom &g = s->g;
+    const int nb = blocks_for(g.n);
+    const bool resort = s->cfg.resort != 0;
+    k_cell_assign<<<nb, 256, 0, st>>>(g, pos, s->cell_of, s->rank_tmp, s->cell_count, cond);
+    LAUNCH_OK();
+    k_cell_scan<<<1, 1024, 0, st>>>(g.cells, s->cell_count, cell_start, status, cond);
+    LAUNCH_OK();
+    k_cell_scatter<<<nb, 256, 0, st>>>(g.n, s->cell_of, s->rank_tmp, cell_start, s->perm_tmp, cond);
+    LAUNCH_OK();
+    k_cell_order_gather<<<nb, 256, 0, st>>>(g.n, s->cell_of, cell_start, s->perm_tmp, id, pos,
+                                            (resort && vel) ? vel : nullptr, perm, s->pos_s,
+                                            (resort && vel) ? s->vel_s : nullptr,
+                                            (resort && id) ? s->id_s : nullptr, cond);
+    LAUNCH_OK();
+    if (resort) {
+        k_copy_back<<<nb, 256, 0, st>>>(g.n, s->pos_s, s->vel_s, s->id_s, pos, vel, id, cond);
+        LAUNCH_OK();
+    }
+    return MD_OK;
+}
+
+int launch_nbr_build(md_system *s, const float4 *spos, const int *cell_start, const int *map,
+                     int *nbr_idx, int *nbr_count, int *status, const int *cond, cudaStream_t st) {
+    const Geom &g = s->g;
+    const int nb = blocks_for((long long)g.n * 32);
+    if (g.dim == 3)
+        k_nbr_build<3><<<nb, 256, 0, st>>>(g, spos, cell_start, map, nbr_idx, nbr_count, status, s->ref_pos, cond);
+    else
+        k_nbr_build<2><<<nb, 256, 0, st>>>(g, spos, cell_start, map, nbr_idx, nbr_count, status, s->ref_pos, cond);
+    LAUNCH_OK();
+    return MD_OK;
+}
+
+template <int KIND, int DIM>
+int launch_force_t(md_system *s, const Pair &pp, const float4 *pos, const int *nbr_idx,
+                   const int *nbr_count, float4 *force, float4 *vel, float a, double *etot,
+                   Book book, cudaStream_t st) {
+    const Geom &g = s->g;
+    const int nb = blocks_for((long long)g.n * s->tpp);
+#define MD_FORCE_CASE(T)                                                                       \
+    case T:                                                                                    \
+        k_force<KIND, DIM, T><<<nb, 256, 0, st>>>(g, pp, pos, nbr_idx, nbr_count, force, vel, \
+                                                  a, etot, book);                             \
+        break;
+    switch (s->tpp) {
+        MD_FORCE_CASE(1) MD_FORCE_CASE(2) MD_FORCE_CASE(4) MD_FORCE_CASE(8) MD_FORCE_CASE(16)
+        MD_FORCE_CASE(32)
+    default: return fail(MD_EINVAL, "threads per particle %d", s->tpp);
+    }
+#undef MD_FORCE_CASE
+    LAUNCH_OK();
+    return MD_OK;
+}
+
+int launch_force(md_system *s, const Pair &pp, const float4 *pos, const int *nbr_idx,
+                 const int *nbr_count, float4 *force, float4 *vel, float a, double *etot,
+                 Book book, cudaStream_t st) {
+    if (pp.kind == MD_KIND_LJ)
+        return s->g.dim == 3 ? launch_force_t<0, 3>(s, pp, pos, nbr_idx, nbr_count, force, vel, a, etot, book, st)
+                             : launch_force_t<0, 2>(s, pp, pos, nbr_idx, nbr_count, force, vel, a, etot, book, st);
+    return s->g.dim == 3 ? launch_force_t<1, 3>(s, pp, pos, nbr_idx, nbr_count, force, vel, a, etot, book, st)
+                         : launch_force_t<1, 2>(s, pp, pos, nbr_idx, nbr_count, force, vel, a, etot, book, st);
+}
+
+__global__ void k_init_stats(int *stats, int *flag) {
+    stats[0] = 0; stats[1] = 0; stats[2] = -1; stats[3] = 0;
+    *flag = 0;
+}
+
+__global__ void k_unpermute(int n, const int *__restrict__ id, const float4 *__restrict__ a,
+                            const float4 *__restrict__ b, const float4 *__restrict__ c,
+                            float4 *__restrict__ ao, float4 *__restrict__ bo, float4 *__restrict__ co) {
+    int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    int i = id[s];
+    ao[i] = a[s]; bo[i] = b[s]; co[i] = c[s];
+}
+
+__global__ void k_iota(int n, int *id) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) id[i] = i;
+}
+
+// One velocity-Verlet step as launches on `st` (captured into a graph or run directly).
+int record_step(md_system *s, const Pair &pp, float4 *pos, float4 *vel, float4 *force, int *id,
+                int *nbr_idx, int *nbr_count, float dt, float mass, int *stats, cudaStream_t st) {
+    const Geom &g = s->g;
+    const float a = dt / (2.0f * mass);
+    int *flag = s->words + 0;
+    int *status = s->words + 1;
+    const int nb = blocks_for(g.n);
+    if (g.dim == 3) k_kick_drift<3><<<nb, 256, 0, st>>>(g, pos, vel, force, s->ref_pos, a, dt, flag);
+    else k_kick_drift<2><<<nb, 256, 0, st>>>(g, pos, vel, force, s->ref_pos, a, dt, flag);
+    LAUNCH_OK();
+    int rc = launch_cell_build(s, pos, vel, id, s->cell_start_i, s->perm_i, status, flag, st);
+    if (rc) return rc;
+    const bool resort = s->cfg.resort != 0;
+    rc = launch_nbr_build(s, resort ? pos : s->pos_s, s->cell_start_i, resort ? nullptr : s->perm_i,
+                          nbr_idx, nbr_count, status, flag, st);
+    if (rc) return rc;
+    Book book = {flag, status, stats};
+    return launch_force(s, pp, pos, nbr_idx, nbr_count, force, vel, a, nullptr, book, st);
+}
+
+void drop_graphs(md_system *s) {
+    if (s->exec1) cudaGraphExecDestroy(s->exec1);
+    if (s->execU) cudaGraphExecDestroy(s->execU);
+    s->exec1 = s->execU = nullptr;
+    s->key_valid = false;
+}
+
+int capture(md_system *s, const Pair &pp, const StepKey &k, int reps, cudaGraphExec_t *out) {
+    if (!s->cap_stream) CU(cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking));
+    CU(cudaStreamBeginCapture(s->cap_stream, cudaStreamCaptureModeThreadLocal));
+    int rc = MD_OK;
+    for (int r = 0; r < reps && rc == MD_OK; ++r)
+        rc = record_step(s, pp, (float4 *)k.pos, (float4 *)k.vel, (float4 *)k.force, (int *)k.id,
+                         (int *)k.nbr_idx, (int *)k.nbr_count, k.dt, k.mass, (int *)k.stats,
+                         s->cap_stream);
+    cudaGraph_t graph = nullptr;
+    cudaError_t e = cudaStreamEndCapture(s->cap_stream, &graph);
+    if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+    if (e != cudaSuccess) return fail(MD_ECUDA, "cudaStreamEndCapture: %s", cudaGetErrorString(e));
+    e = cudaGraphInstantiate(out, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e != cudaSuccess) return fail(MD_ECUDA, "cudaGraphInstantiate: %s", cudaGetErrorString(e));
+    return MD_OK;
+}
+
+} // namespace
+
+// ------------------------------------------------------------------------- C ABI --------
+
+extern "C" {
+
+const char *md_last_error(void) { return g_err; }
+
+int md_workspace_bytes(const md_config *cfg, int n, size_t *bytes) {
+    if (!bytes) return fail(MD_EINVAL, "bytes is NULL");
+    Geom g;
+    int rc = make_geom(cfg, n, &g);
+    if (rc) return rc;
+    *bytes = layout(n, g.cells).total;
+    return MD_OK;
+}
+
+int md_create(const md_config *cfg, int n, void *workspace, size_t bytes, md_system **out) {
+    if (!out) return fail(MD_EINVAL, "out is NULL");
+    *out = nullptr;
+    Geom g;
+    int rc = make_geom(cfg, n, &g);
+    if (rc) return rc;
+    Layout l = layout(n, g.cells);
+    if (!workspace || (reinterpret_cast<uintptr_t>(workspace) % ALIGN) || bytes < l.total)
+        return fail(MD_EWORKSPACE, "workspace must be a 256-byte aligned device buffer of >= %zu bytes (got %zu)", l.total, bytes);
+    cudaPointerAttributes attr;
+    CU(cudaPointerGetAttributes(&attr, workspace));
+    if (attr.type != cudaMemoryTypeDevice && attr.type != cudaMemoryTypeManaged)
+        return fail(MD_EWORKSPACE, "workspace is not device memory");
+    CU(cudaSetDevice(attr.device));
+    md_system *s = new (std::nothrow) md_system;
+    if (!s) return fail(MD_EINVAL, "out of host memory");
+    memset(s, 0, sizeof(*s));
+    s->cfg = *cfg; s->n = n; s->g = g; s->device = attr.device;
+    s->ws = (char *)workspace; s->ws_bytes = bytes;
+    s->words = (int *)(s->ws + l.words);
+    s->cell_count = (int *)(s->ws + l.cell_count);
+    s->cell_start_i = (int *)(s->ws + l.cell_start_i);
+    s->perm_i = (int *)(s->ws + l.perm_i);
+    s->cell_of = (int *)(s->ws + l.cell_of);
+    s->rank_tmp = (int *)(s->ws + l.rank_tmp);
+    s->perm_tmp = (int *)(s->ws + l.perm_tmp);
+    s->id_s = (int *)(s->ws + l.id_s);
+    s->pos_s = (float4 *)(s->ws + l.pos_s);
+    s->vel_s = (float4 *)(s->ws + l.vel_s);
+    s->ref_pos = (float4 *)(s->ws + l.ref_pos);
+    s->tpp = cfg->capacity >= 64 ? 8 : (cfg->capacity >= 32 ? 4 : 2);
+    s->thr = 16.0f;
+    s->use_graph = 1;
+    s->unroll = 8;
+    if (const char *e = getenv("MD_B200_TPP")) { int t = atoi(e); if (t == 1 || t == 2 || t == 4 || t == 8 || t == 16 || t == 32) s->tpp = t; }
+    if (const char *e = getenv("MD_B200_FP64_THRESHOLD")) s->thr = (float)atof(e);
+    if (const char *e = getenv("MD_B200_NO_GRAPH")) s->use_graph = atoi(e) ? 0 : 1;
+    cudaError_t e = cudaMemset(workspace, 0, l.total);
+    if (e == cudaSuccess) e = cudaDeviceSynchronize();
+    if (e != cudaSuccess) { delete s; return fail(MD_ECUDA, "clearing the workspace: %s", cudaGetErrorString(e)); }
+    *out = s;
+    return MD_OK;
+}
+
+int md_destroy(md_system *sys) {
+    if (!sys) return MD_OK;
+    drop_graphs(sys);
+    if (sys->cap_stream) cudaStreamDestroy(sys->cap_stream);
+    delete sys;
+    return MD_OK;
+}
+
+int md_num_cells(const md_system *sys, int *ncell) {
+    if (!sys || !ncell) return fail(MD_EINVAL, "NULL argument");
+    ncell[0] = sys->g.nc[0]; ncell[1] = sys->g.nc[1]; ncell[2] = sys->g.nc[2];
+    return MD_OK;
+}
+
+int md_nbr_layout(const md_system *sys, long *particle_stride, long *slot_stride) {
+    if (!sys || !particle_stride || !slot_stride) return fail(MD_EINVAL, "NULL argument");
+    *particle_stride = sys->g.capacity;
+    *slot_stride = 1;
+    return MD_OK;
+}
+
+int md_set_option(md_system *sys, const char *name, double value) {
+    if (!sys || !name) return fail(MD_EINVAL, "NULL argument");
+    if (!strcmp(name, "fp64_threshold")) sys->thr = (float)value;
+    else if (!strcmp(name, "threads_per_particle")) {
+        int t = (int)value;
+        if (!(t == 1 || t == 2 || t == 4 || t == 8 || t == 16 || t == 32)) return fail(MD_EINVAL, "threads_per_particle must be a power of two <= 32");
+        sys->tpp = t;
+    } else if (!strcmp(name, "use_graph")) sys->use_graph = value != 0.0;
+    else return fail(MD_EINVAL, "unknown option %s", name);
+    drop_graphs(sys);
+    return MD_OK;
+}
+
+int md_cell_list_build(md_system *sys, void *pos, void *vel, int32_t *id, int32_t *cell_start,
+                       int32_t *perm, void *stream) {
+    if (!sys || !pos || !cell_start || !perm) return fail(MD_EINVAL, "NULL argument");
+    if (!aligned16(pos) || (vel && !aligned16(vel))) return fail(MD_EINVAL, "pos/vel must be 16-byte aligned");
+    if (int rc = enter(sys)) return rc;
+    return launch_cell_build(sys, (float4 *)pos, (float4 *)vel, id, cell_start, perm, nullptr,
+                             nullptr, (cudaStream_t)stream);
+}
+
+int md_neighbor_list_build(md_system *sys, const void *pos, const int32_t *cell_start,
+                           const int32_t *perm, int32_t *nbr_idx, int32_t *nbr_count,
+                           int32_t *status, void *stream) {
+    if (!sys || !pos || !cell_start || !perm || !nbr_idx || !nbr_count || !status)
+        return fail(MD_EINVAL, "NULL argument");
+    if (!aligned16(pos) || !aligned16(nbr_idx)) return fail(MD_EINVAL, "pos/nbr_idx must be 16-byte aligned");
+    if (int rc = enter(sys)) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    CU(cudaMemsetAsync(status, 0, 2 * sizeof(int), st));
+    const float4 *spos = (const float4 *)pos;
+    const int *map = nullptr;
+    if (!sys->cfg.resort) {
+        k_gather_pos<<<blocks_for(sys->n), 256, 0, st>>>(sys->n, perm, (const float4 *)pos, sys->pos_s);
+        LAUNCH_OK();
+        spos = sys->pos_s; map = perm;
+    }
+    return launch_nbr_build(sys, spos, cell_start, map, nbr_idx, nbr_count, status, nullptr, st);
+}
+
+int md_needs_rebuild(md_system *sys, const void *pos, int32_t *flag, void *stream) {
+    if (!sys || !pos || !flag) return fail(MD_EINVAL, "NULL argument");
+    if (!aligned16(pos)) return fail(MD_EINVAL, "pos must be 16-byte aligned");
+    if (int rc = enter(sys)) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    CU(cudaMemsetAsync(flag, 0, sizeof(int), st));
+    const int nb = blocks_for(sys->n);
+    if (sys->g.dim == 3) k_needs_rebuild<3><<<nb, 256, 0, st>>>(sys->g, (const float4 *)pos, sys->ref_pos, flag);
+    else k_needs_rebuild<2><<<nb, 256, 0, st>>>(sys->g, (const float4 *)pos, sys->ref_pos, flag);
+    LAUNCH_OK();
+    return MD_OK;
+}
+
+int md_pair_energy_force(md_system *sys, const md_potential *pot, const void *pos,
+                         const int32_t *nbr_idx, const int32_t *nbr_count, void *force,
+                         double *energy_total, void *stream) {
+    if (!sys || !pos || !nbr_idx || !nbr_count || !force) return fail(MD_EINVAL, "NULL argument");
+    if (!aligned16(pos) || !aligned16(force)) return fail(MD_EINVAL, "pos/force must be 16-byte aligned");
+    Pair pp;
+    int rc = make_pair(sys, pot, &pp);
+    if (rc) return rc;
+    if ((rc = enter(sys))) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    if (energy_total) CU(cudaMemsetAsync(energy_total, 0, sizeof(double), st));
+    Book book = {nullptr, nullptr, nullptr};
+    return launch_force(sys, pp, (const float4 *)pos, nbr_idx, nbr_count, (float4 *)force, nullptr,
+                        0.0f, energy_total, book, st);
+}
+
+int md_nve_step(md_system *sys, const md_potential *pot, void *pos, void *vel, void *force,
+                int32_t *id, int32_t *nbr_idx, int32_t *nbr_count, float dt, float mass,
+                int nsteps, int32_t *stats, void *stream) {
+    if (!sys || !pos || !vel || !force || !nbr_idx || !nbr_count || !stats)
+        return fail(MD_EINVAL, "NULL argument");
+    if (!aligned16(pos) || !aligned16(vel) || !aligned16(force)) return fail(MD_EINVAL, "pos/vel/force must be 16-byte aligned");
+    if (!(dt > 0.0f) || !(mass > 0.0f) || nsteps < 0) return fail(MD_EINVAL, "dt and mass must be positive, nsteps >= 0");
+    Pair pp;
+    int rc = make_pair(sys, pot, &pp);
+    if (rc) return rc;
+    if ((rc = enter(sys))) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    k_init_stats<<<1, 1, 0, st>>>(stats, sys->words + 0);
+    LAUNCH_OK();
+    if (!sys->use_graph) {
+        for (int s = 0; s < nsteps; ++s) {
+            rc = record_step(sys, pp, (float4 *)pos, (float4 *)vel, (float4 *)force, id, nbr_idx,
+                             nbr_count, dt, mass, stats, st);
+            if (rc) return rc;
+        }
+        return MD_OK;
+    }
+    StepKey k;
+    memset(&k, 0, sizeof(k));
+    k.pos = pos; k.vel = vel; k.force = force; k.id = id; k.nbr_idx = nbr_idx;
+    k.nbr_count = nbr_count; k.stats = stats; k.dt = dt; k.mass = mass; k.pot = *pot;
+    k.tpp = sys->tpp; k.thr = sys->thr;
+    if (!sys->key_valid || memcmp(&k, &sys->key, sizeof(k)) != 0) {
+        drop_graphs(sys);
+        sys->key = k;
+        sys->key_valid = true;
+    }
+    int left = nsteps;
+    const int U = sys->unroll;
+    if (left >= U) {
+        if (!sys->execU) { rc = capture(sys, pp, k, U, &sys->execU); if (rc) return rc; }
+        for (; left >= U; left -= U) CU(cudaGraphLaunch(sys->execU, st));
+    }
+    if (left > 0) {
+        if (!sys->exec1) { rc = capture(sys, pp, k, 1, &sys->exec1); if (rc) return rc; }
+        for (; left > 0; --left) CU(cudaGraphLaunch(sys->exec1, st));
+    }
+    return MD_OK;
+}
+
+int md_nve_run_host(const md_config *cfg, const md_potential *pot, int n, void *pos_host,
+                    void *vel_host, void *force_host, double *energy_host, float dt, float mass,
+                    int nsteps, int32_t *stats_host) {
+    if (!pos_host || !vel_host) return fail(MD_EINVAL, "NULL host buffer");
+    size_t wsb = 0;
+    int rc = md_workspace_bytes(cfg, n, &wsb);
+    if (rc) return rc;
+    const size_t vec = (size_t)n * sizeof(float4);
+    const size_t list = (size_t)n * cfg->capacity * sizeof(int);
+    // one allocation: pos, vel, force, out x3, id, count, list, small words, workspace
+    size_t o = 0;
+    auto take = [&](size_t b) { size_t at = o; o += up(b); return at; };
+    const size_t o_pos = take(vec), o_vel = take(vec), o_force = take(vec), o_pos2 = take(vec),
+                 o_vel2 = take(vec), o_force2 = take(vec), o_id = take((size_t)n * 4),
+                 o_cnt = take((size_t)n * 4), o_list = take(list), o_small = take(256),
+                 o_ws = take(wsb);
+    char *d = nullptr;
+    CU(cudaMalloc(&d, o));
+    md_system *sys = nullptr;
+    cudaStream_t st = nullptr;
+    rc = md_create(cfg, n, d + o_ws, wsb, &sys);
+    auto done = [&](int code) { if (sys) md_destroy(sys); if (st) cudaStreamDestroy(st); cudaFree(d); return code; };
+    if (rc) return done(rc);
+    cudaError_t e = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking);
+    if (e != cudaSuccess) return done(fail(MD_ECUDA, "cudaStreamCreate: %s", cudaGetErrorString(e)));
+    float4 *pos = (float4 *)(d + o_pos), *vel = (float4 *)(d + o_vel), *force = (float4 *)(d + o_force);
+    int *id = (int *)(d + o_id), *cnt = (int *)(d + o_cnt), *nbr = (int *)(d + o_list);
+    int *small = (int *)(d + o_small);          // [0..1] status, [4..7] stats, [8..9] energy (double)
+    double *etot = (double *)(small + 8);
+#define RUN(x) do { e = (x); if (e != cudaSuccess) return done(fail(MD_ECUDA, "%s: %s", #x, cudaGetErrorString(e))); } while (0)
+#define STEP(x) do { rc = (x); if (rc) return done(rc); } while (0)
+    RUN(cudaMemcpyAsync(pos, pos_host, vec, cudaMemcpyHostToDevice, st));
+    RUN(cudaMemcpyAsync(vel, vel_host, vec, cudaMemcpyHostToDevice, st));
+    k_iota<<<blocks_for(n), 256, 0, st>>>(n, id);
+    STEP(md_cell_list_build(sys, pos, vel, id, sys->cell_start_i, sys->perm_i, st));
+    STEP(md_neighbor_list_build(sys, pos, sys->cell_start_i, sys->perm_i, nbr, cnt, small, st));
+    STEP(md_pair_energy_force(sys, pot, pos, nbr, cnt, force, nullptr, st));
+    STEP(md_nve_step(sys, pot, pos, vel, force, id, nbr, cnt, dt, mass, nsteps, small + 4, st));
+    if (energy_host) STEP(md_pair_energy_force(sys, pot, pos, nbr, cnt, force, etot, st));
+    k_unpermute<<<blocks_for(n), 256, 0, st>>>(n, id, pos, vel, force, (float4 *)(d + o_pos2),
+                                               (float4 *)(d + o_vel2), (float4 *)(d + o_force2));
+    RUN(cudaGetLastError());
+    RUN(cudaMemcpyAsync(pos_host, d + o_pos2, vec, cudaMemcpyDeviceToHost, st));
+    RUN(cudaMemcpyAsync(vel_host, d + o_vel2, vec, cudaMemcpyDeviceToHost, st));
+    if (force_host) RUN(cudaMemcpyAsync(force_host, d + o_force2, vec, cudaMemcpyDeviceToHost, st));
+    if (energy_host) RUN(cudaMemcpyAsync(energy_host, etot, sizeof(double), cudaMemcpyDeviceToHost, st));
+    if (stats_host) RUN(cudaMemcpyAsync(stats_host, small + 4, 4 * sizeof(int), cudaMemcpyDeviceToHost, st));
+    RUN(cudaStreamSynchronize(st));
+#undef RUN
+#undef STEP
+    return done(MD_OK);
+}
+
+} // extern "C"

@@ -139,18 +139,20 @@ def soft_disks(index: int = 1, n: int = 16384, *, phi: float = 0.90,
                     temperature=0.0, steps=steps, resort=1, pos=pos, vel=vel)
 
 
-def config(index: int) -> Workload:
-    """BASELINE.json ``configs[index]``."""
+def config(index: int, replica: int = 0) -> Workload:
+    """BASELINE.json ``configs[index]``; ``replica`` > 0 draws an independent sample of the
+    same workload (seed + 1000 * replica) for multi-GPU replica runs."""
+    seed = SEED0 + index + 1000 * replica
     if index == 0:
-        return lj_fcc(0, 6, steps=100)
+        return lj_fcc(0, 6, steps=100, seed=seed)
     if index == 1:
-        return soft_disks(1, 16384, steps=1000)
+        return soft_disks(1, 16384, steps=1000, seed=seed)
     if index == 2:
-        return lj_fcc(2, 20, steps=1000)
+        return lj_fcc(2, 20, steps=1000, seed=seed)
     if index == 3:
-        return lj_fcc(3, 40, steps=1000)
+        return lj_fcc(3, 40, steps=1000, seed=seed)
     if index == 4:
-        return lj_fcc(4, 64, temperature=2.0, skin=0.2, steps=500)
+        return lj_fcc(4, 64, temperature=2.0, skin=0.2, steps=500, seed=seed)
     raise ValueError(f"no config {index}")
 
 

@@ -1,0 +1,404 @@
+"""GPU parity tests: the CUDA path (through the C ABI) against the fp64 CPU oracle,
+element by element on the same seeded inputs (SURVEY.md §8c "Tolerances").
+
+  neighbor rows   bit-exact after sorting each row (all `capacity` slots + counts)
+  cells           identical membership, cell_start, canonical in-cell order
+  forces          max_i ||F_gpu - F_or|| / max(||F_or||, 1e-3) <= 1e-5
+  total energy    relative 1e-6
+  config 0        positions after 100 NVE steps within 1e-4 (minimum image)
+"""
+import dataclasses
+
+import numpy as np
+import pytest
+import torch
+
+pytestmark = pytest.mark.gpu
+
+FORCE_TOL = 1e-5
+ENERGY_TOL = 1e-6
+
+
+@pytest.fixture(scope="module")
+def B():
+    if not torch.cuda.is_available():
+        pytest.skip("needs a CUDA device")
+    from paper_1912_04232_b200 import build
+    build.build()
+    from paper_1912_04232_b200 import binding
+    binding.lib()
+    return binding
+
+
+def custom_workload(W, pos, box32, dim, kind, r_cut, skin, capacity, resort=1, vel=None, dt=0.005):
+    n = pos.shape[0]
+    return W.Workload(index=-1, name="custom", dim=dim, n=n, box=box32, kind=kind, epsilon=1.0,
+                      sigma=1.0, r_cut=r_cut, skin=skin, capacity=capacity, shift=1 if kind == 0 else 0,
+                      dt=dt, mass=1.0, temperature=0.0, steps=0, resort=resort, pos=pos,
+                      vel=np.zeros((n, 4), np.float32) if vel is None else vel)
+
+
+def gpu_rows_in_original_order(S):
+    """Neighbor rows of the GPU list mapped back to original particle ids, sorted."""
+    n, cap = S.n, S.capacity
+    idx = S.nbr_idx.cpu().numpy().astype(np.int64)
+    cnt = S.nbr_count.cpu().numpy()
+    ids = S.id.cpu().numpy().astype(np.int64)
+    lut = np.concatenate([ids, [n]])                 # pad value n maps to itself
+    mapped = np.sort(lut[idx], axis=1)
+    rows = np.empty_like(mapped)
+    rows[ids] = mapped
+    counts = np.empty_like(cnt)
+    counts[ids] = cnt
+    return rows.astype(np.int32), counts
+
+
+def unpermute(S, t):
+    ids = S.id.cpu().numpy().astype(np.int64)
+    a = t.cpu().numpy()
+    out = np.empty_like(a)
+    out[ids] = a
+    return out
+
+
+def force_error(f_gpu, f_or):
+    num = np.linalg.norm(f_gpu[:, :3].astype(np.float64) - f_or, axis=1)
+    return (num / np.maximum(np.linalg.norm(f_or, axis=1), 1e-3)).max()
+
+
+def check_cells(S, orc, w):
+    """md_cell_list_build vs oracle O2 (run BEFORE anything re-orders S again)."""
+    ncell, cell_of, cell_start_o, members_o = orc.cell_list(w.pos, w.box, w.dim, w.r_cut, w.skin)
+    cs = S.cell_start.cpu().numpy()
+    perm = S.perm.cpu().numpy()
+    assert np.array_equal(cs, cell_start_o)
+    assert cs[0] == 0 and cs[-1] == w.n and np.all(np.diff(cs) >= 0)
+    assert np.array_equal(np.sort(perm), np.arange(w.n))
+    # canonical order inside a cell = ascending id; on the first build id == index
+    assert np.array_equal(perm, members_o)
+    if S.cfg.resort:
+        assert np.array_equal(S.pos.cpu().numpy(), w.pos[perm])
+        assert np.array_equal(S.vel.cpu().numpy(), w.vel[perm])
+        assert np.array_equal(S.id.cpu().numpy(), perm)
+    else:
+        assert np.array_equal(S.pos.cpu().numpy(), w.pos)
+        assert np.array_equal(S.id.cpu().numpy(), np.arange(w.n))
+
+
+def check_list(S, orc, w, method):
+    rows, counts = gpu_rows_in_original_order(S)
+    idx_o, cnt_o, st_o = orc.neighbor_list(w.pos, w.box, w.dim, w.r_cut, w.skin, S.capacity,
+                                           predicate=0, method=method)
+    st = S.status.cpu().numpy()
+    assert np.array_equal(counts, cnt_o)
+    assert st[1] == st_o[1] and st[0] == st_o[0]
+    if st_o[0] == 0:
+        assert np.array_equal(rows, idx_o)
+    return idx_o, cnt_o
+
+
+def check_force(S, orc, w, idx_o=None, cnt_o=None):
+    S.compute_force(want_energy=True)
+    f = unpermute(S, S.force)
+    E = float(S.energy.cpu()[0])
+    diam = w.pos[:, 3].astype(np.float64)
+    f_o, e_o, E_o = orc.energy_force(w.pos, diam, w.box, w.dim, w.kind, w.epsilon, w.sigma,
+                                     float(np.float32(w.r_cut)), w.shift, idx_o, cnt_o)
+    err = force_error(f, f_o)
+    assert err <= FORCE_TOL, err
+    assert abs(E - E_o) <= ENERGY_TOL * abs(E_o), (E, E_o)
+    assert np.abs(f[:, 3] - e_o).max() <= 2e-6 * max(1.0, np.abs(e_o).max())
+    if w.dim == 2:
+        assert np.all(f[:, 2] == 0.0)
+    zero = np.linalg.norm(f_o, axis=1) == 0.0
+    if zero.any():
+        assert np.linalg.norm(f[zero, :3], axis=1).max() <= 1e-8
+    return err
+
+
+# ----------------------------------------------------------------- configs 0, 1, 2 ------
+
+@pytest.mark.parametrize("ci", [0, 1, 2])
+@pytest.mark.parametrize("resort", [1, 0])
+def test_config_build_and_force_parity(B, orc, W, ci, resort):
+    w = W.config(ci)
+    S = B.System(w, resort=resort)
+    S.build()
+    torch.cuda.synchronize()
+    check_cells(S, orc, w)
+    idx_o, cnt_o = check_list(S, orc, w, method=0)        # oracle brute force O(N^2)
+    check_force(S, orc, w)                                # oracle all-pairs definition
+    S.close()
+
+
+@pytest.mark.parametrize("thr", [0.0, 1e30])
+def test_precision_modes(B, orc, W, thr):
+    """thr = 0: every particle through the fp64 chain (must pass); thr = inf: fp32 only --
+    documents why the adaptive re-evaluation exists (errors stay small but are not bounded)."""
+    w = W.config(2)
+    S = B.System(w)
+    S.build()
+    B.md_set_option(S.sys, "fp64_threshold", thr)
+    S.compute_force()
+    f = unpermute(S, S.force)
+    f_o, _, E_o = orc.energy_force(w.pos, None, w.box, 3, 0, 1.0, 1.0, 2.5, 1)
+    err = force_error(f, f_o)
+    if thr == 0.0:
+        assert err <= 2e-7                                  # fp64 chain: only the fp32 store rounds
+    else:
+        assert err <= 1e-3
+    assert abs(float(S.energy.cpu()[0]) - E_o) <= ENERGY_TOL * abs(E_o)
+    S.close()
+
+
+@pytest.mark.parametrize("tpp", [1, 2, 4, 8, 16, 32])
+def test_threads_per_particle_variants(B, orc, W, tpp):
+    w = W.config(0)
+    S = B.System(w)
+    S.build()
+    B.md_set_option(S.sys, "threads_per_particle", tpp)
+    check_force(S, orc, w)
+    S.close()
+
+
+# --------------------------------------------------------------------- edge cases -------
+
+def edge_positions(W, seed, n, dim, box, R):
+    pos, box32 = W.random_box(seed, n, dim, box, diam=(1.0, 1.4))
+    for k in range(dim):
+        L = box32[k]
+        nk = int(np.floor(float(L) / float(R)))
+        specials = [np.float32(0.0), np.nextafter(L, np.float32(0.0), dtype=np.float32)]
+        for c in range(1, nk):
+            face = np.float32(c * float(L) / nk)
+            specials += [face, np.nextafter(face, np.float32(0), dtype=np.float32),
+                         np.nextafter(face, np.float32(1e9), dtype=np.float32)]
+        for s, x in enumerate(specials):
+            pos[(7 * s + 3 * k) % n, k] = x
+    return pos, box32
+
+
+@pytest.mark.parametrize("dim,box,n", [
+    (3, [3.9, 5.2, 6.4], 700),       # 3 x 4 x 5 cells, ragged n
+    (3, [3.76, 3.76, 3.76], 333),    # 3 cells per side: every cell is a periodic neighbor
+    (2, [3.8, 6.3], 257),            # 2-D, 3 x 5 cells
+    (2, [13.0, 4.0], 64),            # many empty cells
+    (3, [5.01, 5.01, 5.01], 1),      # a single particle
+    (3, [5.01, 5.01, 5.01], 2),
+    (3, [40.0, 4.0, 4.0], 50),       # sparse: most cells empty
+])
+@pytest.mark.parametrize("kind", [0, 1])
+def test_edge_cases(B, orc, W, dim, box, n, kind):
+    r_cut, skin = 1.0, 0.25
+    R = np.float32(np.float32(r_cut) + np.float32(skin))
+    pos, box32 = edge_positions(W, 100 + n, n, dim, box, R)
+    if kind == 0:
+        pos[:, 3] = 1.0
+    else:
+        pos[:, 3] = np.where(np.arange(n) < n // 2, 0.7, 1.0)   # d_ij <= 1.0 = list r_cut
+    w = custom_workload(W, pos, box32, dim, kind, r_cut, skin, 192)
+    if kind == 0:
+        w = dataclasses.replace(w, sigma=0.4)    # keeps LJ forces representable at random overlaps
+    for resort in (1, 0):
+        S = B.System(w, resort=resort)
+        S.build()
+        torch.cuda.synchronize()
+        check_cells(S, orc, w)
+        check_list(S, orc, w, method=0)
+        if kind == 1:
+            check_force(S, orc, w)
+        else:
+            # random overlaps give |F| ~ 1e9: compare where the oracle force is sane
+            S.compute_force()
+            f = unpermute(S, S.force)
+            f_o, _, _ = orc.energy_force(w.pos, None, w.box, dim, 0, 1.0, 0.4, float(np.float32(r_cut)), 1)
+            num = np.linalg.norm(f[:, :3].astype(np.float64) - f_o, axis=1)
+            assert (num / np.maximum(np.linalg.norm(f_o, axis=1), 1e-3)).max() <= FORCE_TOL
+        S.close()
+
+
+def test_overflow_flag(B, orc, W):
+    """Static capacity: capacity 64 on config 0 overflows; counts stay true."""
+    w = W.config(0)
+    S = B.System(w, capacity=64)
+    S.build()
+    st = S.status.cpu().numpy()
+    idx_o, cnt_o, st_o = orc.neighbor_list(w.pos, w.box, 3, w.r_cut, w.skin, 64)
+    assert st[0] == 1 and st_o[0] == 1 and st[1] == st_o[1]
+    _, counts = gpu_rows_in_original_order(S)
+    assert np.array_equal(counts, cnt_o)
+    # a later build with room clears the flag
+    S2 = B.System(w, capacity=128)
+    S2.build()
+    assert S2.status.cpu().numpy()[0] == 0
+    S.close(); S2.close()
+
+
+def test_needs_rebuild_constructed(B, orc, W):
+    """P9: half-skin criterion, strict, minimum image."""
+    w = W.config(0)
+    S = B.System(w, resort=0)
+    S.build()
+    ref = S.pos.clone()
+    half = w.skin / 2
+    u = np.array([1.0, 2.0, -2.0]) / 3.0
+
+    def flag_for(p):
+        B.md_needs_rebuild(S.sys, p, S.flag)
+        return int(S.flag.cpu()[0])
+
+    assert flag_for(ref) == 0
+    for scale, want in [(1 - 1e-3, 0), (1 + 1e-3, 1)]:
+        p = ref.clone()
+        x = ref[100, :3].cpu().numpy().astype(np.float64) + u * half * scale
+        p[100, :3] = torch.from_numpy(np.mod(x, w.box).astype(np.float32)).cuda()
+        assert flag_for(p) == want
+        o_flag, _ = orc.needs_rebuild(p.cpu().numpy(), ref.cpu().numpy(), w.box, 3, w.skin)
+        assert o_flag == want
+    # crossing the periodic boundary by 0.01 is a small displacement
+    refc = ref.clone(); refc[5, 0] = 0.004
+    S.pos.copy_(refc); S.build()
+    p = S.pos.clone(); p[5, 0] = float(w.box[0]) - 0.006
+    assert flag_for(p) == 0
+    S.close()
+
+
+# ------------------------------------------------------------------ NVE trajectory ------
+
+def test_nve_config0_trajectory(B, orc, W):
+    """north_star: positions after 100 NVE steps on config 0 within 1e-4 sigma."""
+    w = W.config(0)
+    S = B.System(w)
+    S.build()
+    S.compute_force()
+    f0, _, E0 = orc.energy_force(w.pos, None, w.box, 3, 0, 1.0, 1.0, 2.5, 1)
+    p_o, v_o, f_o, en, _ = orc.nve_run(w.pos, w.vel, f0, None, w.box, 3, 0, 1.0, 1.0, 2.5, 1,
+                                       w.dt, w.mass, w.steps)          # brute force, no list
+    S.step(w.steps)
+    torch.cuda.synchronize()
+    stats = S.stats.cpu().numpy()
+    assert stats[0] == w.steps and 5 <= stats[1] <= 20 and stats[2] == -1 and 70 < stats[3] < 128
+    p = unpermute(S, S.pos)[:, :3].astype(np.float64)
+    d = p - p_o
+    d -= w.box.astype(np.float64) * np.round(d / w.box.astype(np.float64))
+    assert np.abs(d).max() <= 1e-4, np.abs(d).max()
+    v = unpermute(S, S.vel)[:, :3].astype(np.float64)
+    assert np.abs(v - v_o).max() <= 2e-3
+    # positions stay inside the box; ids are a permutation
+    pg = S.pos.cpu().numpy()
+    assert pg[:, :3].min() >= 0 and np.all(pg[:, :3] < w.box)
+    assert np.array_equal(np.sort(S.id.cpu().numpy()), np.arange(w.n))
+    # the final force is F(final positions): snapshot parity
+    w2 = dataclasses.replace(w, pos=unpermute(S, S.pos))
+    f2, _, _ = orc.energy_force(w2.pos, None, w.box, 3, 0, 1.0, 1.0, 2.5, 1)
+    assert force_error(unpermute(S, S.force), f2) <= FORCE_TOL
+    # graph and direct launches give the same bits
+    S2 = B.System(w)
+    B.md_set_option(S2.sys, "use_graph", 0)
+    S2.build(); S2.compute_force(); S2.step(w.steps)
+    assert torch.equal(S2.pos, S.pos) and torch.equal(S2.vel, S.vel)
+    # splitting the run does not change the result (stats restart per call)
+    S3 = B.System(w)
+    S3.build(); S3.compute_force(); S3.step(37); S3.step(w.steps - 37)
+    assert torch.equal(S3.pos, S.pos) and torch.equal(S3.vel, S.vel)
+    S.close(); S2.close(); S3.close()
+
+
+def test_nve_run_host_matches_device_path(B, W):
+    w = W.config(0)
+    S = B.System(w)
+    S.build(); S.compute_force(); S.step(50); S.compute_force()
+    pos = w.pos.copy(); vel = w.vel.copy(); force = np.zeros_like(pos)
+    stats = np.zeros(4, np.int32)
+    E = B.md_nve_run_host(S.cfg, S.pot, pos, vel, force, w.dt, w.mass, 50, stats)
+    assert np.array_equal(pos, unpermute(S, S.pos))
+    assert np.array_equal(vel, unpermute(S, S.vel))
+    assert np.array_equal(force, unpermute(S, S.force))
+    assert abs(E - float(S.energy.cpu()[0])) <= 1e-9 * abs(E)
+    assert np.array_equal(stats, S.stats.cpu().numpy())
+    S.close()
+
+
+def snapshot_checks(B, orc, W, w, steps, method=1):
+    """State-wise parity along a trajectory (SURVEY §8c last row of P): run on the GPU, then
+    hand the GPU snapshot to the oracle and compare list / force / energy at that state; plus
+    momentum and energy invariants."""
+    S = B.System(w)
+    S.build(); S.compute_force()
+    E_pot0 = float(S.energy.cpu()[0])
+    ke0 = 0.5 * w.mass * float((S.vel[:, :3].double() ** 2).sum())
+    mom0 = S.vel[:, :3].double().sum(0).cpu().numpy()
+    S.step(steps)
+    S.compute_force()
+    torch.cuda.synchronize()
+    stats = S.stats.cpu().numpy()
+    assert stats[0] == steps and stats[2] == -1
+    E_pot1 = float(S.energy.cpu()[0])
+    ke1 = 0.5 * w.mass * float((S.vel[:, :3].double() ** 2).sum())
+    mom1 = S.vel[:, :3].double().sum(0).cpu().numpy()
+    assert np.abs(mom1 - mom0).max() <= 2e-5 * np.sqrt(w.n) * max(1.0, w.temperature) + 1e-3
+    assert abs((ke1 + E_pot1) - (ke0 + E_pot0)) <= 5e-4 * abs(ke0 + E_pot0) + 1e-3 * w.n * (w.kind == 1)
+    # Newton's third law on the GPU forces (P5)
+    F = S.force[:, :3].double()
+    assert F.sum(0).abs().max().item() <= 1e-5 * F.norm(dim=1).mean().item() * np.sqrt(w.n)
+    # snapshot -> oracle
+    snap = dataclasses.replace(w, pos=unpermute(S, S.pos))
+    diam = snap.pos[:, 3].astype(np.float64)
+    idx_o, cnt_o, st_o = orc.neighbor_list(snap.pos, w.box, w.dim, w.r_cut, w.skin, w.capacity,
+                                           predicate=1, method=1)
+    f_o, e_o, E_o = orc.energy_force(snap.pos, diam, w.box, w.dim, w.kind, w.epsilon, w.sigma,
+                                     float(np.float32(w.r_cut)), w.shift, idx_o, cnt_o)
+    f = unpermute(S, S.force)
+    assert force_error(f, f_o) <= FORCE_TOL
+    assert abs(E_pot1 - E_o) <= ENERGY_TOL * abs(E_o)
+    # the list in use is still valid: it contains every pair within r_cut of the snapshot
+    rows, counts = gpu_rows_in_original_order(S)
+    idx_c, cnt_c, _ = orc.neighbor_list(snap.pos, w.box, w.dim, float(np.float32(w.r_cut)) * (1 - 1e-6), 0.0,
+                                        w.capacity, predicate=1, method=1)
+    for i in range(0, w.n, max(1, w.n // 2000)):
+        need = set(idx_c[i, : cnt_c[i]].tolist())
+        have = set(rows[i, : counts[i]].tolist())
+        assert need <= have
+    # a fresh build on the snapshot is bit-exact against the oracle's canonical list
+    S2 = B.System(snap)
+    S2.build()
+    check_list(S2, orc, snap, method=method)
+    S2.close()
+    rebuilds = int(stats[1])
+    S.close()
+    return rebuilds
+
+
+def test_config1_snapshots(B, orc, W):
+    w = W.config(1)
+    rebuilds = snapshot_checks(B, orc, W, w, 300)
+    assert rebuilds >= 5
+
+
+def test_config2_snapshots(B, orc, W):
+    w = W.config(2)
+    rebuilds = snapshot_checks(B, orc, W, w, 200)
+    assert 10 <= rebuilds <= 60
+
+
+# ---------------------------------------------- full sizes, bench launch configuration ----
+
+@pytest.mark.parametrize("ci,steps", [(3, 100), (4, 30)])
+def test_full_size_configs(B, orc, W, ci, steps):
+    """Configs 3 and 4 at BASELINE.json's full sizes, in the launch configuration bench.py
+    times (re-sort on, CUDA graph, default threads per particle): bit-exact list and force /
+    energy parity at step 0 against the oracle's cell-binned search, then snapshot parity."""
+    w = W.config(ci)
+    S = B.System(w)
+    S.build()
+    torch.cuda.synchronize()
+    check_cells(S, orc, w)
+    idx_o, cnt_o = check_list(S, orc, w, method=1)
+    # oracle force over its own fp64 list (equal to all pairs by construction)
+    idx64, cnt64, _ = orc.neighbor_list(w.pos, w.box, 3, w.r_cut, w.skin, w.capacity, predicate=1, method=1)
+    check_force(S, orc, w, idx64, cnt64)
+    S.close()
+    del S
+    torch.cuda.empty_cache()
+    rebuilds = snapshot_checks(B, orc, W, w, steps)
+    assert rebuilds >= 3
