@@ -38,7 +38,7 @@ extern "C" {
 
 #define MD_OK          0
 #define MD_EINVAL     (-1)  /* null/unaligned pointer, n<=0, dim not 2|3, capacity<=0 or not a
-                               multiple of 4, skin<0, r_cut<=0, dt<=0, mass<=0, unknown kind */
+                               multiple of 4, skin<0, r_cut<=0, dt<=0, mass<=0, epsilon<=0, unknown kind or option */
 #define MD_EBOX       (-2)  /* a box side holds fewer than 3 cells of side >= r_cut+skin, or the
                                cell side exceeds r_cut+skin by less than 1e-5 of the box side */
 #define MD_EWORKSPACE (-3)  /* workspace null, unaligned (256 B) or too small */
@@ -82,18 +82,25 @@ int md_create(const md_config *cfg, int n, void *workspace, size_t bytes, md_sys
 int md_destroy(md_system *sys);
 
 /* Tuning knobs (host call; drops the cached step graph):
- *   "fp64_threshold"       re-evaluate a particle in fp64 when S > value * max(|F|, 1e-3)
- *                          (default 16; <= 0: every particle in fp64; 1e30: never)
- *   "threads_per_particle" lanes sharing one neighbor row in the force kernel (1..32, 2^k)
+ *   "threads_per_particle" force kernel variant: 0 = streaming kernel (one lane per particle,
+ *                          list rows staged through shared memory by TMA; default for
+ *                          n >= 32768), or 1, 2, 4 lanes sharing one particle (default 4 below)
  *   "use_graph"            0: md_nve_step launches kernels directly instead of a CUDA graph */
 int md_set_option(md_system *sys, const char *name, double value);
 
 /* Cells per side n_k = floor(L_k / R) (1 for unused dimensions) -> host int[3]. */
 int md_num_cells(const md_system *sys, int *ncell);
 
-/* Entry (i,k) of a neighbor list lives at nbr_idx[i*particle_stride + k*slot_stride]
- * (host out-pointers; currently capacity and 1: row-major rows). */
-int md_nbr_layout(const md_system *sys, long *particle_stride, long *slot_stride);
+/*
+ * Layout of a neighbor list (host out-pointers).  The dense N x capacity list of L74 is stored
+ * in tiles of `tile` consecutive particles, slot-major inside a tile, so that the 32 lanes of a
+ * warp read slot k of 32 particles as one 128-byte row: entry (i, k) lives at
+ *     nbr_idx[(i / tile) * tile_stride + (i % tile) * particle_stride + k * slot_stride]
+ * (currently tile = 32, tile_stride = 32 * capacity, particle_stride = 1, slot_stride = 32) and
+ * a list buffer holds `length` = ceil(n / tile) * tile_stride int32.
+ */
+int md_nbr_layout(const md_system *sys, long *tile, long *tile_stride, long *particle_stride,
+                  long *slot_stride, long *length);
 
 /*
  * Cell list (L84 "partition.cell_list ... places them into cells where each cell has size
@@ -114,8 +121,8 @@ int md_cell_list_build(md_system *sys, void *pos, void *vel, int32_t *id,
  * (nearest-image displacement with the box side subtracted from the larger
  * coordinate first; r2 = fma(dz,dz, fma(dy,dy, dx*dx)); strict <).
  *   pos        as left by md_cell_list_build (same cell_start / perm)
- *   nbr_idx    int32[n*capacity] out: row i holds min(count_i, capacity) neighbor indices
- *              (in the particle order of `pos`), then the pad value n up to capacity;
+ *   nbr_idx    int32[length] out (md_nbr_layout): row i holds min(count_i, capacity) neighbor
+ *              indices (in the particle order of `pos`), then the pad value n up to capacity;
  *              order within a row is unspecified
  *   nbr_count  int32[n] out: TRUE count, may exceed capacity
  *   status     int32[2] out: {1 if any count > capacity else 0, max true count}; rows of an
@@ -138,8 +145,10 @@ int md_needs_rebuild(md_system *sys, const void *pos, int32_t *flag, void *strea
  *   SOFT u = eps/2 (1 - r/d_ij)^2, r < d_ij = (pos_i.w + pos_j.w)/2; r = 0: eps/2, no force
  *   force        float4[n] out: (F_i, e_i)
  *   energy_total double* out (may be NULL): sum_i e_i accumulated in fp64
- * Pair terms are evaluated and accumulated in fp64 from fp32 displacements and rounded to
- * fp32 on store.
+ *   nbr_idx / nbr_count  any list in the md_nbr_layout layout whose rows hold every pair
+ *                        within the potential's range (entries beyond it contribute nothing)
+ * Pair terms are evaluated and accumulated in fp64 from exact displacements and rounded to fp32
+ * once, on store.
  */
 int md_pair_energy_force(md_system *sys, const md_potential *pot, const void *pos,
                          const int32_t *nbr_idx, const int32_t *nbr_count, void *force,
@@ -152,7 +161,8 @@ int md_pair_energy_force(md_system *sys, const md_potential *pot, const void *po
  * with the rebuild decision taken on the device.  `force` must hold F(pos) on entry (call
  * md_neighbor_list_build + md_pair_energy_force once first); nbr_idx / nbr_count must be the
  * list of that build.  On exit pos/vel/force are the state after nsteps in the CURRENT
- * particle order; id[s] (may be NULL) = original index of the particle in slot s.
+ * particle order; id[s] (may be NULL) = original index of the particle in slot s.  force.w is
+ * left 0: the step loop does not evaluate energies (call md_pair_energy_force for e_i and E).
  *   stats int32[4] out: {steps done, rebuilds, first step (0-based) whose rebuild
  *                        overflowed or -1, max neighbor count seen in rebuilds}
  * stats is reset at the start of every call.

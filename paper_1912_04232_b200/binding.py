@@ -62,7 +62,7 @@ def lib():
         L.md_destroy.argtypes = [vp]
         L.md_set_option.argtypes = [vp, C.c_char_p, C.c_double]
         L.md_num_cells.argtypes = [vp, C.POINTER(C.c_int * 3)]
-        L.md_nbr_layout.argtypes = [vp, C.POINTER(C.c_long), C.POINTER(C.c_long)]
+        L.md_nbr_layout.argtypes = [vp] + [C.POINTER(C.c_long)] * 5
         L.md_cell_list_build.argtypes = [vp, vp, vp, ip, ip, ip, vp]
         L.md_neighbor_list_build.argtypes = [vp, vp, ip, ip, ip, ip, ip, vp]
         L.md_needs_rebuild.argtypes = [vp, vp, ip, vp]
@@ -146,9 +146,18 @@ def md_num_cells(sys):
 
 
 def md_nbr_layout(sys):
-    a, b = C.c_long(0), C.c_long(0)
-    _check(lib().md_nbr_layout(sys, C.byref(a), C.byref(b)))
-    return int(a.value), int(b.value)
+    """(tile, tile_stride, particle_stride, slot_stride, length), see include/md.h."""
+    v = [C.c_long(0) for _ in range(5)]
+    _check(lib().md_nbr_layout(sys, *[C.byref(x) for x in v]))
+    return tuple(int(x.value) for x in v)
+
+
+def nbr_offsets(layout, n, capacity, device=None):
+    """int64[n, capacity] offsets of entry (i, k) in a list buffer (index marshalling only)."""
+    tile, tile_stride, p_stride, s_stride, _ = layout
+    i = torch.arange(n, dtype=torch.int64, device=device)[:, None]
+    k = torch.arange(capacity, dtype=torch.int64, device=device)[None, :]
+    return (i // tile) * tile_stride + (i % tile) * p_stride + k * s_stride
 
 
 def md_cell_list_build(sys, pos, vel, id, cell_start, perm, stream=None) -> None:
@@ -216,12 +225,23 @@ class System:
         self.id = torch.arange(n, dtype=torch.int32, device=dev)
         self.cell_start = torch.zeros(self.cells + 1, dtype=torch.int32, device=dev)
         self.perm = torch.zeros(n, dtype=torch.int32, device=dev)
-        self.nbr_idx = torch.full((n, cap), -1, dtype=torch.int32, device=dev)
+        self.layout = md_nbr_layout(self.sys)
+        self.nbr_idx = torch.full((self.layout[4],), -1, dtype=torch.int32, device=dev)
         self.nbr_count = torch.zeros(n, dtype=torch.int32, device=dev)
         self.status = torch.zeros(2, dtype=torch.int32, device=dev)
         self.flag = torch.zeros(1, dtype=torch.int32, device=dev)
         self.stats = torch.zeros(4, dtype=torch.int32, device=dev)
         self.energy = torch.zeros(1, dtype=torch.float64, device=dev)
+
+    def nbr_rows(self):
+        """The list as a dense int32[n, capacity] tensor (row i = neighbors of particle i)."""
+        return self.nbr_idx[nbr_offsets(self.layout, self.n, self.capacity, self.device)]
+
+    def set_nbr_rows(self, rows, counts):
+        """Load a dense int32[n, capacity] list (e.g. one built elsewhere) into the layout."""
+        off = nbr_offsets(self.layout, self.n, self.capacity, self.device)
+        self.nbr_idx[off.reshape(-1)] = torch.as_tensor(rows, dtype=torch.int32, device=self.device).reshape(-1)
+        self.nbr_count.copy_(torch.as_tensor(counts, dtype=torch.int32))
 
     def reset(self):
         self.pos.copy_(torch.from_numpy(self.w.pos))

@@ -51,7 +51,6 @@ struct StepKey {
     float dt, mass;
     md_potential pot;
     int tpp;
-    float thr;
 };
 
 } // namespace
@@ -68,8 +67,9 @@ struct md_system {
     int *cell_count, *cell_start_i, *perm_i, *cell_of, *rank_tmp, *perm_tmp, *id_s;
     float4 *pos_s, *vel_s, *ref_pos;
     // tuning
-    int tpp;
-    float thr;           // fp64 re-evaluation threshold on S / max(|F|, 1e-3)
+    int tpp;             // lanes per particle in the force kernel (1, 2, 4)
+    int nb_warps;        // tiles per block in the neighbor-list builder
+    size_t nb_smem;      // its dynamic shared memory per block
     int use_graph;
     // graph cache of md_nve_step
     cudaStream_t cap_stream;
@@ -152,20 +152,19 @@ int make_geom(const md_config *cfg, int n, Geom *g) {
 int make_pair(const md_system *sys, const md_potential *pot, Pair *pp) {
     if (!pot) return fail(MD_EINVAL, "potential is NULL");
     if (pot->kind != MD_KIND_LJ && pot->kind != MD_KIND_SOFT) return fail(MD_EINVAL, "unknown potential kind %d", pot->kind);
+    if (!(pot->epsilon > 0.0f)) return fail(MD_EINVAL, "epsilon must be positive");
     memset(pp, 0, sizeof(*pp));
     pp->kind = pot->kind;
-    pp->eps = pot->epsilon; pp->deps = (double)pot->epsilon;
-    pp->thr = sys->thr;
+    pp->deps = (double)pot->epsilon;
     if (pot->kind == MD_KIND_LJ) {
         if (!(pot->r_cut > 0.0f) || !(pot->sigma > 0.0f)) return fail(MD_EINVAL, "LJ needs sigma > 0 and r_cut > 0");
         if (pot->r_cut > sys->cfg.r_cut) return fail(MD_EINVAL, "potential r_cut %g exceeds the list r_cut %g", pot->r_cut, sys->cfg.r_cut);
         const double s = pot->sigma, rc = pot->r_cut;
-        pp->dsig2 = s * s; pp->drc2 = rc * rc;
+        pp->dsig6x2 = 2.0 * std::pow(s, 6.0); pp->drc2 = rc * rc;
         const double s6 = std::pow(s / rc, 6.0);
-        pp->du_cut = pot->shift ? 4.0 * pp->deps * (s6 * s6 - s6) : 0.0;
-        pp->sig2 = (float)pp->dsig2; pp->rc2 = (float)pp->drc2; pp->u_cut = (float)pp->du_cut;
+        pp->du_cut4 = pot->shift ? (s6 * s6 - s6) : 0.0;
     } else {
-        pp->sig2 = 1.0f; pp->dsig2 = 1.0; pp->rc2 = 3.0e38f; pp->drc2 = 1e300;
+        pp->dsig6x2 = 2.0; pp->drc2 = 1e300;
     }
     return MD_OK;
 }
@@ -198,29 +197,39 @@ int launch_cell_build(md_system *s, float4 *pos, float4 *vel, int *id, int *cell
 int launch_nbr_build(md_system *s, const float4 *spos, const int *cell_start, const int *map,
                      int *nbr_idx, int *nbr_count, int *status, const int *cond, cudaStream_t st) {
     const Geom &g = s->g;
-    const int nb = blocks_for((long long)g.n * 32);
-    if (g.dim == 3)
-        k_nbr_build<3><<<nb, 256, 0, st>>>(g, spos, cell_start, map, nbr_idx, nbr_count, status, s->ref_pos, cond);
-    else
-        k_nbr_build<2><<<nb, 256, 0, st>>>(g, spos, cell_start, map, nbr_idx, nbr_count, status, s->ref_pos, cond);
+    const int ntiles = (g.n + TILE - 1) / TILE;
+    const int nb = (ntiles + s->nb_warps - 1) / s->nb_warps;
+    const int threads = s->nb_warps * 32;
+    if (g.dim == 3) {
+        if (map) k_nbr_build<3, true><<<nb, threads, s->nb_smem, st>>>(g, spos, cell_start, map, nbr_idx, nbr_count, status, s->ref_pos, cond);
+        else k_nbr_build<3, false><<<nb, threads, s->nb_smem, st>>>(g, spos, cell_start, map, nbr_idx, nbr_count, status, s->ref_pos, cond);
+    } else {
+        if (map) k_nbr_build<2, true><<<nb, threads, s->nb_smem, st>>>(g, spos, cell_start, map, nbr_idx, nbr_count, status, s->ref_pos, cond);
+        else k_nbr_build<2, false><<<nb, threads, s->nb_smem, st>>>(g, spos, cell_start, map, nbr_idx, nbr_count, status, s->ref_pos, cond);
+    }
     LAUNCH_OK();
     return MD_OK;
 }
 
-template <int KIND, int DIM>
+template <int KIND, int DIM, bool ENERGY>
 int launch_force_t(md_system *s, const Pair &pp, const float4 *pos, const int *nbr_idx,
                    const int *nbr_count, float4 *force, float4 *vel, float a, double *etot,
                    Book book, cudaStream_t st) {
     const Geom &g = s->g;
-    const int nb = blocks_for((long long)g.n * s->tpp);
+    if (s->tpp == 0) {          // streaming kernel: one lane per particle, one warp per list tile
+        k_force_stream<KIND, DIM, ENERGY><<<blocks_for(g.n, FS_WARPS * 32), FS_WARPS * 32, 0, st>>>(
+            g, pp, pos, nbr_idx, nbr_count, force, vel, a, etot, book);
+        LAUNCH_OK();
+        return MD_OK;
+    }
+    const int nb = blocks_for((long long)g.n * s->tpp, 128);
 #define MD_FORCE_CASE(T)                                                                       \
     case T:                                                                                    \
-        k_force<KIND, DIM, T><<<nb, 256, 0, st>>>(g, pp, pos, nbr_idx, nbr_count, force, vel, \
-                                                  a, etot, book);                             \
+        k_force<KIND, DIM, T, ENERGY><<<nb, 128, 0, st>>>(g, pp, pos, nbr_idx, nbr_count,     \
+                                                          force, vel, a, etot, book);         \
         break;
     switch (s->tpp) {
-        MD_FORCE_CASE(1) MD_FORCE_CASE(2) MD_FORCE_CASE(4) MD_FORCE_CASE(8) MD_FORCE_CASE(16)
-        MD_FORCE_CASE(32)
+        MD_FORCE_CASE(1) MD_FORCE_CASE(2) MD_FORCE_CASE(4)
     default: return fail(MD_EINVAL, "threads per particle %d", s->tpp);
     }
 #undef MD_FORCE_CASE
@@ -228,14 +237,19 @@ int launch_force_t(md_system *s, const Pair &pp, const float4 *pos, const int *n
     return MD_OK;
 }
 
+// want_energy: also e_i into force.w (and the fp64 total when etot != NULL); the step loop
+// does not need it and skips those fp64 operations (force.w = 0 there).
 int launch_force(md_system *s, const Pair &pp, const float4 *pos, const int *nbr_idx,
                  const int *nbr_count, float4 *force, float4 *vel, float a, double *etot,
-                 Book book, cudaStream_t st) {
-    if (pp.kind == MD_KIND_LJ)
-        return s->g.dim == 3 ? launch_force_t<0, 3>(s, pp, pos, nbr_idx, nbr_count, force, vel, a, etot, book, st)
-                             : launch_force_t<0, 2>(s, pp, pos, nbr_idx, nbr_count, force, vel, a, etot, book, st);
-    return s->g.dim == 3 ? launch_force_t<1, 3>(s, pp, pos, nbr_idx, nbr_count, force, vel, a, etot, book, st)
-                         : launch_force_t<1, 2>(s, pp, pos, nbr_idx, nbr_count, force, vel, a, etot, book, st);
+                 bool want_energy, Book book, cudaStream_t st) {
+#define MD_FORCE_DISPATCH(K, D)                                                                 \
+    (want_energy ? launch_force_t<K, D, true>(s, pp, pos, nbr_idx, nbr_count, force, vel, a,   \
+                                              etot, book, st)                                  \
+                 : launch_force_t<K, D, false>(s, pp, pos, nbr_idx, nbr_count, force, vel, a,  \
+                                               etot, book, st))
+    if (pp.kind == MD_KIND_LJ) return s->g.dim == 3 ? MD_FORCE_DISPATCH(0, 3) : MD_FORCE_DISPATCH(0, 2);
+    return s->g.dim == 3 ? MD_FORCE_DISPATCH(1, 3) : MD_FORCE_DISPATCH(1, 2);
+#undef MD_FORCE_DISPATCH
 }
 
 __global__ void k_init_stats(int *stats, int *flag) {
@@ -275,7 +289,7 @@ int record_step(md_system *s, const Pair &pp, float4 *pos, float4 *vel, float4 *
                           nbr_idx, nbr_count, status, flag, st);
     if (rc) return rc;
     Book book = {flag, status, stats};
-    return launch_force(s, pp, pos, nbr_idx, nbr_count, force, vel, a, nullptr, book, st);
+    return launch_force(s, pp, pos, nbr_idx, nbr_count, force, vel, a, nullptr, false, book, st);
 }
 
 void drop_graphs(md_system *s) {
@@ -350,13 +364,30 @@ int md_create(const md_config *cfg, int n, void *workspace, size_t bytes, md_sys
     s->pos_s = (float4 *)(s->ws + l.pos_s);
     s->vel_s = (float4 *)(s->ws + l.vel_s);
     s->ref_pos = (float4 *)(s->ws + l.ref_pos);
-    s->tpp = cfg->capacity >= 64 ? 8 : (cfg->capacity >= 32 ? 4 : 2);
-    s->thr = 16.0f;
+    s->tpp = n >= 32768 ? 0 : 4;     // 0 = streaming kernel; small systems: 4 lanes per particle
     s->use_graph = 1;
     s->unroll = 8;
-    if (const char *e = getenv("MD_B200_TPP")) { int t = atoi(e); if (t == 1 || t == 2 || t == 4 || t == 8 || t == 16 || t == 32) s->tpp = t; }
-    if (const char *e = getenv("MD_B200_FP64_THRESHOLD")) s->thr = (float)atof(e);
+    if (const char *e = getenv("MD_B200_TPP")) { int t = atoi(e); if (t == 0 || t == 1 || t == 2 || t == 4) s->tpp = t; }
     if (const char *e = getenv("MD_B200_NO_GRAPH")) s->use_graph = atoi(e) ? 0 : 1;
+    {   // neighbor-list builder: one warp per tile, a capacity x 32 column block + a candidate
+        // chunk of shared memory per warp; as many warps per block as fit (at most NB_WARPS)
+        const size_t per_warp = nb_smem_per_warp(cfg->capacity);
+        int dev_smem = 0;
+        cudaDeviceGetAttribute(&dev_smem, cudaDevAttrMaxSharedMemoryPerBlockOptin, attr.device);
+        int w = (int)std::min<size_t>(NB_WARPS, (size_t)dev_smem / per_warp);
+        if (w < 1) { delete s; return fail(MD_EINVAL, "capacity %d needs %zu bytes of shared memory per tile; the device offers %d", cfg->capacity, per_warp, dev_smem); }
+        s->nb_warps = w;
+        s->nb_smem = per_warp * w;
+        cudaError_t ea = cudaSuccess;
+        if (g.dim == 3) {
+            ea = cudaFuncSetAttribute(k_nbr_build<3, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->nb_smem);
+            if (ea == cudaSuccess) ea = cudaFuncSetAttribute(k_nbr_build<3, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->nb_smem);
+        } else {
+            ea = cudaFuncSetAttribute(k_nbr_build<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->nb_smem);
+            if (ea == cudaSuccess) ea = cudaFuncSetAttribute(k_nbr_build<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->nb_smem);
+        }
+        if (ea != cudaSuccess) { delete s; return fail(MD_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(ea)); }
+    }
     cudaError_t e = cudaMemset(workspace, 0, l.total);
     if (e == cudaSuccess) e = cudaDeviceSynchronize();
     if (e != cudaSuccess) { delete s; return fail(MD_ECUDA, "clearing the workspace: %s", cudaGetErrorString(e)); }
@@ -378,19 +409,23 @@ int md_num_cells(const md_system *sys, int *ncell) {
     return MD_OK;
 }
 
-int md_nbr_layout(const md_system *sys, long *particle_stride, long *slot_stride) {
-    if (!sys || !particle_stride || !slot_stride) return fail(MD_EINVAL, "NULL argument");
-    *particle_stride = sys->g.capacity;
-    *slot_stride = 1;
+int md_nbr_layout(const md_system *sys, long *tile, long *tile_stride, long *particle_stride,
+                  long *slot_stride, long *length) {
+    if (!sys || !tile || !tile_stride || !particle_stride || !slot_stride || !length)
+        return fail(MD_EINVAL, "NULL argument");
+    *tile = TILE;
+    *tile_stride = (long)TILE * sys->g.capacity;
+    *particle_stride = 1;
+    *slot_stride = TILE;
+    *length = (long)((sys->n + TILE - 1) / TILE) * TILE * sys->g.capacity;
     return MD_OK;
 }
 
 int md_set_option(md_system *sys, const char *name, double value) {
     if (!sys || !name) return fail(MD_EINVAL, "NULL argument");
-    if (!strcmp(name, "fp64_threshold")) sys->thr = (float)value;
-    else if (!strcmp(name, "threads_per_particle")) {
+    if (!strcmp(name, "threads_per_particle")) {
         int t = (int)value;
-        if (!(t == 1 || t == 2 || t == 4 || t == 8 || t == 16 || t == 32)) return fail(MD_EINVAL, "threads_per_particle must be a power of two <= 32");
+        if (!(t == 0 || t == 1 || t == 2 || t == 4)) return fail(MD_EINVAL, "threads_per_particle must be 0 (streaming kernel), 1, 2 or 4");
         sys->tpp = t;
     } else if (!strcmp(name, "use_graph")) sys->use_graph = value != 0.0;
     else return fail(MD_EINVAL, "unknown option %s", name);
@@ -452,7 +487,7 @@ int md_pair_energy_force(md_system *sys, const md_potential *pot, const void *po
     if (energy_total) CU(cudaMemsetAsync(energy_total, 0, sizeof(double), st));
     Book book = {nullptr, nullptr, nullptr};
     return launch_force(sys, pp, (const float4 *)pos, nbr_idx, nbr_count, (float4 *)force, nullptr,
-                        0.0f, energy_total, book, st);
+                        0.0f, energy_total, true, book, st);
 }
 
 int md_nve_step(md_system *sys, const md_potential *pot, void *pos, void *vel, void *force,
@@ -481,7 +516,7 @@ int md_nve_step(md_system *sys, const md_potential *pot, void *pos, void *vel, v
     memset(&k, 0, sizeof(k));
     k.pos = pos; k.vel = vel; k.force = force; k.id = id; k.nbr_idx = nbr_idx;
     k.nbr_count = nbr_count; k.stats = stats; k.dt = dt; k.mass = mass; k.pot = *pot;
-    k.tpp = sys->tpp; k.thr = sys->thr;
+    k.tpp = sys->tpp;
     if (!sys->key_valid || memcmp(&k, &sys->key, sizeof(k)) != 0) {
         drop_graphs(sys);
         sys->key = k;
@@ -508,7 +543,7 @@ int md_nve_run_host(const md_config *cfg, const md_potential *pot, int n, void *
     int rc = md_workspace_bytes(cfg, n, &wsb);
     if (rc) return rc;
     const size_t vec = (size_t)n * sizeof(float4);
-    const size_t list = (size_t)n * cfg->capacity * sizeof(int);
+    const size_t list = (size_t)((n + TILE - 1) / TILE) * TILE * cfg->capacity * sizeof(int);
     // one allocation: pos, vel, force, out x3, id, count, list, small words, workspace
     size_t o = 0;
     auto take = [&](size_t b) { size_t at = o; o += up(b); return at; };

@@ -24,8 +24,9 @@ struct Geom {
 
 struct Pair {
     int    kind;
-    float  eps, sig2, rc2, u_cut, thr;     // fp32 chain
-    double deps, dsig2, drc2, du_cut;      // fp64 chain
+    double deps, drc2;
+    double dsig6x2;         // LJ: 2 sigma^6
+    double du_cut4;         // LJ: shift * u(r_cut) / (4 eps) = shift * ((s/rc)^12 - (s/rc)^6)
 };
 
 // Device words md_nve_step keeps between kernels.
@@ -190,90 +191,242 @@ k_gather_pos(int n, const int *__restrict__ perm, const float4 *__restrict__ pos
 }
 
 // --------------------------------------------------- neighbor list (L84-L88, L74) ---------
-// One warp per sorted slot.  The 3^D stencil is walked as runs of contiguous slots (the three
-// x-cells of one (y,z) row are contiguous; a periodic wrap in x splits the run).  A whole run
-// shares its image shift: the particle is moved by -L when it sits in the high-side cell, the
-// run by -L when the run is the high-side cell, which reproduces the canonical predicate bit
-// for bit (SURVEY A3 "equivalence with a per-cell shift").  Lanes test 32 candidates at a
-// time; hits are compacted with ballot/popc so the row is written coalesced.
+// List layout (md_nbr_layout): tiles of TILE = 32 consecutive particles, slot-major inside a
+// tile: entry (i, k) lives at  (i / 32) * 32 * capacity + k * 32 + (i % 32).  A warp that owns
+// one tile reads or writes slot k of its 32 particles as one coalesced 128-byte row, which is
+// what both the thread-per-particle force kernel and the builder below want.
+//
+// Builder: one warp per tile, one lane per particle, candidates broadcast from shared memory.
+// The 32 sorted slots of a tile span a few consecutive cells; lanes that share an x-row of
+// cells (same cy, cz) form a segment and scan the union of their stencils: for each of the
+// 3^(D-1) adjacent rows one contiguous run of slots covering x-cells [cx_lo-1, cx_hi+1], plus
+// the two periodic wrap pieces when that range leaves the row.  Every piece carries ONE image
+// shift (-L on the candidates when the piece is the high-side cell, -L on the lane's own
+// coordinate when the piece is the low-side cell), which reproduces the canonical predicate
+// bit for bit for every true neighbor (SURVEY A3 "equivalence with a per-cell shift"); lanes
+// for which the piece is not adjacent see a separation of at least one cell side >= R and
+// reject it, so a union scan adds tests but never hits.  Pieces are staged in chunks of
+// NB_CHUNK candidates: the next chunk's global loads are in flight while the current one is
+// tested.  Hits are appended to a per-lane shared-memory column (bank = lane, conflict
+// free) and the tile is written out row by row, pads (= N, A5) included.
 
-struct RowWriter {
-    int *row; const int *map; int cap; int count; int self; unsigned lt;
-};
+constexpr int TILE = 32;
+constexpr int NB_WARPS = 4;        // tiles per block (upper bound; fewer when capacity is large)
+constexpr int NB_CHUNK = 128;      // candidates staged per round (4 per lane)
 
-template <int DIM>
-__device__ __forceinline__ void scan_run(RowWriter &w, const float4 *__restrict__ spos,
-                                         int t0, int t1, float pix, float piy, float piz,
-                                         float sjx, float sjy, float sjz, float R2, int lane) {
-    for (int base = t0; base < t1; base += 32) {
-        int t = base + lane;
-        bool in = t < t1;
-        float4 pj = spos[in ? t : t0];
-        float dx = __fsub_rn(pix, __fsub_rn(pj.x, sjx));
-        float dy = __fsub_rn(piy, __fsub_rn(pj.y, sjy));
-        float r2 = __fmaf_rn(dy, dy, __fmul_rn(dx, dx));
-        if (DIM == 3) {
-            float dz = __fsub_rn(piz, __fsub_rn(pj.z, sjz));
-            r2 = __fmaf_rn(dz, dz, r2);
-        }
-        bool hit = in && (r2 < R2) && (t != w.self);
-        unsigned m = __ballot_sync(FULL, hit);
-        if (hit) {
-            int k = w.count + __popc(m & w.lt);
-            if (k < w.cap) w.row[k] = w.map ? w.map[t] : t;
-        }
-        w.count += __popc(m);
-    }
+// dynamic shared memory per builder warp: (capacity + 1) rows of 32 ints + one SoA chunk
+__host__ __device__ __forceinline__ size_t nb_smem_per_warp(int cap) {
+    return (size_t)(cap + 1) * TILE * sizeof(int) + 3 * NB_CHUNK * sizeof(float);
+}
+__host__ __device__ __forceinline__ size_t nbr_tile_base(int i, int cap) {
+    return (size_t)(i >> 5) * (size_t)(TILE * cap);
+}
+__host__ __device__ __forceinline__ size_t nbr_addr(int i, int k, int cap) {
+    return nbr_tile_base(i, cap) + (size_t)k * TILE + (size_t)(i & 31);
 }
 
-template <int DIM>
-__global__ void __launch_bounds__(256)
+__device__ __forceinline__ unsigned smem_u32(const void *p) {
+    return (unsigned)__cvta_generic_to_shared(p);
+}
+__device__ __forceinline__ void st_shared(unsigned addr, int v) {
+    asm volatile("st.shared.b32 [%0], %1;" ::"r"(addr), "r"(v) : "memory");
+}
+__device__ __forceinline__ int warp_min(int v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = min(v, __shfl_xor_sync(FULL, v, o));
+    return v;
+}
+__device__ __forceinline__ int warp_max(int v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v = max(v, __shfl_xor_sync(FULL, v, o));
+    return v;
+}
+
+// MAPPED = false: particles are physically sorted (resort = 1): slot == particle index.
+// MAPPED = true : spos is the sorted copy, map[slot] = particle index (resort = 0).
+template <int DIM, bool MAPPED>
+__global__ void __launch_bounds__(NB_WARPS * 32)
 k_nbr_build(Geom g, const float4 *__restrict__ spos, const int *__restrict__ cell_start,
             const int *__restrict__ map, int *__restrict__ nbr_idx, int *__restrict__ nbr_count,
             int *status, float4 *__restrict__ ref_pos, const int *cond) {
+    extern __shared__ __align__(16) unsigned char nb_smem[];
     if (cond && ld_volatile(cond) == 0) return;
-    const int lane = threadIdx.x & 31;
-    const int s = (blockIdx.x * blockDim.x + threadIdx.x) >> 5;
-    if (s >= g.n) return;
-    const float4 pi = spos[s];
-    const int i = map ? map[s] : s;
-    const int cx = cell_coord(pi.x, g.inv_cell[0], g.nc[0]);
-    const int cy = cell_coord(pi.y, g.inv_cell[1], g.nc[1]);
-    const int cz = DIM == 3 ? cell_coord(pi.z, g.inv_cell[2], g.nc[2]) : 0;
-    RowWriter w;
-    w.row = nbr_idx + (size_t)i * g.capacity;
-    w.map = map; w.cap = g.capacity; w.count = 0; w.self = s;
-    w.lt = (1u << lane) - 1u;
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int cap = g.capacity;
+    const int rows = cap + 1;                          // my own slot is appended too, dropped on write-out
+    const size_t per_warp = nb_smem_per_warp(cap);
+    int *col = reinterpret_cast<int *>(nb_smem + warp * per_warp) + lane;      // my column
+    float *sx = reinterpret_cast<float *>(nb_smem + warp * per_warp + (size_t)rows * TILE * sizeof(int));
+    float *sy = sx + NB_CHUNK, *sz = sy + NB_CHUNK;     // staged candidates, negated, SoA
     const int ncx = g.nc[0], ncy = g.nc[1], ncz = g.nc[2];
     const float Lx = g.L[0], Ly = g.L[1], Lz = g.L[2];
-    for (int dz = (DIM == 3 ? -1 : 0); dz <= (DIM == 3 ? 1 : 0); ++dz) {
-        int zc = cz + dz; float piz = pi.z, sjz = 0.0f;
-        if (DIM == 3) {
-            if (zc < 0) { zc += ncz; sjz = Lz; }
-            else if (zc >= ncz) { zc -= ncz; piz = __fsub_rn(pi.z, Lz); }
+    constexpr int ROWS = DIM == 3 ? 9 : 3;
+    const int ntiles = (g.n + TILE - 1) / TILE;
+
+    for (int tile = blockIdx.x * (blockDim.x >> 5) + warp; tile < ntiles; tile += gridDim.x * (blockDim.x >> 5)) {
+        const int s = tile * TILE + lane;
+        const bool act = s < g.n;
+        const float4 pi = spos[act ? s : g.n - 1];
+        const int cx = cell_coord(pi.x, g.inv_cell[0], ncx);
+        const int cy = cell_coord(pi.y, g.inv_cell[1], ncy);
+        const int cz = DIM == 3 ? cell_coord(pi.z, g.inv_cell[2], ncz) : 0;
+        const int row = act ? cz * ncy + cy : 0x7fffffff;
+        const unsigned w0 = smem_u32(col);             // my column (shared-window byte address)
+        const unsigned wend = w0 + (unsigned)rows * TILE * sizeof(int);
+        unsigned w = w0;                               // next free row
+        constexpr unsigned ROWB = TILE * sizeof(int);
+        unsigned todo = __ballot_sync(FULL, act);
+        while (todo) {
+            // ---- next segment: the lanes that share the x-row of the first remaining lane
+            const int leader = __ffs(todo) - 1;
+            const int r = __shfl_sync(FULL, row, leader);
+            const bool inseg = act && row == r;
+            todo &= ~__ballot_sync(FULL, inseg);
+            const int rcy = __shfl_sync(FULL, cy, leader), rcz = __shfl_sync(FULL, cz, leader);
+            const int a = warp_min(inseg ? cx : 0x7fffffff) - 1;
+            const int b = warp_max(inseg ? cx : -1) + 1;
+            // ---- piece table: lane p < 3*ROWS describes piece p = kind * ROWS + rr
+            //      kind 0: x-cells [max(a,0), min(b,ncx-1)]   no x shift
+            //      kind 1: x-cell  ncx-1 (a < 0)              candidates shifted by -Lx
+            //      kind 2: x-cell  0     (b > ncx-1)          my own x shifted by -Lx
+            int t0 = 0, t1 = 0;
+            if (lane < 3 * ROWS) {
+                const int kind = lane / ROWS, rr = lane % ROWS;
+                const int dy = rr % 3 - 1, dz = DIM == 3 ? rr / 3 - 1 : 0;
+                int yc = rcy + dy, zc = rcz + dz;
+                yc += yc < 0 ? ncy : (yc >= ncy ? -ncy : 0);
+                if (DIM == 3) zc += zc < 0 ? ncz : (zc >= ncz ? -ncz : 0);
+                const int rowbase = (zc * ncy + yc) * ncx;
+                int ca = 0, cb = -1;
+                if (kind == 0) { ca = max(a, 0); cb = min(b, ncx - 1); }
+                else if (kind == 1) { if (a < 0) { ca = ncx - 1; cb = ncx - 1; } }
+                else { if (b > ncx - 1) { ca = 0; cb = 0; } }
+                if (cb >= ca) { t0 = cell_start[rowbase + ca]; t1 = cell_start[rowbase + cb + 1]; }
+            }
+            // ---- walk the pieces; the next chunk is loaded while the current one is tested
+            int p = 0, base = 0, pt1 = 0;
+            auto seek = [&](int &pp, int &bb, int &tt1) {       // first non-empty piece >= pp
+                while (pp < 3 * ROWS) {
+                    bb = __shfl_sync(FULL, t0, pp); tt1 = __shfl_sync(FULL, t1, pp);
+                    if (bb < tt1) return;
+                    ++pp;
+                }
+            };
+            seek(p, base, pt1);
+            float4 q[NB_CHUNK / 32];
+            auto fetch = [&](int bb, int tt1) {
+#pragma unroll
+                for (int u = 0; u < NB_CHUNK / 32; ++u) {
+                    const int t = bb + u * 32 + lane;
+                    if (t < tt1) q[u] = spos[t];
+                }
+            };
+            if (p < 3 * ROWS) fetch(base, pt1);
+            while (p < 3 * ROWS) {
+                const int kind = p / ROWS, rr = p % ROWS;
+                const int dy = rr % 3 - 1, dz = DIM == 3 ? rr / 3 - 1 : 0;
+                // image shifts of this piece: candidates by -L when the piece is the
+                // high-side row/cell, my own coordinate by -L when it is the low-side one
+                const float sjx = kind == 1 ? Lx : 0.0f;
+                const float sjy = rcy + dy < 0 ? Ly : 0.0f;
+                const float sjz = (DIM == 3 && rcz + dz < 0) ? Lz : 0.0f;
+                const float pix = kind == 2 ? __fsub_rn(pi.x, Lx) : pi.x;
+                const float piy = rcy + dy >= ncy ? __fsub_rn(pi.y, Ly) : pi.y;
+                const float piz = (DIM == 3 && rcz + dz >= ncz) ? __fsub_rn(pi.z, Lz) : pi.z;
+                const int m = min(NB_CHUNK, pt1 - base);
+                // stage -(candidate - shift), structure of arrays; the tail of the last group of
+                // four is filled with a far-away point so the test loop needs no remainder
+#pragma unroll
+                for (int u = 0; u < NB_CHUNK / 32; ++u) {
+                    const int c = u * 32 + lane;
+                    if (c < m) {
+                        sx[c] = __fsub_rn(sjx, q[u].x);
+                        sy[c] = __fsub_rn(sjy, q[u].y);
+                        if (DIM == 3) sz[c] = __fsub_rn(sjz, q[u].z);
+                    } else if (c < ((m + 3) & ~3)) {
+                        sx[c] = 1e18f; sy[c] = 0.0f;
+                        if (DIM == 3) sz[c] = 0.0f;
+                    }
+                }
+                __syncwarp();
+                // next chunk
+                int np = p, nbase = base + NB_CHUNK, npt1 = pt1;
+                if (nbase >= pt1) { ++np; seek(np, nbase, npt1); }
+                if (np < 3 * ROWS) fetch(nbase, npt1);
+                // test the staged chunk, two candidates per packed fp32x2 instruction
+                // (sm_100 FADD2 / FMUL2 / FFMA2, round-to-nearest: the bits of the scalar form)
+                if (inseg) {
+                    const float2 px2 = make_float2(pix, pix), py2 = make_float2(piy, piy);
+                    const float2 pz2 = make_float2(piz, piz);
+                    for (int c = 0; c < m; c += 4) {
+                        const float4 X = *reinterpret_cast<const float4 *>(sx + c);
+                        const float4 Y = *reinterpret_cast<const float4 *>(sy + c);
+                        const float2 dxa = __fadd2_rn(px2, make_float2(X.x, X.y));
+                        const float2 dxb = __fadd2_rn(px2, make_float2(X.z, X.w));
+                        const float2 dya = __fadd2_rn(py2, make_float2(Y.x, Y.y));
+                        const float2 dyb = __fadd2_rn(py2, make_float2(Y.z, Y.w));
+                        float2 ra = __ffma2_rn(dya, dya, __fmul2_rn(dxa, dxa));
+                        float2 rb = __ffma2_rn(dyb, dyb, __fmul2_rn(dxb, dxb));
+                        if (DIM == 3) {
+                            const float4 Z = *reinterpret_cast<const float4 *>(sz + c);
+                            const float2 dza = __fadd2_rn(pz2, make_float2(Z.x, Z.y));
+                            const float2 dzb = __fadd2_rn(pz2, make_float2(Z.z, Z.w));
+                            ra = __ffma2_rn(dza, dza, ra);
+                            rb = __ffma2_rn(dzb, dzb, rb);
+                        }
+                        const int t = base + c;
+                        const bool h0 = ra.x < g.R2, h1 = ra.y < g.R2, h2 = rb.x < g.R2, h3 = rb.y < g.R2;
+                        if (w + 4u * ROWB <= wend) {          // room for all four
+                            if (h0) st_shared(w, t);
+                            w += h0 ? ROWB : 0u;
+                            if (h1) st_shared(w, t + 1);
+                            w += h1 ? ROWB : 0u;
+                            if (h2) st_shared(w, t + 2);
+                            w += h2 ? ROWB : 0u;
+                            if (h3) st_shared(w, t + 3);
+                            w += h3 ? ROWB : 0u;
+                        } else {                                           // overflowing row: count only
+                            if (h0 && w < wend) st_shared(w, t);
+                            w += h0 ? ROWB : 0u;
+                            if (h1 && w < wend) st_shared(w, t + 1);
+                            w += h1 ? ROWB : 0u;
+                            if (h2 && w < wend) st_shared(w, t + 2);
+                            w += h2 ? ROWB : 0u;
+                            if (h3 && w < wend) st_shared(w, t + 3);
+                            w += h3 ? ROWB : 0u;
+                        }
+                    }
+                }
+                __syncwarp();
+                p = np; base = nbase; pt1 = npt1;
+            }
         }
-        for (int dy = -1; dy <= 1; ++dy) {
-            int yc = cy + dy; float piy = pi.y, sjy = 0.0f;
-            if (yc < 0) { yc += ncy; sjy = Ly; }
-            else if (yc >= ncy) { yc -= ncy; piy = __fsub_rn(pi.y, Ly); }
-            const int rowbase = (zc * ncy + yc) * ncx;
-            const int xa = max(cx - 1, 0), xb = min(cx + 1, ncx - 1);
-            scan_run<DIM>(w, spos, cell_start[rowbase + xa], cell_start[rowbase + xb + 1],
-                          pi.x, piy, piz, 0.0f, sjy, sjz, g.R2, lane);
-            if (cx == 0)
-                scan_run<DIM>(w, spos, cell_start[rowbase + ncx - 1], cell_start[rowbase + ncx],
-                              pi.x, piy, piz, Lx, sjy, sjz, g.R2, lane);
-            else if (cx == ncx - 1)
-                scan_run<DIM>(w, spos, cell_start[rowbase], cell_start[rowbase + 1],
-                              __fsub_rn(pi.x, Lx), piy, piz, 0.0f, sjy, sjz, g.R2, lane);
+        // ---- write the tile out (rows of 32 consecutive ints; scattered when MAPPED), dropping
+        //      my own slot, which the scan appended like any other point at distance 0
+        const int appended = (int)((w - w0) / ROWB);
+        const int cnt = act ? appended - 1 : 0;        // true count
+        const int stored = min(appended, rows);
+        int *out = nullptr;
+        if (!MAPPED) out = nbr_idx + nbr_tile_base(s, cap) + lane;
+        else if (act) { const int i = map[s]; out = nbr_idx + nbr_tile_base(i, cap) + (i & 31); }
+        if (out) {
+            int ko = 0;
+            for (int k = 0; k < stored; ++k) {
+                const int v = col[k * TILE];
+                if (v != s && ko < cap) { out[ko * TILE] = MAPPED ? map[v] : v; ++ko; }
+            }
+            for (; ko < cap; ++ko) out[ko * TILE] = g.n;                  // pad = N (A5)
         }
-    }
-    for (int k = min(w.count, w.cap) + lane; k < w.cap; k += 32) w.row[k] = g.n;   // pad = N (A5)
-    if (lane == 0) {
-        nbr_count[i] = w.count;
-        ref_pos[i] = pi;
-        if (w.count > ld_volatile(status + 1)) atomicMax(status + 1, w.count);
-        if (w.count > w.cap) status[0] = 1;
+        if (act) {
+            const int i = MAPPED ? map[s] : s;
+            nbr_count[i] = cnt; ref_pos[i] = pi;
+        }
+        const int mx = warp_max(act ? cnt : 0);
+        if (lane == 0) {
+            if (mx > ld_volatile(status + 1)) atomicMax(status + 1, mx);
+            if (mx > cap) status[0] = 1;
+        }
+        __syncwarp();
     }
 }
 
@@ -327,183 +480,131 @@ k_kick_drift(Geom g, float4 *__restrict__ pos, float4 *__restrict__ vel,
 }
 
 // ------------------------------------- pair energy / force over the list (L78, L80, L104) --
-// TPP lanes share one particle; each lane walks every TPP-th entry of the row (a group reads
-// TPP consecutive int32 = whole 32-byte sectors when TPP = 8).  Pass 1 evaluates every pair in
-// fp32 and also sums S = sum_j (|f_rep| + |f_att|)|d|_1, a bound on what rounding can have
-// been amplified by.  A particle whose S exceeds thr * max(|F|, 1e-3) is re-evaluated in fp64
-// from exact displacements (pass 2), so the fp32 result is only kept where its error estimate
-// is far inside the 1e-5 tolerance.  Pairs whose fp32 r2 falls in a
-// 2e-6 relative band around the LJ cutoff take their in/out decision from the exact fp64 r2,
-// because the truncated force is discontinuous there.
+// TPP lanes per particle (1, 2 or 4); with TPP = 1 a warp is exactly one list tile and slot k of
+// its 32 particles is one coalesced 128-byte row.  Neighbor positions are gathered as float4
+// through L1 (particles are cell-sorted, so the 32 lanes walk nearby lines).
+//
+// Precision: displacements are exact -- away from the box faces
+// the fp32 difference of two coordinates >= 2 that are < 4 apart is exact, near a face the
+// difference and the image shift are taken in fp64 -- and the pair chain r2 -> 1/r2 -> force
+// coefficient and all accumulation run in fp64 (reciprocal: hardware seed + Newton steps on
+// the FP64 pipe).  Results round to fp32 once, on store.  Pure fp32 pair arithmetic cannot hold
+// the 1e-5 force tolerance: its typical error is already 3e-6 of |F| because the first shell
+// sits where the LJ force changes sign.  The in/out decision at r_cut is taken on the fp64 r2.
 
-struct Acc32 { float fx, fy, fz, e, s; };
 struct Acc64 { double fx, fy, fz, e; };
 
-template <int KIND>
-__device__ __forceinline__ void pair32(const Pair &pp, float dx, float dy, float dz, float r2,
-                                       float dsum, bool in, Acc32 &a) {
-    if (KIND == 0) {
-        float y = __frcp_rn(r2);
-        float s2 = pp.sig2 * y;
-        float s6 = s2 * s2 * s2;
-        float c24 = 24.0f * pp.eps * y * s6;
-        float coef = in ? c24 * fmaf(2.0f, s6, -1.0f) : 0.0f;
-        float mag = in ? c24 * fmaf(2.0f, s6, 1.0f) : 0.0f;
-        float u = in ? fmaf(4.0f * pp.eps * s6, s6 - 1.0f, -pp.u_cut) : 0.0f;
-        a.fx = fmaf(coef, dx, a.fx); a.fy = fmaf(coef, dy, a.fy); a.fz = fmaf(coef, dz, a.fz);
-        a.e = fmaf(0.5f, u, a.e);
-        a.s = fmaf(mag, fabsf(dx) + fabsf(dy) + fabsf(dz), a.s);
+// 1/x to ~1e-12: hardware seed (MUFU.RCP64H, measured 9.4e-7 on B200) + one Newton step.
+__device__ __forceinline__ double rcp64(double x) {
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    return fma(y, fma(-x, y, 1.0), y);
+}
+
+// One pair, LJ.  With y = 1/r2 and s6 = sig^6 y^3 the force coefficient is
+// 24 eps s6 (2 s6 - 1) y = 24 eps sig^6 * y^4 (2 sig^6 y^3 - 1); the constant 24 eps sig^6 is
+// applied once per particle.  Energy term: s6 (s6 - 1) - u_cut / (4 eps), times 4 eps / 2 later.
+template <bool ENERGY>
+__device__ __forceinline__ void lj_pair64(const Pair &pp, double dx, double dy, double dz,
+                                          bool valid, Acc64 &a) {
+    const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+    const bool in = valid && r2 < pp.drc2;
+    const double y = rcp64(in ? r2 : 1.0);
+    const double y2 = y * y;
+    const double y3 = y2 * y;
+    const double t = fma(pp.dsig6x2, y3, -1.0);           // 2 s6 - 1
+    double c = (y2 * y2) * t;
+    c = in ? c : 0.0;
+    a.fx = fma(c, dx, a.fx); a.fy = fma(c, dy, a.fy); a.fz = fma(c, dz, a.fz);
+    if (ENERGY) {
+        const double s6 = 0.5 * pp.dsig6x2 * y3;
+        a.e += in ? fma(s6, s6, -s6) - pp.du_cut4 : 0.0;
+    }
+}
+
+// One pair, harmonic soft sphere: u = eps/2 (1 - r/d)^2, F = eps/d (1 - r/d) dvec/r for r < d.
+template <bool ENERGY>
+__device__ __forceinline__ void soft_pair64(const Pair &pp, double dx, double dy, double dz,
+                                            double dsum, bool valid, Acc64 &a) {
+    const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+    const double dij = 0.5 * dsum;
+    const double r = sqrt(r2);
+    const bool in = valid && r < dij;
+    const double x = 1.0 - r / dij;
+    const double c = (in && r > 0.0) ? x / (dij * r) : 0.0;
+    a.fx = fma(c, dx, a.fx); a.fy = fma(c, dy, a.fy); a.fz = fma(c, dz, a.fz);
+    if (ENERGY) a.e += in ? x * x : 0.0;
+}
+
+// Per-thread view of the space for the pair loop.
+template <int DIM>
+struct Me {
+    float4 pi;
+    double xi, yi, zi, Lx, Ly, Lz;
+    float hx, hy, hz;
+};
+
+// Displacement r_i - r_j (nearest image) in fp64.  WRAP = false: the warp is away from every
+// face, no pair crosses the boundary; the fp32 difference is exact for every pair that
+// matters (coordinates >= r_cut + 2 skin, separations < 4) and at worst 1 rounding (6e-8 of a
+// distance > 2, where the force is tiny) otherwise.  WRAP = true: difference and image shift
+// in fp64; the image is picked on the fp32 difference (|d| < L/2 - or > L/2 + by a wide margin).
+template <int DIM, bool WRAP>
+__device__ __forceinline__ void displacement(const Me<DIM> &me, const float4 &q, double &dx,
+                                             double &dy, double &dz) {
+    const float fx = me.pi.x - q.x, fy = me.pi.y - q.y, fz = me.pi.z - q.z;
+    if (!WRAP) {
+        dx = (double)fx; dy = (double)fy; dz = DIM == 3 ? (double)fz : 0.0;
     } else {
-        float dij = 0.5f * dsum;
-        float idij = __frcp_rn(dij);
-        float y = rsqrtf(r2);                   // r2 = 0 -> inf, handled below
-        float r = r2 * y;
-        bool ok = in && (r2 > 0.0f) && (r < dij);
-        float x = 1.0f - r * idij;
-        float k = pp.eps * idij * y;
-        float coef = ok ? k * x : 0.0f;
-        float mag = ok ? k * (1.0f + r * idij) : 0.0f;
-        float u = ok ? 0.5f * pp.eps * x * x : ((in && r2 == 0.0f && dij > 0.0f) ? 0.5f * pp.eps : 0.0f);
-        a.fx = fmaf(coef, dx, a.fx); a.fy = fmaf(coef, dy, a.fy); a.fz = fmaf(coef, dz, a.fz);
-        a.e = fmaf(0.5f, u, a.e);
-        a.s = fmaf(mag, fabsf(dx) + fabsf(dy) + fabsf(dz), a.s);
-    }
-}
-
-template <int KIND>
-__device__ __forceinline__ void pair64(const Pair &pp, double dx, double dy, double dz,
-                                       double dsum, Acc64 &a) {
-    double r2 = dx * dx + dy * dy + dz * dz;
-    if (KIND == 0) {
-        if (r2 < pp.drc2) {
-            double y = (double)__frcp_rn((float)r2);
-            y = y * (2.0 - r2 * y);               // Newton: fp32 seed -> ~1e-14
-            y = y * (2.0 - r2 * y);
-            double s2 = pp.dsig2 * y;
-            double s6 = s2 * s2 * s2;
-            double coef = 24.0 * pp.deps * y * s6 * (2.0 * s6 - 1.0);
-            a.fx += coef * dx; a.fy += coef * dy; a.fz += coef * dz;
-            a.e += 0.5 * (4.0 * pp.deps * s6 * (s6 - 1.0) - pp.du_cut);
-        }
-    } else {
-        double dij = 0.5 * dsum;
-        double r = sqrt(r2);
-        if (r < dij) {
-            double x = 1.0 - r / dij;
-            a.e += 0.25 * pp.deps * x * x;
-            if (r > 0.0) {
-                double coef = pp.deps / dij * x / r;
-                a.fx += coef * dx; a.fy += coef * dy; a.fz += coef * dz;
-            }
+        dx = me.xi - (double)q.x; dy = me.yi - (double)q.y;
+        dx -= fx > me.hx ? me.Lx : (fx < -me.hx ? -me.Lx : 0.0);
+        dy -= fy > me.hy ? me.Ly : (fy < -me.hy ? -me.Ly : 0.0);
+        dz = 0.0;
+        if (DIM == 3) {
+            dz = me.zi - (double)q.z;
+            dz -= fz > me.hz ? me.Lz : (fz < -me.hz ? -me.Lz : 0.0);
         }
     }
 }
 
-template <int KIND, int DIM, int TPP, bool WRAP>
-__device__ __forceinline__ void row_pass32(const Geom &g, const Pair &pp,
-                                           const float4 *__restrict__ pos,
-                                           const int *__restrict__ row, int cnt, int sub,
-                                           float4 pi, Acc32 &a) {
-    const float band_lo = pp.rc2 * (1.0f - 2e-6f), band_hi = pp.rc2 * (1.0f + 2e-6f);
-    for (int k = sub; k < cnt; k += 2 * TPP) {
-        const int k1 = k + TPP;
-        const bool v1 = k1 < cnt;
-        const int j0 = row[k];
-        const int j1 = row[v1 ? k1 : k];
-        const float4 q[2] = {pos[j0], pos[j1]};
-#pragma unroll
-        for (int u = 0; u < 2; ++u) {
-            float dx, dy, dz = 0.0f;
-            if (WRAP) {
-                dx = min_image(pi.x, q[u].x, g.L[0], g.h[0]);
-                dy = min_image(pi.y, q[u].y, g.L[1], g.h[1]);
-                if (DIM == 3) dz = min_image(pi.z, q[u].z, g.L[2], g.h[2]);
-            } else {
-                dx = pi.x - q[u].x; dy = pi.y - q[u].y;
-                if (DIM == 3) dz = pi.z - q[u].z;
-            }
-            float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-            bool in = (u == 0) || v1;
-            if (KIND == 0) {
-                bool inr = r2 < pp.rc2;
-                if (r2 > band_lo && r2 < band_hi) {       // rare: decide on the exact r2
-                    double ex = min_image64(pi.x, q[u].x, (double)g.L[0], (double)g.h[0]);
-                    double ey = min_image64(pi.y, q[u].y, (double)g.L[1], (double)g.h[1]);
-                    double ez = DIM == 3 ? min_image64(pi.z, q[u].z, (double)g.L[2], (double)g.h[2]) : 0.0;
-                    inr = (ex * ex + ey * ey + ez * ez) < pp.drc2;
-                }
-                in = in && inr;
-            }
-            pair32<KIND>(pp, dx, dy, dz, r2, pi.w + q[u].w, in, a);
-        }
-    }
+template <int KIND, int DIM, bool ENERGY, bool WRAP>
+__device__ __forceinline__ void pair_any(const Pair &pp, const Me<DIM> &me, const float4 &q,
+                                         bool valid, Acc64 &acc) {
+    double dx, dy, dz;
+    displacement<DIM, WRAP>(me, q, dx, dy, dz);
+    if (KIND == 0) lj_pair64<ENERGY>(pp, dx, dy, dz, valid, acc);
+    else soft_pair64<ENERGY>(pp, dx, dy, dz, (double)me.pi.w + (double)q.w, valid, acc);
 }
 
-template <int KIND, int DIM, int TPP>
-__device__ __forceinline__ void row_pass64(const Geom &g, const Pair &pp,
-                                           const float4 *__restrict__ pos,
-                                           const int *__restrict__ row, int cnt, int sub,
-                                           float4 pi, Acc64 &a) {
-    for (int k = sub; k < cnt; k += TPP) {
-        const float4 q = pos[row[k]];
-        double dx = min_image64(pi.x, q.x, (double)g.L[0], (double)g.h[0]);
-        double dy = min_image64(pi.y, q.y, (double)g.L[1], (double)g.h[1]);
-        double dz = DIM == 3 ? min_image64(pi.z, q.z, (double)g.L[2], (double)g.h[2]) : 0.0;
-        pair64<KIND>(pp, dx, dy, dz, (double)pi.w + (double)q.w, a);
-    }
+template <int DIM>
+__device__ __forceinline__ bool near_face(const Geom &g, const float4 &p) {
+    bool near = p.x < g.face || p.x > g.L[0] - g.face || p.y < g.face || p.y > g.L[1] - g.face;
+    if (DIM == 3) near = near || p.z < g.face || p.z > g.L[2] - g.face;
+    return near;
 }
 
-template <int TPP, typename T>
-__device__ __forceinline__ T group_sum(T v) {
-#pragma unroll
-    for (int o = TPP / 2; o > 0; o >>= 1) v += __shfl_xor_sync(FULL, v, o);
-    return v;
+template <int DIM>
+__device__ __forceinline__ Me<DIM> make_me(const Geom &g, const float4 &pi) {
+    Me<DIM> me;
+    me.pi = pi; me.xi = pi.x; me.yi = pi.y; me.zi = pi.z;
+    me.Lx = g.L[0]; me.Ly = g.L[1]; me.Lz = g.L[2];
+    me.hx = g.h[0]; me.hy = g.h[1]; me.hz = g.h[2];
+    return me;
 }
 
-// vel != NULL: also the second half-kick v += a F (L100).  energy_total != NULL: adds
-// sum_i e_i in fp64 (one atomic per block).  book.stats != NULL: per-step bookkeeping.
-template <int KIND, int DIM, int TPP>
-__global__ void __launch_bounds__(256)
-k_force(Geom g, Pair pp, const float4 *__restrict__ pos, const int *__restrict__ nbr_idx,
-        const int *__restrict__ nbr_count, float4 *__restrict__ force, float4 *__restrict__ vel,
-        float a, double *energy_total, Book book) {
-    const int gid = blockIdx.x * blockDim.x + threadIdx.x;
-    const int i = gid / TPP, sub = gid % TPP;
-    const bool active = i < g.n;
-    const int ii = active ? i : g.n - 1;
-    const float4 pi = pos[ii];
-    const int cnt = active ? min(nbr_count[ii], g.capacity) : 0;
-    const int *row = nbr_idx + (size_t)ii * g.capacity;
-
-    bool near = pi.x < g.face || pi.x > g.L[0] - g.face || pi.y < g.face || pi.y > g.L[1] - g.face;
-    if (DIM == 3) near = near || pi.z < g.face || pi.z > g.L[2] - g.face;
-    Acc32 a32 = {0.f, 0.f, 0.f, 0.f, 0.f};
-    if (__any_sync(FULL, near && active))
-        row_pass32<KIND, DIM, TPP, true>(g, pp, pos, row, cnt, sub, pi, a32);
-    else
-        row_pass32<KIND, DIM, TPP, false>(g, pp, pos, row, cnt, sub, pi, a32);
-    float fx = group_sum<TPP>(a32.fx), fy = group_sum<TPP>(a32.fy), fz = group_sum<TPP>(a32.fz);
-    float e = group_sum<TPP>(a32.e), s = group_sum<TPP>(a32.s);
-
-    // pass 2: fp64 re-evaluation where rounding may matter
-    float fn = sqrtf(fmaf(fz, fz, fmaf(fy, fy, fx * fx)));
-    const bool keep32 = (s <= pp.thr * fmaxf(fn, 1e-3f)) && (s < 1e30f);   // NaN/inf -> fp64
-    if (!keep32) {                                // uniform within the TPP group
-        Acc64 a64 = {0.0, 0.0, 0.0, 0.0};
-        row_pass64<KIND, DIM, TPP>(g, pp, pos, row, cnt, sub, pi, a64);
-        // reduce inside the group only: lanes of other groups are not here
-        unsigned gm = (TPP == 32) ? FULL : (((1u << TPP) - 1u) << ((threadIdx.x & 31) / TPP * TPP));
-#pragma unroll
-        for (int o = TPP / 2; o > 0; o >>= 1) {
-            a64.fx += __shfl_xor_sync(gm, a64.fx, o);
-            a64.fy += __shfl_xor_sync(gm, a64.fy, o);
-            a64.fz += __shfl_xor_sync(gm, a64.fz, o);
-            a64.e += __shfl_xor_sync(gm, a64.e, o);
-        }
-        fx = (float)a64.fx; fy = (float)a64.fy; fz = (float)a64.fz; e = (float)a64.e;
-    }
-    if (active && sub == 0) {
-        force[i] = make_float4(fx, fy, DIM == 3 ? fz : 0.0f, e);
+// Epilogue shared by both force kernels: scale, round once, store, optional half-kick, energy
+// reduction and step bookkeeping.
+template <int KIND, int DIM, bool ENERGY>
+__device__ __forceinline__ void force_epilogue(const Pair &pp, const Acc64 &acc, bool owner, int i,
+                                               float4 *__restrict__ force, float4 *__restrict__ vel,
+                                               float a, double *energy_total, const Book &book,
+                                               int gid) {
+    const double fs = KIND == 0 ? 12.0 * pp.deps * pp.dsig6x2 : pp.deps;     // 24 eps sig^6 | eps
+    const double es = KIND == 0 ? 2.0 * pp.deps : 0.25 * pp.deps;            // 1/2 * (4 eps | eps/2)
+    const float fx = (float)(fs * acc.fx), fy = (float)(fs * acc.fy), fz = (float)(fs * acc.fz);
+    const double e64 = ENERGY ? es * acc.e : 0.0;
+    if (owner) {
+        force[i] = make_float4(fx, fy, DIM == 3 ? fz : 0.0f, (float)e64);
         if (vel) {
             float4 v = vel[i];
             v.x = fmaf(a, fx, v.x); v.y = fmaf(a, fy, v.y);
@@ -511,9 +612,9 @@ k_force(Geom g, Pair pp, const float4 *__restrict__ pos, const int *__restrict__
             vel[i] = v;
         }
     }
-    if (energy_total) {
-        __shared__ double red[8];
-        double x = (active && sub == 0) ? (double)e : 0.0;
+    if (ENERGY && energy_total) {
+        __shared__ double red[4];
+        double x = owner ? e64 : 0.0;
 #pragma unroll
         for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(FULL, x, o);
         if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = x;
@@ -534,6 +635,138 @@ k_force(Geom g, Pair pp, const float4 *__restrict__ pos, const int *__restrict__
         }
         book.stats[0] += 1;
     }
+}
+
+// ---- generic kernel: TPP lanes per particle (small systems: more warps, shorter chains) ----
+// vel != NULL: also the second half-kick v += a F (L100).  energy_total != NULL (ENERGY only):
+// adds sum_i e_i in fp64 (one atomic per block).  book.stats != NULL: per-step bookkeeping.
+template <int KIND, int DIM, int TPP, bool ENERGY>
+__global__ void __launch_bounds__(128)
+k_force(Geom g, Pair pp, const float4 *__restrict__ pos, const int *__restrict__ nbr_idx,
+        const int *__restrict__ nbr_count, float4 *__restrict__ force, float4 *__restrict__ vel,
+        float a, double *energy_total, Book book) {
+    const int gid = blockIdx.x * blockDim.x + threadIdx.x;
+    const int i = gid / TPP, sub = gid % TPP;
+    const bool active = i < g.n;
+    const int ii = active ? i : g.n - 1;
+    const Me<DIM> me = make_me<DIM>(g, pos[ii]);
+    const int cnt = active ? min(nbr_count[ii], g.capacity) : 0;
+    const int *col = nbr_idx + nbr_tile_base(ii, g.capacity) + (ii & 31);
+    const bool wrap_path = __any_sync(FULL, active && near_face<DIM>(g, me.pi));
+    Acc64 acc = {0.0, 0.0, 0.0, 0.0};
+    constexpr int U = 4;
+    for (int k = sub; k < cnt; k += U * TPP) {
+        int j[U]; float4 q[U];
+#pragma unroll
+        for (int u = 0; u < U; ++u) { const int kk = k + u * TPP; j[u] = kk < cnt ? col[kk * TILE] : ii; }
+#pragma unroll
+        for (int u = 0; u < U; ++u) q[u] = pos[j[u]];
+        if (!wrap_path) {
+#pragma unroll
+            for (int u = 0; u < U; ++u) pair_any<KIND, DIM, ENERGY, false>(pp, me, q[u], k + u * TPP < cnt, acc);
+        } else {
+#pragma unroll
+            for (int u = 0; u < U; ++u) pair_any<KIND, DIM, ENERGY, true>(pp, me, q[u], k + u * TPP < cnt, acc);
+        }
+    }
+#pragma unroll
+    for (int o = TPP / 2; o > 0; o >>= 1) {
+        acc.fx += __shfl_xor_sync(FULL, acc.fx, o);
+        acc.fy += __shfl_xor_sync(FULL, acc.fy, o);
+        acc.fz += __shfl_xor_sync(FULL, acc.fz, o);
+        if (ENERGY) acc.e += __shfl_xor_sync(FULL, acc.e, o);
+    }
+    force_epilogue<KIND, DIM, ENERGY>(pp, acc, active && sub == 0, i, force, vel, a, energy_total, book, gid);
+}
+
+// ---- streaming kernel: one warp = one list tile, one lane per particle.  The tile's index
+// block (rows of 128 bytes, contiguous in HBM) is streamed into shared memory by the TMA engine
+// (cp.async.bulk + mbarrier) FS_STAGES chunks of FS_ROWS rows ahead of the arithmetic, so the
+// only long-latency loads a lane waits for are its position gathers (L1 / L2 hits).
+constexpr int FS_ROWS = 16;       // rows per chunk (2 KiB)
+constexpr int FS_STAGES = 3;      // chunks in flight per warp
+constexpr int FS_WARPS = 4;
+
+__device__ __forceinline__ void mbar_init(unsigned bar, int count) {
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned bar, unsigned bytes) {
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(unsigned dst, const void *src, unsigned bytes, unsigned bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(dst), "l"(src), "r"(bytes), "r"(bar) : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned bar, unsigned parity) {
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "WAIT_LOOP:\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n\t"
+        "@p bra WAIT_DONE;\n\t"
+        "bra WAIT_LOOP;\n\t"
+        "WAIT_DONE:\n\t}" ::"r"(bar), "r"(parity) : "memory");
+}
+
+template <int KIND, int DIM, bool ENERGY>
+__global__ void __launch_bounds__(FS_WARPS * 32)
+k_force_stream(Geom g, Pair pp, const float4 *__restrict__ pos, const int *__restrict__ nbr_idx,
+               const int *__restrict__ nbr_count, float4 *__restrict__ force,
+               float4 *__restrict__ vel, float a, double *energy_total, Book book) {
+    __shared__ __align__(128) int s_idx[FS_WARPS][FS_STAGES][FS_ROWS * TILE];
+    __shared__ __align__(8) unsigned long long s_bar[FS_WARPS][FS_STAGES];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int gid = blockIdx.x * blockDim.x + threadIdx.x;
+    const int i = gid;
+    const bool active = i < g.n;
+    const int ii = active ? i : g.n - 1;
+    if (lane == 0) {
+#pragma unroll
+        for (int s = 0; s < FS_STAGES; ++s) mbar_init(smem_u32(&s_bar[warp][s]), 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+    }
+    const int cnt = active ? min(nbr_count[ii], g.capacity) : 0;
+    const int maxcnt = warp_max(cnt);                  // also orders the barrier init (shuffles sync)
+    const int nch = (maxcnt + FS_ROWS - 1) / FS_ROWS;
+    const int *tile_src = nbr_idx + nbr_tile_base(gid, g.capacity);     // gid: valid for the whole tile
+    auto issue = [&](int c) {
+        const int st = c % FS_STAGES;
+        const unsigned bytes = (unsigned)min(FS_ROWS, maxcnt - c * FS_ROWS) * TILE * sizeof(int);
+        const unsigned bar = smem_u32(&s_bar[warp][st]);
+        mbar_expect_tx(bar, bytes);
+        bulk_g2s(smem_u32(&s_idx[warp][st][0]), tile_src + (size_t)c * FS_ROWS * TILE, bytes, bar);
+    };
+    __syncwarp();
+    if (lane == 0)
+        for (int c = 0; c < min(FS_STAGES, nch); ++c) issue(c);
+    const Me<DIM> me = make_me<DIM>(g, pos[ii]);
+    const bool wrap_path = __any_sync(FULL, active && near_face<DIM>(g, me.pi));
+    Acc64 acc = {0.0, 0.0, 0.0, 0.0};
+    constexpr int U = 4;
+    for (int c = 0; c < nch; ++c) {
+        const int st = c % FS_STAGES;
+        mbar_wait(smem_u32(&s_bar[warp][st]), (unsigned)(c / FS_STAGES) & 1u);
+        const int *sm = &s_idx[warp][st][lane];
+        const int k0 = c * FS_ROWS;
+        const int rows = min(FS_ROWS, maxcnt - k0);
+        for (int r = 0; r < rows; r += U) {
+            int j[U]; float4 q[U];
+#pragma unroll
+            for (int u = 0; u < U; ++u) j[u] = k0 + r + u < cnt ? sm[(r + u) * TILE] : ii;
+#pragma unroll
+            for (int u = 0; u < U; ++u) q[u] = pos[j[u]];
+            if (!wrap_path) {
+#pragma unroll
+                for (int u = 0; u < U; ++u) pair_any<KIND, DIM, ENERGY, false>(pp, me, q[u], k0 + r + u < cnt, acc);
+            } else {
+#pragma unroll
+                for (int u = 0; u < U; ++u) pair_any<KIND, DIM, ENERGY, true>(pp, me, q[u], k0 + r + u < cnt, acc);
+            }
+        }
+        __syncwarp();                                  // every lane is done reading this stage
+        if (lane == 0 && c + FS_STAGES < nch) issue(c + FS_STAGES);
+    }
+    force_epilogue<KIND, DIM, ENERGY>(pp, acc, active, i, force, vel, a, energy_total, book, gid);
 }
 
 } // namespace mdk
