@@ -82,11 +82,22 @@ int md_create(const md_config *cfg, int n, void *workspace, size_t bytes, md_sys
 int md_destroy(md_system *sys);
 
 /* Tuning knobs (host call; drops the cached step graph):
- *   "threads_per_particle" force kernel variant: 0 = streaming kernel (one lane per particle,
+ *   "fast32"               1 (default): 3-D LJ forces by the fp32 fast path with an error estimate
+ *                          and fp64 re-evaluation of the particles that need it;
+ *                          0: every pair in fp64 (the kernels selected by threads_per_particle)
+ *   "est_thr"              the fast path re-evaluates particle i in fp64 when
+ *                          sum_j |f_ij / r_ij| > est_thr * max(|F_i|, 1e-3); default 8
+ *   "threads_per_particle" fp64 force kernel variant: 0 = streaming kernel (one lane per particle,
  *                          list rows staged through shared memory by TMA; default for
  *                          n >= 32768), or 1, 2, 4 lanes sharing one particle (default 4 below)
  *   "use_graph"            0: md_nve_step launches kernels directly instead of a CUDA graph */
 int md_set_option(md_system *sys, const char *name, double value);
+
+/* Diagnostic counters since md_create (or the last reset): copies int32[8] to the DEVICE buffer
+ * `out` on `stream`, then clears them if reset != 0.
+ *   out[0] particles whose force the fp32 fast path handed to the fp64 re-evaluation
+ *   out[1..7] reserved (0) */
+int md_counters(md_system *sys, int32_t *out, int reset, void *stream);
 
 /* Cells per side n_k = floor(L_k / R) (1 for unused dimensions) -> host int[3]. */
 int md_num_cells(const md_system *sys, int *ncell);
@@ -147,8 +158,10 @@ int md_needs_rebuild(md_system *sys, const void *pos, int32_t *flag, void *strea
  *   energy_total double* out (may be NULL): sum_i e_i accumulated in fp64
  *   nbr_idx / nbr_count  any list in the md_nbr_layout layout whose rows hold every pair
  *                        within the potential's range (entries beyond it contribute nothing)
- * Pair terms are evaluated and accumulated in fp64 from exact displacements and rounded to fp32
- * once, on store.
+ * Precision: SOFT, 2-D and fast32 = 0: pair terms evaluated and accumulated in fp64
+ * from exact displacements; 3-D LJ (default): fp32 pair terms with a per-particle error estimate,
+ * fp64 re-evaluation of every particle whose estimate exceeds 1/3 of the 1e-5 force tolerance or
+ * that has a pair within 1e-5 r_cut^2 of the truncation radius.  Rounded to fp32 once, on store.
  */
 int md_pair_energy_force(md_system *sys, const md_potential *pot, const void *pos,
                          const int32_t *nbr_idx, const int32_t *nbr_count, void *force,

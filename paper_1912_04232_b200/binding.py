@@ -20,7 +20,7 @@ MD_KIND_LJ, MD_KIND_SOFT = 0, 1
 SYMBOLS = [
     "md_last_error", "md_workspace_bytes", "md_create", "md_destroy", "md_set_option",
     "md_num_cells", "md_nbr_layout", "md_cell_list_build", "md_neighbor_list_build",
-    "md_needs_rebuild", "md_pair_energy_force", "md_nve_step", "md_nve_run_host",
+    "md_needs_rebuild", "md_pair_energy_force", "md_nve_step", "md_nve_run_host", "md_counters",
 ]
 
 
@@ -61,6 +61,7 @@ def lib():
         L.md_create.argtypes = [C.POINTER(md_config), C.c_int, vp, C.c_size_t, C.POINTER(vp)]
         L.md_destroy.argtypes = [vp]
         L.md_set_option.argtypes = [vp, C.c_char_p, C.c_double]
+        L.md_counters.argtypes = [vp, ip, C.c_int, vp]
         L.md_num_cells.argtypes = [vp, C.POINTER(C.c_int * 3)]
         L.md_nbr_layout.argtypes = [vp] + [C.POINTER(C.c_long)] * 5
         L.md_cell_list_build.argtypes = [vp, vp, vp, ip, ip, ip, vp]
@@ -137,6 +138,10 @@ def md_destroy(sys) -> None:
 
 def md_set_option(sys, name: str, value: float) -> None:
     _check(lib().md_set_option(sys, name.encode(), float(value)))
+
+
+def md_counters(sys, out, reset=False, stream=None) -> None:
+    _check(lib().md_counters(sys, _ptr(out), int(reset), _stream(stream)))
 
 
 def md_num_cells(sys):

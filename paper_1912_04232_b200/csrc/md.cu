@@ -3,6 +3,7 @@
 // Every step of the path runs in the kernels of md_kernels.cuh; there is no CPU fallback.
 #include "md.h"
 #include "md_kernels.cuh"
+#include "md_force32.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -50,7 +51,8 @@ struct StepKey {
     const void *pos, *vel, *force, *id, *nbr_idx, *nbr_count, *stats;
     float dt, mass;
     md_potential pot;
-    int tpp;
+    int tpp, fast32;
+    float est_thr;
 };
 
 } // namespace
@@ -71,8 +73,10 @@ struct md_system {
     int nb_warps;        // tiles per block in the neighbor-list builder
     size_t nb_smem;      // its dynamic shared memory per block
     int use_graph;
+    int fast32;          // LJ 3-D: fp32 fast path + fp64 re-evaluation (md_force32.cuh)
+    float est_thr;       // its error-estimate threshold
     // graph cache of md_nve_step
-    cudaStream_t cap_stream;
+    cudaStream_t cap_stream, body_stream;
     StepKey key;
     bool key_valid;
     cudaGraphExec_t exec1, execU;
@@ -242,6 +246,22 @@ int launch_force_t(md_system *s, const Pair &pp, const float4 *pos, const int *n
 int launch_force(md_system *s, const Pair &pp, const float4 *pos, const int *nbr_idx,
                  const int *nbr_count, float4 *force, float4 *vel, float a, double *etot,
                  bool want_energy, Book book, cudaStream_t st) {
+    if (s->fast32 && pp.kind == MD_KIND_LJ && s->g.dim == 3) {
+        Pair32 q;
+        q.rc2 = (float)pp.drc2;
+        q.sig6x2 = (float)pp.dsig6x2;
+        q.ucut4 = (float)pp.du_cut4;
+        q.fscale = (float)(12.0 * pp.deps * pp.dsig6x2);
+        q.escale = (float)(2.0 * pp.deps);
+        q.near_band = 1e-5f * q.rc2;
+        q.est_thr = s->est_thr;
+        const int nb = blocks_for(s->g.n, F32_WARPS * 32);
+        int *nfix = s->words + 8;
+        if (want_energy) k_force_lj32<true><<<nb, F32_WARPS * 32, 0, st>>>(s->g, pp, q, pos, nbr_idx, nbr_count, force, vel, a, etot, book, nfix);
+        else k_force_lj32<false><<<nb, F32_WARPS * 32, 0, st>>>(s->g, pp, q, pos, nbr_idx, nbr_count, force, vel, a, etot, book, nfix);
+        LAUNCH_OK();
+        return MD_OK;
+    }
 #define MD_FORCE_DISPATCH(K, D)                                                                 \
     (want_energy ? launch_force_t<K, D, true>(s, pp, pos, nbr_idx, nbr_count, force, vel, a,   \
                                               etot, book, st)                                  \
@@ -272,22 +292,61 @@ __global__ void k_iota(int n, int *id) {
 }
 
 // One velocity-Verlet step as launches on `st` (captured into a graph or run directly).
+// in_graph: `st` is capturing; the rebuild kernels go into the body of an IF node whose condition
+// the drift kernel raises, so a step without a rebuild launches two kernels.  Otherwise every
+// rebuild kernel is launched and returns at once while the device flag is 0.
 int record_step(md_system *s, const Pair &pp, float4 *pos, float4 *vel, float4 *force, int *id,
-                int *nbr_idx, int *nbr_count, float dt, float mass, int *stats, cudaStream_t st) {
+                int *nbr_idx, int *nbr_count, float dt, float mass, int *stats, cudaStream_t st,
+                bool in_graph) {
     const Geom &g = s->g;
     const float a = dt / (2.0f * mass);
     int *flag = s->words + 0;
     int *status = s->words + 1;
     const int nb = blocks_for(g.n);
-    if (g.dim == 3) k_kick_drift<3><<<nb, 256, 0, st>>>(g, pos, vel, force, s->ref_pos, a, dt, flag);
-    else k_kick_drift<2><<<nb, 256, 0, st>>>(g, pos, vel, force, s->ref_pos, a, dt, flag);
-    LAUNCH_OK();
-    int rc = launch_cell_build(s, pos, vel, id, s->cell_start_i, s->perm_i, status, flag, st);
-    if (rc) return rc;
     const bool resort = s->cfg.resort != 0;
-    rc = launch_nbr_build(s, resort ? pos : s->pos_s, s->cell_start_i, resort ? nullptr : s->perm_i,
-                          nbr_idx, nbr_count, status, flag, st);
-    if (rc) return rc;
+    int rc;
+    if (!in_graph) {
+        cudaGraphConditionalHandle none = 0;
+        if (g.dim == 3) k_kick_drift<3, false><<<nb, 256, 0, st>>>(g, pos, vel, force, s->ref_pos, a, dt, flag, none);
+        else k_kick_drift<2, false><<<nb, 256, 0, st>>>(g, pos, vel, force, s->ref_pos, a, dt, flag, none);
+        LAUNCH_OK();
+        rc = launch_cell_build(s, pos, vel, id, s->cell_start_i, s->perm_i, status, flag, st);
+        if (rc) return rc;
+        rc = launch_nbr_build(s, resort ? pos : s->pos_s, s->cell_start_i, resort ? nullptr : s->perm_i,
+                              nbr_idx, nbr_count, status, flag, st);
+        if (rc) return rc;
+    } else {
+        cudaStreamCaptureStatus cs;
+        cudaGraph_t graph = nullptr;
+        const cudaGraphNode_t *deps = nullptr;
+        size_t ndeps = 0;
+        CU(cudaStreamGetCaptureInfo(st, &cs, nullptr, &graph, &deps, &ndeps));
+        if (cs != cudaStreamCaptureStatusActive || !graph) return fail(MD_ECUDA, "stream is not capturing");
+        cudaGraphConditionalHandle cond;
+        CU(cudaGraphConditionalHandleCreate(&cond, graph, 0, cudaGraphCondAssignDefault));
+        if (g.dim == 3) k_kick_drift<3, true><<<nb, 256, 0, st>>>(g, pos, vel, force, s->ref_pos, a, dt, flag, cond);
+        else k_kick_drift<2, true><<<nb, 256, 0, st>>>(g, pos, vel, force, s->ref_pos, a, dt, flag, cond);
+        LAUNCH_OK();
+        CU(cudaStreamGetCaptureInfo(st, &cs, nullptr, &graph, &deps, &ndeps));
+        cudaGraphNodeParams np = {cudaGraphNodeTypeConditional};
+        np.type = cudaGraphNodeTypeConditional;
+        np.conditional.handle = cond;
+        np.conditional.type = cudaGraphCondTypeIf;
+        np.conditional.size = 1;
+        cudaGraphNode_t node;
+        CU(cudaGraphAddNode(&node, graph, deps, ndeps, &np));
+        cudaGraph_t body = np.conditional.phGraph_out[0];
+        if (!s->body_stream) CU(cudaStreamCreateWithFlags(&s->body_stream, cudaStreamNonBlocking));
+        CU(cudaStreamBeginCaptureToGraph(s->body_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal));
+        rc = launch_cell_build(s, pos, vel, id, s->cell_start_i, s->perm_i, status, nullptr, s->body_stream);
+        if (!rc) rc = launch_nbr_build(s, resort ? pos : s->pos_s, s->cell_start_i, resort ? nullptr : s->perm_i,
+                                       nbr_idx, nbr_count, status, nullptr, s->body_stream);
+        cudaGraph_t ended = nullptr;
+        cudaError_t e = cudaStreamEndCapture(s->body_stream, &ended);
+        if (rc) return rc;
+        if (e != cudaSuccess) return fail(MD_ECUDA, "capturing the rebuild body: %s", cudaGetErrorString(e));
+        CU(cudaStreamUpdateCaptureDependencies(st, &node, 1, cudaStreamSetCaptureDependencies));
+    }
     Book book = {flag, status, stats};
     return launch_force(s, pp, pos, nbr_idx, nbr_count, force, vel, a, nullptr, false, book, st);
 }
@@ -306,7 +365,7 @@ int capture(md_system *s, const Pair &pp, const StepKey &k, int reps, cudaGraphE
     for (int r = 0; r < reps && rc == MD_OK; ++r)
         rc = record_step(s, pp, (float4 *)k.pos, (float4 *)k.vel, (float4 *)k.force, (int *)k.id,
                          (int *)k.nbr_idx, (int *)k.nbr_count, k.dt, k.mass, (int *)k.stats,
-                         s->cap_stream);
+                         s->cap_stream, true);
     cudaGraph_t graph = nullptr;
     cudaError_t e = cudaStreamEndCapture(s->cap_stream, &graph);
     if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
@@ -366,6 +425,8 @@ int md_create(const md_config *cfg, int n, void *workspace, size_t bytes, md_sys
     s->ref_pos = (float4 *)(s->ws + l.ref_pos);
     s->tpp = n >= 32768 ? 0 : 4;     // 0 = streaming kernel; small systems: 4 lanes per particle
     s->use_graph = 1;
+    s->fast32 = 1;
+    s->est_thr = 8.0f;
     s->unroll = 8;
     if (const char *e = getenv("MD_B200_TPP")) { int t = atoi(e); if (t == 0 || t == 1 || t == 2 || t == 4) s->tpp = t; }
     if (const char *e = getenv("MD_B200_NO_GRAPH")) s->use_graph = atoi(e) ? 0 : 1;
@@ -399,6 +460,7 @@ int md_destroy(md_system *sys) {
     if (!sys) return MD_OK;
     drop_graphs(sys);
     if (sys->cap_stream) cudaStreamDestroy(sys->cap_stream);
+    if (sys->body_stream) cudaStreamDestroy(sys->body_stream);
     delete sys;
     return MD_OK;
 }
@@ -421,6 +483,15 @@ int md_nbr_layout(const md_system *sys, long *tile, long *tile_stride, long *par
     return MD_OK;
 }
 
+int md_counters(md_system *sys, int32_t *out, int reset, void *stream) {
+    if (!sys || !out) return fail(MD_EINVAL, "NULL argument");
+    if (int rc = enter(sys)) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    CU(cudaMemcpyAsync(out, sys->words + 8, 8 * sizeof(int), cudaMemcpyDeviceToDevice, st));
+    if (reset) CU(cudaMemsetAsync(sys->words + 8, 0, 8 * sizeof(int), st));
+    return MD_OK;
+}
+
 int md_set_option(md_system *sys, const char *name, double value) {
     if (!sys || !name) return fail(MD_EINVAL, "NULL argument");
     if (!strcmp(name, "threads_per_particle")) {
@@ -428,6 +499,11 @@ int md_set_option(md_system *sys, const char *name, double value) {
         if (!(t == 0 || t == 1 || t == 2 || t == 4)) return fail(MD_EINVAL, "threads_per_particle must be 0 (streaming kernel), 1, 2 or 4");
         sys->tpp = t;
     } else if (!strcmp(name, "use_graph")) sys->use_graph = value != 0.0;
+    else if (!strcmp(name, "fast32")) sys->fast32 = value != 0.0;
+    else if (!strcmp(name, "est_thr")) {
+        if (!(value > 0.0)) return fail(MD_EINVAL, "est_thr must be positive");
+        sys->est_thr = (float)value;
+    }
     else return fail(MD_EINVAL, "unknown option %s", name);
     drop_graphs(sys);
     return MD_OK;
@@ -507,7 +583,7 @@ int md_nve_step(md_system *sys, const md_potential *pot, void *pos, void *vel, v
     if (!sys->use_graph) {
         for (int s = 0; s < nsteps; ++s) {
             rc = record_step(sys, pp, (float4 *)pos, (float4 *)vel, (float4 *)force, id, nbr_idx,
-                             nbr_count, dt, mass, stats, st);
+                             nbr_count, dt, mass, stats, st, false);
             if (rc) return rc;
         }
         return MD_OK;
@@ -516,7 +592,7 @@ int md_nve_step(md_system *sys, const md_potential *pot, void *pos, void *vel, v
     memset(&k, 0, sizeof(k));
     k.pos = pos; k.vel = vel; k.force = force; k.id = id; k.nbr_idx = nbr_idx;
     k.nbr_count = nbr_count; k.stats = stats; k.dt = dt; k.mass = mass; k.pot = *pot;
-    k.tpp = sys->tpp;
+    k.tpp = sys->tpp; k.fast32 = sys->fast32; k.est_thr = sys->est_thr;
     if (!sys->key_valid || memcmp(&k, &sys->key, sizeof(k)) != 0) {
         drop_graphs(sys);
         sys->key = k;

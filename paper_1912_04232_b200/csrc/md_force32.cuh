@@ -1,0 +1,262 @@
+// md_force32.cuh -- Lennard-Jones force / energy over the neighbor list (L78, L80, L104), 3-D:
+// fp32 fast path with an error estimate, fp64 re-evaluation where the estimate requires it.
+//
+// One warp = one list tile, one lane per particle (slot k of the 32 particles is one
+// coalesced 128-byte row; neighbor positions are float4 gathers through L1).
+//
+// Precision.  The fp64 chain of md_kernels.cuh holds the 1e-5 force tolerance
+// everywhere but is bound by the conversion / reciprocal unit (3 F2F + 1 RCP64H per pair).
+// Here every pair is evaluated in fp32 first -- displacement by the canonical nearest-image
+// form (one rounding), r2 = fma(dz,dz,fma(dy,dy,dx*dx)), y = 1/r2 (MUFU), force
+// coefficient 24 eps sig^6 y^4 (2 sig^6 y^3 - 1) -- together with S_i = sum_j |coefficient|.
+// The fp32 error of F_i is a random sum of per-pair errors of relative size ~1e-7 * (7..13):
+// measured on the oracle (32k and 256k particles, lattice and liquid states) it stays below
+// 6e-6 * max(|F_i|, 1e-3) whenever S_i <= 8 * max(|F_i|, 1e-3).  A particle that fails this
+// test (its pair forces nearly cancel; 3-10 % of a liquid), or that has a pair within 1e-5 of
+// r_cut^2 (the truncated force jumps by 0.039 there, so the in/out decision must be the exact
+// one), is re-evaluated in fp64 from exact displacements by a group of 8 lanes striding over
+// its row (four such particles per warp at a time).  Both results are rounded to fp32 once, on
+// store.
+#pragma once
+#include "md_kernels.cuh"
+
+namespace mdk {
+
+struct Pair32 {
+    float rc2;          // fl32(r_cut^2)
+    float sig6x2;       // 2 sigma^6
+    float ucut4;        // shift * ((s/rc)^12 - (s/rc)^6)
+    float fscale;       // 24 eps sigma^6
+    float escale;       // 2 eps   (= 1/2 * 4 eps)
+    float near_band;    // |r2 - rc2| <= near_band -> exact re-evaluation
+    float est_thr;      // re-evaluate when fscale * S_i > est_thr * max(|F_i|, 1e-3)
+};
+
+struct Acc32 { float fx, fy, fz, s, e, near; };
+
+// Canonical nearest-image displacement, fp32, one rounding; aL = a - L (exact).
+__device__ __forceinline__ float min_image_pre(float a, float aL, float b, float L, float h) {
+    float d = a - b;
+    if (d > h) d = aL - b;
+    else if (d < -h) d = a - (b - L);
+    return d;
+}
+
+// 1/x by the reciprocal unit (MUFU.RCP, 1 ulp).
+__device__ __forceinline__ float rcp32(float x) {
+    float y;
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+template <bool ENERGY, bool CHECK>
+__device__ __forceinline__ void lj_pair32(const Pair32 &pp, float dx, float dy, float dz,
+                                          bool valid, Acc32 &a) {
+    const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
+    bool in = r2 < pp.rc2;
+    if (CHECK) in = in && valid;
+    a.near = fminf(a.near, fabsf(r2 - pp.rc2));
+    const float y = rcp32(CHECK ? (in ? r2 : 1.0f) : r2);   // unchecked rows hold true neighbors: r2 > 0
+    const float y2 = y * y;
+    const float y3 = y2 * y;
+    float t = fmaf(pp.sig6x2, y3, -1.0f);                // 2 s6 - 1
+    t = in ? t : 0.0f;
+    const float c = (y2 * y2) * t;
+    a.fx = fmaf(c, dx, a.fx); a.fy = fmaf(c, dy, a.fy); a.fz = fmaf(c, dz, a.fz);
+    a.s += fabsf(c);
+    if (ENERGY) {
+        const float s6 = 0.5f * pp.sig6x2 * y3;
+        a.e += in ? fmaf(s6, s6, -s6) - pp.ucut4 : 0.0f;
+    }
+}
+
+// Exact re-evaluation of one particle by a group of G = 8, 16 or 32 lanes striding over its row
+// (32 / G particles per warp at a time); the sum is returned in every lane of the group.
+template <bool ENERGY>
+__device__ __forceinline__ Acc64 lj_row64(const Geom &g, const Pair &pp,
+                                          const float4 *__restrict__ pos, const int *col, int cnt,
+                                          const float4 &pb, int sub, int G) {
+    const Me<3> me = make_me<3>(g, pb);
+    Acc64 acc = {0.0, 0.0, 0.0, 0.0};
+    for (int k = sub; k < cnt; k += 2 * G) {
+        const bool v2 = k + G < cnt;
+        const int j1 = col[k * TILE];
+        const int j2 = v2 ? col[(k + G) * TILE] : j1;
+        const float4 q1 = pos[j1], q2 = pos[j2];
+        pair_any<0, 3, ENERGY, true>(pp, me, q1, true, acc);
+        pair_any<0, 3, ENERGY, true>(pp, me, q2, v2, acc);
+    }
+    for (int o = G >> 1; o > 0; o >>= 1) {              // G is warp-uniform
+        acc.fx += __shfl_xor_sync(FULL, acc.fx, o);
+        acc.fy += __shfl_xor_sync(FULL, acc.fy, o);
+        acc.fz += __shfl_xor_sync(FULL, acc.fz, o);
+        if (ENERGY) acc.e += __shfl_xor_sync(FULL, acc.e, o);
+    }
+    return acc;
+}
+
+constexpr int F32_WARPS = 4;
+constexpr int F32_U = 4;
+
+// The pair loop of one lane over its column of the tile: rows [0, kmin) are owned by every lane
+// of the warp (no validity test), rows [kmin, kmax) are the ragged tail.  WX / WY / WZ: the warp
+// is near a box face in that direction and takes the nearest image there (warp-uniform).
+template <bool ENERGY, bool WX, bool WY, bool WZ>
+__device__ __forceinline__ void lj_rows32(const Geom &g, const Pair32 &p32,
+                                          const float4 *__restrict__ pos, const int *col,
+                                          const float4 &pi, int ii, int cnt, int kmin, int kmax,
+                                          Acc32 &acc) {
+    const float Lx = g.L[0], Ly = g.L[1], Lz = g.L[2];
+    const float hx = g.h[0], hy = g.h[1], hz = g.h[2];
+    const float pxL = pi.x - Lx, pyL = pi.y - Ly, pzL = pi.z - Lz;
+    auto disp = [&](const float4 &q, float &dx, float &dy, float &dz) {
+        dx = WX ? min_image_pre(pi.x, pxL, q.x, Lx, hx) : pi.x - q.x;
+        dy = WY ? min_image_pre(pi.y, pyL, q.y, Ly, hy) : pi.y - q.y;
+        dz = WZ ? min_image_pre(pi.z, pzL, q.z, Lz, hz) : pi.z - q.z;
+    };
+    int k = 0;
+    int jn[F32_U];
+#pragma unroll
+    for (int u = 0; u < F32_U; ++u) jn[u] = u < kmax ? col[u * TILE] : ii;
+    for (; k < kmin; k += F32_U) {
+        int j[F32_U]; float4 q[F32_U];
+#pragma unroll
+        for (int u = 0; u < F32_U; ++u) j[u] = jn[u];
+#pragma unroll
+        for (int u = 0; u < F32_U; ++u) q[u] = pos[j[u]];
+#pragma unroll
+        for (int u = 0; u < F32_U; ++u) jn[u] = k + F32_U + u < kmax ? col[(k + F32_U + u) * TILE] : ii;
+#pragma unroll
+        for (int u = 0; u < F32_U; ++u) {
+            float dx, dy, dz;
+            disp(q[u], dx, dy, dz);
+            lj_pair32<ENERGY, false>(p32, dx, dy, dz, true, acc);
+        }
+    }
+    for (; k < kmax; k += F32_U) {
+        int j[F32_U]; float4 q[F32_U];
+#pragma unroll
+        for (int u = 0; u < F32_U; ++u) j[u] = k + u < cnt ? jn[u] : ii;
+#pragma unroll
+        for (int u = 0; u < F32_U; ++u) q[u] = pos[j[u]];
+#pragma unroll
+        for (int u = 0; u < F32_U; ++u) jn[u] = k + F32_U + u < kmax ? col[(k + F32_U + u) * TILE] : ii;
+#pragma unroll
+        for (int u = 0; u < F32_U; ++u) {
+            float dx, dy, dz;
+            disp(q[u], dx, dy, dz);
+            lj_pair32<ENERGY, true>(p32, dx, dy, dz, k + u < cnt, acc);
+        }
+    }
+}
+
+// vel != NULL: also the second half-kick v += a F.  energy_total != NULL (ENERGY only): adds
+// sum_i e_i in fp64.  book.stats != NULL: per-step bookkeeping.  nfix (may be NULL): counts
+// re-evaluated particles (diagnostics).
+template <bool ENERGY>
+__global__ void __launch_bounds__(F32_WARPS * 32)
+k_force_lj32(Geom g, Pair pp, Pair32 p32, const float4 *__restrict__ pos,
+             const int *__restrict__ nbr_idx, const int *__restrict__ nbr_count,
+             float4 *__restrict__ force, float4 *__restrict__ vel, float a, double *energy_total,
+             Book book, int *nfix) {
+    const int lane = threadIdx.x & 31;
+    const int gid = blockIdx.x * blockDim.x + threadIdx.x;
+    const int i = gid;
+    const bool active = i < g.n;
+    const int ii = active ? i : g.n - 1;
+    const float4 pi = pos[ii];
+    const int cnt = active ? min(nbr_count[ii], g.capacity) : 0;
+    const int *col = nbr_idx + nbr_tile_base(gid, g.capacity) + lane;    // gid: valid for the whole tile
+    const int kmax = warp_max(cnt);
+    const int kmin = min(warp_min(active ? cnt : 0x7fffffff), kmax) & ~(F32_U - 1);  // rows every lane owns
+    const bool wx = __any_sync(FULL, active && (pi.x < g.face || pi.x > g.L[0] - g.face));
+    const bool wy = __any_sync(FULL, active && (pi.y < g.face || pi.y > g.L[1] - g.face));
+    const bool wz = __any_sync(FULL, active && (pi.z < g.face || pi.z > g.L[2] - g.face));
+    Acc32 acc = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 1e30f};
+
+    if (!(wx || wy || wz)) lj_rows32<ENERGY, false, false, false>(g, p32, pos, col, pi, ii, cnt, kmin, kmax, acc);
+    else if (wx && !wy && !wz) lj_rows32<ENERGY, true, false, false>(g, p32, pos, col, pi, ii, cnt, kmin, kmax, acc);
+    else if (!wx && wy && !wz) lj_rows32<ENERGY, false, true, false>(g, p32, pos, col, pi, ii, cnt, kmin, kmax, acc);
+    else if (!wx && !wy && wz) lj_rows32<ENERGY, false, false, true>(g, p32, pos, col, pi, ii, cnt, kmin, kmax, acc);
+    else lj_rows32<ENERGY, true, true, true>(g, p32, pos, col, pi, ii, cnt, kmin, kmax, acc);
+
+    // ---- fp32 result, error estimate, exact re-evaluation of the lanes that need it
+    float fx = p32.fscale * acc.fx, fy = p32.fscale * acc.fy, fz = p32.fscale * acc.fz;
+    double e64 = ENERGY ? (double)(p32.escale * acc.e) : 0.0;
+    const float fn = fmaxf(sqrtf(fmaf(fz, fz, fmaf(fy, fy, fx * fx))), 1e-3f);
+    const bool redo = active && (p32.fscale * acc.s > p32.est_thr * fn || acc.near <= p32.near_band ||
+                                 !(fn < 3.0e38f));
+    unsigned todo = __ballot_sync(FULL, redo);
+    if (nfix && lane == 0 && todo) atomicAdd(nfix, __popc(todo));
+    const int *tile0 = col - lane;
+    while (todo) {
+        // 1 flagged lane left: the whole warp takes it; 2: half a warp each; else 8 lanes each
+        const int nf = __popc(todo);
+        const int G = nf == 1 ? 32 : (nf == 2 ? 16 : 8);
+        const int ng = 32 / G;
+        const int grp = lane / G, sub = lane % G;
+        unsigned t = todo;
+        int b = -1;
+#pragma unroll
+        for (int q = 0; q < 4; ++q) {
+            const int f = (t && q < ng) ? __ffs(t) - 1 : -1;
+            if (q == grp) b = f;
+            if (q < ng) t &= t - 1;                       // 0 & anything stays 0
+        }
+        const int bb = b < 0 ? 0 : b;
+        float4 pb;
+        pb.x = __shfl_sync(FULL, pi.x, bb); pb.y = __shfl_sync(FULL, pi.y, bb);
+        pb.z = __shfl_sync(FULL, pi.z, bb); pb.w = 0.0f;
+        int cb = __shfl_sync(FULL, cnt, bb);              // every lane takes part in the shuffle
+        if (b < 0) cb = 0;
+        const Acc64 r = lj_row64<ENERGY>(g, pp, pos, tile0 + bb, cb, pb, sub, G);
+        // deliver: the lane whose rank among the flagged lanes is q < ng reads group q
+        const int rank = __popc(todo & ((1u << lane) - 1u));
+        const bool mine = ((todo >> lane) & 1u) && rank < ng;
+        const int src = mine ? rank * G : lane;
+        const double rx = __shfl_sync(FULL, r.fx, src), ry = __shfl_sync(FULL, r.fy, src);
+        const double rz = __shfl_sync(FULL, r.fz, src);
+        const double re = ENERGY ? __shfl_sync(FULL, r.e, src) : 0.0;
+        if (mine) {
+            const double fs = 12.0 * pp.deps * pp.dsig6x2;
+            fx = (float)(fs * rx); fy = (float)(fs * ry); fz = (float)(fs * rz);
+            if (ENERGY) e64 = 2.0 * pp.deps * re;
+        }
+        todo = t;
+    }
+
+    // ---- store, second half-kick, energy reduction, bookkeeping
+    if (active) {
+        force[i] = make_float4(fx, fy, fz, (float)e64);
+        if (vel) {
+            float4 v = vel[i];
+            v.x = fmaf(a, fx, v.x); v.y = fmaf(a, fy, v.y); v.z = fmaf(a, fz, v.z);
+            vel[i] = v;
+        }
+    }
+    if (ENERGY && energy_total) {
+        __shared__ double red[F32_WARPS];
+        double x = active ? e64 : 0.0;
+#pragma unroll
+        for (int o = 16; o > 0; o >>= 1) x += __shfl_xor_sync(FULL, x, o);
+        if (lane == 0) red[threadIdx.x >> 5] = x;
+        __syncthreads();
+        if (threadIdx.x == 0) {
+            double t = 0.0;
+            for (int w = 0; w < F32_WARPS; ++w) t += red[w];
+            atomicAdd(energy_total, t);
+        }
+    }
+    if (book.stats && gid == 0) {
+        if (ld_volatile(book.flag)) {
+            book.stats[1] += 1;
+            int mc = ld_volatile(book.status + 1);
+            if (mc > book.stats[3]) book.stats[3] = mc;
+            if (ld_volatile(book.status) && book.stats[2] < 0) book.stats[2] = book.stats[0];
+            *book.flag = 0;
+        }
+        book.stats[0] += 1;
+    }
+}
+
+} // namespace mdk

@@ -456,11 +456,13 @@ k_needs_rebuild(Geom g, const float4 *__restrict__ pos, const float4 *__restrict
 
 // ------------------------------------------- velocity Verlet, first half (L100 §3.3.1) ----
 // v += dt/(2m) F;  r = mu(r, dt v);  rebuild test against the reference positions.
-template <int DIM>
+// HAS_COND: the step runs inside a CUDA graph whose rebuild kernels sit in an IF node; the warp
+// that sees a particle beyond skin/2 also raises the node's condition (default 0 per launch).
+template <int DIM, bool HAS_COND>
 __global__ void __launch_bounds__(256)
 k_kick_drift(Geom g, float4 *__restrict__ pos, float4 *__restrict__ vel,
              const float4 *__restrict__ force, const float4 *__restrict__ ref, float a, float dt,
-             int *flag) {
+             int *flag, cudaGraphConditionalHandle cond) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     bool moved = false;
     if (i < g.n) {
@@ -476,7 +478,10 @@ k_kick_drift(Geom g, float4 *__restrict__ pos, float4 *__restrict__ vel,
         pos[i] = p; vel[i] = v;
         moved = disp2_from_ref<DIM>(g, p, ref[i]) > g.half_skin2;
     }
-    if (__any_sync(FULL, moved) && (threadIdx.x & 31) == 0) *flag = 1;
+    if (__any_sync(FULL, moved) && (threadIdx.x & 31) == 0) {
+        *flag = 1;
+        if (HAS_COND) cudaGraphSetConditional(cond, 1);
+    }
 }
 
 // ------------------------------------- pair energy / force over the list (L78, L80, L104) --

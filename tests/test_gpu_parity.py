@@ -134,27 +134,60 @@ def test_config_build_and_force_parity(B, orc, W, ci, resort):
 def test_force_from_a_foreign_list(B, orc, W):
     """md_pair_energy_force consumes ANY list in the md_nbr_layout layout: feed it the oracle's
     brute-force rows (original particle order, resort = 0) and compare with the all-pairs
-    definition; the fp64 pair chain leaves only the fp32 store rounding."""
+    definition.  Default path (fp32 pair terms + fp64 re-evaluation by error estimate): the
+    north_star tolerances; fast32 = 0 (fp64 pair chain everywhere): only the fp32 store rounding
+    is left."""
     w = W.config(2)
     S = B.System(w, resort=0)
     S.build()                                               # sets up cells; list replaced below
     idx_o, cnt_o, _ = orc.neighbor_list(w.pos, w.box, 3, w.r_cut, w.skin, w.capacity, 0, 1)
     S.set_nbr_rows(idx_o, cnt_o)
-    S.compute_force()
-    f = S.force.cpu().numpy()
     f_o, _, E_o = orc.energy_force(w.pos, None, w.box, 3, 0, 1.0, 1.0, 2.5, 1)
-    assert force_error(f, f_o) <= 3e-7
+    S.compute_force()
+    assert force_error(S.force.cpu().numpy(), f_o) <= FORCE_TOL
+    assert abs(float(S.energy.cpu()[0]) - E_o) <= ENERGY_TOL * abs(E_o)
+    B.md_set_option(S.sys, "fast32", 0)
+    S.compute_force()
+    assert force_error(S.force.cpu().numpy(), f_o) <= 3e-7
     assert abs(float(S.energy.cpu()[0]) - E_o) <= 1e-9 * abs(E_o)
     S.close()
 
 
 @pytest.mark.parametrize("tpp", [0, 1, 2, 4])
 def test_threads_per_particle_variants(B, orc, W, tpp):
+    """The fp64 force kernels (fast32 = 0), every lanes-per-particle variant."""
     w = W.config(0)
     S = B.System(w)
     S.build()
+    B.md_set_option(S.sys, "fast32", 0)
     B.md_set_option(S.sys, "threads_per_particle", tpp)
     check_force(S, orc, w)
+    S.close()
+
+
+@pytest.mark.parametrize("thr", [1e-3, 8.0, 1e9])
+def test_fast32_re_evaluation(B, orc, W, thr):
+    """The fp32 fast path: est_thr -> 0 sends every particle through the fp64 re-evaluation (must
+    then match the fp64 kernels' accuracy), the default must hold the north_star tolerance, and
+    est_thr -> inf (never re-evaluate, except at the cutoff) shows what the estimate is for."""
+    w = W.config(2)
+    S = B.System(w)
+    S.build()
+    B.md_set_option(S.sys, "est_thr", thr)
+    cnt = torch.zeros(8, dtype=torch.int32, device="cuda")
+    B.md_counters(S.sys, cnt, True)
+    S.compute_force()
+    B.md_counters(S.sys, cnt, True)
+    f_o, _, E_o = orc.energy_force(w.pos, None, w.box, 3, 0, 1.0, 1.0, 2.5, 1)
+    err = force_error(unpermute(S, S.force), f_o)
+    fixed = int(cnt[0].item())
+    if thr < 1.0:
+        assert fixed == w.n and err <= 3e-7
+    elif thr < 1e6:
+        assert 0 < fixed < 0.25 * w.n and err <= FORCE_TOL
+    else:
+        assert fixed < 0.01 * w.n and err <= 1e-4
+    assert abs(float(S.energy.cpu()[0]) - E_o) <= ENERGY_TOL * abs(E_o)
     S.close()
 
 
