@@ -90,6 +90,8 @@ int md_destroy(md_system *sys);
  *   "threads_per_particle" fp64 force kernel variant: 0 = streaming kernel (one lane per particle,
  *                          list rows staged through shared memory by TMA; default for
  *                          n >= 32768), or 1, 2, 4 lanes sharing one particle (default 4 below)
+ *   "builder"              neighbor-list kernel: 2 (default) records hits in per-lane bit masks,
+ *                          1 appends them to per-lane shared-memory columns (first design)
  *   "use_graph"            0: md_nve_step launches kernels directly instead of a CUDA graph */
 int md_set_option(md_system *sys, const char *name, double value);
 

@@ -8,7 +8,8 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 SRC = [os.path.join(HERE, "csrc", "md.cu")]
 DEPS = SRC + [os.path.join(HERE, "csrc", "md_kernels.cuh"),
-              os.path.join(HERE, "csrc", "md_force32.cuh"), os.path.join(ROOT, "include", "md.h")]
+              os.path.join(HERE, "csrc", "md_force32.cuh"),
+              os.path.join(HERE, "csrc", "md_nbr2.cuh"), os.path.join(ROOT, "include", "md.h")]
 LIB = os.path.join(HERE, "libmd_b200.so")
 
 NVCC_FLAGS = [

@@ -4,6 +4,7 @@
 #include "md.h"
 #include "md_kernels.cuh"
 #include "md_force32.cuh"
+#include "md_nbr2.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -51,7 +52,7 @@ struct StepKey {
     const void *pos, *vel, *force, *id, *nbr_idx, *nbr_count, *stats;
     float dt, mass;
     md_potential pot;
-    int tpp, fast32;
+    int tpp, fast32, builder;
     float est_thr;
 };
 
@@ -73,6 +74,7 @@ struct md_system {
     int nb_warps;        // tiles per block in the neighbor-list builder
     size_t nb_smem;      // its dynamic shared memory per block
     int use_graph;
+    int builder;         // neighbor-list builder: 2 = bit-mask (md_nbr2.cuh), 1 = column append
     int fast32;          // LJ 3-D: fp32 fast path + fp64 re-evaluation (md_force32.cuh)
     float est_thr;       // its error-estimate threshold
     // graph cache of md_nve_step
@@ -199,9 +201,24 @@ int launch_cell_build(md_system *s, float4 *pos, float4 *vel, int *id, int *cell
 }
 
 int launch_nbr_build(md_system *s, const float4 *spos, const int *cell_start, const int *map,
-                     int *nbr_idx, int *nbr_count, int *status, const int *cond, cudaStream_t st) {
+                     int *nbr_idx, int *nbr_count, int *status, const int *cond, int incremental,
+                     cudaStream_t st) {
     const Geom &g = s->g;
     const int ntiles = (g.n + TILE - 1) / TILE;
+    if (s->builder == 2) {          // bit-mask builder (md_nbr2.cuh)
+        const int nb = (ntiles + NB2_WARPS - 1) / NB2_WARPS;
+        const int threads = NB2_WARPS * 32;
+        const size_t sm = NB2_WARPS * sizeof(Nb2Warp);
+        if (g.dim == 3) {
+            if (map) k_nbr_build2<3, true><<<nb, threads, sm, st>>>(g, spos, cell_start, map, nbr_idx, nbr_count, status, s->ref_pos, cond, incremental);
+            else k_nbr_build2<3, false><<<nb, threads, sm, st>>>(g, spos, cell_start, map, nbr_idx, nbr_count, status, s->ref_pos, cond, incremental);
+        } else {
+            if (map) k_nbr_build2<2, true><<<nb, threads, sm, st>>>(g, spos, cell_start, map, nbr_idx, nbr_count, status, s->ref_pos, cond, incremental);
+            else k_nbr_build2<2, false><<<nb, threads, sm, st>>>(g, spos, cell_start, map, nbr_idx, nbr_count, status, s->ref_pos, cond, incremental);
+        }
+        LAUNCH_OK();
+        return MD_OK;
+    }
     const int nb = (ntiles + s->nb_warps - 1) / s->nb_warps;
     const int threads = s->nb_warps * 32;
     if (g.dim == 3) {
@@ -313,7 +330,7 @@ int record_step(md_system *s, const Pair &pp, float4 *pos, float4 *vel, float4 *
         rc = launch_cell_build(s, pos, vel, id, s->cell_start_i, s->perm_i, status, flag, st);
         if (rc) return rc;
         rc = launch_nbr_build(s, resort ? pos : s->pos_s, s->cell_start_i, resort ? nullptr : s->perm_i,
-                              nbr_idx, nbr_count, status, flag, st);
+                              nbr_idx, nbr_count, status, flag, 1, st);
         if (rc) return rc;
     } else {
         cudaStreamCaptureStatus cs;
@@ -340,7 +357,7 @@ int record_step(md_system *s, const Pair &pp, float4 *pos, float4 *vel, float4 *
         CU(cudaStreamBeginCaptureToGraph(s->body_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal));
         rc = launch_cell_build(s, pos, vel, id, s->cell_start_i, s->perm_i, status, nullptr, s->body_stream);
         if (!rc) rc = launch_nbr_build(s, resort ? pos : s->pos_s, s->cell_start_i, resort ? nullptr : s->perm_i,
-                                       nbr_idx, nbr_count, status, nullptr, s->body_stream);
+                                       nbr_idx, nbr_count, status, nullptr, 1, s->body_stream);
         cudaGraph_t ended = nullptr;
         cudaError_t e = cudaStreamEndCapture(s->body_stream, &ended);
         if (rc) return rc;
@@ -426,6 +443,7 @@ int md_create(const md_config *cfg, int n, void *workspace, size_t bytes, md_sys
     s->tpp = n >= 32768 ? 0 : 4;     // 0 = streaming kernel; small systems: 4 lanes per particle
     s->use_graph = 1;
     s->fast32 = 1;
+    s->builder = 2;
     s->est_thr = 8.0f;
     s->unroll = 8;
     if (const char *e = getenv("MD_B200_TPP")) { int t = atoi(e); if (t == 0 || t == 1 || t == 2 || t == 4) s->tpp = t; }
@@ -447,6 +465,11 @@ int md_create(const md_config *cfg, int n, void *workspace, size_t bytes, md_sys
             ea = cudaFuncSetAttribute(k_nbr_build<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->nb_smem);
             if (ea == cudaSuccess) ea = cudaFuncSetAttribute(k_nbr_build<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->nb_smem);
         }
+        const int sm2 = (int)(NB2_WARPS * sizeof(Nb2Warp));
+        if (ea == cudaSuccess) ea = cudaFuncSetAttribute(k_nbr_build2<3, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm2);
+        if (ea == cudaSuccess) ea = cudaFuncSetAttribute(k_nbr_build2<3, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm2);
+        if (ea == cudaSuccess) ea = cudaFuncSetAttribute(k_nbr_build2<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm2);
+        if (ea == cudaSuccess) ea = cudaFuncSetAttribute(k_nbr_build2<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm2);
         if (ea != cudaSuccess) { delete s; return fail(MD_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(ea)); }
     }
     cudaError_t e = cudaMemset(workspace, 0, l.total);
@@ -500,6 +523,10 @@ int md_set_option(md_system *sys, const char *name, double value) {
         sys->tpp = t;
     } else if (!strcmp(name, "use_graph")) sys->use_graph = value != 0.0;
     else if (!strcmp(name, "fast32")) sys->fast32 = value != 0.0;
+    else if (!strcmp(name, "builder")) {
+        if (value != 1.0 && value != 2.0) return fail(MD_EINVAL, "builder must be 1 or 2");
+        sys->builder = (int)value;
+    }
     else if (!strcmp(name, "est_thr")) {
         if (!(value > 0.0)) return fail(MD_EINVAL, "est_thr must be positive");
         sys->est_thr = (float)value;
@@ -534,7 +561,7 @@ int md_neighbor_list_build(md_system *sys, const void *pos, const int32_t *cell_
         LAUNCH_OK();
         spos = sys->pos_s; map = perm;
     }
-    return launch_nbr_build(sys, spos, cell_start, map, nbr_idx, nbr_count, status, nullptr, st);
+    return launch_nbr_build(sys, spos, cell_start, map, nbr_idx, nbr_count, status, nullptr, 0, st);
 }
 
 int md_needs_rebuild(md_system *sys, const void *pos, int32_t *flag, void *stream) {
@@ -592,7 +619,7 @@ int md_nve_step(md_system *sys, const md_potential *pot, void *pos, void *vel, v
     memset(&k, 0, sizeof(k));
     k.pos = pos; k.vel = vel; k.force = force; k.id = id; k.nbr_idx = nbr_idx;
     k.nbr_count = nbr_count; k.stats = stats; k.dt = dt; k.mass = mass; k.pot = *pot;
-    k.tpp = sys->tpp; k.fast32 = sys->fast32; k.est_thr = sys->est_thr;
+    k.tpp = sys->tpp; k.fast32 = sys->fast32; k.builder = sys->builder; k.est_thr = sys->est_thr;
     if (!sys->key_valid || memcmp(&k, &sys->key, sizeof(k)) != 0) {
         drop_graphs(sys);
         sys->key = k;

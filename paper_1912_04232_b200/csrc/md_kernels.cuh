@@ -92,45 +92,46 @@ k_cell_assign(Geom g, const float4 *__restrict__ pos, int *__restrict__ cell_of,
 }
 
 // One block: exclusive scan of cell_count[0..cells) into cell_start[0..cells]; zeroes
-// cell_count for the next build and resets the build status words.
+// cell_count for the next build and resets the build status words.  Every thread owns a run of
+// consecutive cells (its loads are independent, so their latency overlaps), sums it, the 1024
+// partial sums are scanned once through shared memory, and the run is written back.
 __global__ void __launch_bounds__(1024)
 k_cell_scan(int cells, int *__restrict__ cell_count, int *__restrict__ cell_start,
             int *status, const int *cond) {
     if (cond && ld_volatile(cond) == 0) return;
     __shared__ int warp_sum[32];
-    __shared__ int carry;
     const int tid = threadIdx.x, lane = tid & 31, wid = tid >> 5;
-    if (tid == 0) { carry = 0; if (status) { status[0] = 0; status[1] = 0; } }
+    if (tid == 0 && status) { status[0] = 0; status[1] = 0; }
+    const int per = (cells + 1023) / 1024;
+    const int c0 = min(tid * per, cells), c1 = min(c0 + per, cells);
+    int sum = 0;
+    for (int c = c0; c < c1; ++c) sum += cell_count[c];
+    int x = sum;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        int y = __shfl_up_sync(FULL, x, o);
+        if (lane >= o) x += y;
+    }
+    if (lane == 31) warp_sum[wid] = x;
     __syncthreads();
-    for (int base = 0; base < cells; base += 1024) {
-        int c = base + tid;
-        int v = c < cells ? cell_count[c] : 0;
-        if (c < cells) cell_count[c] = 0;
-        int x = v;
+    if (wid == 0) {
+        int w = warp_sum[lane];
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
-            int y = __shfl_up_sync(FULL, x, o);
-            if (lane >= o) x += y;
+            int y = __shfl_up_sync(FULL, w, o);
+            if (lane >= o) w += y;
         }
-        if (lane == 31) warp_sum[wid] = x;
-        __syncthreads();
-        if (wid == 0) {
-            int w = warp_sum[lane];
-#pragma unroll
-            for (int o = 1; o < 32; o <<= 1) {
-                int y = __shfl_up_sync(FULL, w, o);
-                if (lane >= o) w += y;
-            }
-            warp_sum[lane] = w;
-        }
-        __syncthreads();
-        int incl = x + (wid ? warp_sum[wid - 1] : 0) + carry;
-        if (c < cells) cell_start[c] = incl - v;
-        __syncthreads();
-        if (tid == 1023) carry = incl;
-        __syncthreads();
+        warp_sum[lane] = w;
     }
-    if (tid == 0) cell_start[cells] = carry;
+    __syncthreads();
+    int run = x - sum + (wid ? warp_sum[wid - 1] : 0);           // exclusive prefix of my run
+    for (int c = c0; c < c1; ++c) {
+        const int v = cell_count[c];
+        cell_count[c] = 0;
+        cell_start[c] = run;
+        run += v;
+    }
+    if (tid == 1023) cell_start[cells] = warp_sum[31];
 }
 
 __global__ void __launch_bounds__(256)

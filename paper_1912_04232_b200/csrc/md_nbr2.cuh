@@ -9,7 +9,7 @@
 // 12 warps per SM) through a chain of predicated store / pointer bumps, 12.5 instructions per
 // candidate.  Here the sign bit of fl(r2 - R2) -- set exactly when r2 < R2 -- is shifted into a
 // per-lane bit mask, one funnel shift per candidate and no branch, 32 candidates per word; the
-// masks of up to NB2_WORDS words (4 KB per warp) are expanded afterwards, every lane pulling
+// masks of up to NB2_WORDS words (5 KB per warp) are expanded afterwards, every lane pulling
 // its next set bit per iteration, so row k of the tile leaves as one coalesced 128-byte store.
 #pragma once
 #include "md_kernels.cuh"
@@ -17,7 +17,7 @@
 namespace mdk {
 
 constexpr int NB2_WARPS = 8;          // tiles per block
-constexpr int NB2_WORDS = 32;         // mask words per lane per batch (1024 candidates)
+constexpr int NB2_WORDS = 40;         // mask words per lane per batch (1280 candidates)
 constexpr int NB2_CHUNK = 128;        // candidates staged per round (4 words)
 
 struct Nb2Warp {                      // shared memory of one builder warp
@@ -39,7 +39,7 @@ __device__ __forceinline__ unsigned push4(unsigned m, float2 a, float2 b) {
 // already holds the pad value beyond its previous count, so only rows [count, previous count)
 // are re-padded; 0: rows [count, capacity) are written.
 template <int DIM, bool MAPPED>
-__global__ void __launch_bounds__(NB2_WARPS * 32)
+__global__ void __launch_bounds__(NB2_WARPS * 32, 4)
 k_nbr_build2(Geom g, const float4 *__restrict__ spos, const int *__restrict__ cell_start,
              const int *__restrict__ map, int *__restrict__ nbr_idx, int *__restrict__ nbr_count,
              int *status, float4 *__restrict__ ref_pos, const int *cond, int incremental) {
@@ -94,26 +94,138 @@ k_nbr_build2(Geom g, const float4 *__restrict__ spos, const int *__restrict__ ce
                 if (cb >= ca) { t0 = cell_start[rowbase + ca]; t1 = cell_start[rowbase + cb + 1]; }
             }
             int nw = 0;                      // mask words of the current batch (warp-uniform)
-            unsigned nz = 0;                 // which of them are non-zero for this lane
-
-            // every lane pulls its next hit per iteration: row k leaves as one 128-byte store
+            // every lane pulls its next hit per iteration (moving on to its next mask word when the
+            // current one is used up): row k of the tile leaves as one 128-byte store
             auto expand = [&]() {
                 __syncwarp();
-                unsigned pend = inseg ? nz : 0u, word = 0u;
-                int w = 0;
+                const int nwl = inseg ? nw : 0;
+                unsigned word = 0u;
+                int w = -1;
                 while (true) {
-                    if (word == 0u && pend) { w = __ffs(pend) - 1; pend &= pend - 1; word = W.mask[w][lane]; }
-                    if (!__any_sync(FULL, word != 0u)) break;
-                    if (word) {
-                        const int bit = __clz(word);
-                        word &= ~(0x80000000u >> bit);
-                        const int slot = W.wbase[w] + bit;
-                        if (slot != s) {
-                            if (cnt < cap) outp[cnt * TILE] = MAPPED ? map[slot] : slot;
-                            ++cnt;
-                        }
-                    }
+                    const bool more = w + 1 < nwl;
+                    if (word == 0u && more) { ++w; word = W.mask[w][lane]; }
+                    if (!__any_sync(FULL, word != 0u || w + 1 < nwl)) break;
+                    const int bit = __clz(word);                 // 32 when word == 0
+                    const int slot = W.wbase[max(w, 0)] + bit;
+                    const bool hit = word != 0u && slot != s;
+                    word &= 0x7fffffffu >> (bit & 31);           // drop that bit (all above it are 0)
+                    if (hit && cnt < cap) outp[cnt * TILE] = MAPPED ? map[slot] : slot;
+                    cnt += hit ? 1 : 0;
                 }
                 __syncwarp();
-                nw = 0; nz = 0u;
+                nw = 0;
             };
+
+            // ---- walk the pieces; the next chunk is loaded while the current one is tested
+            int p = 0, base = 0, pt1 = 0;
+            auto seek = [&](int &pp, int &bb, int &tt1) {       // first non-empty piece >= pp
+                while (pp < 3 * ROWS) {
+                    bb = __shfl_sync(FULL, t0, pp); tt1 = __shfl_sync(FULL, t1, pp);
+                    if (bb < tt1) return;
+                    ++pp;
+                }
+            };
+            seek(p, base, pt1);
+            float4 q[NB2_CHUNK / 32];
+            auto fetch = [&](int bb, int tt1) {
+#pragma unroll
+                for (int u = 0; u < NB2_CHUNK / 32; ++u) {
+                    const int t = bb + u * 32 + lane;
+                    if (t < tt1) q[u] = spos[t];
+                }
+            };
+            if (p < 3 * ROWS) fetch(base, pt1);
+            while (p < 3 * ROWS) {
+                const int kind = p / ROWS, rr = p % ROWS;
+                const int dy = rr % 3 - 1, dz = DIM == 3 ? rr / 3 - 1 : 0;
+                // image shifts of this piece: candidates by -L when the piece is the
+                // high-side row/cell, my own coordinate by -L when it is the low-side one
+                const float sjx = kind == 1 ? Lx : 0.0f;
+                const float sjy = rcy + dy < 0 ? Ly : 0.0f;
+                const float sjz = (DIM == 3 && rcz + dz < 0) ? Lz : 0.0f;
+                const float pix = kind == 2 ? __fsub_rn(pi.x, Lx) : pi.x;
+                const float piy = rcy + dy >= ncy ? __fsub_rn(pi.y, Ly) : pi.y;
+                const float piz = (DIM == 3 && rcz + dz >= ncz) ? __fsub_rn(pi.z, Lz) : pi.z;
+                const int m = min(NB2_CHUNK, pt1 - base);
+                if (nw + ((m + 31) >> 5) > NB2_WORDS) expand();   // batch full (warp-uniform)
+                // stage -(candidate - shift), structure of arrays; the tail of the last group of
+                // four is a far-away point
+#pragma unroll
+                for (int u = 0; u < NB2_CHUNK / 32; ++u) {
+                    const int c = u * 32 + lane;
+                    if (c < m) {
+                        W.sx[c] = __fsub_rn(sjx, q[u].x);
+                        W.sy[c] = __fsub_rn(sjy, q[u].y);
+                        if (DIM == 3) W.sz[c] = __fsub_rn(sjz, q[u].z);
+                    } else if (c < ((m + 3) & ~3)) {
+                        W.sx[c] = 1e18f; W.sy[c] = 0.0f;
+                        if (DIM == 3) W.sz[c] = 0.0f;
+                    }
+                }
+                if (lane < ((m + 31) >> 5)) W.wbase[nw + lane] = base + lane * 32;
+                __syncwarp();
+                // next chunk
+                int np = p, nbase = base + NB2_CHUNK, npt1 = pt1;
+                if (nbase >= pt1) { ++np; seek(np, nbase, npt1); }
+                if (np < 3 * ROWS) fetch(nbase, npt1);
+                // test the staged chunk: 32 candidates per mask word, two per packed instruction
+                // (FADD2 / FMUL2 / FFMA2, round-to-nearest: the bits of the scalar canonical form)
+                const float2 px2 = make_float2(pix, pix), py2 = make_float2(piy, piy);
+                const float2 pz2 = make_float2(piz, piz);
+                auto four = [&](int c, unsigned acc) {
+                    const float4 X = *reinterpret_cast<const float4 *>(W.sx + c);
+                    const float4 Y = *reinterpret_cast<const float4 *>(W.sy + c);
+                    const float2 dxa = __fadd2_rn(px2, make_float2(X.x, X.y));
+                    const float2 dxb = __fadd2_rn(px2, make_float2(X.z, X.w));
+                    const float2 dya = __fadd2_rn(py2, make_float2(Y.x, Y.y));
+                    const float2 dyb = __fadd2_rn(py2, make_float2(Y.z, Y.w));
+                    float2 ra = __ffma2_rn(dya, dya, __fmul2_rn(dxa, dxa));
+                    float2 rb = __ffma2_rn(dyb, dyb, __fmul2_rn(dxb, dxb));
+                    if (DIM == 3) {
+                        const float4 Z = *reinterpret_cast<const float4 *>(W.sz + c);
+                        const float2 dza = __fadd2_rn(pz2, make_float2(Z.x, Z.y));
+                        const float2 dzb = __fadd2_rn(pz2, make_float2(Z.z, Z.w));
+                        ra = __ffma2_rn(dza, dza, ra);
+                        rb = __ffma2_rn(dzb, dzb, rb);
+                    }
+                    // sign(fl(r2 - R2)) is set exactly when r2 < R2 (a non-zero difference of two
+                    // floats never rounds to zero, and x - x = +0)
+                    return push4(acc, __fadd2_rn(ra, nR2), __fadd2_rn(rb, nR2));
+                };
+                for (int c0 = 0; c0 < m; c0 += 32) {
+                    const int ng = min(8, (m - c0 + 3) >> 2);
+                    unsigned hi = 0u, lo = 0u;
+                    if (ng == 8) {
+#pragma unroll
+                        for (int gq = 0; gq < 4; ++gq) hi = four(c0 + 4 * gq, hi);
+#pragma unroll
+                        for (int gq = 4; gq < 8; ++gq) lo = four(c0 + 4 * gq, lo);
+                        hi = (hi << 16) | lo;
+                    } else {
+                        for (int gq = 0; gq < ng; ++gq) hi = four(c0 + 4 * gq, hi);
+                        hi <<= 32 - 4 * ng;
+                    }
+                    W.mask[nw][lane] = hi;
+                    ++nw;
+                }
+                __syncwarp();
+                p = np; base = nbase; pt1 = npt1;
+            }
+            expand();
+        }
+        // ---- pads (= N, A5), counts, rebuild reference, status
+        if (outp) {
+            const int upto = incremental ? prev : cap;
+            for (int k = min(cnt, cap); k < upto; ++k) outp[k * TILE] = g.n;
+        }
+        if (act) { nbr_count[me] = cnt; ref_pos[me] = pi; }
+        const int mx = warp_max(act ? cnt : 0);
+        if (lane == 0) {
+            if (mx > ld_volatile(status + 1)) atomicMax(status + 1, mx);
+            if (mx > cap) status[0] = 1;
+        }
+        __syncwarp();
+    }
+}
+
+} // namespace mdk

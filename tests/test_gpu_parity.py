@@ -165,6 +165,18 @@ def test_threads_per_particle_variants(B, orc, W, tpp):
     S.close()
 
 
+@pytest.mark.parametrize("ci", [0, 1])
+def test_first_design_builder(B, orc, W, ci):
+    """builder = 1 (per-lane shared-memory columns) still builds the same rows."""
+    w = W.config(ci)
+    S = B.System(w)
+    B.md_set_option(S.sys, "builder", 1)
+    S.build()
+    torch.cuda.synchronize()
+    check_list(S, orc, w, method=0)
+    S.close()
+
+
 @pytest.mark.parametrize("thr", [1e-3, 8.0, 1e9])
 def test_fast32_re_evaluation(B, orc, W, thr):
     """The fp32 fast path: est_thr -> 0 sends every particle through the fp64 re-evaluation (must
