@@ -4,7 +4,7 @@
 One bench "step" = `--md-steps` (default 100) velocity-Verlet steps of config 3 through ONE
 md_nve_step call: the whole hot path (kick/drift/rebuild test, conditional cell list + re-sort
 + neighbor list, LJ force + second kick), rebuilds amortised.  Defaults: 3 warm-up steps (the
-jittered lattice melts), 10 timed steps = the config's 1000 MD steps.
+jittered lattice melts), 20 timed steps = twice the config's 1000 MD steps.
 
   value      device-resident state, CUDA events per bench step on the launching stream,
              L2 flushed between bench steps (not timed), max over ranks
@@ -12,7 +12,8 @@ jittered lattice melts), 10 timed steps = the config's 1000 MD steps.
              out, H2D + list build + steps + D2H all inside the timed region
   roofline   the force kernel (dominant): algorithmic bytes (4*Kbar + 36) * N per launch
               over its average duration, L2 flushed before every launch,
-             against MEASURED_PEAKS.json's hbm_gbs
+             against MEASURED_PEAKS.json's hbm_gbs; `traffic` = DRAM bytes per launch from the
+             committed ncu capture (profiles/r1b_kernels.txt), config 3 only
   cpu_baseline  the fp64 oracle's own list-based loop on the host cores, bounded sample
 
 `--impl reference` times the oracle (this tier's reference arm) instead.
@@ -38,12 +39,15 @@ sys.path.insert(0, ROOT)
 METRIC = "LJ NVE particle-steps/sec at N=256k (incl. amortised rebuilds)"
 UNIT = "particle-steps/s"
 FALLBACK_HBM_GBS = 6650.0      # /opt/skills/guides/B200_PROFILING.md fallback
+# dram__bytes_read.sum + dram__bytes_write.sum of k_force_lj32 at N = 256,000, one ncu --set full
+# capture (profiles/r1b_kernels.txt: 91.37 MB + 3.56 MB)
+FORCE_TRAFFIC_CFG3 = 94.92e6
 
 
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
     ap.add_argument("--config", type=int, default=3, help="BASELINE.json config index")
@@ -65,8 +69,10 @@ def peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md)."""
-    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
+    """nvidia-smi clocks / throttle reasons (B200_PROFILING.md).  Started before the warm-up so
+    that the tool is already printing when the timed region begins; stop(t0, t1) keeps only the
+    samples whose timestamp falls inside the timed region [t0, t1] (host wall clock)."""
+    Q = ("timestamp,index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
          "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
@@ -77,7 +83,7 @@ class ClockSampler:
         try:
             self.proc = subprocess.Popen(
                 ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
-                 "--format=csv,noheader,nounits", "-lms", "100"],
+                 "--format=csv,noheader,nounits", "-lms", "20"],
                 stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
@@ -88,7 +94,8 @@ class ClockSampler:
         for line in self.proc.stdout:
             self.lines.append(line.strip())
 
-    def stop(self):
+    def stop(self, t0=None, t1=None):
+        import datetime
         if not self.proc:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         self.proc.terminate()
@@ -96,22 +103,27 @@ class ClockSampler:
             self.proc.wait(timeout=2)
         except Exception:
             self.proc.kill()
-        sm, mx, reasons = [], [], set()
+        sm, mx, reasons, allsm = [], [], set(), []
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for ln in self.lines:
             f = [x.strip() for x in ln.split(",")]
-            if len(f) < 9:
+            if len(f) < 10:
                 continue
             try:
-                sm.append(float(f[1])); mx.append(float(f[2]))
+                ts = datetime.datetime.strptime(f[0], "%Y/%m/%d %H:%M:%S.%f").timestamp()
+                clk, cmax = float(f[2]), float(f[3])
             except ValueError:
                 continue
-            for name, v in zip(names, f[5:9]):
+            allsm.append(clk)
+            if t0 is not None and not (t0 <= ts <= t1):
+                continue
+            sm.append(clk); mx.append(cmax)
+            for name, v in zip(names, f[6:10]):
                 if v.lower().startswith("active"):
                     reasons.add(name)
         return {"sm_mhz": statistics.median(sm) if sm else None,
                 "sm_max_mhz": max(mx) if mx else None, "samples": len(sm),
-                "reasons": sorted(reasons)}
+                "samples_total": len(allsm), "reasons": sorted(reasons)}
 
 
 def oracle_sample(w, md_steps):
@@ -166,6 +178,7 @@ def main():
     import torch
     import torch.distributed as dist
     from paper_1912_04232_b200 import binding as B
+    from paper_1912_04232_b200 import replicas as R
     from paper_1912_04232_b200 import workloads as W
 
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -180,7 +193,7 @@ def main():
     B.lib()
 
     # replicas: rank r simulates an independent sample of the same config
-    w = W.config(args.config, replica=rank)
+    w = W.config(args.config, replica=R.replica_index(rank))
     S = B.System(w, device=dev)
     stream = torch.cuda.Stream(device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # 2x the 126 MB L2
@@ -195,11 +208,12 @@ def main():
     with torch.cuda.stream(stream):
         S.build(stream)
         S.compute_force(True, stream)
+        sampler = ClockSampler(local)
+        sampler.start()
         for _ in range(args.warmup):
             S.step(md_steps, stream)
         barrier()
-        sampler = ClockSampler(local)
-        sampler.start()
+        t_region0 = time.time()
         ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
               for _ in range(args.steps)]
         rebuilds = 0
@@ -211,7 +225,7 @@ def main():
             b.record(stream)
             stats_acc.append(S.stats.clone())
         barrier()
-        clocks = sampler.stop()
+        clocks = sampler.stop(t_region0, time.time())
         ms = sum(a.elapsed_time(b) for a, b in ev)
         rebuilds = int(sum(int(s[1]) for s in stats_acc))
         max_count = int(max(int(s[3]) for s in stats_acc))
@@ -247,11 +261,8 @@ def main():
             build_ms = statistics.median(a.elapsed_time(b) for a, b in bev)
             S.compute_force(False, stream)
 
-    t_ms = torch.tensor([ms], dtype=torch.float64, device=dev)
-    if world > 1:
-        dist.all_reduce(t_ms, op=dist.ReduceOp.MAX)
-    ms_max = float(t_ms[0])
-    value = world * w.n * md_steps * args.steps / (ms_max * 1e-3)
+    ms_max = R.max_over_ranks(ms, dev)
+    value = R.whole_job_rate(w.n * md_steps * args.steps, ms_max * 1e-3)
 
     # ---- e2e through the host-buffer entry point (pinned host memory)
     e2e = None
@@ -268,10 +279,7 @@ def main():
             B.md_nve_run_host(S.cfg, S.pot, pos_h, vel_h, force_h, w.dt, w.mass, md_steps, stats_h)
         barrier()
         dt_e2e = time.perf_counter() - t0
-        t_e = torch.tensor([dt_e2e], dtype=torch.float64, device=dev)
-        if world > 1:
-            dist.all_reduce(t_e, op=dist.ReduceOp.MAX)
-        e2e = {"value": world * w.n * md_steps * e2e_steps / float(t_e[0]), "unit": UNIT,
+        e2e = {"value": R.whole_job_rate(w.n * md_steps * e2e_steps, R.max_over_ranks(dt_e2e, dev)), "unit": UNIT,
                "h2d_bytes_per_step": 2 * w.n * 16, "d2h_bytes_per_step": 3 * w.n * 16 + 8 + 16,
                "what": f"md_nve_run_host: pinned host pos/vel in, list build + {md_steps} MD steps, host pos/vel/force/energy/stats out"}
 
@@ -301,11 +309,14 @@ def main():
         "max_neighbors": max_count, "overflow": overflow,
         "step_hbm_frac": step_bytes / (1e3 * ms_max / (args.steps * md_steps) * 1e-6) / 1e9 / peak,
         "clocks": clocks,
-        "roofline": {"bound": "hbm", "kernel": "k_force (md_pair_energy_force)", "achieved": achieved,
-                     "peak": peak, "unit": "GB/s", "frac": achieved / peak, "traffic": None,
+        "roofline": {"bound": "hbm", "kernel": "k_force_lj32 (md_pair_energy_force)", "achieved": achieved,
+                     "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": FORCE_TRAFFIC_CFG3 if args.config == 3 else None,
                      "peak_source": peak_src, "algorithmic_bytes": algo_bytes, "kbar": kbar,
                      "launch_ms_cold_l2": force_ms_cold, "launch_ms_warm_l2": force_ms_warm},
-        "gpu_launches": args.steps * (md_steps * 8 + 1),
+        # per bench step: k_init_stats + per MD step k_kick_drift and the force kernel, + 6 kernels
+        # (4 cell list, copy back, neighbor list) in every rebuild that the graph's IF node ran
+        "gpu_launches": args.steps * (2 * md_steps + 1) + 6 * rebuilds,
     }
     if build_ms is not None:
         out["build_ms_per_rebuild"] = build_ms

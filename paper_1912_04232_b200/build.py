@@ -10,7 +10,7 @@ SRC = [os.path.join(HERE, "csrc", "md.cu")]
 DEPS = SRC + [os.path.join(HERE, "csrc", "md_kernels.cuh"),
               os.path.join(HERE, "csrc", "md_force32.cuh"),
               os.path.join(HERE, "csrc", "md_nbr2.cuh"), os.path.join(ROOT, "include", "md.h")]
-LIB = os.path.join(HERE, "libmd_b200.so")
+LIB = os.environ.get("MD_B200_LIB") or os.path.join(HERE, "libmd_b200.so")   # override: a variant build
 
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
@@ -35,7 +35,8 @@ def stale() -> bool:
 
 def build(force: bool = False, verbose: bool = False) -> str:
     if force or stale():
-        cmd = [nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SRC
+        extra = os.environ.get("MD_B200_NVCC_EXTRA", "").split()      # e.g. -DMD_F32_U=8 (tuning builds)
+        cmd = [nvcc()] + NVCC_FLAGS + extra + (["-Xptxas", "-v"] if verbose else []) + ["-o", LIB] + SRC
         subprocess.run(cmd, check=True)
     return LIB
 

@@ -105,7 +105,8 @@ k_cell_scan(int cells, int *__restrict__ cell_count, int *__restrict__ cell_star
     const int per = (cells + 1023) / 1024;
     const int c0 = min(tid * per, cells), c1 = min(c0 + per, cells);
     int sum = 0;
-    for (int c = c0; c < c1; ++c) sum += cell_count[c];
+#pragma unroll 8
+    for (int c = c0; c < c1; ++c) sum += cell_count[c];          // independent loads
     int x = sum;
 #pragma unroll
     for (int o = 1; o < 32; o <<= 1) {
@@ -125,6 +126,7 @@ k_cell_scan(int cells, int *__restrict__ cell_count, int *__restrict__ cell_star
     }
     __syncthreads();
     int run = x - sum + (wid ? warp_sum[wid - 1] : 0);           // exclusive prefix of my run
+#pragma unroll 4
     for (int c = c0; c < c1; ++c) {
         const int v = cell_count[c];
         cell_count[c] = 0;

@@ -16,9 +16,13 @@
 
 namespace mdk {
 
-constexpr int NB2_WARPS = 8;          // tiles per block
+#ifndef MD_NB2_WARPS
+#define MD_NB2_WARPS 4
+#endif
+constexpr int NB2_WARPS = MD_NB2_WARPS;   // tiles per block
 constexpr int NB2_WORDS = 40;         // mask words per lane per batch (1280 candidates)
 constexpr int NB2_CHUNK = 128;        // candidates staged per round (4 words)
+static_assert(NB2_WORDS <= 64, "two 32-bit masks of pending words per lane");
 
 struct Nb2Warp {                      // shared memory of one builder warp
     unsigned mask[NB2_WORDS][TILE];   // [word][lane]
@@ -39,7 +43,7 @@ __device__ __forceinline__ unsigned push4(unsigned m, float2 a, float2 b) {
 // already holds the pad value beyond its previous count, so only rows [count, previous count)
 // are re-padded; 0: rows [count, capacity) are written.
 template <int DIM, bool MAPPED>
-__global__ void __launch_bounds__(NB2_WARPS * 32, 4)
+__global__ void __launch_bounds__(NB2_WARPS * 32, 32 / NB2_WARPS)
 k_nbr_build2(Geom g, const float4 *__restrict__ spos, const int *__restrict__ cell_start,
              const int *__restrict__ map, int *__restrict__ nbr_idx, int *__restrict__ nbr_count,
              int *status, float4 *__restrict__ ref_pos, const int *cond, int incremental) {
@@ -94,26 +98,31 @@ k_nbr_build2(Geom g, const float4 *__restrict__ spos, const int *__restrict__ ce
                 if (cb >= ca) { t0 = cell_start[rowbase + ca]; t1 = cell_start[rowbase + cb + 1]; }
             }
             int nw = 0;                      // mask words of the current batch (warp-uniform)
-            // every lane pulls its next hit per iteration (moving on to its next mask word when the
-            // current one is used up): row k of the tile leaves as one 128-byte store
+            unsigned nzlo = 0u, nzhi = 0u;   // which of them are non-zero for this lane (words 0-31, 32-)
+            // every lane pulls its next hit per iteration (taking its next non-zero mask word when
+            // the current one is used up): row k of the tile leaves as one 128-byte store
             auto expand = [&]() {
                 __syncwarp();
-                const int nwl = inseg ? nw : 0;
+                unsigned plo = inseg ? nzlo : 0u, phi = inseg ? nzhi : 0u;   // words still to visit
                 unsigned word = 0u;
-                int w = -1;
+                int w = 0;
+                int *optr = outp + (size_t)min(cnt, cap) * TILE;
                 while (true) {
-                    const bool more = w + 1 < nwl;
-                    if (word == 0u && more) { ++w; word = W.mask[w][lane]; }
-                    if (!__any_sync(FULL, word != 0u || w + 1 < nwl)) break;
+                    if (word == 0u && (plo | phi)) {
+                        if (plo) { w = __ffs(plo) - 1; plo &= plo - 1u; }
+                        else { w = 31 + __ffs(phi); phi &= phi - 1u; }
+                        word = W.mask[w][lane];
+                    }
+                    if (!__any_sync(FULL, word != 0u)) break;
                     const int bit = __clz(word);                 // 32 when word == 0
-                    const int slot = W.wbase[max(w, 0)] + bit;
+                    const int slot = W.wbase[w] + bit;
                     const bool hit = word != 0u && slot != s;
                     word &= 0x7fffffffu >> (bit & 31);           // drop that bit (all above it are 0)
-                    if (hit && cnt < cap) outp[cnt * TILE] = MAPPED ? map[slot] : slot;
+                    if (hit && cnt < cap) { *optr = MAPPED ? map[slot] : slot; optr += TILE; }
                     cnt += hit ? 1 : 0;
                 }
                 __syncwarp();
-                nw = 0;
+                nw = 0; nzlo = 0u; nzhi = 0u;
             };
 
             // ---- walk the pieces; the next chunk is loaded while the current one is tested
@@ -206,6 +215,8 @@ k_nbr_build2(Geom g, const float4 *__restrict__ spos, const int *__restrict__ ce
                         hi <<= 32 - 4 * ng;
                     }
                     W.mask[nw][lane] = hi;
+                    if (nw < 32) nzlo |= (hi != 0u ? 1u : 0u) << nw;
+                    else nzhi |= (hi != 0u ? 1u : 0u) << (nw - 32);
                     ++nw;
                 }
                 __syncwarp();
