@@ -187,9 +187,11 @@ int md_nve_step(md_system *sys, const md_potential *pot, void *pos, void *vel, v
                 int nsteps, int32_t *stats, void *stream);
 
 /*
- * End-to-end convenience over HOST buffers: allocates device memory, copies pos/vel in,
- * builds the lists, evaluates F, runs nsteps of md_nve_step, copies the state back
- * un-permuted (original particle order) and frees.  Synchronous.
+ * End-to-end convenience over HOST buffers: copies pos/vel in, builds the lists, evaluates F,
+ * runs nsteps of md_nve_step and copies the state back un-permuted (original particle order).
+ * Synchronous.  The device allocation, the system and its step graphs are kept for the next call
+ * with the same (cfg, n, current device) -- one context per process, replaced when they differ,
+ * dropped on any error and by md_nve_run_host_release(); calls are serialised by a mutex.
  *   pos_host, vel_host   host float4[n] in/out
  *   force_host           host float4[n] out (may be NULL)
  *   energy_host          host double out (may be NULL): potential energy of the final state
@@ -198,6 +200,9 @@ int md_nve_step(md_system *sys, const md_potential *pot, void *pos, void *vel, v
 int md_nve_run_host(const md_config *cfg, const md_potential *pot, int n, void *pos_host,
                     void *vel_host, void *force_host, double *energy_host, float dt,
                     float mass, int nsteps, int32_t *stats_host);
+
+/* Frees the context md_nve_run_host keeps between calls (no-op if there is none). */
+int md_nve_run_host_release(void);
 
 #ifdef __cplusplus
 }

@@ -21,6 +21,7 @@ SYMBOLS = [
     "md_last_error", "md_workspace_bytes", "md_create", "md_destroy", "md_set_option",
     "md_num_cells", "md_nbr_layout", "md_cell_list_build", "md_neighbor_list_build",
     "md_needs_rebuild", "md_pair_energy_force", "md_nve_step", "md_nve_run_host", "md_counters",
+    "md_nve_run_host_release",
 ]
 
 
@@ -138,6 +139,10 @@ def md_destroy(sys) -> None:
 
 def md_set_option(sys, name: str, value: float) -> None:
     _check(lib().md_set_option(sys, name.encode(), float(value)))
+
+
+def md_nve_run_host_release() -> None:
+    _check(lib().md_nve_run_host_release())
 
 
 def md_counters(sys, out, reset=False, stream=None) -> None:

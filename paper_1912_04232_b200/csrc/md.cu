@@ -11,6 +11,7 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <mutex>
 #include <new>
 
 using namespace mdk;
@@ -638,6 +639,39 @@ int md_nve_step(md_system *sys, const md_potential *pot, void *pos, void *vel, v
     return MD_OK;
 }
 
+// md_nve_run_host keeps ONE context (device allocation, system, stream, and through the system the
+// captured step graphs) for the last (cfg, n, device) it was called with, so that a caller who
+// streams states through it does not pay cudaMalloc / md_create / graph instantiation per call.
+struct HostCtx {
+    bool valid;
+    md_config cfg;
+    int n, device;
+    char *d;
+    size_t o_pos, o_vel, o_force, o_pos2, o_vel2, o_force2, o_id, o_cnt, o_list, o_small, o_ws;
+    md_system *sys;
+    cudaStream_t st;
+};
+static HostCtx g_host = {};
+static std::mutex g_host_mutex;
+
+static void host_ctx_drop() {
+    if (!g_host.valid) return;
+    int cur = -1;
+    cudaGetDevice(&cur);
+    if (cur != g_host.device) cudaSetDevice(g_host.device);
+    if (g_host.sys) md_destroy(g_host.sys);
+    if (g_host.st) cudaStreamDestroy(g_host.st);
+    if (g_host.d) cudaFree(g_host.d);
+    if (cur >= 0 && cur != g_host.device) cudaSetDevice(cur);
+    memset(&g_host, 0, sizeof(g_host));
+}
+
+int md_nve_run_host_release(void) {
+    std::lock_guard<std::mutex> lock(g_host_mutex);
+    host_ctx_drop();
+    return MD_OK;
+}
+
 int md_nve_run_host(const md_config *cfg, const md_potential *pot, int n, void *pos_host,
                     void *vel_host, void *force_host, double *energy_host, float dt, float mass,
                     int nsteps, int32_t *stats_host) {
@@ -645,27 +679,36 @@ int md_nve_run_host(const md_config *cfg, const md_potential *pot, int n, void *
     size_t wsb = 0;
     int rc = md_workspace_bytes(cfg, n, &wsb);
     if (rc) return rc;
+    std::lock_guard<std::mutex> lock(g_host_mutex);
+    int dev = 0;
+    CU(cudaGetDevice(&dev));
+    HostCtx &h = g_host;
     const size_t vec = (size_t)n * sizeof(float4);
-    const size_t list = (size_t)((n + TILE - 1) / TILE) * TILE * cfg->capacity * sizeof(int);
-    // one allocation: pos, vel, force, out x3, id, count, list, small words, workspace
-    size_t o = 0;
-    auto take = [&](size_t b) { size_t at = o; o += up(b); return at; };
-    const size_t o_pos = take(vec), o_vel = take(vec), o_force = take(vec), o_pos2 = take(vec),
-                 o_vel2 = take(vec), o_force2 = take(vec), o_id = take((size_t)n * 4),
-                 o_cnt = take((size_t)n * 4), o_list = take(list), o_small = take(256),
-                 o_ws = take(wsb);
-    char *d = nullptr;
-    CU(cudaMalloc(&d, o));
-    md_system *sys = nullptr;
-    cudaStream_t st = nullptr;
-    rc = md_create(cfg, n, d + o_ws, wsb, &sys);
-    auto done = [&](int code) { if (sys) md_destroy(sys); if (st) cudaStreamDestroy(st); cudaFree(d); return code; };
-    if (rc) return done(rc);
-    cudaError_t e = cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking);
-    if (e != cudaSuccess) return done(fail(MD_ECUDA, "cudaStreamCreate: %s", cudaGetErrorString(e)));
-    float4 *pos = (float4 *)(d + o_pos), *vel = (float4 *)(d + o_vel), *force = (float4 *)(d + o_force);
-    int *id = (int *)(d + o_id), *cnt = (int *)(d + o_cnt), *nbr = (int *)(d + o_list);
-    int *small = (int *)(d + o_small);          // [0..1] status, [4..7] stats, [8..9] energy (double)
+    if (!(h.valid && h.n == n && h.device == dev && memcmp(&h.cfg, cfg, sizeof(*cfg)) == 0)) {
+        host_ctx_drop();
+        const size_t list = (size_t)((n + TILE - 1) / TILE) * TILE * cfg->capacity * sizeof(int);
+        // one allocation: pos, vel, force, out x3, id, count, list, small words, workspace
+        size_t o = 0;
+        auto take = [&](size_t b) { size_t at = o; o += up(b); return at; };
+        h.o_pos = take(vec); h.o_vel = take(vec); h.o_force = take(vec); h.o_pos2 = take(vec);
+        h.o_vel2 = take(vec); h.o_force2 = take(vec); h.o_id = take((size_t)n * 4);
+        h.o_cnt = take((size_t)n * 4); h.o_list = take(list); h.o_small = take(256);
+        h.o_ws = take(wsb);
+        CU(cudaMalloc(&h.d, o));
+        h.valid = true; h.cfg = *cfg; h.n = n; h.device = dev;      // from here host_ctx_drop frees it
+        rc = md_create(cfg, n, h.d + h.o_ws, wsb, &h.sys);
+        if (rc) { host_ctx_drop(); return rc; }
+        cudaError_t e0 = cudaStreamCreateWithFlags(&h.st, cudaStreamNonBlocking);
+        if (e0 != cudaSuccess) { host_ctx_drop(); return fail(MD_ECUDA, "cudaStreamCreate: %s", cudaGetErrorString(e0)); }
+    }
+    char *d = h.d;
+    md_system *sys = h.sys;
+    cudaStream_t st = h.st;
+    cudaError_t e;
+    auto done = [&](int code) { if (code != MD_OK) host_ctx_drop(); return code; };
+    float4 *pos = (float4 *)(d + h.o_pos), *vel = (float4 *)(d + h.o_vel), *force = (float4 *)(d + h.o_force);
+    int *id = (int *)(d + h.o_id), *cnt = (int *)(d + h.o_cnt), *nbr = (int *)(d + h.o_list);
+    int *small = (int *)(d + h.o_small);        // [0..1] status, [4..7] stats, [8..9] energy (double)
     double *etot = (double *)(small + 8);
 #define RUN(x) do { e = (x); if (e != cudaSuccess) return done(fail(MD_ECUDA, "%s: %s", #x, cudaGetErrorString(e))); } while (0)
 #define STEP(x) do { rc = (x); if (rc) return done(rc); } while (0)
@@ -677,18 +720,18 @@ int md_nve_run_host(const md_config *cfg, const md_potential *pot, int n, void *
     STEP(md_pair_energy_force(sys, pot, pos, nbr, cnt, force, nullptr, st));
     STEP(md_nve_step(sys, pot, pos, vel, force, id, nbr, cnt, dt, mass, nsteps, small + 4, st));
     if (energy_host) STEP(md_pair_energy_force(sys, pot, pos, nbr, cnt, force, etot, st));
-    k_unpermute<<<blocks_for(n), 256, 0, st>>>(n, id, pos, vel, force, (float4 *)(d + o_pos2),
-                                               (float4 *)(d + o_vel2), (float4 *)(d + o_force2));
+    k_unpermute<<<blocks_for(n), 256, 0, st>>>(n, id, pos, vel, force, (float4 *)(d + h.o_pos2),
+                                               (float4 *)(d + h.o_vel2), (float4 *)(d + h.o_force2));
     RUN(cudaGetLastError());
-    RUN(cudaMemcpyAsync(pos_host, d + o_pos2, vec, cudaMemcpyDeviceToHost, st));
-    RUN(cudaMemcpyAsync(vel_host, d + o_vel2, vec, cudaMemcpyDeviceToHost, st));
-    if (force_host) RUN(cudaMemcpyAsync(force_host, d + o_force2, vec, cudaMemcpyDeviceToHost, st));
+    RUN(cudaMemcpyAsync(pos_host, d + h.o_pos2, vec, cudaMemcpyDeviceToHost, st));
+    RUN(cudaMemcpyAsync(vel_host, d + h.o_vel2, vec, cudaMemcpyDeviceToHost, st));
+    if (force_host) RUN(cudaMemcpyAsync(force_host, d + h.o_force2, vec, cudaMemcpyDeviceToHost, st));
     if (energy_host) RUN(cudaMemcpyAsync(energy_host, etot, sizeof(double), cudaMemcpyDeviceToHost, st));
     if (stats_host) RUN(cudaMemcpyAsync(stats_host, small + 4, 4 * sizeof(int), cudaMemcpyDeviceToHost, st));
     RUN(cudaStreamSynchronize(st));
 #undef RUN
 #undef STEP
-    return done(MD_OK);
+    return MD_OK;
 }
 
 } // extern "C"

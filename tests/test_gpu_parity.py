@@ -365,6 +365,31 @@ def test_nve_run_host_matches_device_path(B, W):
     S.close()
 
 
+def test_nve_run_host_context_reuse(B, W):
+    """md_nve_run_host keeps its device context between calls: a second call with the same
+    (cfg, n) must give the same bits, a call with another system must replace the context, and
+    going back must again give the first result."""
+    w0, w2 = W.config(0), W.lj_fcc(0, 7, seed=7)
+
+    def run(w):
+        cfg = B.make_config(w.dim, w.box, w.r_cut, w.skin, w.capacity, w.resort)
+        pot = B.make_potential(w.kind, w.epsilon, w.sigma, w.r_cut, w.shift)
+        pos = w.pos.copy(); vel = w.vel.copy(); force = np.zeros_like(pos)
+        stats = np.zeros(4, np.int32)
+        E = B.md_nve_run_host(cfg, pot, pos, vel, force, w.dt, w.mass, 30, stats)
+        return pos, vel, force, E, stats
+
+    a = run(w0); b = run(w0); c = run(w2); d = run(w0)
+    for x, y in ((a, b), (a, d)):
+        assert all(np.array_equal(p, q) for p, q in zip(x[:3], y[:3])) and np.array_equal(x[4], y[4])
+        assert abs(x[3] - y[3]) <= 1e-12 * abs(x[3])
+    assert c[0].shape[0] == w2.n and np.isfinite(c[0]).all() and c[4][0] == 30
+    B.md_nve_run_host_release()
+    B.md_nve_run_host_release()          # idempotent
+    e = run(w0)
+    assert all(np.array_equal(p, q) for p, q in zip(a[:3], e[:3]))
+
+
 def snapshot_checks(B, orc, W, w, steps, method=1):
     """State-wise parity along a trajectory (SURVEY §8c last row of P): run on the GPU, then
     hand the GPU snapshot to the oracle and compare list / force / energy at that state; plus
