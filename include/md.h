@@ -90,6 +90,9 @@ int md_destroy(md_system *sys);
  *   "threads_per_particle" fp64 force kernel variant: 0 = streaming kernel (one lane per particle,
  *                          list rows staged through shared memory by TMA; default for
  *                          n >= 32768), or 1, 2, 4 lanes sharing one particle (default 4 below)
+ *   "fused"                1 (default): inside md_nve_step's graph the 3-D LJ force kernel also opens
+ *                          the next step (second half-kick, first half-kick, drift into a second
+ *                          position buffer, half-skin test); 0: k_kick_drift every step.  Same bits.
  *   "builder"              neighbor-list kernel: 2 (default) records hits in per-lane bit masks,
  *                          1 appends them to per-lane shared-memory columns (first design)
  *   "use_graph"            0: md_nve_step launches kernels directly instead of a CUDA graph */

@@ -53,7 +53,7 @@ struct StepKey {
     const void *pos, *vel, *force, *id, *nbr_idx, *nbr_count, *stats;
     float dt, mass;
     md_potential pot;
-    int tpp, fast32, builder;
+    int tpp, fast32, builder, fused;
     float est_thr;
 };
 
@@ -67,14 +67,16 @@ struct md_system {
     char *ws;
     size_t ws_bytes;
     // workspace slices
-    int *words;          // [0] rebuild flag, [1..2] internal status, [8..] spare
+    int *words;          // [0] rebuild flag (even steps of a fused graph), [1..2] internal status,
+                         // [3] rebuild flag (odd steps), [8..15] counters
     int *cell_count, *cell_start_i, *perm_i, *cell_of, *rank_tmp, *perm_tmp, *id_s;
-    float4 *pos_s, *vel_s, *ref_pos;
+    float4 *pos_s, *vel_s, *ref_pos, *pos_alt;   // pos_alt: second position buffer of the fused step
     // tuning
     int tpp;             // lanes per particle in the force kernel (1, 2, 4)
     int nb_warps;        // tiles per block in the neighbor-list builder
     size_t nb_smem;      // its dynamic shared memory per block
     int use_graph;
+    int fused;           // fused step: the force kernel also opens the next step (graph mode, fast32)
     int builder;         // neighbor-list builder: 2 = bit-mask (md_nbr2.cuh), 1 = column append
     int fast32;          // LJ 3-D: fp32 fast path + fp64 re-evaluation (md_force32.cuh)
     float est_thr;       // its error-estimate threshold
@@ -99,7 +101,7 @@ int enter(const md_system *s) {
 
 struct Layout {
     size_t words, cell_count, cell_start_i, perm_i, cell_of, rank_tmp, perm_tmp, id_s, pos_s,
-        vel_s, ref_pos, total;
+        vel_s, ref_pos, pos_alt, total;
 };
 
 Layout layout(int n, long long cells) {
@@ -117,6 +119,7 @@ Layout layout(int n, long long cells) {
     l.pos_s = take((size_t)n * sizeof(float4));
     l.vel_s = take((size_t)n * sizeof(float4));
     l.ref_pos = take((size_t)n * sizeof(float4));
+    l.pos_alt = take((size_t)n * sizeof(float4));
     l.total = o;
     return l;
 }
@@ -263,7 +266,7 @@ int launch_force_t(md_system *s, const Pair &pp, const float4 *pos, const int *n
 // does not need it and skips those fp64 operations (force.w = 0 there).
 int launch_force(md_system *s, const Pair &pp, const float4 *pos, const int *nbr_idx,
                  const int *nbr_count, float4 *force, float4 *vel, float a, double *etot,
-                 bool want_energy, Book book, cudaStream_t st) {
+                 bool want_energy, Book book, cudaStream_t st, NextStep nx = NextStep()) {
     if (s->fast32 && pp.kind == MD_KIND_LJ && s->g.dim == 3) {
         Pair32 q;
         q.rc2 = (float)pp.drc2;
@@ -275,8 +278,8 @@ int launch_force(md_system *s, const Pair &pp, const float4 *pos, const int *nbr
         q.est_thr = s->est_thr;
         const int nb = blocks_for(s->g.n, F32_WARPS * 32);
         int *nfix = s->words + 8;
-        if (want_energy) k_force_lj32<true><<<nb, F32_WARPS * 32, 0, st>>>(s->g, pp, q, pos, nbr_idx, nbr_count, force, vel, a, etot, book, nfix);
-        else k_force_lj32<false><<<nb, F32_WARPS * 32, 0, st>>>(s->g, pp, q, pos, nbr_idx, nbr_count, force, vel, a, etot, book, nfix);
+        if (want_energy) k_force_lj32<true><<<nb, F32_WARPS * 32, 0, st>>>(s->g, pp, q, pos, nbr_idx, nbr_count, force, vel, a, etot, book, nfix, nx);
+        else k_force_lj32<false><<<nb, F32_WARPS * 32, 0, st>>>(s->g, pp, q, pos, nbr_idx, nbr_count, force, vel, a, etot, book, nfix, nx);
         LAUNCH_OK();
         return MD_OK;
     }
@@ -290,9 +293,9 @@ int launch_force(md_system *s, const Pair &pp, const float4 *pos, const int *nbr
 #undef MD_FORCE_DISPATCH
 }
 
-__global__ void k_init_stats(int *stats, int *flag) {
+__global__ void k_init_stats(int *stats, int *words) {
     stats[0] = 0; stats[1] = 0; stats[2] = -1; stats[3] = 0;
-    *flag = 0;
+    words[0] = 0; words[3] = 0;          // rebuild flags
 }
 
 __global__ void k_unpermute(int n, const int *__restrict__ id, const float4 *__restrict__ a,
@@ -369,6 +372,76 @@ int record_step(md_system *s, const Pair &pp, float4 *pos, float4 *vel, float4 *
     return launch_force(s, pp, pos, nbr_idx, nbr_count, force, vel, a, nullptr, false, book, st);
 }
 
+// Adds an IF node (condition `cond`) after the current capture front of `st` whose body is the
+// rebuild (cell list + re-sort + neighbor list) of the state held in `pos`; `st` continues after it.
+int record_rebuild_if(md_system *s, cudaStream_t st, cudaGraphConditionalHandle cond, float4 *pos,
+                      float4 *vel, int *id, int *nbr_idx, int *nbr_count) {
+    int *status = s->words + 1;
+    const bool resort = s->cfg.resort != 0;
+    cudaStreamCaptureStatus cs;
+    cudaGraph_t graph = nullptr;
+    const cudaGraphNode_t *deps = nullptr;
+    size_t ndeps = 0;
+    CU(cudaStreamGetCaptureInfo(st, &cs, nullptr, &graph, &deps, &ndeps));
+    if (cs != cudaStreamCaptureStatusActive || !graph) return fail(MD_ECUDA, "stream is not capturing");
+    cudaGraphNodeParams np = {cudaGraphNodeTypeConditional};
+    np.type = cudaGraphNodeTypeConditional;
+    np.conditional.handle = cond;
+    np.conditional.type = cudaGraphCondTypeIf;
+    np.conditional.size = 1;
+    cudaGraphNode_t node;
+    CU(cudaGraphAddNode(&node, graph, deps, ndeps, &np));
+    cudaGraph_t body = np.conditional.phGraph_out[0];
+    if (!s->body_stream) CU(cudaStreamCreateWithFlags(&s->body_stream, cudaStreamNonBlocking));
+    CU(cudaStreamBeginCaptureToGraph(s->body_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal));
+    int rc = launch_cell_build(s, pos, vel, id, s->cell_start_i, s->perm_i, status, nullptr, s->body_stream);
+    if (!rc) rc = launch_nbr_build(s, resort ? pos : s->pos_s, s->cell_start_i, resort ? nullptr : s->perm_i,
+                                   nbr_idx, nbr_count, status, nullptr, 1, s->body_stream);
+    cudaGraph_t ended = nullptr;
+    cudaError_t e = cudaStreamEndCapture(s->body_stream, &ended);
+    if (rc) return rc;
+    if (e != cudaSuccess) return fail(MD_ECUDA, "capturing the rebuild body: %s", cudaGetErrorString(e));
+    CU(cudaStreamUpdateCaptureDependencies(st, &node, 1, cudaStreamSetCaptureDependencies));
+    return MD_OK;
+}
+
+// `reps` fused steps on the capturing stream `st` (3-D LJ fast path): one k_kick_drift opens the
+// first step, every force kernel but the last also opens the next step and writes the drifted
+// positions to the other buffer (pos <-> pos_alt); reps is 1 or odd, so the state ends in `pos`.
+int record_fused(md_system *s, const Pair &pp, float4 *pos, float4 *vel, float4 *force, int *id,
+                 int *nbr_idx, int *nbr_count, float dt, float mass, int *stats, int reps,
+                 cudaStream_t st) {
+    const Geom &g = s->g;
+    const float a = dt / (2.0f * mass);
+    int *flags[2] = {s->words + 0, s->words + 3};
+    int *status = s->words + 1;
+    cudaStreamCaptureStatus cs;
+    cudaGraph_t graph = nullptr;
+    CU(cudaStreamGetCaptureInfo(st, &cs, nullptr, &graph, nullptr, nullptr));
+    if (cs != cudaStreamCaptureStatusActive || !graph) return fail(MD_ECUDA, "stream is not capturing");
+    cudaGraphConditionalHandle cond;
+    CU(cudaGraphConditionalHandleCreate(&cond, graph, 0, cudaGraphCondAssignDefault));
+    k_kick_drift<3, true><<<blocks_for(g.n), 256, 0, st>>>(g, pos, vel, force, s->ref_pos, a, dt, flags[0], cond);
+    LAUNCH_OK();
+    float4 *cur = pos, *other = s->pos_alt;
+    for (int r = 0; r < reps; ++r) {
+        int rc = record_rebuild_if(s, st, cond, cur, vel, id, nbr_idx, nbr_count);
+        if (rc) return rc;
+        Book book = {flags[r & 1], status, stats};
+        NextStep nx = NextStep();
+        if (r + 1 < reps) {
+            CU(cudaGraphConditionalHandleCreate(&cond, graph, 0, cudaGraphCondAssignDefault));
+            nx.pos_out = other; nx.ref = s->ref_pos; nx.dt = dt; nx.flag = flags[(r + 1) & 1];
+            nx.cond = cond; nx.has_cond = 1;
+        }
+        rc = launch_force(s, pp, cur, nbr_idx, nbr_count, force, vel, a, nullptr, false, book, st, nx);
+        if (rc) return rc;
+        if (r + 1 < reps) std::swap(cur, other);
+    }
+    if (cur != pos) return fail(MD_EINVAL, "fused graph of %d steps does not end in the caller's buffer", reps);
+    return MD_OK;
+}
+
 void drop_graphs(md_system *s) {
     if (s->exec1) cudaGraphExecDestroy(s->exec1);
     if (s->execU) cudaGraphExecDestroy(s->execU);
@@ -380,10 +453,15 @@ int capture(md_system *s, const Pair &pp, const StepKey &k, int reps, cudaGraphE
     if (!s->cap_stream) CU(cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking));
     CU(cudaStreamBeginCapture(s->cap_stream, cudaStreamCaptureModeThreadLocal));
     int rc = MD_OK;
-    for (int r = 0; r < reps && rc == MD_OK; ++r)
-        rc = record_step(s, pp, (float4 *)k.pos, (float4 *)k.vel, (float4 *)k.force, (int *)k.id,
-                         (int *)k.nbr_idx, (int *)k.nbr_count, k.dt, k.mass, (int *)k.stats,
-                         s->cap_stream, true);
+    if (s->fast32 && s->fused && pp.kind == MD_KIND_LJ && s->g.dim == 3 && (reps & 1))
+        rc = record_fused(s, pp, (float4 *)k.pos, (float4 *)k.vel, (float4 *)k.force, (int *)k.id,
+                          (int *)k.nbr_idx, (int *)k.nbr_count, k.dt, k.mass, (int *)k.stats, reps,
+                          s->cap_stream);
+    else
+        for (int r = 0; r < reps && rc == MD_OK; ++r)
+            rc = record_step(s, pp, (float4 *)k.pos, (float4 *)k.vel, (float4 *)k.force, (int *)k.id,
+                             (int *)k.nbr_idx, (int *)k.nbr_count, k.dt, k.mass, (int *)k.stats,
+                             s->cap_stream, true);
     cudaGraph_t graph = nullptr;
     cudaError_t e = cudaStreamEndCapture(s->cap_stream, &graph);
     if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
@@ -441,12 +519,14 @@ int md_create(const md_config *cfg, int n, void *workspace, size_t bytes, md_sys
     s->pos_s = (float4 *)(s->ws + l.pos_s);
     s->vel_s = (float4 *)(s->ws + l.vel_s);
     s->ref_pos = (float4 *)(s->ws + l.ref_pos);
+    s->pos_alt = (float4 *)(s->ws + l.pos_alt);
     s->tpp = n >= 32768 ? 0 : 4;     // 0 = streaming kernel; small systems: 4 lanes per particle
     s->use_graph = 1;
     s->fast32 = 1;
     s->builder = 2;
+    s->fused = 1;
     s->est_thr = 8.0f;
-    s->unroll = 8;
+    s->unroll = 9;      // odd: a fused graph swaps position buffers steps-1 times and must end in the caller's
     if (const char *e = getenv("MD_B200_TPP")) { int t = atoi(e); if (t == 0 || t == 1 || t == 2 || t == 4) s->tpp = t; }
     if (const char *e = getenv("MD_B200_NO_GRAPH")) s->use_graph = atoi(e) ? 0 : 1;
     {   // neighbor-list builder: one warp per tile, a capacity x 32 column block + a candidate
@@ -524,6 +604,7 @@ int md_set_option(md_system *sys, const char *name, double value) {
         sys->tpp = t;
     } else if (!strcmp(name, "use_graph")) sys->use_graph = value != 0.0;
     else if (!strcmp(name, "fast32")) sys->fast32 = value != 0.0;
+    else if (!strcmp(name, "fused")) sys->fused = value != 0.0;
     else if (!strcmp(name, "builder")) {
         if (value != 1.0 && value != 2.0) return fail(MD_EINVAL, "builder must be 1 or 2");
         sys->builder = (int)value;
@@ -620,7 +701,7 @@ int md_nve_step(md_system *sys, const md_potential *pot, void *pos, void *vel, v
     memset(&k, 0, sizeof(k));
     k.pos = pos; k.vel = vel; k.force = force; k.id = id; k.nbr_idx = nbr_idx;
     k.nbr_count = nbr_count; k.stats = stats; k.dt = dt; k.mass = mass; k.pot = *pot;
-    k.tpp = sys->tpp; k.fast32 = sys->fast32; k.builder = sys->builder; k.est_thr = sys->est_thr;
+    k.tpp = sys->tpp; k.fast32 = sys->fast32; k.builder = sys->builder; k.fused = sys->fused; k.est_thr = sys->est_thr;
     if (!sys->key_valid || memcmp(&k, &sys->key, sizeof(k)) != 0) {
         drop_graphs(sys);
         sys->key = k;

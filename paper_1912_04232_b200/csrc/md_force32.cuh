@@ -153,12 +153,25 @@ __device__ __forceinline__ void lj_rows32(const Geom &g, const Pair32 &p32,
 // vel != NULL: also the second half-kick v += a F.  energy_total != NULL (ENERGY only): adds
 // sum_i e_i in fp64.  book.stats != NULL: per-step bookkeeping.  nfix (may be NULL): counts
 // re-evaluated particles (diagnostics).
+// Fused step (nx.pos_out != NULL, inside md_nve_step's graph): the epilogue also opens the NEXT
+// step -- v += a F again (its first half-kick), r = mu(r, dt v) written to the other position
+// buffer (other warps still gather from this one), half-skin test against the reference
+// positions, raising nx.flag and the graph condition of the next step's rebuild node.  The
+// arithmetic and its order are those of k_kick_drift, so fused and unfused runs agree bit for bit.
+struct NextStep {
+    float4 *pos_out;            // NULL: plain force kernel
+    const float4 *ref;          // positions at the last list build
+    float dt;
+    int *flag;                  // rebuild-needed word of the next step
+    cudaGraphConditionalHandle cond;
+    int has_cond;
+};
 template <bool ENERGY>
 __global__ void __launch_bounds__(F32_WARPS * 32)
 k_force_lj32(Geom g, Pair pp, Pair32 p32, const float4 *__restrict__ pos,
              const int *__restrict__ nbr_idx, const int *__restrict__ nbr_count,
              float4 *__restrict__ force, float4 *__restrict__ vel, float a, double *energy_total,
-             Book book, int *nfix) {
+             Book book, int *nfix, NextStep nx) {
     const int lane = threadIdx.x & 31;
     const int gid = blockIdx.x * blockDim.x + threadIdx.x;
     const int i = gid;
@@ -226,13 +239,27 @@ k_force_lj32(Geom g, Pair pp, Pair32 p32, const float4 *__restrict__ pos,
     }
 
     // ---- store, second half-kick, energy reduction, bookkeeping
+    bool moved = false;
     if (active) {
         force[i] = make_float4(fx, fy, fz, (float)e64);
         if (vel) {
             float4 v = vel[i];
             v.x = fmaf(a, fx, v.x); v.y = fmaf(a, fy, v.y); v.z = fmaf(a, fz, v.z);
+            if (nx.pos_out) {
+                v.x = fmaf(a, fx, v.x); v.y = fmaf(a, fy, v.y); v.z = fmaf(a, fz, v.z);
+                float4 p = pi;
+                p.x = wrap(fmaf(nx.dt, v.x, p.x), g.L[0], g.inv_L[0]);
+                p.y = wrap(fmaf(nx.dt, v.y, p.y), g.L[1], g.inv_L[1]);
+                p.z = wrap(fmaf(nx.dt, v.z, p.z), g.L[2], g.inv_L[2]);
+                nx.pos_out[i] = p;
+                moved = disp2_from_ref<3>(g, p, nx.ref[i]) > g.half_skin2;
+            }
             vel[i] = v;
         }
+    }
+    if (nx.pos_out && __any_sync(FULL, moved) && lane == 0) {
+        *nx.flag = 1;
+        if (nx.has_cond) cudaGraphSetConditional(nx.cond, 1);
     }
     if (ENERGY && energy_total) {
         __shared__ double red[F32_WARPS];

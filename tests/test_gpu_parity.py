@@ -365,6 +365,27 @@ def test_nve_run_host_matches_device_path(B, W):
     S.close()
 
 
+@pytest.mark.parametrize("ci,steps", [(0, 100), (2, 120)])
+def test_fused_step_same_bits(B, W, ci, steps):
+    """The fused graph (force kernel opens the next step, positions ping-pong between two buffers)
+    and the plain sequence k_kick_drift -> rebuild -> force give the same bits and the same
+    rebuild history, for step counts that exercise both the 9-step and the 1-step graph."""
+    w = W.config(ci)
+    out = []
+    for fused, graph in ((1, 1), (0, 1), (0, 0)):
+        S = B.System(w)
+        B.md_set_option(S.sys, "fused", fused)
+        B.md_set_option(S.sys, "use_graph", graph)
+        S.build(); S.compute_force(); S.step(steps)
+        torch.cuda.synchronize()
+        out.append((S.pos.clone(), S.vel.clone(), S.force.clone(), S.id.clone(), S.stats.clone()))
+        S.close()
+    for o in out[1:]:
+        for x, y in zip(out[0], o):
+            assert torch.equal(x, y)
+    assert int(out[0][4][0]) == steps and int(out[0][4][1]) >= 5
+
+
 def test_nve_run_host_context_reuse(B, W):
     """md_nve_run_host keeps its device context between calls: a second call with the same
     (cfg, n) must give the same bits, a call with another system must replace the context, and
