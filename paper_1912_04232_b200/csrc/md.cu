@@ -69,6 +69,7 @@ struct md_system {
     // workspace slices
     int *words;          // [0] rebuild flag (even steps of a fused graph), [1..2] internal status,
                          // [3] rebuild flag (odd steps), [8..15] counters
+    int *scan_tmp;       // block sums + ticket of the two-launch cell scan
     int *cell_count, *cell_start_i, *perm_i, *cell_of, *rank_tmp, *perm_tmp, *id_s;
     float4 *pos_s, *vel_s, *ref_pos, *pos_alt;   // pos_alt: second position buffer of the fused step
     // tuning
@@ -100,7 +101,7 @@ int enter(const md_system *s) {
 }
 
 struct Layout {
-    size_t words, cell_count, cell_start_i, perm_i, cell_of, rank_tmp, perm_tmp, id_s, pos_s,
+    size_t words, scan_tmp, cell_count, cell_start_i, perm_i, cell_of, rank_tmp, perm_tmp, id_s, pos_s,
         vel_s, ref_pos, pos_alt, total;
 };
 
@@ -109,7 +110,8 @@ Layout layout(int n, long long cells) {
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t at = o; o += up(bytes); return at; };
     l.words = take(64 * sizeof(int));
-    l.cell_count = take((size_t)(cells + 1) * sizeof(int));
+    l.scan_tmp = take((size_t)((cells + SCAN_CHUNK - 1) / SCAN_CHUNK + 2) * sizeof(int));
+    l.cell_count = take((size_t)(cells + 4) * sizeof(int));
     l.cell_start_i = take((size_t)(cells + 1) * sizeof(int));
     l.perm_i = take((size_t)n * sizeof(int));
     l.cell_of = take((size_t)n * sizeof(int));
@@ -188,8 +190,16 @@ int launch_cell_build(md_system *s, float4 *pos, float4 *vel, int *id, int *cell
     const bool resort = s->cfg.resort != 0;
     k_cell_assign<<<nb, 256, 0, st>>>(g, pos, s->cell_of, s->rank_tmp, s->cell_count, cond);
     LAUNCH_OK();
-    k_cell_scan<<<1, 1024, 0, st>>>(g.cells, s->cell_count, cell_start, status, cond);
-    LAUNCH_OK();
+    if (g.cells <= SCAN_ONE_BLOCK) {
+        k_cell_scan<<<1, 1024, 0, st>>>(g.cells, s->cell_count, cell_start, status, cond);
+        LAUNCH_OK();
+    } else {
+        const int nbs = (g.cells + SCAN_CHUNK - 1) / SCAN_CHUNK;
+        k_cell_sum<<<nbs, 1024, 0, st>>>(g.cells, s->cell_count, s->scan_tmp, s->scan_tmp + nbs + 1, status, cond);
+        LAUNCH_OK();
+        k_cell_scan2<<<nbs, 1024, 0, st>>>(g.cells, s->cell_count, cell_start, s->scan_tmp, cond);
+        LAUNCH_OK();
+    }
     k_cell_scatter<<<nb, 256, 0, st>>>(g.n, s->cell_of, s->rank_tmp, cell_start, s->perm_tmp, cond);
     LAUNCH_OK();
     k_cell_order_gather<<<nb, 256, 0, st>>>(g.n, s->cell_of, cell_start, s->perm_tmp, id, pos,
@@ -509,6 +519,7 @@ int md_create(const md_config *cfg, int n, void *workspace, size_t bytes, md_sys
     s->cfg = *cfg; s->n = n; s->g = g; s->device = attr.device;
     s->ws = (char *)workspace; s->ws_bytes = bytes;
     s->words = (int *)(s->ws + l.words);
+    s->scan_tmp = (int *)(s->ws + l.scan_tmp);
     s->cell_count = (int *)(s->ws + l.cell_count);
     s->cell_start_i = (int *)(s->ws + l.cell_start_i);
     s->perm_i = (int *)(s->ws + l.perm_i);

@@ -8,7 +8,10 @@
 // everywhere but is bound by the conversion / reciprocal unit (3 F2F + 1 RCP64H per pair).
 // Here every pair is evaluated in fp32 first -- displacement by the canonical nearest-image
 // form (one rounding), r2 = fma(dz,dz,fma(dy,dy,dx*dx)), y = 1/r2 (MUFU), force
-// coefficient 24 eps sig^6 y^4 (2 sig^6 y^3 - 1) -- together with S_i = sum_j |coefficient|.
+// coefficient 24 eps sig^6 y^4 (2 sig^6 y^3 - 1) -- together with S_i = sum_j max(|coefficient|,
+// 0.2 * 24 eps sig^6 y^4): the coefficient vanishes at r = 2^(1/6) sigma while its rounding error
+// (~3e-7 * 24 eps sig^6 y^4 there) does not, and the floor keeps the error-to-estimate ratio of
+// such a pair (1.5e-6) in line with the ~1e-6 of every other pair.
 // The fp32 error of F_i is a random sum of per-pair errors of relative size ~1e-7 * (7..13):
 // measured on the oracle (32k and 256k particles, lattice and liquid states) it stays below
 // 6e-6 * max(|F_i|, 1e-3) whenever S_i <= 8 * max(|F_i|, 1e-3).  A particle that fails this
@@ -59,11 +62,11 @@ __device__ __forceinline__ void lj_pair32(const Pair32 &pp, float dx, float dy, 
     const float y = rcp32(CHECK ? (in ? r2 : 1.0f) : r2);   // unchecked rows hold true neighbors: r2 > 0
     const float y2 = y * y;
     const float y3 = y2 * y;
-    float t = fmaf(pp.sig6x2, y3, -1.0f);                // 2 s6 - 1
-    t = in ? t : 0.0f;
-    const float c = (y2 * y2) * t;
+    const float t = fmaf(pp.sig6x2, y3, -1.0f);          // 2 s6 - 1
+    const float y4 = in ? y2 * y2 : 0.0f;
+    const float c = y4 * t;
     a.fx = fmaf(c, dx, a.fx); a.fy = fmaf(c, dy, a.fy); a.fz = fmaf(c, dz, a.fz);
-    a.s += fabsf(c);
+    a.s += fmaxf(fabsf(c), 0.2f * y4);                   // |coefficient|, floored near its zero (see above)
     if (ENERGY) {
         const float s6 = 0.5f * pp.sig6x2 * y3;
         a.e += in ? fmaf(s6, s6, -s6) - pp.ucut4 : 0.0f;

@@ -136,6 +136,100 @@ k_cell_scan(int cells, int *__restrict__ cell_count, int *__restrict__ cell_star
     if (tid == 1023) cell_start[cells] = warp_sum[31];
 }
 
+// Large grids (more than SCAN_ONE_BLOCK cells): the scan in two launches.  k_cell_sum: every block
+// sums SCAN_CHUNK consecutive counters; the last block to finish turns the block sums into
+// exclusive offsets.  k_cell_scan2: every block scans its chunk again, adds its offset, writes
+// cell_start and zeroes the counters.
+constexpr int SCAN_CHUNK = 4096;           // counters per block: 1024 threads x 4
+constexpr int SCAN_ONE_BLOCK = 16384;      // up to this many cells k_cell_scan (one block) is used
+
+__device__ __forceinline__ int4 load4_counts(const int *cell_count, int c, int cells) {
+    int4 v = make_int4(0, 0, 0, 0);
+    if (c + 3 < cells) v = *reinterpret_cast<const int4 *>(cell_count + c);
+    else {
+        if (c < cells) v.x = cell_count[c];
+        if (c + 1 < cells) v.y = cell_count[c + 1];
+        if (c + 2 < cells) v.z = cell_count[c + 2];
+    }
+    return v;
+}
+
+// inclusive scan of one value per thread over a block of 1024 threads; returns the inclusive
+// prefix, *total receives the block total (valid in every thread after the call)
+__device__ __forceinline__ int block_scan_1024(int x, int *warp_sum, int *total) {
+    const int lane = threadIdx.x & 31, wid = threadIdx.x >> 5;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        int y = __shfl_up_sync(FULL, x, o);
+        if (lane >= o) x += y;
+    }
+    __syncthreads();                        // warp_sum may still be read from a previous call
+    if (lane == 31) warp_sum[wid] = x;
+    __syncthreads();
+    if (wid == 0) {
+        int w = warp_sum[lane];
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            int y = __shfl_up_sync(FULL, w, o);
+            if (lane >= o) w += y;
+        }
+        warp_sum[lane] = w;
+    }
+    __syncthreads();
+    *total = warp_sum[31];
+    return x + (wid ? warp_sum[wid - 1] : 0);
+}
+
+__global__ void __launch_bounds__(1024)
+k_cell_sum(int cells, const int *__restrict__ cell_count, int *__restrict__ block_sum, int *ticket,
+           int *status, const int *cond) {
+    if (cond && ld_volatile(cond) == 0) return;
+    __shared__ int warp_sum[32];
+    __shared__ int is_last;
+    const int tid = threadIdx.x;
+    const int4 v = load4_counts(cell_count, blockIdx.x * SCAN_CHUNK + tid * 4, cells);
+    int total;
+    block_scan_1024(v.x + v.y + v.z + v.w, warp_sum, &total);
+    if (tid == 0) {
+        block_sum[blockIdx.x] = total;
+        __threadfence();
+        is_last = atomicAdd(ticket, 1) == (int)gridDim.x - 1;
+    }
+    __syncthreads();
+    if (!is_last) return;
+    __threadfence();
+    if (tid == 0) { *ticket = 0; if (status) { status[0] = 0; status[1] = 0; } }
+    int carry = 0;                           // exclusive scan of the block sums, 1024 at a time
+    for (int b0 = 0; b0 < (int)gridDim.x; b0 += 1024) {
+        const int b = b0 + tid;
+        const int x = b < (int)gridDim.x ? ld_volatile(block_sum + b) : 0;
+        int tot;
+        const int incl = block_scan_1024(x, warp_sum, &tot);
+        if (b < (int)gridDim.x) block_sum[b] = carry + incl - x;
+        carry += tot;
+    }
+    if (tid == 0) block_sum[gridDim.x] = carry;
+}
+
+__global__ void __launch_bounds__(1024)
+k_cell_scan2(int cells, int *__restrict__ cell_count, int *__restrict__ cell_start,
+             const int *__restrict__ block_sum, const int *cond) {
+    if (cond && ld_volatile(cond) == 0) return;
+    __shared__ int warp_sum[32];
+    const int tid = threadIdx.x;
+    const int c = blockIdx.x * SCAN_CHUNK + tid * 4;
+    const int4 v = load4_counts(cell_count, c, cells);
+    const int mine = v.x + v.y + v.z + v.w;
+    int total;
+    const int incl = block_scan_1024(mine, warp_sum, &total);
+    int run = block_sum[blockIdx.x] + incl - mine;
+    if (c < cells) { cell_start[c] = run; cell_count[c] = 0; run += v.x; }
+    if (c + 1 < cells) { cell_start[c + 1] = run; cell_count[c + 1] = 0; run += v.y; }
+    if (c + 2 < cells) { cell_start[c + 2] = run; cell_count[c + 2] = 0; run += v.z; }
+    if (c + 3 < cells) { cell_start[c + 3] = run; cell_count[c + 3] = 0; }
+    if (blockIdx.x == gridDim.x - 1 && tid == 0) cell_start[cells] = block_sum[gridDim.x];
+}
+
 __global__ void __launch_bounds__(256)
 k_cell_scatter(int n, const int *__restrict__ cell_of, const int *__restrict__ rank_tmp,
                const int *__restrict__ cell_start, int *__restrict__ perm_tmp, const int *cond) {

@@ -99,30 +99,32 @@ k_nbr_build2(Geom g, const float4 *__restrict__ spos, const int *__restrict__ ce
             }
             int nw = 0;                      // mask words of the current batch (warp-uniform)
             unsigned nzlo = 0u, nzhi = 0u;   // which of them are non-zero for this lane (words 0-31, 32-)
+            int nhit = 0;                    // hits of this lane in the current batch (self excluded)
             // every lane pulls its next hit per iteration (taking its next non-zero mask word when
-            // the current one is used up): row k of the tile leaves as one 128-byte store
+            // the current one is used up): row k of the tile leaves as one 128-byte store.  The trip
+            // count is the largest number of hits any lane holds, so the loop needs no vote.
             auto expand = [&]() {
                 __syncwarp();
                 unsigned plo = inseg ? nzlo : 0u, phi = inseg ? nzhi : 0u;   // words still to visit
+                const int nit = warp_max(inseg ? nhit : 0);
                 unsigned word = 0u;
                 int w = 0;
                 int *optr = outp + (size_t)min(cnt, cap) * TILE;
-                while (true) {
+                for (int it = 0; it < nit; ++it) {
                     if (word == 0u && (plo | phi)) {
                         if (plo) { w = __ffs(plo) - 1; plo &= plo - 1u; }
                         else { w = 31 + __ffs(phi); phi &= phi - 1u; }
                         word = W.mask[w][lane];
                     }
-                    if (!__any_sync(FULL, word != 0u)) break;
-                    const int bit = __clz(word);                 // 32 when word == 0
-                    const int slot = W.wbase[w] + bit;
-                    const bool hit = word != 0u && slot != s;
-                    word &= 0x7fffffffu >> (bit & 31);           // drop that bit (all above it are 0)
-                    if (hit && cnt < cap) { *optr = MAPPED ? map[slot] : slot; optr += TILE; }
-                    cnt += hit ? 1 : 0;
+                    if (word) {
+                        const int bit = __clz(word);
+                        word &= 0x7fffffffu >> bit;              // drop that bit (all above it are 0)
+                        if (cnt < cap) { const int slot = W.wbase[w] + bit; *optr = MAPPED ? map[slot] : slot; optr += TILE; }
+                        ++cnt;
+                    }
                 }
                 __syncwarp();
-                nw = 0; nzlo = 0u; nzhi = 0u;
+                nw = 0; nzlo = 0u; nzhi = 0u; nhit = 0;
             };
 
             // ---- walk the pieces; the next chunk is loaded while the current one is tested
@@ -214,6 +216,11 @@ k_nbr_build2(Geom g, const float4 *__restrict__ spos, const int *__restrict__ ce
                         for (int gq = 0; gq < ng; ++gq) hi = four(c0 + 4 * gq, hi);
                         hi <<= 32 - 4 * ng;
                     }
+                    {   // my own slot passes the test at distance 0: drop its bit here
+                        const unsigned self = (unsigned)(s - (base + c0));
+                        if (self < 32u) hi &= ~(0x80000000u >> self);
+                    }
+                    nhit += __popc(hi);
                     W.mask[nw][lane] = hi;
                     if (nw < 32) nzlo |= (hi != 0u ? 1u : 0u) << nw;
                     else nzhi |= (hi != 0u ? 1u : 0u) << (nw - 32);

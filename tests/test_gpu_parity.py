@@ -177,6 +177,32 @@ def test_first_design_builder(B, orc, W, ci):
     S.close()
 
 
+def test_fast32_dimers_at_the_force_zero(B, orc, W):
+    """Isolated pairs around r = 2^(1/6) sigma, where the LJ force changes sign: the coefficient and
+    with it sum|coefficient| vanish while the fp32 rounding error does not, so the error estimate
+    needs its floor there (md_force32.cuh).  64 dimers in a sparse 3-D box, sigma = 0.4."""
+    rng = np.random.default_rng(5)
+    sig = float(np.float32(0.4))
+    box32 = np.array([30.3, 30.3, 30.3], np.float32)
+    centers = (np.stack(np.meshgrid(*[np.arange(4)] * 3, indexing="ij"), -1).reshape(-1, 3) * 7.0 + 3.0)
+    pos = np.zeros((128, 4), np.float32); pos[:, 3] = 1.0
+    for k, c in enumerate(centers):
+        u = rng.normal(size=3); u /= np.linalg.norm(u)
+        r = 2.0 ** (1.0 / 6.0) * sig * (1.0 + (k - 32) * 1e-4)      # from 0.3 % inside to 0.3 % outside
+        pos[2 * k, :3] = c + 0.5 * r * u
+        pos[2 * k + 1, :3] = c - 0.5 * r * u
+    w = custom_workload(W, pos, box32, 3, 0, 1.0, 0.25, 32)
+    w = dataclasses.replace(w, sigma=0.4)
+    S = B.System(w)
+    S.build(); S.compute_force()
+    f = unpermute(S, S.force)
+    f_o, _, E_o = orc.energy_force(w.pos, None, w.box, 3, 0, 1.0, sig, 1.0, 1)
+    assert np.linalg.norm(f_o, axis=1).max() < 1.0 and np.linalg.norm(f_o, axis=1).min() < 1e-2
+    assert force_error(f, f_o) <= FORCE_TOL
+    assert abs(float(S.energy.cpu()[0]) - E_o) <= ENERGY_TOL * abs(E_o)
+    S.close()
+
+
 @pytest.mark.parametrize("thr", [1e-3, 8.0, 1e9])
 def test_fast32_re_evaluation(B, orc, W, thr):
     """The fp32 fast path: est_thr -> 0 sends every particle through the fp64 re-evaluation (must
@@ -228,6 +254,8 @@ def edge_positions(W, seed, n, dim, box, R):
     (3, [5.01, 5.01, 5.01], 1),      # a single particle
     (3, [5.01, 5.01, 5.01], 2),
     (3, [40.5, 4.0, 4.0], 50),       # sparse: most cells empty
+    (2, [200.7, 190.3], 5000),       # 160 x 152 = 24,320 cells: the two-launch cell scan
+    (3, [40.3, 40.3, 41.1], 3000),   # 32 x 32 x 32 = 32,768 cells, almost all empty
 ])
 @pytest.mark.parametrize("kind", [0, 1])
 def test_edge_cases(B, orc, W, dim, box, n, kind):
@@ -253,7 +281,10 @@ def test_edge_cases(B, orc, W, dim, box, n, kind):
             # random overlaps give |F| ~ 1e9: compare where the oracle force is sane
             S.compute_force()
             f = unpermute(S, S.force)
-            f_o, _, _ = orc.energy_force(w.pos, None, w.box, dim, 0, 1.0, 0.4, float(np.float32(r_cut)), 1)
+            # the ABI carries sigma as fp32: the oracle gets the same value (near the zero of the
+            # pair force a 1.5e-8 difference in sigma is amplified a thousandfold)
+            f_o, _, _ = orc.energy_force(w.pos, None, w.box, dim, 0, 1.0, float(np.float32(0.4)),
+                                         float(np.float32(r_cut)), 1)
             sane = np.linalg.norm(f_o, axis=1) < 1e30        # beyond that fp32 cannot hold F
             num = np.linalg.norm(f[sane, :3].astype(np.float64) - f_o[sane], axis=1)
             if sane.any():
