@@ -54,6 +54,7 @@
 
 #define KIND_LJ 0
 #define KIND_SOFT 1
+#define KIND_MORSE 2
 
 int orc_num_threads(void)
 {
@@ -386,6 +387,18 @@ static void lj_pair(double r2, double eps, double sigma, double *u, double *fr)
     *fr = 24.0 * eps * (2.0 * s12 - s6) / r2;
 }
 
+/* Morse u(r) = D (1 - exp(-alpha (r - r0)))^2 - D and -u'(r)/r (PAPER.md:L104 [75]; the paper
+ * names the potential only: the standard form with well depth D at r0, reading A19). */
+static double g_morse_alpha = 5.0;
+void orc_set_morse_alpha(double alpha) { g_morse_alpha = alpha; }
+
+static void morse_pair(double r, double D, double r0, double alpha, double *u, double *fr)
+{
+    double x = exp(-alpha * (r - r0));
+    *u = D * (1.0 - x) * (1.0 - x) - D;
+    *fr = r > 0.0 ? -2.0 * D * alpha * x * (1.0 - x) / r : 0.0;
+}
+
 static double lj_u_cut(double eps, double sigma, double r_cut)
 {
     double u, fr;
@@ -399,6 +412,8 @@ static double lj_u_cut(double eps, double sigma, double r_cut)
  *   kind 0 LJ:   u = 4 eps[(s/r)^12 - (s/r)^6] - shift*u(r_cut)  for r < r_cut
  *   kind 1 SOFT: u = eps/2 (1 - r/d_ij)^2 for r < d_ij, d_ij = (d_i + d_j)/2
  *                (PAPER.md:L301); r = 0 gives energy eps/2 and zero force
+ *   kind 2 MORSE: u = eps (1 - exp(-alpha (r - sigma)))^2 - eps - shift*u(r_cut) for r < r_cut,
+ *                alpha set by orc_set_morse_alpha (PAPER.md:L104 [75])
  *   nbr_idx == NULL: all pairs j != i (the definition);
  *   else: over the list rows (L80 smap.neighbors), entries >= n are padding.
  *   force double[n*3] (z = 0 in 2-D), e_i double[n], *E double.
@@ -410,9 +425,13 @@ int orc_energy_force(int n, int dim, const double *pos, const double *diam,
                      double *e_i, double *E)
 {
     if (n <= 0 || (dim != 2 && dim != 3)) return ORC_EINVAL;
-    if (kind != KIND_LJ && kind != KIND_SOFT) return ORC_EINVAL;
+    if (kind != KIND_LJ && kind != KIND_SOFT && kind != KIND_MORSE) return ORC_EINVAL;
     if (kind == KIND_SOFT && !diam) return ORC_EINVAL;
     double u_c = (kind == KIND_LJ && shift) ? lj_u_cut(eps, sigma, r_cut) : 0.0;
+    if (kind == KIND_MORSE && shift) {
+        double fr_unused;
+        morse_pair(r_cut, eps, sigma, g_morse_alpha, &u_c, &fr_unused);
+    }
 #pragma omp parallel for schedule(dynamic, 64)
     for (int i = 0; i < n; ++i) {
         double f[3] = {0.0, 0.0, 0.0}, e = 0.0;
@@ -429,6 +448,13 @@ int orc_energy_force(int n, int dim, const double *pos, const double *diam,
                 if (r2 < r_cut * r_cut) {
                     double u, fr;
                     lj_pair(r2, eps, sigma, &u, &fr);
+                    e += 0.5 * (u - u_c);
+                    for (int q = 0; q < dim; ++q) f[q] += fr * d[q];
+                }
+            } else if (kind == KIND_MORSE) {
+                if (r2 < r_cut * r_cut) {
+                    double u, fr;
+                    morse_pair(sqrt(r2), eps, sigma, g_morse_alpha, &u, &fr);
                     e += 0.5 * (u - u_c);
                     for (int q = 0; q < dim; ++q) f[q] += fr * d[q];
                 }

@@ -111,8 +111,15 @@ def predicate_band(pos, box, dim, r_cut, skin, method=1):
     return int(nd.value), float(band.value), float(close.value)
 
 
+def set_morse_alpha(alpha: float) -> None:
+    """alpha of kind 2 (Morse) for the following energy_force / nve_run calls."""
+    lib().orc_set_morse_alpha(C.c_double(alpha))
+
+
 def energy_force(pos, diam, box, dim, kind, eps, sigma, r_cut, shift,
-                 nbr_idx=None, nbr_count=None):
+                 nbr_idx=None, nbr_count=None, alpha=None):
+    if alpha is not None:
+        set_morse_alpha(alpha)
     p = _d(pos3(pos)); b = _d(box)
     n = p.shape[0]
     dm = _d(diam) if diam is not None else None
@@ -140,8 +147,10 @@ def needs_rebuild(pos, ref, box, dim, skin):
 
 
 def nve_run(pos, vel, force, diam, box, dim, kind, eps, sigma, r_cut, shift, dt, mass,
-            nsteps, use_list=0, skin=0.0, capacity=128, want_energies=True):
+            nsteps, use_list=0, skin=0.0, capacity=128, want_energies=True, alpha=None):
     """Returns (pos, vel, force, energies[(nsteps+1),2] or None, stats[3])."""
+    if alpha is not None:
+        set_morse_alpha(alpha)
     p = _d(pos3(pos)).copy(); v = _d(pos3(vel)).copy(); f = _d(pos3(force)).copy()
     b = _d(box)
     dm = _d(diam) if diam is not None else None

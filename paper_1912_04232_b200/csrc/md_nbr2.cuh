@@ -110,18 +110,24 @@ k_nbr_build2(Geom g, const float4 *__restrict__ spos, const int *__restrict__ ce
                 unsigned word = 0u;
                 int w = 0;
                 int *optr = outp + (size_t)min(cnt, cap) * TILE;
+                // branch-free body: selects and predicated memory operations only
                 for (int it = 0; it < nit; ++it) {
-                    if (word == 0u && (plo | phi)) {
-                        if (plo) { w = __ffs(plo) - 1; plo &= plo - 1u; }
-                        else { w = 31 + __ffs(phi); phi &= phi - 1u; }
-                        word = W.mask[w][lane];
-                    }
-                    if (word) {
-                        const int bit = __clz(word);
-                        word &= 0x7fffffffu >> bit;              // drop that bit (all above it are 0)
-                        if (cnt < cap) { const int slot = W.wbase[w] + bit; *optr = MAPPED ? map[slot] : slot; optr += TILE; }
-                        ++cnt;
-                    }
+                    const bool need = word == 0u && (plo | phi) != 0u;
+                    const int wl = __ffs(plo) - 1, wh = 31 + __ffs(phi);
+                    const int wn = plo ? wl : wh;
+                    const unsigned nlo = plo & (plo - 1u), nhi = plo ? phi : (phi & (phi - 1u));
+                    w = need ? wn : w;
+                    plo = need ? nlo : plo;
+                    phi = need ? nhi : phi;
+                    const unsigned fresh = W.mask[w][lane];        // w is always a valid word index
+                    word = need ? fresh : word;
+                    const bool has = word != 0u;
+                    const int bit = __clz(word) & 31;
+                    const int slot = W.wbase[w] + bit;
+                    word &= 0x7fffffffu >> bit;                    // drop that bit (all above it are 0)
+                    if (has && cnt < cap) *optr = MAPPED ? map[slot] : slot;
+                    optr += (has && cnt < cap) ? TILE : 0;
+                    cnt += has ? 1 : 0;
                 }
                 __syncwarp();
                 nw = 0; nzlo = 0u; nzhi = 0u; nhit = 0;

@@ -115,6 +115,56 @@ def test_lj_two_body(orc, axis):
     assert E == 0.0
 
 
+@pytest.mark.parametrize("axis", [0, 2])
+def test_morse_two_body(orc, axis):
+    """Morse [75], u = D (1 - exp(-a (r - r0)))^2 - D: closed forms at r0, at
+    r0 + ln(2)/a (where exp(..) = 1/2), on the repulsive side, and the shifted cutoff."""
+    MORSE = 2
+    D, r0, a, rc = 1.7, 1.1, 4.0, 2.6
+    pos, box, _ = two_body(r0, axis)
+    f, e_i, E = orc.energy_force(pos, None, box, 3, MORSE, D, r0, rc, 0, alpha=a)
+    assert abs(E + D) < 1e-12 and np.abs(f).max() < 1e-12 and np.allclose(e_i, [-D / 2, -D / 2])
+    r = r0 + np.log(2.0) / a
+    pos, box, _ = two_body(r, axis)
+    f, _, E = orc.energy_force(pos, None, box, 3, MORSE, D, r0, rc, 0, alpha=a)
+    assert abs(E - (D * 0.25 - D)) < 1e-12
+    du = 2 * D * a * 0.5 * 0.5                              # u'(r) > 0: attraction
+    assert abs(f[0, axis] - du) < 1e-12 and abs(f[1, axis] + du) < 1e-12
+    r = 0.8 * r0
+    x = np.exp(-a * (r - r0))
+    pos, box, _ = two_body(r, axis)
+    f, _, E0 = orc.energy_force(pos, None, box, 3, MORSE, D, r0, rc, 0, alpha=a)
+    _, _, E1 = orc.energy_force(pos, None, box, 3, MORSE, D, r0, rc, 1, alpha=a)
+    uc = D * (1 - np.exp(-a * (rc - r0))) ** 2 - D
+    assert abs(E0 - (D * (1 - x) ** 2 - D)) < 1e-12 and abs(E1 - (E0 - uc)) < 1e-12
+    assert f[0, axis] < 0 and abs(f[0, axis] - 2 * D * a * x * (1 - x)) < 1e-10   # repulsion
+    pos, box, _ = two_body(rc * (1 - 1e-9), axis)
+    assert abs(orc.energy_force(pos, None, box, 3, MORSE, D, r0, rc, 1, alpha=a)[2]) < 1e-7
+    pos, box, _ = two_body(rc * (1 + 1e-9), axis)
+    f, _, E = orc.energy_force(pos, None, box, 3, MORSE, D, r0, rc, 1, alpha=a)
+    assert E == 0.0 and np.abs(f).max() == 0.0
+
+
+def test_morse_gradient_and_newton(orc, W):
+    """Morse forces are -grad E (central differences) and sum to zero."""
+    MORSE = 2
+    w = W.lj_fcc(0, 3, seed=12)
+    pos, box = w.pos[:, :3].astype(np.float64), w.box.astype(np.float64)
+    args = (MORSE, 1.0, 1.12, 2.5, 1)
+    f, _, _ = orc.energy_force(pos, None, box, 3, *args, alpha=5.0)
+    assert np.abs(f.sum(0)).max() < 1e-10 * np.abs(f).sum()
+    rng = np.random.default_rng(3)
+    h, worst = 1e-5, 0.0
+    for i in rng.choice(pos.shape[0], 8, replace=False):
+        for q in range(3):
+            pp = pos.copy(); pp[i, q] += h
+            pm = pos.copy(); pm[i, q] -= h
+            fd = -(orc.energy_force(pp, None, box, 3, *args, alpha=5.0)[2]
+                   - orc.energy_force(pm, None, box, 3, *args, alpha=5.0)[2]) / (2 * h)
+            worst = max(worst, abs(fd - f[i, q]) / max(1.0, np.abs(f[i]).max()))
+    assert worst < 1e-6, worst
+
+
 @pytest.mark.parametrize("dim", [2, 3])
 def test_soft_two_body(orc, dim):
     eps = 1.3
