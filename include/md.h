@@ -46,6 +46,7 @@ extern "C" {
 
 #define MD_KIND_LJ   0      /* Lennard-Jones [69], L104 §3.3.2 */
 #define MD_KIND_SOFT 1      /* harmonic soft sphere [70], L104; d_ij = (d_i+d_j)/2, L301 App. A */
+#define MD_KIND_MORSE 2     /* Morse [75], L104: u = eps (1 - exp(-alpha (r - sigma)))^2 - eps */
 
 typedef struct md_system md_system;   /* opaque; lives in host memory */
 
@@ -65,7 +66,8 @@ typedef struct md_potential {
     float epsilon;
     float sigma;      /* LJ length; unused for SOFT (diameters come from pos.w) */
     float r_cut;      /* LJ truncation radius (<= config r_cut); unused for SOFT */
-    int   shift;      /* LJ: 1 = u(r) - u(r_cut) for r < r_cut, 0 = plain truncation */
+    int   shift;      /* LJ, MORSE: 1 = u(r) - u(r_cut) for r < r_cut, 0 = plain truncation */
+    float alpha;      /* MORSE: inverse width; sigma is its r0, epsilon its well depth D. Unused otherwise */
 } md_potential;
 
 /* Text of the last error on the calling thread ("" if none). Host pointer, valid until the
@@ -159,6 +161,7 @@ int md_needs_rebuild(md_system *sys, const void *pos, int32_t *flag, void *strea
  * L104 force = -grad U, written in closed form):
  *   LJ   u = 4 eps[(s/r)^12 - (s/r)^6] - shift*u(r_cut), r < r_cut
  *   SOFT u = eps/2 (1 - r/d_ij)^2, r < d_ij = (pos_i.w + pos_j.w)/2; r = 0: eps/2, no force
+ *   MORSE u = eps (1 - exp(-alpha (r - sigma)))^2 - eps - shift*u(r_cut), r < r_cut (fp64 chain)
  *   force        float4[n] out: (F_i, e_i)
  *   energy_total double* out (may be NULL): sum_i e_i accumulated in fp64
  *   nbr_idx / nbr_count  any list in the md_nbr_layout layout whose rows hold every pair

@@ -15,7 +15,7 @@ import torch
 from . import build as _build
 
 MD_OK, MD_EINVAL, MD_EBOX, MD_EWORKSPACE, MD_ECUDA = 0, -1, -2, -3, -4
-MD_KIND_LJ, MD_KIND_SOFT = 0, 1
+MD_KIND_LJ, MD_KIND_SOFT, MD_KIND_MORSE = 0, 1, 2
 
 SYMBOLS = [
     "md_last_error", "md_workspace_bytes", "md_create", "md_destroy", "md_set_option",
@@ -32,7 +32,7 @@ class md_config(C.Structure):
 
 class md_potential(C.Structure):
     _fields_ = [("kind", C.c_int), ("epsilon", C.c_float), ("sigma", C.c_float),
-                ("r_cut", C.c_float), ("shift", C.c_int)]
+                ("r_cut", C.c_float), ("shift", C.c_int), ("alpha", C.c_float)]
 
 
 class MdError(RuntimeError):
@@ -110,8 +110,8 @@ def make_config(dim, box, r_cut, skin, capacity, resort=1) -> md_config:
                      int(resort))
 
 
-def make_potential(kind, epsilon=1.0, sigma=1.0, r_cut=2.5, shift=1) -> md_potential:
-    return md_potential(int(kind), float(epsilon), float(sigma), float(r_cut), int(shift))
+def make_potential(kind, epsilon=1.0, sigma=1.0, r_cut=2.5, shift=1, alpha=0.0) -> md_potential:
+    return md_potential(int(kind), float(epsilon), float(sigma), float(r_cut), int(shift), float(alpha))
 
 
 # ------------------------------------------------------------ the C ABI, same names ----
@@ -219,7 +219,7 @@ class System:
         self.device = torch.device(device)
         self.cfg = make_config(w.dim, w.box, w.r_cut, w.skin, capacity or w.capacity,
                                w.resort if resort is None else resort)
-        self.pot = make_potential(w.kind, w.epsilon, w.sigma, w.r_cut, w.shift)
+        self.pot = make_potential(w.kind, w.epsilon, w.sigma, w.r_cut, w.shift, getattr(w, "alpha", 0.0))
         n, cap = w.n, self.cfg.capacity
         self.n, self.capacity = n, cap
         with torch.cuda.device(self.device):

@@ -163,7 +163,8 @@ int make_geom(const md_config *cfg, int n, Geom *g) {
 
 int make_pair(const md_system *sys, const md_potential *pot, Pair *pp) {
     if (!pot) return fail(MD_EINVAL, "potential is NULL");
-    if (pot->kind != MD_KIND_LJ && pot->kind != MD_KIND_SOFT) return fail(MD_EINVAL, "unknown potential kind %d", pot->kind);
+    if (pot->kind != MD_KIND_LJ && pot->kind != MD_KIND_SOFT && pot->kind != MD_KIND_MORSE)
+        return fail(MD_EINVAL, "unknown potential kind %d", pot->kind);
     if (!(pot->epsilon > 0.0f)) return fail(MD_EINVAL, "epsilon must be positive");
     memset(pp, 0, sizeof(*pp));
     pp->kind = pot->kind;
@@ -175,6 +176,13 @@ int make_pair(const md_system *sys, const md_potential *pot, Pair *pp) {
         pp->dsig6x2 = 2.0 * std::pow(s, 6.0); pp->drc2 = rc * rc;
         const double s6 = std::pow(s / rc, 6.0);
         pp->du_cut4 = pot->shift ? (s6 * s6 - s6) : 0.0;
+    } else if (pot->kind == MD_KIND_MORSE) {
+        if (!(pot->r_cut > 0.0f) || !(pot->sigma > 0.0f) || !(pot->alpha > 0.0f))
+            return fail(MD_EINVAL, "Morse needs sigma (r0) > 0, alpha > 0 and r_cut > 0");
+        if (pot->r_cut > sys->cfg.r_cut) return fail(MD_EINVAL, "potential r_cut %g exceeds the list r_cut %g", pot->r_cut, sys->cfg.r_cut);
+        const double rc = pot->r_cut, x = std::exp(-(double)pot->alpha * (rc - (double)pot->sigma));
+        pp->dalpha = pot->alpha; pp->dr0 = pot->sigma; pp->drc2 = rc * rc; pp->dsig6x2 = 2.0;
+        pp->du_cutm = pot->shift ? ((1.0 - x) * (1.0 - x) - 1.0) : 0.0;
     } else {
         pp->dsig6x2 = 2.0; pp->drc2 = 1e300;
     }
@@ -299,6 +307,7 @@ int launch_force(md_system *s, const Pair &pp, const float4 *pos, const int *nbr
                  : launch_force_t<K, D, false>(s, pp, pos, nbr_idx, nbr_count, force, vel, a,  \
                                                etot, book, st))
     if (pp.kind == MD_KIND_LJ) return s->g.dim == 3 ? MD_FORCE_DISPATCH(0, 3) : MD_FORCE_DISPATCH(0, 2);
+    if (pp.kind == MD_KIND_MORSE) return s->g.dim == 3 ? MD_FORCE_DISPATCH(2, 3) : MD_FORCE_DISPATCH(2, 2);
     return s->g.dim == 3 ? MD_FORCE_DISPATCH(1, 3) : MD_FORCE_DISPATCH(1, 2);
 #undef MD_FORCE_DISPATCH
 }

@@ -27,6 +27,8 @@ struct Pair {
     double deps, drc2;
     double dsig6x2;         // LJ: 2 sigma^6
     double du_cut4;         // LJ: shift * u(r_cut) / (4 eps) = shift * ((s/rc)^12 - (s/rc)^6)
+    double dalpha, dr0;     // MORSE: alpha, r0
+    double du_cutm;         // MORSE: shift * u(r_cut) / eps
 };
 
 // Device words md_nve_step keeps between kernels.
@@ -638,6 +640,20 @@ __device__ __forceinline__ void soft_pair64(const Pair &pp, double dx, double dy
     if (ENERGY) a.e += in ? x * x : 0.0;
 }
 
+// One pair, Morse [75] (L104): u = D (1 - x)^2 - D, x = exp(-alpha (r - r0)); the force
+// coefficient -u'(r)/r = -2 D alpha x (1 - x) / r; D is applied once per particle.
+template <bool ENERGY>
+__device__ __forceinline__ void morse_pair64(const Pair &pp, double dx, double dy, double dz,
+                                             bool valid, Acc64 &a) {
+    const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+    const bool in = valid && r2 < pp.drc2;
+    const double r = sqrt(in ? r2 : 1.0);
+    const double x = exp(-pp.dalpha * (r - pp.dr0));
+    double c = (in && r > 0.0) ? -2.0 * pp.dalpha * x * (1.0 - x) / r : 0.0;
+    a.fx = fma(c, dx, a.fx); a.fy = fma(c, dy, a.fy); a.fz = fma(c, dz, a.fz);
+    if (ENERGY) a.e += in ? (1.0 - x) * (1.0 - x) - 1.0 - pp.du_cutm : 0.0;
+}
+
 // Per-thread view of the space for the pair loop.
 template <int DIM>
 struct Me {
@@ -675,6 +691,7 @@ __device__ __forceinline__ void pair_any(const Pair &pp, const Me<DIM> &me, cons
     double dx, dy, dz;
     displacement<DIM, WRAP>(me, q, dx, dy, dz);
     if (KIND == 0) lj_pair64<ENERGY>(pp, dx, dy, dz, valid, acc);
+    else if (KIND == 2) morse_pair64<ENERGY>(pp, dx, dy, dz, valid, acc);
     else soft_pair64<ENERGY>(pp, dx, dy, dz, (double)me.pi.w + (double)q.w, valid, acc);
 }
 
@@ -701,8 +718,8 @@ __device__ __forceinline__ void force_epilogue(const Pair &pp, const Acc64 &acc,
                                                float4 *__restrict__ force, float4 *__restrict__ vel,
                                                float a, double *energy_total, const Book &book,
                                                int gid) {
-    const double fs = KIND == 0 ? 12.0 * pp.deps * pp.dsig6x2 : pp.deps;     // 24 eps sig^6 | eps
-    const double es = KIND == 0 ? 2.0 * pp.deps : 0.25 * pp.deps;            // 1/2 * (4 eps | eps/2)
+    const double fs = KIND == 0 ? 12.0 * pp.deps * pp.dsig6x2 : pp.deps;     // 24 eps sig^6 | eps | D
+    const double es = KIND == 0 ? 2.0 * pp.deps : (KIND == 2 ? 0.5 * pp.deps : 0.25 * pp.deps);   // 1/2 * (4 eps | D | eps/2)
     const float fx = (float)(fs * acc.fx), fy = (float)(fs * acc.fy), fz = (float)(fs * acc.fz);
     const double e64 = ENERGY ? es * acc.e : 0.0;
     if (owner) {

@@ -28,6 +28,7 @@ RHO_LJ = 0.8442           # LJ number density of configs 0, 2, 3, 4
 
 KIND_LJ = 0
 KIND_SOFT = 1
+KIND_MORSE = 2
 
 
 @dataclasses.dataclass(frozen=True)
@@ -52,6 +53,7 @@ class Workload:
     resort: int
     pos: np.ndarray          # float32[N,4]
     vel: np.ndarray          # float32[N,4]
+    alpha: float = 0.0       # Morse inverse width (KIND_MORSE: sigma = r0, epsilon = D)
 
     @property
     def list_radius(self) -> float:

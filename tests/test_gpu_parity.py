@@ -177,6 +177,44 @@ def test_first_design_builder(B, orc, W, ci):
     S.close()
 
 
+@pytest.mark.parametrize("dim", [3, 2])
+def test_morse_force_energy_and_trajectory(B, orc, W, dim):
+    """SURVEY §8f-f2, first potential beyond the two configs: Morse [75] on the
+    fp64 pair chain.  Force / energy against the oracle's all-pairs definition, then 100 NVE
+    steps against the oracle's fp64 trajectory (brute-force forces), on a jittered lattice."""
+    D, r0 = float(np.float32(0.9)), float(np.float32(1.12))
+    alpha, rc = float(np.float32(5.0)), 2.5
+    if dim == 3:
+        base = W.config(0)
+        pos, vel, box = base.pos.copy(), base.vel.copy(), base.box
+    else:
+        rng = np.random.default_rng(9)
+        g = np.arange(24.0)
+        xy = np.stack(np.meshgrid(g, g, indexing="ij"), -1).reshape(-1, 2) * 1.15 + rng.normal(0, 0.04, (576, 2))
+        box = np.array([24 * 1.15, 24 * 1.15, 1.0], np.float32)
+        pos = np.zeros((576, 4), np.float32); pos[:, :2] = W.into_box_f32(xy, box); pos[:, 3] = 1.0
+        vel = np.zeros((576, 4), np.float32); vel[:, :2] = rng.normal(0, 0.5, (576, 2)); vel[:, :2] -= vel[:, :2].mean(0)
+    w = custom_workload(W, pos, box, dim, 2, rc, 0.3, 128, vel=vel, dt=0.005)
+    w = dataclasses.replace(w, epsilon=D, sigma=r0, alpha=alpha, shift=1)
+    S = B.System(w)
+    S.build(); S.compute_force()
+    f_o, e_o, E_o = orc.energy_force(w.pos, None, w.box, dim, 2, D, r0, rc, 1, alpha=alpha)
+    f = unpermute(S, S.force)
+    assert force_error(f, f_o) <= FORCE_TOL
+    assert abs(float(S.energy.cpu()[0]) - E_o) <= ENERGY_TOL * abs(E_o)
+    assert np.abs(f[:, 3] - e_o).max() <= 2e-6 * max(1.0, np.abs(e_o).max())
+    p_o, v_o, _, _, _ = orc.nve_run(w.pos, w.vel, f_o, None, w.box, dim, 2, D, r0, rc, 1, w.dt, w.mass,
+                                    100, want_energies=False, alpha=alpha)
+    S.step(100)
+    torch.cuda.synchronize()
+    assert int(S.stats[0]) == 100 and int(S.stats[2]) == -1
+    d = unpermute(S, S.pos)[:, :dim].astype(np.float64) - p_o[:, :dim]
+    L = w.box[:dim].astype(np.float64)
+    d -= L * np.round(d / L)
+    assert np.abs(d).max() <= 1e-4, np.abs(d).max()
+    S.close()
+
+
 def test_fast32_dimers_at_the_force_zero(B, orc, W):
     """Isolated pairs around r = 2^(1/6) sigma, where the LJ force changes sign: the coefficient and
     with it sum|coefficient| vanish while the fp32 rounding error does not, so the error estimate
