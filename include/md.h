@@ -126,7 +126,8 @@ int md_nbr_layout(const md_system *sys, long *tile, long *tile_stride, long *par
  * (c_z n_y + c_y) n_x + c_x, counting sort by cell.
  *   cell_start int32[cells+1] out: slots [cell_start[c], cell_start[c+1]) belong to cell c
  *   perm       int32[n]       out: perm[s] = index (on entry) of the particle in slot s;
- *                                  inside a cell slots ascend by id (or by index if id = NULL)
+ *                                  inside a cell slots ascend by x, ties by id (by index if id =
+ *                                  NULL); md_neighbor_list_build relies on this order
  *   resort = 1: pos, vel (may be NULL) and id (may be NULL) are permuted in place so that
  *               new[s] = old[perm[s]];  resort = 0: they are left untouched.
  */

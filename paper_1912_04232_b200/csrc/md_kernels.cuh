@@ -241,9 +241,10 @@ k_cell_scatter(int n, const int *__restrict__ cell_of, const int *__restrict__ r
     perm_tmp[cell_start[cell_of[i]] + rank_tmp[i]] = i;
 }
 
-// Canonical order inside a cell (ascending id, or index when id == NULL) by counting, so the
-// sorted state does not depend on atomic arrival order; gathers the payload into the sorted
-// scratch arrays.  One thread per slot.
+// Canonical order inside a cell by counting: ascending x, ties by id (or index when id == NULL),
+// so the sorted state does not depend on atomic arrival order and every x-row of cells is one
+// run of slots sorted by x (cells are x-bins), which lets the neighbor-list builder cut its scan
+// to the x-range of a tile.  Gathers the payload into the sorted scratch arrays.  One thread per slot.
 __global__ void __launch_bounds__(256)
 k_cell_order_gather(int n, const int *__restrict__ cell_of, const int *__restrict__ cell_start,
                     const int *__restrict__ perm_tmp, const int *__restrict__ id,
@@ -256,16 +257,18 @@ k_cell_order_gather(int n, const int *__restrict__ cell_of, const int *__restric
     int i = perm_tmp[s];
     int c = cell_of[i];
     int t0 = cell_start[c], t1 = cell_start[c + 1];
+    const float4 pi = pos[i];
     int key = id ? id[i] : i;
     int rank = 0;
     for (int t = t0; t < t1; ++t) {
         int j = perm_tmp[t];
         int kj = id ? id[j] : j;
-        rank += kj < key;
+        float xj = pos[j].x;
+        rank += (xj < pi.x) || (xj == pi.x && kj < key);
     }
     int dst = t0 + rank;
     perm[dst] = i;
-    pos_s[dst] = pos[i];
+    pos_s[dst] = pi;
     if (vel_s) vel_s[dst] = vel[i];
     if (id_s) id_s[dst] = id[i];
 }

@@ -55,6 +55,7 @@ k_nbr_build2(Geom g, const float4 *__restrict__ spos, const int *__restrict__ ce
     const int ncx = g.nc[0], ncy = g.nc[1], ncz = g.nc[2];
     const float Lx = g.L[0], Ly = g.L[1], Lz = g.L[2];
     const float2 nR2 = make_float2(-g.R2, -g.R2);
+    const float Rm = sqrtf(g.R2) * 1.0001f + 1e-4f * g.L[0];    // R plus a margin for the fp32 roundings
     constexpr int ROWS = DIM == 3 ? 9 : 3;
     const int ntiles = (g.n + TILE - 1) / TILE;
 
@@ -82,6 +83,12 @@ k_nbr_build2(Geom g, const float4 *__restrict__ spos, const int *__restrict__ ce
             const int rcy = __shfl_sync(FULL, cy, leader), rcz = __shfl_sync(FULL, cz, leader);
             const int a = warp_min(inseg ? cx : 0x7fffffff) - 1;
             const int b = warp_max(inseg ? cx : -1) + 1;
+            float seg_xlo = inseg ? pi.x : 3.0e38f, seg_xhi = inseg ? pi.x : -3.0e38f;
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                seg_xlo = fminf(seg_xlo, __shfl_xor_sync(FULL, seg_xlo, o));
+                seg_xhi = fmaxf(seg_xhi, __shfl_xor_sync(FULL, seg_xhi, o));
+            }
             // ---- piece table (as k_nbr_build): lane p < 3*ROWS describes piece p = kind*ROWS + rr
             int t0 = 0, t1 = 0;
             if (lane < 3 * ROWS) {
@@ -96,6 +103,20 @@ k_nbr_build2(Geom g, const float4 *__restrict__ spos, const int *__restrict__ ce
                 else if (kind == 1) { if (a < 0) { ca = ncx - 1; cb = ncx - 1; } }
                 else { if (b > ncx - 1) { ca = 0; cb = 0; } }
                 if (cb >= ca) { t0 = cell_start[rowbase + ca]; t1 = cell_start[rowbase + cb + 1]; }
+                // md_cell_list_build leaves every x-row of cells sorted by x: cut the piece to the
+                // candidates whose x lies within R (plus a rounding margin) of the segment's lanes
+                const float lo = kind == 1 ? seg_xlo - Rm + Lx : seg_xlo - Rm;
+                const float hi = kind == 2 ? seg_xhi + Rm - Lx : seg_xhi + Rm;
+                if (kind != 2) {                                 // first slot with x >= lo
+                    int a0 = t0, a1 = t1;
+                    while (a0 < a1) { const int mid = (a0 + a1) >> 1; if (spos[mid].x < lo) a0 = mid + 1; else a1 = mid; }
+                    t0 = a0;
+                }
+                if (kind != 1) {                                 // first slot with x > hi
+                    int a0 = t0, a1 = t1;
+                    while (a0 < a1) { const int mid = (a0 + a1) >> 1; if (spos[mid].x <= hi) a0 = mid + 1; else a1 = mid; }
+                    t1 = a0;
+                }
             }
             int nw = 0;                      // mask words of the current batch (warp-uniform)
             unsigned nzlo = 0u, nzhi = 0u;   // which of them are non-zero for this lane (words 0-31, 32-)

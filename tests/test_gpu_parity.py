@@ -74,8 +74,14 @@ def check_cells(S, orc, w):
     assert np.array_equal(cs, cell_start_o)
     assert cs[0] == 0 and cs[-1] == w.n and np.all(np.diff(cs) >= 0)
     assert np.array_equal(np.sort(perm), np.arange(w.n))
-    # canonical order inside a cell = ascending id; on the first build id == index
-    assert np.array_equal(perm, members_o)
+    # membership per cell is the oracle's (order inside a cell is free); the library's
+    # canonical order is ascending x, ties by id (on the first build id == index)
+    cell_of_slot = np.repeat(np.arange(len(cs) - 1), np.diff(cs))
+    order = np.lexsort((perm, cell_of_slot))
+    assert np.array_equal(perm[order], members_o)
+    xs = w.pos[perm, 0]
+    same = cell_of_slot[1:] == cell_of_slot[:-1]
+    assert np.all((xs[1:] > xs[:-1]) | ((xs[1:] == xs[:-1]) & (perm[1:] > perm[:-1])) | ~same)
     if S.cfg.resort:
         assert np.array_equal(S.pos.cpu().numpy(), w.pos[perm])
         assert np.array_equal(S.vel.cpu().numpy(), w.vel[perm])
