@@ -591,3 +591,75 @@ done:
     free(e_i); free(ref); free(idx); free(cnt);
     return rc;
 }
+
+/* ------------------------------------------------------------------ FIRE -- */
+
+/*
+ * orc_fire_run: FIRE minimisation (PAPER.md:L100 names "FIRE Descent" among the simulation
+ * environments and uses it to relax packings in section 4.2; the paper gives no formulas, so
+ * this is the algorithm of its reference [Bitzek et al. 2006] around the same velocity-Verlet
+ * step and force call, reading A20).  Unit mass.  Per step, with the current dt, alpha:
+ *   1. v += dt/2 F;  r = wrap(r + dt v);  F = F(r);  v += dt/2 F          (velocity Verlet)
+ *   2. P = sum F.v,  |F| = sqrt(sum F.F),  |v| = sqrt(sum v.v)
+ *   3. P > 0:  v = (1 - alpha) v + alpha |v| F / |F|;  n_pos += 1;
+ *              if n_pos > n_min: dt = min(dt f_inc, dt_max), alpha = alpha f_alpha
+ *      else:   v = 0;  n_pos = 0;  dt = dt f_dec;  alpha = alpha_start
+ * Forces by the all-pairs definition (orc_energy_force without a list).
+ *   par   in  double[7] = {dt_start, dt_max, n_min, f_inc, f_dec, alpha_start, f_alpha}
+ *   state in/out double[3] = {dt, alpha, n_pos}; pass dt <= 0 to start from dt_start, alpha_start, 0
+ *   energies out (may be NULL) double[nsteps+1]: potential energy at every step boundary
+ */
+int orc_fire_run(int n, int dim, double *pos, double *vel, double *force, const double *diam,
+                 const double *box, int kind, double eps, double sigma, double r_cut, int shift,
+                 const double *par, double *state, int nsteps, double *energies)
+{
+    if (n <= 0 || (dim != 2 && dim != 3) || !par || !state) return ORC_EINVAL;
+    double *e_i = (double *)malloc((size_t)n * sizeof(double));
+    if (!e_i) return ORC_ENOMEM;
+    double dt = state[0], alpha = state[1];
+    int n_pos = (int)state[2];
+    if (dt <= 0.0) { dt = par[0]; alpha = par[5]; n_pos = 0; }
+    double E = 0.0;
+    int rc = orc_energy_force(n, dim, pos, diam, box, kind, eps, sigma, r_cut, shift,
+                              NULL, NULL, 0, force, e_i, &E);
+    if (rc) { free(e_i); return rc; }
+    if (energies) energies[0] = E;
+    for (int s = 0; s < nsteps; ++s) {
+        for (int i = 0; i < n; ++i)
+            for (int q = 0; q < dim; ++q) {
+                size_t t = 3 * (size_t)i + q;
+                vel[t] = vel[t] + 0.5 * dt * force[t];
+                pos[t] = wrap64(pos[t] + dt * vel[t], box[q]);
+            }
+        rc = orc_energy_force(n, dim, pos, diam, box, kind, eps, sigma, r_cut, shift,
+                              NULL, NULL, 0, force, e_i, &E);
+        if (rc) break;
+        double P = 0.0, FF = 0.0, VV = 0.0;
+        for (int i = 0; i < n; ++i)
+            for (int q = 0; q < dim; ++q) {
+                size_t t = 3 * (size_t)i + q;
+                vel[t] = vel[t] + 0.5 * dt * force[t];
+                P += force[t] * vel[t]; FF += force[t] * force[t]; VV += vel[t] * vel[t];
+            }
+        if (P > 0.0) {
+            double c2 = FF > 0.0 ? alpha * sqrt(VV) / sqrt(FF) : 0.0;
+            for (int i = 0; i < n; ++i)
+                for (int q = 0; q < dim; ++q) {
+                    size_t t = 3 * (size_t)i + q;
+                    vel[t] = (1.0 - alpha) * vel[t] + c2 * force[t];
+                }
+            n_pos += 1;
+            if (n_pos > (int)par[2]) {
+                dt = dt * par[3] < par[1] ? dt * par[3] : par[1];
+                alpha = alpha * par[6];
+            }
+        } else {
+            for (size_t t = 0; t < 3 * (size_t)n; ++t) vel[t] = 0.0;
+            n_pos = 0; dt = dt * par[4]; alpha = par[5];
+        }
+        if (energies) energies[s + 1] = E;
+    }
+    state[0] = dt; state[1] = alpha; state[2] = (double)n_pos;
+    free(e_i);
+    return rc;
+}

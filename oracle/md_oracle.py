@@ -161,3 +161,24 @@ def nve_run(pos, vel, force, diam, box, dim, kind, eps, sigma, r_cut, shift, dt,
                              C.c_double(dt), C.c_double(mass), nsteps, use_list,
                              C.c_float(skin), capacity, _pd(en), _pi(stats)), "nve_run")
     return p, v, f, en, stats
+
+
+FIRE_DEFAULT = (0.01, 0.1, 5, 1.1, 0.5, 0.1, 0.99)   # dt_start, dt_max, n_min, f_inc, f_dec, alpha_start, f_alpha
+
+
+def fire_run(pos, vel, diam, box, dim, kind, eps, sigma, r_cut, shift, nsteps, par=FIRE_DEFAULT,
+             state=None, alpha_morse=None):
+    """Returns (pos, vel, force, energies[nsteps+1], state[3] = (dt, alpha, n_pos))."""
+    if alpha_morse is not None:
+        set_morse_alpha(alpha_morse)
+    p = _d(pos3(pos)).copy(); v = _d(pos3(vel)).copy(); f = np.zeros_like(p)
+    b = _d(box)
+    dm = _d(diam) if diam is not None else None
+    pr = _d(par)
+    st = _d(state) if state is not None else np.zeros(3, dtype=np.float64)
+    st = st.copy()
+    en = np.zeros(nsteps + 1, dtype=np.float64)
+    _check(lib().orc_fire_run(p.shape[0], dim, _pd(p), _pd(v), _pd(f), _pd(dm), _pd(b), kind,
+                              C.c_double(eps), C.c_double(sigma), C.c_double(r_cut), shift,
+                              _pd(pr), _pd(st), nsteps, _pd(en)), "fire_run")
+    return p, v, f, en, st

@@ -507,3 +507,60 @@ def test_wrap_convention(orc):
                                 want_energies=False)
     assert np.allclose(p[0], [0.04, 4.96, 2.5], atol=1e-12)
     assert np.all(p >= 0) and np.all(p < box)
+
+
+# ------------------------------------------------------------------ FIRE --
+
+def test_fire_schedule_closed_form(orc):
+    """While P = F.v > 0 the FIRE bookkeeping is a closed form: n_pos = k, and from the (n_min+1)-th
+    step on dt grows by f_inc (capped at dt_max) and alpha shrinks by f_alpha.  Two overlapping
+    soft disks released from rest roll downhill for the whole run."""
+    d = 1.0
+    box = np.array([10.0, 10.0, 1.0])
+    pos = np.array([[4.0, 5.0, 0.0], [4.3, 5.0, 0.0]])          # overlap: r = 0.3 d
+    vel = np.zeros((2, 3))
+    par = (1e-3, 4e-3, 5, 1.1, 0.5, 0.1, 0.99)
+    for k in (1, 5, 6, 12, 30):
+        _, v, f, en, st = orc.fire_run(pos, vel, np.array([d, d]), box, 2, SOFT, 1.0, 1.0, 1.0, 0, k, par=par)
+        grow = max(0, k - 5)
+        assert st[2] == k
+        assert abs(st[0] - min(1e-3 * 1.1 ** grow, 4e-3)) < 1e-15
+        assert abs(st[1] - 0.1 * 0.99 ** grow) < 1e-15
+        assert en[-1] < en[0] and v[0, 0] < 0 < v[1, 0]          # moving apart, energy released
+
+
+def test_fire_uphill_start_is_reset(orc):
+    """Velocities pointing up the energy gradient: P < 0 on the first step, so v = 0, dt is cut by
+    f_dec, alpha returns to alpha_start and n_pos to 0."""
+    box = np.array([10.0, 10.0, 1.0])
+    pos = np.array([[4.0, 5.0, 0.0], [4.6, 5.0, 0.0]])
+    vel = np.array([[0.5, 0.0, 0.0], [-0.5, 0.0, 0.0]])          # approaching: against the repulsion
+    par = (1e-3, 4e-3, 5, 1.1, 0.5, 0.1, 0.99)
+    _, v, _, _, st = orc.fire_run(pos, vel, np.array([1.0, 1.0]), box, 2, SOFT, 1.0, 1.0, 1.0, 0, 1, par=par)
+    assert np.abs(v).max() == 0.0 and st[2] == 0 and abs(st[0] - 5e-4) < 1e-18 and st[1] == 0.1
+
+
+def test_fire_without_mixing_is_velocity_verlet(orc, W):
+    """alpha_start = 0, f_inc = 1: the mixing and the schedule are switched off and, as long as
+    P > 0, FIRE is plain velocity Verlet -- the oracle's NVE loop (P7, P8 pin that one)."""
+    w = W.soft_disks(1, 256)
+    diam = w.pos[:, 3].astype(np.float64)
+    par = (2e-3, 2e-3, 5, 1.0, 0.5, 0.0, 1.0)
+    p, v, f, en, st = orc.fire_run(w.pos, w.vel, diam, w.box, 2, SOFT, 1.0, 1.0, 1.4, 0, 25, par=par)
+    assert st[2] == 25                                            # P > 0 throughout (released from rest)
+    f0, _, _ = orc.energy_force(w.pos, diam, w.box, 2, SOFT, 1.0, 1.0, 1.4, 0)
+    p2, v2, f2, _, _ = orc.nve_run(w.pos, w.vel, f0, diam, w.box, 2, SOFT, 1.0, 1.0, 1.4, 0, 2e-3, 1.0, 25,
+                                   want_energies=False)
+    assert np.abs(p - p2).max() < 1e-13 and np.abs(v - v2).max() < 1e-13
+
+
+def test_fire_relaxes_a_packing(orc, W):
+    """Section 4.2's use: the bidisperse soft-disk packing relaxes -- the energy
+    falls by more than an order of magnitude and the largest force with it."""
+    w = W.soft_disks(1, 512)
+    diam = w.pos[:, 3].astype(np.float64)
+    f0, _, E0 = orc.energy_force(w.pos, diam, w.box, 2, SOFT, 1.0, 1.0, 1.4, 0)
+    p, v, f, en, st = orc.fire_run(w.pos, w.vel, diam, w.box, 2, SOFT, 1.0, 1.0, 1.4, 0, 300)
+    assert en[0] == E0 and en[-1] < 0.05 * E0
+    assert np.abs(f).max() < 0.1 * np.abs(f0).max()
+    assert ((p[:, :2] >= 0) & (p[:, :2] < w.box[:2])).all()
