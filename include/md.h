@@ -193,6 +193,31 @@ int md_nve_step(md_system *sys, const md_potential *pot, void *pos, void *vel, v
                 int32_t *id, int32_t *nbr_idx, int32_t *nbr_count, float dt, float mass,
                 int nsteps, int32_t *stats, void *stream);
 
+/* FIRE parameters (Bitzek et al. 2006; the paper names "FIRE Descent", L100, and uses it in §4.2). */
+typedef struct md_fire_params {
+    float dt_start, dt_max;   /* first step size; cap */
+    int   n_min;              /* steps with P > 0 before dt grows */
+    float f_inc, f_dec;       /* growth (>= 1) and cut (in (0,1)) of dt */
+    float alpha_start;        /* mixing parameter after a reset, in [0,1) */
+    float f_alpha;            /* its decay per growing step, in (0,1] */
+} md_fire_params;
+
+/*
+ * nsteps of FIRE minimisation (L100, L322) with unit mass, around the same drift /
+ * device-side rebuild / force sequence as md_nve_step:
+ *   v += dt/2 F;  r = wrap(r + dt v);  [rebuild];  F = F(r);  v += dt/2 F;
+ *   P = sum F.v:  P > 0: v = (1-alpha) v + alpha |v| F/|F|, n_pos += 1, and once n_pos > n_min
+ *   dt = min(dt f_inc, dt_max), alpha *= f_alpha;  else v = 0, n_pos = 0, dt *= f_dec,
+ *   alpha = alpha_start.
+ *   fire_state  device float[4] in/out = {dt, alpha, n_pos, sign of the last P}; dt <= 0 on entry
+ *               starts from (dt_start, alpha_start, 0); pass it back unchanged to continue a run
+ *   force       must hold F(pos) on entry, holds F of the final positions on exit; the lists as in
+ *               md_nve_step; stats as in md_nve_step.  Kernels are launched directly (no graph).
+ */
+int md_fire_minimize(md_system *sys, const md_potential *pot, const md_fire_params *par, void *pos,
+                     void *vel, void *force, int32_t *id, int32_t *nbr_idx, int32_t *nbr_count,
+                     float *fire_state, int nsteps, int32_t *stats, void *stream);
+
 /*
  * End-to-end convenience over HOST buffers: copies pos/vel in, builds the lists, evaluates F,
  * runs nsteps of md_nve_step and copies the state back un-permuted (original particle order).

@@ -21,7 +21,7 @@ SYMBOLS = [
     "md_last_error", "md_workspace_bytes", "md_create", "md_destroy", "md_set_option",
     "md_num_cells", "md_nbr_layout", "md_cell_list_build", "md_neighbor_list_build",
     "md_needs_rebuild", "md_pair_energy_force", "md_nve_step", "md_nve_run_host", "md_counters",
-    "md_nve_run_host_release",
+    "md_nve_run_host_release", "md_fire_minimize",
 ]
 
 
@@ -33,6 +33,12 @@ class md_config(C.Structure):
 class md_potential(C.Structure):
     _fields_ = [("kind", C.c_int), ("epsilon", C.c_float), ("sigma", C.c_float),
                 ("r_cut", C.c_float), ("shift", C.c_int), ("alpha", C.c_float)]
+
+
+class md_fire_params(C.Structure):
+    _fields_ = [("dt_start", C.c_float), ("dt_max", C.c_float), ("n_min", C.c_int),
+                ("f_inc", C.c_float), ("f_dec", C.c_float), ("alpha_start", C.c_float),
+                ("f_alpha", C.c_float)]
 
 
 class MdError(RuntimeError):
@@ -63,6 +69,8 @@ def lib():
         L.md_destroy.argtypes = [vp]
         L.md_set_option.argtypes = [vp, C.c_char_p, C.c_double]
         L.md_counters.argtypes = [vp, ip, C.c_int, vp]
+        L.md_fire_minimize.argtypes = [vp, C.POINTER(md_potential), C.POINTER(md_fire_params), vp, vp, vp,
+                                       ip, ip, ip, vp, C.c_int, ip, vp]
         L.md_num_cells.argtypes = [vp, C.POINTER(C.c_int * 3)]
         L.md_nbr_layout.argtypes = [vp] + [C.POINTER(C.c_long)] * 5
         L.md_cell_list_build.argtypes = [vp, vp, vp, ip, ip, ip, vp]
@@ -139,6 +147,13 @@ def md_destroy(sys) -> None:
 
 def md_set_option(sys, name: str, value: float) -> None:
     _check(lib().md_set_option(sys, name.encode(), float(value)))
+
+
+def md_fire_minimize(sys, pot: md_potential, par: md_fire_params, pos, vel, force, id, nbr_idx, nbr_count,
+                     fire_state, nsteps, stats, stream=None) -> None:
+    _check(lib().md_fire_minimize(sys, C.byref(pot), C.byref(par), _ptr(pos), _ptr(vel), _ptr(force),
+                                  _ptr(id), _ptr(nbr_idx), _ptr(nbr_count), _ptr(fire_state), int(nsteps),
+                                  _ptr(stats), _stream(stream)))
 
 
 def md_nve_run_host_release() -> None:

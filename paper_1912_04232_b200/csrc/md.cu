@@ -5,6 +5,7 @@
 #include "md_kernels.cuh"
 #include "md_force32.cuh"
 #include "md_nbr2.cuh"
+#include "md_fire.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -70,6 +71,7 @@ struct md_system {
     int *words;          // [0] rebuild flag (even steps of a fused graph), [1..2] internal status,
                          // [3] rebuild flag (odd steps), [8..15] counters
     int *scan_tmp;       // block sums + ticket of the two-launch cell scan
+    double *fire_tmp;    // md_fire_minimize: per-block partial sums, then {c1, c2} as floats
     int *cell_count, *cell_start_i, *perm_i, *cell_of, *rank_tmp, *perm_tmp, *id_s;
     float4 *pos_s, *vel_s, *ref_pos, *pos_alt;   // pos_alt: second position buffer of the fused step
     // tuning
@@ -101,7 +103,7 @@ int enter(const md_system *s) {
 }
 
 struct Layout {
-    size_t words, scan_tmp, cell_count, cell_start_i, perm_i, cell_of, rank_tmp, perm_tmp, id_s, pos_s,
+    size_t words, scan_tmp, fire_tmp, cell_count, cell_start_i, perm_i, cell_of, rank_tmp, perm_tmp, id_s, pos_s,
         vel_s, ref_pos, pos_alt, total;
 };
 
@@ -111,6 +113,7 @@ Layout layout(int n, long long cells) {
     auto take = [&](size_t bytes) { size_t at = o; o += up(bytes); return at; };
     l.words = take(64 * sizeof(int));
     l.scan_tmp = take((size_t)((cells + SCAN_CHUNK - 1) / SCAN_CHUNK + 2) * sizeof(int));
+    l.fire_tmp = take(((size_t)(n + FIRE_BLOCK - 1) / FIRE_BLOCK * 3 + 2) * sizeof(double));
     l.cell_count = take((size_t)(cells + 4) * sizeof(int));
     l.cell_start_i = take((size_t)(cells + 1) * sizeof(int));
     l.perm_i = take((size_t)n * sizeof(int));
@@ -529,6 +532,7 @@ int md_create(const md_config *cfg, int n, void *workspace, size_t bytes, md_sys
     s->ws = (char *)workspace; s->ws_bytes = bytes;
     s->words = (int *)(s->ws + l.words);
     s->scan_tmp = (int *)(s->ws + l.scan_tmp);
+    s->fire_tmp = (double *)(s->ws + l.fire_tmp);
     s->cell_count = (int *)(s->ws + l.cell_count);
     s->cell_start_i = (int *)(s->ws + l.cell_start_i);
     s->perm_i = (int *)(s->ws + l.perm_i);
@@ -736,6 +740,55 @@ int md_nve_step(md_system *sys, const md_potential *pot, void *pos, void *vel, v
     if (left > 0) {
         if (!sys->exec1) { rc = capture(sys, pp, k, 1, &sys->exec1); if (rc) return rc; }
         for (; left > 0; --left) CU(cudaGraphLaunch(sys->exec1, st));
+    }
+    return MD_OK;
+}
+
+int md_fire_minimize(md_system *sys, const md_potential *pot, const md_fire_params *par, void *pos,
+                     void *vel, void *force, int32_t *id, int32_t *nbr_idx, int32_t *nbr_count,
+                     float *fire_state, int nsteps, int32_t *stats, void *stream) {
+    if (!sys || !par || !pos || !vel || !force || !nbr_idx || !nbr_count || !fire_state || !stats)
+        return fail(MD_EINVAL, "NULL argument");
+    if (!aligned16(pos) || !aligned16(vel) || !aligned16(force)) return fail(MD_EINVAL, "pos/vel/force must be 16-byte aligned");
+    if (!(par->dt_start > 0.0f) || !(par->dt_max >= par->dt_start) || par->n_min < 0 || !(par->f_inc >= 1.0f) ||
+        !(par->f_dec > 0.0f && par->f_dec < 1.0f) || !(par->alpha_start >= 0.0f && par->alpha_start < 1.0f) ||
+        !(par->f_alpha > 0.0f && par->f_alpha <= 1.0f) || nsteps < 0)
+        return fail(MD_EINVAL, "FIRE parameters out of range");
+    Pair pp;
+    int rc = make_pair(sys, pot, &pp);
+    if (rc) return rc;
+    if ((rc = enter(sys))) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const Geom &g = sys->g;
+    const FirePar fp = {par->dt_start, par->dt_max, par->n_min, par->f_inc, par->f_dec, par->alpha_start, par->f_alpha};
+    int *flag = sys->words + 0, *status = sys->words + 1;
+    const bool resort = sys->cfg.resort != 0;
+    const int nb = blocks_for(g.n), nbr = blocks_for(g.n, FIRE_BLOCK);
+    double *partial = sys->fire_tmp;
+    float *coef = reinterpret_cast<float *>(sys->fire_tmp + (size_t)nbr * 3);
+    float4 *p4 = (float4 *)pos, *v4 = (float4 *)vel, *f4 = (float4 *)force;
+    k_init_stats<<<1, 1, 0, st>>>(stats, sys->words + 0);
+    LAUNCH_OK();
+    k_fire_init<<<1, 1, 0, st>>>(fp, fire_state);
+    LAUNCH_OK();
+    for (int s = 0; s < nsteps; ++s) {
+        if (g.dim == 3) k_fire_kick_drift<3><<<nb, 256, 0, st>>>(g, p4, v4, f4, sys->ref_pos, fire_state, flag);
+        else k_fire_kick_drift<2><<<nb, 256, 0, st>>>(g, p4, v4, f4, sys->ref_pos, fire_state, flag);
+        LAUNCH_OK();
+        rc = launch_cell_build(sys, p4, v4, id, sys->cell_start_i, sys->perm_i, status, flag, st);
+        if (rc) return rc;
+        rc = launch_nbr_build(sys, resort ? p4 : sys->pos_s, sys->cell_start_i, resort ? nullptr : sys->perm_i,
+                              nbr_idx, nbr_count, status, flag, 1, st);
+        if (rc) return rc;
+        Book book = {flag, status, stats};
+        rc = launch_force(sys, pp, p4, nbr_idx, nbr_count, f4, nullptr, 0.0f, nullptr, false, book, st);
+        if (rc) return rc;
+        k_fire_kick_reduce<<<nbr, FIRE_BLOCK, 0, st>>>(g.n, g.dim, v4, f4, fire_state, partial);
+        LAUNCH_OK();
+        k_fire_finalize<<<1, 256, 0, st>>>(nbr, partial, fp, fire_state, coef);
+        LAUNCH_OK();
+        k_fire_mix<<<nb, 256, 0, st>>>(g.n, v4, f4, coef);
+        LAUNCH_OK();
     }
     return MD_OK;
 }

@@ -221,6 +221,57 @@ def test_morse_force_energy_and_trajectory(B, orc, W, dim):
     S.close()
 
 
+@pytest.mark.parametrize("which", ["soft2d", "lj3d"])
+def test_fire_minimize_against_the_oracle(B, orc, W, which):
+    """FIRE on the same drift / device-side rebuild / force sequence.  State after 20 /
+    80 steps against the oracle's fp64 FIRE with all-pairs forces: positions to 1e-4, the device-side
+    schedule (dt, alpha, n_pos) and the energy; then the run is continued from the returned state."""
+    if which == "soft2d":
+        w = W.soft_disks(1, 2048)                       # the paper's packing (L293-L305), smaller
+        par = (0.01, 0.1, 5, 1.1, 0.5, 0.1, 0.99)
+        diam = w.pos[:, 3].astype(np.float64)
+    else:
+        w = W.config(0)
+        w = dataclasses.replace(w, vel=np.zeros_like(w.vel))
+        par = (0.002, 0.02, 5, 1.1, 0.5, 0.1, 0.99)
+        diam = None
+    # fp32 state against an fp64 trajectory: in the packing's box (L = 51) one ulp of a position is
+    # 3.8e-6, dt grows to 0.1 and contacts open and close: measured deviation 1.9e-6 after 1 step,
+    # 3.5e-5 after 20, 4.6e-4 after 40.  The LJ lattice (L = 10) is benign.
+    steps = 20 if which == "soft2d" else 80
+    S = B.System(w)
+    S.build(); S.compute_force()
+    fp = B.md_fire_params(par[0], par[1], int(par[2]), par[3], par[4], par[5], par[6])
+    state = torch.zeros(4, dtype=torch.float32, device="cuda")
+    B.md_fire_minimize(S.sys, S.pot, fp, S.pos, S.vel, S.force, S.id, S.nbr_idx, S.nbr_count, state, steps, S.stats)
+    torch.cuda.synchronize()
+    p_o, v_o, f_o, en, st_o = orc.fire_run(w.pos, w.vel, diam, w.box, w.dim, w.kind, w.epsilon, w.sigma,
+                                           w.r_cut, w.shift, steps, par=par)
+    st = state.cpu().numpy()
+    assert int(S.stats[0]) == steps and int(S.stats[2]) == -1
+    assert int(st[2]) == int(st_o[2])
+    assert abs(st[0] - st_o[0]) <= 1e-5 * st_o[0] and abs(st[1] - st_o[1]) <= 1e-5 * st_o[1]
+    d = unpermute(S, S.pos)[:, :w.dim].astype(np.float64) - p_o[:, :w.dim]
+    L = w.box[:w.dim].astype(np.float64)
+    d -= L * np.round(d / L)
+    assert np.abs(d).max() <= 1e-4, np.abs(d).max()
+    # the force md_fire_minimize leaves is F of ITS final positions (forces of two states 1e-5
+    # apart differ by far more than the tolerance near a minimum): state-wise parity
+    f_own, _, _ = orc.energy_force(unpermute(S, S.pos), diam, w.box, w.dim, w.kind, w.epsilon, w.sigma,
+                                   w.r_cut, w.shift)
+    assert force_error(unpermute(S, S.force), f_own) <= FORCE_TOL
+    S.compute_force()
+    E = float(S.energy.cpu()[0])
+    assert abs(E - en[-1]) <= 1e-4 * abs(en[-1]) and en[-1] < en[0]
+    # continuing from the returned state keeps the schedule going (no restart from dt_start)
+    dt_before = float(state[0])
+    B.md_fire_minimize(S.sys, S.pot, fp, S.pos, S.vel, S.force, S.id, S.nbr_idx, S.nbr_count, state, 1, S.stats)
+    torch.cuda.synchronize()
+    assert float(state[0]) in (np.float32(dt_before), np.float32(min(dt_before * par[3], par[1])),
+                               np.float32(dt_before * par[4]))
+    S.close()
+
+
 def test_fast32_dimers_at_the_force_zero(B, orc, W):
     """Isolated pairs around r = 2^(1/6) sigma, where the LJ force changes sign: the coefficient and
     with it sum|coefficient| vanish while the fp32 rounding error does not, so the error estimate
