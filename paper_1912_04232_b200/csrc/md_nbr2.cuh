@@ -42,8 +42,11 @@ __device__ __forceinline__ unsigned push4(unsigned m, float2 a, float2 b) {
 // MAPPED as in k_nbr_build.  incremental != 0 (a rebuild inside md_nve_step): every column
 // already holds the pad value beyond its previous count, so only rows [count, previous count)
 // are re-padded; 0: rows [count, capacity) are written.
+#ifndef MD_NB2_MINBLOCKS
+#define MD_NB2_MINBLOCKS (32 / MD_NB2_WARPS)
+#endif
 template <int DIM, bool MAPPED>
-__global__ void __launch_bounds__(NB2_WARPS * 32, 32 / NB2_WARPS)
+__global__ void __launch_bounds__(NB2_WARPS * 32, MD_NB2_MINBLOCKS)
 k_nbr_build2(Geom g, const float4 *__restrict__ spos, const int *__restrict__ cell_start,
              const int *__restrict__ map, int *__restrict__ nbr_idx, int *__restrict__ nbr_count,
              int *status, float4 *__restrict__ ref_pos, const int *cond, int incremental) {
