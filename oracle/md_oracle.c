@@ -663,3 +663,70 @@ int orc_fire_run(int n, int dim, double *pos, double *vel, double *force, const 
     free(e_i);
     return rc;
 }
+
+/* -------------------------------------------------- Brownian / gradient descent -- */
+
+/*
+ * Counter-based standard normals (SURVEY 8f-f3 "needs a counter-based device RNG"; each side
+ * implements the same generator): key = (seed, step, particle id, pair index c) -> splitmix64
+ * finaliser -> two 24-bit uniforms u1 in (0,1], u2 in [0,1) -> Box-Muller pair
+ *   g0 = sqrt(-2 ln u1) cos(2 pi u2),  g1 = sqrt(-2 ln u1) sin(2 pi u2).
+ * Components x, y come from c = 0, component z from g0 of c = 1.
+ */
+static void orc_normal_pair(uint32_t seed, uint32_t step, uint32_t id, uint32_t c, double *g0, double *g1)
+{
+    uint64_t z = (uint64_t)seed * 0x9E3779B97F4A7C15ull + (uint64_t)step * 0xBF58476D1CE4E5B9ull
+               + (uint64_t)id * 0x94D049BB133111EBull + (uint64_t)c;
+    z ^= z >> 30; z *= 0xBF58476D1CE4E5B9ull;
+    z ^= z >> 27; z *= 0x94D049BB133111EBull;
+    z ^= z >> 31;
+    double u1 = (double)((z >> 40) + 1ull) * (1.0 / 16777216.0);
+    double u2 = (double)((z >> 8) & 0xFFFFFFull) * (1.0 / 16777216.0);
+    double r = sqrt(-2.0 * log(u1)), a = 2.0 * 3.14159265358979323846 * u2;
+    *g0 = r * cos(a); *g1 = r * sin(a);
+}
+
+void orc_normals(uint32_t seed, uint32_t step, int n, int dim, double *out /* n*3 */)
+{
+    for (int i = 0; i < n; ++i) {
+        double g0, g1, g2, g3;
+        orc_normal_pair(seed, step, (uint32_t)i, 0u, &g0, &g1);
+        orc_normal_pair(seed, step, (uint32_t)i, 1u, &g2, &g3);
+        out[3 * (size_t)i] = g0; out[3 * (size_t)i + 1] = g1; out[3 * (size_t)i + 2] = dim == 3 ? g2 : 0.0;
+    }
+}
+
+/*
+ * orc_brownian_run: overdamped (Brownian) dynamics at temperature kT, "Brownian
+ * simulations at constant temperature"; kT = 0 is the paper's "Gradient Descent" (L100).  The paper
+ * gives no formulas: Euler-Maruyama, reading A21.  Per step s (global index step0 + s):
+ *   r_i = wrap(r_i + (dt/gamma) F_i(r) + sqrt(2 kT dt / gamma) xi_i),  xi_i = orc_normals(seed, step, i)
+ * with F by the all-pairs definition.  force holds F of the final positions on exit.
+ */
+int orc_brownian_run(int n, int dim, double *pos, double *force, const double *diam, const double *box,
+                     int kind, double eps, double sigma, double r_cut, int shift, double dt,
+                     double gamma, double kT, uint32_t seed, uint32_t step0, int nsteps, double *energies)
+{
+    if (n <= 0 || (dim != 2 && dim != 3) || dt <= 0.0 || gamma <= 0.0 || kT < 0.0) return ORC_EINVAL;
+    double *e_i = (double *)malloc((size_t)n * sizeof(double));
+    if (!e_i) return ORC_ENOMEM;
+    double E = 0.0;
+    int rc = orc_energy_force(n, dim, pos, diam, box, kind, eps, sigma, r_cut, shift, NULL, NULL, 0, force, e_i, &E);
+    if (energies) energies[0] = E;
+    const double mu = dt / gamma, amp = sqrt(2.0 * kT * dt / gamma);
+    for (int s = 0; s < nsteps && !rc; ++s) {
+        for (int i = 0; i < n; ++i) {
+            double g[4];
+            orc_normal_pair(seed, step0 + (uint32_t)s, (uint32_t)i, 0u, &g[0], &g[1]);
+            orc_normal_pair(seed, step0 + (uint32_t)s, (uint32_t)i, 1u, &g[2], &g[3]);
+            for (int q = 0; q < dim; ++q) {
+                size_t t = 3 * (size_t)i + q;
+                pos[t] = wrap64(pos[t] + mu * force[t] + amp * g[q], box[q]);
+            }
+        }
+        rc = orc_energy_force(n, dim, pos, diam, box, kind, eps, sigma, r_cut, shift, NULL, NULL, 0, force, e_i, &E);
+        if (energies) energies[s + 1] = E;
+    }
+    free(e_i);
+    return rc;
+}

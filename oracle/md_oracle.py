@@ -182,3 +182,26 @@ def fire_run(pos, vel, diam, box, dim, kind, eps, sigma, r_cut, shift, nsteps, p
                               C.c_double(eps), C.c_double(sigma), C.c_double(r_cut), shift,
                               _pd(pr), _pd(st), nsteps, _pd(en)), "fire_run")
     return p, v, f, en, st
+
+
+def normals(seed, step, n, dim):
+    """The counter-based standard normals of step `step` for particles 0..n-1, float64[n,3]."""
+    out = np.zeros((n, 3), dtype=np.float64)
+    lib().orc_normals(C.c_uint32(seed), C.c_uint32(step), n, dim, _pd(out))
+    return out
+
+
+def brownian_run(pos, diam, box, dim, kind, eps, sigma, r_cut, shift, dt, gamma, kT, seed, nsteps,
+                 step0=0, alpha_morse=None):
+    """Returns (pos, force, energies[nsteps+1])."""
+    if alpha_morse is not None:
+        set_morse_alpha(alpha_morse)
+    p = _d(pos3(pos)).copy(); f = np.zeros_like(p)
+    b = _d(box)
+    dm = _d(diam) if diam is not None else None
+    en = np.zeros(nsteps + 1, dtype=np.float64)
+    _check(lib().orc_brownian_run(p.shape[0], dim, _pd(p), _pd(f), _pd(dm), _pd(b), kind, C.c_double(eps),
+                                  C.c_double(sigma), C.c_double(r_cut), shift, C.c_double(dt),
+                                  C.c_double(gamma), C.c_double(kT), C.c_uint32(seed), C.c_uint32(step0),
+                                  nsteps, _pd(en)), "brownian_run")
+    return p, f, en

@@ -564,3 +564,64 @@ def test_fire_relaxes_a_packing(orc, W):
     assert en[0] == E0 and en[-1] < 0.05 * E0
     assert np.abs(f).max() < 0.1 * np.abs(f0).max()
     assert ((p[:, :2] >= 0) & (p[:, :2] < w.box[:2])).all()
+
+
+# ------------------------------------- Brownian / gradient descent --
+
+def test_counter_based_normals(orc):
+    """The generator both sides implement: standard-normal moments, no correlation between
+    components, steps or neighbors, and a pure function of (seed, step, id)."""
+    n = 200000
+    g = orc.normals(11, 5, n, 3)
+    assert np.abs(g.mean(0)).max() < 5 / np.sqrt(n)
+    assert np.abs(g.var(0) - 1).max() < 5 * np.sqrt(2 / n)
+    assert np.abs((g ** 4).mean(0) - 3).max() < 0.1
+    c = np.corrcoef(g.T)
+    assert np.abs(c - np.eye(3)).max() < 5 / np.sqrt(n)
+    g2 = orc.normals(11, 6, n, 3)
+    assert abs(np.corrcoef(g[:, 0], g2[:, 0])[0, 1]) < 5 / np.sqrt(n)
+    assert abs(np.corrcoef(g[:-1, 0], g[1:, 0])[0, 1]) < 5 / np.sqrt(n)
+    assert np.array_equal(g, orc.normals(11, 5, n, 3)) and not np.array_equal(g, orc.normals(12, 5, n, 3))
+    assert np.array_equal(orc.normals(11, 5, 10, 2)[:, 2], np.zeros(10))
+    assert np.array_equal(orc.normals(11, 5, 10, 2)[:, :2], g[:10, :2])
+
+
+def test_brownian_free_diffusion(orc):
+    """No forces (particles farther apart than r_cut): <|dr|^2> = 2 dim (kT/gamma) t."""
+    m = 16
+    g = np.arange(m, dtype=np.float64)
+    pos = np.stack(np.meshgrid(g, g, g, indexing="ij"), -1).reshape(-1, 3) * 3.0 + 1.0
+    box = np.array([3.0 * m] * 3)
+    dt, gamma, kT, steps = 1e-3, 2.0, 0.7, 40
+    p, f, en = orc.brownian_run(pos, None, box, 3, LJ, 1.0, 1.0, 1.2, 1, dt, gamma, kT, 3, steps)
+    assert np.abs(f).max() == 0.0 and np.abs(en).max() == 0.0
+    d = p - pos
+    d -= box * np.round(d / box)
+    msd = (d ** 2).sum(1).mean()
+    want = 2 * 3 * (kT / gamma) * steps * dt
+    assert abs(msd / want - 1) < 5 * np.sqrt(2.0 / (3 * pos.shape[0]))      # chi-square spread
+    # the increments are exactly the generator's normals
+    p1, _, _ = orc.brownian_run(pos, None, box, 3, LJ, 1.0, 1.0, 1.2, 1, dt, gamma, kT, 3, 1, step0=9)
+    assert np.allclose(p1 - pos, np.sqrt(2 * kT * dt / gamma) * orc.normals(3, 9, pos.shape[0], 3), atol=1e-13)
+
+
+def test_gradient_descent_is_brownian_at_zero_temperature(orc, W):
+    """kT = 0: r += (dt/gamma) F ("Gradient Descent").  One step by hand; two
+    overlapping soft disks close their overlap geometrically; a packing's energy only falls."""
+    w = W.soft_disks(1, 512)
+    diam = w.pos[:, 3].astype(np.float64)
+    pos = w.pos[:, :3].astype(np.float64); box = w.box.astype(np.float64)
+    f0, _, E0 = orc.energy_force(pos, diam, box, 2, SOFT, 1.0, 1.0, 1.4, 0)
+    p, f, en = orc.brownian_run(pos, diam, box, 2, SOFT, 1.0, 1.0, 1.4, 0, 0.05, 2.0, 0.0, 1, 1)
+    want = pos + 0.025 * f0
+    want[:, :2] -= box[:2] * np.floor(want[:, :2] / box[:2])
+    assert np.abs(p - want).max() < 1e-13 and en[0] == E0
+    p, f, en = orc.brownian_run(pos, diam, box, 2, SOFT, 1.0, 1.0, 1.4, 0, 0.05, 2.0, 0.0, 1, 60)
+    assert np.all(np.diff(en) <= 0) and en[-1] < 0.5 * en[0]
+    # dimer: overlap delta = d - r obeys delta' = delta (1 - 2 mu eps / d^2)
+    d, mu = 1.0, 0.01
+    box2 = np.array([10.0, 10.0, 1.0])
+    pp = np.array([[4.0, 5.0, 0.0], [4.6, 5.0, 0.0]])
+    q, _, _ = orc.brownian_run(pp, np.array([d, d]), box2, 2, SOFT, 1.0, 1.0, 1.0, 0, mu, 1.0, 0.0, 1, 25)
+    delta = d - (q[1, 0] - q[0, 0])
+    assert abs(delta - 0.4 * (1 - 2 * mu / d ** 2) ** 25) < 1e-13
