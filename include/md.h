@@ -193,6 +193,20 @@ int md_nve_step(md_system *sys, const md_potential *pot, void *pos, void *vel, v
                 int32_t *id, int32_t *nbr_idx, int32_t *nbr_count, float dt, float mass,
                 int nsteps, int32_t *stats, void *stream);
 
+/*
+ * nsteps of overdamped (Brownian) dynamics at temperature kT (L100), kT = 0 being
+ * gradient descent (L100), around the same device-side rebuild / force sequence:
+ *   r_i = wrap(r_i + (dt/gamma) F_i + sqrt(2 kT dt / gamma) xi_i);  [rebuild];  F = F(r)
+ * xi_i: standard normals of a counter-based generator keyed by (seed, step0 + s, id[i], pair
+ * index) -- splitmix64 finaliser, two 24-bit uniforms, Box-Muller -- so a run is reproducible and
+ * independent of the particle order the re-sort leaves; id = NULL keys by slot (resort = 0 only).
+ *   force   must hold F(pos) on entry, holds F of the final positions on exit; there are no
+ *           velocities; lists and stats as in md_nve_step.  Kernels are launched directly (no graph).
+ */
+int md_brownian_step(md_system *sys, const md_potential *pot, void *pos, void *force, int32_t *id,
+                     int32_t *nbr_idx, int32_t *nbr_count, float dt, float gamma, float kT,
+                     uint32_t seed, uint32_t step0, int nsteps, int32_t *stats, void *stream);
+
 /* FIRE parameters (Bitzek et al. 2006; the paper names "FIRE Descent", L100, and uses it in §4.2). */
 typedef struct md_fire_params {
     float dt_start, dt_max;   /* first step size; cap */

@@ -21,7 +21,7 @@ SYMBOLS = [
     "md_last_error", "md_workspace_bytes", "md_create", "md_destroy", "md_set_option",
     "md_num_cells", "md_nbr_layout", "md_cell_list_build", "md_neighbor_list_build",
     "md_needs_rebuild", "md_pair_energy_force", "md_nve_step", "md_nve_run_host", "md_counters",
-    "md_nve_run_host_release", "md_fire_minimize",
+    "md_nve_run_host_release", "md_fire_minimize", "md_brownian_step",
 ]
 
 
@@ -69,6 +69,8 @@ def lib():
         L.md_destroy.argtypes = [vp]
         L.md_set_option.argtypes = [vp, C.c_char_p, C.c_double]
         L.md_counters.argtypes = [vp, ip, C.c_int, vp]
+        L.md_brownian_step.argtypes = [vp, C.POINTER(md_potential), vp, vp, ip, ip, ip, C.c_float, C.c_float,
+                                       C.c_float, C.c_uint32, C.c_uint32, C.c_int, ip, vp]
         L.md_fire_minimize.argtypes = [vp, C.POINTER(md_potential), C.POINTER(md_fire_params), vp, vp, vp,
                                        ip, ip, ip, vp, C.c_int, ip, vp]
         L.md_num_cells.argtypes = [vp, C.POINTER(C.c_int * 3)]
@@ -147,6 +149,13 @@ def md_destroy(sys) -> None:
 
 def md_set_option(sys, name: str, value: float) -> None:
     _check(lib().md_set_option(sys, name.encode(), float(value)))
+
+
+def md_brownian_step(sys, pot: md_potential, pos, force, id, nbr_idx, nbr_count, dt, gamma, kT, seed, step0,
+                     nsteps, stats, stream=None) -> None:
+    _check(lib().md_brownian_step(sys, C.byref(pot), _ptr(pos), _ptr(force), _ptr(id), _ptr(nbr_idx),
+                                  _ptr(nbr_count), float(dt), float(gamma), float(kT), int(seed), int(step0),
+                                  int(nsteps), _ptr(stats), _stream(stream)))
 
 
 def md_fire_minimize(sys, pot: md_potential, par: md_fire_params, pos, vel, force, id, nbr_idx, nbr_count,

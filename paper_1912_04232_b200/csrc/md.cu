@@ -6,6 +6,7 @@
 #include "md_force32.cuh"
 #include "md_nbr2.cuh"
 #include "md_fire.cuh"
+#include "md_brownian.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -740,6 +741,42 @@ int md_nve_step(md_system *sys, const md_potential *pot, void *pos, void *vel, v
     if (left > 0) {
         if (!sys->exec1) { rc = capture(sys, pp, k, 1, &sys->exec1); if (rc) return rc; }
         for (; left > 0; --left) CU(cudaGraphLaunch(sys->exec1, st));
+    }
+    return MD_OK;
+}
+
+int md_brownian_step(md_system *sys, const md_potential *pot, void *pos, void *force, int32_t *id,
+                     int32_t *nbr_idx, int32_t *nbr_count, float dt, float gamma, float kT,
+                     uint32_t seed, uint32_t step0, int nsteps, int32_t *stats, void *stream) {
+    if (!sys || !pos || !force || !nbr_idx || !nbr_count || !stats) return fail(MD_EINVAL, "NULL argument");
+    if (!aligned16(pos) || !aligned16(force)) return fail(MD_EINVAL, "pos/force must be 16-byte aligned");
+    if (!(dt > 0.0f) || !(gamma > 0.0f) || !(kT >= 0.0f) || nsteps < 0)
+        return fail(MD_EINVAL, "dt and gamma must be positive, kT and nsteps non-negative");
+    Pair pp;
+    int rc = make_pair(sys, pot, &pp);
+    if (rc) return rc;
+    if ((rc = enter(sys))) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const Geom &g = sys->g;
+    int *flag = sys->words + 0, *status = sys->words + 1;
+    const bool resort = sys->cfg.resort != 0;
+    const int nb = blocks_for(g.n);
+    const float mu = dt / gamma, amp = std::sqrt(2.0f * kT * dt / gamma);
+    float4 *p4 = (float4 *)pos, *f4 = (float4 *)force;
+    k_init_stats<<<1, 1, 0, st>>>(stats, sys->words + 0);
+    LAUNCH_OK();
+    for (int s = 0; s < nsteps; ++s) {
+        if (g.dim == 3) k_brownian_drift<3><<<nb, 256, 0, st>>>(g, p4, f4, id, sys->ref_pos, mu, amp, seed, step0 + (uint32_t)s, flag);
+        else k_brownian_drift<2><<<nb, 256, 0, st>>>(g, p4, f4, id, sys->ref_pos, mu, amp, seed, step0 + (uint32_t)s, flag);
+        LAUNCH_OK();
+        rc = launch_cell_build(sys, p4, nullptr, id, sys->cell_start_i, sys->perm_i, status, flag, st);
+        if (rc) return rc;
+        rc = launch_nbr_build(sys, resort ? p4 : sys->pos_s, sys->cell_start_i, resort ? nullptr : sys->perm_i,
+                              nbr_idx, nbr_count, status, flag, 1, st);
+        if (rc) return rc;
+        Book book = {flag, status, stats};
+        rc = launch_force(sys, pp, p4, nbr_idx, nbr_count, f4, nullptr, 0.0f, nullptr, false, book, st);
+        if (rc) return rc;
     }
     return MD_OK;
 }

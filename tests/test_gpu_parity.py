@@ -272,6 +272,48 @@ def test_fire_minimize_against_the_oracle(B, orc, W, which):
     S.close()
 
 
+@pytest.mark.parametrize("which", ["lj3d_kT", "soft2d_descent"])
+def test_brownian_and_gradient_descent_against_the_oracle(B, orc, W, which):
+    """Brownian dynamics (and gradient descent, kT = 0) with the noise of the shared
+    counter-based generator, keyed by the original particle id so the re-sort does not matter."""
+    if which == "lj3d_kT":
+        w, diam, dt, gamma, kT, steps = W.config(0), None, 2e-4, 1.0, 0.8, 60
+    else:
+        w = W.soft_disks(1, 2048)
+        diam, dt, gamma, kT, steps = w.pos[:, 3].astype(np.float64), 0.02, 1.0, 0.0, 30
+    seed = 77
+    S = B.System(w)
+    S.build(); S.compute_force()
+    # one step: the increment is (dt/gamma) F + amp * xi(id)
+    f0 = unpermute(S, S.force)[:, :w.dim].astype(np.float64)
+    B.md_brownian_step(S.sys, S.pot, S.pos, S.force, S.id, S.nbr_idx, S.nbr_count, dt, gamma, kT, seed, 5, 1, S.stats)
+    torch.cuda.synchronize()
+    L = w.box[:w.dim].astype(np.float64)
+    d = unpermute(S, S.pos)[:, :w.dim].astype(np.float64) - w.pos[:, :w.dim]
+    d -= L * np.round(d / L)
+    want = dt / gamma * f0 + np.sqrt(2 * kT * dt / gamma) * orc.normals(seed, 5, w.n, w.dim)[:, :w.dim]
+    assert np.abs(d - want).max() <= 2e-6 * max(1.0, float(L.max()) / 10)     # fp32 positions
+    S.close()
+    # a run against the oracle
+    S = B.System(w)
+    S.build(); S.compute_force()
+    B.md_brownian_step(S.sys, S.pot, S.pos, S.force, S.id, S.nbr_idx, S.nbr_count, dt, gamma, kT, seed, 0, steps, S.stats)
+    torch.cuda.synchronize()
+    p_o, f_o, en = orc.brownian_run(w.pos, diam, w.box, w.dim, w.kind, w.epsilon, w.sigma, w.r_cut, w.shift,
+                                    dt, gamma, kT, seed, steps)
+    assert int(S.stats[0]) == steps and int(S.stats[2]) == -1
+    d = unpermute(S, S.pos)[:, :w.dim].astype(np.float64) - p_o[:, :w.dim]
+    d -= L * np.round(d / L)
+    assert np.abs(d).max() <= 1e-4, np.abs(d).max()
+    f_own, _, _ = orc.energy_force(unpermute(S, S.pos), diam, w.box, w.dim, w.kind, w.epsilon, w.sigma,
+                                   w.r_cut, w.shift)
+    assert force_error(unpermute(S, S.force), f_own) <= FORCE_TOL
+    if kT == 0.0:
+        S.compute_force()
+        assert abs(float(S.energy.cpu()[0]) - en[-1]) <= 1e-4 * abs(en[-1]) and en[-1] < en[0]
+    S.close()
+
+
 def test_fast32_dimers_at_the_force_zero(B, orc, W):
     """Isolated pairs around r = 2^(1/6) sigma, where the LJ force changes sign: the coefficient and
     with it sum|coefficient| vanish while the fp32 rounding error does not, so the error estimate
