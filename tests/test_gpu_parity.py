@@ -533,15 +533,16 @@ def test_nve_run_host_matches_device_path(B, W):
     S.close()
 
 
+@pytest.mark.parametrize("resort", [1, 0])
 @pytest.mark.parametrize("ci,steps", [(0, 100), (2, 120)])
-def test_fused_step_same_bits(B, W, ci, steps):
+def test_fused_step_same_bits(B, W, ci, steps, resort):
     """The fused graph (force kernel opens the next step, positions ping-pong between two buffers)
     and the plain sequence k_kick_drift -> rebuild -> force give the same bits and the same
     rebuild history, for step counts that exercise both the 9-step and the 1-step graph."""
     w = W.config(ci)
     out = []
     for fused, graph in ((1, 1), (0, 1), (0, 0)):
-        S = B.System(w)
+        S = B.System(w, resort=resort)
         B.md_set_option(S.sys, "fused", fused)
         B.md_set_option(S.sys, "use_graph", graph)
         S.build(); S.compute_force(); S.step(steps)
