@@ -730,3 +730,50 @@ int orc_brownian_run(int n, int dim, double *pos, double *force, const double *d
     free(e_i);
     return rc;
 }
+
+/* ------------------------------------------------------------- Langevin -- */
+
+/*
+ * orc_langevin_run: Langevin dynamics at temperature kT ("Langevin ... simulations
+ * at constant temperature"; no formulas in the paper: the BAOAB splitting, reading A22).
+ * Per step s (global index step0 + s), a = dt/(2m):
+ *   B: v += a F;  A: r += dt/2 v;  O: v = c1 v + c2 xi, c1 = exp(-gamma dt), c2 = sqrt(kT/m (1 - c1^2));
+ *   A: r = wrap(r + dt/2 v);  F = F(r);  B: v += a F
+ * xi = orc_normals(seed, step, i).  gamma = 0 (c1 = 1, c2 = 0) is velocity Verlet.  All-pairs forces;
+ * force must hold F(pos) on entry.
+ */
+int orc_langevin_run(int n, int dim, double *pos, double *vel, double *force, const double *diam,
+                     const double *box, int kind, double eps, double sigma, double r_cut, int shift,
+                     double dt, double mass, double gamma, double kT, uint32_t seed, uint32_t step0,
+                     int nsteps)
+{
+    if (n <= 0 || (dim != 2 && dim != 3) || dt <= 0.0 || mass <= 0.0 || gamma < 0.0 || kT < 0.0) return ORC_EINVAL;
+    double *e_i = (double *)malloc((size_t)n * sizeof(double));
+    if (!e_i) return ORC_ENOMEM;
+    const double a = dt / (2.0 * mass), c1 = exp(-gamma * dt), c2 = sqrt(kT / mass * (1.0 - c1 * c1));
+    double E = 0.0;
+    int rc = ORC_OK;
+    for (int s = 0; s < nsteps && !rc; ++s) {
+        for (int i = 0; i < n; ++i) {
+            double g[4];
+            orc_normal_pair(seed, step0 + (uint32_t)s, (uint32_t)i, 0u, &g[0], &g[1]);
+            orc_normal_pair(seed, step0 + (uint32_t)s, (uint32_t)i, 1u, &g[2], &g[3]);
+            for (int q = 0; q < dim; ++q) {
+                size_t t = 3 * (size_t)i + q;
+                double v = vel[t] + a * force[t];
+                double r = pos[t] + 0.5 * dt * v;
+                v = c1 * v + c2 * g[q];
+                pos[t] = wrap64(r + 0.5 * dt * v, box[q]);
+                vel[t] = v;
+            }
+        }
+        rc = orc_energy_force(n, dim, pos, diam, box, kind, eps, sigma, r_cut, shift, NULL, NULL, 0, force, e_i, &E);
+        for (int i = 0; i < n; ++i)
+            for (int q = 0; q < dim; ++q) {
+                size_t t = 3 * (size_t)i + q;
+                vel[t] = vel[t] + a * force[t];
+            }
+    }
+    free(e_i);
+    return rc;
+}

@@ -205,3 +205,16 @@ def brownian_run(pos, diam, box, dim, kind, eps, sigma, r_cut, shift, dt, gamma,
                                   C.c_double(gamma), C.c_double(kT), C.c_uint32(seed), C.c_uint32(step0),
                                   nsteps, _pd(en)), "brownian_run")
     return p, f, en
+
+
+def langevin_run(pos, vel, force, diam, box, dim, kind, eps, sigma, r_cut, shift, dt, mass, gamma, kT,
+                 seed, nsteps, step0=0):
+    """BAOAB Langevin; returns (pos, vel, force)."""
+    p = _d(pos3(pos)).copy(); v = _d(pos3(vel)).copy(); f = _d(pos3(force)).copy()
+    b = _d(box)
+    dm = _d(diam) if diam is not None else None
+    _check(lib().orc_langevin_run(p.shape[0], dim, _pd(p), _pd(v), _pd(f), _pd(dm), _pd(b), kind,
+                                  C.c_double(eps), C.c_double(sigma), C.c_double(r_cut), shift,
+                                  C.c_double(dt), C.c_double(mass), C.c_double(gamma), C.c_double(kT),
+                                  C.c_uint32(seed), C.c_uint32(step0), nsteps), "langevin_run")
+    return p, v, f

@@ -625,3 +625,40 @@ def test_gradient_descent_is_brownian_at_zero_temperature(orc, W):
     q, _, _ = orc.brownian_run(pp, np.array([d, d]), box2, 2, SOFT, 1.0, 1.0, 1.0, 0, mu, 1.0, 0.0, 1, 25)
     delta = d - (q[1, 0] - q[0, 0])
     assert abs(delta - 0.4 * (1 - 2 * mu / d ** 2) ** 25) < 1e-13
+
+
+# ---------------------------------------------------------- Langevin --
+
+def test_langevin_without_bath_is_velocity_verlet(orc, W):
+    """gamma = 0: c1 = 1, c2 = 0 and BAOAB is kick-drift-kick velocity Verlet (the NVE oracle)."""
+    w = W.lj_fcc(0, 3, seed=4)
+    f0, _, _ = orc.energy_force(w.pos, None, w.box, 3, LJ, 1.0, 1.0, 2.5, 1)
+    p, v, f = orc.langevin_run(w.pos, w.vel, f0, None, w.box, 3, LJ, 1.0, 1.0, 2.5, 1, 0.004, 1.0, 0.0, 0.7, 5, 30)
+    p2, v2, f2, _, _ = orc.nve_run(w.pos, w.vel, f0, None, w.box, 3, LJ, 1.0, 1.0, 2.5, 1, 0.004, 1.0, 30,
+                                   want_energies=False)
+    assert np.abs(p - p2).max() < 1e-12 and np.abs(v - v2).max() < 1e-11
+
+
+def test_langevin_free_particles(orc):
+    """No forces.  kT = 0: v_n = v_0 exp(-gamma dt)^n exactly.  kT > 0: the O step keeps the
+    Maxwell-Boltzmann variance kT/m stationary, and from rest <v^2> = kT/m (1 - c1^(2n))."""
+    m_ = 16
+    g = np.arange(m_, dtype=np.float64)
+    pos = np.stack(np.meshgrid(g, g, g, indexing="ij"), -1).reshape(-1, 3) * 3.0 + 1.0
+    box = np.array([3.0 * m_] * 3)
+    n = pos.shape[0]
+    f0 = np.zeros((n, 3))
+    rng = np.random.default_rng(2)
+    v0 = rng.normal(0, 1.0, (n, 3))
+    dt, mass, gamma, steps = 5e-3, 2.0, 3.0, 40
+    _, v, f = orc.langevin_run(pos, v0, f0, None, box, 3, LJ, 1.0, 1.0, 1.2, 1, dt, mass, gamma, 0.0, 1, steps)
+    assert np.abs(f).max() == 0.0
+    assert np.abs(v - v0 * np.exp(-gamma * dt) ** steps).max() < 1e-13
+    kT = 0.9
+    _, v, _ = orc.langevin_run(pos, np.zeros((n, 3)), f0, None, box, 3, LJ, 1.0, 1.0, 1.2, 1, dt, mass, gamma, kT, 1, steps)
+    want = kT / mass * (1 - np.exp(-2 * gamma * dt * steps))
+    assert abs((v ** 2).mean() / want - 1) < 5 * np.sqrt(2.0 / (3 * n))
+    # one O step from rest is c2 * xi
+    _, v1, _ = orc.langevin_run(pos, np.zeros((n, 3)), f0, None, box, 3, LJ, 1.0, 1.0, 1.2, 1, dt, mass, gamma, kT, 1, 1, step0=4)
+    c1 = np.exp(-gamma * dt)
+    assert np.allclose(v1, np.sqrt(kT / mass * (1 - c1 * c1)) * orc.normals(1, 4, n, 3), atol=1e-14)
