@@ -207,6 +207,19 @@ int md_brownian_step(md_system *sys, const md_potential *pot, void *pos, void *f
                      int32_t *nbr_idx, int32_t *nbr_count, float dt, float gamma, float kT,
                      uint32_t seed, uint32_t step0, int nsteps, int32_t *stats, void *stream);
 
+/*
+ * nsteps of Langevin dynamics at temperature kT (L100), BAOAB splitting:
+ *   v += dt/(2m) F;  r += dt/2 v;  v = c1 v + c2 xi (c1 = exp(-gamma dt), c2 = sqrt(kT/m (1-c1^2)));
+ *   r = wrap(r + dt/2 v);  [rebuild];  F = F(r);  v += dt/(2m) F
+ * xi as in md_brownian_step (same generator, keyed by seed, step0 + s, id[i]).  gamma = 0 is
+ * md_nve_step's velocity Verlet.  force must hold F(pos) on entry; lists and stats as in md_nve_step.
+ * Kernels are launched directly (no graph).
+ */
+int md_langevin_step(md_system *sys, const md_potential *pot, void *pos, void *vel, void *force,
+                     int32_t *id, int32_t *nbr_idx, int32_t *nbr_count, float dt, float mass,
+                     float gamma, float kT, uint32_t seed, uint32_t step0, int nsteps, int32_t *stats,
+                     void *stream);
+
 /* FIRE parameters (Bitzek et al. 2006; the paper names "FIRE Descent", L100, and uses it in §4.2). */
 typedef struct md_fire_params {
     float dt_start, dt_max;   /* first step size; cap */

@@ -781,6 +781,45 @@ int md_brownian_step(md_system *sys, const md_potential *pot, void *pos, void *f
     return MD_OK;
 }
 
+int md_langevin_step(md_system *sys, const md_potential *pot, void *pos, void *vel, void *force,
+                     int32_t *id, int32_t *nbr_idx, int32_t *nbr_count, float dt, float mass,
+                     float gamma, float kT, uint32_t seed, uint32_t step0, int nsteps, int32_t *stats,
+                     void *stream) {
+    if (!sys || !pos || !vel || !force || !nbr_idx || !nbr_count || !stats) return fail(MD_EINVAL, "NULL argument");
+    if (!aligned16(pos) || !aligned16(vel) || !aligned16(force)) return fail(MD_EINVAL, "pos/vel/force must be 16-byte aligned");
+    if (!(dt > 0.0f) || !(mass > 0.0f) || !(gamma >= 0.0f) || !(kT >= 0.0f) || nsteps < 0)
+        return fail(MD_EINVAL, "dt and mass must be positive, gamma, kT and nsteps non-negative");
+    Pair pp;
+    int rc = make_pair(sys, pot, &pp);
+    if (rc) return rc;
+    if ((rc = enter(sys))) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const Geom &g = sys->g;
+    int *flag = sys->words + 0, *status = sys->words + 1;
+    const bool resort = sys->cfg.resort != 0;
+    const int nb = blocks_for(g.n);
+    const float a = dt / (2.0f * mass);
+    const double c1d = std::exp(-(double)gamma * (double)dt);
+    const float c1 = (float)c1d, c2 = (float)std::sqrt((double)kT / (double)mass * (1.0 - c1d * c1d));
+    float4 *p4 = (float4 *)pos, *v4 = (float4 *)vel, *f4 = (float4 *)force;
+    k_init_stats<<<1, 1, 0, st>>>(stats, sys->words + 0);
+    LAUNCH_OK();
+    for (int s = 0; s < nsteps; ++s) {
+        if (g.dim == 3) k_langevin_baoa<3><<<nb, 256, 0, st>>>(g, p4, v4, f4, id, sys->ref_pos, a, dt, c1, c2, seed, step0 + (uint32_t)s, flag);
+        else k_langevin_baoa<2><<<nb, 256, 0, st>>>(g, p4, v4, f4, id, sys->ref_pos, a, dt, c1, c2, seed, step0 + (uint32_t)s, flag);
+        LAUNCH_OK();
+        rc = launch_cell_build(sys, p4, v4, id, sys->cell_start_i, sys->perm_i, status, flag, st);
+        if (rc) return rc;
+        rc = launch_nbr_build(sys, resort ? p4 : sys->pos_s, sys->cell_start_i, resort ? nullptr : sys->perm_i,
+                              nbr_idx, nbr_count, status, flag, 1, st);
+        if (rc) return rc;
+        Book book = {flag, status, stats};
+        rc = launch_force(sys, pp, p4, nbr_idx, nbr_count, f4, v4, a, nullptr, false, book, st);
+        if (rc) return rc;
+    }
+    return MD_OK;
+}
+
 int md_fire_minimize(md_system *sys, const md_potential *pot, const md_fire_params *par, void *pos,
                      void *vel, void *force, int32_t *id, int32_t *nbr_idx, int32_t *nbr_count,
                      float *fire_state, int nsteps, int32_t *stats, void *stream) {

@@ -51,4 +51,42 @@ k_brownian_drift(Geom g, float4 *__restrict__ pos, const float4 *__restrict__ fo
     if (__any_sync(FULL, moved) && (threadIdx.x & 31) == 0) *flag = 1;
 }
 
+// Langevin dynamics, BAOAB (reading A22), first four letters:
+//   B: v += a F;  A: r += dt/2 v;  O: v = c1 v + c2 xi;  A: r = mu(r, dt/2 v);  half-skin test.
+// The force kernel that follows applies the closing B (its second half-kick).
+template <int DIM>
+__global__ void __launch_bounds__(256)
+k_langevin_baoa(Geom g, float4 *__restrict__ pos, float4 *__restrict__ vel,
+                const float4 *__restrict__ force, const int *__restrict__ id,
+                const float4 *__restrict__ ref, float a, float dt, float c1, float c2,
+                unsigned seed, unsigned step, int *flag) {
+    int i = blockIdx.x * blockDim.x + threadIdx.x;
+    bool moved = false;
+    if (i < g.n) {
+        float4 p = pos[i], v = vel[i];
+        const float4 f = force[i];
+        float gx = 0.0f, gy = 0.0f, gz = 0.0f, unused;
+        if (c2 != 0.0f) {
+            const unsigned key = (unsigned)(id ? id[i] : i);
+            normal_pair(seed, step, key, 0u, gx, gy);
+            if (DIM == 3) normal_pair(seed, step, key, 1u, gz, unused);
+        }
+        const float hdt = 0.5f * dt;
+        v.x = fmaf(a, f.x, v.x); v.y = fmaf(a, f.y, v.y);
+        float rx = fmaf(hdt, v.x, p.x), ry = fmaf(hdt, v.y, p.y);
+        v.x = fmaf(c2, gx, c1 * v.x); v.y = fmaf(c2, gy, c1 * v.y);
+        p.x = wrap(fmaf(hdt, v.x, rx), g.L[0], g.inv_L[0]);
+        p.y = wrap(fmaf(hdt, v.y, ry), g.L[1], g.inv_L[1]);
+        if (DIM == 3) {
+            v.z = fmaf(a, f.z, v.z);
+            const float rz = fmaf(hdt, v.z, p.z);
+            v.z = fmaf(c2, gz, c1 * v.z);
+            p.z = wrap(fmaf(hdt, v.z, rz), g.L[2], g.inv_L[2]);
+        }
+        pos[i] = p; vel[i] = v;
+        moved = disp2_from_ref<DIM>(g, p, ref[i]) > g.half_skin2;
+    }
+    if (__any_sync(FULL, moved) && (threadIdx.x & 31) == 0) *flag = 1;
+}
+
 } // namespace mdk

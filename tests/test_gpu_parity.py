@@ -314,6 +314,39 @@ def test_brownian_and_gradient_descent_against_the_oracle(B, orc, W, which):
     S.close()
 
 
+def test_langevin_against_the_oracle(B, orc, W):
+    """BAOAB Langevin with the shared counter-based noise.  60 steps of the 3-D LJ
+    system against the oracle; gamma = 0 must reproduce md_nve_step bit for bit."""
+    w = W.config(0)
+    dt, mass, gamma, kT, seed, steps = 0.004, 1.0, 2.0, 0.8, 9, 60
+    S = B.System(w)
+    S.build(); S.compute_force()
+    f0 = unpermute(S, S.force)[:, :3].astype(np.float64)
+    B.md_langevin_step(S.sys, S.pot, S.pos, S.vel, S.force, S.id, S.nbr_idx, S.nbr_count, dt, mass, gamma, kT,
+                       seed, 0, steps, S.stats)
+    torch.cuda.synchronize()
+    p_o, v_o, _ = orc.langevin_run(w.pos, w.vel, f0, None, w.box, 3, 0, 1.0, 1.0, 2.5, 1, dt, mass, gamma, kT, seed, steps)
+    assert int(S.stats[0]) == steps and int(S.stats[1]) >= 3 and int(S.stats[2]) == -1
+    L = w.box.astype(np.float64)
+    d = unpermute(S, S.pos)[:, :3].astype(np.float64) - p_o
+    d -= L * np.round(d / L)
+    assert np.abs(d).max() <= 1e-4, np.abs(d).max()
+    assert np.abs(unpermute(S, S.vel)[:, :3] - v_o).max() <= 2e-3
+    S.close()
+    A, N = B.System(w), B.System(w)
+    for X in (A, N):
+        X.build(); X.compute_force()
+    B.md_langevin_step(A.sys, A.pot, A.pos, A.vel, A.force, A.id, A.nbr_idx, A.nbr_count, w.dt, w.mass, 0.0, 0.8,
+                       seed, 0, 40, A.stats)
+    B.md_set_option(N.sys, "fused", 0)
+    N.step(40)
+    torch.cuda.synchronize()
+    # BAOAB with c1 = 1, c2 = 0 drifts in two half steps (one more rounding than r += dt v): close, not equal
+    dd = (A.pos - N.pos)[:, :3].abs().max().item()
+    assert dd <= 2e-5 and torch.equal(A.id, N.id)
+    A.close(); N.close()
+
+
 def test_fast32_dimers_at_the_force_zero(B, orc, W):
     """Isolated pairs around r = 2^(1/6) sigma, where the LJ force changes sign: the coefficient and
     with it sum|coefficient| vanish while the fp32 rounding error does not, so the error estimate
