@@ -777,3 +777,70 @@ int orc_langevin_run(int n, int dim, double *pos, double *vel, double *force, co
     free(e_i);
     return rc;
 }
+
+/* ---------------------------------------------------------- Nose-Hoover -- */
+
+/*
+ * orc_nose_hoover_run: NVT by a Nose-Hoover thermostat ("Nose-Hoover [67]"; no
+ * formulas in the paper: one thermostat variable, the explicit reversible splitting of Martyna,
+ * Tuckerman, Tobias and Klein around the velocity-Verlet step, reading A23).
+ * dof = dim n, Q = dof kT tau^2.  Thermostat half step T(dt):
+ *   K2 = sum m v^2;  G = (K2 - dof kT)/Q;  vxi += dt/4 G;  s = exp(-dt/2 vxi);  v *= s;
+ *   xi += dt/2 vxi;  K2 *= s^2;  G = (K2 - dof kT)/Q;  vxi += dt/4 G
+ * Step: T(dt);  v += dt/(2m) F;  r = wrap(r + dt v);  F = F(r);  v += dt/(2m) F;  T(dt).
+ * Conserved: H' = K + U + Q vxi^2 / 2 + dof kT xi.
+ *   state in/out double[2] = {xi, vxi};  conserved out (may be NULL) double[nsteps+1] = H'
+ */
+static void nh_half(int n, int dim, double *vel, double mass, double dofkT, double Q, double dt,
+                    double *xi, double *vxi)
+{
+    double K2 = 0.0;
+    for (int i = 0; i < n; ++i)
+        for (int q = 0; q < dim; ++q) K2 += mass * vel[3 * (size_t)i + q] * vel[3 * (size_t)i + q];
+    double G = (K2 - dofkT) / Q;
+    *vxi += 0.25 * dt * G;
+    double sc = exp(-0.5 * dt * *vxi);
+    for (int i = 0; i < n; ++i)
+        for (int q = 0; q < dim; ++q) vel[3 * (size_t)i + q] *= sc;
+    *xi += 0.5 * dt * *vxi;
+    K2 *= sc * sc;
+    G = (K2 - dofkT) / Q;
+    *vxi += 0.25 * dt * G;
+}
+
+int orc_nose_hoover_run(int n, int dim, double *pos, double *vel, double *force, const double *diam,
+                        const double *box, int kind, double eps, double sigma, double r_cut, int shift,
+                        double dt, double mass, double kT, double tau, double *state, int nsteps,
+                        double *conserved)
+{
+    if (n <= 0 || (dim != 2 && dim != 3) || dt <= 0.0 || mass <= 0.0 || kT <= 0.0 || tau <= 0.0 || !state)
+        return ORC_EINVAL;
+    double *e_i = (double *)malloc((size_t)n * sizeof(double));
+    if (!e_i) return ORC_ENOMEM;
+    const double dofkT = (double)dim * n * kT, Q = dofkT * tau * tau, a = dt / (2.0 * mass);
+    double xi = state[0], vxi = state[1], E = 0.0;
+    int rc = orc_energy_force(n, dim, pos, diam, box, kind, eps, sigma, r_cut, shift, NULL, NULL, 0, force, e_i, &E);
+    for (int s = 0; s <= nsteps && !rc; ++s) {
+        if (conserved) {
+            double K2 = 0.0;
+            for (int i = 0; i < n; ++i)
+                for (int q = 0; q < dim; ++q) K2 += mass * vel[3 * (size_t)i + q] * vel[3 * (size_t)i + q];
+            conserved[s] = 0.5 * K2 + E + 0.5 * Q * vxi * vxi + dofkT * xi;
+        }
+        if (s == nsteps) break;
+        nh_half(n, dim, vel, mass, dofkT, Q, dt, &xi, &vxi);
+        for (int i = 0; i < n; ++i)
+            for (int q = 0; q < dim; ++q) {
+                size_t t = 3 * (size_t)i + q;
+                vel[t] += a * force[t];
+                pos[t] = wrap64(pos[t] + dt * vel[t], box[q]);
+            }
+        rc = orc_energy_force(n, dim, pos, diam, box, kind, eps, sigma, r_cut, shift, NULL, NULL, 0, force, e_i, &E);
+        for (int i = 0; i < n; ++i)
+            for (int q = 0; q < dim; ++q) vel[3 * (size_t)i + q] += a * force[3 * (size_t)i + q];
+        nh_half(n, dim, vel, mass, dofkT, Q, dt, &xi, &vxi);
+    }
+    state[0] = xi; state[1] = vxi;
+    free(e_i);
+    return rc;
+}

@@ -218,3 +218,18 @@ def langevin_run(pos, vel, force, diam, box, dim, kind, eps, sigma, r_cut, shift
                                   C.c_double(dt), C.c_double(mass), C.c_double(gamma), C.c_double(kT),
                                   C.c_uint32(seed), C.c_uint32(step0), nsteps), "langevin_run")
     return p, v, f
+
+
+def nose_hoover_run(pos, vel, diam, box, dim, kind, eps, sigma, r_cut, shift, dt, mass, kT, tau, nsteps,
+                    state=None):
+    """Returns (pos, vel, force, conserved[nsteps+1], state[2] = (xi, v_xi))."""
+    p = _d(pos3(pos)).copy(); v = _d(pos3(vel)).copy(); f = np.zeros_like(p)
+    b = _d(box)
+    dm = _d(diam) if diam is not None else None
+    st = (_d(state) if state is not None else np.zeros(2, dtype=np.float64)).copy()
+    cons = np.zeros(nsteps + 1, dtype=np.float64)
+    _check(lib().orc_nose_hoover_run(p.shape[0], dim, _pd(p), _pd(v), _pd(f), _pd(dm), _pd(b), kind,
+                                     C.c_double(eps), C.c_double(sigma), C.c_double(r_cut), shift,
+                                     C.c_double(dt), C.c_double(mass), C.c_double(kT), C.c_double(tau),
+                                     _pd(st), nsteps, _pd(cons)), "nose_hoover_run")
+    return p, v, f, cons, st

@@ -662,3 +662,37 @@ def test_langevin_free_particles(orc):
     _, v1, _ = orc.langevin_run(pos, np.zeros((n, 3)), f0, None, box, 3, LJ, 1.0, 1.0, 1.2, 1, dt, mass, gamma, kT, 1, 1, step0=4)
     c1 = np.exp(-gamma * dt)
     assert np.allclose(v1, np.sqrt(kT / mass * (1 - c1 * c1)) * orc.normals(1, 4, n, 3), atol=1e-14)
+
+
+# ------------------------------------------------------- Nose-Hoover --
+
+def test_nose_hoover_decoupled_is_nve(orc, W):
+    """tau -> infinity: Q -> infinity, the thermostat never moves and the step is velocity Verlet."""
+    w = W.lj_fcc(0, 3, seed=6)
+    f0, _, _ = orc.energy_force(w.pos, None, w.box, 3, LJ, 1.0, 1.0, 2.5, 1)
+    p, v, f, cons, st = orc.nose_hoover_run(w.pos, w.vel, None, w.box, 3, LJ, 1.0, 1.0, 2.5, 1, 0.004, 1.0, 0.5, 1e9, 30)
+    p2, v2, _, _, _ = orc.nve_run(w.pos, w.vel, f0, None, w.box, 3, LJ, 1.0, 1.0, 2.5, 1, 0.004, 1.0, 30,
+                                  want_energies=False)
+    assert np.abs(p - p2).max() < 1e-10 and np.abs(v - v2).max() < 1e-10 and abs(st[1]) < 1e-12
+
+
+def test_nose_hoover_conserved_quantity_and_temperature(orc, W):
+    """H' = K + U + Q v_xi^2/2 + dof kT xi is conserved to second order in dt (halving dt cuts its
+    excursion ~4x), and the thermostat drives the kinetic temperature toward kT: started at T = 1
+    with target 0.4 the time-averaged temperature of the second half lies near the target."""
+    w = W.lj_fcc(0, 3, seed=8)                      # 108 particles, T = 1
+    kT, tau = 0.4, 0.1
+    out = {}
+    for dt, steps in ((0.004, 400), (0.002, 800)):
+        p, v, f, cons, st = orc.nose_hoover_run(w.pos, w.vel, None, w.box, 3, LJ, 1.0, 1.0, 2.5, 1, dt, 1.0, kT, tau, steps)
+        out[dt] = np.abs(cons - cons[0]).max()
+    assert out[0.004] < 2e-3 * abs(cons[0]) + 0.05
+    assert 2.5 < out[0.004] / out[0.002] < 6.0
+    # temperature: run in chunks and average the second half
+    state, pos, vel, temps = None, w.pos, w.vel, []
+    for chunk in range(40):
+        pos4 = np.zeros((w.n, 4), np.float32); pos4[:, :3] = pos[:, :3]
+        p, v, f, cons, state = orc.nose_hoover_run(pos, vel, None, w.box, 3, LJ, 1.0, 1.0, 2.5, 1, 0.004, 1.0, kT, tau, 25, state=state)
+        temps.append((v ** 2).sum() / (3 * w.n))
+        pos, vel = p, v
+    assert abs(np.mean(temps[20:]) - kT) < 0.1 * kT
