@@ -220,6 +220,20 @@ int md_langevin_step(md_system *sys, const md_potential *pot, void *pos, void *v
                      float gamma, float kT, uint32_t seed, uint32_t step0, int nsteps, int32_t *stats,
                      void *stream);
 
+/*
+ * nsteps of NVT by one Nose-Hoover thermostat (L100 [67]) around the velocity-Verlet
+ * step, Martyna-Tuckerman-Tobias-Klein splitting; dof = dim n, Q = dof kT tau^2:
+ *   T(dt);  v += dt/(2m) F;  r = wrap(r + dt v);  [rebuild];  F = F(r);  v += dt/(2m) F;  T(dt)
+ *   T(dt): K2 = sum m v^2; G = (K2 - dof kT)/Q; vxi += dt/4 G; v *= exp(-dt/2 vxi); xi += dt/2 vxi;
+ *          K2 *= exp(-dt vxi); G = (K2 - dof kT)/Q; vxi += dt/4 G
+ *   nh_state  device double[2] in/out = {xi, vxi} (zero to start); H' = K + U + Q vxi^2/2 + dof kT xi
+ *             is the conserved quantity
+ * force must hold F(pos) on entry; lists and stats as in md_nve_step.  Direct launches (no graph).
+ */
+int md_nose_hoover_step(md_system *sys, const md_potential *pot, void *pos, void *vel, void *force,
+                        int32_t *id, int32_t *nbr_idx, int32_t *nbr_count, float dt, float mass,
+                        float kT, float tau, double *nh_state, int nsteps, int32_t *stats, void *stream);
+
 /* FIRE parameters (Bitzek et al. 2006; the paper names "FIRE Descent", L100, and uses it in §4.2). */
 typedef struct md_fire_params {
     float dt_start, dt_max;   /* first step size; cap */

@@ -22,7 +22,7 @@ SYMBOLS = [
     "md_num_cells", "md_nbr_layout", "md_cell_list_build", "md_neighbor_list_build",
     "md_needs_rebuild", "md_pair_energy_force", "md_nve_step", "md_nve_run_host", "md_counters",
     "md_nve_run_host_release", "md_fire_minimize", "md_brownian_step",
-    "md_langevin_step",
+    "md_langevin_step", "md_nose_hoover_step",
 ]
 
 
@@ -74,6 +74,8 @@ def lib():
                                        C.c_float, C.c_uint32, C.c_uint32, C.c_int, ip, vp]
         L.md_langevin_step.argtypes = [vp, C.POINTER(md_potential), vp, vp, vp, ip, ip, ip, C.c_float, C.c_float,
                                        C.c_float, C.c_float, C.c_uint32, C.c_uint32, C.c_int, ip, vp]
+        L.md_nose_hoover_step.argtypes = [vp, C.POINTER(md_potential), vp, vp, vp, ip, ip, ip, C.c_float,
+                                          C.c_float, C.c_float, C.c_float, vp, C.c_int, ip, vp]
         L.md_fire_minimize.argtypes = [vp, C.POINTER(md_potential), C.POINTER(md_fire_params), vp, vp, vp,
                                        ip, ip, ip, vp, C.c_int, ip, vp]
         L.md_num_cells.argtypes = [vp, C.POINTER(C.c_int * 3)]
@@ -166,6 +168,13 @@ def md_langevin_step(sys, pot: md_potential, pos, vel, force, id, nbr_idx, nbr_c
     _check(lib().md_langevin_step(sys, C.byref(pot), _ptr(pos), _ptr(vel), _ptr(force), _ptr(id),
                                   _ptr(nbr_idx), _ptr(nbr_count), float(dt), float(mass), float(gamma),
                                   float(kT), int(seed), int(step0), int(nsteps), _ptr(stats), _stream(stream)))
+
+
+def md_nose_hoover_step(sys, pot: md_potential, pos, vel, force, id, nbr_idx, nbr_count, dt, mass, kT, tau,
+                        nh_state, nsteps, stats, stream=None) -> None:
+    _check(lib().md_nose_hoover_step(sys, C.byref(pot), _ptr(pos), _ptr(vel), _ptr(force), _ptr(id),
+                                     _ptr(nbr_idx), _ptr(nbr_count), float(dt), float(mass), float(kT),
+                                     float(tau), _ptr(nh_state), int(nsteps), _ptr(stats), _stream(stream)))
 
 
 def md_fire_minimize(sys, pot: md_potential, par: md_fire_params, pos, vel, force, id, nbr_idx, nbr_count,

@@ -7,6 +7,7 @@
 #include "md_nbr2.cuh"
 #include "md_fire.cuh"
 #include "md_brownian.cuh"
+#include "md_nh.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -816,6 +817,52 @@ int md_langevin_step(md_system *sys, const md_potential *pot, void *pos, void *v
         Book book = {flag, status, stats};
         rc = launch_force(sys, pp, p4, nbr_idx, nbr_count, f4, v4, a, nullptr, false, book, st);
         if (rc) return rc;
+    }
+    return MD_OK;
+}
+
+int md_nose_hoover_step(md_system *sys, const md_potential *pot, void *pos, void *vel, void *force,
+                        int32_t *id, int32_t *nbr_idx, int32_t *nbr_count, float dt, float mass,
+                        float kT, float tau, double *nh_state, int nsteps, int32_t *stats, void *stream) {
+    if (!sys || !pos || !vel || !force || !nbr_idx || !nbr_count || !nh_state || !stats)
+        return fail(MD_EINVAL, "NULL argument");
+    if (!aligned16(pos) || !aligned16(vel) || !aligned16(force)) return fail(MD_EINVAL, "pos/vel/force must be 16-byte aligned");
+    if (!(dt > 0.0f) || !(mass > 0.0f) || !(kT > 0.0f) || !(tau > 0.0f) || nsteps < 0)
+        return fail(MD_EINVAL, "dt, mass, kT and tau must be positive, nsteps non-negative");
+    Pair pp;
+    int rc = make_pair(sys, pot, &pp);
+    if (rc) return rc;
+    if ((rc = enter(sys))) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    const Geom &g = sys->g;
+    int *flag = sys->words + 0, *status = sys->words + 1;
+    const bool resort = sys->cfg.resort != 0;
+    const int nb = blocks_for(g.n), nbk = blocks_for(g.n, NH_BLOCK);
+    const float a = dt / (2.0f * mass);
+    const double dofkT = (double)g.dim * g.n * (double)kT, Q = dofkT * (double)tau * (double)tau;
+    double *partial = sys->fire_tmp;
+    float *scale = reinterpret_cast<float *>(sys->fire_tmp + nbk);
+    float4 *p4 = (float4 *)pos, *v4 = (float4 *)vel, *f4 = (float4 *)force;
+    k_init_stats<<<1, 1, 0, st>>>(stats, sys->words + 0);
+    LAUNCH_OK();
+    for (int s = 0; s < nsteps; ++s) {
+        k_nh_ke<<<nbk, NH_BLOCK, 0, st>>>(g.n, g.dim, v4, partial);
+        k_nh_finalize<<<1, 256, 0, st>>>(nbk, partial, (double)mass, dofkT, Q, (double)dt, nh_state, scale);
+        if (g.dim == 3) k_nh_kick_drift<3><<<nb, 256, 0, st>>>(g, p4, v4, f4, sys->ref_pos, a, dt, scale, flag);
+        else k_nh_kick_drift<2><<<nb, 256, 0, st>>>(g, p4, v4, f4, sys->ref_pos, a, dt, scale, flag);
+        LAUNCH_OK();
+        rc = launch_cell_build(sys, p4, v4, id, sys->cell_start_i, sys->perm_i, status, flag, st);
+        if (rc) return rc;
+        rc = launch_nbr_build(sys, resort ? p4 : sys->pos_s, sys->cell_start_i, resort ? nullptr : sys->perm_i,
+                              nbr_idx, nbr_count, status, flag, 1, st);
+        if (rc) return rc;
+        Book book = {flag, status, stats};
+        rc = launch_force(sys, pp, p4, nbr_idx, nbr_count, f4, v4, a, nullptr, false, book, st);
+        if (rc) return rc;
+        k_nh_ke<<<nbk, NH_BLOCK, 0, st>>>(g.n, g.dim, v4, partial);
+        k_nh_finalize<<<1, 256, 0, st>>>(nbk, partial, (double)mass, dofkT, Q, (double)dt, nh_state, scale);
+        k_nh_scale<<<nb, 256, 0, st>>>(g.n, v4, scale);
+        LAUNCH_OK();
     }
     return MD_OK;
 }

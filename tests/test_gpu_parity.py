@@ -347,6 +347,39 @@ def test_langevin_against_the_oracle(B, orc, W):
     A.close(); N.close()
 
 
+def test_nose_hoover_against_the_oracle(B, orc, W):
+    """Nose-Hoover NVT (MTK splitting, thermostat state on the device).  80 steps of
+    the 3-D LJ system quenched from T = 1 toward kT = 0.5 against the oracle: positions, velocities
+    and the thermostat variables; the run split in two calls continues from the returned state."""
+    w = W.config(0)
+    dt, mass, kT, tau, steps = 0.004, 1.0, 0.5, 0.2, 80
+    S = B.System(w)
+    S.build(); S.compute_force()
+    state = torch.zeros(2, dtype=torch.float64, device="cuda")
+    B.md_nose_hoover_step(S.sys, S.pot, S.pos, S.vel, S.force, S.id, S.nbr_idx, S.nbr_count, dt, mass, kT, tau,
+                          state, steps, S.stats)
+    torch.cuda.synchronize()
+    p_o, v_o, f_o, cons, st_o = orc.nose_hoover_run(w.pos, w.vel, None, w.box, 3, 0, 1.0, 1.0, 2.5, 1, dt, mass, kT, tau, steps)
+    assert int(S.stats[0]) == steps and int(S.stats[1]) >= 3 and int(S.stats[2]) == -1
+    st = state.cpu().numpy()
+    assert np.abs(st - st_o).max() <= 1e-4 * np.abs(st_o).max()
+    L = w.box.astype(np.float64)
+    d = unpermute(S, S.pos)[:, :3].astype(np.float64) - p_o
+    d -= L * np.round(d / L)
+    assert np.abs(d).max() <= 1e-4, np.abs(d).max()
+    assert np.abs(unpermute(S, S.vel)[:, :3] - v_o).max() <= 2e-3
+    assert (v_o ** 2).sum() < 0.8 * (w.vel[:, :3].astype(np.float64) ** 2).sum()      # it did cool
+    S2 = B.System(w)
+    S2.build(); S2.compute_force()
+    state2 = torch.zeros(2, dtype=torch.float64, device="cuda")
+    for k in (30, 50):
+        B.md_nose_hoover_step(S2.sys, S2.pot, S2.pos, S2.vel, S2.force, S2.id, S2.nbr_idx, S2.nbr_count, dt, mass,
+                              kT, tau, state2, k, S2.stats)
+    torch.cuda.synchronize()
+    assert torch.equal(S2.pos, S.pos) and torch.equal(S2.vel, S.vel) and torch.equal(state2, state)
+    S.close(); S2.close()
+
+
 def test_fast32_dimers_at_the_force_zero(B, orc, W):
     """Isolated pairs around r = 2^(1/6) sigma, where the LJ force changes sign: the coefficient and
     with it sum|coefficient| vanish while the fp32 rounding error does not, so the error estimate
