@@ -55,6 +55,7 @@
 #define KIND_LJ 0
 #define KIND_SOFT 1
 #define KIND_MORSE 2
+#define KIND_BUCK 3
 
 int orc_num_threads(void)
 {
@@ -399,6 +400,16 @@ static void morse_pair(double r, double D, double r0, double alpha, double *u, d
     *fr = r > 0.0 ? -2.0 * D * alpha * x * (1.0 - x) / r : 0.0;
 }
 
+/* Buckingham-type u(r) = A exp(-B r) - C / r^6 and -u'(r)/r (PAPER.md:L104 [71-73]; the paper names
+ * the family only: the exp-6 form without the Coulomb term of BKS, reading A24).
+ * A = eps, B = the alpha of orc_set_morse_alpha, C = sigma. */
+static void buck_pair(double r, double A, double B, double Cc, double *u, double *fr)
+{
+    double x = A * exp(-B * r), r2 = r * r, r6 = r2 * r2 * r2;
+    *u = x - Cc / r6;
+    *fr = r > 0.0 ? (B * x - 6.0 * Cc / (r6 * r)) / r : 0.0;
+}
+
 static double lj_u_cut(double eps, double sigma, double r_cut)
 {
     double u, fr;
@@ -414,6 +425,8 @@ static double lj_u_cut(double eps, double sigma, double r_cut)
  *                (PAPER.md:L301); r = 0 gives energy eps/2 and zero force
  *   kind 2 MORSE: u = eps (1 - exp(-alpha (r - sigma)))^2 - eps - shift*u(r_cut) for r < r_cut,
  *                alpha set by orc_set_morse_alpha (PAPER.md:L104 [75])
+ *   kind 3 BUCKINGHAM: u = eps exp(-alpha r) - sigma / r^6 - shift*u(r_cut) for r < r_cut
+ *                (A = eps, B = alpha, C = sigma; PAPER.md:L104 [71-73])
  *   nbr_idx == NULL: all pairs j != i (the definition);
  *   else: over the list rows (L80 smap.neighbors), entries >= n are padding.
  *   force double[n*3] (z = 0 in 2-D), e_i double[n], *E double.
@@ -425,12 +438,16 @@ int orc_energy_force(int n, int dim, const double *pos, const double *diam,
                      double *e_i, double *E)
 {
     if (n <= 0 || (dim != 2 && dim != 3)) return ORC_EINVAL;
-    if (kind != KIND_LJ && kind != KIND_SOFT && kind != KIND_MORSE) return ORC_EINVAL;
+    if (kind != KIND_LJ && kind != KIND_SOFT && kind != KIND_MORSE && kind != KIND_BUCK) return ORC_EINVAL;
     if (kind == KIND_SOFT && !diam) return ORC_EINVAL;
     double u_c = (kind == KIND_LJ && shift) ? lj_u_cut(eps, sigma, r_cut) : 0.0;
     if (kind == KIND_MORSE && shift) {
         double fr_unused;
         morse_pair(r_cut, eps, sigma, g_morse_alpha, &u_c, &fr_unused);
+    }
+    if (kind == KIND_BUCK && shift) {
+        double fr_unused;
+        buck_pair(r_cut, eps, g_morse_alpha, sigma, &u_c, &fr_unused);
     }
 #pragma omp parallel for schedule(dynamic, 64)
     for (int i = 0; i < n; ++i) {
@@ -448,6 +465,13 @@ int orc_energy_force(int n, int dim, const double *pos, const double *diam,
                 if (r2 < r_cut * r_cut) {
                     double u, fr;
                     lj_pair(r2, eps, sigma, &u, &fr);
+                    e += 0.5 * (u - u_c);
+                    for (int q = 0; q < dim; ++q) f[q] += fr * d[q];
+                }
+            } else if (kind == KIND_BUCK) {
+                if (r2 < r_cut * r_cut) {
+                    double u, fr;
+                    buck_pair(sqrt(r2), eps, g_morse_alpha, sigma, &u, &fr);
                     e += 0.5 * (u - u_c);
                     for (int q = 0; q < dim; ++q) f[q] += fr * d[q];
                 }

@@ -696,3 +696,37 @@ def test_nose_hoover_conserved_quantity_and_temperature(orc, W):
         temps.append((v ** 2).sum() / (3 * w.n))
         pos, vel = p, v
     assert abs(np.mean(temps[20:]) - kT) < 0.1 * kT
+
+
+# ------------------------------------------------- Buckingham --
+
+def test_buckingham_two_body_and_gradient(orc, W):
+    """u = A exp(-B r) - C / r^6 (PAPER.md:L104 [71-73]): closed form at one distance, the force as
+    -u'(r) with its sign, shifted cutoff, and -grad E by central differences on a lattice."""
+    BUCK = 3
+    A, Bc, Cc, rc = 1000.0, 9.0, 1.5, 2.5
+    r = 1.3
+    pos, box, _ = two_body(r, 0)
+    f, e_i, E0 = orc.energy_force(pos, None, box, 3, BUCK, A, Cc, rc, 0, alpha=Bc)
+    u = A * np.exp(-Bc * r) - Cc / r ** 6
+    du = -A * Bc * np.exp(-Bc * r) + 6 * Cc / r ** 7
+    assert abs(E0 - u) < 1e-13 and abs(f[0, 0] - du) < 1e-12 and abs(f[1, 0] + du) < 1e-12
+    _, _, E1 = orc.energy_force(pos, None, box, 3, BUCK, A, Cc, rc, 1, alpha=Bc)
+    assert abs(E1 - (u - (A * np.exp(-Bc * rc) - Cc / rc ** 6))) < 1e-13
+    pos, box, _ = two_body(rc * (1 + 1e-9), 0)
+    assert orc.energy_force(pos, None, box, 3, BUCK, A, Cc, rc, 1, alpha=Bc)[2] == 0.0
+    w = W.lj_fcc(0, 3, seed=13)
+    pos, box = w.pos[:, :3].astype(np.float64), w.box.astype(np.float64)
+    args = (BUCK, A, Cc, rc, 1)
+    f, _, _ = orc.energy_force(pos, None, box, 3, *args, alpha=Bc)
+    assert np.abs(f.sum(0)).max() < 1e-10 * np.abs(f).sum()
+    rng = np.random.default_rng(4)
+    h, worst = 1e-5, 0.0
+    for i in rng.choice(pos.shape[0], 6, replace=False):
+        for q in range(3):
+            pp = pos.copy(); pp[i, q] += h
+            pm = pos.copy(); pm[i, q] -= h
+            fd = -(orc.energy_force(pp, None, box, 3, *args, alpha=Bc)[2]
+                   - orc.energy_force(pm, None, box, 3, *args, alpha=Bc)[2]) / (2 * h)
+            worst = max(worst, abs(fd - f[i, q]) / max(1.0, np.abs(f[i]).max()))
+    assert worst < 1e-6, worst
