@@ -47,6 +47,8 @@ extern "C" {
 #define MD_KIND_LJ   0      /* Lennard-Jones [69], L104 §3.3.2 */
 #define MD_KIND_SOFT 1      /* harmonic soft sphere [70], L104; d_ij = (d_i+d_j)/2, L301 App. A */
 #define MD_KIND_MORSE 2     /* Morse [75], L104: u = eps (1 - exp(-alpha (r - sigma)))^2 - eps */
+#define MD_KIND_BUCKINGHAM 3 /* Buckingham-type exp-6 [71-73], L104: u = eps exp(-alpha r) - sigma / r^6
+                               (epsilon = A, alpha = B, sigma = C) */
 
 typedef struct md_system md_system;   /* opaque; lives in host memory */
 
@@ -163,6 +165,7 @@ int md_needs_rebuild(md_system *sys, const void *pos, int32_t *flag, void *strea
  *   LJ   u = 4 eps[(s/r)^12 - (s/r)^6] - shift*u(r_cut), r < r_cut
  *   SOFT u = eps/2 (1 - r/d_ij)^2, r < d_ij = (pos_i.w + pos_j.w)/2; r = 0: eps/2, no force
  *   MORSE u = eps (1 - exp(-alpha (r - sigma)))^2 - eps - shift*u(r_cut), r < r_cut (fp64 chain)
+ *   BUCKINGHAM u = eps exp(-alpha r) - sigma / r^6 - shift*u(r_cut), r < r_cut (fp64 chain)
  *   force        float4[n] out: (F_i, e_i)
  *   energy_total double* out (may be NULL): sum_i e_i accumulated in fp64
  *   nbr_idx / nbr_count  any list in the md_nbr_layout layout whose rows hold every pair

@@ -168,7 +168,8 @@ int make_geom(const md_config *cfg, int n, Geom *g) {
 
 int make_pair(const md_system *sys, const md_potential *pot, Pair *pp) {
     if (!pot) return fail(MD_EINVAL, "potential is NULL");
-    if (pot->kind != MD_KIND_LJ && pot->kind != MD_KIND_SOFT && pot->kind != MD_KIND_MORSE)
+    if (pot->kind != MD_KIND_LJ && pot->kind != MD_KIND_SOFT && pot->kind != MD_KIND_MORSE &&
+        pot->kind != MD_KIND_BUCKINGHAM)
         return fail(MD_EINVAL, "unknown potential kind %d", pot->kind);
     if (!(pot->epsilon > 0.0f)) return fail(MD_EINVAL, "epsilon must be positive");
     memset(pp, 0, sizeof(*pp));
@@ -188,6 +189,13 @@ int make_pair(const md_system *sys, const md_potential *pot, Pair *pp) {
         const double rc = pot->r_cut, x = std::exp(-(double)pot->alpha * (rc - (double)pot->sigma));
         pp->dalpha = pot->alpha; pp->dr0 = pot->sigma; pp->drc2 = rc * rc; pp->dsig6x2 = 2.0;
         pp->du_cutm = pot->shift ? ((1.0 - x) * (1.0 - x) - 1.0) : 0.0;
+    } else if (pot->kind == MD_KIND_BUCKINGHAM) {
+        if (!(pot->r_cut > 0.0f) || !(pot->sigma >= 0.0f) || !(pot->alpha > 0.0f))
+            return fail(MD_EINVAL, "Buckingham needs alpha (B) > 0, sigma (C) >= 0 and r_cut > 0");
+        if (pot->r_cut > sys->cfg.r_cut) return fail(MD_EINVAL, "potential r_cut %g exceeds the list r_cut %g", pot->r_cut, sys->cfg.r_cut);
+        const double rc = pot->r_cut;
+        pp->dA = pot->epsilon; pp->dalpha = pot->alpha; pp->dC = pot->sigma; pp->drc2 = rc * rc; pp->dsig6x2 = 2.0;
+        pp->du_cutm = pot->shift ? (pp->dA * std::exp(-pp->dalpha * rc) - pp->dC / std::pow(rc, 6.0)) : 0.0;
     } else {
         pp->dsig6x2 = 2.0; pp->drc2 = 1e300;
     }
@@ -313,6 +321,7 @@ int launch_force(md_system *s, const Pair &pp, const float4 *pos, const int *nbr
                                                etot, book, st))
     if (pp.kind == MD_KIND_LJ) return s->g.dim == 3 ? MD_FORCE_DISPATCH(0, 3) : MD_FORCE_DISPATCH(0, 2);
     if (pp.kind == MD_KIND_MORSE) return s->g.dim == 3 ? MD_FORCE_DISPATCH(2, 3) : MD_FORCE_DISPATCH(2, 2);
+    if (pp.kind == MD_KIND_BUCKINGHAM) return s->g.dim == 3 ? MD_FORCE_DISPATCH(3, 3) : MD_FORCE_DISPATCH(3, 2);
     return s->g.dim == 3 ? MD_FORCE_DISPATCH(1, 3) : MD_FORCE_DISPATCH(1, 2);
 #undef MD_FORCE_DISPATCH
 }

@@ -28,7 +28,8 @@ struct Pair {
     double dsig6x2;         // LJ: 2 sigma^6
     double du_cut4;         // LJ: shift * u(r_cut) / (4 eps) = shift * ((s/rc)^12 - (s/rc)^6)
     double dalpha, dr0;     // MORSE: alpha, r0
-    double du_cutm;         // MORSE: shift * u(r_cut) / eps
+    double du_cutm;         // MORSE: shift * u(r_cut) / eps;  BUCKINGHAM: shift * u(r_cut)
+    double dA, dC;          // BUCKINGHAM: A, C (B is dalpha)
 };
 
 // Device words md_nve_step keeps between kernels.
@@ -657,6 +658,21 @@ __device__ __forceinline__ void morse_pair64(const Pair &pp, double dx, double d
     if (ENERGY) a.e += in ? (1.0 - x) * (1.0 - x) - 1.0 - pp.du_cutm : 0.0;
 }
 
+// One pair, Buckingham-type exp-6 [71-73] (L104): u = A exp(-B r) - C / r^6; the force coefficient
+// -u'(r)/r = (A B exp(-B r) - 6 C / r^7) / r.  Nothing is factored out (fs = 1).
+template <bool ENERGY>
+__device__ __forceinline__ void buck_pair64(const Pair &pp, double dx, double dy, double dz,
+                                            bool valid, Acc64 &a) {
+    const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+    const bool in = valid && r2 < pp.drc2 && r2 > 0.0;
+    const double r2s = in ? r2 : 1.0;
+    const double r = sqrt(r2s), x = pp.dA * exp(-pp.dalpha * r);
+    const double y = rcp64(r2s), y3 = y * y * y;                    // 1/r^6
+    const double c = in ? (pp.dalpha * x * r - 6.0 * pp.dC * y3) * y : 0.0;   // (B x r - 6C/r^6)/r^2
+    a.fx = fma(c, dx, a.fx); a.fy = fma(c, dy, a.fy); a.fz = fma(c, dz, a.fz);
+    if (ENERGY) a.e += in ? x - pp.dC * y3 - pp.du_cutm : 0.0;
+}
+
 // Per-thread view of the space for the pair loop.
 template <int DIM>
 struct Me {
@@ -695,6 +711,7 @@ __device__ __forceinline__ void pair_any(const Pair &pp, const Me<DIM> &me, cons
     displacement<DIM, WRAP>(me, q, dx, dy, dz);
     if (KIND == 0) lj_pair64<ENERGY>(pp, dx, dy, dz, valid, acc);
     else if (KIND == 2) morse_pair64<ENERGY>(pp, dx, dy, dz, valid, acc);
+    else if (KIND == 3) buck_pair64<ENERGY>(pp, dx, dy, dz, valid, acc);
     else soft_pair64<ENERGY>(pp, dx, dy, dz, (double)me.pi.w + (double)q.w, valid, acc);
 }
 
@@ -721,8 +738,8 @@ __device__ __forceinline__ void force_epilogue(const Pair &pp, const Acc64 &acc,
                                                float4 *__restrict__ force, float4 *__restrict__ vel,
                                                float a, double *energy_total, const Book &book,
                                                int gid) {
-    const double fs = KIND == 0 ? 12.0 * pp.deps * pp.dsig6x2 : pp.deps;     // 24 eps sig^6 | eps | D
-    const double es = KIND == 0 ? 2.0 * pp.deps : (KIND == 2 ? 0.5 * pp.deps : 0.25 * pp.deps);   // 1/2 * (4 eps | D | eps/2)
+    const double fs = KIND == 0 ? 12.0 * pp.deps * pp.dsig6x2 : (KIND == 3 ? 1.0 : pp.deps);   // 24 eps sig^6 | eps | D | 1
+    const double es = KIND == 0 ? 2.0 * pp.deps : (KIND == 2 ? 0.5 * pp.deps : (KIND == 3 ? 0.5 : 0.25 * pp.deps));   // 1/2 * (4 eps | D | 1 | eps/2)
     const float fx = (float)(fs * acc.fx), fy = (float)(fs * acc.fy), fz = (float)(fs * acc.fz);
     const double e64 = ENERGY ? es * acc.e : 0.0;
     if (owner) {

@@ -29,6 +29,7 @@ RHO_LJ = 0.8442           # LJ number density of configs 0, 2, 3, 4
 KIND_LJ = 0
 KIND_SOFT = 1
 KIND_MORSE = 2
+KIND_BUCKINGHAM = 3
 
 
 @dataclasses.dataclass(frozen=True)

@@ -380,6 +380,31 @@ def test_nose_hoover_against_the_oracle(B, orc, W):
     S.close(); S2.close()
 
 
+def test_buckingham_force_energy_and_trajectory(B, orc, W):
+    """Buckingham-type exp-6 (PAPER.md:L104 [71-73]) on the fp64 pair chain: force and
+    energy against the all-pairs definition, then 100 NVE steps against the oracle."""
+    # exp-6 with alpha = 14, eps = 1, r_m = 1.12: A = 6 eps e^alpha/(alpha-6), B = alpha/r_m, C = eps alpha r_m^6/(alpha-6)
+    A, Bc, Cc, rc = float(np.float32(9.02e5)), float(np.float32(12.5)), float(np.float32(3.454)), 2.5
+    base = W.config(0)
+    w = custom_workload(W, base.pos.copy(), base.box, 3, 3, rc, 0.3, 128, vel=base.vel.copy(), dt=0.004)
+    w = dataclasses.replace(w, epsilon=A, sigma=Cc, alpha=Bc, shift=1)
+    S = B.System(w)
+    S.build(); S.compute_force()
+    f_o, e_o, E_o = orc.energy_force(w.pos, None, w.box, 3, 3, A, Cc, rc, 1, alpha=Bc)
+    f = unpermute(S, S.force)
+    assert force_error(f, f_o) <= FORCE_TOL
+    assert abs(float(S.energy.cpu()[0]) - E_o) <= ENERGY_TOL * abs(E_o)
+    p_o, v_o, _, _, _ = orc.nve_run(w.pos, w.vel, f_o, None, w.box, 3, 3, A, Cc, rc, 1, w.dt, w.mass, 100,
+                                    want_energies=False, alpha=Bc)
+    S.step(100)
+    torch.cuda.synchronize()
+    d = unpermute(S, S.pos)[:, :3].astype(np.float64) - p_o
+    L = w.box.astype(np.float64)
+    d -= L * np.round(d / L)
+    assert np.abs(d).max() <= 1e-4, np.abs(d).max()
+    S.close()
+
+
 def test_fast32_dimers_at_the_force_zero(B, orc, W):
     """Isolated pairs around r = 2^(1/6) sigma, where the LJ force changes sign: the coefficient and
     with it sum|coefficient| vanish while the fp32 rounding error does not, so the error estimate
