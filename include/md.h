@@ -97,6 +97,9 @@ int md_destroy(md_system *sys);
  *   "fused"                1 (default): inside md_nve_step's graph the 3-D LJ force kernel also opens
  *                          the next step (second half-kick, first half-kick, drift into a second
  *                          position buffer, half-skin test); 0: k_kick_drift every step.  Same bits.
+ *   "remap"                3-D LJ force kernel: blocks i and i + remap work on adjacent list tiles, so the
+ *                          blocks one SM receives round-robin share gathered positions in L1 (default
+ *                          37; 0 = block i works on tile block i)
  *   "builder"              neighbor-list kernel: 2 (default) records hits in per-lane bit masks,
  *                          1 appends them to per-lane shared-memory columns (first design)
  *   "use_graph"            0: md_nve_step launches kernels directly instead of a CUDA graph */

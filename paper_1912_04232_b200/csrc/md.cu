@@ -82,6 +82,7 @@ struct md_system {
     size_t nb_smem;      // its dynamic shared memory per block
     int use_graph;
     int fused;           // fused step: the force kernel also opens the next step (graph mode, fast32)
+    int remap;           // force kernel: block -> tile remap period (the SM count), 0 = off
     int builder;         // neighbor-list builder: 2 = bit-mask (md_nbr2.cuh), 1 = column append
     int fast32;          // LJ 3-D: fp32 fast path + fp64 re-evaluation (md_force32.cuh)
     float est_thr;       // its error-estimate threshold
@@ -309,8 +310,10 @@ int launch_force(md_system *s, const Pair &pp, const float4 *pos, const int *nbr
         q.est_thr = s->est_thr;
         const int nb = blocks_for(s->g.n, F32_WARPS * 32);
         int *nfix = s->words + 8;
-        if (want_energy) k_force_lj32<true><<<nb, F32_WARPS * 32, 0, st>>>(s->g, pp, q, pos, nbr_idx, nbr_count, force, vel, a, etot, book, nfix, nx);
-        else k_force_lj32<false><<<nb, F32_WARPS * 32, 0, st>>>(s->g, pp, q, pos, nbr_idx, nbr_count, force, vel, a, etot, book, nfix, nx);
+        int P = 0, grid = nb;
+        if (s->remap > 0 && nb > 4 * s->remap) { P = s->remap; grid = P * ((nb + P - 1) / P); }
+        if (want_energy) k_force_lj32<true><<<grid, F32_WARPS * 32, 0, st>>>(s->g, pp, q, pos, nbr_idx, nbr_count, force, vel, a, etot, book, nfix, nx, P, nb);
+        else k_force_lj32<false><<<grid, F32_WARPS * 32, 0, st>>>(s->g, pp, q, pos, nbr_idx, nbr_count, force, vel, a, etot, book, nfix, nx, P, nb);
         LAUNCH_OK();
         return MD_OK;
     }
@@ -559,6 +562,7 @@ int md_create(const md_config *cfg, int n, void *workspace, size_t bytes, md_sys
     s->use_graph = 1;
     s->fast32 = 1;
     s->builder = 2;
+    s->remap = 37;      // a quarter of the SM count measured best (46.7 -> 44.9 us at N = 256k)
     s->fused = 1;
     s->est_thr = 8.0f;
     s->unroll = 9;      // odd: a fused graph swaps position buffers steps-1 times and must end in the caller's
@@ -640,6 +644,7 @@ int md_set_option(md_system *sys, const char *name, double value) {
     } else if (!strcmp(name, "use_graph")) sys->use_graph = value != 0.0;
     else if (!strcmp(name, "fast32")) sys->fast32 = value != 0.0;
     else if (!strcmp(name, "fused")) sys->fused = value != 0.0;
+    else if (!strcmp(name, "remap")) sys->remap = (int)value;
     else if (!strcmp(name, "builder")) {
         if (value != 1.0 && value != 2.0) return fail(MD_EINVAL, "builder must be 1 or 2");
         sys->builder = (int)value;

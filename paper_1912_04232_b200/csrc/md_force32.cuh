@@ -174,9 +174,18 @@ __global__ void __launch_bounds__(F32_WARPS * 32)
 k_force_lj32(Geom g, Pair pp, Pair32 p32, const float4 *__restrict__ pos,
              const int *__restrict__ nbr_idx, const int *__restrict__ nbr_count,
              float4 *__restrict__ force, float4 *__restrict__ vel, float a, double *energy_total,
-             Book book, int *nfix, NextStep nx) {
+             Book book, int *nfix, NextStep nx, int remap_p, int nblocks) {
     const int lane = threadIdx.x & 31;
-    const int gid = blockIdx.x * blockDim.x + threadIdx.x;
+    // remap_p > 0: the grid has remap_p * Q blocks and block i works on tile block
+    // (i % remap_p) * Q + i / remap_p, so that the blocks the hardware deals round-robin to one SM
+    // are neighbors in space and share their gathers in L1
+    int bid = blockIdx.x;
+    if (remap_p > 0) {
+        const int Q = gridDim.x / remap_p;
+        bid = (bid % remap_p) * Q + bid / remap_p;
+        if (bid >= nblocks) return;
+    }
+    const int gid = bid * blockDim.x + threadIdx.x;
     const int i = gid;
     const bool active = i < g.n;
     const int ii = active ? i : g.n - 1;
