@@ -75,7 +75,7 @@ __device__ __forceinline__ void lj_pair32(const Pair32 &pp, float dx, float dy, 
 
 // Exact re-evaluation of one particle by a group of G = 8, 16 or 32 lanes striding over its row
 // (32 / G particles per warp at a time); the sum is returned in every lane of the group.
-template <bool ENERGY>
+template <bool ENERGY, bool WRAP>
 __device__ __forceinline__ Acc64 lj_row64(const Geom &g, const Pair &pp,
                                           const float4 *__restrict__ pos, const int *col, int cnt,
                                           const float4 &pb, int sub, int G) {
@@ -86,8 +86,8 @@ __device__ __forceinline__ Acc64 lj_row64(const Geom &g, const Pair &pp,
         const int j1 = col[k * TILE];
         const int j2 = v2 ? col[(k + G) * TILE] : j1;
         const float4 q1 = pos[j1], q2 = pos[j2];
-        pair_any<0, 3, ENERGY, true>(pp, me, q1, true, acc);
-        pair_any<0, 3, ENERGY, true>(pp, me, q2, v2, acc);
+        pair_any<0, 3, ENERGY, WRAP>(pp, me, q1, true, acc);
+        pair_any<0, 3, ENERGY, WRAP>(pp, me, q2, v2, acc);
     }
     for (int o = G >> 1; o > 0; o >>= 1) {              // G is warp-uniform
         acc.fx += __shfl_xor_sync(FULL, acc.fx, o);
@@ -234,7 +234,9 @@ k_force_lj32(Geom g, Pair pp, Pair32 p32, const float4 *__restrict__ pos,
         pb.z = __shfl_sync(FULL, pi.z, bb); pb.w = 0.0f;
         int cb = __shfl_sync(FULL, cnt, bb);              // every lane takes part in the shuffle
         if (b < 0) cb = 0;
-        const Acc64 r = lj_row64<ENERGY>(g, pp, pos, tile0 + bb, cb, pb, sub, G);
+        // away from every face the fp32 difference is exact for every pair inside the cutoff
+        const Acc64 r = (wx || wy || wz) ? lj_row64<ENERGY, true>(g, pp, pos, tile0 + bb, cb, pb, sub, G)
+                                         : lj_row64<ENERGY, false>(g, pp, pos, tile0 + bb, cb, pb, sub, G);
         // deliver: the lane whose rank among the flagged lanes is q < ng reads group q
         const int rank = __popc(todo & ((1u << lane) - 1u));
         const bool mine = ((todo >> lane) & 1u) && rank < ng;
