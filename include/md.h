@@ -100,6 +100,8 @@ int md_destroy(md_system *sys);
  *   "remap"                3-D LJ force kernel: blocks i and i + remap work on adjacent list tiles, so the
  *                          blocks one SM receives round-robin share gathered positions in L1 (default
  *                          37; 0 = block i works on tile block i)
+ *   "builder_parts"        warps that share one list tile in the builder: 1, 2, 4, or 0 (default) = 4 up to
+ *                          65,536 particles, else 1
  *   "builder"              neighbor-list kernel: 2 (default) records hits in per-lane bit masks,
  *                          1 appends them to per-lane shared-memory columns (first design)
  *   "use_graph"            0: md_nve_step launches kernels directly instead of a CUDA graph */

@@ -83,6 +83,7 @@ struct md_system {
     int use_graph;
     int fused;           // fused step: the force kernel also opens the next step (graph mode, fast32)
     int remap;           // force kernel: block -> tile remap period (the SM count), 0 = off
+    int nb_parts;        // builder: warps per tile (0 = by system size, 1, 2, 4)
     int builder;         // neighbor-list builder: 2 = bit-mask (md_nbr2.cuh), 1 = column append
     int fast32;          // LJ 3-D: fp32 fast path + fp64 re-evaluation (md_force32.cuh)
     float est_thr;       // its error-estimate threshold
@@ -242,16 +243,21 @@ int launch_nbr_build(md_system *s, const float4 *spos, const int *cell_start, co
     const Geom &g = s->g;
     const int ntiles = (g.n + TILE - 1) / TILE;
     if (s->builder == 2) {          // bit-mask builder (md_nbr2.cuh)
-        const int nb = (ntiles + NB2_WARPS - 1) / NB2_WARPS;
+        // warps per tile: small systems wait for the latency of one tile, large ones for throughput
+        int parts = s->nb_parts;
+        // measured (nbr build, us): 864 particles 58 / 39 / 33 for 1 / 2 / 4 warps per tile, 32k 62 / 48 / 44,
+        // 256k 151 / 200 / 182, 1M 414 / 662 / 618: sharing pays only while the GPU is not full
+        if (parts == 0) parts = ntiles <= 2048 ? 4 : 1;
+        const int tpb = NB2_WARPS / parts;
+        const int nb = (ntiles + tpb - 1) / tpb;
         const int threads = NB2_WARPS * 32;
         const size_t sm = NB2_WARPS * sizeof(Nb2Warp);
-        if (g.dim == 3) {
-            if (map) k_nbr_build2<3, true><<<nb, threads, sm, st>>>(g, spos, cell_start, map, nbr_idx, nbr_count, status, s->ref_pos, cond, incremental);
-            else k_nbr_build2<3, false><<<nb, threads, sm, st>>>(g, spos, cell_start, map, nbr_idx, nbr_count, status, s->ref_pos, cond, incremental);
-        } else {
-            if (map) k_nbr_build2<2, true><<<nb, threads, sm, st>>>(g, spos, cell_start, map, nbr_idx, nbr_count, status, s->ref_pos, cond, incremental);
-            else k_nbr_build2<2, false><<<nb, threads, sm, st>>>(g, spos, cell_start, map, nbr_idx, nbr_count, status, s->ref_pos, cond, incremental);
-        }
+#define MD_NB2_LAUNCH(D, M, P) k_nbr_build2<D, M, P><<<nb, threads, sm, st>>>(g, spos, cell_start, map, nbr_idx, nbr_count, status, s->ref_pos, cond, incremental)
+#define MD_NB2_PARTS(D, M) do { if (parts == 4) MD_NB2_LAUNCH(D, M, 4); else if (parts == 2) MD_NB2_LAUNCH(D, M, 2); else MD_NB2_LAUNCH(D, M, 1); } while (0)
+        if (g.dim == 3) { if (map) MD_NB2_PARTS(3, true); else MD_NB2_PARTS(3, false); }
+        else { if (map) MD_NB2_PARTS(2, true); else MD_NB2_PARTS(2, false); }
+#undef MD_NB2_PARTS
+#undef MD_NB2_LAUNCH
         LAUNCH_OK();
         return MD_OK;
     }
@@ -586,10 +592,11 @@ int md_create(const md_config *cfg, int n, void *workspace, size_t bytes, md_sys
             if (ea == cudaSuccess) ea = cudaFuncSetAttribute(k_nbr_build<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)s->nb_smem);
         }
         const int sm2 = (int)(NB2_WARPS * sizeof(Nb2Warp));
-        if (ea == cudaSuccess) ea = cudaFuncSetAttribute(k_nbr_build2<3, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm2);
-        if (ea == cudaSuccess) ea = cudaFuncSetAttribute(k_nbr_build2<3, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm2);
-        if (ea == cudaSuccess) ea = cudaFuncSetAttribute(k_nbr_build2<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm2);
-        if (ea == cudaSuccess) ea = cudaFuncSetAttribute(k_nbr_build2<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm2);
+#define MD_NB2_ATTR(D, M, P) if (ea == cudaSuccess) ea = cudaFuncSetAttribute(k_nbr_build2<D, M, P>, cudaFuncAttributeMaxDynamicSharedMemorySize, sm2)
+        MD_NB2_ATTR(3, true, 1); MD_NB2_ATTR(3, false, 1); MD_NB2_ATTR(2, true, 1); MD_NB2_ATTR(2, false, 1);
+        MD_NB2_ATTR(3, true, 2); MD_NB2_ATTR(3, false, 2); MD_NB2_ATTR(2, true, 2); MD_NB2_ATTR(2, false, 2);
+        MD_NB2_ATTR(3, true, 4); MD_NB2_ATTR(3, false, 4); MD_NB2_ATTR(2, true, 4); MD_NB2_ATTR(2, false, 4);
+#undef MD_NB2_ATTR
         if (ea != cudaSuccess) { delete s; return fail(MD_ECUDA, "cudaFuncSetAttribute: %s", cudaGetErrorString(ea)); }
     }
     cudaError_t e = cudaMemset(workspace, 0, l.total);
@@ -645,6 +652,10 @@ int md_set_option(md_system *sys, const char *name, double value) {
     else if (!strcmp(name, "fast32")) sys->fast32 = value != 0.0;
     else if (!strcmp(name, "fused")) sys->fused = value != 0.0;
     else if (!strcmp(name, "remap")) sys->remap = (int)value;
+    else if (!strcmp(name, "builder_parts")) {
+        if (value != 0.0 && value != 1.0 && value != 2.0 && value != 4.0) return fail(MD_EINVAL, "builder_parts must be 0, 1, 2 or 4");
+        sys->nb_parts = (int)value;
+    }
     else if (!strcmp(name, "builder")) {
         if (value != 1.0 && value != 2.0) return fail(MD_EINVAL, "builder must be 1 or 2");
         sys->builder = (int)value;

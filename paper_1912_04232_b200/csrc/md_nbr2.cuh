@@ -45,14 +45,31 @@ __device__ __forceinline__ unsigned push4(unsigned m, float2 a, float2 b) {
 #ifndef MD_NB2_MINBLOCKS
 #define MD_NB2_MINBLOCKS (32 / MD_NB2_WARPS)
 #endif
-template <int DIM, bool MAPPED>
+// PARTS = 1, 2 or 4 warps share one tile: they build the same piece table, scan every PARTS-th
+// piece each, exchange their per-lane hit counts through shared memory (a named barrier per tile)
+// and expand their masks into disjoint row ranges of the tile.  The list is the same set of rows;
+// a tile's critical path is 1/PARTS as long, which is what small systems (a few tiles per SM) and
+// the last wave of large ones wait for, at the price of PARTS copies of the per-tile prologue.
+__device__ __forceinline__ void bar_group(int id, int nthreads) {
+    asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory");
+}
+__device__ __forceinline__ int warp_sum_i(int v) {
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(FULL, v, o);
+    return v;
+}
+
+template <int DIM, bool MAPPED, int PARTS>
 __global__ void __launch_bounds__(NB2_WARPS * 32, MD_NB2_MINBLOCKS)
 k_nbr_build2(Geom g, const float4 *__restrict__ spos, const int *__restrict__ cell_start,
              const int *__restrict__ map, int *__restrict__ nbr_idx, int *__restrict__ nbr_count,
              int *status, float4 *__restrict__ ref_pos, const int *cond, int incremental) {
     extern __shared__ __align__(16) unsigned char nb2_smem[];
     if (cond && ld_volatile(cond) == 0) return;
+    __shared__ int coop[NB2_WARPS][TILE];                  // per-lane hit counts of the parts of a tile
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    constexpr int TPB = NB2_WARPS / PARTS;                  // tiles per block
+    const int tl = warp / PARTS, part = warp % PARTS;
     Nb2Warp &W = reinterpret_cast<Nb2Warp *>(nb2_smem)[warp];
     const int cap = g.capacity;
     const int ncx = g.nc[0], ncy = g.nc[1], ncz = g.nc[2];
@@ -62,7 +79,7 @@ k_nbr_build2(Geom g, const float4 *__restrict__ spos, const int *__restrict__ ce
     constexpr int ROWS = DIM == 3 ? 9 : 3;
     const int ntiles = (g.n + TILE - 1) / TILE;
 
-    for (int tile = blockIdx.x * NB2_WARPS + warp; tile < ntiles; tile += gridDim.x * NB2_WARPS) {
+    for (int tile = blockIdx.x * TPB + tl; tile < ntiles; tile += gridDim.x * TPB) {
         const int s = tile * TILE + lane;
         const bool act = s < g.n;
         const float4 pi = spos[act ? s : g.n - 1];
@@ -74,7 +91,7 @@ k_nbr_build2(Geom g, const float4 *__restrict__ spos, const int *__restrict__ ce
         int *outp = nullptr;                                     // its column of the list
         if (!MAPPED) outp = nbr_idx + nbr_tile_base(s, cap) + lane;
         else if (act) outp = nbr_idx + nbr_tile_base(me, cap) + (me & 31);
-        const int prev = incremental ? (act ? min(nbr_count[me], cap) : 0) : cap;
+        const int prev = incremental ? ((act && part == 0) ? min(nbr_count[me], cap) : 0) : cap;
         int cnt = 0;                                             // hits so far, self excluded
         unsigned todo = __ballot_sync(FULL, act);
         while (todo) {
@@ -121,6 +138,15 @@ k_nbr_build2(Geom g, const float4 *__restrict__ spos, const int *__restrict__ ce
                     t1 = a0;
                 }
             }
+            // a part whose pieces would not fit one batch of masks cannot flush on its own (its rows
+            // start after the other parts' hits): part 0 then scans the whole segment alone
+            bool solo = false;
+            if (PARTS > 1) {
+                const int words = lane < 3 * ROWS ? ((t1 - t0 + 31) >> 5) + 1 : 0;
+#pragma unroll
+                for (int q = 0; q < PARTS; ++q)
+                    solo = solo || warp_sum_i(lane % PARTS == q ? words : 0) > NB2_WORDS;
+            }
             int nw = 0;                      // mask words of the current batch (warp-uniform)
             unsigned nzlo = 0u, nzhi = 0u;   // which of them are non-zero for this lane (words 0-31, 32-)
             int nhit = 0;                    // hits of this lane in the current batch (self excluded)
@@ -162,7 +188,7 @@ k_nbr_build2(Geom g, const float4 *__restrict__ spos, const int *__restrict__ ce
             auto seek = [&](int &pp, int &bb, int &tt1) {       // first non-empty piece >= pp
                 while (pp < 3 * ROWS) {
                     bb = __shfl_sync(FULL, t0, pp); tt1 = __shfl_sync(FULL, t1, pp);
-                    if (bb < tt1) return;
+                    if (bb < tt1 && (PARTS == 1 || (solo ? part == 0 : pp % PARTS == part))) return;
                     ++pp;
                 }
             };
@@ -259,9 +285,28 @@ k_nbr_build2(Geom g, const float4 *__restrict__ spos, const int *__restrict__ ce
                 __syncwarp();
                 p = np; base = nbase; pt1 = npt1;
             }
-            expand();
+            if (PARTS == 1) {
+                expand();
+            } else {
+                // rows of this tile: part 0's hits, then part 1's, ...; every part learns the total
+                coop[warp][lane] = inseg ? nhit : 0;
+                bar_group(1 + tl, 32 * PARTS);
+                int offset = 0, total = 0;
+#pragma unroll
+                for (int q = 0; q < PARTS; ++q) {
+                    const int v = coop[tl * PARTS + q][lane];
+                    offset += q < part ? v : 0;
+                    total += v;
+                }
+                const int base_cnt = cnt;       // hits flushed earlier (solo part 0) or of an earlier segment
+                cnt = base_cnt + offset;
+                expand();
+                cnt = base_cnt + total;
+                bar_group(1 + tl, 32 * PARTS);  // coop is rewritten by the next segment
+            }
         }
-        // ---- pads (= N, A5), counts, rebuild reference, status
+        // ---- pads (= N, A5), counts, rebuild reference, status (one part does it)
+        if (PARTS > 1 && part != 0) continue;
         if (outp) {
             const int upto = incremental ? prev : cap;
             for (int k = min(cnt, cap); k < upto; ++k) outp[k * TILE] = g.n;

@@ -171,6 +171,29 @@ def test_threads_per_particle_variants(B, orc, W, tpp):
     S.close()
 
 
+@pytest.mark.parametrize("parts", [1, 2, 4])
+@pytest.mark.parametrize("ci,resort", [(0, 1), (1, 1), (2, 1), (2, 0)])
+def test_builder_warps_per_tile(B, orc, W, ci, resort, parts):
+    """1, 2 or 4 warps share a tile in the bit-mask builder: same rows, same counts, and the lists
+    stay right through the rebuilds of a short run (incremental pads)."""
+    w = W.config(ci)
+    S = B.System(w, resort=resort)
+    B.md_set_option(S.sys, "builder_parts", parts)
+    S.build()
+    torch.cuda.synchronize()
+    check_list(S, orc, w, method=0 if ci < 2 else 1)
+    S.compute_force()
+    S.step(40)
+    torch.cuda.synchronize()
+    assert int(S.stats[1]) >= 2 and int(S.stats[2]) == -1
+    pos = unpermute(S, S.pos)
+    w2 = dataclasses.replace(w, pos=pos)
+    S.build()                                   # a full build of the final state for comparison
+    torch.cuda.synchronize()
+    check_list(S, orc, w2, method=1)
+    S.close()
+
+
 @pytest.mark.parametrize("ci", [0, 1])
 def test_first_design_builder(B, orc, W, ci):
     """builder = 1 (per-lane shared-memory columns) still builds the same rows."""
