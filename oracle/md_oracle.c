@@ -56,6 +56,7 @@
 #define KIND_SOFT 1
 #define KIND_MORSE 2
 #define KIND_BUCK 3
+#define KIND_LJ_SPECIES 4
 
 int orc_num_threads(void)
 {
@@ -410,6 +411,21 @@ static void buck_pair(double r, double A, double B, double Cc, double *u, double
     *fr = r > 0.0 ? (B * x - 6.0 * Cc / (r6 * r)) / r : 0.0;
 }
 
+/* Species x species Lennard-Jones (PAPER.md:L104 pair potentials with per-species parameters, the
+ * sigma matrix of L298-L305 App. A): kind 4 reads eps_ab, sigma_ab and the truncation radius rc_ab
+ * from tables set here; the species of particle i is (int)diam[i] (the pos.w channel). */
+#define ORC_MAX_SPECIES 4
+static int g_ns = 0;
+static double g_sp_eps[ORC_MAX_SPECIES * ORC_MAX_SPECIES], g_sp_sig[ORC_MAX_SPECIES * ORC_MAX_SPECIES],
+              g_sp_rc[ORC_MAX_SPECIES * ORC_MAX_SPECIES];
+int orc_set_species_lj(int ns, const double *eps, const double *sigma, const double *rc)
+{
+    if (ns < 1 || ns > ORC_MAX_SPECIES) return ORC_EINVAL;
+    g_ns = ns;
+    for (int k = 0; k < ns * ns; ++k) { g_sp_eps[k] = eps[k]; g_sp_sig[k] = sigma[k]; g_sp_rc[k] = rc[k]; }
+    return ORC_OK;
+}
+
 static double lj_u_cut(double eps, double sigma, double r_cut)
 {
     double u, fr;
@@ -425,6 +441,8 @@ static double lj_u_cut(double eps, double sigma, double r_cut)
  *                (PAPER.md:L301); r = 0 gives energy eps/2 and zero force
  *   kind 2 MORSE: u = eps (1 - exp(-alpha (r - sigma)))^2 - eps - shift*u(r_cut) for r < r_cut,
  *                alpha set by orc_set_morse_alpha (PAPER.md:L104 [75])
+ *   kind 4 LJ_SPECIES: LJ with eps, sigma, r_cut taken per species pair from orc_set_species_lj,
+ *                species = (int)diam[i]; eps, sigma, r_cut arguments unused
  *   kind 3 BUCKINGHAM: u = eps exp(-alpha r) - sigma / r^6 - shift*u(r_cut) for r < r_cut
  *                (A = eps, B = alpha, C = sigma; PAPER.md:L104 [71-73])
  *   nbr_idx == NULL: all pairs j != i (the definition);
@@ -438,8 +456,10 @@ int orc_energy_force(int n, int dim, const double *pos, const double *diam,
                      double *e_i, double *E)
 {
     if (n <= 0 || (dim != 2 && dim != 3)) return ORC_EINVAL;
-    if (kind != KIND_LJ && kind != KIND_SOFT && kind != KIND_MORSE && kind != KIND_BUCK) return ORC_EINVAL;
-    if (kind == KIND_SOFT && !diam) return ORC_EINVAL;
+    if (kind != KIND_LJ && kind != KIND_SOFT && kind != KIND_MORSE && kind != KIND_BUCK &&
+        kind != KIND_LJ_SPECIES) return ORC_EINVAL;
+    if ((kind == KIND_SOFT || kind == KIND_LJ_SPECIES) && !diam) return ORC_EINVAL;
+    if (kind == KIND_LJ_SPECIES && g_ns < 1) return ORC_EINVAL;
     double u_c = (kind == KIND_LJ && shift) ? lj_u_cut(eps, sigma, r_cut) : 0.0;
     if (kind == KIND_MORSE && shift) {
         double fr_unused;
@@ -466,6 +486,16 @@ int orc_energy_force(int n, int dim, const double *pos, const double *diam,
                     double u, fr;
                     lj_pair(r2, eps, sigma, &u, &fr);
                     e += 0.5 * (u - u_c);
+                    for (int q = 0; q < dim; ++q) f[q] += fr * d[q];
+                }
+            } else if (kind == KIND_LJ_SPECIES) {
+                int sa = (int)diam[i], sb = (int)diam[j];
+                if (sa < 0 || sa >= g_ns || sb < 0 || sb >= g_ns) continue;
+                int t = sa * g_ns + sb;
+                if (r2 < g_sp_rc[t] * g_sp_rc[t]) {
+                    double u, fr;
+                    lj_pair(r2, g_sp_eps[t], g_sp_sig[t], &u, &fr);
+                    e += 0.5 * (u - (shift ? lj_u_cut(g_sp_eps[t], g_sp_sig[t], g_sp_rc[t]) : 0.0));
                     for (int q = 0; q < dim; ++q) f[q] += fr * d[q];
                 }
             } else if (kind == KIND_BUCK) {

@@ -111,6 +111,14 @@ def predicate_band(pos, box, dim, r_cut, skin, method=1):
     return int(nd.value), float(band.value), float(close.value)
 
 
+def set_species_lj(eps, sigma, rc) -> None:
+    """Tables of kind 4 (species x species LJ): square arrays eps_ab, sigma_ab, rc_ab."""
+    e = _d(eps); sg = _d(sigma); r = _d(rc)
+    ns = e.shape[0]
+    _check(lib().orc_set_species_lj(ns, _pd(e.reshape(-1).copy()), _pd(sg.reshape(-1).copy()),
+                                    _pd(r.reshape(-1).copy())), "set_species_lj")
+
+
 def set_morse_alpha(alpha: float) -> None:
     """alpha of kind 2 (Morse) for the following energy_force / nve_run calls."""
     lib().orc_set_morse_alpha(C.c_double(alpha))

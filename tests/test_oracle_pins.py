@@ -730,3 +730,47 @@ def test_buckingham_two_body_and_gradient(orc, W):
                    - orc.energy_force(pm, None, box, 3, *args, alpha=Bc)[2]) / (2 * h)
             worst = max(worst, abs(fd - f[i, q]) / max(1.0, np.abs(f[i]).max()))
     assert worst < 1e-6, worst
+
+
+# ------------------------------------------- species x species LJ --
+
+KA_EPS = np.array([[1.0, 1.5], [1.5, 0.5]])
+KA_SIG = np.array([[1.0, 0.8], [0.8, 0.88]])
+
+
+def test_species_lj_reduces_to_lj_and_mixed_pair_closed_form(orc, W):
+    """Kind 4: identical species tables give plain LJ (the pinned kind 0); a mixed A-B pair of the
+    Kob-Andersen tables follows the closed form with eps_AB, sigma_AB and its own cutoff; forces are
+    -grad E and sum to zero on a binary mixture."""
+    SPEC = 4
+    w = W.lj_fcc(0, 3, seed=21)
+    pos, box = w.pos[:, :3].astype(np.float64), w.box.astype(np.float64)
+    one = np.ones((2, 2))
+    orc.set_species_lj(one, one, 2.5 * one)
+    sp = (np.arange(w.n) % 5 == 0).astype(np.float64)             # 20 % species 1
+    f4, e4, E4 = orc.energy_force(pos, sp, box, 3, SPEC, 0.0, 0.0, 0.0, 1)
+    f0, e0, E0 = orc.energy_force(pos, None, box, 3, LJ, 1.0, 1.0, 2.5, 1)
+    assert np.array_equal(f4, f0) and np.array_equal(e4, e0) and E4 == E0
+    orc.set_species_lj(KA_EPS, KA_SIG, 2.5 * KA_SIG)
+    r = 0.95
+    p2, b2, _ = two_body(r, 1)
+    f, _, E = orc.energy_force(p2, np.array([0.0, 1.0]), b2, 3, SPEC, 0.0, 0.0, 0.0, 1)
+    eps, sig, rc = 1.5, 0.8, 2.0
+    u = 4 * eps * ((sig / r) ** 12 - (sig / r) ** 6) - 4 * eps * ((sig / rc) ** 12 - (sig / rc) ** 6)
+    du = 4 * eps * (-12 * sig ** 12 / r ** 13 + 6 * sig ** 6 / r ** 7)
+    assert abs(E - u) < 1e-13 and abs(f[0, 1] - du) < 1e-12 and abs(f[1, 1] + du) < 1e-12
+    p2, b2, _ = two_body(2.0 * (1 + 1e-9), 1)                     # beyond rc_AB = 2.0 but inside rc_AA = 2.5
+    assert orc.energy_force(p2, np.array([0.0, 1.0]), b2, 3, SPEC, 0.0, 0.0, 0.0, 1)[2] == 0.0
+    assert orc.energy_force(p2, np.array([0.0, 0.0]), b2, 3, SPEC, 0.0, 0.0, 0.0, 1)[2] != 0.0
+    f, _, _ = orc.energy_force(pos, sp, box, 3, SPEC, 0.0, 0.0, 0.0, 1)
+    assert np.abs(f.sum(0)).max() < 1e-10 * np.abs(f).sum()
+    rng = np.random.default_rng(6)
+    h, worst = 1e-5, 0.0
+    for i in rng.choice(pos.shape[0], 6, replace=False):
+        for q in range(3):
+            pp = pos.copy(); pp[i, q] += h
+            pm = pos.copy(); pm[i, q] -= h
+            fd = -(orc.energy_force(pp, sp, box, 3, SPEC, 0.0, 0.0, 0.0, 1)[2]
+                   - orc.energy_force(pm, sp, box, 3, SPEC, 0.0, 0.0, 0.0, 1)[2]) / (2 * h)
+            worst = max(worst, abs(fd - f[i, q]) / max(1.0, np.abs(f[i]).max()))
+    assert worst < 1e-6, worst
