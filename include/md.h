@@ -47,6 +47,7 @@ extern "C" {
 #define MD_KIND_LJ   0      /* Lennard-Jones [69], L104 §3.3.2 */
 #define MD_KIND_SOFT 1      /* harmonic soft sphere [70], L104; d_ij = (d_i+d_j)/2, L301 App. A */
 #define MD_KIND_MORSE 2     /* Morse [75], L104: u = eps (1 - exp(-alpha (r - sigma)))^2 - eps */
+#define MD_KIND_LJ_SPECIES 4 /* LJ with eps, sigma, r_cut per species pair (md_set_species_lj); species = (int)pos.w */
 #define MD_KIND_BUCKINGHAM 3 /* Buckingham-type exp-6 [71-73], L104: u = eps exp(-alpha r) - sigma / r^6
                                (epsilon = A, alpha = B, sigma = C) */
 
@@ -106,6 +107,13 @@ int md_destroy(md_system *sys);
  *                          1 appends them to per-lane shared-memory columns (first design)
  *   "use_graph"            0: md_nve_step launches kernels directly instead of a CUDA graph */
 int md_set_option(md_system *sys, const char *name, double value);
+
+/* Species x species Lennard-Jones tables (L104 pair potentials with per-species parameters; the
+ * sigma matrix of L298-L305): host float[nspecies * nspecies], row-major, 1 <= nspecies <= 4, every
+ * r_cut <= the list r_cut.  Used by MD_KIND_LJ_SPECIES (whose epsilon / sigma / r_cut fields are
+ * ignored; shift applies per pair); the species of a particle is (int)pos.w.  fp64 pair chain. */
+int md_set_species_lj(md_system *sys, int nspecies, const float *epsilon, const float *sigma,
+                      const float *r_cut);
 
 /* Diagnostic counters since md_create (or the last reset): copies int32[8] to the DEVICE buffer
  * `out` on `stream`, then clears them if reset != 0.

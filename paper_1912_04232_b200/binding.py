@@ -15,14 +15,14 @@ import torch
 from . import build as _build
 
 MD_OK, MD_EINVAL, MD_EBOX, MD_EWORKSPACE, MD_ECUDA = 0, -1, -2, -3, -4
-MD_KIND_LJ, MD_KIND_SOFT, MD_KIND_MORSE, MD_KIND_BUCKINGHAM = 0, 1, 2, 3
+MD_KIND_LJ, MD_KIND_SOFT, MD_KIND_MORSE, MD_KIND_BUCKINGHAM, MD_KIND_LJ_SPECIES = 0, 1, 2, 3, 4
 
 SYMBOLS = [
     "md_last_error", "md_workspace_bytes", "md_create", "md_destroy", "md_set_option",
     "md_num_cells", "md_nbr_layout", "md_cell_list_build", "md_neighbor_list_build",
     "md_needs_rebuild", "md_pair_energy_force", "md_nve_step", "md_nve_run_host", "md_counters",
     "md_nve_run_host_release", "md_fire_minimize", "md_brownian_step",
-    "md_langevin_step", "md_nose_hoover_step",
+    "md_langevin_step", "md_nose_hoover_step", "md_set_species_lj",
 ]
 
 
@@ -70,6 +70,7 @@ def lib():
         L.md_destroy.argtypes = [vp]
         L.md_set_option.argtypes = [vp, C.c_char_p, C.c_double]
         L.md_counters.argtypes = [vp, ip, C.c_int, vp]
+        L.md_set_species_lj.argtypes = [vp, C.c_int, C.POINTER(C.c_float), C.POINTER(C.c_float), C.POINTER(C.c_float)]
         L.md_brownian_step.argtypes = [vp, C.POINTER(md_potential), vp, vp, ip, ip, ip, C.c_float, C.c_float,
                                        C.c_float, C.c_uint32, C.c_uint32, C.c_int, ip, vp]
         L.md_langevin_step.argtypes = [vp, C.POINTER(md_potential), vp, vp, vp, ip, ip, ip, C.c_float, C.c_float,
@@ -186,6 +187,16 @@ def md_fire_minimize(sys, pot: md_potential, par: md_fire_params, pos, vel, forc
 
 def md_nve_run_host_release() -> None:
     _check(lib().md_nve_run_host_release())
+
+
+def md_set_species_lj(sys, epsilon, sigma, r_cut) -> None:
+    """Square host arrays eps_ab, sigma_ab, rc_ab (up to 4 x 4)."""
+    import numpy as np
+    e = np.ascontiguousarray(epsilon, dtype=np.float32); sg = np.ascontiguousarray(sigma, dtype=np.float32)
+    r = np.ascontiguousarray(r_cut, dtype=np.float32)
+    fp = C.POINTER(C.c_float)
+    _check(lib().md_set_species_lj(sys, int(e.shape[0]), e.ctypes.data_as(fp), sg.ctypes.data_as(fp),
+                                   r.ctypes.data_as(fp)))
 
 
 def md_counters(sys, out, reset=False, stream=None) -> None:

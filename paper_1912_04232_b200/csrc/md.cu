@@ -84,6 +84,8 @@ struct md_system {
     int fused;           // fused step: the force kernel also opens the next step (graph mode, fast32)
     int remap;           // force kernel: block -> tile remap period (the SM count), 0 = off
     int nb_parts;        // builder: warps per tile (0 = by system size, 1, 2, 4)
+    int ns;              // md_set_species_lj: number of species and the tables (row-major)
+    float sp_eps[16], sp_sig[16], sp_rc[16];
     int builder;         // neighbor-list builder: 2 = bit-mask (md_nbr2.cuh), 1 = column append
     int fast32;          // LJ 3-D: fp32 fast path + fp64 re-evaluation (md_force32.cuh)
     float est_thr;       // its error-estimate threshold
@@ -171,7 +173,7 @@ int make_geom(const md_config *cfg, int n, Geom *g) {
 int make_pair(const md_system *sys, const md_potential *pot, Pair *pp) {
     if (!pot) return fail(MD_EINVAL, "potential is NULL");
     if (pot->kind != MD_KIND_LJ && pot->kind != MD_KIND_SOFT && pot->kind != MD_KIND_MORSE &&
-        pot->kind != MD_KIND_BUCKINGHAM)
+        pot->kind != MD_KIND_BUCKINGHAM && pot->kind != MD_KIND_LJ_SPECIES)
         return fail(MD_EINVAL, "unknown potential kind %d", pot->kind);
     if (!(pot->epsilon > 0.0f)) return fail(MD_EINVAL, "epsilon must be positive");
     memset(pp, 0, sizeof(*pp));
@@ -191,6 +193,16 @@ int make_pair(const md_system *sys, const md_potential *pot, Pair *pp) {
         const double rc = pot->r_cut, x = std::exp(-(double)pot->alpha * (rc - (double)pot->sigma));
         pp->dalpha = pot->alpha; pp->dr0 = pot->sigma; pp->drc2 = rc * rc; pp->dsig6x2 = 2.0;
         pp->du_cutm = pot->shift ? ((1.0 - x) * (1.0 - x) - 1.0) : 0.0;
+    } else if (pot->kind == MD_KIND_LJ_SPECIES) {
+        if (sys->ns < 1) return fail(MD_EINVAL, "MD_KIND_LJ_SPECIES needs md_set_species_lj first");
+        pp->ns = sys->ns; pp->dsig6x2 = 2.0; pp->drc2 = 0.0;
+        for (int t = 0; t < sys->ns * sys->ns; ++t) {
+            const double e = sys->sp_eps[t], sg = sys->sp_sig[t], rc = sys->sp_rc[t];
+            if (rc > sys->cfg.r_cut) return fail(MD_EINVAL, "species r_cut %g exceeds the list r_cut %g", rc, sys->cfg.r_cut);
+            const double s6 = std::pow(sg, 6.0), q6 = std::pow(sg / rc, 6.0);
+            pp->sp_sig6x2[t] = 2.0 * s6; pp->sp_fs[t] = 24.0 * e * s6; pp->sp_es[t] = 2.0 * e;
+            pp->sp_rc2[t] = rc * rc; pp->sp_ucut4[t] = pot->shift ? (q6 * q6 - q6) : 0.0;
+        }
     } else if (pot->kind == MD_KIND_BUCKINGHAM) {
         if (!(pot->r_cut > 0.0f) || !(pot->sigma >= 0.0f) || !(pot->alpha > 0.0f))
             return fail(MD_EINVAL, "Buckingham needs alpha (B) > 0, sigma (C) >= 0 and r_cut > 0");
@@ -330,6 +342,7 @@ int launch_force(md_system *s, const Pair &pp, const float4 *pos, const int *nbr
                                                etot, book, st))
     if (pp.kind == MD_KIND_LJ) return s->g.dim == 3 ? MD_FORCE_DISPATCH(0, 3) : MD_FORCE_DISPATCH(0, 2);
     if (pp.kind == MD_KIND_MORSE) return s->g.dim == 3 ? MD_FORCE_DISPATCH(2, 3) : MD_FORCE_DISPATCH(2, 2);
+    if (pp.kind == MD_KIND_LJ_SPECIES) return s->g.dim == 3 ? MD_FORCE_DISPATCH(4, 3) : MD_FORCE_DISPATCH(4, 2);
     if (pp.kind == MD_KIND_BUCKINGHAM) return s->g.dim == 3 ? MD_FORCE_DISPATCH(3, 3) : MD_FORCE_DISPATCH(3, 2);
     return s->g.dim == 3 ? MD_FORCE_DISPATCH(1, 3) : MD_FORCE_DISPATCH(1, 2);
 #undef MD_FORCE_DISPATCH
@@ -630,6 +643,19 @@ int md_nbr_layout(const md_system *sys, long *tile, long *tile_stride, long *par
     *particle_stride = 1;
     *slot_stride = TILE;
     *length = (long)((sys->n + TILE - 1) / TILE) * TILE * sys->g.capacity;
+    return MD_OK;
+}
+
+int md_set_species_lj(md_system *sys, int nspecies, const float *epsilon, const float *sigma,
+                      const float *r_cut) {
+    if (!sys || !epsilon || !sigma || !r_cut) return fail(MD_EINVAL, "NULL argument");
+    if (nspecies < 1 || nspecies > 4) return fail(MD_EINVAL, "nspecies = %d must be in 1..4", nspecies);
+    for (int t = 0; t < nspecies * nspecies; ++t)
+        if (!(epsilon[t] >= 0.0f) || !(sigma[t] > 0.0f) || !(r_cut[t] > 0.0f) || r_cut[t] > sys->cfg.r_cut)
+            return fail(MD_EINVAL, "species pair %d: epsilon >= 0, sigma > 0, 0 < r_cut <= list r_cut", t);
+    sys->ns = nspecies;
+    for (int t = 0; t < nspecies * nspecies; ++t) { sys->sp_eps[t] = epsilon[t]; sys->sp_sig[t] = sigma[t]; sys->sp_rc[t] = r_cut[t]; }
+    drop_graphs(sys);
     return MD_OK;
 }
 

@@ -30,6 +30,13 @@ struct Pair {
     double dalpha, dr0;     // MORSE: alpha, r0
     double du_cutm;         // MORSE: shift * u(r_cut) / eps;  BUCKINGHAM: shift * u(r_cut)
     double dA, dC;          // BUCKINGHAM: A, C (B is dalpha)
+    // LJ_SPECIES: per species pair t = a * ns + b (species = (int)pos.w)
+    int ns;
+    double sp_sig6x2[16];   // 2 sigma_ab^6
+    double sp_fs[16];       // 24 eps_ab sigma_ab^6
+    double sp_es[16];       // 2 eps_ab  (1/2 * 4 eps_ab)
+    double sp_rc2[16];      // rc_ab^2
+    double sp_ucut4[16];    // shift * ((s/rc)^12 - (s/rc)^6)
 };
 
 // Device words md_nve_step keeps between kernels.
@@ -673,6 +680,26 @@ __device__ __forceinline__ void buck_pair64(const Pair &pp, double dx, double dy
     if (ENERGY) a.e += in ? x - pp.dC * y3 - pp.du_cutm : 0.0;
 }
 
+// One pair, species x species LJ (L104; the sigma matrix of L298-L305): as lj_pair64 with the
+// constants of the pair's species; nothing is factored out (fs = es = 1).
+template <bool ENERGY>
+__device__ __forceinline__ void ljs_pair64(const Pair &pp, double dx, double dy, double dz, float wi,
+                                           float wj, bool valid, Acc64 &a) {
+    const int sa = min(max((int)wi, 0), pp.ns - 1), sb = min(max((int)wj, 0), pp.ns - 1);
+    const int t = sa * pp.ns + sb;
+    const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+    const bool in = valid && r2 < pp.sp_rc2[t];
+    const double y = rcp64(in ? r2 : 1.0);
+    const double y2 = y * y, y3 = y2 * y;
+    const double tt = fma(pp.sp_sig6x2[t], y3, -1.0);
+    const double c = in ? pp.sp_fs[t] * (y2 * y2) * tt : 0.0;
+    a.fx = fma(c, dx, a.fx); a.fy = fma(c, dy, a.fy); a.fz = fma(c, dz, a.fz);
+    if (ENERGY) {
+        const double s6 = 0.5 * pp.sp_sig6x2[t] * y3;
+        a.e += in ? pp.sp_es[t] * (fma(s6, s6, -s6) - pp.sp_ucut4[t]) : 0.0;
+    }
+}
+
 // Per-thread view of the space for the pair loop.
 template <int DIM>
 struct Me {
@@ -712,6 +739,7 @@ __device__ __forceinline__ void pair_any(const Pair &pp, const Me<DIM> &me, cons
     if (KIND == 0) lj_pair64<ENERGY>(pp, dx, dy, dz, valid, acc);
     else if (KIND == 2) morse_pair64<ENERGY>(pp, dx, dy, dz, valid, acc);
     else if (KIND == 3) buck_pair64<ENERGY>(pp, dx, dy, dz, valid, acc);
+    else if (KIND == 4) ljs_pair64<ENERGY>(pp, dx, dy, dz, me.pi.w, q.w, valid, acc);
     else soft_pair64<ENERGY>(pp, dx, dy, dz, (double)me.pi.w + (double)q.w, valid, acc);
 }
 
@@ -738,8 +766,9 @@ __device__ __forceinline__ void force_epilogue(const Pair &pp, const Acc64 &acc,
                                                float4 *__restrict__ force, float4 *__restrict__ vel,
                                                float a, double *energy_total, const Book &book,
                                                int gid) {
-    const double fs = KIND == 0 ? 12.0 * pp.deps * pp.dsig6x2 : (KIND == 3 ? 1.0 : pp.deps);   // 24 eps sig^6 | eps | D | 1
-    const double es = KIND == 0 ? 2.0 * pp.deps : (KIND == 2 ? 0.5 * pp.deps : (KIND == 3 ? 0.5 : 0.25 * pp.deps));   // 1/2 * (4 eps | D | 1 | eps/2)
+    const double fs = KIND == 0 ? 12.0 * pp.deps * pp.dsig6x2 : (KIND == 3 || KIND == 4 ? 1.0 : pp.deps);   // 24 eps sig^6 | eps | D | 1
+    const double es = KIND == 0 ? 2.0 * pp.deps
+                    : (KIND == 2 ? 0.5 * pp.deps : (KIND == 3 ? 0.5 : (KIND == 4 ? 1.0 : 0.25 * pp.deps)));   // 1/2 * (4 eps | D | 1 | eps/2)
     const float fx = (float)(fs * acc.fx), fy = (float)(fs * acc.fy), fz = (float)(fs * acc.fz);
     const double e64 = ENERGY ? es * acc.e : 0.0;
     if (owner) {

@@ -30,6 +30,7 @@ KIND_LJ = 0
 KIND_SOFT = 1
 KIND_MORSE = 2
 KIND_BUCKINGHAM = 3
+KIND_LJ_SPECIES = 4
 
 
 @dataclasses.dataclass(frozen=True)

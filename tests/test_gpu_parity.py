@@ -428,6 +428,48 @@ def test_buckingham_force_energy_and_trajectory(B, orc, W):
     S.close()
 
 
+def test_species_lj_binary_mixture(B, orc, W):
+    """species x species LJ.  The 80:20 Kob-Andersen
+    mixture on the jittered lattice of config 0: force / energy against the all-pairs definition,
+    100 NVE steps against the oracle, and equal tables reproducing plain LJ."""
+    eps = np.array([[1.0, 1.5], [1.5, 0.5]], np.float32)
+    sig = np.array([[1.0, 0.8], [0.8, 0.88]], np.float32)
+    rc = (2.5 * sig).astype(np.float32)
+    base = W.config(0)
+    pos = base.pos.copy()
+    pos[:, 3] = (np.arange(base.n) % 5 == 0).astype(np.float32)            # species in pos.w
+    w = custom_workload(W, pos, base.box, 3, 4, 2.5, 0.3, 128, vel=base.vel.copy(), dt=0.004)
+    w = dataclasses.replace(w, shift=1)
+    S = B.System(w)
+    B.md_set_species_lj(S.sys, eps, sig, rc)
+    S.build(); S.compute_force()
+    orc.set_species_lj(eps.astype(np.float64), sig.astype(np.float64), rc.astype(np.float64))
+    sp = pos[:, 3].astype(np.float64)
+    f_o, e_o, E_o = orc.energy_force(w.pos, sp, w.box, 3, 4, 0.0, 0.0, 0.0, 1)
+    assert force_error(unpermute(S, S.force), f_o) <= FORCE_TOL
+    assert abs(float(S.energy.cpu()[0]) - E_o) <= ENERGY_TOL * abs(E_o)
+    p_o, v_o, _, _, _ = orc.nve_run(w.pos, w.vel, f_o, sp, w.box, 3, 4, 0.0, 0.0, 0.0, 1, w.dt, w.mass, 100,
+                                    want_energies=False)
+    S.step(100)
+    torch.cuda.synchronize()
+    d = unpermute(S, S.pos)[:, :3].astype(np.float64) - p_o
+    L = w.box.astype(np.float64)
+    d -= L * np.round(d / L)
+    assert np.abs(d).max() <= 1e-4, np.abs(d).max()
+    assert np.array_equal(unpermute(S, S.pos)[:, 3], pos[:, 3])            # species travel with the re-sort
+    S.close()
+    # equal tables: the fp64 LJ chain
+    one = np.ones((2, 2), np.float32)
+    S1, S0 = B.System(w), B.System(dataclasses.replace(w, kind=0))
+    B.md_set_species_lj(S1.sys, one, one, 2.5 * one)
+    B.md_set_option(S0.sys, "fast32", 0)
+    for X in (S1, S0):
+        X.build(); X.compute_force()
+    torch.cuda.synchronize()
+    assert (S1.force[:, :3] - S0.force[:, :3]).abs().max().item() <= 1e-5 * S0.force[:, :3].abs().max().item()
+    S1.close(); S0.close()
+
+
 def test_fast32_dimers_at_the_force_zero(B, orc, W):
     """Isolated pairs around r = 2^(1/6) sigma, where the LJ force changes sign: the coefficient and
     with it sum|coefficient| vanish while the fp32 rounding error does not, so the error estimate
