@@ -367,66 +367,6 @@ __global__ void k_iota(int n, int *id) {
     if (i < n) id[i] = i;
 }
 
-// One velocity-Verlet step as launches on `st` (captured into a graph or run directly).
-// in_graph: `st` is capturing; the rebuild kernels go into the body of an IF node whose condition
-// the drift kernel raises, so a step without a rebuild launches two kernels.  Otherwise every
-// rebuild kernel is launched and returns at once while the device flag is 0.
-int record_step(md_system *s, const Pair &pp, float4 *pos, float4 *vel, float4 *force, int *id,
-                int *nbr_idx, int *nbr_count, float dt, float mass, int *stats, cudaStream_t st,
-                bool in_graph) {
-    const Geom &g = s->g;
-    const float a = dt / (2.0f * mass);
-    int *flag = s->words + 0;
-    int *status = s->words + 1;
-    const int nb = blocks_for(g.n);
-    const bool resort = s->cfg.resort != 0;
-    int rc;
-    if (!in_graph) {
-        cudaGraphConditionalHandle none = 0;
-        if (g.dim == 3) k_kick_drift<3, false><<<nb, 256, 0, st>>>(g, pos, vel, force, s->ref_pos, a, dt, flag, none);
-        else k_kick_drift<2, false><<<nb, 256, 0, st>>>(g, pos, vel, force, s->ref_pos, a, dt, flag, none);
-        LAUNCH_OK();
-        rc = launch_cell_build(s, pos, vel, id, s->cell_start_i, s->perm_i, status, flag, st);
-        if (rc) return rc;
-        rc = launch_nbr_build(s, resort ? pos : s->pos_s, s->cell_start_i, resort ? nullptr : s->perm_i,
-                              nbr_idx, nbr_count, status, flag, 1, st);
-        if (rc) return rc;
-    } else {
-        cudaStreamCaptureStatus cs;
-        cudaGraph_t graph = nullptr;
-        const cudaGraphNode_t *deps = nullptr;
-        size_t ndeps = 0;
-        CU(cudaStreamGetCaptureInfo(st, &cs, nullptr, &graph, &deps, &ndeps));
-        if (cs != cudaStreamCaptureStatusActive || !graph) return fail(MD_ECUDA, "stream is not capturing");
-        cudaGraphConditionalHandle cond;
-        CU(cudaGraphConditionalHandleCreate(&cond, graph, 0, cudaGraphCondAssignDefault));
-        if (g.dim == 3) k_kick_drift<3, true><<<nb, 256, 0, st>>>(g, pos, vel, force, s->ref_pos, a, dt, flag, cond);
-        else k_kick_drift<2, true><<<nb, 256, 0, st>>>(g, pos, vel, force, s->ref_pos, a, dt, flag, cond);
-        LAUNCH_OK();
-        CU(cudaStreamGetCaptureInfo(st, &cs, nullptr, &graph, &deps, &ndeps));
-        cudaGraphNodeParams np = {cudaGraphNodeTypeConditional};
-        np.type = cudaGraphNodeTypeConditional;
-        np.conditional.handle = cond;
-        np.conditional.type = cudaGraphCondTypeIf;
-        np.conditional.size = 1;
-        cudaGraphNode_t node;
-        CU(cudaGraphAddNode(&node, graph, deps, ndeps, &np));
-        cudaGraph_t body = np.conditional.phGraph_out[0];
-        if (!s->body_stream) CU(cudaStreamCreateWithFlags(&s->body_stream, cudaStreamNonBlocking));
-        CU(cudaStreamBeginCaptureToGraph(s->body_stream, body, nullptr, nullptr, 0, cudaStreamCaptureModeThreadLocal));
-        rc = launch_cell_build(s, pos, vel, id, s->cell_start_i, s->perm_i, status, nullptr, s->body_stream);
-        if (!rc) rc = launch_nbr_build(s, resort ? pos : s->pos_s, s->cell_start_i, resort ? nullptr : s->perm_i,
-                                       nbr_idx, nbr_count, status, nullptr, 1, s->body_stream);
-        cudaGraph_t ended = nullptr;
-        cudaError_t e = cudaStreamEndCapture(s->body_stream, &ended);
-        if (rc) return rc;
-        if (e != cudaSuccess) return fail(MD_ECUDA, "capturing the rebuild body: %s", cudaGetErrorString(e));
-        CU(cudaStreamUpdateCaptureDependencies(st, &node, 1, cudaStreamSetCaptureDependencies));
-    }
-    Book book = {flag, status, stats};
-    return launch_force(s, pp, pos, nbr_idx, nbr_count, force, vel, a, nullptr, false, book, st);
-}
-
 // Adds an IF node (condition `cond`) after the current capture front of `st` whose body is the
 // rebuild (cell list + re-sort + neighbor list) of the state held in `pos`; `st` continues after it.
 int record_rebuild_if(md_system *s, cudaStream_t st, cudaGraphConditionalHandle cond, float4 *pos,
@@ -458,6 +398,47 @@ int record_rebuild_if(md_system *s, cudaStream_t st, cudaGraphConditionalHandle 
     if (e != cudaSuccess) return fail(MD_ECUDA, "capturing the rebuild body: %s", cudaGetErrorString(e));
     CU(cudaStreamUpdateCaptureDependencies(st, &node, 1, cudaStreamSetCaptureDependencies));
     return MD_OK;
+}
+
+// One velocity-Verlet step as launches on `st` (captured into a graph or run directly).
+// in_graph: `st` is capturing; the rebuild kernels go into the body of an IF node whose condition
+// the drift kernel raises, so a step without a rebuild launches two kernels.  Otherwise every
+// rebuild kernel is launched and returns at once while the device flag is 0.
+int record_step(md_system *s, const Pair &pp, float4 *pos, float4 *vel, float4 *force, int *id,
+                int *nbr_idx, int *nbr_count, float dt, float mass, int *stats, cudaStream_t st,
+                bool in_graph) {
+    const Geom &g = s->g;
+    const float a = dt / (2.0f * mass);
+    int *flag = s->words + 0;
+    int *status = s->words + 1;
+    const int nb = blocks_for(g.n);
+    const bool resort = s->cfg.resort != 0;
+    int rc;
+    if (!in_graph) {
+        cudaGraphConditionalHandle none = 0;
+        if (g.dim == 3) k_kick_drift<3, false><<<nb, 256, 0, st>>>(g, pos, vel, force, s->ref_pos, a, dt, flag, none);
+        else k_kick_drift<2, false><<<nb, 256, 0, st>>>(g, pos, vel, force, s->ref_pos, a, dt, flag, none);
+        LAUNCH_OK();
+        rc = launch_cell_build(s, pos, vel, id, s->cell_start_i, s->perm_i, status, flag, st);
+        if (rc) return rc;
+        rc = launch_nbr_build(s, resort ? pos : s->pos_s, s->cell_start_i, resort ? nullptr : s->perm_i,
+                              nbr_idx, nbr_count, status, flag, 1, st);
+        if (rc) return rc;
+    } else {
+        cudaStreamCaptureStatus cs;
+        cudaGraph_t graph = nullptr;
+        CU(cudaStreamGetCaptureInfo(st, &cs, nullptr, &graph, nullptr, nullptr));
+        if (cs != cudaStreamCaptureStatusActive || !graph) return fail(MD_ECUDA, "stream is not capturing");
+        cudaGraphConditionalHandle cond;
+        CU(cudaGraphConditionalHandleCreate(&cond, graph, 0, cudaGraphCondAssignDefault));
+        if (g.dim == 3) k_kick_drift<3, true><<<nb, 256, 0, st>>>(g, pos, vel, force, s->ref_pos, a, dt, flag, cond);
+        else k_kick_drift<2, true><<<nb, 256, 0, st>>>(g, pos, vel, force, s->ref_pos, a, dt, flag, cond);
+        LAUNCH_OK();
+        rc = record_rebuild_if(s, st, cond, pos, vel, id, nbr_idx, nbr_count);
+        if (rc) return rc;
+    }
+    Book book = {flag, status, stats};
+    return launch_force(s, pp, pos, nbr_idx, nbr_count, force, vel, a, nullptr, false, book, st);
 }
 
 // `reps` fused steps on the capturing stream `st` (3-D LJ fast path): one k_kick_drift opens the
