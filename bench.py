@@ -54,7 +54,7 @@ def parse():
     ap.add_argument("--md-steps", type=int, default=100, help="MD steps per bench step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
-    ap.add_argument("--breakdown", action="store_true", help="also time build and force separately")
+    ap.add_argument("--breakdown", action="store_true", help="(kept for compatibility: the build time per rebuild is always reported)")
     return ap.parse_args()
 
 
@@ -250,7 +250,7 @@ def main():
         torch.cuda.synchronize(dev)
         force_ms_warm = a0.elapsed_time(b0) / reps
         build_ms = None
-        if args.breakdown:
+        if True:
             bev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(10)]
             for a, b in bev:
                 flush.zero_()

@@ -19,6 +19,13 @@
  *   orc_nve_run         L100 §3.3.1 NVE (init, update);  L72 shift function mu
  *   displacement        L72 §3.2.1 "displacement between a particle and the
  *                       nearest image of the second particle"
+ *   (the "next" rows)
+ *   kinds 2, 3, 4       L104 Morse [75], Buckingham-type [71-73], per-species LJ tables (L298-L305)
+ *   orc_fire_run        L100 "Fire Descent [68]", used at L322 (Bitzek et al.'s algorithm)
+ *   orc_brownian_run    L100 "Brownian" (Euler-Maruyama; kT = 0: "Gradient Descent")
+ *   orc_langevin_run    L100 "Langevin" (BAOAB splitting)
+ *   orc_nose_hoover_run L100 "Nose-Hoover [67]" (one thermostat, MTK splitting)
+ *   orc_normals         the counter-based normal generator both sides implement
  * Readings of everything the paper leaves open (strict <, half-skin, truncated
  * and shifted LJ, wrap convention, rounding of the inclusion predicate) are
  * SURVEY.md §8c A1-A18, restated in DESIGN.md §3.
@@ -27,7 +34,11 @@
  * something other than itself -- FCC shell counts and lattice sums, two-body
  * closed forms, finite differences, Newton's third law, translation
  * invariance, scipy's periodic cKDTree, NVE invariants, the harmonic
- * oscillator's exact discrete frequency.  The one unpinned thing is a chaotic
+ * oscillator's exact discrete frequency; for the "next" rows: closed-form two-body
+ * values and gradients of every potential, FIRE's schedule in closed form and its
+ * reduction to velocity Verlet, generator moments, free diffusion, exact friction
+ * decay and stationary variance, Nose-Hoover's conserved quantity at second order
+ * and its decoupled limit.  The one unpinned thing is a chaotic
  * trajectory beyond ~100 steps ("parity unpinned" by design).
  *
  * Arithmetic: fp64 everywhere, except the canonical inclusion predicate
