@@ -14,12 +14,13 @@
 // such a pair (1.5e-6) in line with the ~1e-6 of every other pair.
 // The fp32 error of F_i is a random sum of per-pair errors of relative size ~1e-7 * (7..13):
 // measured on the oracle (32k and 256k particles, lattice and liquid states) it stays below
-// 6e-6 * max(|F_i|, 1e-3) whenever S_i <= 8 * max(|F_i|, 1e-3).  A particle that fails this
-// test (its pair forces nearly cancel; 3-10 % of a liquid), or that has a pair within 1e-5 of
+// 5.4e-6 * max(|F_i|, 1e-3) whenever S_i <= 8 * max(|F_i|, 1e-3).  A particle that fails this
+// test (its pair forces nearly cancel; 3-4 % of a liquid, 12 % of the jittered lattice), or that has a pair within 1e-5 of
 // r_cut^2 (the truncated force jumps by 0.039 there, so the in/out decision must be the exact
-// one), is re-evaluated in fp64 from exact displacements by a group of 8 lanes striding over
-// its row (four such particles per warp at a time).  Both results are rounded to fp32 once, on
-// store.
+// one), is re-evaluated in fp64 from exact displacements inside its own warp: groups of 32, 16 or
+// 8 lanes stride over the particle's row (1, 2 or up to 4 flagged particles at a time) and reduce
+// by shuffles.  Both results are rounded to fp32 once, on store.  (A separate queue + second kernel
+// for the re-evaluation was measured slower.)
 #pragma once
 #include "md_kernels.cuh"
 
