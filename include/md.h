@@ -217,7 +217,8 @@ int md_nve_step(md_system *sys, const md_potential *pot, void *pos, void *vel, v
  * index) -- splitmix64 finaliser, two 24-bit uniforms, Box-Muller -- so a run is reproducible and
  * independent of the particle order the re-sort leaves; id = NULL keys by slot (resort = 0 only).
  *   force   must hold F(pos) on entry, holds F of the final positions on exit; there are no
- *           velocities; lists and stats as in md_nve_step.  Kernels are launched directly (no graph).
+ *           velocities; lists and stats as in md_nve_step.  Runs as CUDA graphs of 8 steps (rebuild in an IF
+ *           node) unless use_graph = 0.
  */
 int md_brownian_step(md_system *sys, const md_potential *pot, void *pos, void *force, int32_t *id,
                      int32_t *nbr_idx, int32_t *nbr_count, float dt, float gamma, float kT,
@@ -229,7 +230,7 @@ int md_brownian_step(md_system *sys, const md_potential *pot, void *pos, void *f
  *   r = wrap(r + dt/2 v);  [rebuild];  F = F(r);  v += dt/(2m) F
  * xi as in md_brownian_step (same generator, keyed by seed, step0 + s, id[i]).  gamma = 0 is
  * md_nve_step's velocity Verlet.  force must hold F(pos) on entry; lists and stats as in md_nve_step.
- * Kernels are launched directly (no graph).
+ * CUDA graphs of 8 steps unless use_graph = 0.
  */
 int md_langevin_step(md_system *sys, const md_potential *pot, void *pos, void *vel, void *force,
                      int32_t *id, int32_t *nbr_idx, int32_t *nbr_count, float dt, float mass,
@@ -244,7 +245,8 @@ int md_langevin_step(md_system *sys, const md_potential *pot, void *pos, void *v
  *          K2 *= exp(-dt vxi); G = (K2 - dof kT)/Q; vxi += dt/4 G
  *   nh_state  device double[2] in/out = {xi, vxi} (zero to start); H' = K + U + Q vxi^2/2 + dof kT xi
  *             is the conserved quantity
- * force must hold F(pos) on entry; lists and stats as in md_nve_step.  Direct launches (no graph).
+ * force must hold F(pos) on entry; lists and stats as in md_nve_step.  CUDA graphs of 8 steps unless
+ * use_graph = 0.
  */
 int md_nose_hoover_step(md_system *sys, const md_potential *pot, void *pos, void *vel, void *force,
                         int32_t *id, int32_t *nbr_idx, int32_t *nbr_count, float dt, float mass,
@@ -269,7 +271,7 @@ typedef struct md_fire_params {
  *   fire_state  device float[4] in/out = {dt, alpha, n_pos, sign of the last P}; dt <= 0 on entry
  *               starts from (dt_start, alpha_start, 0); pass it back unchanged to continue a run
  *   force       must hold F(pos) on entry, holds F of the final positions on exit; the lists as in
- *               md_nve_step; stats as in md_nve_step.  Kernels are launched directly (no graph).
+ *               md_nve_step; stats as in md_nve_step.  CUDA graphs of 8 steps unless use_graph = 0.
  */
 int md_fire_minimize(md_system *sys, const md_potential *pot, const md_fire_params *par, void *pos,
                      void *vel, void *force, int32_t *id, int32_t *nbr_idx, int32_t *nbr_count,

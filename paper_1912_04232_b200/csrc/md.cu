@@ -52,6 +52,22 @@ size_t up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 int blocks_for(long long threads, int block = 256) { return (int)((threads + block - 1) / block); }
 
+enum { RULE_FIRE = 1, RULE_BROWNIAN, RULE_LANGEVIN, RULE_NH };
+
+// Everything one step of an update rule other than NVE depends on (plain data, compared bytewise
+// to decide whether the cached graphs still apply).
+struct RuleArgs {
+    int rule;
+    void *pos, *vel, *force, *state;
+    int *id, *nbr_idx, *nbr_count, *stats;
+    md_potential pot;
+    float dt, mass, gamma, kT, tau;
+    unsigned seed, step0;
+    md_fire_params fire;
+    int fast32, builder, nb_parts, remap;
+    float est_thr;
+};
+
 struct StepKey {
     const void *pos, *vel, *force, *id, *nbr_idx, *nbr_count, *stats;
     float dt, mass;
@@ -95,6 +111,10 @@ struct md_system {
     bool key_valid;
     cudaGraphExec_t exec1, execU;
     int unroll;
+    // graph cache of the other update rules (FIRE, Brownian, Langevin, Nose-Hoover)
+    RuleArgs rule_key;
+    bool rule_key_valid;
+    cudaGraphExec_t rule_exec1, rule_execU;
 };
 
 namespace {
@@ -481,8 +501,11 @@ int record_fused(md_system *s, const Pair &pp, float4 *pos, float4 *vel, float4 
 void drop_graphs(md_system *s) {
     if (s->exec1) cudaGraphExecDestroy(s->exec1);
     if (s->execU) cudaGraphExecDestroy(s->execU);
-    s->exec1 = s->execU = nullptr;
+    if (s->rule_exec1) cudaGraphExecDestroy(s->rule_exec1);
+    if (s->rule_execU) cudaGraphExecDestroy(s->rule_execU);
+    s->exec1 = s->execU = s->rule_exec1 = s->rule_execU = nullptr;
     s->key_valid = false;
+    s->rule_key_valid = false;
 }
 
 int capture(md_system *s, const Pair &pp, const StepKey &k, int reps, cudaGraphExec_t *out) {
@@ -505,6 +528,139 @@ int capture(md_system *s, const Pair &pp, const StepKey &k, int reps, cudaGraphE
     e = cudaGraphInstantiate(out, graph, 0);
     cudaGraphDestroy(graph);
     if (e != cudaSuccess) return fail(MD_ECUDA, "cudaGraphInstantiate: %s", cudaGetErrorString(e));
+    return MD_OK;
+}
+
+// One step of an update rule other than NVE on `st`: the rule's opening kernels up to the drift (which
+// raises the rebuild flag / graph condition), the rebuild (an IF node when capturing, kernels that
+// return at once on a zero flag otherwise), the force, the rule's closing kernels.
+int record_rule_step(md_system *s, const Pair &pp, const RuleArgs &A, cudaStream_t st, bool in_graph) {
+    const Geom &g = s->g;
+    int *flag = s->words + 0, *status = s->words + 1;
+    const bool resort = s->cfg.resort != 0;
+    const int nb = blocks_for(g.n);
+    float4 *p4 = (float4 *)A.pos, *v4 = (float4 *)A.vel, *f4 = (float4 *)A.force;
+    Raise rs = {flag, 0, 0};
+    if (in_graph) {
+        cudaStreamCaptureStatus cs;
+        cudaGraph_t graph = nullptr;
+        CU(cudaStreamGetCaptureInfo(st, &cs, nullptr, &graph, nullptr, nullptr));
+        if (cs != cudaStreamCaptureStatusActive || !graph) return fail(MD_ECUDA, "stream is not capturing");
+        CU(cudaGraphConditionalHandleCreate(&rs.cond, graph, 0, cudaGraphCondAssignDefault));
+        rs.has_cond = 1;
+    }
+    const float a = A.dt / (2.0f * A.mass);           // half-kick factor (Langevin, Nose-Hoover)
+    float4 *force_vel = nullptr;                      // velocities the force kernel half-kicks
+    float force_a = 0.0f;
+    const int nbk = blocks_for(g.n, NH_BLOCK), nbf = blocks_for(g.n, FIRE_BLOCK);
+    double *partial = s->fire_tmp;
+    switch (A.rule) {
+    case RULE_FIRE:
+        if (g.dim == 3) k_fire_kick_drift<3><<<nb, 256, 0, st>>>(g, p4, v4, f4, s->ref_pos, (const float *)A.state, rs);
+        else k_fire_kick_drift<2><<<nb, 256, 0, st>>>(g, p4, v4, f4, s->ref_pos, (const float *)A.state, rs);
+        break;
+    case RULE_BROWNIAN: {
+        const float mu = A.dt / A.gamma, amp = std::sqrt(2.0f * A.kT * A.dt / A.gamma);
+        if (g.dim == 3) k_brownian_drift<3><<<nb, 256, 0, st>>>(g, p4, f4, A.id, s->ref_pos, mu, amp, A.seed, A.step0, A.stats, rs);
+        else k_brownian_drift<2><<<nb, 256, 0, st>>>(g, p4, f4, A.id, s->ref_pos, mu, amp, A.seed, A.step0, A.stats, rs);
+        break;
+    }
+    case RULE_LANGEVIN: {
+        const double c1d = std::exp(-(double)A.gamma * (double)A.dt);
+        const float c1 = (float)c1d, c2 = (float)std::sqrt((double)A.kT / (double)A.mass * (1.0 - c1d * c1d));
+        if (g.dim == 3) k_langevin_baoa<3><<<nb, 256, 0, st>>>(g, p4, v4, f4, A.id, s->ref_pos, a, A.dt, c1, c2, A.seed, A.step0, A.stats, rs);
+        else k_langevin_baoa<2><<<nb, 256, 0, st>>>(g, p4, v4, f4, A.id, s->ref_pos, a, A.dt, c1, c2, A.seed, A.step0, A.stats, rs);
+        force_vel = v4; force_a = a;
+        break;
+    }
+    case RULE_NH: {
+        const double dofkT = (double)g.dim * g.n * (double)A.kT, Q = dofkT * (double)A.tau * (double)A.tau;
+        float *scale = reinterpret_cast<float *>(s->fire_tmp + nbk);
+        k_nh_ke<<<nbk, NH_BLOCK, 0, st>>>(g.n, g.dim, v4, partial);
+        k_nh_finalize<<<1, 256, 0, st>>>(nbk, partial, (double)A.mass, dofkT, Q, (double)A.dt, (double *)A.state, scale);
+        if (g.dim == 3) k_nh_kick_drift<3><<<nb, 256, 0, st>>>(g, p4, v4, f4, s->ref_pos, a, A.dt, scale, rs);
+        else k_nh_kick_drift<2><<<nb, 256, 0, st>>>(g, p4, v4, f4, s->ref_pos, a, A.dt, scale, rs);
+        force_vel = v4; force_a = a;
+        break;
+    }
+    default: return fail(MD_EINVAL, "unknown update rule %d", A.rule);
+    }
+    LAUNCH_OK();
+    float4 *sort_vel = A.rule == RULE_BROWNIAN ? nullptr : v4;
+    int rc;
+    if (in_graph) {
+        rc = record_rebuild_if(s, st, rs.cond, p4, sort_vel, A.id, A.nbr_idx, A.nbr_count);
+        if (rc) return rc;
+    } else {
+        rc = launch_cell_build(s, p4, sort_vel, A.id, s->cell_start_i, s->perm_i, status, flag, st);
+        if (rc) return rc;
+        rc = launch_nbr_build(s, resort ? p4 : s->pos_s, s->cell_start_i, resort ? nullptr : s->perm_i,
+                              A.nbr_idx, A.nbr_count, status, flag, 1, st);
+        if (rc) return rc;
+    }
+    Book book = {flag, status, A.stats};
+    rc = launch_force(s, pp, p4, A.nbr_idx, A.nbr_count, f4, force_vel, force_a, nullptr, false, book, st);
+    if (rc) return rc;
+    if (A.rule == RULE_FIRE) {
+        const FirePar fp = {A.fire.dt_start, A.fire.dt_max, A.fire.n_min, A.fire.f_inc, A.fire.f_dec,
+                            A.fire.alpha_start, A.fire.f_alpha};
+        float *coef = reinterpret_cast<float *>(s->fire_tmp + (size_t)nbf * 3);
+        k_fire_kick_reduce<<<nbf, FIRE_BLOCK, 0, st>>>(g.n, g.dim, v4, f4, (const float *)A.state, partial);
+        k_fire_finalize<<<1, 256, 0, st>>>(nbf, partial, fp, (float *)A.state, coef);
+        k_fire_mix<<<nb, 256, 0, st>>>(g.n, v4, f4, coef);
+        LAUNCH_OK();
+    } else if (A.rule == RULE_NH) {
+        const double dofkT = (double)g.dim * g.n * (double)A.kT, Q = dofkT * (double)A.tau * (double)A.tau;
+        float *scale = reinterpret_cast<float *>(s->fire_tmp + nbk);
+        k_nh_ke<<<nbk, NH_BLOCK, 0, st>>>(g.n, g.dim, v4, partial);
+        k_nh_finalize<<<1, 256, 0, st>>>(nbk, partial, (double)A.mass, dofkT, Q, (double)A.dt, (double *)A.state, scale);
+        k_nh_scale<<<nb, 256, 0, st>>>(g.n, v4, scale);
+        LAUNCH_OK();
+    }
+    return MD_OK;
+}
+
+int capture_rule(md_system *s, const Pair &pp, const RuleArgs &A, int reps, cudaGraphExec_t *out) {
+    if (!s->cap_stream) CU(cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking));
+    CU(cudaStreamBeginCapture(s->cap_stream, cudaStreamCaptureModeThreadLocal));
+    int rc = MD_OK;
+    for (int r = 0; r < reps && rc == MD_OK; ++r) rc = record_rule_step(s, pp, A, s->cap_stream, true);
+    cudaGraph_t graph = nullptr;
+    cudaError_t e = cudaStreamEndCapture(s->cap_stream, &graph);
+    if (rc) { if (graph) cudaGraphDestroy(graph); return rc; }
+    if (e != cudaSuccess) return fail(MD_ECUDA, "cudaStreamEndCapture: %s", cudaGetErrorString(e));
+    e = cudaGraphInstantiate(out, graph, 0);
+    cudaGraphDestroy(graph);
+    if (e != cudaSuccess) return fail(MD_ECUDA, "cudaGraphInstantiate: %s", cudaGetErrorString(e));
+    return MD_OK;
+}
+
+// nsteps of an update rule: stats reset, then graphs of 8 steps and of 1 step (or direct launches).
+int run_rule(md_system *s, const Pair &pp, RuleArgs &A, int nsteps, cudaStream_t st) {
+    A.fast32 = s->fast32; A.builder = s->builder; A.nb_parts = s->nb_parts; A.remap = s->remap; A.est_thr = s->est_thr;
+    k_init_stats<<<1, 1, 0, st>>>(A.stats, s->words + 0);
+    LAUNCH_OK();
+    if (!s->use_graph) {
+        for (int k = 0; k < nsteps; ++k) { int rc = record_rule_step(s, pp, A, st, false); if (rc) return rc; }
+        return MD_OK;
+    }
+    if (!s->rule_key_valid || memcmp(&A, &s->rule_key, sizeof(A)) != 0) {
+        if (s->rule_exec1) cudaGraphExecDestroy(s->rule_exec1);
+        if (s->rule_execU) cudaGraphExecDestroy(s->rule_execU);
+        s->rule_exec1 = s->rule_execU = nullptr;
+        s->rule_key = A;
+        s->rule_key_valid = true;
+    }
+    const int U = 8;
+    int left = nsteps, rc;
+    if (left >= U) {
+        if (!s->rule_execU) { rc = capture_rule(s, pp, A, U, &s->rule_execU); if (rc) return rc; }
+        for (; left >= U; left -= U) CU(cudaGraphLaunch(s->rule_execU, st));
+    }
+    if (left > 0) {
+        if (!s->rule_exec1) { rc = capture_rule(s, pp, A, 1, &s->rule_exec1); if (rc) return rc; }
+        for (; left > 0; --left) CU(cudaGraphLaunch(s->rule_exec1, st));
+    }
     return MD_OK;
 }
 
@@ -789,29 +945,11 @@ int md_brownian_step(md_system *sys, const md_potential *pot, void *pos, void *f
     int rc = make_pair(sys, pot, &pp);
     if (rc) return rc;
     if ((rc = enter(sys))) return rc;
-    cudaStream_t st = (cudaStream_t)stream;
-    const Geom &g = sys->g;
-    int *flag = sys->words + 0, *status = sys->words + 1;
-    const bool resort = sys->cfg.resort != 0;
-    const int nb = blocks_for(g.n);
-    const float mu = dt / gamma, amp = std::sqrt(2.0f * kT * dt / gamma);
-    float4 *p4 = (float4 *)pos, *f4 = (float4 *)force;
-    k_init_stats<<<1, 1, 0, st>>>(stats, sys->words + 0);
-    LAUNCH_OK();
-    for (int s = 0; s < nsteps; ++s) {
-        if (g.dim == 3) k_brownian_drift<3><<<nb, 256, 0, st>>>(g, p4, f4, id, sys->ref_pos, mu, amp, seed, step0 + (uint32_t)s, flag);
-        else k_brownian_drift<2><<<nb, 256, 0, st>>>(g, p4, f4, id, sys->ref_pos, mu, amp, seed, step0 + (uint32_t)s, flag);
-        LAUNCH_OK();
-        rc = launch_cell_build(sys, p4, nullptr, id, sys->cell_start_i, sys->perm_i, status, flag, st);
-        if (rc) return rc;
-        rc = launch_nbr_build(sys, resort ? p4 : sys->pos_s, sys->cell_start_i, resort ? nullptr : sys->perm_i,
-                              nbr_idx, nbr_count, status, flag, 1, st);
-        if (rc) return rc;
-        Book book = {flag, status, stats};
-        rc = launch_force(sys, pp, p4, nbr_idx, nbr_count, f4, nullptr, 0.0f, nullptr, false, book, st);
-        if (rc) return rc;
-    }
-    return MD_OK;
+    RuleArgs A;
+    memset(&A, 0, sizeof(A));
+    A.rule = RULE_BROWNIAN; A.pos = pos; A.force = force; A.id = id; A.nbr_idx = nbr_idx; A.nbr_count = nbr_count;
+    A.stats = stats; A.pot = *pot; A.dt = dt; A.mass = 1.0f; A.gamma = gamma; A.kT = kT; A.seed = seed; A.step0 = step0;
+    return run_rule(sys, pp, A, nsteps, (cudaStream_t)stream);
 }
 
 int md_langevin_step(md_system *sys, const md_potential *pot, void *pos, void *vel, void *force,
@@ -826,31 +964,12 @@ int md_langevin_step(md_system *sys, const md_potential *pot, void *pos, void *v
     int rc = make_pair(sys, pot, &pp);
     if (rc) return rc;
     if ((rc = enter(sys))) return rc;
-    cudaStream_t st = (cudaStream_t)stream;
-    const Geom &g = sys->g;
-    int *flag = sys->words + 0, *status = sys->words + 1;
-    const bool resort = sys->cfg.resort != 0;
-    const int nb = blocks_for(g.n);
-    const float a = dt / (2.0f * mass);
-    const double c1d = std::exp(-(double)gamma * (double)dt);
-    const float c1 = (float)c1d, c2 = (float)std::sqrt((double)kT / (double)mass * (1.0 - c1d * c1d));
-    float4 *p4 = (float4 *)pos, *v4 = (float4 *)vel, *f4 = (float4 *)force;
-    k_init_stats<<<1, 1, 0, st>>>(stats, sys->words + 0);
-    LAUNCH_OK();
-    for (int s = 0; s < nsteps; ++s) {
-        if (g.dim == 3) k_langevin_baoa<3><<<nb, 256, 0, st>>>(g, p4, v4, f4, id, sys->ref_pos, a, dt, c1, c2, seed, step0 + (uint32_t)s, flag);
-        else k_langevin_baoa<2><<<nb, 256, 0, st>>>(g, p4, v4, f4, id, sys->ref_pos, a, dt, c1, c2, seed, step0 + (uint32_t)s, flag);
-        LAUNCH_OK();
-        rc = launch_cell_build(sys, p4, v4, id, sys->cell_start_i, sys->perm_i, status, flag, st);
-        if (rc) return rc;
-        rc = launch_nbr_build(sys, resort ? p4 : sys->pos_s, sys->cell_start_i, resort ? nullptr : sys->perm_i,
-                              nbr_idx, nbr_count, status, flag, 1, st);
-        if (rc) return rc;
-        Book book = {flag, status, stats};
-        rc = launch_force(sys, pp, p4, nbr_idx, nbr_count, f4, v4, a, nullptr, false, book, st);
-        if (rc) return rc;
-    }
-    return MD_OK;
+    RuleArgs A;
+    memset(&A, 0, sizeof(A));
+    A.rule = RULE_LANGEVIN; A.pos = pos; A.vel = vel; A.force = force; A.id = id; A.nbr_idx = nbr_idx;
+    A.nbr_count = nbr_count; A.stats = stats; A.pot = *pot; A.dt = dt; A.mass = mass; A.gamma = gamma; A.kT = kT;
+    A.seed = seed; A.step0 = step0;
+    return run_rule(sys, pp, A, nsteps, (cudaStream_t)stream);
 }
 
 int md_nose_hoover_step(md_system *sys, const md_potential *pot, void *pos, void *vel, void *force,
@@ -865,38 +984,11 @@ int md_nose_hoover_step(md_system *sys, const md_potential *pot, void *pos, void
     int rc = make_pair(sys, pot, &pp);
     if (rc) return rc;
     if ((rc = enter(sys))) return rc;
-    cudaStream_t st = (cudaStream_t)stream;
-    const Geom &g = sys->g;
-    int *flag = sys->words + 0, *status = sys->words + 1;
-    const bool resort = sys->cfg.resort != 0;
-    const int nb = blocks_for(g.n), nbk = blocks_for(g.n, NH_BLOCK);
-    const float a = dt / (2.0f * mass);
-    const double dofkT = (double)g.dim * g.n * (double)kT, Q = dofkT * (double)tau * (double)tau;
-    double *partial = sys->fire_tmp;
-    float *scale = reinterpret_cast<float *>(sys->fire_tmp + nbk);
-    float4 *p4 = (float4 *)pos, *v4 = (float4 *)vel, *f4 = (float4 *)force;
-    k_init_stats<<<1, 1, 0, st>>>(stats, sys->words + 0);
-    LAUNCH_OK();
-    for (int s = 0; s < nsteps; ++s) {
-        k_nh_ke<<<nbk, NH_BLOCK, 0, st>>>(g.n, g.dim, v4, partial);
-        k_nh_finalize<<<1, 256, 0, st>>>(nbk, partial, (double)mass, dofkT, Q, (double)dt, nh_state, scale);
-        if (g.dim == 3) k_nh_kick_drift<3><<<nb, 256, 0, st>>>(g, p4, v4, f4, sys->ref_pos, a, dt, scale, flag);
-        else k_nh_kick_drift<2><<<nb, 256, 0, st>>>(g, p4, v4, f4, sys->ref_pos, a, dt, scale, flag);
-        LAUNCH_OK();
-        rc = launch_cell_build(sys, p4, v4, id, sys->cell_start_i, sys->perm_i, status, flag, st);
-        if (rc) return rc;
-        rc = launch_nbr_build(sys, resort ? p4 : sys->pos_s, sys->cell_start_i, resort ? nullptr : sys->perm_i,
-                              nbr_idx, nbr_count, status, flag, 1, st);
-        if (rc) return rc;
-        Book book = {flag, status, stats};
-        rc = launch_force(sys, pp, p4, nbr_idx, nbr_count, f4, v4, a, nullptr, false, book, st);
-        if (rc) return rc;
-        k_nh_ke<<<nbk, NH_BLOCK, 0, st>>>(g.n, g.dim, v4, partial);
-        k_nh_finalize<<<1, 256, 0, st>>>(nbk, partial, (double)mass, dofkT, Q, (double)dt, nh_state, scale);
-        k_nh_scale<<<nb, 256, 0, st>>>(g.n, v4, scale);
-        LAUNCH_OK();
-    }
-    return MD_OK;
+    RuleArgs A;
+    memset(&A, 0, sizeof(A));
+    A.rule = RULE_NH; A.pos = pos; A.vel = vel; A.force = force; A.state = nh_state; A.id = id; A.nbr_idx = nbr_idx;
+    A.nbr_count = nbr_count; A.stats = stats; A.pot = *pot; A.dt = dt; A.mass = mass; A.kT = kT; A.tau = tau;
+    return run_rule(sys, pp, A, nsteps, (cudaStream_t)stream);
 }
 
 int md_fire_minimize(md_system *sys, const md_potential *pot, const md_fire_params *par, void *pos,
@@ -914,38 +1006,14 @@ int md_fire_minimize(md_system *sys, const md_potential *pot, const md_fire_para
     if (rc) return rc;
     if ((rc = enter(sys))) return rc;
     cudaStream_t st = (cudaStream_t)stream;
-    const Geom &g = sys->g;
     const FirePar fp = {par->dt_start, par->dt_max, par->n_min, par->f_inc, par->f_dec, par->alpha_start, par->f_alpha};
-    int *flag = sys->words + 0, *status = sys->words + 1;
-    const bool resort = sys->cfg.resort != 0;
-    const int nb = blocks_for(g.n), nbr = blocks_for(g.n, FIRE_BLOCK);
-    double *partial = sys->fire_tmp;
-    float *coef = reinterpret_cast<float *>(sys->fire_tmp + (size_t)nbr * 3);
-    float4 *p4 = (float4 *)pos, *v4 = (float4 *)vel, *f4 = (float4 *)force;
-    k_init_stats<<<1, 1, 0, st>>>(stats, sys->words + 0);
-    LAUNCH_OK();
     k_fire_init<<<1, 1, 0, st>>>(fp, fire_state);
     LAUNCH_OK();
-    for (int s = 0; s < nsteps; ++s) {
-        if (g.dim == 3) k_fire_kick_drift<3><<<nb, 256, 0, st>>>(g, p4, v4, f4, sys->ref_pos, fire_state, flag);
-        else k_fire_kick_drift<2><<<nb, 256, 0, st>>>(g, p4, v4, f4, sys->ref_pos, fire_state, flag);
-        LAUNCH_OK();
-        rc = launch_cell_build(sys, p4, v4, id, sys->cell_start_i, sys->perm_i, status, flag, st);
-        if (rc) return rc;
-        rc = launch_nbr_build(sys, resort ? p4 : sys->pos_s, sys->cell_start_i, resort ? nullptr : sys->perm_i,
-                              nbr_idx, nbr_count, status, flag, 1, st);
-        if (rc) return rc;
-        Book book = {flag, status, stats};
-        rc = launch_force(sys, pp, p4, nbr_idx, nbr_count, f4, nullptr, 0.0f, nullptr, false, book, st);
-        if (rc) return rc;
-        k_fire_kick_reduce<<<nbr, FIRE_BLOCK, 0, st>>>(g.n, g.dim, v4, f4, fire_state, partial);
-        LAUNCH_OK();
-        k_fire_finalize<<<1, 256, 0, st>>>(nbr, partial, fp, fire_state, coef);
-        LAUNCH_OK();
-        k_fire_mix<<<nb, 256, 0, st>>>(g.n, v4, f4, coef);
-        LAUNCH_OK();
-    }
-    return MD_OK;
+    RuleArgs A;
+    memset(&A, 0, sizeof(A));
+    A.rule = RULE_FIRE; A.pos = pos; A.vel = vel; A.force = force; A.state = fire_state; A.id = id; A.nbr_idx = nbr_idx;
+    A.nbr_count = nbr_count; A.stats = stats; A.pot = *pot; A.mass = 1.0f; A.fire = *par;
+    return run_rule(sys, pp, A, nsteps, st);
 }
 
 // md_nve_run_host keeps ONE context (device allocation, system, stream, and through the system the

@@ -30,7 +30,8 @@ template <int DIM>
 __global__ void __launch_bounds__(256)
 k_brownian_drift(Geom g, float4 *__restrict__ pos, const float4 *__restrict__ force,
                  const int *__restrict__ id, const float4 *__restrict__ ref, float mu, float amp,
-                 unsigned seed, unsigned step, int *flag) {
+                 unsigned seed, unsigned step0, const int *__restrict__ steps_done, Raise rs) {
+    const unsigned step = step0 + (unsigned)*steps_done;      // stats[0]: steps finished in this call
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     bool moved = false;
     if (i < g.n) {
@@ -48,7 +49,7 @@ k_brownian_drift(Geom g, float4 *__restrict__ pos, const float4 *__restrict__ fo
         pos[i] = p;
         moved = disp2_from_ref<DIM>(g, p, ref[i]) > g.half_skin2;
     }
-    if (__any_sync(FULL, moved) && (threadIdx.x & 31) == 0) *flag = 1;
+    if (__any_sync(FULL, moved) && (threadIdx.x & 31) == 0) raise_rebuild(rs);
 }
 
 // Langevin dynamics, BAOAB (reading A22), first four letters:
@@ -59,7 +60,8 @@ __global__ void __launch_bounds__(256)
 k_langevin_baoa(Geom g, float4 *__restrict__ pos, float4 *__restrict__ vel,
                 const float4 *__restrict__ force, const int *__restrict__ id,
                 const float4 *__restrict__ ref, float a, float dt, float c1, float c2,
-                unsigned seed, unsigned step, int *flag) {
+                unsigned seed, unsigned step0, const int *__restrict__ steps_done, Raise rs) {
+    const unsigned step = step0 + (unsigned)*steps_done;      // stats[0]: steps finished in this call
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     bool moved = false;
     if (i < g.n) {
@@ -86,7 +88,7 @@ k_langevin_baoa(Geom g, float4 *__restrict__ pos, float4 *__restrict__ vel,
         pos[i] = p; vel[i] = v;
         moved = disp2_from_ref<DIM>(g, p, ref[i]) > g.half_skin2;
     }
-    if (__any_sync(FULL, moved) && (threadIdx.x & 31) == 0) *flag = 1;
+    if (__any_sync(FULL, moved) && (threadIdx.x & 31) == 0) raise_rebuild(rs);
 }
 
 } // namespace mdk

@@ -23,7 +23,7 @@ template <int DIM>
 __global__ void __launch_bounds__(256)
 k_fire_kick_drift(Geom g, float4 *__restrict__ pos, float4 *__restrict__ vel,
                   const float4 *__restrict__ force, const float4 *__restrict__ ref,
-                  const float *__restrict__ state, int *flag) {
+                  const float *__restrict__ state, Raise rs) {
     const float dt = state[0], a = 0.5f * dt;
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     bool moved = false;
@@ -40,7 +40,7 @@ k_fire_kick_drift(Geom g, float4 *__restrict__ pos, float4 *__restrict__ vel,
         pos[i] = p; vel[i] = v;
         moved = disp2_from_ref<DIM>(g, p, ref[i]) > g.half_skin2;
     }
-    if (__any_sync(FULL, moved) && (threadIdx.x & 31) == 0) *flag = 1;
+    if (__any_sync(FULL, moved) && (threadIdx.x & 31) == 0) raise_rebuild(rs);
 }
 
 // second half-kick and the three sums; block b writes its partial sums to partial[3 b ..]

@@ -48,6 +48,18 @@ struct Book {
 
 __device__ __forceinline__ int ld_volatile(const int *p) { return *(const volatile int *)p; }
 
+// What a drift kernel does when one of its particles has moved beyond skin/2: raise the device
+// flag and, when the step runs inside a CUDA graph, the condition of the rebuild's IF node.
+struct Raise {
+    int *flag;
+    cudaGraphConditionalHandle cond;
+    int has_cond;
+};
+__device__ __forceinline__ void raise_rebuild(const Raise &r) {
+    *r.flag = 1;
+    if (r.has_cond) cudaGraphSetConditional(r.cond, 1);
+}
+
 // ---------------------------------------------------------------- space (L72 §3.2.1) ----
 
 // Canonical cell coordinate c_k = min(n_k-1, (int)(x_k * inv_k)).

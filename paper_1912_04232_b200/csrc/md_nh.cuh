@@ -62,7 +62,7 @@ template <int DIM>
 __global__ void __launch_bounds__(256)
 k_nh_kick_drift(Geom g, float4 *__restrict__ pos, float4 *__restrict__ vel,
                 const float4 *__restrict__ force, const float4 *__restrict__ ref, float a, float dt,
-                const float *__restrict__ scale, int *flag) {
+                const float *__restrict__ scale, Raise rs) {
     const float sc = *scale;
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     bool moved = false;
@@ -79,7 +79,7 @@ k_nh_kick_drift(Geom g, float4 *__restrict__ pos, float4 *__restrict__ vel,
         pos[i] = p; vel[i] = v;
         moved = disp2_from_ref<DIM>(g, p, ref[i]) > g.half_skin2;
     }
-    if (__any_sync(FULL, moved) && (threadIdx.x & 31) == 0) *flag = 1;
+    if (__any_sync(FULL, moved) && (threadIdx.x & 31) == 0) raise_rebuild(rs);
 }
 
 __global__ void __launch_bounds__(256)

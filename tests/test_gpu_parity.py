@@ -470,6 +470,41 @@ def test_species_lj_binary_mixture(B, orc, W):
     S1.close(); S0.close()
 
 
+@pytest.mark.parametrize("rule", ["fire", "brownian", "langevin", "nose_hoover"])
+def test_update_rules_graph_and_direct_launch_agree(B, W, rule):
+    """Every update rule beyond NVE runs as CUDA graphs of 8 steps (rebuild in an IF node, step
+    counter and rule state on the device) or, with use_graph = 0, as direct launches: same bits,
+    also when the run is split into calls that mix both graph sizes."""
+    w = W.config(0)
+    out = []
+    for graph, split in ((1, (37,)), (0, (37,)), (1, (5, 16, 16))):
+        S = B.System(w)
+        B.md_set_option(S.sys, "use_graph", graph)
+        S.build(); S.compute_force()
+        st32 = torch.zeros(4, dtype=torch.float32, device="cuda")
+        st64 = torch.zeros(2, dtype=torch.float64, device="cuda")
+        done = 0
+        for k in split:
+            if rule == "fire":
+                fp = B.md_fire_params(0.002, 0.02, 5, 1.1, 0.5, 0.1, 0.99)
+                B.md_fire_minimize(S.sys, S.pot, fp, S.pos, S.vel, S.force, S.id, S.nbr_idx, S.nbr_count, st32, k, S.stats)
+            elif rule == "brownian":
+                B.md_brownian_step(S.sys, S.pot, S.pos, S.force, S.id, S.nbr_idx, S.nbr_count, 2e-4, 1.0, 0.8, 3, done, k, S.stats)
+            elif rule == "langevin":
+                B.md_langevin_step(S.sys, S.pot, S.pos, S.vel, S.force, S.id, S.nbr_idx, S.nbr_count, 0.004, 1.0, 2.0, 0.8,
+                                   3, done, k, S.stats)
+            else:
+                B.md_nose_hoover_step(S.sys, S.pot, S.pos, S.vel, S.force, S.id, S.nbr_idx, S.nbr_count, 0.004, 1.0, 0.5,
+                                      0.2, st64, k, S.stats)
+            done += k
+        torch.cuda.synchronize()
+        out.append((S.pos.clone(), S.vel.clone(), S.force.clone(), S.id.clone(), st32.clone(), st64.clone()))
+        S.close()
+    for o in out[1:]:
+        for x, y in zip(out[0], o):
+            assert torch.equal(x, y)
+
+
 def test_fast32_dimers_at_the_force_zero(B, orc, W):
     """Isolated pairs around r = 2^(1/6) sigma, where the LJ force changes sign: the coefficient and
     with it sum|coefficient| vanish while the fp32 rounding error does not, so the error estimate
