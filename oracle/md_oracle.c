@@ -909,3 +909,105 @@ int orc_nose_hoover_run(int n, int dim, double *pos, double *vel, double *force,
     free(e_i);
     return rc;
 }
+
+/* -------------------------------------------------------------- flocking -- */
+
+/*
+ * Boids as an energy model (App. B), 2-D, state (R_i, theta_i), N(theta) =
+ * (cos theta, sin theta).  DESIGN.md reading A25 for what the text leaves open:
+ *   rho(r; Rc)   = (1/alpha)(1 - r/Rc)^alpha for r < Rc, else 0                          (eq. 6)
+ *   E_align      = 1/2 sum_{i != j} J_al rho(r_ij; R_al) (1 - N_i.N_j)^2                  (eq. 7)
+ *                  with a stop-gradient on the displacement: it has NO gradient in R
+ *   E_avoid      = 1/2 sum_{i != j} J_av rho(r_ij; R_av)                                  (eq. 8)
+ *   E_cohesion   = sum_i 1/2 J_co (1 - Dhat_i.N_i)^2,  D_i = sum_{j in N_i} (R_j - R_i),
+ *                  N_i = {j : r_ij < R_co}; 0 when N_i is empty or D_i = 0       (eqs. 9-10; the
+ *                  normalised mean of eq. 9 equals the normalised sum; the set is held fixed)
+ * par = {J_al, R_al, J_av, R_av, J_co, R_co, alpha}.  Outputs: energies[3] = (align, avoid, cohesion),
+ * gR double[n*2] = grad_R E (align excluded by the stop-gradient), gth double[n] = grad_theta E.
+ */
+static double flock_rho(double r, double Rc, double alpha) { return r < Rc ? pow(1.0 - r / Rc, alpha) / alpha : 0.0; }
+static double flock_drho(double r, double Rc, double alpha) { return r < Rc ? -pow(1.0 - r / Rc, alpha - 1.0) / Rc : 0.0; }
+
+int orc_flock_energy_grad(int n, const double *pos /* n*3, z ignored */, const double *theta, const double *box,
+                          const double *par, double *energies, double *gR, double *gth)
+{
+    if (n <= 0 || !par) return ORC_EINVAL;
+    const double Jal = par[0], Ral = par[1], Jav = par[2], Rav = par[3], Jco = par[4], Rco = par[5], al = par[6];
+    double *G = (double *)calloc((size_t)n * 2, sizeof(double));      /* g_i = d e_i / d D_i */
+    int *cntN = (int *)calloc((size_t)n, sizeof(int));
+    if (!G || !cntN) { free(G); free(cntN); return ORC_ENOMEM; }
+    double Ea = 0.0, Ev = 0.0, Ec = 0.0;
+    for (int i = 0; i < n; ++i) { gR[2 * i] = gR[2 * i + 1] = 0.0; gth[i] = 0.0; }
+    for (int i = 0; i < n; ++i) {
+        const double ci = cos(theta[i]), si = sin(theta[i]);
+        double D[2] = {0.0, 0.0};
+        int m = 0;
+        for (int j = 0; j < n; ++j) {
+            if (j == i) continue;
+            double d[2];
+            d[0] = disp64(pos[3 * (size_t)i], pos[3 * (size_t)j], box[0]);       /* R_i - R_j */
+            d[1] = disp64(pos[3 * (size_t)i + 1], pos[3 * (size_t)j + 1], box[1]);
+            const double r = sqrt(d[0] * d[0] + d[1] * d[1]);
+            /* alignment: theta gradient only */
+            const double cd = ci * cos(theta[j]) + si * sin(theta[j]);            /* N_i.N_j = cos(th_i - th_j) */
+            const double sd = si * cos(theta[j]) - ci * sin(theta[j]);            /* sin(th_i - th_j) */
+            const double ra = flock_rho(r, Ral, al);
+            Ea += 0.5 * Jal * ra * (1.0 - cd) * (1.0 - cd);
+            gth[i] += Jal * ra * 2.0 * (1.0 - cd) * sd;                           /* both ordered pairs: 1/2 * 2 */
+            /* avoidance */
+            Ev += 0.5 * Jav * flock_rho(r, Rav, al);
+            if (r > 0.0) {
+                const double dr = Jav * flock_drho(r, Rav, al);                   /* 1/2 * 2 ordered pairs */
+                gR[2 * i] += dr * d[0] / r; gR[2 * i + 1] += dr * d[1] / r;
+            }
+            if (r < Rco) { D[0] -= d[0]; D[1] -= d[1]; ++m; }                     /* R_j - R_i */
+        }
+        cntN[i] = m;
+        const double Dn = sqrt(D[0] * D[0] + D[1] * D[1]);
+        if (m > 0 && Dn > 0.0) {
+            const double hx = D[0] / Dn, hy = D[1] / Dn, c = hx * ci + hy * si;
+            Ec += 0.5 * Jco * (1.0 - c) * (1.0 - c);
+            /* d e / d D = -J (1 - c) (N - c Dhat) / |D| */
+            G[2 * i] = -Jco * (1.0 - c) * (ci - c * hx) / Dn;
+            G[2 * i + 1] = -Jco * (1.0 - c) * (si - c * hy) / Dn;
+            /* d e / d theta = -J (1 - c) Dhat . dN/dtheta,  dN/dtheta = (-sin, cos) */
+            gth[i] += -Jco * (1.0 - c) * (-hx * si + hy * ci);
+        }
+    }
+    /* grad_{R_k} E_co = -|N_k| g_k + sum_{i : k in N_i} g_i  (the relation r < R_co is symmetric) */
+    for (int k = 0; k < n; ++k) {
+        gR[2 * k] += -cntN[k] * G[2 * k]; gR[2 * k + 1] += -cntN[k] * G[2 * k + 1];
+        for (int i = 0; i < n; ++i) {
+            if (i == k) continue;
+            const double dx = disp64(pos[3 * (size_t)k], pos[3 * (size_t)i], box[0]);
+            const double dy = disp64(pos[3 * (size_t)k + 1], pos[3 * (size_t)i + 1], box[1]);
+            if (sqrt(dx * dx + dy * dy) < Rco) { gR[2 * k] += G[2 * i]; gR[2 * k + 1] += G[2 * i + 1]; }
+        }
+    }
+    if (energies) { energies[0] = Ea; energies[1] = Ev; energies[2] = Ec; }
+    free(G); free(cntN);
+    return ORC_OK;
+}
+
+/*
+ * orc_flock_run: forward Euler (eqs. 4-5): R_i' = mu(R_i, dt (v N(theta_i) - grad_{R_i} E)),
+ * theta_i' = theta_i - dt grad_{theta_i} E, both from the state at the start of the step.
+ */
+int orc_flock_run(int n, double *pos, double *theta, const double *box, const double *par, double speed,
+                  double dt, int nsteps)
+{
+    double *gR = (double *)malloc((size_t)n * 2 * sizeof(double)), *gth = (double *)malloc((size_t)n * sizeof(double));
+    if (!gR || !gth) { free(gR); free(gth); return ORC_ENOMEM; }
+    int rc = ORC_OK;
+    for (int s = 0; s < nsteps && !rc; ++s) {
+        rc = orc_flock_energy_grad(n, pos, theta, box, par, NULL, gR, gth);
+        for (int i = 0; i < n && !rc; ++i) {
+            const double c = cos(theta[i]), sn = sin(theta[i]);
+            pos[3 * (size_t)i] = wrap64(pos[3 * (size_t)i] + dt * (speed * c - gR[2 * i]), box[0]);
+            pos[3 * (size_t)i + 1] = wrap64(pos[3 * (size_t)i + 1] + dt * (speed * sn - gR[2 * i + 1]), box[1]);
+            theta[i] -= dt * gth[i];
+        }
+    }
+    free(gR); free(gth);
+    return rc;
+}

@@ -241,3 +241,20 @@ def nose_hoover_run(pos, vel, diam, box, dim, kind, eps, sigma, r_cut, shift, dt
                                      C.c_double(dt), C.c_double(mass), C.c_double(kT), C.c_double(tau),
                                      _pd(st), nsteps, _pd(cons)), "nose_hoover_run")
     return p, v, f, cons, st
+
+
+def flock_energy_grad(pos, theta, box, par):
+    """par = (J_al, R_al, J_av, R_av, J_co, R_co, alpha). Returns (energies[3], gR[n,2], gtheta[n])."""
+    p = _d(pos3(pos)); th = _d(theta); b = _d(box); pr = _d(par)
+    n = p.shape[0]
+    en = np.zeros(3); gR = np.zeros((n, 2)); gth = np.zeros(n)
+    _check(lib().orc_flock_energy_grad(n, _pd(p), _pd(th), _pd(b), _pd(pr), _pd(en), _pd(gR), _pd(gth)),
+           "flock_energy_grad")
+    return en, gR, gth
+
+
+def flock_run(pos, theta, box, par, speed, dt, nsteps):
+    p = _d(pos3(pos)).copy(); th = _d(theta).copy(); b = _d(box); pr = _d(par)
+    _check(lib().orc_flock_run(p.shape[0], _pd(p), _pd(th), _pd(b), _pd(pr), C.c_double(speed), C.c_double(dt),
+                               nsteps), "flock_run")
+    return p, th

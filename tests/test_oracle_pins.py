@@ -774,3 +774,95 @@ def test_species_lj_reduces_to_lj_and_mixed_pair_closed_form(orc, W):
                    - orc.energy_force(pm, sp, box, 3, SPEC, 0.0, 0.0, 0.0, 1)[2]) / (2 * h)
             worst = max(worst, abs(fd - f[i, q]) / max(1.0, np.abs(f[i]).max()))
     assert worst < 1e-6, worst
+
+
+# ----------------------------------------------------------- flocking --
+
+FLOCK_PAR = (1.0, 3.0, 25.0, 1.5, 0.5, 4.0, 3.0)      # J_al, R_al, J_av, R_av, J_co, R_co, alpha
+
+
+def test_flocking_two_boid_closed_forms(orc):
+    """Eqs. (6)-(10) of PAPER.md App. B on a pair: rho, the alignment, avoidance and cohesion energies
+    and their gradients written out by hand (reading A25 of DESIGN.md)."""
+    Jal, Ral, Jav, Rav, Jco, Rco, al = FLOCK_PAR
+    box = np.array([50.0, 50.0, 1.0])
+    r, t0, t1 = 1.2, 0.3, 1.1
+    pos = np.array([[10.0, 10.0, 0.0], [10.0 + r, 10.0, 0.0]])
+    th = np.array([t0, t1])
+    en, gR, gth = orc.flock_energy_grad(pos, th, box, FLOCK_PAR)
+    rho = lambda x, Rc: (1 - x / Rc) ** al / al if x < Rc else 0.0
+    drho = lambda x, Rc: -(1 - x / Rc) ** (al - 1) / Rc if x < Rc else 0.0
+    c = np.cos(t0 - t1)
+    assert abs(en[0] - Jal * rho(r, Ral) * (1 - c) ** 2) < 1e-14            # one pair, counted once
+    assert abs(en[1] - Jav * rho(r, Rav)) < 1e-14
+    # cohesion: boid 0 sees boid 1 along +x, boid 1 sees boid 0 along -x
+    e0 = 0.5 * Jco * (1 - np.cos(t0)) ** 2
+    e1 = 0.5 * Jco * (1 + np.cos(t1)) ** 2
+    assert abs(en[2] - (e0 + e1)) < 1e-14
+    # avoidance pushes apart: grad_R0 E_avoid = J rho'(r) * (R0 - R1)/r = -J rho' along +x ... boid 0 sits at smaller x
+    ga = Jav * drho(r, Rav) * (-1.0)
+    # cohesion gradient in x vanishes for a pair (D only changes length along the line of centres)
+    assert abs(gR[0, 0] - ga) < 1e-12 and abs(gR[1, 0] + ga) < 1e-12
+    # theta gradients
+    g0 = Jal * rho(r, Ral) * 2 * (1 - c) * np.sin(t0 - t1) + Jco * (1 - np.cos(t0)) * np.sin(t0)
+    assert abs(gth[0] - g0) < 1e-12
+    # beyond every range: nothing
+    pos[1, 0] = 10.0 + 4.5
+    en, gR, gth = orc.flock_energy_grad(pos, th, box, FLOCK_PAR)
+    assert np.abs(en).max() == 0.0 and np.abs(gR).max() == 0.0 and np.abs(gth).max() == 0.0
+
+
+def test_flocking_gradients_and_invariances(orc):
+    """grad_theta E and grad_R (E_avoid + E_cohesion) by central differences (the alignment term has
+    no R gradient: stop-gradient, PAPER.md B.2.2); E is invariant under a rigid rotation of
+    positions and headings and under a translation across the periodic boundary."""
+    rng = np.random.default_rng(1)
+    n, L = 150, 18.0
+    pos = np.zeros((n, 3)); pos[:, :2] = rng.uniform(0, L, (n, 2))
+    th = rng.uniform(-np.pi, np.pi, n)
+    box = np.array([L, L, 1.0])
+    en, gR, gth = orc.flock_energy_grad(pos, th, box, FLOCK_PAR)
+    h, worst = 1e-6, 0.0
+    for i in rng.choice(n, 8, replace=False):
+        tp = th.copy(); tp[i] += h
+        tm = th.copy(); tm[i] -= h
+        fd = (orc.flock_energy_grad(pos, tp, box, FLOCK_PAR)[0].sum() - orc.flock_energy_grad(pos, tm, box, FLOCK_PAR)[0].sum()) / (2 * h)
+        worst = max(worst, abs(fd - gth[i]))
+        for q in range(2):
+            pp = pos.copy(); pp[i, q] += h
+            pm = pos.copy(); pm[i, q] -= h
+            fd = (orc.flock_energy_grad(pp, th, box, FLOCK_PAR)[0][1:].sum()
+                  - orc.flock_energy_grad(pm, th, box, FLOCK_PAR)[0][1:].sum()) / (2 * h)
+            worst = max(worst, abs(fd - gR[i, q]))
+    assert worst < 1e-6, worst
+    shift = np.array([7.3, -4.1, 0.0])
+    p2 = pos + shift; p2[:, :2] -= L * np.floor(p2[:, :2] / L)
+    en2, gR2, gth2 = orc.flock_energy_grad(p2, th, box, FLOCK_PAR)
+    assert np.abs(en2 - en).max() < 1e-10 and np.abs(gR2 - gR).max() < 1e-10
+    # rotation about the centre of a cluster that does not touch the boundary
+    big = np.array([200.0, 200.0, 1.0])
+    c = pos[:, :2] + 90.0
+    phi = 0.7
+    Rm = np.array([[np.cos(phi), -np.sin(phi)], [np.sin(phi), np.cos(phi)]])
+    p3 = np.zeros((n, 3)); p3[:, :2] = (c - 100.0) @ Rm.T + 100.0
+    pc = np.zeros((n, 3)); pc[:, :2] = c
+    e_a = orc.flock_energy_grad(pc, th, big, FLOCK_PAR)[0]
+    e_b = orc.flock_energy_grad(p3, th + phi, big, FLOCK_PAR)[0]
+    assert np.abs(e_a - e_b).max() < 1e-9
+
+
+def test_flocking_forward_euler(orc):
+    """Eqs. (4)-(5): a lone boid swims straight at speed v; two boids within R_al only (avoidance and
+    cohesion switched off) turn toward each other's heading by the alignment gradient."""
+    box = np.array([30.0, 30.0, 1.0])
+    p, th = orc.flock_run(np.array([[5.0, 5.0, 0.0]]), np.array([0.5]), box, FLOCK_PAR, 0.8, 0.1, 10)
+    assert abs(p[0, 0] - (5 + 0.8 * np.cos(0.5))) < 1e-12 and abs(p[0, 1] - (5 + 0.8 * np.sin(0.5))) < 1e-12 and th[0] == 0.5
+    par = (1.0, 3.0, 0.0, 1.5, 0.0, 4.0, 3.0)
+    pos = np.array([[5.0, 5.0, 0.0], [6.0, 5.0, 0.0]])
+    th0 = np.array([0.2, 1.4])
+    p, th = orc.flock_run(pos, th0, box, par, 0.0, 0.05, 1)
+    g = (1 - 1.0 / 3.0) ** 3 / 3 * 2 * (1 - np.cos(-1.2)) * np.sin(-1.2)
+    assert abs(th[0] - (0.2 - 0.05 * g)) < 1e-13 and abs(th[1] - (1.4 + 0.05 * g)) < 1e-13
+    assert np.array_equal(p[:, :2], pos[:, :2])                       # speed 0, no R gradient from alignment
+    p, th = orc.flock_run(pos, th0, box, par, 0.0, 0.05, 200)
+    assert abs(th[0] - th[1]) < abs(th0[0] - th0[1]) * 0.7
