@@ -252,6 +252,29 @@ int md_nose_hoover_step(md_system *sys, const md_potential *pot, void *pos, void
                         int32_t *id, int32_t *nbr_idx, int32_t *nbr_count, float dt, float mass,
                         float kT, float tau, double *nh_state, int nsteps, int32_t *stats, void *stream);
 
+/* Flocking as an energy model (App. B, eqs. 3-10): ranges and strengths of
+ * the alignment, avoidance and cohesion terms, the exponent of the cutoff function rho (eq. 6) and
+ * the swimming speed v of eq. 4. */
+typedef struct md_flock_params {
+    float J_align, R_align;        /* eq. 7 (stop-gradient on the displacement: no position gradient) */
+    float J_avoid, R_avoid;        /* eq. 8 */
+    float J_cohesion, R_cohesion;  /* eqs. 9-10, D_i = sum over r < R_cohesion of (R_j - R_i) */
+    float alpha;                   /* rho(r; Rc) = (1/alpha)(1 - r/Rc)^alpha, alpha >= 1 */
+    float speed;                   /* v */
+} md_flock_params;
+
+/*
+ * nsteps of the boids model by forward Euler (eqs. 4-5) on a 2-D system:
+ *   R_i' = wrap(R_i + dt (v N(theta_i) - grad_{R_i} E));  theta_i' = theta_i - dt grad_{theta_i} E
+ * with E = E_align + E_avoid + E_cohesion over the neighbor list (every range <= the list r_cut), both
+ * updates from the state at the start of the step; then the device-side rebuild test and rebuild.
+ *   pos   float4[n] in/out: (x, y, 0, theta_i) -- the heading travels in pos.w
+ *   lists, id and stats as in md_nve_step (the list must be valid for pos on entry)
+ * CUDA graphs of 8 steps unless use_graph = 0.  fp64 accumulation over the list, fp32 state.
+ */
+int md_flock_step(md_system *sys, const md_flock_params *par, void *pos, int32_t *id, int32_t *nbr_idx,
+                  int32_t *nbr_count, float dt, int nsteps, int32_t *stats, void *stream);
+
 /* FIRE parameters (Bitzek et al. 2006; the paper names "FIRE Descent", L100, and uses it in §4.2). */
 typedef struct md_fire_params {
     float dt_start, dt_max;   /* first step size; cap */

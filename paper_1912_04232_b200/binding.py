@@ -23,6 +23,7 @@ SYMBOLS = [
     "md_needs_rebuild", "md_pair_energy_force", "md_nve_step", "md_nve_run_host", "md_counters",
     "md_nve_run_host_release", "md_fire_minimize", "md_brownian_step",
     "md_langevin_step", "md_nose_hoover_step", "md_set_species_lj",
+    "md_flock_step",
 ]
 
 
@@ -40,6 +41,11 @@ class md_fire_params(C.Structure):
     _fields_ = [("dt_start", C.c_float), ("dt_max", C.c_float), ("n_min", C.c_int),
                 ("f_inc", C.c_float), ("f_dec", C.c_float), ("alpha_start", C.c_float),
                 ("f_alpha", C.c_float)]
+
+
+class md_flock_params(C.Structure):
+    _fields_ = [("J_align", C.c_float), ("R_align", C.c_float), ("J_avoid", C.c_float), ("R_avoid", C.c_float),
+                ("J_cohesion", C.c_float), ("R_cohesion", C.c_float), ("alpha", C.c_float), ("speed", C.c_float)]
 
 
 class MdError(RuntimeError):
@@ -77,6 +83,7 @@ def lib():
                                        C.c_float, C.c_float, C.c_uint32, C.c_uint32, C.c_int, ip, vp]
         L.md_nose_hoover_step.argtypes = [vp, C.POINTER(md_potential), vp, vp, vp, ip, ip, ip, C.c_float,
                                           C.c_float, C.c_float, C.c_float, vp, C.c_int, ip, vp]
+        L.md_flock_step.argtypes = [vp, C.POINTER(md_flock_params), vp, ip, ip, ip, C.c_float, C.c_int, ip, vp]
         L.md_fire_minimize.argtypes = [vp, C.POINTER(md_potential), C.POINTER(md_fire_params), vp, vp, vp,
                                        ip, ip, ip, vp, C.c_int, ip, vp]
         L.md_num_cells.argtypes = [vp, C.POINTER(C.c_int * 3)]
@@ -176,6 +183,11 @@ def md_nose_hoover_step(sys, pot: md_potential, pos, vel, force, id, nbr_idx, nb
     _check(lib().md_nose_hoover_step(sys, C.byref(pot), _ptr(pos), _ptr(vel), _ptr(force), _ptr(id),
                                      _ptr(nbr_idx), _ptr(nbr_count), float(dt), float(mass), float(kT),
                                      float(tau), _ptr(nh_state), int(nsteps), _ptr(stats), _stream(stream)))
+
+
+def md_flock_step(sys, par: md_flock_params, pos, id, nbr_idx, nbr_count, dt, nsteps, stats, stream=None) -> None:
+    _check(lib().md_flock_step(sys, C.byref(par), _ptr(pos), _ptr(id), _ptr(nbr_idx), _ptr(nbr_count), float(dt),
+                               int(nsteps), _ptr(stats), _stream(stream)))
 
 
 def md_fire_minimize(sys, pot: md_potential, par: md_fire_params, pos, vel, force, id, nbr_idx, nbr_count,

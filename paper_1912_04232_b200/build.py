@@ -12,7 +12,7 @@ DEPS = SRC + [os.path.join(HERE, "csrc", "md_kernels.cuh"),
               os.path.join(HERE, "csrc", "md_nbr2.cuh"),
               os.path.join(HERE, "csrc", "md_fire.cuh"),
               os.path.join(HERE, "csrc", "md_brownian.cuh"),
-              os.path.join(HERE, "csrc", "md_nh.cuh"), os.path.join(ROOT, "include", "md.h")]
+              os.path.join(HERE, "csrc", "md_nh.cuh"), os.path.join(HERE, "csrc", "md_flock.cuh"), os.path.join(ROOT, "include", "md.h")]
 LIB = os.environ.get("MD_B200_LIB") or os.path.join(HERE, "libmd_b200.so")   # override: a variant build
 
 NVCC_FLAGS = [

@@ -8,6 +8,7 @@
 #include "md_fire.cuh"
 #include "md_brownian.cuh"
 #include "md_nh.cuh"
+#include "md_flock.cuh"
 
 #include <cmath>
 #include <cstdarg>
@@ -52,7 +53,7 @@ size_t up(size_t x) { return (x + ALIGN - 1) / ALIGN * ALIGN; }
 bool aligned16(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 15u) == 0; }
 int blocks_for(long long threads, int block = 256) { return (int)((threads + block - 1) / block); }
 
-enum { RULE_FIRE = 1, RULE_BROWNIAN, RULE_LANGEVIN, RULE_NH };
+enum { RULE_FIRE = 1, RULE_BROWNIAN, RULE_LANGEVIN, RULE_NH, RULE_FLOCK };
 
 // Everything one step of an update rule other than NVE depends on (plain data, compared bytewise
 // to decide whether the cached graphs still apply).
@@ -64,6 +65,7 @@ struct RuleArgs {
     float dt, mass, gamma, kT, tau;
     unsigned seed, step0;
     md_fire_params fire;
+    md_flock_params flock;
     int fast32, builder, nb_parts, remap;
     float est_thr;
 };
@@ -583,10 +585,21 @@ int record_rule_step(md_system *s, const Pair &pp, const RuleArgs &A, cudaStream
         force_vel = v4; force_a = a;
         break;
     }
+    case RULE_FLOCK: {
+        // forward Euler uses the gradients of the CURRENT state: two passes over the list, then the
+        // update (which raises the rebuild), the rebuild for the next step, the bookkeeping
+        const FlockPar fq = {A.flock.J_align, A.flock.R_align, A.flock.J_avoid, A.flock.R_avoid,
+                             A.flock.J_cohesion, A.flock.R_cohesion, A.flock.alpha, A.flock.speed};
+        const int nbp = blocks_for(g.n, 128);
+        k_flock_pass1<<<nbp, 128, 0, st>>>(g, fq, p4, A.nbr_idx, A.nbr_count, s->vel_s, s->pos_alt);
+        k_flock_pass2<<<nbp, 128, 0, st>>>(g, fq, p4, A.nbr_idx, A.nbr_count, s->vel_s, s->pos_alt);
+        k_flock_update<<<nb, 256, 0, st>>>(g, fq, p4, s->vel_s, s->ref_pos, A.dt, rs);
+        break;
+    }
     default: return fail(MD_EINVAL, "unknown update rule %d", A.rule);
     }
     LAUNCH_OK();
-    float4 *sort_vel = A.rule == RULE_BROWNIAN ? nullptr : v4;
+    float4 *sort_vel = (A.rule == RULE_BROWNIAN || A.rule == RULE_FLOCK) ? nullptr : v4;
     int rc;
     if (in_graph) {
         rc = record_rebuild_if(s, st, rs.cond, p4, sort_vel, A.id, A.nbr_idx, A.nbr_count);
@@ -599,6 +612,11 @@ int record_rule_step(md_system *s, const Pair &pp, const RuleArgs &A, cudaStream
         if (rc) return rc;
     }
     Book book = {flag, status, A.stats};
+    if (A.rule == RULE_FLOCK) {
+        k_flock_book<<<1, 1, 0, st>>>(book);
+        LAUNCH_OK();
+        return MD_OK;
+    }
     rc = launch_force(s, pp, p4, A.nbr_idx, A.nbr_count, f4, force_vel, force_a, nullptr, false, book, st);
     if (rc) return rc;
     if (A.rule == RULE_FIRE) {
@@ -988,6 +1006,26 @@ int md_nose_hoover_step(md_system *sys, const md_potential *pot, void *pos, void
     memset(&A, 0, sizeof(A));
     A.rule = RULE_NH; A.pos = pos; A.vel = vel; A.force = force; A.state = nh_state; A.id = id; A.nbr_idx = nbr_idx;
     A.nbr_count = nbr_count; A.stats = stats; A.pot = *pot; A.dt = dt; A.mass = mass; A.kT = kT; A.tau = tau;
+    return run_rule(sys, pp, A, nsteps, (cudaStream_t)stream);
+}
+
+int md_flock_step(md_system *sys, const md_flock_params *par, void *pos, int32_t *id, int32_t *nbr_idx,
+                  int32_t *nbr_count, float dt, int nsteps, int32_t *stats, void *stream) {
+    if (!sys || !par || !pos || !nbr_idx || !nbr_count || !stats) return fail(MD_EINVAL, "NULL argument");
+    if (!aligned16(pos)) return fail(MD_EINVAL, "pos must be 16-byte aligned");
+    if (sys->g.dim != 2) return fail(MD_EINVAL, "flocking is 2-D (dim = %d)", sys->g.dim);
+    if (!(dt > 0.0f) || nsteps < 0 || !(par->alpha >= 1.0f) || !(par->R_align > 0.0f) || !(par->R_avoid > 0.0f) ||
+        !(par->R_cohesion > 0.0f) || !(par->J_align >= 0.0f) || !(par->J_avoid >= 0.0f) || !(par->J_cohesion >= 0.0f))
+        return fail(MD_EINVAL, "flocking parameters out of range");
+    const float rmax = std::max(par->R_align, std::max(par->R_avoid, par->R_cohesion));
+    if (rmax > sys->cfg.r_cut) return fail(MD_EINVAL, "interaction range %g exceeds the list r_cut %g", rmax, sys->cfg.r_cut);
+    if (int rc = enter(sys)) return rc;
+    Pair pp;
+    memset(&pp, 0, sizeof(pp));
+    RuleArgs A;
+    memset(&A, 0, sizeof(A));
+    A.rule = RULE_FLOCK; A.pos = pos; A.id = id; A.nbr_idx = nbr_idx; A.nbr_count = nbr_count; A.stats = stats;
+    A.dt = dt; A.mass = 1.0f; A.flock = *par;
     return run_rule(sys, pp, A, nsteps, (cudaStream_t)stream);
 }
 

@@ -1,0 +1,123 @@
+// md_flock.cuh -- flocking as an energy model on the same cell / neighbor list (
+// PAPER.md App. B: eqs. 3-10 and the forward-Euler dynamics of eqs. 4-5; what the text
+// leaves open is DESIGN.md reading A25).  2-D; the heading theta_i travels in pos.w, so a neighbor's
+// heading arrives with its position in one gather and follows the re-sort.
+//   rho(r; Rc) = (1/alpha)(1 - r/Rc)^alpha, r < Rc
+//   E_align = 1/2 sum_{i!=j} J_al rho(r; R_al)(1 - N_i.N_j)^2   (stop-gradient: no R gradient)
+//   E_avoid = 1/2 sum_{i!=j} J_av rho(r; R_av)
+//   E_coh   = sum_i 1/2 J_co (1 - Dhat_i.N_i)^2,  D_i = sum_{j: r < R_co} (R_j - R_i)
+//   R_i' = mu(R_i, dt (v N_i - grad_{R_i} E)),  theta_i' = theta_i - dt grad_{theta_i} E
+// grad_{R_k} E_coh = -|N_k| g_k + sum_{i: r_ki < R_co} g_i with g_i = dE_coh,i/dD_i, hence two passes
+// over the list (g first, then its gather) before the update.  fp64 accumulation, fp32 state.
+#pragma once
+#include "md_kernels.cuh"
+
+namespace mdk {
+
+struct FlockPar { double Jal, Ral, Jav, Rav, Jco, Rco, alpha, speed; };
+
+__device__ __forceinline__ void flock_disp(const Geom &g, const float4 &pi, const float4 &q, double &dx, double &dy) {
+    dx = (double)pi.x - (double)q.x; dy = (double)pi.y - (double)q.y;
+    const double hx = 0.5 * (double)g.L[0], hy = 0.5 * (double)g.L[1];
+    dx -= dx > hx ? (double)g.L[0] : (dx < -hx ? -(double)g.L[0] : 0.0);
+    dy -= dy > hy ? (double)g.L[1] : (dy < -hy ? -(double)g.L[1] : 0.0);
+}
+
+// pass 1: acc[i] = (grad_R without the gathered cohesion part, grad_theta, |N_i|), gco[i] = g_i
+__global__ void __launch_bounds__(128)
+k_flock_pass1(Geom g, FlockPar fp, const float4 *__restrict__ pos, const int *__restrict__ nbr_idx,
+              const int *__restrict__ nbr_count, float4 *__restrict__ acc, float4 *__restrict__ gco) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= g.n) return;
+    const float4 pi = pos[i];
+    const int cnt = min(nbr_count[i], g.capacity);
+    const int *col = nbr_idx + nbr_tile_base(i, g.capacity) + (i & 31);
+    double si, ci;
+    sincos((double)pi.w, &si, &ci);
+    double gx = 0.0, gy = 0.0, gt = 0.0, Dx = 0.0, Dy = 0.0;
+    int m = 0;
+    for (int k = 0; k < cnt; ++k) {
+        const float4 q = pos[col[k * TILE]];
+        double dx, dy;
+        flock_disp(g, pi, q, dx, dy);
+        const double r = sqrt(dx * dx + dy * dy);
+        if (r < fp.Ral) {
+            double sd, cd;
+            sincos((double)pi.w - (double)q.w, &sd, &cd);
+            const double ra = pow(1.0 - r / fp.Ral, fp.alpha) / fp.alpha;
+            gt += fp.Jal * ra * 2.0 * (1.0 - cd) * sd;
+        }
+        if (r < fp.Rav && r > 0.0) {
+            const double dr = -fp.Jav * pow(1.0 - r / fp.Rav, fp.alpha - 1.0) / fp.Rav;
+            gx += dr * dx / r; gy += dr * dy / r;
+        }
+        if (r < fp.Rco) { Dx -= dx; Dy -= dy; ++m; }
+    }
+    double Gx = 0.0, Gy = 0.0;
+    const double Dn = sqrt(Dx * Dx + Dy * Dy);
+    if (m > 0 && Dn > 0.0) {
+        const double hx = Dx / Dn, hy = Dy / Dn, c = hx * ci + hy * si;
+        Gx = -fp.Jco * (1.0 - c) * (ci - c * hx) / Dn;
+        Gy = -fp.Jco * (1.0 - c) * (si - c * hy) / Dn;
+        gt += -fp.Jco * (1.0 - c) * (-hx * si + hy * ci);
+        gx -= m * Gx; gy -= m * Gy;
+    }
+    acc[i] = make_float4((float)gx, (float)gy, (float)gt, (float)m);
+    gco[i] = make_float4((float)Gx, (float)Gy, 0.0f, 0.0f);
+}
+
+// pass 2: acc[i].xy += sum over the neighbors within R_co of their g
+__global__ void __launch_bounds__(128)
+k_flock_pass2(Geom g, FlockPar fp, const float4 *__restrict__ pos, const int *__restrict__ nbr_idx,
+              const int *__restrict__ nbr_count, float4 *__restrict__ acc, const float4 *__restrict__ gco) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= g.n) return;
+    const float4 pi = pos[i];
+    const int cnt = min(nbr_count[i], g.capacity);
+    const int *col = nbr_idx + nbr_tile_base(i, g.capacity) + (i & 31);
+    double gx = 0.0, gy = 0.0;
+    for (int k = 0; k < cnt; ++k) {
+        const int j = col[k * TILE];
+        double dx, dy;
+        flock_disp(g, pi, pos[j], dx, dy);
+        if (sqrt(dx * dx + dy * dy) < fp.Rco) { const float4 G = gco[j]; gx += (double)G.x; gy += (double)G.y; }
+    }
+    float4 a = acc[i];
+    a.x = (float)((double)a.x + gx); a.y = (float)((double)a.y + gy);
+    acc[i] = a;
+}
+
+// forward Euler (eqs. 4-5), half-skin test
+__global__ void __launch_bounds__(256)
+k_flock_update(Geom g, FlockPar fp, float4 *__restrict__ pos, const float4 *__restrict__ acc,
+               const float4 *__restrict__ ref, float dt, Raise rs) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    bool moved = false;
+    if (i < g.n) {
+        float4 p = pos[i];
+        const float4 a = acc[i];
+        float sn, cs;
+        sincosf(p.w, &sn, &cs);
+        const float v = (float)fp.speed;
+        p.x = wrap(fmaf(dt, fmaf(v, cs, -a.x), p.x), g.L[0], g.inv_L[0]);
+        p.y = wrap(fmaf(dt, fmaf(v, sn, -a.y), p.y), g.L[1], g.inv_L[1]);
+        p.w = fmaf(-dt, a.z, p.w);
+        pos[i] = p;
+        moved = disp2_from_ref<2>(g, p, ref[i]) > g.half_skin2;
+    }
+    if (__any_sync(FULL, moved) && (threadIdx.x & 31) == 0) raise_rebuild(rs);
+}
+
+// step bookkeeping (what the force kernel does for the other rules)
+__global__ void k_flock_book(Book book) {
+    if (ld_volatile(book.flag)) {
+        book.stats[1] += 1;
+        const int mc = ld_volatile(book.status + 1);
+        if (mc > book.stats[3]) book.stats[3] = mc;
+        if (ld_volatile(book.status) && book.stats[2] < 0) book.stats[2] = book.stats[0];
+        *book.flag = 0;
+    }
+    book.stats[0] += 1;
+}
+
+} // namespace mdk
