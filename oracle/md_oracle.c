@@ -26,6 +26,7 @@
  *   orc_langevin_run    L100 "Langevin" (BAOAB splitting)
  *   orc_nose_hoover_run L100 "Nose-Hoover [67]" (one thermostat, MTK splitting)
  *   orc_normals         the counter-based normal generator both sides implement
+ *   orc_flock_*         App. B: boids energies eqs. 3-10, forward Euler eqs. 4-5
  * Readings of everything the paper leaves open (strict <, half-skin, truncated
  * and shifted LJ, wrap convention, rounding of the inclusion predicate) are
  * SURVEY.md §8c A1-A18, restated in DESIGN.md §3.
@@ -38,7 +39,8 @@
  * values and gradients of every potential, FIRE's schedule in closed form and its
  * reduction to velocity Verlet, generator moments, free diffusion, exact friction
  * decay and stationary variance, Nose-Hoover's conserved quantity at second order
- * and its decoupled limit.  The one unpinned thing is a chaotic
+ * and its decoupled limit, the boids energies on a pair by hand with finite-difference
+ * gradients and rotation / translation invariance.  The one unpinned thing is a chaotic
  * trajectory beyond ~100 steps ("parity unpinned" by design).
  *
  * Arithmetic: fp64 everywhere, except the canonical inclusion predicate
