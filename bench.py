@@ -325,7 +325,8 @@ def main():
     if e2e is not None:
         out["e2e"] = e2e
     if not args.no_cpu_baseline:
-        sample_steps = {0: 100, 1: 200, 2: 50, 3: 20, 4: 5}[args.config]
+        # about 5-10 s of wall time on 16 host cores (80-160 core-seconds) per config
+        sample_steps = {0: 10000, 1: 5000, 2: 1500, 3: 150, 4: 30}[args.config]
         t, cores = oracle_sample(w, sample_steps)
         out["cpu_baseline"] = {"value": w.n * sample_steps / t, "unit": UNIT, "cores": cores,
                                "kind": "oracle",
