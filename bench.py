@@ -142,13 +142,14 @@ def oracle_sample(w, md_steps):
 
 def run_reference(args):
     """This tier's reference arm: the oracle as it stands, timed on the host cores; each
-    bench step is a bounded sample (2 MD steps) of the same workload."""
+    bench step is a bounded sample of the same workload (about 1 s of wall time: the initial
+    list build, then MD steps with the half-skin rebuilds they trigger)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
     from paper_1912_04232_b200 import workloads as W
     w = W.config(args.config)
-    sample = 2
+    sample = {0: 2000, 1: 500, 2: 200, 3: 20, 4: 5}[args.config]
     for _ in range(min(args.warmup, 1)):
         oracle_sample(w, 1)
     times = []
@@ -158,7 +159,7 @@ def run_reference(args):
         times.append(t)
     total = sum(times)
     value = w.n * sample * args.steps / total
-    desc = f"{sample} MD steps of config {args.config} (N={w.n}) per bench step incl. one list build"
+    desc = f"{sample} MD steps of config {args.config} (N={w.n}) per bench step incl. the initial list build and half-skin rebuilds"
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus,
         "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total / args.steps,
