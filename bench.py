@@ -54,6 +54,8 @@ def parse():
     ap.add_argument("--md-steps", type=int, default=100, help="MD steps per bench step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--next-rows", action="store_true",
+                    help="time the SURVEY 8(f) rows instead (one JSON line per row; not the contract line)")
     ap.add_argument("--breakdown", action="store_true", help="(kept for compatibility: the build time per rebuild is always reported)")
     return ap.parse_args()
 
@@ -171,10 +173,118 @@ def run_reference(args):
     }))
 
 
+def run_next_rows(args):
+    """SURVEY 8(f) rows on the headline geometry (config 3's particles and box unless stated):
+    the pair force per launch (L2 flushed before each) for the other potentials, and us per step
+    of the other update rules through their graph-captured loops (rebuilds amortised)."""
+    import dataclasses
+    import torch
+    from paper_1912_04232_b200 import binding as B
+    from paper_1912_04232_b200 import workloads as W
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(dev)
+    base = W.config(args.config)
+    n = base.n
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+
+    def emit(row, what, us, **kw):
+        print(json.dumps({"row": row, "what": what, "n": kw.pop("n", n), "us": us, **kw}), flush=True)
+
+    def time_force(S, reps=10):
+        S.build(); S.compute_force()
+        ts = []
+        for _ in range(reps):
+            flush.fill_(1)
+            a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            a.record(); S.compute_force(want_energy=False); b.record()
+            torch.cuda.synchronize()
+            ts.append(a.elapsed_time(b) * 1e3)
+        return statistics.median(ts)
+
+    def time_rule(call, nsteps):
+        call(nsteps)                                    # warm-up: graph capture, first rebuilds
+        torch.cuda.synchronize()
+        flush.fill_(1)
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(); call(nsteps); b.record()
+        torch.cuda.synchronize()
+        return a.elapsed_time(b) * 1e3 / nsteps
+
+    # f2: potentials on the fp64 pair chain (LJ first, for scale: fp32 fast path, then fp64 chain)
+    S = B.System(base)
+    emit("f2", "LJ force, fp32 fast path with fp64 re-evaluation (the headline kernel)", time_force(S))
+    B.md_set_option(S.sys, "fast32", 0)
+    emit("f2", "LJ force, fp64 pair chain", time_force(S))
+    S.close()
+    w = dataclasses.replace(base, kind=W.KIND_MORSE, epsilon=1.0, sigma=1.12, alpha=5.0)
+    S = B.System(w); emit("f2", "Morse force (D=1, alpha=5, r0=1.12), fp64 pair chain", time_force(S)); S.close()
+    w = dataclasses.replace(base, kind=W.KIND_BUCKINGHAM, epsilon=float(np.float32(9.02e5)),
+                            sigma=float(np.float32(3.454)), alpha=12.5)
+    S = B.System(w); emit("f2", "Buckingham exp-6 force, fp64 pair chain", time_force(S)); S.close()
+    pos = base.pos.copy()
+    pos[:, 3] = (np.arange(n) % 5 == 0).astype(np.float32)
+    w = dataclasses.replace(base, kind=W.KIND_LJ_SPECIES, pos=pos)
+    S = B.System(w)
+    eps = np.array([[1.0, 1.5], [1.5, 0.5]], np.float32)
+    sig = np.array([[1.0, 0.8], [0.8, 0.88]], np.float32)
+    B.md_set_species_lj(S.sys, eps, sig, (2.5 * sig).astype(np.float32))
+    emit("f2", "species x species LJ force (80:20 binary mixture), fp64 pair chain", time_force(S)); S.close()
+
+    # f3: update rules, LJ fast path, 200 steps each
+    steps = 200
+    S = B.System(base); S.build(); S.compute_force()
+    emit("f3", "NVE (fused graph; for scale)", time_rule(lambda k: S.step(k), steps), steps=steps); S.close()
+    S = B.System(base); S.build(); S.compute_force()
+    emit("f3", "Brownian dynamics kT=0.8 gamma=1", time_rule(lambda k: B.md_brownian_step(
+        S.sys, S.pot, S.pos, S.force, S.id, S.nbr_idx, S.nbr_count, 1e-4, 1.0, 0.8, 7, 0, k, S.stats), steps),
+        steps=steps); S.close()
+    S = B.System(base); S.build(); S.compute_force()
+    emit("f3", "Langevin (BAOAB) kT=1 gamma=1", time_rule(lambda k: B.md_langevin_step(
+        S.sys, S.pot, S.pos, S.vel, S.force, S.id, S.nbr_idx, S.nbr_count, base.dt, base.mass, 1.0, 1.0, 7, 0, k,
+        S.stats), steps), steps=steps); S.close()
+    S = B.System(base); S.build(); S.compute_force()
+    nh = torch.zeros(2, dtype=torch.float64, device=dev)
+    emit("f3", "Nose-Hoover kT=1 tau=0.2", time_rule(lambda k: B.md_nose_hoover_step(
+        S.sys, S.pot, S.pos, S.vel, S.force, S.id, S.nbr_idx, S.nbr_count, base.dt, base.mass, 1.0, 0.2, nh, k,
+        S.stats), steps), steps=steps); S.close()
+    w = dataclasses.replace(base, vel=np.zeros_like(base.vel))
+    S = B.System(w); S.build(); S.compute_force()
+    fs = torch.zeros(4, dtype=torch.float32, device=dev)
+    fp = B.md_fire_params(0.002, 0.02, 5, 1.1, 0.5, 0.1, 0.99)
+    emit("f3", "FIRE minimisation", time_rule(lambda k: B.md_fire_minimize(
+        S.sys, S.pot, fp, S.pos, S.vel, S.force, S.id, S.nbr_idx, S.nbr_count, fs, k, S.stats), steps),
+        steps=steps); S.close()
+
+    # f4: flocking, 2-D, 262,144 boids on a jittered square lattice, spacing 1.26 (~24 neighbors in R + skin)
+    m = 512
+    nb = m * m
+    L = np.float32(m * 1.26 + 0.37)
+    rng = np.random.default_rng(5)
+    g = (np.arange(m) + 0.5) * (float(L) / m)
+    box = np.array([L, L, 1.0], np.float32)
+    p = np.zeros((nb, 4), np.float32)
+    p[:, :2] = W.into_box_f32(np.stack(np.meshgrid(g, g, indexing="ij"), -1).reshape(-1, 2)
+                              + rng.normal(0, 0.15, (nb, 2)), box)
+    p[:, 3] = rng.uniform(-np.pi, np.pi, nb).astype(np.float32)
+    w = dataclasses.replace(base, name="flock2d", n=nb, dim=2, box=box, pos=p, vel=np.zeros((nb, 4), np.float32),
+                            kind=W.KIND_SOFT, r_cut=3.0, skin=0.5, capacity=64)
+    S = B.System(w); S.build()
+    par = B.md_flock_params(1.0, 3.0, 10.0, 1.0, 0.5, 3.0, 3.0, 0.5)
+    us = time_rule(lambda k: B.md_flock_step(S.sys, par, S.pos, S.id, S.nbr_idx, S.nbr_count, 0.01, k, S.stats), steps)
+    emit("f4", "flocking (align + avoid + cohesion), forward Euler", us, steps=steps, n=nb,
+         rebuilds=int(S.stats[1]), mean_neighbors=float(S.nbr_count.float().mean()))
+    S.close()
+
+
 def main():
     args = parse()
     if args.impl == "reference":
         return run_reference(args)
+    if args.next_rows:
+        return run_next_rows(args)
 
     import torch
     import torch.distributed as dist

@@ -591,7 +591,17 @@ int record_rule_step(md_system *s, const Pair &pp, const RuleArgs &A, cudaStream
         const FlockPar fq = {A.flock.J_align, A.flock.R_align, A.flock.J_avoid, A.flock.R_avoid,
                              A.flock.J_cohesion, A.flock.R_cohesion, A.flock.alpha, A.flock.speed};
         const int nbp = blocks_for(g.n, 128);
-        k_flock_pass1<<<nbp, 128, 0, st>>>(g, fq, p4, A.nbr_idx, A.nbr_count, s->vel_s, s->pos_alt);
+        double2 *cs = reinterpret_cast<double2 *>(s->pos_s);       // free between rebuilds
+        k_flock_trig<<<nb, 256, 0, st>>>(g.n, p4, cs);
+        const int ai = (int)A.flock.alpha;
+#define FLOCK_PASS1(AI) k_flock_pass1<AI><<<nbp, 128, 0, st>>>(g, fq, p4, cs, A.nbr_idx, A.nbr_count, s->vel_s, s->pos_alt)
+        if ((float)ai != A.flock.alpha) FLOCK_PASS1(0);
+        else if (ai == 1) FLOCK_PASS1(1);
+        else if (ai == 2) FLOCK_PASS1(2);
+        else if (ai == 3) FLOCK_PASS1(3);
+        else if (ai == 4) FLOCK_PASS1(4);
+        else FLOCK_PASS1(0);
+#undef FLOCK_PASS1
         k_flock_pass2<<<nbp, 128, 0, st>>>(g, fq, p4, A.nbr_idx, A.nbr_count, s->vel_s, s->pos_alt);
         k_flock_update<<<nb, 256, 0, st>>>(g, fq, p4, s->vel_s, s->ref_pos, A.dt, rs);
         break;

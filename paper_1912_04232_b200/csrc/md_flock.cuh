@@ -14,6 +14,8 @@
 
 namespace mdk {
 
+constexpr int FLOCK_U = 4;
+
 struct FlockPar { double Jal, Ral, Jav, Rav, Jco, Rco, alpha, speed; };
 
 __device__ __forceinline__ void flock_disp(const Geom &g, const float4 &pi, const float4 &q, double &dx, double &dy) {
@@ -23,35 +25,73 @@ __device__ __forceinline__ void flock_disp(const Geom &g, const float4 &pi, cons
     dy -= dy > hy ? (double)g.L[1] : (dy < -hy ? -(double)g.L[1] : 0.0);
 }
 
+// x^a for x in (0, 1].  AI > 0: a = AI is a small integer known at compile time (the usual alpha = 3)
+// and the power is AI - 1 multiplications; AI = 0: any real a by pow.  NEG1: the exponent is a - 1.
+template <int AI, bool NEG1>
+__device__ __forceinline__ double flock_pow(double x, double a) {
+    if (AI == 0) return pow(x, NEG1 ? a - 1.0 : a);
+    constexpr int n = NEG1 ? AI - 1 : AI;
+    double y = 1.0;
+#pragma unroll
+    for (int k = 0; k < n; ++k) y *= x;
+    return y;
+}
+
+// (cos theta_i, sin theta_i) in fp64, once per boid and step: pass 1 forms the sine and cosine of
+// theta_i - theta_j from these by the angle-difference identities instead of one fp64 sincos per pair.
+__global__ void __launch_bounds__(256)
+k_flock_trig(int n, const float4 *__restrict__ pos, double2 *__restrict__ cs) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    double si, ci;
+    sincos((double)pos[i].w, &si, &ci);
+    cs[i] = make_double2(ci, si);
+}
+
 // pass 1: acc[i] = (grad_R without the gathered cohesion part, grad_theta, |N_i|), gco[i] = g_i
+template <int AI>
 __global__ void __launch_bounds__(128)
-k_flock_pass1(Geom g, FlockPar fp, const float4 *__restrict__ pos, const int *__restrict__ nbr_idx,
-              const int *__restrict__ nbr_count, float4 *__restrict__ acc, float4 *__restrict__ gco) {
+k_flock_pass1(Geom g, FlockPar fp, const float4 *__restrict__ pos, const double2 *__restrict__ cs,
+              const int *__restrict__ nbr_idx, const int *__restrict__ nbr_count,
+              float4 *__restrict__ acc, float4 *__restrict__ gco) {
     const int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= g.n) return;
     const float4 pi = pos[i];
     const int cnt = min(nbr_count[i], g.capacity);
     const int *col = nbr_idx + nbr_tile_base(i, g.capacity) + (i & 31);
-    double si, ci;
-    sincos((double)pi.w, &si, &ci);
+    const double2 ti = cs[i];
+    const double ci = ti.x, si = ti.y;
+    const double iRal = 1.0 / fp.Ral, iRav = 1.0 / fp.Rav;
+    const double cal = 2.0 * fp.Jal / fp.alpha, cav = -fp.Jav * iRav;
     double gx = 0.0, gy = 0.0, gt = 0.0, Dx = 0.0, Dy = 0.0;
     int m = 0;
-    for (int k = 0; k < cnt; ++k) {
-        const float4 q = pos[col[k * TILE]];
-        double dx, dy;
-        flock_disp(g, pi, q, dx, dy);
-        const double r = sqrt(dx * dx + dy * dy);
-        if (r < fp.Ral) {
-            double sd, cd;
-            sincos((double)pi.w - (double)q.w, &sd, &cd);
-            const double ra = pow(1.0 - r / fp.Ral, fp.alpha) / fp.alpha;
-            gt += fp.Jal * ra * 2.0 * (1.0 - cd) * sd;
+    for (int k = 0; k < cnt; k += FLOCK_U) {            // FLOCK_U independent gathers in flight
+        int j[FLOCK_U]; float4 q[FLOCK_U]; double2 tj[FLOCK_U];
+#pragma unroll
+        for (int u = 0; u < FLOCK_U; ++u) j[u] = k + u < cnt ? col[(k + u) * TILE] : i;
+#pragma unroll
+        for (int u = 0; u < FLOCK_U; ++u) { q[u] = pos[j[u]]; tj[u] = cs[j[u]]; }
+#pragma unroll
+        for (int u = 0; u < FLOCK_U; ++u) {
+            double dx, dy;
+            flock_disp(g, pi, q[u], dx, dy);
+            // r and 1/r: fp32 rsqrt refined by one Newton step in fp64 (relative error ~1e-13)
+            // instead of an fp64 square root and an fp64 division per pair
+            const double r2 = dx * dx + dy * dy;
+            double ir = (double)rsqrtf((float)r2);
+            ir = r2 > 0.0 ? ir * (1.5 - 0.5 * r2 * ir * ir) : 0.0;
+            const double r = r2 * ir;
+            const bool valid = k + u < cnt;
+            if (valid && r < fp.Ral) {
+                const double sd = si * tj[u].x - ci * tj[u].y, cd = ci * tj[u].x + si * tj[u].y;
+                gt += cal * flock_pow<AI, false>(1.0 - r * iRal, fp.alpha) * (1.0 - cd) * sd;
+            }
+            if (valid && r < fp.Rav && r > 0.0) {
+                const double dr = cav * flock_pow<AI, true>(1.0 - r * iRav, fp.alpha) * ir;
+                gx += dr * dx; gy += dr * dy;
+            }
+            if (valid && r < fp.Rco) { Dx -= dx; Dy -= dy; ++m; }
         }
-        if (r < fp.Rav && r > 0.0) {
-            const double dr = -fp.Jav * pow(1.0 - r / fp.Rav, fp.alpha - 1.0) / fp.Rav;
-            gx += dr * dx / r; gy += dr * dy / r;
-        }
-        if (r < fp.Rco) { Dx -= dx; Dy -= dy; ++m; }
     }
     double Gx = 0.0, Gy = 0.0;
     const double Dn = sqrt(Dx * Dx + Dy * Dy);
@@ -75,12 +115,20 @@ k_flock_pass2(Geom g, FlockPar fp, const float4 *__restrict__ pos, const int *__
     const float4 pi = pos[i];
     const int cnt = min(nbr_count[i], g.capacity);
     const int *col = nbr_idx + nbr_tile_base(i, g.capacity) + (i & 31);
+    const double Rco2 = fp.Rco * fp.Rco;
     double gx = 0.0, gy = 0.0;
-    for (int k = 0; k < cnt; ++k) {
-        const int j = col[k * TILE];
-        double dx, dy;
-        flock_disp(g, pi, pos[j], dx, dy);
-        if (sqrt(dx * dx + dy * dy) < fp.Rco) { const float4 G = gco[j]; gx += (double)G.x; gy += (double)G.y; }
+    for (int k = 0; k < cnt; k += FLOCK_U) {
+        int j[FLOCK_U]; float4 q[FLOCK_U], G[FLOCK_U];
+#pragma unroll
+        for (int u = 0; u < FLOCK_U; ++u) j[u] = k + u < cnt ? col[(k + u) * TILE] : i;
+#pragma unroll
+        for (int u = 0; u < FLOCK_U; ++u) { q[u] = pos[j[u]]; G[u] = gco[j[u]]; }
+#pragma unroll
+        for (int u = 0; u < FLOCK_U; ++u) {
+            double dx, dy;
+            flock_disp(g, pi, q[u], dx, dy);
+            if (k + u < cnt && dx * dx + dy * dy < Rco2) { gx += (double)G[u].x; gy += (double)G[u].y; }
+        }
     }
     float4 a = acc[i];
     a.x = (float)((double)a.x + gx); a.y = (float)((double)a.y + gy);

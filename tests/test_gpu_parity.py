@@ -527,21 +527,22 @@ def test_flocking_against_the_oracle(B, orc, W):
     w = custom_workload(W, pos, box32, 2, 1, 4.0, 0.5, 128)
     th0 = pos[:, 3].astype(np.float64)
 
-    # (a)
-    par = (1.0, 3.0, 10.0, 1.5, 0.5, 4.0, 3.0)
-    S = B.System(w)
-    S.build()
-    B.md_flock_step(S.sys, B.md_flock_params(*par, speed), S.pos, S.id, S.nbr_idx, S.nbr_count, dt, 1, S.stats)
-    torch.cuda.synchronize()
-    en, gR, gth = orc.flock_energy_grad(pos, th0, box32, par)
-    one = unpermute(S, S.pos)
-    d = one[:, :2].astype(np.float64) - pos[:, :2]
-    d -= L * np.round(d / L)
-    want = dt * (speed * np.stack([np.cos(th0), np.sin(th0)], 1) - gR)
-    scale = max(1.0, np.abs(want).max())
-    assert np.abs(d - want).max() <= 4e-6 * scale                      # fp32 positions at L = 40
-    assert np.abs((one[:, 3].astype(np.float64) - th0) + dt * gth).max() <= 1e-6 * max(1.0, np.abs(gth).max())
-    S.close()
+    # (a) alpha = 3, 2 (compile-time integer powers) and 2.5 (pow)
+    for alpha in (3.0, 2.0, 2.5):
+        par = (1.0, 3.0, 10.0, 1.5, 0.5, 4.0, alpha)
+        S = B.System(w)
+        S.build()
+        B.md_flock_step(S.sys, B.md_flock_params(*par, speed), S.pos, S.id, S.nbr_idx, S.nbr_count, dt, 1, S.stats)
+        torch.cuda.synchronize()
+        en, gR, gth = orc.flock_energy_grad(pos, th0, box32, par)
+        one = unpermute(S, S.pos)
+        d = one[:, :2].astype(np.float64) - pos[:, :2]
+        d -= L * np.round(d / L)
+        want = dt * (speed * np.stack([np.cos(th0), np.sin(th0)], 1) - gR)
+        scale = max(1.0, np.abs(want).max())
+        assert np.abs(d - want).max() <= 4e-6 * scale                  # fp32 positions at L = 40
+        assert np.abs((one[:, 3].astype(np.float64) - th0) + dt * gth).max() <= 1e-6 * max(1.0, np.abs(gth).max())
+        S.close()
 
     # (b)
     par = (1.0, 3.0, 10.0, 1.5, 0.0, 4.0, 3.0)
