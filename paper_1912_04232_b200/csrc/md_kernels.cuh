@@ -665,14 +665,22 @@ __device__ __forceinline__ void soft_pair64(const Pair &pp, double dx, double dy
 
 // One pair, Morse [75] (L104): u = D (1 - x)^2 - D, x = exp(-alpha (r - r0)); the force
 // coefficient -u'(r)/r = -2 D alpha x (1 - x) / r; D is applied once per particle.
+// 1/sqrt(x), x > 0 of ordinary magnitude: the fp32 reciprocal square root refined by one Newton
+// step in fp64 (relative error ~1e-13), in place of an fp64 square root and an fp64 division.
+__device__ __forceinline__ double rsqrt64(double x) {
+    const double y = (double)rsqrtf((float)x);
+    return y * fma(-0.5 * x, y * y, 1.5);
+}
+
 template <bool ENERGY>
 __device__ __forceinline__ void morse_pair64(const Pair &pp, double dx, double dy, double dz,
                                              bool valid, Acc64 &a) {
     const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
     const bool in = valid && r2 < pp.drc2;
-    const double r = sqrt(in ? r2 : 1.0);
+    const double r2v = in ? r2 : 1.0, r2s = r2v > 0.0 ? r2v : 1.0;
+    const double ir = rsqrt64(r2s), r = r2v * ir;                   // r = 0 for coincident particles
     const double x = exp(-pp.dalpha * (r - pp.dr0));
-    double c = (in && r > 0.0) ? -2.0 * pp.dalpha * x * (1.0 - x) / r : 0.0;
+    double c = (in && r2 > 0.0) ? -2.0 * pp.dalpha * x * (1.0 - x) * ir : 0.0;
     a.fx = fma(c, dx, a.fx); a.fy = fma(c, dy, a.fy); a.fz = fma(c, dz, a.fz);
     if (ENERGY) a.e += in ? (1.0 - x) * (1.0 - x) - 1.0 - pp.du_cutm : 0.0;
 }
