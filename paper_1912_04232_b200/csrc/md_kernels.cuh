@@ -702,21 +702,34 @@ __device__ __forceinline__ void buck_pair64(const Pair &pp, double dx, double dy
 
 // One pair, species x species LJ (L104; the sigma matrix of L298-L305): as lj_pair64 with the
 // constants of the pair's species; nothing is factored out (fs = es = 1).
+// The species tables as one block of shared memory (a per-pair index into kernel parameters is a
+// divergent constant load, replayed once per distinct species pair in the warp):
+// sp[0..15] = 2 sigma^6, [16..31] = 24 eps sigma^6, [32..47] = 2 eps, [48..63] = rc^2, [64..79] = shift term.
+constexpr int SP_TAB = 80;
+__device__ __forceinline__ void species_tables_to_shared(const Pair &pp, double *sp) {
+    for (int t = threadIdx.x; t < 16; t += blockDim.x) {
+        sp[t] = pp.sp_sig6x2[t]; sp[16 + t] = pp.sp_fs[t]; sp[32 + t] = pp.sp_es[t];
+        sp[48 + t] = pp.sp_rc2[t]; sp[64 + t] = pp.sp_ucut4[t];
+    }
+    __syncthreads();
+}
+
 template <bool ENERGY>
-__device__ __forceinline__ void ljs_pair64(const Pair &pp, double dx, double dy, double dz, float wi,
-                                           float wj, bool valid, Acc64 &a) {
+__device__ __forceinline__ void ljs_pair64(const Pair &pp, const double *sp, double dx, double dy, double dz,
+                                           float wi, float wj, bool valid, Acc64 &a) {
     const int sa = min(max((int)wi, 0), pp.ns - 1), sb = min(max((int)wj, 0), pp.ns - 1);
     const int t = sa * pp.ns + sb;
+    const double sig6x2 = sp[t];
     const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
-    const bool in = valid && r2 < pp.sp_rc2[t];
+    const bool in = valid && r2 < sp[48 + t];
     const double y = rcp64(in ? r2 : 1.0);
     const double y2 = y * y, y3 = y2 * y;
-    const double tt = fma(pp.sp_sig6x2[t], y3, -1.0);
-    const double c = in ? pp.sp_fs[t] * (y2 * y2) * tt : 0.0;
+    const double tt = fma(sig6x2, y3, -1.0);
+    const double c = in ? sp[16 + t] * (y2 * y2) * tt : 0.0;
     a.fx = fma(c, dx, a.fx); a.fy = fma(c, dy, a.fy); a.fz = fma(c, dz, a.fz);
     if (ENERGY) {
-        const double s6 = 0.5 * pp.sp_sig6x2[t] * y3;
-        a.e += in ? pp.sp_es[t] * (fma(s6, s6, -s6) - pp.sp_ucut4[t]) : 0.0;
+        const double s6 = 0.5 * sig6x2 * y3;
+        a.e += in ? sp[32 + t] * (fma(s6, s6, -s6) - sp[64 + t]) : 0.0;
     }
 }
 
@@ -753,13 +766,13 @@ __device__ __forceinline__ void displacement(const Me<DIM> &me, const float4 &q,
 
 template <int KIND, int DIM, bool ENERGY, bool WRAP>
 __device__ __forceinline__ void pair_any(const Pair &pp, const Me<DIM> &me, const float4 &q,
-                                         bool valid, Acc64 &acc) {
+                                         bool valid, Acc64 &acc, const double *sp = nullptr) {
     double dx, dy, dz;
     displacement<DIM, WRAP>(me, q, dx, dy, dz);
     if (KIND == 0) lj_pair64<ENERGY>(pp, dx, dy, dz, valid, acc);
     else if (KIND == 2) morse_pair64<ENERGY>(pp, dx, dy, dz, valid, acc);
     else if (KIND == 3) buck_pair64<ENERGY>(pp, dx, dy, dz, valid, acc);
-    else if (KIND == 4) ljs_pair64<ENERGY>(pp, dx, dy, dz, me.pi.w, q.w, valid, acc);
+    else if (KIND == 4) ljs_pair64<ENERGY>(pp, sp, dx, dy, dz, me.pi.w, q.w, valid, acc);
     else soft_pair64<ENERGY>(pp, dx, dy, dz, (double)me.pi.w + (double)q.w, valid, acc);
 }
 
@@ -833,6 +846,8 @@ __global__ void __launch_bounds__(128)
 k_force(Geom g, Pair pp, const float4 *__restrict__ pos, const int *__restrict__ nbr_idx,
         const int *__restrict__ nbr_count, float4 *__restrict__ force, float4 *__restrict__ vel,
         float a, double *energy_total, Book book) {
+    __shared__ double sp[KIND == 4 ? SP_TAB : 1];
+    if (KIND == 4) species_tables_to_shared(pp, sp);
     const int gid = blockIdx.x * blockDim.x + threadIdx.x;
     const int i = gid / TPP, sub = gid % TPP;
     const bool active = i < g.n;
@@ -851,10 +866,10 @@ k_force(Geom g, Pair pp, const float4 *__restrict__ pos, const int *__restrict__
         for (int u = 0; u < U; ++u) q[u] = pos[j[u]];
         if (!wrap_path) {
 #pragma unroll
-            for (int u = 0; u < U; ++u) pair_any<KIND, DIM, ENERGY, false>(pp, me, q[u], k + u * TPP < cnt, acc);
+            for (int u = 0; u < U; ++u) pair_any<KIND, DIM, ENERGY, false>(pp, me, q[u], k + u * TPP < cnt, acc, sp);
         } else {
 #pragma unroll
-            for (int u = 0; u < U; ++u) pair_any<KIND, DIM, ENERGY, true>(pp, me, q[u], k + u * TPP < cnt, acc);
+            for (int u = 0; u < U; ++u) pair_any<KIND, DIM, ENERGY, true>(pp, me, q[u], k + u * TPP < cnt, acc, sp);
         }
     }
 #pragma unroll
@@ -902,6 +917,8 @@ k_force_stream(Geom g, Pair pp, const float4 *__restrict__ pos, const int *__res
                float4 *__restrict__ vel, float a, double *energy_total, Book book) {
     __shared__ __align__(128) int s_idx[FS_WARPS][FS_STAGES][FS_ROWS * TILE];
     __shared__ __align__(8) unsigned long long s_bar[FS_WARPS][FS_STAGES];
+    __shared__ double sp[KIND == 4 ? SP_TAB : 1];
+    if (KIND == 4) species_tables_to_shared(pp, sp);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int gid = blockIdx.x * blockDim.x + threadIdx.x;
     const int i = gid;
@@ -945,10 +962,10 @@ k_force_stream(Geom g, Pair pp, const float4 *__restrict__ pos, const int *__res
             for (int u = 0; u < U; ++u) q[u] = pos[j[u]];
             if (!wrap_path) {
 #pragma unroll
-                for (int u = 0; u < U; ++u) pair_any<KIND, DIM, ENERGY, false>(pp, me, q[u], k0 + r + u < cnt, acc);
+                for (int u = 0; u < U; ++u) pair_any<KIND, DIM, ENERGY, false>(pp, me, q[u], k0 + r + u < cnt, acc, sp);
             } else {
 #pragma unroll
-                for (int u = 0; u < U; ++u) pair_any<KIND, DIM, ENERGY, true>(pp, me, q[u], k0 + r + u < cnt, acc);
+                for (int u = 0; u < U; ++u) pair_any<KIND, DIM, ENERGY, true>(pp, me, q[u], k0 + r + u < cnt, acc, sp);
             }
         }
         __syncwarp();                                  // every lane is done reading this stage
