@@ -60,14 +60,16 @@ __device__ __forceinline__ void lj_pair32(const Pair32 &pp, float dx, float dy, 
     bool in = r2 < pp.rc2;
     if (CHECK) in = in && valid;
     a.near = fminf(a.near, fabsf(r2 - pp.rc2));
-    const float y = rcp32(CHECK ? (in ? r2 : 1.0f) : r2);   // unchecked rows hold true neighbors: r2 > 0
+    // pairs outside the cutoff (and padded slots) take 1/r2 = 1/inf = 0: every power and the
+    // coefficient vanish with it, no later select
+    const float y = rcp32(in ? r2 : __int_as_float(0x7f800000));
     const float y2 = y * y;
     const float y3 = y2 * y;
     const float t = fmaf(pp.sig6x2, y3, -1.0f);          // 2 s6 - 1
-    const float y4 = in ? y2 * y2 : 0.0f;
+    const float y4 = y2 * y2;
     const float c = y4 * t;
     a.fx = fmaf(c, dx, a.fx); a.fy = fmaf(c, dy, a.fy); a.fz = fmaf(c, dz, a.fz);
-    a.s += fmaxf(fabsf(c), 0.2f * y4);                   // |coefficient|, floored near its zero (see above)
+    a.s = fmaf(y4, fmaxf(fabsf(t), 0.2f), a.s);          // |coefficient|, floored near its zero (see above)
     if (ENERGY) {
         const float s6 = 0.5f * pp.sig6x2 * y3;
         a.e += in ? fmaf(s6, s6, -s6) - pp.ucut4 : 0.0f;
