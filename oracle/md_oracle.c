@@ -26,7 +26,8 @@
  *   orc_langevin_run    L100 "Langevin" (BAOAB splitting)
  *   orc_nose_hoover_run L100 "Nose-Hoover [67]" (one thermostat, MTK splitting)
  *   orc_normals         the counter-based normal generator both sides implement
- *   orc_flock_*         App. B: boids energies eqs. 3-10, forward Euler eqs. 4-5
+ *   orc_flock_*         App. B: boids energies eqs. 3-10, forward Euler eqs. 4-5;
+ *                       obstacles eq. 11 (L411-L418)
  * Readings of everything the paper leaves open (strict <, half-skin, truncated
  * and shifted LJ, wrap convention, rounding of the inclusion predicate) are
  * SURVEY.md §8c A1-A18, restated in DESIGN.md §3.
@@ -992,6 +993,59 @@ int orc_flock_energy_grad(int n, const double *pos /* n*3, z ignored */, const d
 }
 
 /*
+ * Obstacles (App. B.3.1, eq. 11): disks o with centre C_o and radius D_o;
+ *   e_io = J_ob rho(r_io; D_o) (1 + N_i . Rhat_io)^2,  R_io = C_o - R_i (nearest image), r_io = |R_io|
+ * -- zero unless the boid is inside the disk, smallest when it heads straight away from the centre
+ * (reading A26: the range of rho is the disk's own radius; R_io points from the boid to
+ * the obstacle, the sign convention of eqs. 9-10; gradients in R and theta both act).
+ *   d e / d theta = 2 J rho (1 + c) (-sin th u_x + cos th u_y),      u = R_io / r, c = N . u
+ *   grad_{R_i} e  = -J [ rho'(r) (1 + c)^2 u + 2 rho (1 + c) (N - c u) / r ]
+ * orc_flock_obstacle_energy_grad ADDS to gR / gth and returns the energy in *energy.
+ */
+int orc_flock_obstacle_energy_grad(int n, const double *pos, const double *theta, const double *box, int nobs,
+                                   const double *centre /* nobs*2 */, const double *radius, double J,
+                                   double alpha, double *energy, double *gR, double *gth)
+{
+    if (n <= 0 || nobs < 0) return ORC_EINVAL;
+    double E = 0.0;
+    for (int i = 0; i < n; ++i) {
+        const double ci = cos(theta[i]), si = sin(theta[i]);
+        for (int o = 0; o < nobs; ++o) {
+            const double dx = disp64(centre[2 * o], pos[3 * (size_t)i], box[0]);          /* C_o - R_i */
+            const double dy = disp64(centre[2 * o + 1], pos[3 * (size_t)i + 1], box[1]);
+            const double r = sqrt(dx * dx + dy * dy);
+            if (!(r < radius[o]) || !(r > 0.0)) continue;
+            const double ux = dx / r, uy = dy / r, c = ci * ux + si * uy;
+            const double rho = flock_rho(r, radius[o], alpha), drho = flock_drho(r, radius[o], alpha);
+            E += J * rho * (1.0 + c) * (1.0 + c);
+            if (gth) gth[i] += 2.0 * J * rho * (1.0 + c) * (-si * ux + ci * uy);
+            if (gR) {
+                gR[2 * i] += -J * (drho * (1.0 + c) * (1.0 + c) * ux + 2.0 * rho * (1.0 + c) * (ci - c * ux) / r);
+                gR[2 * i + 1] += -J * (drho * (1.0 + c) * (1.0 + c) * uy + 2.0 * rho * (1.0 + c) * (si - c * uy) / r);
+            }
+        }
+    }
+    if (energy) *energy = E;
+    return ORC_OK;
+}
+
+/* obstacles seen by orc_flock_run (none by default) */
+#define ORC_MAX_OBSTACLES 16
+static int g_nobs = 0;
+static double g_obs_centre[2 * ORC_MAX_OBSTACLES], g_obs_radius[ORC_MAX_OBSTACLES], g_obs_J = 0.0;
+
+int orc_flock_set_obstacles(int nobs, const double *centre, const double *radius, double J)
+{
+    if (nobs < 0 || nobs > ORC_MAX_OBSTACLES) return ORC_EINVAL;
+    g_nobs = nobs; g_obs_J = J;
+    for (int o = 0; o < nobs; ++o) {
+        g_obs_centre[2 * o] = centre[2 * o]; g_obs_centre[2 * o + 1] = centre[2 * o + 1];
+        g_obs_radius[o] = radius[o];
+    }
+    return ORC_OK;
+}
+
+/*
  * orc_flock_run: forward Euler (eqs. 4-5): R_i' = mu(R_i, dt (v N(theta_i) - grad_{R_i} E)),
  * theta_i' = theta_i - dt grad_{theta_i} E, both from the state at the start of the step.
  */
@@ -1003,6 +1057,9 @@ int orc_flock_run(int n, double *pos, double *theta, const double *box, const do
     int rc = ORC_OK;
     for (int s = 0; s < nsteps && !rc; ++s) {
         rc = orc_flock_energy_grad(n, pos, theta, box, par, NULL, gR, gth);
+        if (!rc && g_nobs > 0)
+            rc = orc_flock_obstacle_energy_grad(n, pos, theta, box, g_nobs, g_obs_centre, g_obs_radius, g_obs_J,
+                                                par[6], NULL, gR, gth);
         for (int i = 0; i < n && !rc; ++i) {
             const double c = cos(theta[i]), sn = sin(theta[i]);
             pos[3 * (size_t)i] = wrap64(pos[3 * (size_t)i] + dt * (speed * c - gR[2 * i]), box[0]);

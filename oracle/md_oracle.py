@@ -253,6 +253,24 @@ def flock_energy_grad(pos, theta, box, par):
     return en, gR, gth
 
 
+def flock_obstacle_energy_grad(pos, theta, box, centre, radius, J, alpha):
+    """Eq. 11 alone: returns (energy, gR[n,2], gtheta[n]) of the obstacle term."""
+    p = _d(pos3(pos)); th = _d(theta); b = _d(box)
+    c = _d(np.asarray(centre, np.float64).reshape(-1, 2)); r = _d(radius)
+    n = p.shape[0]
+    en = np.zeros(1); gR = np.zeros((n, 2)); gth = np.zeros(n)
+    _check(lib().orc_flock_obstacle_energy_grad(n, _pd(p), _pd(th), _pd(b), int(c.shape[0]), _pd(c), _pd(r),
+                                                C.c_double(J), C.c_double(alpha), _pd(en), _pd(gR), _pd(gth)),
+           "flock_obstacle_energy_grad")
+    return float(en[0]), gR, gth
+
+
+def flock_set_obstacles(centre=(), radius=(), J=0.0):
+    """Obstacles seen by flock_run from now on (none: call without arguments)."""
+    c = _d(np.asarray(centre, np.float64).reshape(-1, 2)); r = _d(np.asarray(radius, np.float64).reshape(-1))
+    _check(lib().orc_flock_set_obstacles(int(c.shape[0]), _pd(c), _pd(r), C.c_double(J)), "flock_set_obstacles")
+
+
 def flock_run(pos, theta, box, par, speed, dt, nsteps):
     p = _d(pos3(pos)).copy(); th = _d(theta).copy(); b = _d(box); pr = _d(par)
     _check(lib().orc_flock_run(p.shape[0], _pd(p), _pd(th), _pd(b), _pd(pr), C.c_double(speed), C.c_double(dt),

@@ -866,3 +866,61 @@ def test_flocking_forward_euler(orc):
     assert np.array_equal(p[:, :2], pos[:, :2])                       # speed 0, no R gradient from alignment
     p, th = orc.flock_run(pos, th0, box, par, 0.0, 0.05, 200)
     assert abs(th[0] - th[1]) < abs(th0[0] - th0[1]) * 0.7
+
+
+def test_flocking_obstacles(orc):
+    """Eq. (11) (A26).  Closed forms for one boid and one disk: heading
+    straight at the centre e = 4 J rho, straight away e = 0 with zero gradients, sideways e = J rho;
+    nothing outside the disk; gradients by central differences; the disk acts across the periodic
+    boundary; a boid inside a disk and heading away from it is left alone by the Euler step while one
+    heading at it is turned and pushed out."""
+    box = np.array([20.0, 20.0, 1.0])
+    J, D, al = 2.0, 3.0, 3.0
+    cen = np.array([[10.0, 10.0]])
+    rho = lambda r: (1 - r / D) ** al / al
+    at = lambda x, y: np.array([[x, y, 0.0]])
+    # boid at distance 1.2 to the left of the centre: R_io = (+1.2, 0), u = (1, 0)
+    e, gR, gth = orc.flock_obstacle_energy_grad(at(8.8, 10.0), [0.0], box, cen, [D], J, al)     # heading at it
+    assert abs(e - 4 * J * rho(1.2)) < 1e-14 and abs(gth[0]) < 1e-14
+    e, gR, gth = orc.flock_obstacle_energy_grad(at(8.8, 10.0), [np.pi], box, cen, [D], J, al)   # heading away
+    assert abs(e) < 1e-28 and np.abs(gR).max() < 1e-13 and abs(gth[0]) < 1e-13
+    e, gR, gth = orc.flock_obstacle_energy_grad(at(8.8, 10.0), [np.pi / 2], box, cen, [D], J, al)
+    assert abs(e - J * rho(1.2)) < 1e-14
+    assert abs(gth[0] - 2 * J * rho(1.2) * (-1.0)) < 1e-13              # d/dtheta (1 + cos theta)^2 at pi/2
+    e, gR, gth = orc.flock_obstacle_energy_grad(at(6.9, 10.0), [0.0], box, cen, [D], J, al)     # r = 3.1 > D
+    assert e == 0.0 and not gR.any() and not gth.any()
+    # across the boundary: disk at x = 0.5, boid at x = 19.5 (distance 1)
+    e, _, _ = orc.flock_obstacle_energy_grad(at(19.5, 4.0), [0.0], box, [[0.5, 4.0]], [D], J, al)
+    assert abs(e - 4 * J * rho(1.0)) < 1e-13
+    # central differences, several boids and disks
+    rng = np.random.default_rng(3)
+    n = 40
+    pos = np.zeros((n, 3)); pos[:, :2] = rng.uniform(0, 20, (n, 2))
+    th = rng.uniform(-np.pi, np.pi, n)
+    cens = rng.uniform(0, 20, (5, 2)); rad = rng.uniform(2.0, 5.0, 5)
+    e0, gR, gth = orc.flock_obstacle_energy_grad(pos, th, box, cens, rad, J, 2.5)
+    assert e0 > 0
+    E = lambda p, t: orc.flock_obstacle_energy_grad(p, t, box, cens, rad, J, 2.5)[0]
+    h, worst = 1e-6, 0.0
+    for i in range(n):
+        tp = th.copy(); tp[i] += h; tm = th.copy(); tm[i] -= h
+        worst = max(worst, abs((E(pos, tp) - E(pos, tm)) / (2 * h) - gth[i]))
+        for q in range(2):
+            pp = pos.copy(); pp[i, q] += h; pm = pos.copy(); pm[i, q] -= h
+            worst = max(worst, abs((E(pp, th) - E(pm, th)) / (2 * h) - gR[i, q]))
+    assert worst < 2e-7, worst
+    # forward Euler with the obstacle switched on, all boid-boid terms off
+    par0 = (0.0, 3.0, 0.0, 1.5, 0.0, 4.0, al)
+    orc.flock_set_obstacles(cen, [D], J)
+    try:
+        p, t = orc.flock_run(at(8.8, 10.0), [np.pi], box, par0, 0.5, 0.1, 5)
+        assert abs(p[0, 0] - (8.8 - 0.25)) < 1e-12 and abs(t[0] - np.pi) < 1e-12     # swims away undisturbed
+        p, t = orc.flock_run(at(8.8, 10.2), [0.1], box, par0, 0.0, 0.05, 40)
+        r0 = np.hypot(1.2, 0.2); r1 = np.hypot(10.0 - p[0, 0], 10.0 - p[0, 1])
+        assert r1 > r0                                                               # pushed outward
+        u = np.array([10.0 - p[0, 0], 10.0 - p[0, 1]]) / r1
+        assert np.cos(t[0]) * u[0] + np.sin(t[0]) * u[1] < np.cos(0.1) * 1.2 / r0 + np.sin(0.1) * (-0.2) / r0   # turned away
+    finally:
+        orc.flock_set_obstacles()
+    p, t = orc.flock_run(at(8.8, 10.0), [0.0], box, par0, 0.5, 0.1, 1)               # obstacles cleared
+    assert abs(p[0, 0] - 8.85) < 1e-12
