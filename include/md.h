@@ -264,9 +264,21 @@ typedef struct md_flock_params {
 } md_flock_params;
 
 /*
+ * Disk obstacles of the boids model (App. B.3.1, eq. 11; reading A26):
+ *   e_io = J rho(r_io; D_o) (1 + N_i . Rhat_io)^2,  R_io = C_o - R_i (nearest image)
+ * added to E in md_flock_step from the next call on (gradients in R_i and theta_i).
+ *   nobs    0..MD_MAX_OBSTACLES (0 removes them)
+ *   centre  HOST float[nobs*2], inside the box;  radius  HOST float[nobs], 0 < D_o < L/2;  J >= 0
+ * The values are copied into the context; MD_EINVAL otherwise.
+ */
+#define MD_MAX_OBSTACLES 16
+int md_flock_obstacles(md_system *sys, int nobs, const float *centre, const float *radius, float J);
+
+/*
  * nsteps of the boids model by forward Euler (eqs. 4-5) on a 2-D system:
  *   R_i' = wrap(R_i + dt (v N(theta_i) - grad_{R_i} E));  theta_i' = theta_i - dt grad_{theta_i} E
- * with E = E_align + E_avoid + E_cohesion over the neighbor list (every range <= the list r_cut), both
+ * with E = E_align + E_avoid + E_cohesion over the neighbor list (every range <= the list r_cut) plus the
+ * obstacle term of md_flock_obstacles, both
  * updates from the state at the start of the step; then the device-side rebuild test and rebuild.
  *   pos   float4[n] in/out: (x, y, 0, theta_i) -- the heading travels in pos.w
  *   lists, id and stats as in md_nve_step (the list must be valid for pos on entry)

@@ -23,7 +23,7 @@ SYMBOLS = [
     "md_needs_rebuild", "md_pair_energy_force", "md_nve_step", "md_nve_run_host", "md_counters",
     "md_nve_run_host_release", "md_fire_minimize", "md_brownian_step",
     "md_langevin_step", "md_nose_hoover_step", "md_set_species_lj",
-    "md_flock_step",
+    "md_flock_step", "md_flock_obstacles",
 ]
 
 
@@ -83,6 +83,7 @@ def lib():
                                        C.c_float, C.c_float, C.c_uint32, C.c_uint32, C.c_int, ip, vp]
         L.md_nose_hoover_step.argtypes = [vp, C.POINTER(md_potential), vp, vp, vp, ip, ip, ip, C.c_float,
                                           C.c_float, C.c_float, C.c_float, vp, C.c_int, ip, vp]
+        L.md_flock_obstacles.argtypes = [vp, C.c_int, C.POINTER(C.c_float), C.POINTER(C.c_float), C.c_float]
         L.md_flock_step.argtypes = [vp, C.POINTER(md_flock_params), vp, ip, ip, ip, C.c_float, C.c_int, ip, vp]
         L.md_fire_minimize.argtypes = [vp, C.POINTER(md_potential), C.POINTER(md_fire_params), vp, vp, vp,
                                        ip, ip, ip, vp, C.c_int, ip, vp]
@@ -183,6 +184,16 @@ def md_nose_hoover_step(sys, pot: md_potential, pos, vel, force, id, nbr_idx, nb
     _check(lib().md_nose_hoover_step(sys, C.byref(pot), _ptr(pos), _ptr(vel), _ptr(force), _ptr(id),
                                      _ptr(nbr_idx), _ptr(nbr_count), float(dt), float(mass), float(kT),
                                      float(tau), _ptr(nh_state), int(nsteps), _ptr(stats), _stream(stream)))
+
+
+def md_flock_obstacles(sys, centre=(), radius=(), J=0.0) -> None:
+    import numpy as np
+    c = np.ascontiguousarray(np.asarray(centre, np.float32).reshape(-1, 2))
+    r = np.ascontiguousarray(np.asarray(radius, np.float32).reshape(-1))
+    if c.shape[0] != r.shape[0]:
+        raise ValueError("one radius per centre")
+    fp = C.POINTER(C.c_float)
+    _check(lib().md_flock_obstacles(sys, int(r.shape[0]), c.ctypes.data_as(fp), r.ctypes.data_as(fp), float(J)))
 
 
 def md_flock_step(sys, par: md_flock_params, pos, id, nbr_idx, nbr_count, dt, nsteps, stats, stream=None) -> None:

@@ -66,6 +66,8 @@ struct RuleArgs {
     unsigned seed, step0;
     md_fire_params fire;
     md_flock_params flock;
+    int nobs;                       // md_flock_obstacles: disks (x, y, radius) and J
+    float obs[3 * MD_MAX_OBSTACLES], J_obs;
     int fast32, builder, nb_parts, remap;
     float est_thr;
 };
@@ -104,6 +106,8 @@ struct md_system {
     int nb_parts;        // builder: warps per tile (0 = by system size, 1, 2, 4)
     int ns;              // md_set_species_lj: number of species and the tables (row-major)
     float sp_eps[16], sp_sig[16], sp_rc[16];
+    int nobs;            // md_flock_obstacles
+    float obs[3 * MD_MAX_OBSTACLES], J_obs;
     int builder;         // neighbor-list builder: 2 = bit-mask (md_nbr2.cuh), 1 = column append
     int fast32;          // LJ 3-D: fp32 fast path + fp64 re-evaluation (md_force32.cuh)
     float est_thr;       // its error-estimate threshold
@@ -588,8 +592,10 @@ int record_rule_step(md_system *s, const Pair &pp, const RuleArgs &A, cudaStream
     case RULE_FLOCK: {
         // forward Euler uses the gradients of the CURRENT state: two passes over the list, then the
         // update (which raises the rebuild), the rebuild for the next step, the bookkeeping
-        const FlockPar fq = {A.flock.J_align, A.flock.R_align, A.flock.J_avoid, A.flock.R_avoid,
-                             A.flock.J_cohesion, A.flock.R_cohesion, A.flock.alpha, A.flock.speed};
+        FlockPar fq = {A.flock.J_align, A.flock.R_align, A.flock.J_avoid, A.flock.R_avoid,
+                       A.flock.J_cohesion, A.flock.R_cohesion, A.flock.alpha, A.flock.speed};
+        fq.nobs = A.nobs; fq.Job = A.J_obs;
+        for (int o = 0; o < A.nobs; ++o) { fq.ox[o] = A.obs[3 * o]; fq.oy[o] = A.obs[3 * o + 1]; fq.oD[o] = A.obs[3 * o + 2]; }
         const int nbp = blocks_for(g.n, 128);
         double2 *cs = reinterpret_cast<double2 *>(s->pos_s);       // free between rebuilds
         k_flock_trig<<<nb, 256, 0, st>>>(g.n, p4, cs);
@@ -1019,6 +1025,25 @@ int md_nose_hoover_step(md_system *sys, const md_potential *pot, void *pos, void
     return run_rule(sys, pp, A, nsteps, (cudaStream_t)stream);
 }
 
+int md_flock_obstacles(md_system *sys, int nobs, const float *centre, const float *radius, float J) {
+    if (!sys) return fail(MD_EINVAL, "NULL argument");
+    if (nobs < 0 || nobs > MD_MAX_OBSTACLES) return fail(MD_EINVAL, "nobs = %d must be in 0..%d", nobs, MD_MAX_OBSTACLES);
+    if (nobs > 0 && (!centre || !radius)) return fail(MD_EINVAL, "NULL argument");
+    if (!(J >= 0.0f)) return fail(MD_EINVAL, "J_obstacle must be >= 0");
+    for (int o = 0; o < nobs; ++o) {
+        if (!(radius[o] > 0.0f) || !(2.0f * radius[o] < std::min(sys->g.L[0], sys->g.L[1])))
+            return fail(MD_EINVAL, "obstacle %d: radius %g must be positive and below half the box", o, radius[o]);
+        if (!(centre[2 * o] >= 0.0f && centre[2 * o] < sys->g.L[0] && centre[2 * o + 1] >= 0.0f && centre[2 * o + 1] < sys->g.L[1]))
+            return fail(MD_EINVAL, "obstacle %d: centre outside the box", o);
+    }
+    sys->nobs = nobs; sys->J_obs = J;
+    memset(sys->obs, 0, sizeof(sys->obs));
+    for (int o = 0; o < nobs; ++o) {
+        sys->obs[3 * o] = centre[2 * o]; sys->obs[3 * o + 1] = centre[2 * o + 1]; sys->obs[3 * o + 2] = radius[o];
+    }
+    return MD_OK;
+}
+
 int md_flock_step(md_system *sys, const md_flock_params *par, void *pos, int32_t *id, int32_t *nbr_idx,
                   int32_t *nbr_count, float dt, int nsteps, int32_t *stats, void *stream) {
     if (!sys || !par || !pos || !nbr_idx || !nbr_count || !stats) return fail(MD_EINVAL, "NULL argument");
@@ -1036,6 +1061,8 @@ int md_flock_step(md_system *sys, const md_flock_params *par, void *pos, int32_t
     memset(&A, 0, sizeof(A));
     A.rule = RULE_FLOCK; A.pos = pos; A.id = id; A.nbr_idx = nbr_idx; A.nbr_count = nbr_count; A.stats = stats;
     A.dt = dt; A.mass = 1.0f; A.flock = *par;
+    A.nobs = sys->nobs; A.J_obs = sys->J_obs;
+    memcpy(A.obs, sys->obs, sizeof(float) * 3 * (size_t)sys->nobs);
     return run_rule(sys, pp, A, nsteps, (cudaStream_t)stream);
 }
 

@@ -16,7 +16,12 @@ namespace mdk {
 
 constexpr int FLOCK_U = 4;
 
-struct FlockPar { double Jal, Ral, Jav, Rav, Jco, Rco, alpha, speed; };
+struct FlockPar {
+    double Jal, Ral, Jav, Rav, Jco, Rco, alpha, speed;
+    int nobs;                                   // obstacles (App. B.3.1): centres, radii, J
+    double Job;
+    float ox[MD_MAX_OBSTACLES], oy[MD_MAX_OBSTACLES], oD[MD_MAX_OBSTACLES];
+};
 
 __device__ __forceinline__ void flock_disp(const Geom &g, const float4 &pi, const float4 &q, double &dx, double &dy) {
     dx = (double)pi.x - (double)q.x; dy = (double)pi.y - (double)q.y;
@@ -101,6 +106,20 @@ k_flock_pass1(Geom g, FlockPar fp, const float4 *__restrict__ pos, const double2
         Gy = -fp.Jco * (1.0 - c) * (si - c * hy) / Dn;
         gt += -fp.Jco * (1.0 - c) * (-hx * si + hy * ci);
         gx -= m * Gx; gy -= m * Gy;
+    }
+    // obstacles, eq. 11: e = J rho(r; D_o)(1 + N.u)^2, u = (C_o - R_i)/r, inside the disk only
+    for (int o = 0; o < fp.nobs; ++o) {
+        double dx, dy;
+        flock_disp(g, pi, make_float4(fp.ox[o], fp.oy[o], 0.0f, 0.0f), dx, dy);      // R_i - C_o
+        const double r = sqrt(dx * dx + dy * dy), D = (double)fp.oD[o];
+        if (r < D && r > 0.0) {
+            const double ux = -dx / r, uy = -dy / r, c = ci * ux + si * uy, x = 1.0 - r / D;
+            const double rho = flock_pow<AI, false>(x, fp.alpha) / fp.alpha;
+            const double drho = -flock_pow<AI, true>(x, fp.alpha) / D;
+            gt += 2.0 * fp.Job * rho * (1.0 + c) * (-si * ux + ci * uy);
+            gx += -fp.Job * (drho * (1.0 + c) * (1.0 + c) * ux + 2.0 * rho * (1.0 + c) * (ci - c * ux) / r);
+            gy += -fp.Job * (drho * (1.0 + c) * (1.0 + c) * uy + 2.0 * rho * (1.0 + c) * (si - c * uy) / r);
+        }
     }
     acc[i] = make_float4((float)gx, (float)gy, (float)gt, (float)m);
     gco[i] = make_float4((float)Gx, (float)Gy, 0.0f, 0.0f);

@@ -586,6 +586,52 @@ def test_flocking_against_the_oracle(B, orc, W):
     assert np.abs(got[:, 3].astype(np.float64) - th_o).max() <= 1e-4
     S.close()
 
+    # (d) disk obstacles (App. B.3.1, eq. 11): the obstacle term alone after one step, then 60 steps of
+    #     alignment + avoidance + obstacles; one disk straddles the periodic boundary
+    cen_o = np.array([[10.2, 11.7], [0.9, 30.1], [25.3, 20.4], [33.0, 5.5]], np.float32)
+    rad_o = np.array([4.0, 3.0, 5.5, 2.5], np.float32)
+    Jo = 4.0
+    par0 = (0.0, 3.0, 0.0, 1.5, 0.0, 4.0, 3.0)
+    S = B.System(w)
+    B.md_flock_obstacles(S.sys, cen_o, rad_o, Jo)
+    S.build()
+    B.md_flock_step(S.sys, B.md_flock_params(*par0, speed), S.pos, S.id, S.nbr_idx, S.nbr_count, dt, 1, S.stats)
+    torch.cuda.synchronize()
+    e_ob, gR, gth = orc.flock_obstacle_energy_grad(pos, th0, box32, cen_o, rad_o, Jo, 3.0)
+    assert e_ob > 0 and (np.abs(gR).sum(1) > 0).sum() > 50              # boids do sit inside the disks
+    one = unpermute(S, S.pos)
+    d = one[:, :2].astype(np.float64) - pos[:, :2]
+    d -= L * np.round(d / L)
+    want = dt * (speed * np.stack([np.cos(th0), np.sin(th0)], 1) - gR)
+    assert np.abs(d - want).max() <= 4e-6 * max(1.0, np.abs(want).max())
+    assert np.abs((one[:, 3].astype(np.float64) - th0) + dt * gth).max() <= 1e-6 * max(1.0, np.abs(gth).max())
+    S.close()
+    par = (1.0, 3.0, 10.0, 1.5, 0.0, 4.0, 3.0)
+    S = B.System(w)
+    B.md_flock_obstacles(S.sys, cen_o, rad_o, Jo)
+    S.build()
+    B.md_flock_step(S.sys, B.md_flock_params(*par, speed), S.pos, S.id, S.nbr_idx, S.nbr_count, dt, 60, S.stats)
+    torch.cuda.synchronize()
+    orc.flock_set_obstacles(cen_o, rad_o, Jo)
+    try:
+        p_o, th_o = orc.flock_run(pos, th0, box32, par, speed, dt, 60)
+    finally:
+        orc.flock_set_obstacles()
+    got = unpermute(S, S.pos)
+    d = got[:, :2].astype(np.float64) - p_o[:, :2]
+    d -= L * np.round(d / L)
+    assert np.abs(d).max() <= 1e-4, np.abs(d).max()
+    assert np.abs(got[:, 3].astype(np.float64) - th_o).max() <= 1e-4
+    # removing the obstacles restores the plain model (and re-captures the graph)
+    B.md_flock_obstacles(S.sys)
+    S.reset(); S.build()
+    B.md_flock_step(S.sys, B.md_flock_params(*par, speed), S.pos, S.id, S.nbr_idx, S.nbr_count, dt, 60, S.stats)
+    torch.cuda.synchronize()
+    assert torch.equal(S.pos, outs[0][1])
+    with pytest.raises(B.MdError):
+        B.md_flock_obstacles(S.sys, [[1.0, 1.0]], [30.0], 1.0)          # radius above half the box
+    S.close()
+
 
 def test_fast32_dimers_at_the_force_zero(B, orc, W):
     """Isolated pairs around r = 2^(1/6) sigma, where the LJ force changes sign: the coefficient and
