@@ -20,7 +20,8 @@
  *   displacement        L72 §3.2.1 "displacement between a particle and the
  *                       nearest image of the second particle"
  *   (the "next" rows)
- *   kinds 2, 3, 4       L104 Morse [75], Buckingham-type [71-73], per-species LJ tables (L298-L305)
+ *   kinds 2, 3, 4, 5    L104 Morse [75], Buckingham-type [71-73], per-species LJ tables (L298-L305),
+ *                       BKS-type exp-6 + damped shifted-force Coulomb per species pair
  *   orc_fire_run        L100 "Fire Descent [68]", used at L322 (Bitzek et al.'s algorithm)
  *   orc_brownian_run    L100 "Brownian" (Euler-Maruyama; kT = 0: "Gradient Descent")
  *   orc_langevin_run    L100 "Langevin" (BAOAB splitting)
@@ -71,6 +72,7 @@
 #define KIND_MORSE 2
 #define KIND_BUCK 3
 #define KIND_LJ_SPECIES 4
+#define KIND_BKS 5
 
 int orc_num_threads(void)
 {
@@ -440,6 +442,34 @@ int orc_set_species_lj(int ns, const double *eps, const double *sigma, const dou
     return ORC_OK;
 }
 
+/* BKS-type potential ("Buckingham / BKS" [71-73]; named only, reading A27):
+ * the exp-6 term with per-species-pair A_ab, B_ab, C_ab plus the Coulomb interaction of point charges
+ * q_a.  A bare 1/r cannot live on a cutoff list, so the Coulomb term is the damped shifted-force form
+ * (Fennell & Gezelter 2006), whose energy AND force vanish at r_c:
+ *   u_C(r) = k q_a q_b [ erfc(a r)/r - erfc(a rc)/rc + (erfc(a rc)/rc^2 + 2a/sqrt(pi) exp(-a^2 rc^2)/rc)(r - rc) ]
+ *   -u_C'(r) = k q_a q_b [ erfc(a r)/r^2 + 2a/sqrt(pi) exp(-a^2 r^2)/r - erfc(a rc)/rc^2 - 2a/sqrt(pi) exp(-a^2 rc^2)/rc ]
+ * kind 5: species = (int)diam[i]; r_cut is the one truncation radius; shift applies to the exp-6 term. */
+static double g_bks_A[ORC_MAX_SPECIES * ORC_MAX_SPECIES], g_bks_B[ORC_MAX_SPECIES * ORC_MAX_SPECIES],
+              g_bks_C[ORC_MAX_SPECIES * ORC_MAX_SPECIES], g_bks_q[ORC_MAX_SPECIES], g_bks_a = 0.0, g_bks_k = 1.0;
+static int g_bks_ns = 0;
+int orc_set_species_bks(int ns, const double *A, const double *B, const double *Cc, const double *q,
+                        double coulomb_alpha, double k_e)
+{
+    if (ns < 1 || ns > ORC_MAX_SPECIES || !(coulomb_alpha >= 0.0)) return ORC_EINVAL;
+    g_bks_ns = ns; g_bks_a = coulomb_alpha; g_bks_k = k_e;
+    for (int k = 0; k < ns * ns; ++k) { g_bks_A[k] = A[k]; g_bks_B[k] = B[k]; g_bks_C[k] = Cc[k]; }
+    for (int k = 0; k < ns; ++k) g_bks_q[k] = q[k];
+    return ORC_OK;
+}
+
+static void dsf_pair(double r, double qq, double a, double rc, double *u, double *fr)
+{
+    const double tsp = 2.0 * a / sqrt(3.14159265358979323846);
+    const double ec = erfc(a * rc) / rc, fc = ec / rc + tsp * exp(-a * a * rc * rc) / rc;
+    *u = qq * (erfc(a * r) / r - ec + fc * (r - rc));
+    *fr = qq * (erfc(a * r) / (r * r) + tsp * exp(-a * a * r * r) / r - fc) / r;
+}
+
 static double lj_u_cut(double eps, double sigma, double r_cut)
 {
     double u, fr;
@@ -459,6 +489,8 @@ static double lj_u_cut(double eps, double sigma, double r_cut)
  *                species = (int)diam[i]; eps, sigma, r_cut arguments unused
  *   kind 3 BUCKINGHAM: u = eps exp(-alpha r) - sigma / r^6 - shift*u(r_cut) for r < r_cut
  *                (A = eps, B = alpha, C = sigma; PAPER.md:L104 [71-73])
+ *   kind 5 BKS:  exp-6 with A, B, C per species pair plus damped shifted-force Coulomb between the
+ *                species' charges (orc_set_species_bks); eps, sigma unused; one r_cut
  *   nbr_idx == NULL: all pairs j != i (the definition);
  *   else: over the list rows (L80 smap.neighbors), entries >= n are padding.
  *   force double[n*3] (z = 0 in 2-D), e_i double[n], *E double.
@@ -471,9 +503,10 @@ int orc_energy_force(int n, int dim, const double *pos, const double *diam,
 {
     if (n <= 0 || (dim != 2 && dim != 3)) return ORC_EINVAL;
     if (kind != KIND_LJ && kind != KIND_SOFT && kind != KIND_MORSE && kind != KIND_BUCK &&
-        kind != KIND_LJ_SPECIES) return ORC_EINVAL;
-    if ((kind == KIND_SOFT || kind == KIND_LJ_SPECIES) && !diam) return ORC_EINVAL;
+        kind != KIND_LJ_SPECIES && kind != KIND_BKS) return ORC_EINVAL;
+    if ((kind == KIND_SOFT || kind == KIND_LJ_SPECIES || kind == KIND_BKS) && !diam) return ORC_EINVAL;
     if (kind == KIND_LJ_SPECIES && g_ns < 1) return ORC_EINVAL;
+    if (kind == KIND_BKS && g_bks_ns < 1) return ORC_EINVAL;
     double u_c = (kind == KIND_LJ && shift) ? lj_u_cut(eps, sigma, r_cut) : 0.0;
     if (kind == KIND_MORSE && shift) {
         double fr_unused;
@@ -511,6 +544,19 @@ int orc_energy_force(int n, int dim, const double *pos, const double *diam,
                     lj_pair(r2, g_sp_eps[t], g_sp_sig[t], &u, &fr);
                     e += 0.5 * (u - (shift ? lj_u_cut(g_sp_eps[t], g_sp_sig[t], g_sp_rc[t]) : 0.0));
                     for (int q = 0; q < dim; ++q) f[q] += fr * d[q];
+                }
+            } else if (kind == KIND_BKS) {
+                int sa = (int)diam[i], sb = (int)diam[j];
+                if (sa < 0 || sa >= g_bks_ns || sb < 0 || sb >= g_bks_ns) continue;
+                int t = sa * g_bks_ns + sb;
+                if (r2 < r_cut * r_cut && r2 > 0.0) {
+                    double u, fr, uc, fc_unused, ue, fe;
+                    const double r = sqrt(r2);
+                    buck_pair(r, g_bks_A[t], g_bks_B[t], g_bks_C[t], &u, &fr);
+                    buck_pair(r_cut, g_bks_A[t], g_bks_B[t], g_bks_C[t], &uc, &fc_unused);
+                    dsf_pair(r, g_bks_k * g_bks_q[sa] * g_bks_q[sb], g_bks_a, r_cut, &ue, &fe);
+                    e += 0.5 * (u - (shift ? uc : 0.0) + ue);
+                    for (int q = 0; q < dim; ++q) f[q] += (fr + fe) * d[q];
                 }
             } else if (kind == KIND_BUCK) {
                 if (r2 < r_cut * r_cut) {

@@ -119,6 +119,15 @@ def set_species_lj(eps, sigma, rc) -> None:
                                     _pd(r.reshape(-1).copy())), "set_species_lj")
 
 
+def set_species_bks(A, B, Cc, q, coulomb_alpha, k_e=1.0):
+    """Tables of kind 5 (BKS-type): square arrays A_ab, B_ab, C_ab, charges q_a, DSF damping, Coulomb constant."""
+    A = _d(A); B = _d(B); Cc = _d(Cc); q = _d(q)
+    ns = q.shape[0]
+    assert A.shape == (ns, ns) and B.shape == (ns, ns) and Cc.shape == (ns, ns)
+    _check(lib().orc_set_species_bks(ns, _pd(A), _pd(B), _pd(Cc), _pd(q), C.c_double(coulomb_alpha),
+                                     C.c_double(k_e)), "set_species_bks")
+
+
 def set_morse_alpha(alpha: float) -> None:
     """alpha of kind 2 (Morse) for the following energy_force / nve_run calls."""
     lib().orc_set_morse_alpha(C.c_double(alpha))

@@ -924,3 +924,72 @@ def test_flocking_obstacles(orc):
         orc.flock_set_obstacles()
     p, t = orc.flock_run(at(8.8, 10.0), [0.0], box, par0, 0.5, 0.1, 1)               # obstacles cleared
     assert abs(p[0, 0] - 8.85) < 1e-12
+
+
+def test_bks_type_potential(orc):
+    """Kind 5 ("Buckingham / BKS" [71-73]; A27): exp-6 per species pair plus damped
+    shifted-force Coulomb.
+    (a) the rock-salt lattice: energy per ion plus the Wolf self term reproduces the Madelung constant
+        1.747565 (exact lattice sum) to 1e-5, forces vanish by symmetry;
+    (b) no damping: the textbook shifted-force Coulomb q q'(1/r - 1/rc + (r - rc)/rc^2), and bare q q'/r as
+        rc -> infinity; energy and force both vanish at the cutoff; like charges repel;
+    (c) zero charges: kind 3 (Buckingham, pinned on its own) with the same A, B, C;
+    (d) forces are minus the central differences of the energy for a random binary configuration."""
+    from math import erfc, sqrt, pi
+    m, rc, a = 6, 5.9, 0.6
+    g = np.stack(np.meshgrid(*[np.arange(2 * m)] * 3, indexing="ij"), -1).reshape(-1, 3)
+    pos = g.astype(np.float64) + 0.25
+    sp = (g.sum(1) % 2).astype(np.float64)
+    box = np.array([2.0 * m] * 3)
+    z = np.zeros((2, 2))
+    orc.set_species_bks(z, z + 1.0, z, [1.0, -1.0], a, 1.0)
+    f, e, E = orc.energy_force(pos, sp, box, 3, 5, 0.0, 0.0, rc, 0)
+    per_ion = E / len(pos) - (erfc(a * rc) / (2 * rc) + a / sqrt(pi))
+    assert abs(per_ion - (-1.747565 / 2)) < 1e-5, per_ion
+    assert np.abs(f).max() < 1e-12
+    # (b)
+    big = np.array([400.0, 400.0, 400.0])
+    two = lambda r: np.array([[100.0, 100.0, 100.0], [100.0 + r, 100.0, 100.0]])
+    orc.set_species_bks(z, z + 1.0, z, [2.0, -0.5], 0.0, 3.0)
+    for r in (0.8, 1.7, 2.9):
+        f, e, E = orc.energy_force(two(r), [0.0, 1.0], big, 3, 5, 0.0, 0.0, 3.0, 0)
+        qq = 3.0 * 2.0 * -0.5
+        assert abs(E - qq * (1 / r - 1 / 3.0 + (r - 3.0) / 9.0)) < 1e-13
+        assert abs(f[0, 0] - (-qq * (1 / r**2 - 1 / 9.0))) < 1e-13 and f[0, 0] > 0      # attracted toward +x
+        assert np.allclose(f[0], -f[1], atol=1e-15)
+    f, e, E = orc.energy_force(two(1.3), [0.0, 0.0], big, 3, 5, 0.0, 0.0, 3.0, 0)
+    assert E > 0 and f[0, 0] < 0                                                         # like charges repel
+    f, e, E = orc.energy_force(two(2.0), [0.0, 1.0], big, 3, 5, 0.0, 0.0, 150.0, 0)
+    assert abs(E - (-3.0 / 2.0)) < 0.05                                                  # 2 q q' / rc away from bare Coulomb
+    orc.set_species_bks(z, z + 1.0, z, [1.0, -1.0], 0.35, 1.0)
+    f, e, E = orc.energy_force(two(3.0 - 1e-7), [0.0, 1.0], big, 3, 5, 0.0, 0.0, 3.0, 0)
+    assert abs(E) < 1e-13 and np.abs(f).max() < 1e-7
+    f, e, E = orc.energy_force(two(3.0 + 1e-7), [0.0, 1.0], big, 3, 5, 0.0, 0.0, 3.0, 0)
+    assert E == 0.0 and not f.any()
+    # (c)
+    rng = np.random.default_rng(2)
+    n, L = 200, 9.0
+    gq = (np.arange(6) + 0.5) * (L / 6)
+    p = np.stack(np.meshgrid(gq, gq, gq, indexing="ij"), -1).reshape(-1, 3)[:n] + rng.normal(0, 0.08, (n, 3))
+    bx = np.array([L, L, L])
+    A, Bq, Cq = 9.02e5, 12.5, 3.454
+    one = np.ones((2, 2))
+    spc = (np.arange(n) % 2).astype(np.float64)
+    orc.set_species_bks(A * one, Bq * one, Cq * one, [0.0, 0.0], 0.3, 1.0)
+    f5, e5, E5 = orc.energy_force(p, spc, bx, 3, 5, 0.0, 0.0, 2.5, 1)
+    f3, e3, E3 = orc.energy_force(p, None, bx, 3, 3, A, Cq, 2.5, 1, alpha=Bq)
+    assert np.abs(f5 - f3).max() < 1e-12 * np.abs(f3).max() and abs(E5 - E3) < 1e-12 * abs(E3)
+    # (d) distinct tables per pair, charges on
+    Am = A * np.array([[1.0, 0.7], [0.7, 0.5]]); Bm = Bq * np.array([[1.0, 1.05], [1.05, 1.1]])
+    Cm = Cq * np.array([[1.0, 0.6], [0.6, 0.3]])
+    orc.set_species_bks(Am, Bm, Cm, [0.6, -0.6], 0.3, 1.0)
+    f, e, E = orc.energy_force(p, spc, bx, 3, 5, 0.0, 0.0, 2.5, 1)
+    h, worst = 1e-6, 0.0
+    for i in rng.choice(n, 6, replace=False):
+        for q in range(3):
+            pp = p.copy(); pp[i, q] += h; pm = p.copy(); pm[i, q] -= h
+            fd = -(orc.energy_force(pp, spc, bx, 3, 5, 0.0, 0.0, 2.5, 1)[2]
+                   - orc.energy_force(pm, spc, bx, 3, 5, 0.0, 0.0, 2.5, 1)[2]) / (2 * h)
+            worst = max(worst, abs(fd - f[i, q]))
+    assert worst < 1e-6 * max(1.0, np.abs(f).max()), worst
+    assert np.abs(f.sum(0)).max() < 1e-10 * np.abs(f).max()                              # Newton's third law
