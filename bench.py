@@ -233,6 +233,12 @@ def run_next_rows(args):
     B.md_set_species_lj(S.sys, eps, sig, (2.5 * sig).astype(np.float32))
     emit("f2", "species x species LJ force (80:20 binary mixture), fp64 pair chain", time_force(S)); S.close()
 
+    w = dataclasses.replace(base, kind=W.KIND_BKS, pos=pos, r_cut=2.5)
+    S = B.System(w)
+    one = np.ones((2, 2), np.float32)
+    B.md_set_species_bks(S.sys, 9.02e5 * one, 12.5 * one, 3.454 * one, np.array([0.6, -0.6], np.float32), 0.3, 1.0)
+    emit("f2", "BKS-type force (exp-6 + damped shifted-force Coulomb, 2 species), fp64 pair chain", time_force(S)); S.close()
+
     # f3: update rules, LJ fast path, 200 steps each
     steps = 200
     S = B.System(base); S.build(); S.compute_force()

@@ -48,6 +48,7 @@ extern "C" {
 #define MD_KIND_SOFT 1      /* harmonic soft sphere [70], L104; d_ij = (d_i+d_j)/2, L301 App. A */
 #define MD_KIND_MORSE 2     /* Morse [75], L104: u = eps (1 - exp(-alpha (r - sigma)))^2 - eps */
 #define MD_KIND_LJ_SPECIES 4 /* LJ with eps, sigma, r_cut per species pair (md_set_species_lj); species = (int)pos.w */
+#define MD_KIND_BKS 5        /* exp-6 per species pair + damped shifted-force Coulomb (md_set_species_bks) */
 #define MD_KIND_BUCKINGHAM 3 /* Buckingham-type exp-6 [71-73], L104: u = eps exp(-alpha r) - sigma / r^6
                                (epsilon = A, alpha = B, sigma = C) */
 
@@ -114,6 +115,17 @@ int md_set_option(md_system *sys, const char *name, double value);
  * ignored; shift applies per pair); the species of a particle is (int)pos.w.  fp64 pair chain. */
 int md_set_species_lj(md_system *sys, int nspecies, const float *epsilon, const float *sigma,
                       const float *r_cut);
+
+/* BKS-type potential (L104 "Buckingham / BKS" [71-73], named only; reading A27): per species
+ * pair the exp-6 term A_ab exp(-B_ab r) - C_ab / r^6, plus the Coulomb interaction of the species' point
+ * charges in its damped shifted-force form (energy and force both vanish at r_cut):
+ *   u_C = k_e q_a q_b [erfc(a r)/r - erfc(a rc)/rc + (erfc(a rc)/rc^2 + 2a/sqrt(pi) exp(-a^2 rc^2)/rc)(r - rc)]
+ * host float[nspecies * nspecies] A, B, C (row-major, A >= 0, B > 0, C >= 0), host float[nspecies] charge,
+ * 1 <= nspecies <= 4, coulomb_alpha = a >= 0, k_e >= 0.  Used by MD_KIND_BKS: md_potential.r_cut is the one
+ * truncation radius (<= the list r_cut), shift applies to the exp-6 term, epsilon / sigma / alpha are
+ * ignored; the species of a particle is (int)pos.w.  fp64 pair chain. */
+int md_set_species_bks(md_system *sys, int nspecies, const float *A, const float *B, const float *C,
+                       const float *charge, float coulomb_alpha, float k_e);
 
 /* Diagnostic counters since md_create (or the last reset): copies int32[8] to the DEVICE buffer
  * `out` on `stream`, then clears them if reset != 0.

@@ -23,7 +23,7 @@ SYMBOLS = [
     "md_needs_rebuild", "md_pair_energy_force", "md_nve_step", "md_nve_run_host", "md_counters",
     "md_nve_run_host_release", "md_fire_minimize", "md_brownian_step",
     "md_langevin_step", "md_nose_hoover_step", "md_set_species_lj",
-    "md_flock_step", "md_flock_obstacles",
+    "md_flock_step", "md_flock_obstacles", "md_set_species_bks",
 ]
 
 
@@ -83,6 +83,7 @@ def lib():
                                        C.c_float, C.c_float, C.c_uint32, C.c_uint32, C.c_int, ip, vp]
         L.md_nose_hoover_step.argtypes = [vp, C.POINTER(md_potential), vp, vp, vp, ip, ip, ip, C.c_float,
                                           C.c_float, C.c_float, C.c_float, vp, C.c_int, ip, vp]
+        L.md_set_species_bks.argtypes = [vp, C.c_int] + [C.POINTER(C.c_float)] * 4 + [C.c_float, C.c_float]
         L.md_flock_obstacles.argtypes = [vp, C.c_int, C.POINTER(C.c_float), C.POINTER(C.c_float), C.c_float]
         L.md_flock_step.argtypes = [vp, C.POINTER(md_flock_params), vp, ip, ip, ip, C.c_float, C.c_int, ip, vp]
         L.md_fire_minimize.argtypes = [vp, C.POINTER(md_potential), C.POINTER(md_fire_params), vp, vp, vp,
@@ -220,6 +221,16 @@ def md_set_species_lj(sys, epsilon, sigma, r_cut) -> None:
     fp = C.POINTER(C.c_float)
     _check(lib().md_set_species_lj(sys, int(e.shape[0]), e.ctypes.data_as(fp), sg.ctypes.data_as(fp),
                                    r.ctypes.data_as(fp)))
+
+
+def md_set_species_bks(sys, A, B, Cc, charge, coulomb_alpha, k_e=1.0) -> None:
+    import numpy as np
+    q = np.ascontiguousarray(np.asarray(charge, np.float32).reshape(-1))
+    ns = q.shape[0]
+    tabs = [np.ascontiguousarray(np.asarray(t, np.float32).reshape(ns * ns)) for t in (A, B, Cc)]
+    fp = C.POINTER(C.c_float)
+    _check(lib().md_set_species_bks(sys, ns, *[t.ctypes.data_as(fp) for t in tabs], q.ctypes.data_as(fp),
+                                    float(coulomb_alpha), float(k_e)))
 
 
 def md_counters(sys, out, reset=False, stream=None) -> None:

@@ -106,6 +106,8 @@ struct md_system {
     int nb_parts;        // builder: warps per tile (0 = by system size, 1, 2, 4)
     int ns;              // md_set_species_lj: number of species and the tables (row-major)
     float sp_eps[16], sp_sig[16], sp_rc[16];
+    int bks_ns;          // md_set_species_bks: A, B, C per species pair, charges, DSF damping, Coulomb constant
+    float bks_A[16], bks_B[16], bks_C[16], bks_q[4], bks_alpha, bks_ke;
     int nobs;            // md_flock_obstacles
     float obs[3 * MD_MAX_OBSTACLES], J_obs;
     int builder;         // neighbor-list builder: 2 = bit-mask (md_nbr2.cuh), 1 = column append
@@ -199,9 +201,10 @@ int make_geom(const md_config *cfg, int n, Geom *g) {
 int make_pair(const md_system *sys, const md_potential *pot, Pair *pp) {
     if (!pot) return fail(MD_EINVAL, "potential is NULL");
     if (pot->kind != MD_KIND_LJ && pot->kind != MD_KIND_SOFT && pot->kind != MD_KIND_MORSE &&
-        pot->kind != MD_KIND_BUCKINGHAM && pot->kind != MD_KIND_LJ_SPECIES)
+        pot->kind != MD_KIND_BUCKINGHAM && pot->kind != MD_KIND_LJ_SPECIES && pot->kind != MD_KIND_BKS)
         return fail(MD_EINVAL, "unknown potential kind %d", pot->kind);
-    if (!(pot->epsilon > 0.0f)) return fail(MD_EINVAL, "epsilon must be positive");
+    if (pot->kind != MD_KIND_LJ_SPECIES && pot->kind != MD_KIND_BKS && !(pot->epsilon > 0.0f))
+        return fail(MD_EINVAL, "epsilon must be positive");
     memset(pp, 0, sizeof(*pp));
     pp->kind = pot->kind;
     pp->deps = (double)pot->epsilon;
@@ -229,6 +232,22 @@ int make_pair(const md_system *sys, const md_potential *pot, Pair *pp) {
             pp->sp_sig6x2[t] = 2.0 * s6; pp->sp_fs[t] = 24.0 * e * s6; pp->sp_es[t] = 2.0 * e;
             pp->sp_rc2[t] = rc * rc; pp->sp_ucut4[t] = pot->shift ? (q6 * q6 - q6) : 0.0;
         }
+    } else if (pot->kind == MD_KIND_BKS) {
+        if (sys->bks_ns < 1) return fail(MD_EINVAL, "MD_KIND_BKS needs md_set_species_bks first");
+        if (!(pot->r_cut > 0.0f) || pot->r_cut > sys->cfg.r_cut)
+            return fail(MD_EINVAL, "potential r_cut %g must be positive and at most the list r_cut %g", pot->r_cut, sys->cfg.r_cut);
+        const double rc = pot->r_cut, a = sys->bks_alpha;
+        pp->ns = sys->bks_ns; pp->dsig6x2 = 2.0; pp->drc2 = rc * rc;
+        for (int t = 0; t < sys->bks_ns * sys->bks_ns; ++t) {
+            const double A = sys->bks_A[t], B = sys->bks_B[t], Cc = sys->bks_C[t];
+            pp->sp_sig6x2[t] = A; pp->sp_fs[t] = B; pp->sp_es[t] = Cc;
+            pp->sp_rc2[t] = (double)sys->bks_ke * (double)sys->bks_q[t / sys->bks_ns] * (double)sys->bks_q[t % sys->bks_ns];
+            pp->sp_ucut4[t] = pot->shift ? (A * std::exp(-B * rc) - Cc / std::pow(rc, 6.0)) : 0.0;
+        }
+        pp->bks_a = a; pp->bks_tsp = 2.0 * a / std::sqrt(3.14159265358979323846);
+        pp->bks_ec = std::erfc(a * rc) / rc;
+        pp->bks_fc = pp->bks_ec / rc + pp->bks_tsp * std::exp(-a * a * rc * rc) / rc;
+        pp->bks_rc = rc;
     } else if (pot->kind == MD_KIND_BUCKINGHAM) {
         if (!(pot->r_cut > 0.0f) || !(pot->sigma >= 0.0f) || !(pot->alpha > 0.0f))
             return fail(MD_EINVAL, "Buckingham needs alpha (B) > 0, sigma (C) >= 0 and r_cut > 0");
@@ -370,6 +389,7 @@ int launch_force(md_system *s, const Pair &pp, const float4 *pos, const int *nbr
     if (pp.kind == MD_KIND_MORSE) return s->g.dim == 3 ? MD_FORCE_DISPATCH(2, 3) : MD_FORCE_DISPATCH(2, 2);
     if (pp.kind == MD_KIND_LJ_SPECIES) return s->g.dim == 3 ? MD_FORCE_DISPATCH(4, 3) : MD_FORCE_DISPATCH(4, 2);
     if (pp.kind == MD_KIND_BUCKINGHAM) return s->g.dim == 3 ? MD_FORCE_DISPATCH(3, 3) : MD_FORCE_DISPATCH(3, 2);
+    if (pp.kind == MD_KIND_BKS) return s->g.dim == 3 ? MD_FORCE_DISPATCH(5, 3) : MD_FORCE_DISPATCH(5, 2);
     return s->g.dim == 3 ? MD_FORCE_DISPATCH(1, 3) : MD_FORCE_DISPATCH(1, 2);
 #undef MD_FORCE_DISPATCH
 }
@@ -1023,6 +1043,21 @@ int md_nose_hoover_step(md_system *sys, const md_potential *pot, void *pos, void
     A.rule = RULE_NH; A.pos = pos; A.vel = vel; A.force = force; A.state = nh_state; A.id = id; A.nbr_idx = nbr_idx;
     A.nbr_count = nbr_count; A.stats = stats; A.pot = *pot; A.dt = dt; A.mass = mass; A.kT = kT; A.tau = tau;
     return run_rule(sys, pp, A, nsteps, (cudaStream_t)stream);
+}
+
+int md_set_species_bks(md_system *sys, int nspecies, const float *A, const float *B, const float *C,
+                       const float *charge, float coulomb_alpha, float k_e) {
+    if (!sys || !A || !B || !C || !charge) return fail(MD_EINVAL, "NULL argument");
+    if (nspecies < 1 || nspecies > 4) return fail(MD_EINVAL, "nspecies = %d must be in 1..4", nspecies);
+    if (!(coulomb_alpha >= 0.0f) || !(k_e >= 0.0f)) return fail(MD_EINVAL, "coulomb_alpha and k_e must be >= 0");
+    for (int t = 0; t < nspecies * nspecies; ++t)
+        if (!(A[t] >= 0.0f) || !(B[t] > 0.0f) || !(C[t] >= 0.0f))
+            return fail(MD_EINVAL, "species pair %d: need A >= 0, B > 0, C >= 0", t);
+    sys->bks_ns = nspecies; sys->bks_alpha = coulomb_alpha; sys->bks_ke = k_e;
+    for (int t = 0; t < nspecies * nspecies; ++t) { sys->bks_A[t] = A[t]; sys->bks_B[t] = B[t]; sys->bks_C[t] = C[t]; }
+    for (int t = 0; t < nspecies; ++t) sys->bks_q[t] = charge[t];
+    drop_graphs(sys);
+    return MD_OK;
 }
 
 int md_flock_obstacles(md_system *sys, int nobs, const float *centre, const float *radius, float J) {

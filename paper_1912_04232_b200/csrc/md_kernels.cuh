@@ -37,6 +37,9 @@ struct Pair {
     double sp_es[16];       // 2 eps_ab  (1/2 * 4 eps_ab)
     double sp_rc2[16];      // rc_ab^2
     double sp_ucut4[16];    // shift * ((s/rc)^12 - (s/rc)^6)
+    // BKS (kind 5) reuses the five tables as A_ab, B_ab, C_ab, k q_a q_b, shift * u_exp6(r_cut) and adds
+    // the damped shifted-force Coulomb constants: a, 2a/sqrt(pi), erfc(a rc)/rc, its force shift, rc
+    double bks_a, bks_tsp, bks_ec, bks_fc, bks_rc;
 };
 
 // Device words md_nve_step keeps between kernels.
@@ -733,6 +736,25 @@ __device__ __forceinline__ void ljs_pair64(const Pair &pp, const double *sp, dou
     }
 }
 
+// One pair, BKS-type (L104 [71-73]; A27): exp-6 with A, B, C of the species pair plus the
+// damped shifted-force Coulomb term between the species' charges; one cutoff; nothing factored out.
+//   -u'/r = (A B e^{-B r} - 6 C / r^7)/r + k q q' (erfc(a r)/r^2 + (2a/sqrt(pi)) e^{-a^2 r^2}/r - f_c)/r
+template <bool ENERGY>
+__device__ __forceinline__ void bks_pair64(const Pair &pp, const double *sp, double dx, double dy, double dz,
+                                           float wi, float wj, bool valid, Acc64 &a) {
+    const int sa = min(max((int)wi, 0), pp.ns - 1), sb = min(max((int)wj, 0), pp.ns - 1);
+    const int t = sa * pp.ns + sb;
+    const double r2 = fma(dz, dz, fma(dy, dy, dx * dx));
+    const bool in = valid && r2 < pp.drc2 && r2 > 0.0;
+    const double r2s = in ? r2 : 1.0;
+    const double ir = rsqrt64(r2s), r = r2s * ir, y = ir * ir, y3 = y * y * y;
+    const double x = sp[t] * exp(-sp[16 + t] * r), C6 = sp[32 + t] * y3, qq = sp[48 + t];
+    const double er = erfc(pp.bks_a * r), ex = pp.bks_tsp * exp(-pp.bks_a * pp.bks_a * r2s);
+    const double c = in ? (sp[16 + t] * x * r - 6.0 * C6) * y + qq * (er * y + ex * ir - pp.bks_fc) * ir : 0.0;
+    a.fx = fma(c, dx, a.fx); a.fy = fma(c, dy, a.fy); a.fz = fma(c, dz, a.fz);
+    if (ENERGY) a.e += in ? x - C6 - sp[64 + t] + qq * (er * ir - pp.bks_ec + pp.bks_fc * (r - pp.bks_rc)) : 0.0;
+}
+
 // Per-thread view of the space for the pair loop.
 template <int DIM>
 struct Me {
@@ -773,6 +795,7 @@ __device__ __forceinline__ void pair_any(const Pair &pp, const Me<DIM> &me, cons
     else if (KIND == 2) morse_pair64<ENERGY>(pp, dx, dy, dz, valid, acc);
     else if (KIND == 3) buck_pair64<ENERGY>(pp, dx, dy, dz, valid, acc);
     else if (KIND == 4) ljs_pair64<ENERGY>(pp, sp, dx, dy, dz, me.pi.w, q.w, valid, acc);
+    else if (KIND == 5) bks_pair64<ENERGY>(pp, sp, dx, dy, dz, me.pi.w, q.w, valid, acc);
     else soft_pair64<ENERGY>(pp, dx, dy, dz, (double)me.pi.w + (double)q.w, valid, acc);
 }
 
@@ -799,9 +822,9 @@ __device__ __forceinline__ void force_epilogue(const Pair &pp, const Acc64 &acc,
                                                float4 *__restrict__ force, float4 *__restrict__ vel,
                                                float a, double *energy_total, const Book &book,
                                                int gid) {
-    const double fs = KIND == 0 ? 12.0 * pp.deps * pp.dsig6x2 : (KIND == 3 || KIND == 4 ? 1.0 : pp.deps);   // 24 eps sig^6 | eps | D | 1
+    const double fs = KIND == 0 ? 12.0 * pp.deps * pp.dsig6x2 : (KIND == 3 || KIND == 4 || KIND == 5 ? 1.0 : pp.deps);   // 24 eps sig^6 | eps | D | 1
     const double es = KIND == 0 ? 2.0 * pp.deps
-                    : (KIND == 2 ? 0.5 * pp.deps : (KIND == 3 ? 0.5 : (KIND == 4 ? 1.0 : 0.25 * pp.deps)));   // 1/2 * (4 eps | D | 1 | eps/2)
+                    : (KIND == 2 ? 0.5 * pp.deps : (KIND == 3 || KIND == 5 ? 0.5 : (KIND == 4 ? 1.0 : 0.25 * pp.deps)));   // 1/2 * (4 eps | D | 1 | eps/2)
     const float fx = (float)(fs * acc.fx), fy = (float)(fs * acc.fy), fz = (float)(fs * acc.fz);
     const double e64 = ENERGY ? es * acc.e : 0.0;
     if (owner) {
@@ -846,8 +869,8 @@ __global__ void __launch_bounds__(128)
 k_force(Geom g, Pair pp, const float4 *__restrict__ pos, const int *__restrict__ nbr_idx,
         const int *__restrict__ nbr_count, float4 *__restrict__ force, float4 *__restrict__ vel,
         float a, double *energy_total, Book book) {
-    __shared__ double sp[KIND == 4 ? SP_TAB : 1];
-    if (KIND == 4) species_tables_to_shared(pp, sp);
+    __shared__ double sp[KIND == 4 || KIND == 5 ? SP_TAB : 1];
+    if (KIND == 4 || KIND == 5) species_tables_to_shared(pp, sp);
     const int gid = blockIdx.x * blockDim.x + threadIdx.x;
     const int i = gid / TPP, sub = gid % TPP;
     const bool active = i < g.n;
@@ -917,8 +940,8 @@ k_force_stream(Geom g, Pair pp, const float4 *__restrict__ pos, const int *__res
                float4 *__restrict__ vel, float a, double *energy_total, Book book) {
     __shared__ __align__(128) int s_idx[FS_WARPS][FS_STAGES][FS_ROWS * TILE];
     __shared__ __align__(8) unsigned long long s_bar[FS_WARPS][FS_STAGES];
-    __shared__ double sp[KIND == 4 ? SP_TAB : 1];
-    if (KIND == 4) species_tables_to_shared(pp, sp);
+    __shared__ double sp[KIND == 4 || KIND == 5 ? SP_TAB : 1];
+    if (KIND == 4 || KIND == 5) species_tables_to_shared(pp, sp);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int gid = blockIdx.x * blockDim.x + threadIdx.x;
     const int i = gid;

@@ -31,6 +31,7 @@ KIND_SOFT = 1
 KIND_MORSE = 2
 KIND_BUCKINGHAM = 3
 KIND_LJ_SPECIES = 4
+KIND_BKS = 5
 
 
 @dataclasses.dataclass(frozen=True)

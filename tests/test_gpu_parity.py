@@ -470,6 +470,57 @@ def test_species_lj_binary_mixture(B, orc, W):
     S1.close(); S0.close()
 
 
+def test_bks_type_binary_crystal(B, orc, W):
+    """BKS-type potential (PAPER.md:L104 [71-73]; A27): exp-6 with distinct A, B, C
+    per species pair plus damped shifted-force Coulomb between charges +-0.6 on the jittered lattice of
+    config 0: force / energy against the all-pairs definition, 100 NVE steps against the oracle; zero
+    charges and equal tables reproduce the Buckingham kind."""
+    A0, B0, C0, rc = 9.02e5, 12.5, 3.454, 2.5
+    f32 = lambda a: np.asarray(a, np.float32)
+    Am = f32(A0 * np.array([[1.0, 0.7], [0.7, 0.5]])); Bm = f32(B0 * np.array([[1.0, 1.05], [1.05, 1.1]]))
+    Cm = f32(C0 * np.array([[1.0, 0.6], [0.6, 0.3]])); q = f32([0.6, -0.6])
+    alpha_c, ke = float(np.float32(0.3)), float(np.float32(1.0))
+    base = W.config(0)
+    pos = base.pos.copy()
+    pos[:, 3] = (np.arange(base.n) % 2).astype(np.float32)
+    w = custom_workload(W, pos, base.box, 3, 5, rc, 0.3, 128, vel=base.vel.copy(), dt=0.004)
+    w = dataclasses.replace(w, shift=1)
+    S = B.System(w)
+    B.md_set_species_bks(S.sys, Am, Bm, Cm, q, alpha_c, ke)
+    S.build(); S.compute_force()
+    d64 = lambda a: np.asarray(a, np.float64)
+    orc.set_species_bks(d64(Am), d64(Bm), d64(Cm), d64(q), alpha_c, ke)
+    sp = pos[:, 3].astype(np.float64)
+    f_o, e_o, E_o = orc.energy_force(w.pos, sp, w.box, 3, 5, 0.0, 0.0, rc, 1)
+    assert force_error(unpermute(S, S.force), f_o) <= FORCE_TOL
+    assert abs(float(S.energy.cpu()[0]) - E_o) <= ENERGY_TOL * abs(E_o)
+    p_o, v_o, _, _, _ = orc.nve_run(w.pos, w.vel, f_o, sp, w.box, 3, 5, 0.0, 0.0, rc, 1, w.dt, w.mass, 100,
+                                    want_energies=False)
+    S.step(100)
+    torch.cuda.synchronize()
+    d = unpermute(S, S.pos)[:, :3].astype(np.float64) - p_o
+    L = w.box.astype(np.float64)
+    d -= L * np.round(d / L)
+    assert np.abs(d).max() <= 1e-4, np.abs(d).max()
+    S.close()
+    # zero charges, equal tables: the Buckingham kind
+    one = np.ones((2, 2), np.float32)
+    S5 = B.System(w)
+    B.md_set_species_bks(S5.sys, f32(A0) * one, f32(B0) * one, f32(C0) * one, f32([0.0, 0.0]), alpha_c, ke)
+    w3 = dataclasses.replace(w, kind=3, epsilon=float(np.float32(A0)), sigma=float(np.float32(C0)), alpha=float(np.float32(B0)))
+    S3 = B.System(w3)
+    for X in (S5, S3):
+        X.build(); X.compute_force()
+    torch.cuda.synchronize()
+    assert (S5.force[:, :3] - S3.force[:, :3]).abs().max().item() <= 1e-5 * S3.force[:, :3].abs().max().item()
+    assert abs(float(S5.energy[0]) - float(S3.energy[0])) <= 1e-9 * abs(float(S3.energy[0]))
+    S5.close(); S3.close()
+    Sx = B.System(w)
+    with pytest.raises(B.MdError):
+        Sx.build(); Sx.compute_force()                                   # tables not set
+    Sx.close()
+
+
 @pytest.mark.parametrize("rule", ["fire", "brownian", "langevin", "nose_hoover"])
 def test_update_rules_graph_and_direct_launch_agree(B, W, rule):
     """Every update rule beyond NVE runs as CUDA graphs of 8 steps (rebuild in an IF node, step
