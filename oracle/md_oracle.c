@@ -28,7 +28,7 @@
  *   orc_nose_hoover_run L100 "Nose-Hoover [67]" (one thermostat, MTK splitting)
  *   orc_normals         the counter-based normal generator both sides implement
  *   orc_flock_*         App. B: boids energies eqs. 3-10, forward Euler eqs. 4-5;
- *                       obstacles eq. 11 (L411-L418)
+ *                       obstacles eq. 11 (L411-L418), predators eqs. 12-13 (L420-L438)
  * Readings of everything the paper leaves open (strict <, half-skin, truncated
  * and shifted LJ, wrap convention, rounding of the inclusion predicate) are
  * SURVEY.md §8c A1-A18, restated in DESIGN.md §3.
@@ -1089,6 +1089,93 @@ int orc_flock_set_obstacles(int nobs, const double *centre, const double *radius
         g_obs_radius[o] = radius[o];
     }
     return ORC_OK;
+}
+
+/*
+ * Predators (App. B.3.2, eqs. 12-13; reading A28): a second, small population with
+ * the same kind of state (R_p, theta_p).  Two-player game: each side descends ITS OWN energy in its own
+ * coordinates only.
+ *   boids:     E_boid = eqs. 7-10 + obstacles + sum_{i,p} J_flee rho(r_ip; R_flee)(1 + N_i . Rhat_ip)^2
+ *              -- "the same obstacle avoiding energy" with the predator as a moving disk of radius R_flee:
+ *              orc_flock_obstacle_energy_grad with centre = predator positions serves it unchanged.
+ *   predators: E_pred = sum_p [ 1/2 J_chase (1 - Dhat_p . N_p)^2 + obstacles ],
+ *              D_p = sum_{i: |R_i - R_p| < R_chase} (R_i - R_p) -- "reuse the cohesion function": the
+ *              predator heads for the centre of mass of the boids near it; 0 if there are none.
+ *              d e/d theta_p = -J (1 - c)(-hx sin + hy cos);  grad_{R_p} e = +m J (1 - c)(N - c Dhat)/|D|
+ *              (the set held fixed, m its size), c = Dhat . N.
+ * orc_predator_energy_grad: the chase term alone; gR double[np*2], gth double[np] are OVERWRITTEN.
+ */
+int orc_predator_energy_grad(int n, const double *pos, const double *box, int np, const double *ppos /* np*2 */,
+                             const double *pth, double J, double R, double *energy, double *gR, double *gth)
+{
+    if (n <= 0 || np < 0) return ORC_EINVAL;
+    double E = 0.0;
+    for (int p = 0; p < np; ++p) {
+        double D[2] = {0.0, 0.0};
+        int m = 0;
+        for (int i = 0; i < n; ++i) {
+            const double dx = disp64(pos[3 * (size_t)i], ppos[2 * p], box[0]);            /* R_i - R_p */
+            const double dy = disp64(pos[3 * (size_t)i + 1], ppos[2 * p + 1], box[1]);
+            if (sqrt(dx * dx + dy * dy) < R) { D[0] += dx; D[1] += dy; ++m; }
+        }
+        gR[2 * p] = gR[2 * p + 1] = 0.0; gth[p] = 0.0;
+        const double Dn = sqrt(D[0] * D[0] + D[1] * D[1]);
+        if (m > 0 && Dn > 0.0) {
+            const double cp = cos(pth[p]), sn = sin(pth[p]);
+            const double hx = D[0] / Dn, hy = D[1] / Dn, c = hx * cp + hy * sn;
+            E += 0.5 * J * (1.0 - c) * (1.0 - c);
+            gth[p] = -J * (1.0 - c) * (-hx * sn + hy * cp);
+            gR[2 * p] = m * J * (1.0 - c) * (cp - c * hx) / Dn;
+            gR[2 * p + 1] = m * J * (1.0 - c) * (sn - c * hy) / Dn;
+        }
+    }
+    if (energy) *energy = E;
+    return ORC_OK;
+}
+
+/*
+ * orc_flock_run_predators: forward Euler for both populations, every gradient from the state at the
+ * start of the step.  ppar = {J_flee, R_flee, J_chase, R_chase, speed_pred}; obstacles as set by
+ * orc_flock_set_obstacles act on both.  ppos double[np*2], pth double[np] in/out.
+ */
+int orc_flock_run_predators(int n, double *pos, double *theta, const double *box, const double *par, double speed,
+                            double dt, int nsteps, int np, double *ppos, double *pth, const double *ppar)
+{
+    if (np < 0 || np > ORC_MAX_OBSTACLES) return ORC_EINVAL;
+    double *gR = (double *)malloc((size_t)n * 2 * sizeof(double)), *gth = (double *)malloc((size_t)n * sizeof(double));
+    if (!gR || !gth) { free(gR); free(gth); return ORC_ENOMEM; }
+    double qR[2 * ORC_MAX_OBSTACLES], qth[ORC_MAX_OBSTACLES], p3[3 * ORC_MAX_OBSTACLES], rfl[ORC_MAX_OBSTACLES];
+    int rc = ORC_OK;
+    for (int s = 0; s < nsteps && !rc; ++s) {
+        rc = orc_flock_energy_grad(n, pos, theta, box, par, NULL, gR, gth);
+        if (!rc && g_nobs > 0)
+            rc = orc_flock_obstacle_energy_grad(n, pos, theta, box, g_nobs, g_obs_centre, g_obs_radius, g_obs_J,
+                                                par[6], NULL, gR, gth);
+        for (int p = 0; p < np; ++p) rfl[p] = ppar[1];
+        if (!rc && np > 0)          /* boids flee: predators as moving disks */
+            rc = orc_flock_obstacle_energy_grad(n, pos, theta, box, np, ppos, rfl, ppar[0], par[6], NULL, gR, gth);
+        if (!rc && np > 0) {        /* predators chase, and avoid the obstacles */
+            rc = orc_predator_energy_grad(n, pos, box, np, ppos, pth, ppar[2], ppar[3], NULL, qR, qth);
+            for (int p = 0; p < np; ++p) { p3[3 * p] = ppos[2 * p]; p3[3 * p + 1] = ppos[2 * p + 1]; p3[3 * p + 2] = 0.0; }
+            if (!rc && g_nobs > 0)
+                rc = orc_flock_obstacle_energy_grad(np, p3, pth, box, g_nobs, g_obs_centre, g_obs_radius, g_obs_J,
+                                                    par[6], NULL, qR, qth);
+        }
+        for (int i = 0; i < n && !rc; ++i) {
+            const double c = cos(theta[i]), sn = sin(theta[i]);
+            pos[3 * (size_t)i] = wrap64(pos[3 * (size_t)i] + dt * (speed * c - gR[2 * i]), box[0]);
+            pos[3 * (size_t)i + 1] = wrap64(pos[3 * (size_t)i + 1] + dt * (speed * sn - gR[2 * i + 1]), box[1]);
+            theta[i] -= dt * gth[i];
+        }
+        for (int p = 0; p < np && !rc; ++p) {
+            const double c = cos(pth[p]), sn = sin(pth[p]);
+            ppos[2 * p] = wrap64(ppos[2 * p] + dt * (ppar[4] * c - qR[2 * p]), box[0]);
+            ppos[2 * p + 1] = wrap64(ppos[2 * p + 1] + dt * (ppar[4] * sn - qR[2 * p + 1]), box[1]);
+            pth[p] -= dt * qth[p];
+        }
+    }
+    free(gR); free(gth);
+    return rc;
 }
 
 /*

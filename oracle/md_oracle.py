@@ -280,6 +280,28 @@ def flock_set_obstacles(centre=(), radius=(), J=0.0):
     _check(lib().orc_flock_set_obstacles(int(c.shape[0]), _pd(c), _pd(r), C.c_double(J)), "flock_set_obstacles")
 
 
+def predator_energy_grad(pos, box, ppos, pth, J, R):
+    """The predators' chase term (eq. 13): returns (energy, gR[np,2], gtheta[np])."""
+    p = _d(pos3(pos)); b = _d(box)
+    pp = _d(np.asarray(ppos, np.float64).reshape(-1, 2)); pt = _d(pth)
+    k = pp.shape[0]
+    en = np.zeros(1); gR = np.zeros((k, 2)); gth = np.zeros(k)
+    _check(lib().orc_predator_energy_grad(p.shape[0], _pd(p), _pd(b), k, _pd(pp), _pd(pt), C.c_double(J),
+                                          C.c_double(R), _pd(en), _pd(gR), _pd(gth)), "predator_energy_grad")
+    return float(en[0]), gR, gth
+
+
+def flock_run_predators(pos, theta, box, par, speed, dt, nsteps, ppos, pth, ppar):
+    """Boids and predators together; ppar = (J_flee, R_flee, J_chase, R_chase, speed_pred).
+    Returns (pos, theta, ppos, ptheta)."""
+    p = _d(pos3(pos)).copy(); th = _d(theta).copy(); b = _d(box); pr = _d(par)
+    pp = _d(np.asarray(ppos, np.float64).reshape(-1, 2)).copy(); pt = _d(pth).copy(); pq = _d(ppar)
+    _check(lib().orc_flock_run_predators(p.shape[0], _pd(p), _pd(th), _pd(b), _pd(pr), C.c_double(speed),
+                                         C.c_double(dt), nsteps, pp.shape[0], _pd(pp), _pd(pt), _pd(pq)),
+           "flock_run_predators")
+    return p, th, pp, pt
+
+
 def flock_run(pos, theta, box, par, speed, dt, nsteps):
     p = _d(pos3(pos)).copy(); th = _d(theta).copy(); b = _d(box); pr = _d(par)
     _check(lib().orc_flock_run(p.shape[0], _pd(p), _pd(th), _pd(b), _pd(pr), C.c_double(speed), C.c_double(dt),

@@ -993,3 +993,57 @@ def test_bks_type_potential(orc):
             worst = max(worst, abs(fd - f[i, q]))
     assert worst < 1e-6 * max(1.0, np.abs(f).max()), worst
     assert np.abs(f.sum(0)).max() < 1e-10 * np.abs(f).max()                              # Newton's third law
+
+
+def test_flocking_predators(orc):
+    """Eqs. (12)-(13) (A28).  The chase term: a predator beside a clump of
+    boids has e = J/2 (1 - cos phi)^2, phi the angle between its heading and the direction of the clump's
+    centre of mass; nothing in range gives zero; gradients by central differences (clump well inside the
+    range, so the set is fixed).  Dynamics: the predator turns toward and closes in on the clump; boids
+    within R_flee of a predator end up farther from it than the same boids without predators; with no
+    predators the run is orc_flock_run."""
+    box = np.array([40.0, 40.0, 1.0])
+    rng = np.random.default_rng(4)
+    clump = np.zeros((30, 3)); clump[:, :2] = np.array([20.0, 20.0]) + rng.normal(0, 0.5, (30, 2))
+    com = clump[:, :2].mean(0)
+    ppos = np.array([[16.0, 18.5]])
+    u = (com - ppos[0]) / np.linalg.norm(com - ppos[0])
+    J, R = 3.0, 8.0
+    for th in (-2.0, 0.3, 1.9):
+        e, gR, gth = orc.predator_energy_grad(clump, box, ppos, [th], J, R)
+        cphi = np.cos(th) * u[0] + np.sin(th) * u[1]
+        assert abs(e - 0.5 * J * (1 - cphi) ** 2) < 1e-13
+    e, gR, gth = orc.predator_energy_grad(clump, box, [[2.0, 2.0]], [0.3], J, R)
+    assert e == 0.0 and not gR.any() and not gth.any()
+    th = 1.9
+    e0, gR, gth = orc.predator_energy_grad(clump, box, ppos, [th], J, R)
+    h = 1e-6
+    E = lambda pp, t: orc.predator_energy_grad(clump, box, pp, [t], J, R)[0]
+    assert abs((E(ppos, th + h) - E(ppos, th - h)) / (2 * h) - gth[0]) < 1e-8
+    for q in range(2):
+        a = ppos.copy(); a[0, q] += h; b = ppos.copy(); b[0, q] -= h
+        assert abs((E(a, th) - E(b, th)) / (2 * h) - gR[0, q]) < 1e-8
+    # two predators, one across the periodic boundary from its prey
+    far = np.zeros((5, 3)); far[:, :2] = np.array([39.0, 5.0]) + rng.normal(0, 0.3, (5, 2))
+    both = np.concatenate([clump, far])
+    e2, gR2, gth2 = orc.predator_energy_grad(both, box, [[16.0, 18.5], [1.5, 5.0]], [th, 0.0], J, R)
+    assert abs(gth2[0] - gth[0]) < 1e-14 and e2 > e0          # the second predator looks away from its prey (at -x)
+    # dynamics
+    par = (1.0, 3.0, 10.0, 1.5, 0.0, 4.0, 3.0)
+    ppar = (5.0, 4.0, 3.0, 8.0, 0.6)
+    th_b = rng.uniform(-np.pi, np.pi, 30)
+    p1, t1, pp1, pt1 = orc.flock_run_predators(clump, th_b, box, par, 0.2, 0.02, 150, ppos, [1.9], ppar)
+    d0 = np.linalg.norm(com - ppos[0]); d1 = np.linalg.norm(p1[:, :2].mean(0) - pp1[0])
+    u1 = (p1[:, :2].mean(0) - pp1[0]) / d1
+    assert np.cos(pt1[0]) * u1[0] + np.sin(pt1[0]) * u1[1] > np.cos(1.9) * u[0] + np.sin(1.9) * u[1]   # turned toward
+    assert d1 < d0                                                                                      # closed in
+    near = np.zeros((12, 3)); near[:, :2] = np.array([10.0, 30.0]) + rng.normal(0, 1.2, (12, 2))
+    th_n = rng.uniform(-np.pi, np.pi, 12)
+    hunter = np.array([[10.0, 30.0]])
+    pa, _, ppa, _ = orc.flock_run_predators(near, th_n, box, par, 0.0, 0.02, 100, hunter, [0.0], (5.0, 4.0, 0.0, 8.0, 0.0))
+    pb, _ = orc.flock_run(near, th_n, box, par, 0.0, 0.02, 100)
+    ra = np.linalg.norm(pa[:, :2] - hunter[0], axis=1).mean(); rb = np.linalg.norm(pb[:, :2] - hunter[0], axis=1).mean()
+    assert np.array_equal(ppa, hunter) and ra > rb + 0.05
+    pc, tc, _, _ = orc.flock_run_predators(near, th_n, box, par, 0.3, 0.02, 20, np.zeros((0, 2)), [], ppar)
+    pd_, td = orc.flock_run(near, th_n, box, par, 0.3, 0.02, 20)
+    assert np.array_equal(pc, pd_) and np.array_equal(tc, td)
