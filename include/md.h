@@ -287,10 +287,30 @@ typedef struct md_flock_params {
 int md_flock_obstacles(md_system *sys, int nobs, const float *centre, const float *radius, float J);
 
 /*
+ * Predators of the boids model (App. B.3.2, eqs. 12-13; reading A28): a second,
+ * small population with the same state.  Each side descends its own energy in its own coordinates:
+ *   boids add      sum_p J_flee rho(r_ip; R_flee) (1 + N_i . Rhat_ip)^2   (the obstacle energy, predator = disk)
+ *   predators use  1/2 J_chase (1 - Dhat_p . N_p)^2 + the obstacle term,  D_p = sum_{r_ip < R_chase} (R_i - R_p)
+ * and move by forward Euler at their own speed, all from the state at the start of the step.
+ *   npred  0..MD_MAX_PREDATORS (0 removes them)
+ *   pred   DEVICE float4[npred] in/out: (x, y, 0, theta_p); owned by the caller, read and written by every
+ *          md_flock_step until replaced; 16-byte aligned
+ *   par    J >= 0, R_flee and R_chase in (0, L/2), speed >= 0 (copied)
+ * The chase sum runs over all boids (one block per predator), not over the neighbor list.
+ */
+#define MD_MAX_PREDATORS 16
+typedef struct md_predator_params {
+    float J_flee, R_flee;      /* boids: eq. 12's boid-predator term */
+    float J_chase, R_chase;    /* predators: eq. 13's predator-boid term */
+    float speed;               /* predators' swimming speed */
+} md_predator_params;
+int md_flock_predators(md_system *sys, int npred, void *pred, const md_predator_params *par);
+
+/*
  * nsteps of the boids model by forward Euler (eqs. 4-5) on a 2-D system:
  *   R_i' = wrap(R_i + dt (v N(theta_i) - grad_{R_i} E));  theta_i' = theta_i - dt grad_{theta_i} E
  * with E = E_align + E_avoid + E_cohesion over the neighbor list (every range <= the list r_cut) plus the
- * obstacle term of md_flock_obstacles, both
+ * obstacle term of md_flock_obstacles and the predators of md_flock_predators, both
  * updates from the state at the start of the step; then the device-side rebuild test and rebuild.
  *   pos   float4[n] in/out: (x, y, 0, theta_i) -- the heading travels in pos.w
  *   lists, id and stats as in md_nve_step (the list must be valid for pos on entry)

@@ -23,7 +23,7 @@ SYMBOLS = [
     "md_needs_rebuild", "md_pair_energy_force", "md_nve_step", "md_nve_run_host", "md_counters",
     "md_nve_run_host_release", "md_fire_minimize", "md_brownian_step",
     "md_langevin_step", "md_nose_hoover_step", "md_set_species_lj",
-    "md_flock_step", "md_flock_obstacles", "md_set_species_bks",
+    "md_flock_step", "md_flock_obstacles", "md_set_species_bks", "md_flock_predators",
 ]
 
 
@@ -46,6 +46,11 @@ class md_fire_params(C.Structure):
 class md_flock_params(C.Structure):
     _fields_ = [("J_align", C.c_float), ("R_align", C.c_float), ("J_avoid", C.c_float), ("R_avoid", C.c_float),
                 ("J_cohesion", C.c_float), ("R_cohesion", C.c_float), ("alpha", C.c_float), ("speed", C.c_float)]
+
+
+class md_predator_params(C.Structure):
+    _fields_ = [("J_flee", C.c_float), ("R_flee", C.c_float), ("J_chase", C.c_float), ("R_chase", C.c_float),
+                ("speed", C.c_float)]
 
 
 class MdError(RuntimeError):
@@ -84,6 +89,7 @@ def lib():
         L.md_nose_hoover_step.argtypes = [vp, C.POINTER(md_potential), vp, vp, vp, ip, ip, ip, C.c_float,
                                           C.c_float, C.c_float, C.c_float, vp, C.c_int, ip, vp]
         L.md_set_species_bks.argtypes = [vp, C.c_int] + [C.POINTER(C.c_float)] * 4 + [C.c_float, C.c_float]
+        L.md_flock_predators.argtypes = [vp, C.c_int, vp, C.POINTER(md_predator_params)]
         L.md_flock_obstacles.argtypes = [vp, C.c_int, C.POINTER(C.c_float), C.POINTER(C.c_float), C.c_float]
         L.md_flock_step.argtypes = [vp, C.POINTER(md_flock_params), vp, ip, ip, ip, C.c_float, C.c_int, ip, vp]
         L.md_fire_minimize.argtypes = [vp, C.POINTER(md_potential), C.POINTER(md_fire_params), vp, vp, vp,
@@ -195,6 +201,14 @@ def md_flock_obstacles(sys, centre=(), radius=(), J=0.0) -> None:
         raise ValueError("one radius per centre")
     fp = C.POINTER(C.c_float)
     _check(lib().md_flock_obstacles(sys, int(r.shape[0]), c.ctypes.data_as(fp), r.ctypes.data_as(fp), float(J)))
+
+
+def md_flock_predators(sys, pred=None, par: md_predator_params | None = None) -> None:
+    """pred: device float32[npred, 4] tensor (x, y, 0, theta), kept by pointer; None removes the predators."""
+    if pred is None:
+        _check(lib().md_flock_predators(sys, 0, None, None))
+    else:
+        _check(lib().md_flock_predators(sys, int(pred.shape[0]), _ptr(pred), C.byref(par)))
 
 
 def md_flock_step(sys, par: md_flock_params, pos, id, nbr_idx, nbr_count, dt, nsteps, stats, stream=None) -> None:

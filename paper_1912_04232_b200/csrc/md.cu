@@ -68,6 +68,9 @@ struct RuleArgs {
     md_flock_params flock;
     int nobs;                       // md_flock_obstacles: disks (x, y, radius) and J
     float obs[3 * MD_MAX_OBSTACLES], J_obs;
+    int npred;                      // md_flock_predators
+    void *pred;
+    md_predator_params ppar;
     int fast32, builder, nb_parts, remap;
     float est_thr;
 };
@@ -110,6 +113,9 @@ struct md_system {
     float bks_A[16], bks_B[16], bks_C[16], bks_q[4], bks_alpha, bks_ke;
     int nobs;            // md_flock_obstacles
     float obs[3 * MD_MAX_OBSTACLES], J_obs;
+    int npred;           // md_flock_predators: count, DEVICE state (caller's), parameters
+    void *pred;
+    md_predator_params ppar;
     int builder;         // neighbor-list builder: 2 = bit-mask (md_nbr2.cuh), 1 = column append
     int fast32;          // LJ 3-D: fp32 fast path + fp64 re-evaluation (md_force32.cuh)
     float est_thr;       // its error-estimate threshold
@@ -616,6 +622,8 @@ int record_rule_step(md_system *s, const Pair &pp, const RuleArgs &A, cudaStream
                        A.flock.J_cohesion, A.flock.R_cohesion, A.flock.alpha, A.flock.speed};
         fq.nobs = A.nobs; fq.Job = A.J_obs;
         for (int o = 0; o < A.nobs; ++o) { fq.ox[o] = A.obs[3 * o]; fq.oy[o] = A.obs[3 * o + 1]; fq.oD[o] = A.obs[3 * o + 2]; }
+        fq.npred = A.npred; fq.pred = (const float4 *)A.pred;
+        fq.Jfl = A.ppar.J_flee; fq.Rfl = A.ppar.R_flee; fq.Jch = A.ppar.J_chase; fq.Rch = A.ppar.R_chase; fq.vpred = A.ppar.speed;
         const int nbp = blocks_for(g.n, 128);
         double2 *cs = reinterpret_cast<double2 *>(s->pos_s);       // free between rebuilds
         k_flock_trig<<<nb, 256, 0, st>>>(g.n, p4, cs);
@@ -629,6 +637,16 @@ int record_rule_step(md_system *s, const Pair &pp, const RuleArgs &A, cudaStream
         else FLOCK_PASS1(0);
 #undef FLOCK_PASS1
         k_flock_pass2<<<nbp, 128, 0, st>>>(g, fq, p4, A.nbr_idx, A.nbr_count, s->vel_s, s->pos_alt);
+        if (A.npred > 0) {
+#define FLOCK_PRED(AI) k_flock_predators<AI><<<A.npred, 256, 0, st>>>(g, fq, p4, (float4 *)A.pred, A.dt)
+            if ((float)ai != A.flock.alpha) FLOCK_PRED(0);
+            else if (ai == 1) FLOCK_PRED(1);
+            else if (ai == 2) FLOCK_PRED(2);
+            else if (ai == 3) FLOCK_PRED(3);
+            else if (ai == 4) FLOCK_PRED(4);
+            else FLOCK_PRED(0);
+#undef FLOCK_PRED
+        }
         k_flock_update<<<nb, 256, 0, st>>>(g, fq, p4, s->vel_s, s->ref_pos, A.dt, rs);
         break;
     }
@@ -1079,6 +1097,21 @@ int md_flock_obstacles(md_system *sys, int nobs, const float *centre, const floa
     return MD_OK;
 }
 
+int md_flock_predators(md_system *sys, int npred, void *pred, const md_predator_params *par) {
+    if (!sys) return fail(MD_EINVAL, "NULL argument");
+    if (npred < 0 || npred > MD_MAX_PREDATORS) return fail(MD_EINVAL, "npred = %d must be in 0..%d", npred, MD_MAX_PREDATORS);
+    if (npred == 0) { sys->npred = 0; sys->pred = nullptr; memset(&sys->ppar, 0, sizeof(sys->ppar)); return MD_OK; }
+    if (!pred || !par) return fail(MD_EINVAL, "NULL argument");
+    if (!aligned16(pred)) return fail(MD_EINVAL, "pred must be 16-byte aligned");
+    if (!(par->J_flee >= 0.0f) || !(par->R_flee > 0.0f) || !(par->J_chase >= 0.0f) || !(par->R_chase > 0.0f) ||
+        !(par->speed >= 0.0f))
+        return fail(MD_EINVAL, "predator parameters out of range");
+    if (2.0f * std::max(par->R_flee, par->R_chase) >= std::min(sys->g.L[0], sys->g.L[1]))
+        return fail(MD_EINVAL, "R_flee and R_chase must be below half the box");
+    sys->npred = npred; sys->pred = pred; sys->ppar = *par;
+    return MD_OK;
+}
+
 int md_flock_step(md_system *sys, const md_flock_params *par, void *pos, int32_t *id, int32_t *nbr_idx,
                   int32_t *nbr_count, float dt, int nsteps, int32_t *stats, void *stream) {
     if (!sys || !par || !pos || !nbr_idx || !nbr_count || !stats) return fail(MD_EINVAL, "NULL argument");
@@ -1098,6 +1131,9 @@ int md_flock_step(md_system *sys, const md_flock_params *par, void *pos, int32_t
     A.dt = dt; A.mass = 1.0f; A.flock = *par;
     A.nobs = sys->nobs; A.J_obs = sys->J_obs;
     memcpy(A.obs, sys->obs, sizeof(float) * 3 * (size_t)sys->nobs);
+    A.npred = sys->npred; A.pred = sys->pred; A.ppar = sys->ppar;
+    if (sys->npred > 0 && std::max(sys->ppar.R_flee, 0.0f) * 2.0f >= std::min(sys->g.L[0], sys->g.L[1]))
+        return fail(MD_EINVAL, "R_flee %g must be below half the box", sys->ppar.R_flee);
     return run_rule(sys, pp, A, nsteps, (cudaStream_t)stream);
 }
 

@@ -21,6 +21,9 @@ struct FlockPar {
     int nobs;                                   // obstacles (App. B.3.1): centres, radii, J
     double Job;
     float ox[MD_MAX_OBSTACLES], oy[MD_MAX_OBSTACLES], oD[MD_MAX_OBSTACLES];
+    int npred;                                  // predators (App. B.3.2): device state (x, y, 0, theta)
+    const float4 *pred;
+    double Jfl, Rfl, Jch, Rch, vpred;
 };
 
 __device__ __forceinline__ void flock_disp(const Geom &g, const float4 &pi, const float4 &q, double &dx, double &dy) {
@@ -40,6 +43,25 @@ __device__ __forceinline__ double flock_pow(double x, double a) {
 #pragma unroll
     for (int k = 0; k < n; ++k) y *= x;
     return y;
+}
+
+// The disk term of eq. 11 for one boid (or predator) at pi heading (ci, si) and one disk (centre, radius D):
+// e = J rho(r; D)(1 + N.u)^2, u = (C - R)/r, inside the disk only; adds its gradients.
+template <int AI>
+__device__ __forceinline__ void flock_disk_term(const Geom &g, const FlockPar &fp, const float4 &pi, double ci,
+                                                double si, float cx, float cy, double D, double J,
+                                                double &gx, double &gy, double &gt) {
+    double dx, dy;
+    flock_disp(g, pi, make_float4(cx, cy, 0.0f, 0.0f), dx, dy);                      // R - C
+    const double r = sqrt(dx * dx + dy * dy);
+    if (r < D && r > 0.0) {
+        const double ux = -dx / r, uy = -dy / r, c = ci * ux + si * uy, x = 1.0 - r / D;
+        const double rho = flock_pow<AI, false>(x, fp.alpha) / fp.alpha;
+        const double drho = -flock_pow<AI, true>(x, fp.alpha) / D;
+        gt += 2.0 * J * rho * (1.0 + c) * (-si * ux + ci * uy);
+        gx += -J * (drho * (1.0 + c) * (1.0 + c) * ux + 2.0 * rho * (1.0 + c) * (ci - c * ux) / r);
+        gy += -J * (drho * (1.0 + c) * (1.0 + c) * uy + 2.0 * rho * (1.0 + c) * (si - c * uy) / r);
+    }
 }
 
 // (cos theta_i, sin theta_i) in fp64, once per boid and step: pass 1 forms the sine and cosine of
@@ -107,19 +129,12 @@ k_flock_pass1(Geom g, FlockPar fp, const float4 *__restrict__ pos, const double2
         gt += -fp.Jco * (1.0 - c) * (-hx * si + hy * ci);
         gx -= m * Gx; gy -= m * Gy;
     }
-    // obstacles, eq. 11: e = J rho(r; D_o)(1 + N.u)^2, u = (C_o - R_i)/r, inside the disk only
-    for (int o = 0; o < fp.nobs; ++o) {
-        double dx, dy;
-        flock_disp(g, pi, make_float4(fp.ox[o], fp.oy[o], 0.0f, 0.0f), dx, dy);      // R_i - C_o
-        const double r = sqrt(dx * dx + dy * dy), D = (double)fp.oD[o];
-        if (r < D && r > 0.0) {
-            const double ux = -dx / r, uy = -dy / r, c = ci * ux + si * uy, x = 1.0 - r / D;
-            const double rho = flock_pow<AI, false>(x, fp.alpha) / fp.alpha;
-            const double drho = -flock_pow<AI, true>(x, fp.alpha) / D;
-            gt += 2.0 * fp.Job * rho * (1.0 + c) * (-si * ux + ci * uy);
-            gx += -fp.Job * (drho * (1.0 + c) * (1.0 + c) * ux + 2.0 * rho * (1.0 + c) * (ci - c * ux) / r);
-            gy += -fp.Job * (drho * (1.0 + c) * (1.0 + c) * uy + 2.0 * rho * (1.0 + c) * (si - c * uy) / r);
-        }
+    // obstacles (eq. 11), then the predators as moving disks of radius R_flee (eq. 12)
+    for (int o = 0; o < fp.nobs; ++o)
+        flock_disk_term<AI>(g, fp, pi, ci, si, fp.ox[o], fp.oy[o], (double)fp.oD[o], fp.Job, gx, gy, gt);
+    for (int p = 0; p < fp.npred; ++p) {
+        const float4 q = fp.pred[p];
+        flock_disk_term<AI>(g, fp, pi, ci, si, q.x, q.y, fp.Rfl, fp.Jfl, gx, gy, gt);
     }
     acc[i] = make_float4((float)gx, (float)gy, (float)gt, (float)m);
     gco[i] = make_float4((float)Gx, (float)Gy, 0.0f, 0.0f);
@@ -152,6 +167,55 @@ k_flock_pass2(Geom g, FlockPar fp, const float4 *__restrict__ pos, const int *__
     float4 a = acc[i];
     a.x = (float)((double)a.x + gx); a.y = (float)((double)a.y + gy);
     acc[i] = a;
+}
+
+// Predators (eq. 13): block p sums D_p = sum over boids within R_chase of (R_i - R_p) in a fixed order,
+// then one thread takes the chase gradient, adds the obstacles, and moves the predator by forward Euler.
+// Runs after the boids' passes (which read the old predator state) and before the boids' update (this
+// kernel reads the old boid positions).
+template <int AI>
+__global__ void __launch_bounds__(256)
+k_flock_predators(Geom g, FlockPar fp, const float4 *__restrict__ pos, float4 *pred, float dt) {
+    __shared__ double sx[8], sy[8];
+    __shared__ int sm[8];
+    const int p = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const float4 q = pred[p];
+    const double R2 = fp.Rch * fp.Rch;
+    double Dx = 0.0, Dy = 0.0;
+    int m = 0;
+    for (int i = threadIdx.x; i < g.n; i += 256) {
+        double dx, dy;
+        flock_disp(g, pos[i], q, dx, dy);                                            // R_i - R_p
+        if (dx * dx + dy * dy < R2) { Dx += dx; Dy += dy; ++m; }
+    }
+    for (int o = 16; o > 0; o >>= 1) {
+        Dx += __shfl_xor_sync(FULL, Dx, o); Dy += __shfl_xor_sync(FULL, Dy, o); m += __shfl_xor_sync(FULL, m, o);
+    }
+    if (lane == 0) { sx[warp] = Dx; sy[warp] = Dy; sm[warp] = m; }
+    __syncthreads();
+    if (threadIdx.x != 0) return;
+    Dx = Dy = 0.0; m = 0;
+    for (int w = 0; w < 8; ++w) { Dx += sx[w]; Dy += sy[w]; m += sm[w]; }
+    double sn, cp;
+    sincos((double)q.w, &sn, &cp);
+    double gx = 0.0, gy = 0.0, gt = 0.0;
+    const double Dn = sqrt(Dx * Dx + Dy * Dy);
+    if (m > 0 && Dn > 0.0) {
+        const double hx = Dx / Dn, hy = Dy / Dn, c = hx * cp + hy * sn;
+        gt = -fp.Jch * (1.0 - c) * (-hx * sn + hy * cp);
+        gx = m * fp.Jch * (1.0 - c) * (cp - c * hx) / Dn;
+        gy = m * fp.Jch * (1.0 - c) * (sn - c * hy) / Dn;
+    }
+    for (int o = 0; o < fp.nobs; ++o)
+        flock_disk_term<AI>(g, fp, q, cp, sn, fp.ox[o], fp.oy[o], (double)fp.oD[o], fp.Job, gx, gy, gt);
+    float4 out = q;
+    const float v = (float)fp.vpred, ax = (float)gx, ay = (float)gy, at = (float)gt;
+    float snf, csf;
+    sincosf(q.w, &snf, &csf);
+    out.x = wrap(fmaf(dt, fmaf(v, csf, -ax), q.x), g.L[0], g.inv_L[0]);
+    out.y = wrap(fmaf(dt, fmaf(v, snf, -ay), q.y), g.L[1], g.inv_L[1]);
+    out.w = fmaf(-dt, at, q.w);
+    pred[p] = out;
 }
 
 // forward Euler (eqs. 4-5), half-skin test

@@ -683,6 +683,62 @@ def test_flocking_against_the_oracle(B, orc, W):
         B.md_flock_obstacles(S.sys, [[1.0, 1.0]], [30.0], 1.0)          # radius above half the box
     S.close()
 
+    # (e) predators (App. B.3.2, eqs. 12-13) with obstacles.  One step of both populations on the uniform
+    #     flock against the oracle's gradients; then 60 steps on four separated clumps of 64 boids with a
+    #     predator beside each -- like eq. 10, the chase term is singular where the prey surrounds the
+    #     predator evenly (|D_p| -> 0: in the uniform flock fp32 and fp64 runs part within 5 steps), so the
+    #     trajectory is compared where |D_p| is bounded below.
+    def run_both(wk, p0, t0, bx, Lb, pp0, pt0, ppar, cen, rad, steps, tol):
+        S = B.System(wk)
+        pred0 = np.zeros((len(pt0), 4), np.float32); pred0[:, :2] = pp0; pred0[:, 3] = pt0
+        pred = torch.from_numpy(pred0).cuda()
+        B.md_flock_obstacles(S.sys, cen, rad, Jo)
+        B.md_flock_predators(S.sys, pred, B.md_predator_params(*ppar))
+        S.build()
+        B.md_flock_step(S.sys, B.md_flock_params(*par, speed), S.pos, S.id, S.nbr_idx, S.nbr_count, dt, steps, S.stats)
+        torch.cuda.synchronize()
+        orc.flock_set_obstacles(cen, rad, Jo)
+        try:
+            p_o, th_o, pp_o, pt_o = orc.flock_run_predators(p0, t0, bx, par, speed, dt, steps, pp0, pt0, ppar)
+        finally:
+            orc.flock_set_obstacles()
+        got = unpermute(S, S.pos)
+        d = got[:, :2].astype(np.float64) - p_o[:, :2]
+        d -= Lb * np.round(d / Lb)
+        assert np.abs(d).max() <= tol, (steps, np.abs(d).max())
+        assert np.abs(got[:, 3].astype(np.float64) - th_o).max() <= tol
+        gp = pred.cpu().numpy()
+        dp = gp[:, :2].astype(np.float64) - pp_o
+        dp -= Lb * np.round(dp / Lb)
+        assert np.abs(dp).max() <= tol, (steps, np.abs(dp).max())
+        assert np.abs(gp[:, 3].astype(np.float64) - pt_o).max() <= tol
+        B.md_flock_predators(S.sys)                                      # removable
+        S.close()
+        return pp_o, pt_o
+
+    par = (1.0, 3.0, 10.0, 1.5, 0.0, 4.0, 3.0)
+    pp0 = np.array([[5.3, 6.1], [20.7, 21.9], [39.6, 12.2], [30.2, 33.3]], np.float32)
+    pt0 = np.array([0.4, -2.1, 3.0, 1.2], np.float32)
+    ppar = (5.0, 4.0, 3.0, 6.0, 0.8)
+    run_both(w, pos, th0, box32, L, pp0, pt0, ppar, cen_o, rad_o, 1, 4e-6)
+    _, gq, _ = orc.predator_energy_grad(pos, box32, pp0, pt0, ppar[2], ppar[3])
+    e_f, _, _ = orc.flock_obstacle_energy_grad(pos, th0, box32, pp0, [ppar[1]] * 4, ppar[0], 3.0)
+    assert np.abs(gq).max() > 0 and e_f > 0                # predators felt their prey, boids their predators
+    Lc = 60.3
+    boxc = np.array([Lc, Lc, 1.0], np.float32)
+    cents = np.array([[15.0, 15.0], [45.0, 15.0], [15.0, 45.0], [45.0, 45.0]])
+    g8 = (np.arange(8) - 3.5) * 1.0
+    cl = np.stack(np.meshgrid(g8, g8, indexing="ij"), -1).reshape(-1, 2)
+    pc = np.zeros((256, 4), np.float32)
+    pc[:, :2] = (cents[:, None, :] + cl[None, :, :] + rng.normal(0, 0.12, (4, 64, 2))).reshape(-1, 2)
+    pc[:, 3] = rng.uniform(-np.pi, np.pi, 256).astype(np.float32)
+    ppc = (cents + np.array([[-6.0, 0.5], [0.4, 6.0], [6.0, -0.3], [-4.5, -4.5]])).astype(np.float32)
+    ptc = np.array([2.0, 0.3, -1.0, 2.5], np.float32)
+    wc = custom_workload(W, pc, boxc, 2, 1, 4.0, 0.5, 64)
+    pp_o, pt_o = run_both(wc, pc, pc[:, 3].astype(np.float64), boxc, Lc, ppc, ptc, (5.0, 4.0, 3.0, 14.0, 0.8),
+                          np.array([[18.5, 17.0], [45.0, 50.5]], np.float32), np.array([3.0, 4.0], np.float32), 60, 1e-4)
+    assert np.abs(pp_o - ppc).max() > 0.5 and np.abs(pt_o - ptc).max() > 1.0     # they did turn and travel
+
 
 def test_fast32_dimers_at_the_force_zero(B, orc, W):
     """Isolated pairs around r = 2^(1/6) sigma, where the LJ force changes sign: the coefficient and
