@@ -1089,3 +1089,11 @@ def test_full_size_configs(B, orc, W, ci, steps):
     torch.cuda.empty_cache()
     rebuilds = snapshot_checks(B, orc, W, w, steps)
     assert rebuilds >= 3
+
+
+def test_config3_long_run(B, orc, W):
+    """2000 MD steps of config 3 (twice the config's own run, ~260 rebuilds) through the fused graph:
+    energy and momentum conserved, the list in use still complete, and force / energy / a fresh list
+    of the final state against the oracle."""
+    rebuilds = snapshot_checks(B, orc, W, W.config(3), 2000)
+    assert rebuilds >= 200
