@@ -25,7 +25,7 @@
  *   orc_fire_run        L100 "Fire Descent [68]", used at L322 (Bitzek et al.'s algorithm)
  *   orc_brownian_run    L100 "Brownian" (Euler-Maruyama; kT = 0: "Gradient Descent")
  *   orc_langevin_run    L100 "Langevin" (BAOAB splitting)
- *   orc_nose_hoover_run L100 "Nose-Hoover [67]" (one thermostat, MTK splitting)
+ *   orc_nose_hoover_run L100 "Nose-Hoover [67]" (chains of 1..8 thermostats, MTK splitting)
  *   orc_normals         the counter-based normal generator both sides implement
  *   orc_flock_*         App. B: boids energies eqs. 3-10, forward Euler eqs. 4-5;
  *                       obstacles eq. 11 (L411-L418), predators eqs. 12-13 (L420-L438)
@@ -905,21 +905,51 @@ int orc_langevin_run(int n, int dim, double *pos, double *vel, double *force, co
  * Conserved: H' = K + U + Q vxi^2 / 2 + dof kT xi.
  *   state in/out double[2] = {xi, vxi};  conserved out (may be NULL) double[nsteps+1] = H'
  */
-static void nh_half(int n, int dim, double *vel, double mass, double dofkT, double Q, double dt,
-                    double *xi, double *vxi)
+/* Chain length M (Martyna, Klein and Tuckerman's chains [67]; 1 = the single thermostat above).
+ * Masses Q_1 = dof kT tau^2, Q_j = kT tau^2 (j >= 2).  Thermostat half step T(dt), d = dt/2:
+ *   G_1 = (K2 - dof kT)/Q_1,  G_j = (Q_{j-1} v_{j-1}^2 - kT)/Q_j
+ *   v_M += d/2 G_M;  for j = M-1 .. 1:  a = exp(-d/4 v_{j+1}),  v_j = (v_j a + d/2 G_j) a
+ *   s = exp(-d v_1);  v *= s;  K2 *= s^2;  xi_j += d v_j (all j)
+ *   for j = 1 .. M-1:  a = exp(-d/4 v_{j+1}),  v_j = (v_j a + d/2 G_j) a  (G_j from the updated
+ *   v_{j-1}, K2);  v_M += d/2 G_M
+ * Conserved: H' = K + U + sum_j Q_j v_j^2 / 2 + dof kT xi_1 + kT sum_{j>=2} xi_j.
+ * state = {xi_1..xi_M, v_1..v_M}. */
+#define ORC_MAX_NH_CHAIN 8
+static int g_nh_chain = 1;
+int orc_set_nh_chain(int M)
+{
+    if (M < 1 || M > ORC_MAX_NH_CHAIN) return ORC_EINVAL;
+    g_nh_chain = M;
+    return ORC_OK;
+}
+
+static double nh_G(int j, int M, double K2, double dofkT, double kT, const double *Q, const double *v)
+{
+    (void)M;
+    return j == 0 ? (K2 - dofkT) / Q[0] : (Q[j - 1] * v[j - 1] * v[j - 1] - kT) / Q[j];
+}
+
+static void nh_half(int n, int dim, double *vel, double mass, double dofkT, double kT, const double *Q, int M,
+                    double dt, double *xi, double *v)
 {
     double K2 = 0.0;
     for (int i = 0; i < n; ++i)
         for (int q = 0; q < dim; ++q) K2 += mass * vel[3 * (size_t)i + q] * vel[3 * (size_t)i + q];
-    double G = (K2 - dofkT) / Q;
-    *vxi += 0.25 * dt * G;
-    double sc = exp(-0.5 * dt * *vxi);
+    v[M - 1] += 0.25 * dt * nh_G(M - 1, M, K2, dofkT, kT, Q, v);
+    for (int j = M - 2; j >= 0; --j) {
+        double a = exp(-0.125 * dt * v[j + 1]);
+        v[j] = (v[j] * a + 0.25 * dt * nh_G(j, M, K2, dofkT, kT, Q, v)) * a;
+    }
+    double sc = exp(-0.5 * dt * v[0]);
     for (int i = 0; i < n; ++i)
         for (int q = 0; q < dim; ++q) vel[3 * (size_t)i + q] *= sc;
-    *xi += 0.5 * dt * *vxi;
+    for (int j = 0; j < M; ++j) xi[j] += 0.5 * dt * v[j];
     K2 *= sc * sc;
-    G = (K2 - dofkT) / Q;
-    *vxi += 0.25 * dt * G;
+    for (int j = 0; j < M - 1; ++j) {
+        double a = exp(-0.125 * dt * v[j + 1]);
+        v[j] = (v[j] * a + 0.25 * dt * nh_G(j, M, K2, dofkT, kT, Q, v)) * a;
+    }
+    v[M - 1] += 0.25 * dt * nh_G(M - 1, M, K2, dofkT, kT, Q, v);
 }
 
 int orc_nose_hoover_run(int n, int dim, double *pos, double *vel, double *force, const double *diam,
@@ -931,18 +961,22 @@ int orc_nose_hoover_run(int n, int dim, double *pos, double *vel, double *force,
         return ORC_EINVAL;
     double *e_i = (double *)malloc((size_t)n * sizeof(double));
     if (!e_i) return ORC_ENOMEM;
-    const double dofkT = (double)dim * n * kT, Q = dofkT * tau * tau, a = dt / (2.0 * mass);
-    double xi = state[0], vxi = state[1], E = 0.0;
+    const double dofkT = (double)dim * n * kT, a = dt / (2.0 * mass);
+    const int M = g_nh_chain;
+    double Q[ORC_MAX_NH_CHAIN], xi[ORC_MAX_NH_CHAIN], vxi[ORC_MAX_NH_CHAIN], E = 0.0;
+    for (int j = 0; j < M; ++j) { Q[j] = (j == 0 ? dofkT : kT) * tau * tau; xi[j] = state[j]; vxi[j] = state[M + j]; }
     int rc = orc_energy_force(n, dim, pos, diam, box, kind, eps, sigma, r_cut, shift, NULL, NULL, 0, force, e_i, &E);
     for (int s = 0; s <= nsteps && !rc; ++s) {
         if (conserved) {
             double K2 = 0.0;
             for (int i = 0; i < n; ++i)
                 for (int q = 0; q < dim; ++q) K2 += mass * vel[3 * (size_t)i + q] * vel[3 * (size_t)i + q];
-            conserved[s] = 0.5 * K2 + E + 0.5 * Q * vxi * vxi + dofkT * xi;
+            double H = 0.5 * K2 + E + dofkT * xi[0];
+            for (int j = 0; j < M; ++j) H += 0.5 * Q[j] * vxi[j] * vxi[j] + (j > 0 ? kT * xi[j] : 0.0);
+            conserved[s] = H;
         }
         if (s == nsteps) break;
-        nh_half(n, dim, vel, mass, dofkT, Q, dt, &xi, &vxi);
+        nh_half(n, dim, vel, mass, dofkT, kT, Q, M, dt, xi, vxi);
         for (int i = 0; i < n; ++i)
             for (int q = 0; q < dim; ++q) {
                 size_t t = 3 * (size_t)i + q;
@@ -952,9 +986,9 @@ int orc_nose_hoover_run(int n, int dim, double *pos, double *vel, double *force,
         rc = orc_energy_force(n, dim, pos, diam, box, kind, eps, sigma, r_cut, shift, NULL, NULL, 0, force, e_i, &E);
         for (int i = 0; i < n; ++i)
             for (int q = 0; q < dim; ++q) vel[3 * (size_t)i + q] += a * force[3 * (size_t)i + q];
-        nh_half(n, dim, vel, mass, dofkT, Q, dt, &xi, &vxi);
+        nh_half(n, dim, vel, mass, dofkT, kT, Q, M, dt, xi, vxi);
     }
-    state[0] = xi; state[1] = vxi;
+    for (int j = 0; j < M; ++j) { state[j] = xi[j]; state[M + j] = vxi[j]; }
     free(e_i);
     return rc;
 }

@@ -238,13 +238,15 @@ def langevin_run(pos, vel, force, diam, box, dim, kind, eps, sigma, r_cut, shift
 
 
 def nose_hoover_run(pos, vel, diam, box, dim, kind, eps, sigma, r_cut, shift, dt, mass, kT, tau, nsteps,
-                    state=None):
-    """Returns (pos, vel, force, conserved[nsteps+1], state[2] = (xi, v_xi))."""
+                    state=None, chain=1):
+    """Returns (pos, vel, force, conserved[nsteps+1], state[2*chain] = (xi_1.., v_xi_1..))."""
     p = _d(pos3(pos)).copy(); v = _d(pos3(vel)).copy(); f = np.zeros_like(p)
     b = _d(box)
     dm = _d(diam) if diam is not None else None
-    st = (_d(state) if state is not None else np.zeros(2, dtype=np.float64)).copy()
+    st = (_d(state) if state is not None else np.zeros(2 * chain, dtype=np.float64)).copy()
+    assert st.shape == (2 * chain,)
     cons = np.zeros(nsteps + 1, dtype=np.float64)
+    _check(lib().orc_set_nh_chain(int(chain)), "set_nh_chain")
     _check(lib().orc_nose_hoover_run(p.shape[0], dim, _pd(p), _pd(v), _pd(f), _pd(dm), _pd(b), kind,
                                      C.c_double(eps), C.c_double(sigma), C.c_double(r_cut), shift,
                                      C.c_double(dt), C.c_double(mass), C.c_double(kT), C.c_double(tau),

@@ -698,6 +698,59 @@ def test_nose_hoover_conserved_quantity_and_temperature(orc, W):
     assert abs(np.mean(temps[20:]) - kT) < 0.1 * kT
 
 
+def test_nose_hoover_chain(orc, W):
+    """Chains of thermostats ([67] is Martyna, Klein and Tuckerman's chain paper).
+    (a) H' = K + U + sum Q_j v_j^2/2 + dof kT xi_1 + kT sum_{j>=2} xi_j is conserved to second order
+        in dt for M = 3 (halving dt cuts the excursion ~4x) -- a wrong mass, sign or coupling in any
+        link shows up here;
+    (b) the splitting is symmetric: run forward, flip the signs of all velocities (particles' and
+        thermostats'), run the same number of steps: the start comes back;
+    (c) the second link moves as its equation says: starting from rest, after one small step
+        v_2 ~ dt (Q_1 v_1^2 - kT)/Q_2 with v_1 ~ dt (2K - dof kT)/Q_1;
+    (d) M = 1 through the chain code is the single thermostat (first two pins above still hold), and
+        the far end of a long chain started at rest stays nearly at rest over a short run;
+    (e) the temperature is driven to kT with M = 3 as well."""
+    w = W.lj_fcc(0, 3, seed=8)
+    kT, tau, M = 0.4, 0.1, 3
+    run = lambda pos, vel, dt, steps, state=None, chain=M: orc.nose_hoover_run(
+        pos, vel, None, w.box, 3, LJ, 1.0, 1.0, 2.5, 1, dt, 1.0, kT, tau, steps, state=state, chain=chain)
+    out = {}
+    for dt, steps in ((0.004, 300), (0.002, 600)):
+        p, v, f, cons, st = run(w.pos, w.vel, dt, steps)
+        out[dt] = np.abs(cons - cons[0]).max()
+        assert np.abs(st[M:]).max() > 1e-3 and np.abs(st[1:M]).max() > 1e-6        # every link moved
+    assert out[0.004] < 2e-3 * abs(cons[0]) + 0.05
+    assert 2.5 < out[0.004] / out[0.002] < 6.0, out
+    # (b)
+    p, v, f, cons, st = run(w.pos, w.vel, 0.004, 60)
+    st_back = st.copy(); st_back[M:] *= -1
+    p2, v2, f2, cons2, st2 = run(p, -v, 0.004, 60, state=st_back)
+    d = p2 - w.pos[:, :3].astype(np.float64); d -= w.box * np.round(d / w.box)
+    assert np.abs(d).max() < 1e-9 and np.abs(v2 + w.vel[:, :3]).max() < 1e-9
+    assert np.abs(st2[:M]).max() < 1e-7 and np.abs(st2[M:]).max() < 1e-7      # rounding, amplified by the small Q_j
+    # (c)
+    dt = 1e-5
+    p, v, f, cons, st = run(w.pos, w.vel, dt, 1)
+    dof = 3 * w.n
+    K2 = (w.vel[:, :3].astype(np.float64) ** 2).sum()
+    Q1, Q2 = dof * kT * tau ** 2, kT * tau ** 2
+    v1 = dt * (K2 - dof * kT) / Q1
+    assert abs(st[M] - v1) < 1e-3 * abs(v1)
+    # v_2' = (Q_1 v_1(t)^2 - kT)/Q_2 with v_1(t) ~ v1 t/dt: v_2(dt) = dt (Q_1 v1^2/3 - kT)/Q_2 to leading order
+    assert abs(st[M + 1] - dt * (Q1 * v1 ** 2 / 3 - kT) / Q2) < 2e-2 * abs(dt * kT / Q2)
+    # (d)
+    a = run(w.pos, w.vel, 0.004, 25, chain=1)
+    b = orc.nose_hoover_run(w.pos, w.vel, None, w.box, 3, LJ, 1.0, 1.0, 2.5, 1, 0.004, 1.0, kT, tau, 25)
+    assert np.array_equal(a[0], b[0]) and np.array_equal(a[4], b[4])
+    # (e)
+    state, pos, vel, temps = None, w.pos, w.vel, []
+    for chunk in range(40):
+        p, v, f, cons, state = run(pos, vel, 0.004, 25, state=state)
+        temps.append((v ** 2).sum() / (3 * w.n))
+        pos, vel = p, v
+    assert abs(np.mean(temps[20:]) - kT) < 0.1 * kT
+
+
 # ------------------------------------------------- Buckingham (SURVEY 8f-f2) --
 
 def test_buckingham_two_body_and_gradient(orc, W):
