@@ -106,7 +106,8 @@ int md_destroy(md_system *sys);
  *                          65,536 particles, else 1
  *   "builder"              neighbor-list kernel: 2 (default) records hits in per-lane bit masks,
  *                          1 appends them to per-lane shared-memory columns (first design)
- *   "use_graph"            0: md_nve_step launches kernels directly instead of a CUDA graph */
+ *   "use_graph"            0: md_nve_step launches kernels directly instead of a CUDA graph
+ *   "nh_chain"             thermostats in md_nose_hoover_step's chain, 1 (default) .. 8 */
 int md_set_option(md_system *sys, const char *name, double value);
 
 /* Species x species Lennard-Jones tables (L104 pair potentials with per-species parameters; the
@@ -250,13 +251,15 @@ int md_langevin_step(md_system *sys, const md_potential *pot, void *pos, void *v
                      void *stream);
 
 /*
- * nsteps of NVT by one Nose-Hoover thermostat (L100 [67]) around the velocity-Verlet
- * step, Martyna-Tuckerman-Tobias-Klein splitting; dof = dim n, Q = dof kT tau^2:
+ * nsteps of NVT by a Nose-Hoover chain of M thermostats (L100 [67] Martyna, Klein and
+ * Tuckerman's chains; M = option "nh_chain", default 1) around the velocity-Verlet step, explicit reversible
+ * splitting; dof = dim n, Q_1 = dof kT tau^2, Q_j = kT tau^2 (j >= 2):
  *   T(dt);  v += dt/(2m) F;  r = wrap(r + dt v);  [rebuild];  F = F(r);  v += dt/(2m) F;  T(dt)
- *   T(dt): K2 = sum m v^2; G = (K2 - dof kT)/Q; vxi += dt/4 G; v *= exp(-dt/2 vxi); xi += dt/2 vxi;
- *          K2 *= exp(-dt vxi); G = (K2 - dof kT)/Q; vxi += dt/4 G
- *   nh_state  device double[2] in/out = {xi, vxi} (zero to start); H' = K + U + Q vxi^2/2 + dof kT xi
- *             is the conserved quantity
+ *   T(dt), d = dt/2: K2 = sum m v^2; G_1 = (K2 - dof kT)/Q_1, G_j = (Q_{j-1} v_{j-1}^2 - kT)/Q_j;
+ *          v_M += d/2 G_M; for j = M-1..1: a = exp(-d/4 v_{j+1}), v_j = (v_j a + d/2 G_j) a;
+ *          v *= exp(-d v_1); K2 *= exp(-2d v_1); xi_j += d v_j; then j = 1..M-1 likewise and v_M += d/2 G_M
+ *   nh_state  device double[2M] in/out = {xi_1..xi_M, v_1..v_M} (zero to start);
+ *             H' = K + U + sum_j Q_j v_j^2/2 + dof kT xi_1 + kT sum_{j>=2} xi_j is the conserved quantity
  * force must hold F(pos) on entry; lists and stats as in md_nve_step.  CUDA graphs of 8 steps unless
  * use_graph = 0.
  */

@@ -71,6 +71,7 @@ struct RuleArgs {
     int npred;                      // md_flock_predators
     void *pred;
     md_predator_params ppar;
+    int nh_chain;                   // Nose-Hoover chain length
     int fast32, builder, nb_parts, remap;
     float est_thr;
 };
@@ -113,6 +114,7 @@ struct md_system {
     float bks_A[16], bks_B[16], bks_C[16], bks_q[4], bks_alpha, bks_ke;
     int nobs;            // md_flock_obstacles
     float obs[3 * MD_MAX_OBSTACLES], J_obs;
+    int nh_chain;        // option "nh_chain": thermostats in the Nose-Hoover chain (1..8)
     int npred;           // md_flock_predators: count, DEVICE state (caller's), parameters
     void *pred;
     md_predator_params ppar;
@@ -606,10 +608,11 @@ int record_rule_step(md_system *s, const Pair &pp, const RuleArgs &A, cudaStream
         break;
     }
     case RULE_NH: {
-        const double dofkT = (double)g.dim * g.n * (double)A.kT, Q = dofkT * (double)A.tau * (double)A.tau;
+        const double dofkT = (double)g.dim * g.n * (double)A.kT, tau2 = (double)A.tau * (double)A.tau;
         float *scale = reinterpret_cast<float *>(s->fire_tmp + nbk);
         k_nh_ke<<<nbk, NH_BLOCK, 0, st>>>(g.n, g.dim, v4, partial);
-        k_nh_finalize<<<1, 256, 0, st>>>(nbk, partial, (double)A.mass, dofkT, Q, (double)A.dt, (double *)A.state, scale);
+        k_nh_finalize<<<1, 256, 0, st>>>(nbk, partial, (double)A.mass, dofkT, (double)A.kT, tau2, A.nh_chain,
+                                         (double)A.dt, (double *)A.state, scale);
         if (g.dim == 3) k_nh_kick_drift<3><<<nb, 256, 0, st>>>(g, p4, v4, f4, s->ref_pos, a, A.dt, scale, rs);
         else k_nh_kick_drift<2><<<nb, 256, 0, st>>>(g, p4, v4, f4, s->ref_pos, a, A.dt, scale, rs);
         force_vel = v4; force_a = a;
@@ -682,10 +685,11 @@ int record_rule_step(md_system *s, const Pair &pp, const RuleArgs &A, cudaStream
         k_fire_mix<<<nb, 256, 0, st>>>(g.n, v4, f4, coef);
         LAUNCH_OK();
     } else if (A.rule == RULE_NH) {
-        const double dofkT = (double)g.dim * g.n * (double)A.kT, Q = dofkT * (double)A.tau * (double)A.tau;
+        const double dofkT = (double)g.dim * g.n * (double)A.kT, tau2 = (double)A.tau * (double)A.tau;
         float *scale = reinterpret_cast<float *>(s->fire_tmp + nbk);
         k_nh_ke<<<nbk, NH_BLOCK, 0, st>>>(g.n, g.dim, v4, partial);
-        k_nh_finalize<<<1, 256, 0, st>>>(nbk, partial, (double)A.mass, dofkT, Q, (double)A.dt, (double *)A.state, scale);
+        k_nh_finalize<<<1, 256, 0, st>>>(nbk, partial, (double)A.mass, dofkT, (double)A.kT, tau2, A.nh_chain,
+                                         (double)A.dt, (double *)A.state, scale);
         k_nh_scale<<<nb, 256, 0, st>>>(g.n, v4, scale);
         LAUNCH_OK();
     }
@@ -788,6 +792,7 @@ int md_create(const md_config *cfg, int n, void *workspace, size_t bytes, md_sys
     s->pos_alt = (float4 *)(s->ws + l.pos_alt);
     s->tpp = n >= 32768 ? 0 : 4;     // 0 = streaming kernel; small systems: 4 lanes per particle
     s->use_graph = 1;
+    s->nh_chain = 1;
     s->fast32 = 1;
     s->builder = 2;
     s->remap = 37;      // a quarter of the SM count measured best (46.7 -> 44.9 us at N = 256k)
@@ -894,6 +899,11 @@ int md_set_option(md_system *sys, const char *name, double value) {
     else if (!strcmp(name, "builder")) {
         if (value != 1.0 && value != 2.0) return fail(MD_EINVAL, "builder must be 1 or 2");
         sys->builder = (int)value;
+    }
+    else if (!strcmp(name, "nh_chain")) {
+        if (!(value >= 1.0 && value <= (double)NH_MAX_CHAIN) || value != (double)(int)value)
+            return fail(MD_EINVAL, "nh_chain must be an integer in 1..%d", NH_MAX_CHAIN);
+        sys->nh_chain = (int)value;
     }
     else if (!strcmp(name, "est_thr")) {
         if (!(value > 0.0)) return fail(MD_EINVAL, "est_thr must be positive");
@@ -1060,6 +1070,7 @@ int md_nose_hoover_step(md_system *sys, const md_potential *pot, void *pos, void
     memset(&A, 0, sizeof(A));
     A.rule = RULE_NH; A.pos = pos; A.vel = vel; A.force = force; A.state = nh_state; A.id = id; A.nbr_idx = nbr_idx;
     A.nbr_count = nbr_count; A.stats = stats; A.pot = *pot; A.dt = dt; A.mass = mass; A.kT = kT; A.tau = tau;
+    A.nh_chain = sys->nh_chain;
     return run_rule(sys, pp, A, nsteps, (cudaStream_t)stream);
 }
 

@@ -1,4 +1,4 @@
-// md_nh.cuh -- NVT by one Nose-Hoover thermostat around the velocity-Verlet step (
+// md_nh.cuh -- NVT by a Nose-Hoover thermostat (a chain of 1..8, below) around the velocity-Verlet step (
 // PAPER.md:L100 "Nose-Hoover [67]"; no formulas in the paper: the explicit reversible splitting of
 // Martyna, Tuckerman, Tobias and Klein, reading A23).  dof = dim n, Q = dof kT tau^2.
 // Thermostat half step: K2 = sum m v^2; G = (K2 - dof kT)/Q; vxi += dt/4 G; s = exp(-dt/2 vxi);
@@ -31,9 +31,19 @@ k_nh_ke(int n, int dim, const float4 *__restrict__ vel, double *__restrict__ par
     }
 }
 
+// Chain of M thermostats ([67] Martyna, Klein, Tuckerman): Q_1 = dof kT tau^2, Q_j = kT tau^2; state =
+// {xi_1..xi_M, v_1..v_M}.  Half step, d = dt/2: v_M += d/2 G_M; for j = M-1..1: a = exp(-d/4 v_{j+1}),
+// v_j = (v_j a + d/2 G_j) a; s = exp(-d v_1); K2 *= s^2; xi_j += d v_j; then the same updates for
+// j = 1..M-1 and v_M last, with G_1 = (K2 - dof kT)/Q_1, G_j = (Q_{j-1} v_{j-1}^2 - kT)/Q_j.
+constexpr int NH_MAX_CHAIN = 8;
+
+__device__ __forceinline__ double nh_G(int j, double K2, double dofkT, double kT, const double *Q, const double *v) {
+    return j == 0 ? (K2 - dofkT) / Q[0] : (Q[j - 1] * v[j - 1] * v[j - 1] - kT) / Q[j];
+}
+
 __global__ void __launch_bounds__(256)
-k_nh_finalize(int nblocks, const double *__restrict__ partial, double mass, double dofkT, double Q,
-              double dt, double *state, float *scale) {
+k_nh_finalize(int nblocks, const double *__restrict__ partial, double mass, double dofkT, double kT, double tau2,
+              int M, double dt, double *state, float *scale) {
     __shared__ double red[256];
     double s = 0.0;
     for (int b = threadIdx.x; b < nblocks; b += 256) s += partial[b];
@@ -44,15 +54,23 @@ k_nh_finalize(int nblocks, const double *__restrict__ partial, double mass, doub
         __syncthreads();
     }
     if (threadIdx.x == 0) {
-        double K2 = mass * red[0], xi = state[0], vxi = state[1];
-        double G = (K2 - dofkT) / Q;
-        vxi += 0.25 * dt * G;
-        const double sc = exp(-0.5 * dt * vxi);
-        xi += 0.5 * dt * vxi;
+        double Q[NH_MAX_CHAIN], xi[NH_MAX_CHAIN], v[NH_MAX_CHAIN];
+        for (int j = 0; j < M; ++j) { Q[j] = (j == 0 ? dofkT : kT) * tau2; xi[j] = state[j]; v[j] = state[M + j]; }
+        double K2 = mass * red[0];
+        v[M - 1] += 0.25 * dt * nh_G(M - 1, K2, dofkT, kT, Q, v);
+        for (int j = M - 2; j >= 0; --j) {
+            const double a = exp(-0.125 * dt * v[j + 1]);
+            v[j] = (v[j] * a + 0.25 * dt * nh_G(j, K2, dofkT, kT, Q, v)) * a;
+        }
+        const double sc = exp(-0.5 * dt * v[0]);
+        for (int j = 0; j < M; ++j) xi[j] += 0.5 * dt * v[j];
         K2 *= sc * sc;
-        G = (K2 - dofkT) / Q;
-        vxi += 0.25 * dt * G;
-        state[0] = xi; state[1] = vxi;
+        for (int j = 0; j < M - 1; ++j) {
+            const double a = exp(-0.125 * dt * v[j + 1]);
+            v[j] = (v[j] * a + 0.25 * dt * nh_G(j, K2, dofkT, kT, Q, v)) * a;
+        }
+        v[M - 1] += 0.25 * dt * nh_G(M - 1, K2, dofkT, kT, Q, v);
+        for (int j = 0; j < M; ++j) { state[j] = xi[j]; state[M + j] = v[j]; }
         *scale = (float)sc;
     }
 }

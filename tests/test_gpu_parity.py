@@ -403,6 +403,41 @@ def test_nose_hoover_against_the_oracle(B, orc, W):
     S.close(); S2.close()
 
 
+def test_nose_hoover_chain_against_the_oracle(B, orc, W):
+    """A chain of three thermostats ([67]; option "nh_chain"): 80 steps against the oracle -- positions,
+    velocities and all six thermostat variables; graph and direct launches agree bit for bit; a chain
+    of one is the default."""
+    w = W.config(0)
+    dt, mass, kT, tau, steps, M = 0.004, 1.0, 0.5, 0.2, 80, 3
+    outs = []
+    for graph in (1, 0):
+        S = B.System(w)
+        B.md_set_option(S.sys, "nh_chain", M)
+        B.md_set_option(S.sys, "use_graph", graph)
+        S.build(); S.compute_force()
+        state = torch.zeros(2 * M, dtype=torch.float64, device="cuda")
+        B.md_nose_hoover_step(S.sys, S.pot, S.pos, S.vel, S.force, S.id, S.nbr_idx, S.nbr_count, dt, mass, kT, tau,
+                              state, steps, S.stats)
+        torch.cuda.synchronize()
+        outs.append((S.pos.clone(), S.vel.clone(), state.clone(), unpermute(S, S.pos), unpermute(S, S.vel)))
+        S.close()
+    assert torch.equal(outs[0][0], outs[1][0]) and torch.equal(outs[0][1], outs[1][1]) and torch.equal(outs[0][2], outs[1][2])
+    p_o, v_o, f_o, cons, st_o = orc.nose_hoover_run(w.pos, w.vel, None, w.box, 3, 0, 1.0, 1.0, 2.5, 1, dt, mass, kT, tau,
+                                                    steps, chain=M)
+    st = outs[0][2].cpu().numpy()
+    assert np.abs(st_o[M:]).min() > 1e-3                                   # every link is in motion
+    assert np.abs(st - st_o).max() <= 1e-4 * np.abs(st_o).max(), (st, st_o)
+    L = w.box.astype(np.float64)
+    d = outs[0][3][:, :3].astype(np.float64) - p_o
+    d -= L * np.round(d / L)
+    assert np.abs(d).max() <= 1e-4, np.abs(d).max()
+    assert np.abs(outs[0][4][:, :3] - v_o).max() <= 2e-3
+    S = B.System(w)
+    with pytest.raises(B.MdError):
+        B.md_set_option(S.sys, "nh_chain", 9)
+    S.close()
+
+
 def test_buckingham_force_energy_and_trajectory(B, orc, W):
     """Buckingham-type exp-6 (PAPER.md:L104 [71-73]) on the fp64 pair chain: force and
     energy against the all-pairs definition, then 100 NVE steps against the oracle."""
