@@ -117,6 +117,30 @@ int md_set_option(md_system *sys, const char *name, double value);
 int md_set_species_lj(md_system *sys, int nspecies, const float *epsilon, const float *sigma,
                       const float *r_cut);
 
+/*
+ * Multi-GPU by replicated positions and a split neighbor list: every rank holds
+ * all positions and runs the same cell list and re-sort, but builds list rows and computes forces only for
+ * its own range of (cell-sorted) particles, integrates those, and the ranks exchange their position ranges
+ * every step (velocities at rebuilds).  The list -- 4 * capacity bytes per particle against 16 for a
+ * position -- is what is split.
+ *
+ * md_set_range: this context owns particles [begin, end): begin a multiple of 32 (a list tile), end a
+ * multiple of 32 or n.  From then on md_neighbor_list_build writes rows, counts and rebuild references of
+ * that range only, md_pair_energy_force (3-D Lennard-Jones fast path) forces, e_i and the energy sum of that
+ * range only; md_cell_list_build stays global; the step calls (md_nve_step, ...) return MD_EINVAL -- the
+ * step is driven from outside with the two calls below around the exchange.  [0, n) restores the default.
+ */
+int md_set_range(md_system *sys, int begin, int end);
+
+/* First half of a velocity-Verlet step on the context's range: v += dt/(2m) F; r = wrap(r + dt v); *flag
+ * (DEVICE int32) = 1 if a particle of the range is now more than skin/2 from its position at the last list
+ * build, else 0.  The arithmetic of md_nve_step's own opening kernel. */
+int md_kick_drift(md_system *sys, void *pos, void *vel, const void *force, float dt, float mass,
+                  int32_t *flag, void *stream);
+
+/* Closing half-kick on the context's range: v += dt/(2m) F. */
+int md_half_kick(md_system *sys, void *vel, const void *force, float dt, float mass, void *stream);
+
 /* BKS-type potential (L104 "Buckingham / BKS" [71-73], named only; reading A27): per species
  * pair the exp-6 term A_ab exp(-B_ab r) - C_ab / r^6, plus the Coulomb interaction of the species' point
  * charges in its damped shifted-force form (energy and force both vanish at r_cut):

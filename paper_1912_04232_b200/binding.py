@@ -24,6 +24,7 @@ SYMBOLS = [
     "md_nve_run_host_release", "md_fire_minimize", "md_brownian_step",
     "md_langevin_step", "md_nose_hoover_step", "md_set_species_lj",
     "md_flock_step", "md_flock_obstacles", "md_set_species_bks", "md_flock_predators",
+    "md_set_range", "md_kick_drift", "md_half_kick",
 ]
 
 
@@ -89,6 +90,9 @@ def lib():
         L.md_nose_hoover_step.argtypes = [vp, C.POINTER(md_potential), vp, vp, vp, ip, ip, ip, C.c_float,
                                           C.c_float, C.c_float, C.c_float, vp, C.c_int, ip, vp]
         L.md_set_species_bks.argtypes = [vp, C.c_int] + [C.POINTER(C.c_float)] * 4 + [C.c_float, C.c_float]
+        L.md_set_range.argtypes = [vp, C.c_int, C.c_int]
+        L.md_kick_drift.argtypes = [vp, vp, vp, vp, C.c_float, C.c_float, ip, vp]
+        L.md_half_kick.argtypes = [vp, vp, vp, C.c_float, C.c_float, vp]
         L.md_flock_predators.argtypes = [vp, C.c_int, vp, C.POINTER(md_predator_params)]
         L.md_flock_obstacles.argtypes = [vp, C.c_int, C.POINTER(C.c_float), C.POINTER(C.c_float), C.c_float]
         L.md_flock_step.argtypes = [vp, C.POINTER(md_flock_params), vp, ip, ip, ip, C.c_float, C.c_int, ip, vp]
@@ -245,6 +249,19 @@ def md_set_species_bks(sys, A, B, Cc, charge, coulomb_alpha, k_e=1.0) -> None:
     fp = C.POINTER(C.c_float)
     _check(lib().md_set_species_bks(sys, ns, *[t.ctypes.data_as(fp) for t in tabs], q.ctypes.data_as(fp),
                                     float(coulomb_alpha), float(k_e)))
+
+
+def md_set_range(sys, begin: int, end: int) -> None:
+    _check(lib().md_set_range(sys, int(begin), int(end)))
+
+
+def md_kick_drift(sys, pos, vel, force, dt, mass, flag, stream=None) -> None:
+    _check(lib().md_kick_drift(sys, _ptr(pos), _ptr(vel), _ptr(force), float(dt), float(mass), _ptr(flag),
+                               _stream(stream)))
+
+
+def md_half_kick(sys, vel, force, dt, mass, stream=None) -> None:
+    _check(lib().md_half_kick(sys, _ptr(vel), _ptr(force), float(dt), float(mass), _stream(stream)))
 
 
 def md_counters(sys, out, reset=False, stream=None) -> None:

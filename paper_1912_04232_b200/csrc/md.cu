@@ -114,6 +114,7 @@ struct md_system {
     float bks_A[16], bks_B[16], bks_C[16], bks_q[4], bks_alpha, bks_ke;
     int nobs;            // md_flock_obstacles
     float obs[3 * MD_MAX_OBSTACLES], J_obs;
+    int r0, r1;          // md_set_range: the particles [r0, r1) this context builds rows and forces for
     int nh_chain;        // option "nh_chain": thermostats in the Nose-Hoover chain (1..8)
     int npred;           // md_flock_predators: count, DEVICE state (caller's), parameters
     void *pred;
@@ -314,10 +315,11 @@ int launch_nbr_build(md_system *s, const float4 *spos, const int *cell_start, co
         // 256k 151 / 200 / 182, 1M 414 / 662 / 618: sharing pays only while the GPU is not full
         if (parts == 0) parts = ntiles <= 2048 ? 4 : 1;
         const int tpb = NB2_WARPS / parts;
-        const int nb = (ntiles + tpb - 1) / tpb;
+        const int tile0 = s->r0 / TILE, tile1 = (s->r1 + TILE - 1) / TILE;          // md_set_range
+        const int nb = std::max(1, (tile1 - tile0 + tpb - 1) / tpb);
         const int threads = NB2_WARPS * 32;
         const size_t sm = NB2_WARPS * sizeof(Nb2Warp);
-#define MD_NB2_LAUNCH(D, M, P) k_nbr_build2<D, M, P><<<nb, threads, sm, st>>>(g, spos, cell_start, map, nbr_idx, nbr_count, status, s->ref_pos, cond, incremental)
+#define MD_NB2_LAUNCH(D, M, P) k_nbr_build2<D, M, P><<<nb, threads, sm, st>>>(g, spos, cell_start, map, nbr_idx, nbr_count, status, s->ref_pos, cond, incremental, tile0, tile1)
 #define MD_NB2_PARTS(D, M) do { if (parts == 4) MD_NB2_LAUNCH(D, M, 4); else if (parts == 2) MD_NB2_LAUNCH(D, M, 2); else MD_NB2_LAUNCH(D, M, 1); } while (0)
         if (g.dim == 3) { if (map) MD_NB2_PARTS(3, true); else MD_NB2_PARTS(3, false); }
         else { if (map) MD_NB2_PARTS(2, true); else MD_NB2_PARTS(2, false); }
@@ -326,6 +328,7 @@ int launch_nbr_build(md_system *s, const float4 *spos, const int *cell_start, co
         LAUNCH_OK();
         return MD_OK;
     }
+    if (s->r0 != 0 || s->r1 != g.n) return fail(MD_EINVAL, "md_set_range needs the bit-mask builder (builder = 2)");
     const int nb = (ntiles + s->nb_warps - 1) / s->nb_warps;
     const int threads = s->nb_warps * 32;
     if (g.dim == 3) {
@@ -379,15 +382,19 @@ int launch_force(md_system *s, const Pair &pp, const float4 *pos, const int *nbr
         q.escale = (float)(2.0 * pp.deps);
         q.near_band = 1e-5f * q.rc2;
         q.est_thr = s->est_thr;
-        const int nb = blocks_for(s->g.n, F32_WARPS * 32);
+        Geom gr = s->g;
+        gr.n = s->r1;                                  // md_set_range: lanes beyond r1 are idle
+        const int nb = blocks_for(s->r1 - s->r0, F32_WARPS * 32);
         int *nfix = s->words + 8;
         int P = 0, grid = nb;
         if (s->remap > 0 && nb > 4 * s->remap) { P = s->remap; grid = P * ((nb + P - 1) / P); }
-        if (want_energy) k_force_lj32<true><<<grid, F32_WARPS * 32, 0, st>>>(s->g, pp, q, pos, nbr_idx, nbr_count, force, vel, a, etot, book, nfix, nx, P, nb);
-        else k_force_lj32<false><<<grid, F32_WARPS * 32, 0, st>>>(s->g, pp, q, pos, nbr_idx, nbr_count, force, vel, a, etot, book, nfix, nx, P, nb);
+        if (want_energy) k_force_lj32<true><<<grid, F32_WARPS * 32, 0, st>>>(gr, pp, q, pos, nbr_idx, nbr_count, force, vel, a, etot, book, nfix, nx, P, nb, s->r0);
+        else k_force_lj32<false><<<grid, F32_WARPS * 32, 0, st>>>(gr, pp, q, pos, nbr_idx, nbr_count, force, vel, a, etot, book, nfix, nx, P, nb, s->r0);
         LAUNCH_OK();
         return MD_OK;
     }
+    if (s->r0 != 0 || s->r1 != s->g.n)
+        return fail(MD_EINVAL, "md_set_range: only the 3-D Lennard-Jones fast path computes forces of a range");
 #define MD_FORCE_DISPATCH(K, D)                                                                 \
     (want_energy ? launch_force_t<K, D, true>(s, pp, pos, nbr_idx, nbr_count, force, vel, a,   \
                                               etot, book, st)                                  \
@@ -713,6 +720,7 @@ int capture_rule(md_system *s, const Pair &pp, const RuleArgs &A, int reps, cuda
 
 // nsteps of an update rule: stats reset, then graphs of 8 steps and of 1 step (or direct launches).
 int run_rule(md_system *s, const Pair &pp, RuleArgs &A, int nsteps, cudaStream_t st) {
+    if (s->r0 != 0 || s->r1 != s->g.n) return fail(MD_EINVAL, "a range is set (md_set_range): drive the step with md_kick_drift / md_half_kick");
     A.fast32 = s->fast32; A.builder = s->builder; A.nb_parts = s->nb_parts; A.remap = s->remap; A.est_thr = s->est_thr;
     k_init_stats<<<1, 1, 0, st>>>(A.stats, s->words + 0);
     LAUNCH_OK();
@@ -793,6 +801,7 @@ int md_create(const md_config *cfg, int n, void *workspace, size_t bytes, md_sys
     s->tpp = n >= 32768 ? 0 : 4;     // 0 = streaming kernel; small systems: 4 lanes per particle
     s->use_graph = 1;
     s->nh_chain = 1;
+    s->r0 = 0; s->r1 = n;
     s->fast32 = 1;
     s->builder = 2;
     s->remap = 37;      // a quarter of the SM count measured best (46.7 -> 44.9 us at N = 256k)
@@ -978,6 +987,7 @@ int md_nve_step(md_system *sys, const md_potential *pot, void *pos, void *vel, v
         return fail(MD_EINVAL, "NULL argument");
     if (!aligned16(pos) || !aligned16(vel) || !aligned16(force)) return fail(MD_EINVAL, "pos/vel/force must be 16-byte aligned");
     if (!(dt > 0.0f) || !(mass > 0.0f) || nsteps < 0) return fail(MD_EINVAL, "dt and mass must be positive, nsteps >= 0");
+    if (sys->r0 != 0 || sys->r1 != sys->g.n) return fail(MD_EINVAL, "a range is set (md_set_range): drive the step with md_kick_drift / md_half_kick");
     Pair pp;
     int rc = make_pair(sys, pot, &pp);
     if (rc) return rc;
@@ -1072,6 +1082,46 @@ int md_nose_hoover_step(md_system *sys, const md_potential *pot, void *pos, void
     A.nbr_count = nbr_count; A.stats = stats; A.pot = *pot; A.dt = dt; A.mass = mass; A.kT = kT; A.tau = tau;
     A.nh_chain = sys->nh_chain;
     return run_rule(sys, pp, A, nsteps, (cudaStream_t)stream);
+}
+
+int md_set_range(md_system *sys, int begin, int end) {
+    if (!sys) return fail(MD_EINVAL, "NULL argument");
+    if (begin < 0 || end > sys->n || begin >= end || begin % TILE != 0 || (end % TILE != 0 && end != sys->n))
+        return fail(MD_EINVAL, "range [%d, %d) must be non-empty, inside [0, %d) and aligned to list tiles of %d", begin, end, sys->n, TILE);
+    sys->r0 = begin; sys->r1 = end;
+    drop_graphs(sys);
+    return MD_OK;
+}
+
+int md_kick_drift(md_system *sys, void *pos, void *vel, const void *force, float dt, float mass,
+                  int32_t *flag, void *stream) {
+    if (!sys || !pos || !vel || !force || !flag) return fail(MD_EINVAL, "NULL argument");
+    if (!aligned16(pos) || !aligned16(vel) || !aligned16(force)) return fail(MD_EINVAL, "pos/vel/force must be 16-byte aligned");
+    if (!(dt > 0.0f) || !(mass > 0.0f)) return fail(MD_EINVAL, "dt and mass must be positive");
+    if (int rc = enter(sys)) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    CU(cudaMemsetAsync(flag, 0, sizeof(int), st));
+    Geom gr = sys->g;
+    gr.n = sys->r1 - sys->r0;                          // an elementwise kernel: the range by pointer offset
+    const size_t o = (size_t)sys->r0;
+    const float a = dt / (2.0f * mass);
+    cudaGraphConditionalHandle none = 0;
+    if (gr.dim == 3) k_kick_drift<3, false><<<blocks_for(gr.n), 256, 0, st>>>(gr, (float4 *)pos + o, (float4 *)vel + o, (const float4 *)force + o, sys->ref_pos + o, a, dt, flag, none);
+    else k_kick_drift<2, false><<<blocks_for(gr.n), 256, 0, st>>>(gr, (float4 *)pos + o, (float4 *)vel + o, (const float4 *)force + o, sys->ref_pos + o, a, dt, flag, none);
+    LAUNCH_OK();
+    return MD_OK;
+}
+
+int md_half_kick(md_system *sys, void *vel, const void *force, float dt, float mass, void *stream) {
+    if (!sys || !vel || !force) return fail(MD_EINVAL, "NULL argument");
+    if (!aligned16(vel) || !aligned16(force)) return fail(MD_EINVAL, "vel/force must be 16-byte aligned");
+    if (!(dt > 0.0f) || !(mass > 0.0f)) return fail(MD_EINVAL, "dt and mass must be positive");
+    if (int rc = enter(sys)) return rc;
+    const int m = sys->r1 - sys->r0;
+    const size_t o = (size_t)sys->r0;
+    k_half_kick<<<blocks_for(m), 256, 0, (cudaStream_t)stream>>>(m, sys->g.dim, (float4 *)vel + o, (const float4 *)force + o, dt / (2.0f * mass));
+    LAUNCH_OK();
+    return MD_OK;
 }
 
 int md_set_species_bks(md_system *sys, int nspecies, const float *A, const float *B, const float *C,

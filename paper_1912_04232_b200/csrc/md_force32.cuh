@@ -177,7 +177,7 @@ __global__ void __launch_bounds__(F32_WARPS * 32)
 k_force_lj32(Geom g, Pair pp, Pair32 p32, const float4 *__restrict__ pos,
              const int *__restrict__ nbr_idx, const int *__restrict__ nbr_count,
              float4 *__restrict__ force, float4 *__restrict__ vel, float a, double *energy_total,
-             Book book, int *nfix, NextStep nx, int remap_p, int nblocks) {
+             Book book, int *nfix, NextStep nx, int remap_p, int nblocks, int i0) {
     const int lane = threadIdx.x & 31;
     // remap_p > 0: the grid has remap_p * Q blocks and block i works on tile block
     // (i % remap_p) * Q + i / remap_p, so that the blocks the hardware deals round-robin to one SM
@@ -188,7 +188,7 @@ k_force_lj32(Geom g, Pair pp, Pair32 p32, const float4 *__restrict__ pos,
         bid = (bid % remap_p) * Q + bid / remap_p;
         if (bid >= nblocks) return;
     }
-    const int gid = bid * blockDim.x + threadIdx.x;
+    const int gid = i0 + bid * blockDim.x + threadIdx.x;      // i0: first particle of this context's range
     const int i = gid;
     const bool active = i < g.n;
     const int ii = active ? i : g.n - 1;

@@ -583,6 +583,19 @@ k_needs_rebuild(Geom g, const float4 *__restrict__ pos, const float4 *__restrict
 // v += dt/(2m) F;  r = mu(r, dt v);  rebuild test against the reference positions.
 // HAS_COND: the step runs inside a CUDA graph whose rebuild kernels sit in an IF node; the warp
 // that sees a particle beyond skin/2 also raises the node's condition (default 0 per launch).
+// v += a F on m particles (the closing half-kick as a kernel of its own: md_half_kick; inside
+// md_nve_step it is the force kernel's epilogue, same fma on the same rounded force)
+__global__ void __launch_bounds__(256)
+k_half_kick(int m, int dim, float4 *__restrict__ vel, const float4 *__restrict__ force, float a) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= m) return;
+    float4 v = vel[i];
+    const float4 f = force[i];
+    v.x = fmaf(a, f.x, v.x); v.y = fmaf(a, f.y, v.y);
+    if (dim == 3) v.z = fmaf(a, f.z, v.z);
+    vel[i] = v;
+}
+
 template <int DIM, bool HAS_COND>
 __global__ void __launch_bounds__(256)
 k_kick_drift(Geom g, float4 *__restrict__ pos, float4 *__restrict__ vel,

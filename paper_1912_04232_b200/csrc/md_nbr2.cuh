@@ -63,7 +63,8 @@ template <int DIM, bool MAPPED, int PARTS>
 __global__ void __launch_bounds__(NB2_WARPS * 32, MD_NB2_MINBLOCKS)
 k_nbr_build2(Geom g, const float4 *__restrict__ spos, const int *__restrict__ cell_start,
              const int *__restrict__ map, int *__restrict__ nbr_idx, int *__restrict__ nbr_count,
-             int *status, float4 *__restrict__ ref_pos, const int *cond, int incremental) {
+             int *status, float4 *__restrict__ ref_pos, const int *cond, int incremental,
+             int tile0, int tile1) {
     extern __shared__ __align__(16) unsigned char nb2_smem[];
     if (cond && ld_volatile(cond) == 0) return;
     __shared__ int coop[NB2_WARPS][TILE];                  // per-lane hit counts of the parts of a tile
@@ -77,9 +78,9 @@ k_nbr_build2(Geom g, const float4 *__restrict__ spos, const int *__restrict__ ce
     const float2 nR2 = make_float2(-g.R2, -g.R2);
     const float Rm = sqrtf(g.R2) * 1.0001f + 1e-4f * g.L[0];    // R plus a margin for the fp32 roundings
     constexpr int ROWS = DIM == 3 ? 9 : 3;
-    const int ntiles = (g.n + TILE - 1) / TILE;
+    const int ntiles = min(tile1, (g.n + TILE - 1) / TILE);     // this context's tiles: [tile0, tile1)
 
-    for (int tile = blockIdx.x * TPB + tl; tile < ntiles; tile += gridDim.x * TPB) {
+    for (int tile = tile0 + blockIdx.x * TPB + tl; tile < ntiles; tile += gridDim.x * TPB) {
         const int s = tile * TILE + lane;
         const bool act = s < g.n;
         const float4 pi = spos[act ? s : g.n - 1];

@@ -1132,3 +1132,48 @@ def test_config3_long_run(B, orc, W):
     of the final state against the oracle."""
     rebuilds = snapshot_checks(B, orc, W, W.config(3), 2000)
     assert rebuilds >= 200
+
+
+@pytest.mark.parametrize("world,m,steps", [(2, 6, 100), (3, 6, 100), (4, 12, 60)])
+def test_split_list_ranks_equal_one_gpu(B, W, world, m, steps):
+    """SURVEY §8f-f1 (replicated positions, split list; decomposition.py): `world` contexts in one
+    process, each owning a range of list tiles, stepped in lockstep with the all-gather replaced by a
+    stack -- positions, velocities, forces and ids after `steps` steps are bit-identical to md_nve_step
+    on one context, with the same number of rebuilds; each rank's list holds rows of its range only."""
+    from paper_1912_04232_b200 import decomposition as D
+    w = W.lj_fcc(0, m, seed=3)
+    one = B.System(w)
+    one.build(); one.compute_force()
+    one.step(steps)
+    torch.cuda.synchronize()
+    loops = []
+    for r in range(world):
+        S = B.System(w)
+        loops.append(D.RankLoop(S, r, world))
+    for lp in loops:
+        lp.start()
+    D.run_local(loops, steps)
+    D.gather_state_local(loops)
+    torch.cuda.synchronize()
+    assert int(one.stats[1]) >= 3
+    for lp in loops:
+        assert lp.rebuilds == int(one.stats[1])
+        assert torch.equal(lp.S.pos, one.pos) and torch.equal(lp.S.vel, one.vel) and torch.equal(lp.S.id, one.id)
+        assert torch.equal(lp.S.force[:, :3], one.force[:, :3])
+        b, e = lp.range
+        assert torch.equal(lp.S.nbr_count[b:e], one.nbr_count[b:e])
+    # the energy of the ranges adds up to the total
+    one.compute_force()
+    E = 0.0
+    for lp in loops:
+        lp.S.compute_force(want_energy=True)
+        E += float(lp.S.energy[0])
+    assert abs(E - float(one.energy[0])) <= 1e-12 * abs(float(one.energy[0]))
+    # a range is not steppable from inside, and only tile-aligned ranges are accepted
+    with pytest.raises(B.MdError):
+        loops[0].S.step(1)
+    with pytest.raises(B.MdError):
+        B.md_set_range(loops[0].S.sys, 16, 64)
+    for lp in loops:
+        lp.S.close()
+    one.close()
