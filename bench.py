@@ -54,6 +54,9 @@ def parse():
     ap.add_argument("--md-steps", type=int, default=100, help="MD steps per bench step")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--decompose", action="store_true",
+                    help="time the split-list multi-GPU loop (SURVEY 8f-f1) instead: ONE system over all ranks, "
+                         "strong scaling; not the contract line")
     ap.add_argument("--next-rows", action="store_true",
                     help="time the SURVEY 8(f) rows instead (one JSON line per row; not the contract line)")
     ap.add_argument("--breakdown", action="store_true", help="(kept for compatibility: the build time per rebuild is always reported)")
@@ -285,12 +288,82 @@ def run_next_rows(args):
     S.close()
 
 
+def run_decomposed(args):
+    """SURVEY 8(f)-f1: one system of config `--config` over all ranks (replicated positions, split list;
+    paper_1912_04232_b200/decomposition.py).  A bench step is `--md-steps` MD steps; device time by CUDA
+    events on the current stream, max over ranks; value = N * md_steps / that time (strong scaling).  With
+    one rank it measures what the host-driven step costs against md_nve_step's graph."""
+    import torch
+    import torch.distributed as dist
+    from paper_1912_04232_b200 import binding as B
+    from paper_1912_04232_b200 import decomposition as D
+    from paper_1912_04232_b200 import replicas as R
+    from paper_1912_04232_b200 import workloads as W
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+        exchange = D.DistExchange()
+    else:
+        class Solo:
+            def all_gather(self, slot):
+                return slot.unsqueeze(0)
+        exchange = Solo()
+    w = W.config(args.config)                       # the SAME system on every rank
+    S = B.System(w, device=dev)
+    loop = D.RankLoop(S, rank, world)
+    loop.start()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)
+
+    def barrier():
+        torch.cuda.synchronize(dev)
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize(dev)
+
+    for _ in range(args.warmup):
+        D.run(loop, exchange, args.md_steps)
+    barrier()
+    r0 = loop.rebuilds
+    ms = 0.0
+    for _ in range(args.steps):
+        flush.zero_()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        D.run(loop, exchange, args.md_steps)
+        b.record()
+        torch.cuda.synchronize(dev)
+        ms += a.elapsed_time(b)
+    barrier()
+    ms = R.max_over_ranks(ms, dev) if world > 1 else ms
+    if rank == 0:
+        total = args.steps * args.md_steps
+        print(json.dumps({
+            "mode": "decompose", "metric": METRIC, "value": w.n * total / (ms * 1e-3), "unit": UNIT,
+            "n_gpus": world, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
+            "us_per_md_step": 1e3 * ms / total, "higher_is_better": True, "scaling": "strong",
+            "dtype": "f32", "data": "synthetic",
+            "config": {"workload": w.name, "n": w.n, "md_steps_per_step": args.md_steps,
+                       "parallelism": f"split list x{world} (replicated positions, one all-gather per step)"},
+            "rebuilds": loop.rebuilds - r0, "range_rank0": list(loop.range)}))
+    if world > 1:
+        dist.destroy_process_group()
+
+
 def main():
     args = parse()
     if args.impl == "reference":
         return run_reference(args)
     if args.next_rows:
         return run_next_rows(args)
+    if args.decompose:
+        return run_decomposed(args)
 
     import torch
     import torch.distributed as dist

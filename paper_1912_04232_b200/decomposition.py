@@ -11,8 +11,8 @@ the re-sort moves particles -- and with them ownership -- between ranges.  What 
 This module is plumbing only: ranges, the packing of what travels, and the order of the C-ABI calls.
 All arithmetic runs in the library's kernels, and a run on P ranks is bit-identical to md_nve_step on
 one (same kernels, same per-particle operation order).  `exchange` is torch.distributed's all-gather
-(NCCL over NVLink on GPUs, gloo in the CPU test) or, for tests on one GPU, `LocalExchange`, which
-steps P contexts of one process in lockstep.
+(NCCL over NVLink on GPUs, gloo in the CPU test); for tests on one GPU `run_local` steps P contexts
+of one process in lockstep.
 """
 from __future__ import annotations
 
@@ -39,21 +39,24 @@ def slot_rows(n: int, world: int) -> int:
     return max(e - b for b, e in ranges(n, world)) + 1
 
 
-def pack(x: torch.Tensor, rng: tuple[int, int], rows: int, flag: torch.Tensor | None = None) -> torch.Tensor:
-    """This rank's slot: x[begin:end], zero padding, and in the last row the flag (as a float)."""
+def pack(x: torch.Tensor, rng: tuple[int, int], rows: int, flag: torch.Tensor | None = None,
+         out: torch.Tensor | None = None) -> torch.Tensor:
+    """This rank's slot: x[begin:end], zero padding, and in the last row the flag (as a float).
+    `out`: a slot buffer to reuse (its padding rows stay as they are: zero from its creation)."""
     b, e = rng
-    slot = torch.zeros(rows, x.shape[1], dtype=x.dtype, device=x.device)
+    slot = out if out is not None else torch.zeros(rows, x.shape[1], dtype=x.dtype, device=x.device)
     slot[: e - b] = x[b:e]
-    if flag is not None:
-        slot[rows - 1, 0] = flag.to(x.dtype)[0]
+    slot[rows - 1, 0] = flag.to(x.dtype)[0] if flag is not None else 0.0
     return slot
 
 
-def unpack(slots: torch.Tensor, n: int, world: int, out: torch.Tensor) -> torch.Tensor:
-    """slots [world, rows, 4] -> out[begin_r:end_r] for every r; returns the OR of the flags (0-d bool)."""
+def unpack(slots: torch.Tensor, n: int, world: int, out: torch.Tensor, skip: int = -1) -> torch.Tensor:
+    """slots [world, rows, 4] -> out[begin_r:end_r] for every r but `skip` (the caller's own range, which
+    it already holds); returns the OR of the flags (0-d bool)."""
     rows = slots.shape[1]
     for r, (b, e) in enumerate(ranges(n, world)):
-        out[b:e] = slots[r, : e - b]
+        if r != skip:
+            out[b:e] = slots[r, : e - b]
     return (slots[:, rows - 1, 0] != 0).any()
 
 
@@ -84,6 +87,7 @@ class RankLoop:
         self.rows = slot_rows(self.n, world)
         B.md_set_range(system.sys, *self.range)
         self.rebuilds = 0
+        self.slot = torch.zeros(self.rows, 4, dtype=torch.float32, device=system.pos.device)    # reused every step
 
     # -- the phases of one step; `exchange` sits between them
     def start(self):
@@ -94,16 +98,16 @@ class RankLoop:
     def move(self) -> torch.Tensor:
         w = self.S.w
         self.B.md_kick_drift(self.S.sys, self.S.pos, self.S.vel, self.S.force, w.dt, w.mass, self.S.flag)
-        return pack(self.S.pos, self.range, self.rows, self.S.flag)
+        return pack(self.S.pos, self.range, self.rows, self.S.flag, out=self.slot)
 
     def absorb_positions(self, slots: torch.Tensor) -> bool:
-        return bool(unpack(slots, self.n, self.world, self.S.pos))
+        return bool(unpack(slots, self.n, self.world, self.S.pos, skip=self.rank))
 
     def velocity_slot(self) -> torch.Tensor:
-        return pack(self.S.vel, self.range, self.rows)
+        return pack(self.S.vel, self.range, self.rows, out=self.slot)
 
     def rebuild(self, vel_slots: torch.Tensor):
-        unpack(vel_slots, self.n, self.world, self.S.vel)
+        unpack(vel_slots, self.n, self.world, self.S.vel, skip=self.rank)
         self.S.build()                     # global cell list + re-sort, list rows of the own range
         self.rebuilds += 1
 
