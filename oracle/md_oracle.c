@@ -41,8 +41,11 @@
  * values and gradients of every potential, FIRE's schedule in closed form and its
  * reduction to velocity Verlet, generator moments, free diffusion, exact friction
  * decay and stationary variance, Nose-Hoover's conserved quantity at second order
- * and its decoupled limit, the boids energies on a pair by hand with finite-difference
- * gradients and rotation / translation invariance.  The one unpinned thing is a chaotic
+ * (single thermostat and chains), its decoupled limit, time reversibility and the second
+ * link's equation of motion, the Madelung constant of rock salt for the damped
+ * shifted-force Coulomb term, the boids energies on a pair by hand with finite-difference
+ * gradients and rotation / translation invariance, the obstacle and predator terms in
+ * closed form for one boid / one clump.  The one unpinned thing is a chaotic
  * trajectory beyond ~100 steps ("parity unpinned" by design).
  *
  * Arithmetic: fp64 everywhere, except the canonical inclusion predicate
