@@ -138,6 +138,12 @@ int md_set_range(md_system *sys, int begin, int end);
 int md_kick_drift(md_system *sys, void *pos, void *vel, const void *force, float dt, float mass,
                   int32_t *flag, void *stream);
 
+/* Second half of a velocity-Verlet step on the context's range in one launch: F = F(pos) over the list (no
+ * energies: force.w = 0), then v += dt/(2m) F in the force kernel's epilogue -- md_nve_step's own closing
+ * kernel.  Arguments as md_pair_energy_force, plus vel float4[n] in/out. */
+int md_force_half_kick(md_system *sys, const md_potential *pot, const void *pos, const int32_t *nbr_idx,
+                       const int32_t *nbr_count, void *force, void *vel, float dt, float mass, void *stream);
+
 /* Closing half-kick on the context's range: v += dt/(2m) F. */
 int md_half_kick(md_system *sys, void *vel, const void *force, float dt, float mass, void *stream);
 

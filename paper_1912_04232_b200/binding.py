@@ -24,7 +24,7 @@ SYMBOLS = [
     "md_nve_run_host_release", "md_fire_minimize", "md_brownian_step",
     "md_langevin_step", "md_nose_hoover_step", "md_set_species_lj",
     "md_flock_step", "md_flock_obstacles", "md_set_species_bks", "md_flock_predators",
-    "md_set_range", "md_kick_drift", "md_half_kick",
+    "md_set_range", "md_kick_drift", "md_half_kick", "md_force_half_kick",
 ]
 
 
@@ -92,6 +92,7 @@ def lib():
         L.md_set_species_bks.argtypes = [vp, C.c_int] + [C.POINTER(C.c_float)] * 4 + [C.c_float, C.c_float]
         L.md_set_range.argtypes = [vp, C.c_int, C.c_int]
         L.md_kick_drift.argtypes = [vp, vp, vp, vp, C.c_float, C.c_float, ip, vp]
+        L.md_force_half_kick.argtypes = [vp, C.POINTER(md_potential), vp, ip, ip, vp, vp, C.c_float, C.c_float, vp]
         L.md_half_kick.argtypes = [vp, vp, vp, C.c_float, C.c_float, vp]
         L.md_flock_predators.argtypes = [vp, C.c_int, vp, C.POINTER(md_predator_params)]
         L.md_flock_obstacles.argtypes = [vp, C.c_int, C.POINTER(C.c_float), C.POINTER(C.c_float), C.c_float]
@@ -258,6 +259,11 @@ def md_set_range(sys, begin: int, end: int) -> None:
 def md_kick_drift(sys, pos, vel, force, dt, mass, flag, stream=None) -> None:
     _check(lib().md_kick_drift(sys, _ptr(pos), _ptr(vel), _ptr(force), float(dt), float(mass), _ptr(flag),
                                _stream(stream)))
+
+
+def md_force_half_kick(sys, pot: md_potential, pos, nbr_idx, nbr_count, force, vel, dt, mass, stream=None) -> None:
+    _check(lib().md_force_half_kick(sys, C.byref(pot), _ptr(pos), _ptr(nbr_idx), _ptr(nbr_count), _ptr(force),
+                                    _ptr(vel), float(dt), float(mass), _stream(stream)))
 
 
 def md_half_kick(sys, vel, force, dt, mass, stream=None) -> None:

@@ -1112,6 +1112,20 @@ int md_kick_drift(md_system *sys, void *pos, void *vel, const void *force, float
     return MD_OK;
 }
 
+int md_force_half_kick(md_system *sys, const md_potential *pot, const void *pos, const int32_t *nbr_idx,
+                       const int32_t *nbr_count, void *force, void *vel, float dt, float mass, void *stream) {
+    if (!sys || !pos || !nbr_idx || !nbr_count || !force || !vel) return fail(MD_EINVAL, "NULL argument");
+    if (!aligned16(pos) || !aligned16(force) || !aligned16(vel)) return fail(MD_EINVAL, "pos/force/vel must be 16-byte aligned");
+    if (!(dt > 0.0f) || !(mass > 0.0f)) return fail(MD_EINVAL, "dt and mass must be positive");
+    Pair pp;
+    int rc = make_pair(sys, pot, &pp);
+    if (rc) return rc;
+    if ((rc = enter(sys))) return rc;
+    Book book = {nullptr, nullptr, nullptr};
+    return launch_force(sys, pp, (const float4 *)pos, nbr_idx, nbr_count, (float4 *)force, (float4 *)vel,
+                        dt / (2.0f * mass), nullptr, false, book, (cudaStream_t)stream);
+}
+
 int md_half_kick(md_system *sys, void *vel, const void *force, float dt, float mass, void *stream) {
     if (!sys || !vel || !force) return fail(MD_EINVAL, "NULL argument");
     if (!aligned16(vel) || !aligned16(force)) return fail(MD_EINVAL, "vel/force must be 16-byte aligned");

@@ -114,9 +114,10 @@ class RankLoop:
     def force(self):
         self.S.compute_force(want_energy=False)
 
-    def finish(self):
-        w = self.S.w
-        self.B.md_half_kick(self.S.sys, self.S.vel, self.S.force, w.dt, w.mass)
+    def force_and_kick(self):
+        """The second half of the step in one launch (md_nve_step's own closing kernel)."""
+        S, w = self.S, self.S.w
+        self.B.md_force_half_kick(S.sys, S.pot, S.pos, S.nbr_idx, S.nbr_count, S.force, S.vel, w.dt, w.mass)
 
 
 def run(loop: RankLoop, exchange, nsteps: int) -> None:
@@ -125,8 +126,7 @@ def run(loop: RankLoop, exchange, nsteps: int) -> None:
         slots = exchange.all_gather(loop.move())
         if loop.absorb_positions(slots):
             loop.rebuild(exchange.all_gather(loop.velocity_slot()))
-        loop.force()
-        loop.finish()
+        loop.force_and_kick()
 
 
 def gather_state(loop: RankLoop, exchange) -> None:
@@ -147,8 +147,7 @@ def run_local(loops: list[RankLoop], nsteps: int) -> None:
             for lp in loops:
                 lp.rebuild(vel)
         for lp in loops:
-            lp.force()
-            lp.finish()
+            lp.force_and_kick()
 
 
 def gather_state_local(loops: list[RankLoop]) -> None:
