@@ -13,7 +13,7 @@ jittered lattice melts), 20 timed steps = twice the config's 1000 MD steps.
   roofline   the force kernel (dominant): algorithmic bytes (4*Kbar + 36) * N per launch
               over its average duration, L2 flushed before every launch,
              against MEASURED_PEAKS.json's hbm_gbs; `traffic` = DRAM bytes per launch from the
-             committed ncu capture (profiles/r1d_kernels.txt), config 3 only
+             committed ncu capture (profiles/r1f_kernels.txt), config 3 only
   cpu_baseline  the fp64 oracle's own list-based loop on the host cores, bounded sample
 
 `--impl reference` times the oracle (this tier's reference arm) instead.
@@ -40,8 +40,8 @@ METRIC = "LJ NVE particle-steps/sec at N=256k (incl. amortised rebuilds)"
 UNIT = "particle-steps/s"
 FALLBACK_HBM_GBS = 6650.0      # /opt/skills/guides/B200_PROFILING.md fallback
 # dram__bytes_read.sum + dram__bytes_write.sum of k_force_lj32 at N = 256,000, one ncu --set full
-# capture (profiles/r1d_kernels.txt: 91.16 MB + 3.87 MB)
-FORCE_TRAFFIC_CFG3 = 95.03e6
+# capture (profiles/r1f_kernels.txt: 91.33 MB + 3.91 MB)
+FORCE_TRAFFIC_CFG3 = 95.24e6
 
 
 def parse():
