@@ -1134,7 +1134,7 @@ def test_config3_long_run(B, orc, W):
     assert rebuilds >= 200
 
 
-@pytest.mark.parametrize("world,m,steps", [(2, 6, 100), (3, 6, 100), (4, 12, 60)])
+@pytest.mark.parametrize("world,m,steps", [(2, 6, 100), (3, 6, 100), (3, 7, 80), (4, 12, 60)])      # m = 7: 1372 particles, a ragged last tile
 def test_split_list_ranks_equal_one_gpu(B, W, world, m, steps):
     """SURVEY §8f-f1 (replicated positions, split list; decomposition.py): `world` contexts in one
     process, each owning a range of list tiles, stepped in lockstep with the all-gather replaced by a
