@@ -126,8 +126,7 @@ int md_set_species_lj(md_system *sys, int nspecies, const float *epsilon, const 
  *
  * md_set_range: this context owns particles [begin, end): begin a multiple of 32 (a list tile), end a
  * multiple of 32 or n.  From then on md_neighbor_list_build writes rows, counts and rebuild references of
- * that range only, md_pair_energy_force (3-D Lennard-Jones fast path) forces, e_i and the energy sum of that
- * range only; md_cell_list_build stays global; the step calls (md_nve_step, ...) return MD_EINVAL -- the
+ * that range only, md_pair_energy_force forces, e_i and the energy sum of that range only; md_cell_list_build stays global; the step calls (md_nve_step, ...) return MD_EINVAL -- the
  * step is driven from outside with the two calls below around the exchange.  [0, n) restores the default.
  */
 int md_set_range(md_system *sys, int begin, int end);

@@ -346,18 +346,20 @@ template <int KIND, int DIM, bool ENERGY>
 int launch_force_t(md_system *s, const Pair &pp, const float4 *pos, const int *nbr_idx,
                    const int *nbr_count, float4 *force, float4 *vel, float a, double *etot,
                    Book book, cudaStream_t st) {
-    const Geom &g = s->g;
+    Geom g = s->g;
+    g.n = s->r1;                    // md_set_range: particles [r0, r1) of this context
+    const int m = s->r1 - s->r0;
     if (s->tpp == 0) {          // streaming kernel: one lane per particle, one warp per list tile
-        k_force_stream<KIND, DIM, ENERGY><<<blocks_for(g.n, FS_WARPS * 32), FS_WARPS * 32, 0, st>>>(
-            g, pp, pos, nbr_idx, nbr_count, force, vel, a, etot, book);
+        k_force_stream<KIND, DIM, ENERGY><<<blocks_for(m, FS_WARPS * 32), FS_WARPS * 32, 0, st>>>(
+            g, pp, pos, nbr_idx, nbr_count, force, vel, a, etot, book, s->r0);
         LAUNCH_OK();
         return MD_OK;
     }
-    const int nb = blocks_for((long long)g.n * s->tpp, 128);
+    const int nb = blocks_for((long long)m * s->tpp, 128);
 #define MD_FORCE_CASE(T)                                                                       \
     case T:                                                                                    \
         k_force<KIND, DIM, T, ENERGY><<<nb, 128, 0, st>>>(g, pp, pos, nbr_idx, nbr_count,     \
-                                                          force, vel, a, etot, book);         \
+                                                          force, vel, a, etot, book, s->r0);  \
         break;
     switch (s->tpp) {
         MD_FORCE_CASE(1) MD_FORCE_CASE(2) MD_FORCE_CASE(4)
@@ -393,8 +395,6 @@ int launch_force(md_system *s, const Pair &pp, const float4 *pos, const int *nbr
         LAUNCH_OK();
         return MD_OK;
     }
-    if (s->r0 != 0 || s->r1 != s->g.n)
-        return fail(MD_EINVAL, "md_set_range: only the 3-D Lennard-Jones fast path computes forces of a range");
 #define MD_FORCE_DISPATCH(K, D)                                                                 \
     (want_energy ? launch_force_t<K, D, true>(s, pp, pos, nbr_idx, nbr_count, force, vel, a,   \
                                               etot, book, st)                                  \

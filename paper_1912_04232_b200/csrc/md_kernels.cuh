@@ -881,10 +881,10 @@ template <int KIND, int DIM, int TPP, bool ENERGY>
 __global__ void __launch_bounds__(128)
 k_force(Geom g, Pair pp, const float4 *__restrict__ pos, const int *__restrict__ nbr_idx,
         const int *__restrict__ nbr_count, float4 *__restrict__ force, float4 *__restrict__ vel,
-        float a, double *energy_total, Book book) {
+        float a, double *energy_total, Book book, int i0) {
     __shared__ double sp[KIND == 4 || KIND == 5 ? SP_TAB : 1];
     if (KIND == 4 || KIND == 5) species_tables_to_shared(pp, sp);
-    const int gid = blockIdx.x * blockDim.x + threadIdx.x;
+    const int gid = i0 * TPP + blockIdx.x * blockDim.x + threadIdx.x;     // i0: first particle of the range
     const int i = gid / TPP, sub = gid % TPP;
     const bool active = i < g.n;
     const int ii = active ? i : g.n - 1;
@@ -950,13 +950,13 @@ template <int KIND, int DIM, bool ENERGY>
 __global__ void __launch_bounds__(FS_WARPS * 32)
 k_force_stream(Geom g, Pair pp, const float4 *__restrict__ pos, const int *__restrict__ nbr_idx,
                const int *__restrict__ nbr_count, float4 *__restrict__ force,
-               float4 *__restrict__ vel, float a, double *energy_total, Book book) {
+               float4 *__restrict__ vel, float a, double *energy_total, Book book, int i0) {
     __shared__ __align__(128) int s_idx[FS_WARPS][FS_STAGES][FS_ROWS * TILE];
     __shared__ __align__(8) unsigned long long s_bar[FS_WARPS][FS_STAGES];
     __shared__ double sp[KIND == 4 || KIND == 5 ? SP_TAB : 1];
     if (KIND == 4 || KIND == 5) species_tables_to_shared(pp, sp);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int gid = blockIdx.x * blockDim.x + threadIdx.x;
+    const int gid = i0 + blockIdx.x * blockDim.x + threadIdx.x;
     const int i = gid;
     const bool active = i < g.n;
     const int ii = active ? i : g.n - 1;

@@ -1177,3 +1177,46 @@ def test_split_list_ranks_equal_one_gpu(B, W, world, m, steps):
     for lp in loops:
         lp.S.close()
     one.close()
+
+
+@pytest.mark.parametrize("which", ["soft2d", "morse3d", "lj64"])
+def test_split_list_ranks_other_kernels(B, W, which):
+    """The range offset of the generic force kernels (fp64 pair chain, 2-D, threads-per-particle variants):
+    three ranks in lockstep against one context, bit for bit."""
+    from paper_1912_04232_b200 import decomposition as D
+    if which == "soft2d":
+        w = W.soft_disks(1, 3000)
+        rng = np.random.default_rng(2)
+        v = np.zeros_like(w.vel); v[:, :2] = rng.normal(0, 0.05, (w.n, 2)).astype(np.float32)
+        w = dataclasses.replace(w, vel=v, dt=0.02)
+        opts = {}
+    elif which == "morse3d":
+        w = dataclasses.replace(W.lj_fcc(0, 7, seed=5), kind=W.KIND_MORSE, sigma=1.12, alpha=5.0)
+        opts = {"threads_per_particle": 2}
+    else:
+        w = W.lj_fcc(0, 7, seed=5)
+        opts = {"fast32": 0, "threads_per_particle": 0}
+    steps, world = 80, 3
+
+    def make():
+        S = B.System(w)
+        for k, val in opts.items():
+            B.md_set_option(S.sys, k, val)
+        return S
+
+    one = make()
+    one.build(); one.compute_force()
+    one.step(steps)
+    torch.cuda.synchronize()
+    loops = [D.RankLoop(make(), r, world) for r in range(world)]
+    for lp in loops:
+        lp.start()
+    D.run_local(loops, steps)
+    D.gather_state_local(loops)
+    torch.cuda.synchronize()
+    for lp in loops:
+        assert lp.rebuilds == int(one.stats[1])
+        assert torch.equal(lp.S.pos, one.pos) and torch.equal(lp.S.vel, one.vel) and torch.equal(lp.S.id, one.id)
+        assert torch.equal(lp.S.force[:, :3], one.force[:, :3])
+        lp.S.close()
+    one.close()
