@@ -286,6 +286,15 @@ def run_next_rows(args):
     emit("f4", "flocking (align + avoid + cohesion), forward Euler", us, steps=steps, n=nb,
          rebuilds=int(S.stats[1]), mean_neighbors=float(S.nbr_count.float().mean()))
     S.close()
+    S = B.System(w); S.build()
+    cen = rng.uniform(5.0, float(L) - 5.0, (16, 2)).astype(np.float32)
+    B.md_flock_obstacles(S.sys, cen, np.full(16, 4.0, np.float32), 4.0)
+    pred = torch.zeros(16, 4, dtype=torch.float32, device=dev)
+    pred[:, :2] = torch.from_numpy(rng.uniform(5.0, float(L) - 5.0, (16, 2)).astype(np.float32)).to(dev)
+    B.md_flock_predators(S.sys, pred, B.md_predator_params(5.0, 4.0, 3.0, 12.0, 0.8))
+    us = time_rule(lambda k: B.md_flock_step(S.sys, par, S.pos, S.id, S.nbr_idx, S.nbr_count, 0.01, k, S.stats), steps)
+    emit("f4", "flocking + 16 disk obstacles + 16 predators", us, steps=steps, n=nb, rebuilds=int(S.stats[1]))
+    S.close()
 
 
 def run_decomposed(args):

@@ -98,6 +98,7 @@ struct md_system {
                          // [3] rebuild flag (odd steps), [8..15] counters
     int *scan_tmp;       // block sums + ticket of the two-launch cell scan
     double *fire_tmp;    // md_fire_minimize: per-block partial sums, then {c1, c2} as floats
+    double *pred_tmp;    // md_flock_predators: per-chunk partial sums (D_x, D_y, count)
     int *cell_count, *cell_start_i, *perm_i, *cell_of, *rank_tmp, *perm_tmp, *id_s;
     float4 *pos_s, *vel_s, *ref_pos, *pos_alt;   // pos_alt: second position buffer of the fused step
     // tuning
@@ -146,7 +147,7 @@ int enter(const md_system *s) {
 }
 
 struct Layout {
-    size_t words, scan_tmp, fire_tmp, cell_count, cell_start_i, perm_i, cell_of, rank_tmp, perm_tmp, id_s, pos_s,
+    size_t words, scan_tmp, fire_tmp, pred_tmp, cell_count, cell_start_i, perm_i, cell_of, rank_tmp, perm_tmp, id_s, pos_s,
         vel_s, ref_pos, pos_alt, total;
 };
 
@@ -157,6 +158,7 @@ Layout layout(int n, long long cells) {
     l.words = take(64 * sizeof(int));
     l.scan_tmp = take((size_t)((cells + SCAN_CHUNK - 1) / SCAN_CHUNK + 2) * sizeof(int));
     l.fire_tmp = take(((size_t)(n + FIRE_BLOCK - 1) / FIRE_BLOCK * 3 + 2) * sizeof(double));
+    l.pred_tmp = take((size_t)FLOCK_PRED_CHUNKS * MD_MAX_PREDATORS * 3 * sizeof(double));
     l.cell_count = take((size_t)(cells + 4) * sizeof(int));
     l.cell_start_i = take((size_t)(cells + 1) * sizeof(int));
     l.perm_i = take((size_t)n * sizeof(int));
@@ -648,7 +650,10 @@ int record_rule_step(md_system *s, const Pair &pp, const RuleArgs &A, cudaStream
 #undef FLOCK_PASS1
         k_flock_pass2<<<nbp, 128, 0, st>>>(g, fq, p4, A.nbr_idx, A.nbr_count, s->vel_s, s->pos_alt);
         if (A.npred > 0) {
-#define FLOCK_PRED(AI) k_flock_predators<AI><<<A.npred, 256, 0, st>>>(g, fq, p4, (float4 *)A.pred, A.dt)
+            const int nchunk = std::max(1, std::min(FLOCK_PRED_CHUNKS, g.n / 1024));
+            double *part = s->pred_tmp;
+            k_flock_pred_partial<<<dim3(nchunk, A.npred), 256, 0, st>>>(g, fq, p4, (const float4 *)A.pred, part);
+#define FLOCK_PRED(AI) k_flock_predators<AI><<<A.npred, 32, 0, st>>>(g, fq, (float4 *)A.pred, part, nchunk, A.dt)
             if ((float)ai != A.flock.alpha) FLOCK_PRED(0);
             else if (ai == 1) FLOCK_PRED(1);
             else if (ai == 2) FLOCK_PRED(2);
@@ -787,6 +792,7 @@ int md_create(const md_config *cfg, int n, void *workspace, size_t bytes, md_sys
     s->words = (int *)(s->ws + l.words);
     s->scan_tmp = (int *)(s->ws + l.scan_tmp);
     s->fire_tmp = (double *)(s->ws + l.fire_tmp);
+    s->pred_tmp = (double *)(s->ws + l.pred_tmp);
     s->cell_count = (int *)(s->ws + l.cell_count);
     s->cell_start_i = (int *)(s->ws + l.cell_start_i);
     s->perm_i = (int *)(s->ws + l.perm_i);

@@ -53,9 +53,10 @@ __device__ __forceinline__ void flock_disk_term(const Geom &g, const FlockPar &f
                                                 double &gx, double &gy, double &gt) {
     double dx, dy;
     flock_disp(g, pi, make_float4(cx, cy, 0.0f, 0.0f), dx, dy);                      // R - C
-    const double r = sqrt(dx * dx + dy * dy);
-    if (r < D && r > 0.0) {
-        const double ux = -dx / r, uy = -dy / r, c = ci * ux + si * uy, x = 1.0 - r / D;
+    const double r2 = dx * dx + dy * dy;
+    if (r2 < D * D && r2 > 0.0) {                     // most boids are outside most disks: no root for them
+        const double r = sqrt(r2);
+        const double ux = -dx / r, uy = -dy / r, c = ci * ux + si * uy, x = fmax(1.0 - r / D, 0.0);
         const double rho = flock_pow<AI, false>(x, fp.alpha) / fp.alpha;
         const double drho = -flock_pow<AI, true>(x, fp.alpha) / D;
         gt += 2.0 * J * rho * (1.0 + c) * (-si * ux + ci * uy);
@@ -169,33 +170,53 @@ k_flock_pass2(Geom g, FlockPar fp, const float4 *__restrict__ pos, const int *__
     acc[i] = a;
 }
 
-// Predators (eq. 13): block p sums D_p = sum over boids within R_chase of (R_i - R_p) in a fixed order,
-// then one thread takes the chase gradient, adds the obstacles, and moves the predator by forward Euler.
-// Runs after the boids' passes (which read the old predator state) and before the boids' update (this
-// kernel reads the old boid positions).
-template <int AI>
+// Predators (eq. 13), two stages so that the sum over all boids uses the whole GPU and still has a fixed
+// order: block (c, p) sums its chunk of boids within R_chase of predator p into part[(p * nchunk + c) * 3],
+// then one warp per predator adds the chunks in order, takes the chase gradient, adds the obstacles and
+// moves the predator by forward Euler.  Both run after the boids' passes (which read the old predator
+// state) and before the boids' update (they read the old boid positions).
+constexpr int FLOCK_PRED_CHUNKS = 64;
+
 __global__ void __launch_bounds__(256)
-k_flock_predators(Geom g, FlockPar fp, const float4 *__restrict__ pos, float4 *pred, float dt) {
-    __shared__ double sx[8], sy[8];
-    __shared__ int sm[8];
-    const int p = blockIdx.x, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+k_flock_pred_partial(Geom g, FlockPar fp, const float4 *__restrict__ pos, const float4 *__restrict__ pred,
+                     double *__restrict__ part) {
+    __shared__ double sx[8], sy[8], sm[8];
+    const int p = blockIdx.y, lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const float4 q = pred[p];
     const double R2 = fp.Rch * fp.Rch;
-    double Dx = 0.0, Dy = 0.0;
-    int m = 0;
-    for (int i = threadIdx.x; i < g.n; i += 256) {
+    const int per = (g.n + gridDim.x - 1) / gridDim.x;
+    const int i1 = min(g.n, (int)(blockIdx.x + 1) * per);
+    double Dx = 0.0, Dy = 0.0, m = 0.0;
+    for (int i = blockIdx.x * per + threadIdx.x; i < i1; i += 256) {
         double dx, dy;
         flock_disp(g, pos[i], q, dx, dy);                                            // R_i - R_p
-        if (dx * dx + dy * dy < R2) { Dx += dx; Dy += dy; ++m; }
+        if (dx * dx + dy * dy < R2) { Dx += dx; Dy += dy; m += 1.0; }
     }
     for (int o = 16; o > 0; o >>= 1) {
         Dx += __shfl_xor_sync(FULL, Dx, o); Dy += __shfl_xor_sync(FULL, Dy, o); m += __shfl_xor_sync(FULL, m, o);
     }
     if (lane == 0) { sx[warp] = Dx; sy[warp] = Dy; sm[warp] = m; }
     __syncthreads();
+    if (threadIdx.x == 0) {
+        Dx = Dy = m = 0.0;
+        for (int w = 0; w < 8; ++w) { Dx += sx[w]; Dy += sy[w]; m += sm[w]; }
+        double *out = part + ((size_t)p * gridDim.x + blockIdx.x) * 3;
+        out[0] = Dx; out[1] = Dy; out[2] = m;
+    }
+}
+
+template <int AI>
+__global__ void __launch_bounds__(32)
+k_flock_predators(Geom g, FlockPar fp, float4 *pred, const double *__restrict__ part, int nchunk, float dt) {
+    const int p = blockIdx.x;
     if (threadIdx.x != 0) return;
-    Dx = Dy = 0.0; m = 0;
-    for (int w = 0; w < 8; ++w) { Dx += sx[w]; Dy += sy[w]; m += sm[w]; }
+    const float4 q = pred[p];
+    double Dx = 0.0, Dy = 0.0, md = 0.0;
+    for (int c = 0; c < nchunk; ++c) {
+        const double *in = part + ((size_t)p * nchunk + c) * 3;
+        Dx += in[0]; Dy += in[1]; md += in[2];
+    }
+    const int m = (int)md;
     double sn, cp;
     sincos((double)q.w, &sn, &cp);
     double gx = 0.0, gy = 0.0, gt = 0.0;
