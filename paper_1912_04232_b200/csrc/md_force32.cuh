@@ -76,6 +76,36 @@ __device__ __forceinline__ void lj_pair32(const Pair32 &pp, float dx, float dy, 
     }
 }
 
+// Two list entries of one particle at once with packed fp32x2 arithmetic (FADD2 / FMUL2 / FFMA2:
+// one instruction, two lanes of data), the same operations in the same order as lj_pair32 -- so the
+// bits of every pair term are those of the scalar form.  Outside the cutoff (and for the far-away
+// point that stands in for a missing slot) 1/r2 is multiplied by 0: every power and the coefficient
+// vanish with it, no later select.
+struct Acc2s { float2 fx, fy, fz, s, e; float near; };
+
+template <bool ENERGY>
+__device__ __forceinline__ void lj_pair32x2(const Pair32 &pp, float2 dx, float2 dy, float2 dz, Acc2s &a) {
+    const float2 r2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
+    const float2 w = __fadd2_rn(r2, make_float2(-pp.rc2, -pp.rc2));
+    a.near = fminf(a.near, fminf(fabsf(w.x), fabsf(w.y)));
+    const float2 m = make_float2(w.x < 0.0f ? 1.0f : 0.0f, w.y < 0.0f ? 1.0f : 0.0f);
+    const float2 y = __fmul2_rn(make_float2(rcp32(r2.x), rcp32(r2.y)), m);
+    const float2 y2 = __fmul2_rn(y, y);
+    const float2 y3 = __fmul2_rn(y2, y);
+    const float2 t = __ffma2_rn(make_float2(pp.sig6x2, pp.sig6x2), y3, make_float2(-1.0f, -1.0f));
+    const float2 y4 = __fmul2_rn(y2, y2);
+    const float2 c = __fmul2_rn(y4, t);
+    a.fx = __ffma2_rn(c, dx, a.fx); a.fy = __ffma2_rn(c, dy, a.fy); a.fz = __ffma2_rn(c, dz, a.fz);
+    a.s = __ffma2_rn(y4, make_float2(fmaxf(fabsf(t.x), 0.2f), fmaxf(fabsf(t.y), 0.2f)), a.s);
+    if (ENERGY) {
+        const float hs = 0.5f * pp.sig6x2;
+        const float2 s6 = __fmul2_rn(make_float2(hs, hs), y3);
+        float2 e = __ffma2_rn(s6, s6, make_float2(-s6.x, -s6.y));
+        e = __ffma2_rn(m, make_float2(-pp.ucut4, -pp.ucut4), e);
+        a.e = __fadd2_rn(a.e, e);
+    }
+}
+
 // Exact re-evaluation of one particle by a group of G = 8, 16 or 32 lanes striding over its row
 // (32 / G particles per warp at a time); the sum is returned in every lane of the group.
 template <bool ENERGY, bool WRAP>
@@ -101,8 +131,17 @@ __device__ __forceinline__ Acc64 lj_row64(const Geom &g, const Pair &pp,
     return acc;
 }
 
-constexpr int F32_WARPS = 4;
-constexpr int F32_U = 4;
+#ifndef MD_F32_WARPS
+#define MD_F32_WARPS 2
+#endif
+#ifndef MD_F32_MINBLOCKS
+#define MD_F32_MINBLOCKS 14
+#endif
+constexpr int F32_WARPS = MD_F32_WARPS;
+#ifndef MD_F32_U
+#define MD_F32_U 4
+#endif
+constexpr int F32_U = MD_F32_U;
 
 // The pair loop of one lane over its column of the tile: rows [0, kmin) are owned by every lane
 // of the warp (no validity test), rows [kmin, kmax) are the ragged tail.  WX / WY / WZ: the warp
@@ -111,7 +150,10 @@ template <bool ENERGY, bool WX, bool WY, bool WZ>
 __device__ __forceinline__ void lj_rows32(const Geom &g, const Pair32 &p32,
                                           const float4 *__restrict__ pos, const int *col,
                                           const float4 &pi, int ii, int cnt, int kmin, int kmax,
-                                          Acc32 &acc) {
+                                          bool active, Acc32 &acc) {
+    // an idle lane of a ragged last tile owns no column: it loads no index (its column may hold
+    // anything) and gathers its stand-in particle ii
+    const int kload = active ? kmax : 0;
     const float Lx = g.L[0], Ly = g.L[1], Lz = g.L[2];
     const float hx = g.h[0], hy = g.h[1], hz = g.h[2];
     const float pxL = pi.x - Lx, pyL = pi.y - Ly, pzL = pi.z - Lz;
@@ -120,10 +162,20 @@ __device__ __forceinline__ void lj_rows32(const Geom &g, const Pair32 &p32,
         dy = WY ? min_image_pre(pi.y, pyL, q.y, Ly, hy) : pi.y - q.y;
         dz = WZ ? min_image_pre(pi.z, pzL, q.z, Lz, hz) : pi.z - q.z;
     };
+    static_assert(F32_U % 2 == 0, "the pair loop takes two slots per packed evaluation");
+    Acc2s a2;
+    a2.fx = a2.fy = a2.fz = a2.s = a2.e = make_float2(0.0f, 0.0f);
+    a2.near = acc.near;
+    auto two = [&](const float4 &qa, const float4 &qb) {
+        float ax, ay, az, bx, by, bz;
+        disp(qa, ax, ay, az);
+        disp(qb, bx, by, bz);
+        lj_pair32x2<ENERGY>(p32, make_float2(ax, bx), make_float2(ay, by), make_float2(az, bz), a2);
+    };
     int k = 0;
     int jn[F32_U];
 #pragma unroll
-    for (int u = 0; u < F32_U; ++u) jn[u] = u < kmax ? col[u * TILE] : ii;
+    for (int u = 0; u < F32_U; ++u) jn[u] = u < kload ? col[u * TILE] : ii;
     for (; k < kmin; k += F32_U) {
         int j[F32_U]; float4 q[F32_U];
 #pragma unroll
@@ -131,14 +183,12 @@ __device__ __forceinline__ void lj_rows32(const Geom &g, const Pair32 &p32,
 #pragma unroll
         for (int u = 0; u < F32_U; ++u) q[u] = pos[j[u]];
 #pragma unroll
-        for (int u = 0; u < F32_U; ++u) jn[u] = k + F32_U + u < kmax ? col[(k + F32_U + u) * TILE] : ii;
+        for (int u = 0; u < F32_U; ++u) jn[u] = k + F32_U + u < kload ? col[(k + F32_U + u) * TILE] : ii;
 #pragma unroll
-        for (int u = 0; u < F32_U; ++u) {
-            float dx, dy, dz;
-            disp(q[u], dx, dy, dz);
-            lj_pair32<ENERGY, false>(p32, dx, dy, dz, true, acc);
-        }
+        for (int u = 0; u < F32_U; u += 2) two(q[u], q[u + 1]);
     }
+    // ragged tail: a slot this lane does not own reads the lane's own position (a valid address)
+    // and is then moved 1e18 away, where it contributes exactly zero
     for (; k < kmax; k += F32_U) {
         int j[F32_U]; float4 q[F32_U];
 #pragma unroll
@@ -146,14 +196,14 @@ __device__ __forceinline__ void lj_rows32(const Geom &g, const Pair32 &p32,
 #pragma unroll
         for (int u = 0; u < F32_U; ++u) q[u] = pos[j[u]];
 #pragma unroll
-        for (int u = 0; u < F32_U; ++u) jn[u] = k + F32_U + u < kmax ? col[(k + F32_U + u) * TILE] : ii;
+        for (int u = 0; u < F32_U; ++u) jn[u] = k + F32_U + u < kload ? col[(k + F32_U + u) * TILE] : ii;
 #pragma unroll
-        for (int u = 0; u < F32_U; ++u) {
-            float dx, dy, dz;
-            disp(q[u], dx, dy, dz);
-            lj_pair32<ENERGY, true>(p32, dx, dy, dz, k + u < cnt, acc);
-        }
+        for (int u = 0; u < F32_U; ++u) if (!(k + u < cnt)) q[u].x = 1e18f;
+#pragma unroll
+        for (int u = 0; u < F32_U; u += 2) two(q[u], q[u + 1]);
     }
+    acc.fx += a2.fx.x + a2.fx.y; acc.fy += a2.fy.x + a2.fy.y; acc.fz += a2.fz.x + a2.fz.y;
+    acc.s += a2.s.x + a2.s.y; acc.e += a2.e.x + a2.e.y; acc.near = a2.near;
 }
 
 // vel != NULL: also the second half-kick v += a F.  energy_total != NULL (ENERGY only): adds
@@ -173,7 +223,7 @@ struct NextStep {
     int has_cond;
 };
 template <bool ENERGY>
-__global__ void __launch_bounds__(F32_WARPS * 32)
+__global__ void __launch_bounds__(F32_WARPS * 32, MD_F32_MINBLOCKS)
 k_force_lj32(Geom g, Pair pp, Pair32 p32, const float4 *__restrict__ pos,
              const int *__restrict__ nbr_idx, const int *__restrict__ nbr_count,
              float4 *__restrict__ force, float4 *__restrict__ vel, float a, double *energy_total,
@@ -202,11 +252,11 @@ k_force_lj32(Geom g, Pair pp, Pair32 p32, const float4 *__restrict__ pos,
     const bool wz = __any_sync(FULL, active && (pi.z < g.face || pi.z > g.L[2] - g.face));
     Acc32 acc = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 1e30f};
 
-    if (!(wx || wy || wz)) lj_rows32<ENERGY, false, false, false>(g, p32, pos, col, pi, ii, cnt, kmin, kmax, acc);
-    else if (wx && !wy && !wz) lj_rows32<ENERGY, true, false, false>(g, p32, pos, col, pi, ii, cnt, kmin, kmax, acc);
-    else if (!wx && wy && !wz) lj_rows32<ENERGY, false, true, false>(g, p32, pos, col, pi, ii, cnt, kmin, kmax, acc);
-    else if (!wx && !wy && wz) lj_rows32<ENERGY, false, false, true>(g, p32, pos, col, pi, ii, cnt, kmin, kmax, acc);
-    else lj_rows32<ENERGY, true, true, true>(g, p32, pos, col, pi, ii, cnt, kmin, kmax, acc);
+    if (!(wx || wy || wz)) lj_rows32<ENERGY, false, false, false>(g, p32, pos, col, pi, ii, cnt, kmin, kmax, active, acc);
+    else if (wx && !wy && !wz) lj_rows32<ENERGY, true, false, false>(g, p32, pos, col, pi, ii, cnt, kmin, kmax, active, acc);
+    else if (!wx && wy && !wz) lj_rows32<ENERGY, false, true, false>(g, p32, pos, col, pi, ii, cnt, kmin, kmax, active, acc);
+    else if (!wx && !wy && wz) lj_rows32<ENERGY, false, false, true>(g, p32, pos, col, pi, ii, cnt, kmin, kmax, active, acc);
+    else lj_rows32<ENERGY, true, true, true>(g, p32, pos, col, pi, ii, cnt, kmin, kmax, active, acc);
 
     // ---- fp32 result, error estimate, exact re-evaluation of the lanes that need it
     float fx = p32.fscale * acc.fx, fy = p32.fscale * acc.fy, fz = p32.fscale * acc.fz;
