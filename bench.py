@@ -10,10 +10,14 @@ jittered lattice melts), 20 timed steps = twice the config's 1000 MD steps.
              L2 flushed between bench steps (not timed), max over ranks
   e2e        the same metric through md_nve_run_host: pinned HOST buffers in, host buffers
              out, H2D + list build + steps + D2H all inside the timed region
-  roofline   the force kernel (dominant): algorithmic bytes (4*Kbar + 36) * N per launch
-              over its average duration, L2 flushed before every launch,
-             against MEASURED_PEAKS.json's hbm_gbs; `traffic` = DRAM bytes per launch from the
-             committed ncu capture (profiles/r1f_kernels.txt), config 3 only
+  roofline   the force kernel (dominant) in the variant the step loop runs (no energy, second
+             half-kick in the epilogue: md_force_half_kick): algorithmic bytes (4*Kbar + 68) * N
+             per launch (SURVEY 8d / DESIGN.md §6) over its median duration, L2 flushed before
+             every launch, against MEASURED_PEAKS.json's hbm_gbs; `traffic` = DRAM bytes per
+             launch read from profiles/r2_traffic.json (one ncu --set full capture; the file
+             names the capture and the build it was taken on), null when there is none for the config
+  survey_timing  SURVEY 8(d)'s protocol beside the contract's: initial state restored, 50 warm-up
+             steps, the config's own step count in ONE md_nve_step call, 5 repeats, median
   cpu_baseline  the fp64 oracle's own list-based loop on the host cores, bounded sample
 
 `--impl reference` times the oracle (this tier's reference arm) instead.
@@ -39,9 +43,17 @@ sys.path.insert(0, ROOT)
 METRIC = "LJ NVE particle-steps/sec at N=256k (incl. amortised rebuilds)"
 UNIT = "particle-steps/s"
 FALLBACK_HBM_GBS = 6650.0      # /opt/skills/guides/B200_PROFILING.md fallback
-# dram__bytes_read.sum + dram__bytes_write.sum of k_force_lj32 at N = 256,000, one ncu --set full
-# capture (profiles/r1f_kernels.txt: 91.33 MB + 3.91 MB)
-FORCE_TRAFFIC_CFG3 = 95.24e6
+CONFIG_STEPS = {0: 100, 1: 1000, 2: 1000, 3: 1000, 4: 500}      # BASELINE.json: each config's own run length
+
+
+def measured_traffic(config):
+    """DRAM bytes per launch of the force kernel from the committed ncu capture, with its source."""
+    p = os.path.join(ROOT, "profiles", "r2_traffic.json")
+    try:
+        t = json.load(open(p))[str(config)]
+        return float(t["dram_bytes_per_launch"]), t["source"]
+    except Exception:
+        return None, None
 
 
 def parse():
@@ -59,7 +71,10 @@ def parse():
                          "strong scaling; not the contract line")
     ap.add_argument("--next-rows", action="store_true",
                     help="time the SURVEY 8(f) rows instead (one JSON line per row; not the contract line)")
-    ap.add_argument("--breakdown", action="store_true", help="(kept for compatibility: the build time per rebuild is always reported)")
+    ap.add_argument("--no-graph", action="store_true",
+                    help="run md_nve_step as plain launches (same kernels, rebuild kernels return at once on a zero "
+                         "flag): what a profiler can list kernel by kernel; not the contract line")
+    ap.add_argument("--no-survey-timing", action="store_true")
     return ap.parse_args()
 
 
@@ -365,8 +380,25 @@ def run_decomposed(args):
         dist.destroy_process_group()
 
 
+def respawn_under_torchrun(args):
+    """`python bench.py --gpus N` without torchrun: start N ranks on this node ourselves."""
+    import socket
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", f"--nproc-per-node={args.gpus}",
+           "--master-addr", "127.0.0.1", "--master-port", str(port), os.path.abspath(__file__)] + sys.argv[1:]
+    raise SystemExit(subprocess.call(cmd))
+
+
 def main():
     args = parse()
+    if args.gpus < 1:
+        raise SystemExit("--gpus must be >= 1")
+    if "WORLD_SIZE" not in os.environ and args.gpus > 1:
+        return respawn_under_torchrun(args)
+    if int(os.environ.get("WORLD_SIZE", "1")) != args.gpus:
+        raise SystemExit(f"--gpus {args.gpus} but WORLD_SIZE={os.environ.get('WORLD_SIZE', '1')}: launch one rank per GPU")
     if args.impl == "reference":
         return run_reference(args)
     if args.next_rows:
@@ -385,6 +417,8 @@ def main():
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    if local >= torch.cuda.device_count():
+        raise SystemExit(f"rank {rank}: local rank {local} but only {torch.cuda.device_count()} CUDA device(s) here")
     torch.cuda.set_device(local)
     dev = torch.device("cuda", local)
     if world > 1:
@@ -394,6 +428,8 @@ def main():
     # replicas: rank r simulates an independent sample of the same config
     w = W.config(args.config, replica=R.replica_index(rank))
     S = B.System(w, device=dev)
+    if args.no_graph:
+        B.md_set_option(S.sys, "use_graph", 0)
     stream = torch.cuda.Stream(device=dev)
     flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # 2x the 126 MB L2
     md_steps = args.md_steps
@@ -430,21 +466,27 @@ def main():
         max_count = int(max(int(s[3]) for s in stats_acc))
         overflow = any(int(s[2]) >= 0 for s in stats_acc)
 
-        # ---- roofline of the force kernel: cold L2, event pair per launch
+        # ---- roofline of the force kernel: the loop's variant (no energy, half-kick in the epilogue,
+        # on a scratch copy of the velocities), cold L2, event pair per launch
         kbar = float(S.nbr_count.float().mean())
         reps = 30
+        vel_scratch = S.vel.clone()
+
+        def force_launch():
+            B.md_force_half_kick(S.sys, S.pot, S.pos, S.nbr_idx, S.nbr_count, S.force, vel_scratch, w.dt, w.mass, stream)
+
         fev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(reps)]
         for a, b in fev:
             flush.zero_()
             a.record(stream)
-            S.compute_force(False, stream)
+            force_launch()
             b.record(stream)
         torch.cuda.synchronize(dev)
         force_ms_cold = statistics.median(a.elapsed_time(b) for a, b in fev)
         a0, b0 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a0.record(stream)
         for _ in range(reps):
-            S.compute_force(False, stream)
+            force_launch()
         b0.record(stream)
         torch.cuda.synchronize(dev)
         force_ms_warm = a0.elapsed_time(b0) / reps
@@ -458,6 +500,26 @@ def main():
         torch.cuda.synchronize(dev)
         build_ms = statistics.median(a.elapsed_time(b) for a, b in bev)
         S.compute_force(False, stream)
+
+        # ---- initial state, 50 warm-up steps, the config's step count in one call, 5 repeats
+        survey = None
+        if not args.no_survey_timing:
+            nst = CONFIG_STEPS[args.config]
+            ts, rb = [], []
+            for _ in range(5):
+                S.reset()
+                S.build(stream); S.compute_force(False, stream)
+                S.step(50, stream)
+                a1, b1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                a1.record(stream)
+                S.step(nst, stream)
+                b1.record(stream)
+                torch.cuda.synchronize(dev)
+                ts.append(a1.elapsed_time(b1)); rb.append(int(S.stats[1]))
+            t_med = statistics.median(ts)
+            survey = {"md_steps": nst, "repeats": 5, "warmup_md_steps": 50, "state": "restored initial state per repeat",
+                      "median_ms": t_med, "us_per_md_step": 1e3 * t_med / nst,
+                      "particle_steps_per_s": w.n * nst / (t_med * 1e-3), "rebuilds": rb[len(rb) // 2]}
 
     ms_max = R.max_over_ranks(ms, dev)
     value = R.whole_job_rate(w.n * md_steps * args.steps, ms_max * 1e-3)
@@ -487,8 +549,9 @@ def main():
         return
 
     peak, peak_src = peaks()
+    traffic, traffic_src = measured_traffic(args.config)
     fused = (w.kind == W.KIND_LJ and w.dim == 3)      # the configs md_nve_step runs as fused graphs
-    algo_bytes = (4.0 * kbar + 36.0) * w.n
+    algo_bytes = (4.0 * kbar + 68.0) * w.n          # list + count + pos + vel read, force + vel written
     achieved = algo_bytes / (force_ms_cold * 1e-3) / 1e9
     step_bytes = (4.0 * kbar + 164.0) * w.n
     out = {
@@ -508,9 +571,10 @@ def main():
         "max_neighbors": max_count, "overflow": overflow,
         "step_hbm_frac": step_bytes / (1e3 * ms_max / (args.steps * md_steps) * 1e-6) / 1e9 / peak,
         "clocks": clocks,
-        "roofline": {"bound": "hbm", "kernel": "k_force_lj32 (md_pair_energy_force)", "achieved": achieved,
-                     "peak": peak, "unit": "GB/s", "frac": achieved / peak,
-                     "traffic": FORCE_TRAFFIC_CFG3 if args.config == 3 else None,
+        "roofline": {"bound": "hbm", "kernel": "force kernel of the step loop: no energy, second half-kick in the "
+                                               "epilogue (md_force_half_kick)" if fused else "force kernel (md_force_half_kick)",
+                     "achieved": achieved, "peak": peak, "unit": "GB/s", "frac": achieved / peak,
+                     "traffic": traffic, "traffic_source": traffic_src,
                      "peak_source": peak_src, "algorithmic_bytes": algo_bytes, "kbar": kbar,
                      "launch_ms_cold_l2": force_ms_cold, "launch_ms_warm_l2": force_ms_warm},
         # per bench step: k_init_stats + one force kernel per MD step + one k_kick_drift per graph
@@ -521,6 +585,14 @@ def main():
     }
     if build_ms is not None:
         out["build_ms_per_rebuild"] = build_ms
+        # BASELINE.json config 4 asks for these three side by side (reported for every config)
+        out["three_numbers"] = {"neighbor_build_us_per_rebuild": 1e3 * build_ms,
+                                "pair_force_us_per_step": 1e3 * force_ms_cold,
+                                "nve_particle_steps_per_s": value,
+                                "what": "cell list + re-sort + neighbor list through the API (cold L2) / the loop's force kernel "
+                                        "per launch (cold L2) / the whole loop incl. rebuilds"}
+    if survey is not None:
+        out["survey_timing"] = survey
     if e2e is not None:
         out["e2e"] = e2e
     if not args.no_cpu_baseline:

@@ -541,6 +541,42 @@ int record_fused(md_system *s, const Pair &pp, float4 *pos, float4 *vel, float4 
     return MD_OK;
 }
 
+// The fused step loop as plain launches (option use_graph = 0; what a profiler can list kernel by
+// kernel): the kernels and their order are those of record_fused, the rebuild kernels are launched
+// every step and return at once while the step's device flag is 0.  nsteps must be odd (the
+// position buffers swap nsteps - 1 times and the state must end in the caller's).
+int run_fused_direct(md_system *s, const Pair &pp, float4 *pos, float4 *vel, float4 *force, int *id,
+                     int *nbr_idx, int *nbr_count, float dt, float mass, int *stats, int nsteps,
+                     cudaStream_t st) {
+    const Geom &g = s->g;
+    const float a = dt / (2.0f * mass);
+    int *flags[2] = {s->words + 0, s->words + 3};
+    int *status = s->words + 1;
+    const bool resort = s->cfg.resort != 0;
+    cudaGraphConditionalHandle none = 0;
+    k_kick_drift<3, false><<<blocks_for(g.n), 256, 0, st>>>(g, pos, vel, force, s->ref_pos, a, dt, flags[0], none);
+    LAUNCH_OK();
+    float4 *cur = pos, *other = s->pos_alt;
+    for (int r = 0; r < nsteps; ++r) {
+        int *flag = flags[r & 1];
+        int rc = launch_cell_build(s, cur, vel, id, s->cell_start_i, s->perm_i, status, flag, st);
+        if (!rc) rc = launch_nbr_build(s, resort ? cur : s->pos_s, s->cell_start_i, resort ? nullptr : s->perm_i,
+                                       nbr_idx, nbr_count, status, flag, 1, st);
+        if (rc) return rc;
+        Book book = {flag, status, stats};
+        NextStep nx = NextStep();
+        if (r + 1 < nsteps) {
+            nx.pos_out = other; nx.ref = s->ref_pos; nx.dt = dt; nx.flag = flags[(r + 1) & 1];
+            nx.cond = none; nx.has_cond = 0;
+        }
+        rc = launch_force(s, pp, cur, nbr_idx, nbr_count, force, vel, a, nullptr, false, book, st, nx);
+        if (rc) return rc;
+        if (r + 1 < nsteps) std::swap(cur, other);
+    }
+    if (cur != pos) return fail(MD_EINVAL, "fused loop of %d steps does not end in the caller's buffer", nsteps);
+    return MD_OK;
+}
+
 void drop_graphs(md_system *s) {
     if (s->exec1) cudaGraphExecDestroy(s->exec1);
     if (s->execU) cudaGraphExecDestroy(s->execU);
@@ -814,8 +850,6 @@ int md_create(const md_config *cfg, int n, void *workspace, size_t bytes, md_sys
     s->fused = 1;
     s->est_thr = 8.0f;
     s->unroll = 9;      // odd: a fused graph swaps position buffers steps-1 times and must end in the caller's
-    if (const char *e = getenv("MD_B200_TPP")) { int t = atoi(e); if (t == 0 || t == 1 || t == 2 || t == 4) s->tpp = t; }
-    if (const char *e = getenv("MD_B200_NO_GRAPH")) s->use_graph = atoi(e) ? 0 : 1;
     {   // neighbor-list builder: one warp per tile, a capacity x 32 column block + a candidate
         // chunk of shared memory per warp; as many warps per block as fit (at most NB_WARPS)
         const size_t per_warp = nb_smem_per_warp(cfg->capacity);
@@ -1002,7 +1036,19 @@ int md_nve_step(md_system *sys, const md_potential *pot, void *pos, void *vel, v
     k_init_stats<<<1, 1, 0, st>>>(stats, sys->words + 0);
     LAUNCH_OK();
     if (!sys->use_graph) {
-        for (int s = 0; s < nsteps; ++s) {
+        int left = nsteps;
+        if (sys->fast32 && sys->fused && pp.kind == MD_KIND_LJ && sys->g.dim == 3 && left > 0) {
+            // fused loop over an odd number of steps; an even count takes its first step unfused
+            if (!(left & 1)) {
+                rc = record_step(sys, pp, (float4 *)pos, (float4 *)vel, (float4 *)force, id, nbr_idx,
+                                 nbr_count, dt, mass, stats, st, false);
+                if (rc) return rc;
+                --left;
+            }
+            return run_fused_direct(sys, pp, (float4 *)pos, (float4 *)vel, (float4 *)force, id, nbr_idx,
+                                    nbr_count, dt, mass, stats, left, st);
+        }
+        for (int s = 0; s < left; ++s) {
             rc = record_step(sys, pp, (float4 *)pos, (float4 *)vel, (float4 *)force, id, nbr_idx,
                              nbr_count, dt, mass, stats, st, false);
             if (rc) return rc;

@@ -166,7 +166,10 @@ k_cell_scan(int cells, int *__restrict__ cell_count, int *__restrict__ cell_star
 // exclusive offsets.  k_cell_scan2: every block scans its chunk again, adds its offset, writes
 // cell_start and zeroes the counters.
 constexpr int SCAN_CHUNK = 4096;           // counters per block: 1024 threads x 4
-constexpr int SCAN_ONE_BLOCK = 16384;      // up to this many cells k_cell_scan (one block) is used
+#ifndef MD_SCAN_ONE_BLOCK
+#define MD_SCAN_ONE_BLOCK 16384
+#endif
+constexpr int SCAN_ONE_BLOCK = MD_SCAN_ONE_BLOCK;      // up to this many cells k_cell_scan (one block) is used
 
 __device__ __forceinline__ int4 load4_counts(const int *cell_count, int c, int cells) {
     int4 v = make_int4(0, 0, 0, 0);

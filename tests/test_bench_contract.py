@@ -27,9 +27,24 @@ def test_reference_arm_prints_the_contract_line():
 
 def test_reference_arm_other_ranks_do_nothing():
     env = dict(os.environ, RANK="1", WORLD_SIZE="2")
-    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--steps", "1"],
-                         capture_output=True, text=True, timeout=120, env=env)
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2",
+                          "--steps", "1"], capture_output=True, text=True, timeout=120, env=env)
     assert out.returncode == 0 and out.stdout.strip() == ""
+
+
+def test_gpus_flag_must_match_the_launch():
+    """--gpus N is never silently ignored: under a launcher it must equal WORLD_SIZE, and without one
+    bench.py starts N ranks itself (which fail loudly on a box with fewer devices) instead of printing
+    a one-GPU line."""
+    env = dict(os.environ, RANK="0", WORLD_SIZE="1")
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "1"],
+                         capture_output=True, text=True, timeout=120, env=env)
+    assert out.returncode != 0 and "WORLD_SIZE" in (out.stderr + out.stdout)
+    env = {k: v for k, v in os.environ.items() if k not in ("RANK", "WORLD_SIZE", "LOCAL_RANK")}
+    out = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "1", "--warmup", "0",
+                          "--no-cpu-baseline", "--no-e2e"], capture_output=True, text=True, timeout=300, env=env)
+    assert out.returncode != 0
+    assert '"n_gpus": 1' not in out.stdout
 
 
 def test_clock_sampler_keeps_the_timed_region_only():
