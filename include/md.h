@@ -14,9 +14,12 @@
  *   - Pointers are DEVICE pointers unless the parameter says "host".  The
  *     caller owns every buffer, the workspace included; the library allocates
  *     no caller-visible memory and keeps no pointer past a call except the
- *     workspace and (md_nve_step only) a cached CUDA graph of the last call's
- *     arguments.  No call except md_create / md_destroy / md_nve_run_host
- *     synchronises with the host.
+ *     workspace and (md_nve_step and the other step calls) a cached CUDA graph of
+ *     the last call's arguments.  No call except md_create / md_destroy /
+ *     md_nve_run_host synchronises with the host.  No behaviour depends on
+ *     environment variables: every knob is an md_set_option.
+ *   - A call makes the device that owns the workspace current on the calling thread for
+ *     its own duration and restores the caller's current device before it returns.
  *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default
  *     stream).  Work is ordered on that stream only.
  *   - Particle arrays are float4[n], 16-byte aligned:
@@ -66,10 +69,13 @@ typedef struct md_config {
 
 /* Pair potential u(r) (L78 §3.2.2, L104 §3.3.2). */
 typedef struct md_potential {
-    int   kind;       /* MD_KIND_LJ | MD_KIND_SOFT */
+    int   kind;       /* MD_KIND_LJ | MD_KIND_SOFT | MD_KIND_MORSE | MD_KIND_BUCKINGHAM | MD_KIND_LJ_SPECIES |
+                         MD_KIND_BKS (the last two read their tables from md_set_species_lj / _bks) */
     float epsilon;
     float sigma;      /* LJ length; unused for SOFT (diameters come from pos.w) */
-    float r_cut;      /* LJ truncation radius (<= config r_cut); unused for SOFT */
+    float r_cut;      /* truncation radius (<= config r_cut); unused for SOFT, whose cutoff is the pair's own
+                         d_ij = (d_i + d_j) / 2: the caller keeps every d_ij <= config r_cut (the list radius),
+                         a larger overlap range is cut at the list (not checked: diameters are device data) */
     int   shift;      /* LJ, MORSE: 1 = u(r) - u(r_cut) for r < r_cut, 0 = plain truncation */
     float alpha;      /* MORSE: inverse width; sigma is its r0, epsilon its well depth D. Unused otherwise */
 } md_potential;
@@ -101,12 +107,14 @@ int md_destroy(md_system *sys);
  *                          position buffer, half-skin test); 0: k_kick_drift every step.  Same bits.
  *   "remap"                3-D LJ force kernel: blocks i and i + remap work on adjacent list tiles, so the
  *                          blocks one SM receives round-robin share gathered positions in L1 (default
- *                          37; 0 = block i works on tile block i)
+ *                          a quarter of the device's SM count; 0 = block i works on tile block i)
  *   "builder_parts"        warps that share one list tile in the builder: 1, 2, 4, or 0 (default) = 4 up to
  *                          65,536 particles, else 1
  *   "builder"              neighbor-list kernel: 2 (default) records hits in per-lane bit masks,
  *                          1 appends them to per-lane shared-memory columns (first design)
- *   "use_graph"            0: md_nve_step launches kernels directly instead of a CUDA graph
+ *   "use_graph"            0: the step calls launch their kernels directly instead of CUDA graphs -- the same
+ *                          kernels in the same order (so a profiler lists them one by one); the rebuild kernels
+ *                          are then launched every step and return at once while the step's device flag is 0
  *   "nh_chain"             thermostats in md_nose_hoover_step's chain, 1 (default) .. 8 */
 int md_set_option(md_system *sys, const char *name, double value);
 
@@ -124,7 +132,8 @@ int md_set_species_lj(md_system *sys, int nspecies, const float *epsilon, const 
  * every step (velocities at rebuilds).  The list -- 4 * capacity bytes per particle against 16 for a
  * position -- is what is split.
  *
- * md_set_range: this context owns particles [begin, end): begin a multiple of 32 (a list tile), end a
+ * md_set_range (needs a system created with resort = 1: a range is a range of the cell-sorted order; MD_EINVAL
+ * otherwise): this context owns particles [begin, end): begin a multiple of 32 (a list tile), end a
  * multiple of 32 or n.  From then on md_neighbor_list_build writes rows, counts and rebuild references of
  * that range only, md_pair_energy_force forces, e_i and the energy sum of that range only; md_cell_list_build stays global; the step calls (md_nve_step, ...) return MD_EINVAL -- the
  * step is driven from outside with the two calls below around the exchange.  [0, n) restores the default.

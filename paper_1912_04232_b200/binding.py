@@ -15,7 +15,7 @@ import torch
 from . import build as _build
 
 MD_OK, MD_EINVAL, MD_EBOX, MD_EWORKSPACE, MD_ECUDA = 0, -1, -2, -3, -4
-MD_KIND_LJ, MD_KIND_SOFT, MD_KIND_MORSE, MD_KIND_BUCKINGHAM, MD_KIND_LJ_SPECIES = 0, 1, 2, 3, 4
+MD_KIND_LJ, MD_KIND_SOFT, MD_KIND_MORSE, MD_KIND_BUCKINGHAM, MD_KIND_LJ_SPECIES, MD_KIND_BKS = 0, 1, 2, 3, 4, 5
 
 SYMBOLS = [
     "md_last_error", "md_workspace_bytes", "md_create", "md_destroy", "md_set_option",

@@ -137,14 +137,21 @@ struct md_system {
 
 namespace {
 
-// The library links its own (static) CUDA runtime: make the device that owns the workspace
-// current on the calling thread before touching streams or launching.
-int enter(const md_system *s) {
-    int cur = -1;
-    CU(cudaGetDevice(&cur));
-    if (cur != s->device) CU(cudaSetDevice(s->device));
-    return MD_OK;
-}
+// The library links its own (static) CUDA runtime: every ABI call makes the device that owns the
+// workspace current on the calling thread for its duration and puts the caller's device back on return.
+struct DeviceScope {
+    int prev, rc;
+    explicit DeviceScope(int device) : prev(-1), rc(MD_OK) {
+        cudaError_t e = cudaGetDevice(&prev);
+        if (e == cudaSuccess && prev != device) e = cudaSetDevice(device); else if (e == cudaSuccess) prev = -1;
+        if (e != cudaSuccess) { prev = -1; rc = fail(MD_ECUDA, "selecting device %d: %s", device, cudaGetErrorString(e)); }
+    }
+    ~DeviceScope() { if (prev >= 0) cudaSetDevice(prev); }
+    DeviceScope(const DeviceScope &) = delete;
+    DeviceScope &operator=(const DeviceScope &) = delete;
+};
+static_assert(sizeof(md_potential) == 24 && sizeof(md_fire_params) == 28 && sizeof(md_flock_params) == 32 &&
+              sizeof(md_predator_params) == 20, "graph keys are compared bytewise: these structs hold no padding");
 
 struct Layout {
     size_t words, scan_tmp, fire_tmp, pred_tmp, cell_count, cell_start_i, perm_i, cell_of, rank_tmp, perm_tmp, id_s, pos_s,
@@ -416,6 +423,11 @@ __global__ void k_init_stats(int *stats, int *words) {
     words[0] = 0; words[3] = 0;          // rebuild flags
 }
 
+// the noise stream of a stochastic rule: {seed, step0} as device words ([20], [21])
+__global__ void k_set_noise(int *words, unsigned seed, unsigned step0) {
+    words[20] = (int)seed; words[21] = (int)step0;
+}
+
 __global__ void k_unpermute(int n, const int *__restrict__ id, const float4 *__restrict__ a,
                             const float4 *__restrict__ b, const float4 *__restrict__ c,
                             float4 *__restrict__ ao, float4 *__restrict__ bo, float4 *__restrict__ co) {
@@ -640,15 +652,15 @@ int record_rule_step(md_system *s, const Pair &pp, const RuleArgs &A, cudaStream
         break;
     case RULE_BROWNIAN: {
         const float mu = A.dt / A.gamma, amp = std::sqrt(2.0f * A.kT * A.dt / A.gamma);
-        if (g.dim == 3) k_brownian_drift<3><<<nb, 256, 0, st>>>(g, p4, f4, A.id, s->ref_pos, mu, amp, A.seed, A.step0, A.stats, rs);
-        else k_brownian_drift<2><<<nb, 256, 0, st>>>(g, p4, f4, A.id, s->ref_pos, mu, amp, A.seed, A.step0, A.stats, rs);
+        if (g.dim == 3) k_brownian_drift<3><<<nb, 256, 0, st>>>(g, p4, f4, A.id, s->ref_pos, mu, amp, reinterpret_cast<const unsigned *>(s->words + 20), A.stats, rs);
+        else k_brownian_drift<2><<<nb, 256, 0, st>>>(g, p4, f4, A.id, s->ref_pos, mu, amp, reinterpret_cast<const unsigned *>(s->words + 20), A.stats, rs);
         break;
     }
     case RULE_LANGEVIN: {
         const double c1d = std::exp(-(double)A.gamma * (double)A.dt);
         const float c1 = (float)c1d, c2 = (float)std::sqrt((double)A.kT / (double)A.mass * (1.0 - c1d * c1d));
-        if (g.dim == 3) k_langevin_baoa<3><<<nb, 256, 0, st>>>(g, p4, v4, f4, A.id, s->ref_pos, a, A.dt, c1, c2, A.seed, A.step0, A.stats, rs);
-        else k_langevin_baoa<2><<<nb, 256, 0, st>>>(g, p4, v4, f4, A.id, s->ref_pos, a, A.dt, c1, c2, A.seed, A.step0, A.stats, rs);
+        if (g.dim == 3) k_langevin_baoa<3><<<nb, 256, 0, st>>>(g, p4, v4, f4, A.id, s->ref_pos, a, A.dt, c1, c2, reinterpret_cast<const unsigned *>(s->words + 20), A.stats, rs);
+        else k_langevin_baoa<2><<<nb, 256, 0, st>>>(g, p4, v4, f4, A.id, s->ref_pos, a, A.dt, c1, c2, reinterpret_cast<const unsigned *>(s->words + 20), A.stats, rs);
         force_vel = v4; force_a = a;
         break;
     }
@@ -764,7 +776,9 @@ int run_rule(md_system *s, const Pair &pp, RuleArgs &A, int nsteps, cudaStream_t
     if (s->r0 != 0 || s->r1 != s->g.n) return fail(MD_EINVAL, "a range is set (md_set_range): drive the step with md_kick_drift / md_half_kick");
     A.fast32 = s->fast32; A.builder = s->builder; A.nb_parts = s->nb_parts; A.remap = s->remap; A.est_thr = s->est_thr;
     k_init_stats<<<1, 1, 0, st>>>(A.stats, s->words + 0);
+    k_set_noise<<<1, 1, 0, st>>>(s->words, A.seed, A.step0);
     LAUNCH_OK();
+    A.seed = 0; A.step0 = 0;          // not part of what a captured graph depends on
     if (!s->use_graph) {
         for (int k = 0; k < nsteps; ++k) { int rc = record_rule_step(s, pp, A, st, false); if (rc) return rc; }
         return MD_OK;
@@ -819,7 +833,8 @@ int md_create(const md_config *cfg, int n, void *workspace, size_t bytes, md_sys
     CU(cudaPointerGetAttributes(&attr, workspace));
     if (attr.type != cudaMemoryTypeDevice && attr.type != cudaMemoryTypeManaged)
         return fail(MD_EWORKSPACE, "workspace is not device memory");
-    CU(cudaSetDevice(attr.device));
+    DeviceScope scope_(attr.device);
+    if (scope_.rc) return scope_.rc;
     md_system *s = new (std::nothrow) md_system;
     if (!s) return fail(MD_EINVAL, "out of host memory");
     memset(s, 0, sizeof(*s));
@@ -846,7 +861,11 @@ int md_create(const md_config *cfg, int n, void *workspace, size_t bytes, md_sys
     s->r0 = 0; s->r1 = n;
     s->fast32 = 1;
     s->builder = 2;
-    s->remap = 37;      // a quarter of the SM count measured best (46.7 -> 44.9 us at N = 256k)
+    {   // block -> tile remap period: a quarter of the SM count measured best (46.7 -> 44.9 us at N = 256k on 148 SMs)
+        int sms = 0;
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, attr.device);
+        s->remap = sms >= 4 ? sms / 4 : 0;
+    }
     s->fused = 1;
     s->est_thr = 8.0f;
     s->unroll = 9;      // odd: a fused graph swaps position buffers steps-1 times and must end in the caller's
@@ -884,6 +903,7 @@ int md_create(const md_config *cfg, int n, void *workspace, size_t bytes, md_sys
 
 int md_destroy(md_system *sys) {
     if (!sys) return MD_OK;
+    DeviceScope scope_(sys->device);
     drop_graphs(sys);
     if (sys->cap_stream) cudaStreamDestroy(sys->cap_stream);
     if (sys->body_stream) cudaStreamDestroy(sys->body_stream);
@@ -924,7 +944,8 @@ int md_set_species_lj(md_system *sys, int nspecies, const float *epsilon, const 
 
 int md_counters(md_system *sys, int32_t *out, int reset, void *stream) {
     if (!sys || !out) return fail(MD_EINVAL, "NULL argument");
-    if (int rc = enter(sys)) return rc;
+    DeviceScope scope_(sys->device);
+    if (scope_.rc) return scope_.rc;
     cudaStream_t st = (cudaStream_t)stream;
     CU(cudaMemcpyAsync(out, sys->words + 8, 8 * sizeof(int), cudaMemcpyDeviceToDevice, st));
     if (reset) CU(cudaMemsetAsync(sys->words + 8, 0, 8 * sizeof(int), st));
@@ -967,7 +988,8 @@ int md_cell_list_build(md_system *sys, void *pos, void *vel, int32_t *id, int32_
                        int32_t *perm, void *stream) {
     if (!sys || !pos || !cell_start || !perm) return fail(MD_EINVAL, "NULL argument");
     if (!aligned16(pos) || (vel && !aligned16(vel))) return fail(MD_EINVAL, "pos/vel must be 16-byte aligned");
-    if (int rc = enter(sys)) return rc;
+    DeviceScope scope_(sys->device);
+    if (scope_.rc) return scope_.rc;
     return launch_cell_build(sys, (float4 *)pos, (float4 *)vel, id, cell_start, perm, nullptr,
                              nullptr, (cudaStream_t)stream);
 }
@@ -978,7 +1000,8 @@ int md_neighbor_list_build(md_system *sys, const void *pos, const int32_t *cell_
     if (!sys || !pos || !cell_start || !perm || !nbr_idx || !nbr_count || !status)
         return fail(MD_EINVAL, "NULL argument");
     if (!aligned16(pos) || !aligned16(nbr_idx)) return fail(MD_EINVAL, "pos/nbr_idx must be 16-byte aligned");
-    if (int rc = enter(sys)) return rc;
+    DeviceScope scope_(sys->device);
+    if (scope_.rc) return scope_.rc;
     cudaStream_t st = (cudaStream_t)stream;
     CU(cudaMemsetAsync(status, 0, 2 * sizeof(int), st));
     const float4 *spos = (const float4 *)pos;
@@ -994,7 +1017,8 @@ int md_neighbor_list_build(md_system *sys, const void *pos, const int32_t *cell_
 int md_needs_rebuild(md_system *sys, const void *pos, int32_t *flag, void *stream) {
     if (!sys || !pos || !flag) return fail(MD_EINVAL, "NULL argument");
     if (!aligned16(pos)) return fail(MD_EINVAL, "pos must be 16-byte aligned");
-    if (int rc = enter(sys)) return rc;
+    DeviceScope scope_(sys->device);
+    if (scope_.rc) return scope_.rc;
     cudaStream_t st = (cudaStream_t)stream;
     CU(cudaMemsetAsync(flag, 0, sizeof(int), st));
     const int nb = blocks_for(sys->n);
@@ -1012,7 +1036,8 @@ int md_pair_energy_force(md_system *sys, const md_potential *pot, const void *po
     Pair pp;
     int rc = make_pair(sys, pot, &pp);
     if (rc) return rc;
-    if ((rc = enter(sys))) return rc;
+    DeviceScope scope_(sys->device);
+    if (scope_.rc) return scope_.rc;
     cudaStream_t st = (cudaStream_t)stream;
     if (energy_total) CU(cudaMemsetAsync(energy_total, 0, sizeof(double), st));
     Book book = {nullptr, nullptr, nullptr};
@@ -1031,7 +1056,8 @@ int md_nve_step(md_system *sys, const md_potential *pot, void *pos, void *vel, v
     Pair pp;
     int rc = make_pair(sys, pot, &pp);
     if (rc) return rc;
-    if ((rc = enter(sys))) return rc;
+    DeviceScope scope_(sys->device);
+    if (scope_.rc) return scope_.rc;
     cudaStream_t st = (cudaStream_t)stream;
     k_init_stats<<<1, 1, 0, st>>>(stats, sys->words + 0);
     LAUNCH_OK();
@@ -1088,7 +1114,8 @@ int md_brownian_step(md_system *sys, const md_potential *pot, void *pos, void *f
     Pair pp;
     int rc = make_pair(sys, pot, &pp);
     if (rc) return rc;
-    if ((rc = enter(sys))) return rc;
+    DeviceScope scope_(sys->device);
+    if (scope_.rc) return scope_.rc;
     RuleArgs A;
     memset(&A, 0, sizeof(A));
     A.rule = RULE_BROWNIAN; A.pos = pos; A.force = force; A.id = id; A.nbr_idx = nbr_idx; A.nbr_count = nbr_count;
@@ -1107,7 +1134,8 @@ int md_langevin_step(md_system *sys, const md_potential *pot, void *pos, void *v
     Pair pp;
     int rc = make_pair(sys, pot, &pp);
     if (rc) return rc;
-    if ((rc = enter(sys))) return rc;
+    DeviceScope scope_(sys->device);
+    if (scope_.rc) return scope_.rc;
     RuleArgs A;
     memset(&A, 0, sizeof(A));
     A.rule = RULE_LANGEVIN; A.pos = pos; A.vel = vel; A.force = force; A.id = id; A.nbr_idx = nbr_idx;
@@ -1127,7 +1155,8 @@ int md_nose_hoover_step(md_system *sys, const md_potential *pot, void *pos, void
     Pair pp;
     int rc = make_pair(sys, pot, &pp);
     if (rc) return rc;
-    if ((rc = enter(sys))) return rc;
+    DeviceScope scope_(sys->device);
+    if (scope_.rc) return scope_.rc;
     RuleArgs A;
     memset(&A, 0, sizeof(A));
     A.rule = RULE_NH; A.pos = pos; A.vel = vel; A.force = force; A.state = nh_state; A.id = id; A.nbr_idx = nbr_idx;
@@ -1138,6 +1167,10 @@ int md_nose_hoover_step(md_system *sys, const md_potential *pot, void *pos, void
 
 int md_set_range(md_system *sys, int begin, int end) {
     if (!sys) return fail(MD_EINVAL, "NULL argument");
+    // a range is a range of the cell-sorted order: without the physical re-sort the builder's rows,
+    // counts and reference positions of slots [begin, end) belong to particles anywhere in [0, n)
+    if (!sys->cfg.resort && !(begin == 0 && end == sys->n))
+        return fail(MD_EINVAL, "md_set_range needs a system created with resort = 1");
     if (begin < 0 || end > sys->n || begin >= end || begin % TILE != 0 || (end % TILE != 0 && end != sys->n))
         return fail(MD_EINVAL, "range [%d, %d) must be non-empty, inside [0, %d) and aligned to list tiles of %d", begin, end, sys->n, TILE);
     sys->r0 = begin; sys->r1 = end;
@@ -1150,7 +1183,8 @@ int md_kick_drift(md_system *sys, void *pos, void *vel, const void *force, float
     if (!sys || !pos || !vel || !force || !flag) return fail(MD_EINVAL, "NULL argument");
     if (!aligned16(pos) || !aligned16(vel) || !aligned16(force)) return fail(MD_EINVAL, "pos/vel/force must be 16-byte aligned");
     if (!(dt > 0.0f) || !(mass > 0.0f)) return fail(MD_EINVAL, "dt and mass must be positive");
-    if (int rc = enter(sys)) return rc;
+    DeviceScope scope_(sys->device);
+    if (scope_.rc) return scope_.rc;
     cudaStream_t st = (cudaStream_t)stream;
     CU(cudaMemsetAsync(flag, 0, sizeof(int), st));
     Geom gr = sys->g;
@@ -1172,7 +1206,8 @@ int md_force_half_kick(md_system *sys, const md_potential *pot, const void *pos,
     Pair pp;
     int rc = make_pair(sys, pot, &pp);
     if (rc) return rc;
-    if ((rc = enter(sys))) return rc;
+    DeviceScope scope_(sys->device);
+    if (scope_.rc) return scope_.rc;
     Book book = {nullptr, nullptr, nullptr};
     return launch_force(sys, pp, (const float4 *)pos, nbr_idx, nbr_count, (float4 *)force, (float4 *)vel,
                         dt / (2.0f * mass), nullptr, false, book, (cudaStream_t)stream);
@@ -1182,7 +1217,8 @@ int md_half_kick(md_system *sys, void *vel, const void *force, float dt, float m
     if (!sys || !vel || !force) return fail(MD_EINVAL, "NULL argument");
     if (!aligned16(vel) || !aligned16(force)) return fail(MD_EINVAL, "vel/force must be 16-byte aligned");
     if (!(dt > 0.0f) || !(mass > 0.0f)) return fail(MD_EINVAL, "dt and mass must be positive");
-    if (int rc = enter(sys)) return rc;
+    DeviceScope scope_(sys->device);
+    if (scope_.rc) return scope_.rc;
     const int m = sys->r1 - sys->r0;
     const size_t o = (size_t)sys->r0;
     k_half_kick<<<blocks_for(m), 256, 0, (cudaStream_t)stream>>>(m, sys->g.dim, (float4 *)vel + o, (const float4 *)force + o, dt / (2.0f * mass));
@@ -1249,7 +1285,8 @@ int md_flock_step(md_system *sys, const md_flock_params *par, void *pos, int32_t
         return fail(MD_EINVAL, "flocking parameters out of range");
     const float rmax = std::max(par->R_align, std::max(par->R_avoid, par->R_cohesion));
     if (rmax > sys->cfg.r_cut) return fail(MD_EINVAL, "interaction range %g exceeds the list r_cut %g", rmax, sys->cfg.r_cut);
-    if (int rc = enter(sys)) return rc;
+    DeviceScope scope_(sys->device);
+    if (scope_.rc) return scope_.rc;
     Pair pp;
     memset(&pp, 0, sizeof(pp));
     RuleArgs A;
@@ -1277,7 +1314,8 @@ int md_fire_minimize(md_system *sys, const md_potential *pot, const md_fire_para
     Pair pp;
     int rc = make_pair(sys, pot, &pp);
     if (rc) return rc;
-    if ((rc = enter(sys))) return rc;
+    DeviceScope scope_(sys->device);
+    if (scope_.rc) return scope_.rc;
     cudaStream_t st = (cudaStream_t)stream;
     const FirePar fp = {par->dt_start, par->dt_max, par->n_min, par->f_inc, par->f_dec, par->alpha_start, par->f_alpha};
     k_fire_init<<<1, 1, 0, st>>>(fp, fire_state);

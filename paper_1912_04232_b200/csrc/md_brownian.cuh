@@ -30,8 +30,11 @@ template <int DIM>
 __global__ void __launch_bounds__(256)
 k_brownian_drift(Geom g, float4 *__restrict__ pos, const float4 *__restrict__ force,
                  const int *__restrict__ id, const float4 *__restrict__ ref, float mu, float amp,
-                 unsigned seed, unsigned step0, const int *__restrict__ steps_done, Raise rs) {
-    const unsigned step = step0 + (unsigned)*steps_done;      // stats[0]: steps finished in this call
+                 const unsigned *__restrict__ seed_step0, const int *__restrict__ steps_done, Raise rs) {
+    // {seed, step0} live in device words (written before every call), so that a caller who continues a
+    // noise stream with a new step0 re-uses the captured graphs
+    const unsigned seed = seed_step0[0];
+    const unsigned step = seed_step0[1] + (unsigned)*steps_done;      // stats[0]: steps finished in this call
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     bool moved = false;
     if (i < g.n) {
@@ -60,8 +63,9 @@ __global__ void __launch_bounds__(256)
 k_langevin_baoa(Geom g, float4 *__restrict__ pos, float4 *__restrict__ vel,
                 const float4 *__restrict__ force, const int *__restrict__ id,
                 const float4 *__restrict__ ref, float a, float dt, float c1, float c2,
-                unsigned seed, unsigned step0, const int *__restrict__ steps_done, Raise rs) {
-    const unsigned step = step0 + (unsigned)*steps_done;      // stats[0]: steps finished in this call
+                const unsigned *__restrict__ seed_step0, const int *__restrict__ steps_done, Raise rs) {
+    const unsigned seed = seed_step0[0];
+    const unsigned step = seed_step0[1] + (unsigned)*steps_done;      // stats[0]: steps finished in this call
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     bool moved = false;
     if (i < g.n) {

@@ -85,6 +85,8 @@ class RankLoop:
         if self.range[0] == self.range[1]:
             raise ValueError(f"rank {rank} of {world} owns no list tile of {self.n} particles")
         self.rows = slot_rows(self.n, world)
+        if not system.cfg.resort:
+            raise ValueError("a split list needs resort = 1: ranges are ranges of the cell-sorted order")
         B.md_set_range(system.sys, *self.range)
         self.rebuilds = 0
         self.slot = torch.zeros(self.rows, 4, dtype=torch.float32, device=system.pos.device)    # reused every step

@@ -106,10 +106,10 @@ def _pack(x32: np.ndarray, w: np.ndarray | float) -> np.ndarray:
 
 def lj_fcc(index: int, m: int, *, temperature: float = 1.0, skin: float = 0.3,
            steps: int = 100, resort: int = 1, jitter: float = 0.05,
-           seed: int | None = None, name: str | None = None) -> Workload:
-    """3-D LJ fluid on a jittered FCC lattice at rho = 0.8442 (configs 0,2,3,4)."""
+           seed: int | None = None, name: str | None = None, rho: float = RHO_LJ) -> Workload:
+    """3-D LJ fluid on a jittered FCC lattice at rho = 0.8442 (configs 0,2,3,4; other densities: tests)."""
     n = 4 * m ** 3
-    L64 = (n / RHO_LJ) ** (1.0 / 3.0)
+    L64 = (n / rho) ** (1.0 / 3.0)
     box = np.array([L64, L64, L64], dtype=np.float32)
     rng = np.random.default_rng(SEED0 + index if seed is None else seed)
     sites = fcc_sites(m, float(box[0]) / m)
