@@ -190,7 +190,7 @@ int make_geom(const md_config *cfg, int n, Geom *g) {
     if (!(cfg->r_cut > 0.0f)) return fail(MD_EINVAL, "r_cut must be positive");
     if (!(cfg->skin >= 0.0f)) return fail(MD_EINVAL, "skin must be non-negative");
     memset(g, 0, sizeof(*g));
-    g->dim = cfg->dim; g->n = n; g->capacity = cfg->capacity;
+    g->dim = cfg->dim; g->n = n; g->ntot = n; g->capacity = cfg->capacity;
     const float R = cfg->r_cut + cfg->skin;              // fl32(r_cut + skin)
     g->R2 = R * R;
     const float hs = cfg->skin * 0.5f;

@@ -118,6 +118,7 @@ __device__ __forceinline__ Acc64 lj_row64(const Geom &g, const Pair &pp,
         const bool v2 = k + G < cnt;
         const int j1 = col[k * TILE];
         const int j2 = v2 ? col[(k + G) * TILE] : j1;
+        MD_CHECK(j1 >= 0 && j1 < g.ntot && j2 >= 0 && j2 < g.ntot);
         const float4 q1 = pos[j1], q2 = pos[j2];
         pair_any<0, 3, ENERGY, WRAP>(pp, me, q1, true, acc);
         pair_any<0, 3, ENERGY, WRAP>(pp, me, q2, v2, acc);
@@ -181,7 +182,7 @@ __device__ __forceinline__ void lj_rows32(const Geom &g, const Pair32 &p32,
 #pragma unroll
         for (int u = 0; u < F32_U; ++u) j[u] = jn[u];
 #pragma unroll
-        for (int u = 0; u < F32_U; ++u) q[u] = pos[j[u]];
+        for (int u = 0; u < F32_U; ++u) { MD_CHECK(j[u] >= 0 && j[u] < g.ntot); q[u] = pos[j[u]]; }
 #pragma unroll
         for (int u = 0; u < F32_U; ++u) jn[u] = k + F32_U + u < kload ? col[(k + F32_U + u) * TILE] : ii;
 #pragma unroll
@@ -194,7 +195,7 @@ __device__ __forceinline__ void lj_rows32(const Geom &g, const Pair32 &p32,
 #pragma unroll
         for (int u = 0; u < F32_U; ++u) j[u] = k + u < cnt ? jn[u] : ii;
 #pragma unroll
-        for (int u = 0; u < F32_U; ++u) q[u] = pos[j[u]];
+        for (int u = 0; u < F32_U; ++u) { MD_CHECK(j[u] >= 0 && j[u] < g.ntot); q[u] = pos[j[u]]; }
 #pragma unroll
         for (int u = 0; u < F32_U; ++u) jn[u] = k + F32_U + u < kload ? col[(k + F32_U + u) * TILE] : ii;
 #pragma unroll

@@ -5,6 +5,16 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+// -DMD_CHECKED: device-side asserts on every index the hot path reads or writes through (list entries,
+// gather indices, cell ids, sorted slots).  The pool's compute-sanitizer is closed, so this build is
+// what the memory-safety workout of the tests runs against (profiles/r2_sanitizer.md).
+#ifdef MD_CHECKED
+#include <assert.h>
+#define MD_CHECK(c) assert(c)
+#else
+#define MD_CHECK(c) ((void)0)
+#endif
+
 namespace mdk {
 
 constexpr unsigned FULL = 0xffffffffu;
@@ -12,6 +22,7 @@ constexpr unsigned FULL = 0xffffffffu;
 // Everything a kernel needs to know about the space and the partition (by value).
 struct Geom {
     int   dim, n, capacity, cells;
+    int   ntot;             // particles of the whole system (n is a context's range end under md_set_range)
     int   nc[3];            // cells per side n_k = floor(L_k / R)
     float L[3];             // box sides
     float h[3];             // fl(L/2)
@@ -112,6 +123,7 @@ k_cell_assign(Geom g, const float4 *__restrict__ pos, int *__restrict__ cell_of,
     int cy = cell_coord(p.y, g.inv_cell[1], g.nc[1]);
     int cz = g.dim == 3 ? cell_coord(p.z, g.inv_cell[2], g.nc[2]) : 0;
     int c = (cz * g.nc[1] + cy) * g.nc[0] + cx;
+    MD_CHECK(c >= 0 && c < g.cells);
     cell_of[i] = c;
     rank_tmp[i] = atomicAdd(&cell_count[c], 1);   // arrival order; made canonical later
 }
@@ -264,6 +276,7 @@ k_cell_scatter(int n, const int *__restrict__ cell_of, const int *__restrict__ r
     if (cond && ld_volatile(cond) == 0) return;
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
+    MD_CHECK(cell_start[cell_of[i]] + rank_tmp[i] >= 0 && cell_start[cell_of[i]] + rank_tmp[i] < n);
     perm_tmp[cell_start[cell_of[i]] + rank_tmp[i]] = i;
 }
 
@@ -293,6 +306,7 @@ k_cell_order_gather(int n, const int *__restrict__ cell_of, const int *__restric
         rank += (xj < pi.x) || (xj == pi.x && kj < key);
     }
     int dst = t0 + rank;
+    MD_CHECK(i >= 0 && i < n && rank < t1 - t0 && dst >= 0 && dst < n);
     perm[dst] = i;
     pos_s[dst] = pi;
     if (vel_s) vel_s[dst] = vel[i];
@@ -902,7 +916,7 @@ k_force(Geom g, Pair pp, const float4 *__restrict__ pos, const int *__restrict__
 #pragma unroll
         for (int u = 0; u < U; ++u) { const int kk = k + u * TPP; j[u] = kk < cnt ? col[kk * TILE] : ii; }
 #pragma unroll
-        for (int u = 0; u < U; ++u) q[u] = pos[j[u]];
+        for (int u = 0; u < U; ++u) { MD_CHECK(j[u] >= 0 && j[u] < g.ntot); q[u] = pos[j[u]]; }
         if (!wrap_path) {
 #pragma unroll
             for (int u = 0; u < U; ++u) pair_any<KIND, DIM, ENERGY, false>(pp, me, q[u], k + u * TPP < cnt, acc, sp);
@@ -998,7 +1012,7 @@ k_force_stream(Geom g, Pair pp, const float4 *__restrict__ pos, const int *__res
 #pragma unroll
             for (int u = 0; u < U; ++u) j[u] = k0 + r + u < cnt ? sm[(r + u) * TILE] : ii;
 #pragma unroll
-            for (int u = 0; u < U; ++u) q[u] = pos[j[u]];
+            for (int u = 0; u < U; ++u) { MD_CHECK(j[u] >= 0 && j[u] < g.ntot); q[u] = pos[j[u]]; }
             if (!wrap_path) {
 #pragma unroll
                 for (int u = 0; u < U; ++u) pair_any<KIND, DIM, ENERGY, false>(pp, me, q[u], k0 + r + u < cnt, acc, sp);

@@ -170,12 +170,15 @@ k_nbr_build2(Geom g, const float4 *__restrict__ spos, const int *__restrict__ ce
                     w = need ? wn : w;
                     plo = need ? nlo : plo;
                     phi = need ? nhi : phi;
+                    MD_CHECK(w >= 0 && w < NB2_WORDS);
                     const unsigned fresh = W.mask[w][lane];        // w is always a valid word index
                     word = need ? fresh : word;
                     const bool has = word != 0u;
                     const int bit = __clz(word) & 31;
                     const int slot = W.wbase[w] + bit;
                     word &= 0x7fffffffu >> bit;                    // drop that bit (all above it are 0)
+                    MD_CHECK(!has || (slot >= 0 && slot < g.n && slot != s));
+                    MD_CHECK(!(has && cnt < cap) || (optr >= outp && optr < outp + (size_t)cap * TILE));
                     if (has && cnt < cap) *optr = MAPPED ? map[slot] : slot;
                     optr += (has && cnt < cap) ? TILE : 0;
                     cnt += has ? 1 : 0;
@@ -216,6 +219,7 @@ k_nbr_build2(Geom g, const float4 *__restrict__ spos, const int *__restrict__ ce
                 const float piz = (DIM == 3 && rcz + dz >= ncz) ? __fsub_rn(pi.z, Lz) : pi.z;
                 const int m = min(NB2_CHUNK, pt1 - base);
                 if (nw + ((m + 31) >> 5) > NB2_WORDS) expand();   // batch full (warp-uniform)
+                MD_CHECK(m > 0 && base >= 0 && pt1 <= g.n && nw + ((m + 31) >> 5) <= NB2_WORDS);
                 // stage -(candidate - shift), structure of arrays; the tail of the last group of
                 // four is a far-away point
 #pragma unroll

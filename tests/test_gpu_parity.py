@@ -1108,6 +1108,46 @@ def test_config2_snapshots(B, orc, W):
     assert 80 <= rebuilds <= 200
 
 
+def test_sanitizer_workout(B, W):
+    """A short pass over every hot-path kernel on configs 0 and 1 -- both builders' part counts, the fused
+    and the unfused step, graph and direct launches, a ragged last tile with an un-sorted system and a list
+    buffer full of garbage -- cheap enough to run under a sanitizer or against a library built with
+    -DMD_CHECKED (device-side index asserts; profiles/r2_sanitizer.md).  Here it checks that fused / unfused
+    and graph / direct runs agree bit for bit."""
+    ref = {}
+    for ci in (0, 1):
+        w = W.config(ci)
+        for parts in (1, 2, 4):
+            for fused, graph in ((1, 1), (0, 1), (1, 0)):
+                S = B.System(w)
+                B.md_set_option(S.sys, "builder_parts", parts)
+                B.md_set_option(S.sys, "fused", fused)
+                B.md_set_option(S.sys, "use_graph", graph)
+                S.build(); S.compute_force()
+                B.md_needs_rebuild(S.sys, S.pos, S.flag)
+                S.step(41)
+                torch.cuda.synchronize()
+                st = S.stats.cpu().numpy()
+                assert st[0] == 41 and st[1] >= 2 and st[2] == -1
+                key = (ci, parts)             # the row order, hence the rounding, depends on the part count
+                state = (S.pos.clone(), S.vel.clone(), S.id.clone())
+                if key in ref:
+                    assert all(torch.equal(a, b) for a, b in zip(state, ref[key]))
+                else:
+                    ref[key] = state
+                S.close()
+    # ragged last tile (n % 32 != 0), no physical re-sort, the list buffer pre-filled with garbage
+    w = W.lj_fcc(0, 7, seed=5)
+    w = dataclasses.replace(w, n=w.n - 5, pos=w.pos[:-5].copy(), vel=w.vel[:-5].copy())
+    for resort in (0, 1):
+        S = B.System(w, resort=resort)
+        S.nbr_idx.fill_(0x7fffffff)
+        S.build(); S.compute_force(); S.step(21)
+        torch.cuda.synchronize()
+        assert int(S.stats[0]) == 21 and int(S.stats[2]) == -1 and torch.isfinite(S.force).all()
+        S.close()
+
+
 # ------------------------- SURVEY 8(f) rows and the fast path at the sizes bench.py times ----
 
 def state_force_parity(S, orc, w, alpha=None, species=None):
