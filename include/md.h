@@ -112,6 +112,8 @@ int md_destroy(md_system *sys);
  *                          65,536 particles, else 1
  *   "builder"              neighbor-list kernel: 2 (default) records hits in per-lane bit masks,
  *                          1 appends them to per-lane shared-memory columns (first design)
+ *   "cell_coop"            1: the cell list as ONE cooperative launch (grid barriers between its phases), 0: five
+ *                          kernels; default 1 up to 65,536 particles (where it is faster), else 0.  Same results.
  *   "use_graph"            0: the step calls launch their kernels directly instead of CUDA graphs -- the same
  *                          kernels in the same order (so a profiler lists them one by one); the rebuild kernels
  *                          are then launched every step and return at once while the step's device flag is 0

@@ -109,6 +109,8 @@ struct md_system {
     int fused;           // fused step: the force kernel also opens the next step (graph mode, fast32)
     int remap;           // force kernel: block -> tile remap period (the SM count), 0 = off
     int nb_parts;        // builder: warps per tile (0 = by system size, 1, 2, 4)
+    int cell_coop;       // cell list as one cooperative launch with this many blocks at most (0: five kernels)
+    int cell_coop_max;   // what the device allows
     int ns;              // md_set_species_lj: number of species and the tables (row-major)
     float sp_eps[16], sp_sig[16], sp_rc[16];
     int bks_ns;          // md_set_species_bks: A, B, C per species pair, charges, DSF damping, Coulomb constant
@@ -163,7 +165,7 @@ Layout layout(int n, long long cells) {
     size_t o = 0;
     auto take = [&](size_t bytes) { size_t at = o; o += up(bytes); return at; };
     l.words = take(64 * sizeof(int));
-    l.scan_tmp = take((size_t)((cells + SCAN_CHUNK - 1) / SCAN_CHUNK + 2) * sizeof(int));
+    l.scan_tmp = take((size_t)std::max<long long>((cells + SCAN_CHUNK - 1) / SCAN_CHUNK + 2, 4096) * sizeof(int));   // also the cooperative cell list's block sums
     l.fire_tmp = take(((size_t)(n + FIRE_BLOCK - 1) / FIRE_BLOCK * 3 + 2) * sizeof(double));
     l.pred_tmp = take((size_t)FLOCK_PRED_CHUNKS * MD_MAX_PREDATORS * 3 * sizeof(double));
     l.cell_count = take((size_t)(cells + 4) * sizeof(int));
@@ -286,6 +288,21 @@ int launch_cell_build(md_system *s, float4 *pos, float4 *vel, int *id, int *cell
     const Geom &g = s->g;
     const int nb = blocks_for(g.n);
     const bool resort = s->cfg.resort != 0;
+    if (s->cell_coop > 0) {
+        // one cooperative launch (grid-wide barriers between the phases); needs every block resident
+        const int grid = std::min(nb, s->cell_coop);
+        Geom gg = g;
+        float4 *velp = (resort && vel) ? vel : nullptr, *vel_s = (resort && vel) ? s->vel_s : nullptr;
+        int *idp = id, *id_s = (resort && id) ? s->id_s : nullptr;
+        int *cell_of = s->cell_of, *rank_tmp = s->rank_tmp, *cell_count = s->cell_count, *perm_tmp = s->perm_tmp;
+        float4 *pos_s = s->pos_s;
+        int *block_sum = s->scan_tmp;
+        int rs = resort ? 1 : 0;
+        void *args[] = {&gg, &pos, &velp, &idp, &cell_of, &rank_tmp, &cell_count, &cell_start, &perm_tmp, &perm,
+                        &pos_s, &vel_s, &id_s, &block_sum, &status, &cond, &rs};
+        CU(cudaLaunchCooperativeKernel((const void *)k_cell_all, dim3(grid), dim3(256), args, 0, st));
+        return MD_OK;
+    }
     k_cell_assign<<<nb, 256, 0, st>>>(g, pos, s->cell_of, s->rank_tmp, s->cell_count, cond);
     LAUNCH_OK();
     if (g.cells <= SCAN_ONE_BLOCK) {
@@ -867,6 +884,16 @@ int md_create(const md_config *cfg, int n, void *workspace, size_t bytes, md_sys
         s->remap = sms >= 4 ? sms / 4 : 0;
     }
     s->fused = 1;
+    {   // the cell list as one cooperative launch: as many blocks as are resident at once
+        int per_sm = 0, sms = 0, coop = 0;
+        cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, attr.device);
+        cudaDeviceGetAttribute(&coop, cudaDevAttrCooperativeLaunch, attr.device);
+        if (coop && cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, k_cell_all, 256, 0) == cudaSuccess)
+        {
+                s->cell_coop_max = std::min(std::min(per_sm, 4) * sms, 4095);
+                s->cell_coop = n <= 65536 ? s->cell_coop_max : 0;     // measured: pays below, costs above
+            }
+    }
     s->est_thr = 8.0f;
     s->unroll = 9;      // odd: a fused graph swaps position buffers steps-1 times and must end in the caller's
     {   // neighbor-list builder: one warp per tile, a capacity x 32 column block + a candidate
@@ -962,6 +989,10 @@ int md_set_option(md_system *sys, const char *name, double value) {
     else if (!strcmp(name, "fast32")) sys->fast32 = value != 0.0;
     else if (!strcmp(name, "fused")) sys->fused = value != 0.0;
     else if (!strcmp(name, "remap")) sys->remap = (int)value;
+    else if (!strcmp(name, "cell_coop")) {
+        if (value != 0.0 && !(sys->cell_coop_max > 0)) return fail(MD_EINVAL, "the device offers no cooperative launch");
+        sys->cell_coop = value != 0.0 ? sys->cell_coop_max : 0;
+    }
     else if (!strcmp(name, "builder_parts")) {
         if (value != 0.0 && value != 1.0 && value != 2.0 && value != 4.0) return fail(MD_EINVAL, "builder_parts must be 0, 1, 2 or 4");
         sys->nb_parts = (int)value;

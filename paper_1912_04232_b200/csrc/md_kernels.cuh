@@ -3,6 +3,7 @@
 // of open points: SURVEY.md §8c A1..A18 / DESIGN.md §3.  Shares nothing with oracle/.
 #pragma once
 #include <cuda_runtime.h>
+#include <cooperative_groups.h>
 #include <stdint.h>
 
 // -DMD_CHECKED: device-side asserts on every index the hot path reads or writes through (list entries,
@@ -323,6 +324,110 @@ k_copy_back(int n, const float4 *__restrict__ pos_s, const float4 *__restrict__ 
     pos[s] = pos_s[s];
     if (vel) vel[s] = vel_s[s];
     if (id) id[s] = id_s[s];
+}
+
+// The whole cell list in ONE cooperative launch (grid-wide barriers between the phases instead of
+// kernel boundaries).  Pays for small systems, whose five launches are launch- and latency-bound
+// (config 1, 16,384 disks: 29 us against 41 us); at 256,000 particles and above the phases are bound by
+// their own gathers and the one resident wave of a cooperative grid is slower than full grids
+// (52 against 55 us at 256k, 101 against 77 us at 1M), so md_create selects it up to 65,536 particles.  Phases: assign -> scan (every block scans its own run of cells, then adds the
+// sum of the runs before it) -> scatter -> in-cell order + payload gather -> copy back (re-sort).
+// Same arithmetic and the same results as the five kernels above.  block_sum: gridDim.x + 1 ints.
+__global__ void __launch_bounds__(256)
+k_cell_all(Geom g, float4 *__restrict__ pos, float4 *__restrict__ vel, int *__restrict__ id,
+           int *__restrict__ cell_of, int *__restrict__ rank_tmp, int *__restrict__ cell_count,
+           int *__restrict__ cell_start, int *__restrict__ perm_tmp, int *__restrict__ perm,
+           float4 *__restrict__ pos_s, float4 *__restrict__ vel_s, int *__restrict__ id_s,
+           int *__restrict__ block_sum, int *status, const int *cond, int resort) {
+    if (cond && ld_volatile(cond) == 0) return;          // grid-uniform: nobody reaches a barrier
+    namespace cg = cooperative_groups;
+    cg::grid_group grid = cg::this_grid();
+    __shared__ int sh[256];
+    const int tid = threadIdx.x, nthr = gridDim.x * blockDim.x, gtid = blockIdx.x * blockDim.x + tid;
+    const int n = g.n, cells = g.cells;
+    // ---- assign
+    for (int i = gtid; i < n; i += nthr) {
+        const float4 p = pos[i];
+        const int cx = cell_coord(p.x, g.inv_cell[0], g.nc[0]);
+        const int cy = cell_coord(p.y, g.inv_cell[1], g.nc[1]);
+        const int cz = g.dim == 3 ? cell_coord(p.z, g.inv_cell[2], g.nc[2]) : 0;
+        const int c = (cz * g.nc[1] + cy) * g.nc[0] + cx;
+        MD_CHECK(c >= 0 && c < cells);
+        cell_of[i] = c;
+        rank_tmp[i] = atomicAdd(&cell_count[c], 1);
+    }
+    grid.sync();
+    // ---- scan, part 1: block b owns cells [b * per, (b + 1) * per), thread t the run [c0, c1) inside it
+    const int per = (cells + gridDim.x - 1) / gridDim.x;
+    const int b0 = min(blockIdx.x * per, cells), b1 = min(b0 + per, cells);
+    const int tper = (per + blockDim.x - 1) / blockDim.x;
+    const int c0 = min(b0 + tid * tper, b1), c1 = min(c0 + tper, b1);
+    int sum = 0;
+    for (int c = c0; c < c1; ++c) sum += cell_count[c];
+    sh[tid] = sum;
+    __syncthreads();
+    for (int o = 1; o < 256; o <<= 1) {                  // inclusive scan of the 256 run sums
+        const int v = tid >= o ? sh[tid - o] : 0;
+        __syncthreads();
+        sh[tid] += v;
+        __syncthreads();
+    }
+    const int excl = sh[tid] - sum;                       // exclusive prefix of my run inside the block
+    if (tid == 255) block_sum[blockIdx.x] = sh[255];
+    if (gtid == 0 && status) { status[0] = 0; status[1] = 0; }
+    grid.sync();
+    // ---- scan, part 2: the sum of the blocks before mine
+    int before = 0;
+    for (int b = tid; b < (int)blockIdx.x; b += blockDim.x) before += block_sum[b];
+    __syncthreads();                                      // sh is read above by every thread
+    sh[tid] = before;
+    __syncthreads();
+    for (int o = 128; o > 0; o >>= 1) { if (tid < o) sh[tid] += sh[tid + o]; __syncthreads(); }
+    int run = sh[0] + excl;
+    for (int c = c0; c < c1; ++c) {
+        const int v = cell_count[c];
+        cell_count[c] = 0;
+        cell_start[c] = run;
+        run += v;
+    }
+    if (gtid == 0) cell_start[cells] = n;
+    grid.sync();
+    // ---- scatter
+    for (int i = gtid; i < n; i += nthr) {
+        const int dst = cell_start[cell_of[i]] + rank_tmp[i];
+        MD_CHECK(dst >= 0 && dst < n);
+        perm_tmp[dst] = i;
+    }
+    grid.sync();
+    // ---- canonical order inside a cell (ascending x, ties by id) and payload gather
+    for (int s = gtid; s < n; s += nthr) {
+        const int i = perm_tmp[s];
+        const int c = cell_of[i];
+        const int t0 = cell_start[c], t1 = cell_start[c + 1];
+        const float4 pi = pos[i];
+        const int key = id ? id[i] : i;
+        int rank = 0;
+        for (int t = t0; t < t1; ++t) {
+            const int j = perm_tmp[t];
+            const int kj = id ? id[j] : j;
+            const float xj = pos[j].x;
+            rank += (xj < pi.x) || (xj == pi.x && kj < key);
+        }
+        const int dst = t0 + rank;
+        MD_CHECK(rank < t1 - t0 && dst < n);
+        perm[dst] = i;
+        pos_s[dst] = pi;
+        if (vel_s) vel_s[dst] = vel[i];
+        if (id_s) id_s[dst] = id[i];
+    }
+    if (!resort) return;
+    grid.sync();
+    // ---- copy back: the caller's arrays in cell order
+    for (int s = gtid; s < n; s += nthr) {
+        pos[s] = pos_s[s];
+        if (vel) vel[s] = vel_s[s];
+        if (id) id[s] = id_s[s];
+    }
 }
 
 __global__ void __launch_bounds__(256)
