@@ -69,6 +69,9 @@ def parse():
     ap.add_argument("--decompose", action="store_true",
                     help="time the split-list multi-GPU loop (SURVEY 8f-f1) instead: ONE system over all ranks, "
                          "strong scaling; not the contract line")
+    ap.add_argument("--slabs", type=int, default=0,
+                    help="time the slab decomposition (SURVEY 8f-f1, second version) with this many ranks stepped in "
+                         "lockstep on ONE GPU: what the protocol costs, not a multi-GPU number; not the contract line")
     ap.add_argument("--next-rows", action="store_true",
                     help="time the SURVEY 8(f) rows instead (one JSON line per row; not the contract line)")
     ap.add_argument("--no-graph", action="store_true",
@@ -320,6 +323,43 @@ def run_next_rows(args):
     S.close()
 
 
+def run_slabs(args):
+    """SURVEY 8(f)-f1, second version: `--slabs P` ranks (slabs along x with halos; paper_1912_04232_b200/slabs.py)
+    of config `--config`, all in this process on one GPU, stepped in lockstep.  One GPU executes the work of P
+    ranks one after the other, so us_per_md_step is (sum over ranks) and says what the decomposition costs in
+    total work -- halo copies, per-step exchange, host-driven phases -- against md_nve_step on one context."""
+    import torch
+    from paper_1912_04232_b200 import binding as B
+    from paper_1912_04232_b200 import slabs as SL
+    from paper_1912_04232_b200 import workloads as W
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the product has no CPU fallback")
+    w = W.config(args.config)
+    run = SL.SlabRun(B, w, args.slabs)
+    for _ in range(args.warmup):
+        run.step(args.md_steps)
+    torch.cuda.synchronize()
+    r0 = run.rebuilds
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for _ in range(args.steps):
+        run.step(args.md_steps)
+    b.record()
+    torch.cuda.synchronize()
+    ms = a.elapsed_time(b)
+    total = args.steps * args.md_steps
+    owned = [int((S.id[: S.n] >= 0).sum()) for S in run.ranks]
+    print(json.dumps({
+        "mode": "slabs", "metric": METRIC, "value": w.n * total / (ms * 1e-3), "unit": UNIT, "n_gpus": 1,
+        "ranks_on_this_gpu": args.slabs, "steps": args.steps, "warmup": args.warmup, "ms_per_step": ms / args.steps,
+        "us_per_md_step_all_ranks": 1e3 * ms / total, "higher_is_better": True, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": w.name, "n": w.n, "md_steps_per_step": args.md_steps,
+                   "parallelism": f"{args.slabs} slabs along x with halos of width r_cut + skin, in lockstep on one GPU"},
+        "rebuilds": run.rebuilds - r0, "owned_per_rank": owned, "local_per_rank": [S.n for S in run.ranks],
+        "rows_per_step_per_link": run.exchange_plan()}))
+    run.close()
+
+
 def run_decomposed(args):
     """SURVEY 8(f)-f1: one system of config `--config` over all ranks (replicated positions, split list;
     paper_1912_04232_b200/decomposition.py).  A bench step is `--md-steps` MD steps; device time by CUDA
@@ -413,6 +453,8 @@ def main():
         return run_next_rows(args)
     if args.decompose:
         return run_decomposed(args)
+    if args.slabs:
+        return run_slabs(args)
 
     import torch
     import torch.distributed as dist

@@ -157,6 +157,47 @@ int md_force_half_kick(md_system *sys, const md_potential *pot, const void *pos,
 /* Closing half-kick on the context's range: v += dt/(2m) F. */
 int md_half_kick(md_system *sys, void *vel, const void *force, float dt, float mass, void *stream);
 
+/*
+ * Multi-GPU by spatial decomposition: slabs along x with halos (second version;
+ * DESIGN.md §8; the protocol is paper_1912_04232_b200/slabs.py).  A rank runs an ordinary md_system on a LOCAL
+ * periodic box that holds its slab, copies of the neighbouring slabs' particles within r_cut + skin of it
+ * (its halo) and an empty gap.  Local x = global x - T, except for the one periodic image the first and the
+ * last rank take through the box boundary; every such translation is exact in fp32 (L72: the space is a
+ * torus, a frame is a choice of origin), so pair displacements in a local frame are bit-identical to the
+ * global ones.  The calls below are the coordinate plumbing of that scheme; the frame is plain data the
+ * caller computes once (slabs.frames).
+ *   kind 0 (first rank):  local = x, or (x - L) + Lx for x >= g2l_thr (the image of x near L);
+ *                         global = local, or (local - Lx) + L for local >= l2g_thr
+ *   kind 1 (middle):      local = x - T;  global = local + T
+ *   kind 2 (last rank):   local = x for x < g2l_thr (the image of x near 0, raw), else x - T  (Lx = L - T);
+ *                         global = local for local < l2g_thr, else local + T
+ * A global x that rounds to >= L becomes 0.
+ */
+typedef struct md_slab_frame {
+    int   kind;       /* 0 first, 1 middle, 2 last */
+    float T;          /* translation (a multiple of 2^-8, >= 0) */
+    float Lx;         /* local box side in x */
+    float L;          /* global box side in x */
+    float g2l_thr;    /* global x at which the image branch starts (kind 0) / ends (kind 2) */
+    float l2g_thr;    /* local x at which the image zone starts (kind 0) / ends (kind 2) */
+} md_slab_frame;
+
+/* md_kick_drift on the whole local system, then every x put back on the GLOBAL fp32 grid
+ * (x = to_local(to_global(x))): the rounding the global coordinate would get, so that a decomposed run
+ * differs from md_nve_step only in the order forces are summed. */
+int md_slab_kick_drift(md_system *sys, const md_slab_frame *frame, void *pos, void *vel, const void *force,
+                       float dt, float mass, int32_t *flag, void *stream);
+
+/* In place on the x component of n float4 positions: to_local != 0: global -> local, else local -> global. */
+int md_slab_convert(const md_slab_frame *frame, void *pos, int n, int to_local, void *stream);
+
+/* rows_out[k] = pos[slots[k]] with x made global (what a rank sends: its border particles);
+ * pos[slots[k]] = rows[k] with x made local (what it receives: its halo copies).  slots: DEVICE int32[k]. */
+int md_slab_pack(const md_slab_frame *frame, const void *pos, const int32_t *slots, int k, void *rows_out,
+                 void *stream);
+int md_slab_unpack(const md_slab_frame *frame, const void *rows, const int32_t *slots, int k, void *pos,
+                   void *stream);
+
 /* BKS-type potential (L104 "Buckingham / BKS" [71-73], named only; reading A27): per species
  * pair the exp-6 term A_ab exp(-B_ab r) - C_ab / r^6, plus the Coulomb interaction of the species' point
  * charges in its damped shifted-force form (energy and force both vanish at r_cut):

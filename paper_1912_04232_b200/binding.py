@@ -25,6 +25,7 @@ SYMBOLS = [
     "md_langevin_step", "md_nose_hoover_step", "md_set_species_lj",
     "md_flock_step", "md_flock_obstacles", "md_set_species_bks", "md_flock_predators",
     "md_set_range", "md_kick_drift", "md_half_kick", "md_force_half_kick",
+    "md_slab_kick_drift", "md_slab_convert", "md_slab_pack", "md_slab_unpack",
 ]
 
 
@@ -47,6 +48,11 @@ class md_fire_params(C.Structure):
 class md_flock_params(C.Structure):
     _fields_ = [("J_align", C.c_float), ("R_align", C.c_float), ("J_avoid", C.c_float), ("R_avoid", C.c_float),
                 ("J_cohesion", C.c_float), ("R_cohesion", C.c_float), ("alpha", C.c_float), ("speed", C.c_float)]
+
+
+class md_slab_frame(C.Structure):
+    _fields_ = [("kind", C.c_int), ("T", C.c_float), ("Lx", C.c_float), ("L", C.c_float),
+                ("g2l_thr", C.c_float), ("l2g_thr", C.c_float)]
 
 
 class md_predator_params(C.Structure):
@@ -94,6 +100,10 @@ def lib():
         L.md_kick_drift.argtypes = [vp, vp, vp, vp, C.c_float, C.c_float, ip, vp]
         L.md_force_half_kick.argtypes = [vp, C.POINTER(md_potential), vp, ip, ip, vp, vp, C.c_float, C.c_float, vp]
         L.md_half_kick.argtypes = [vp, vp, vp, C.c_float, C.c_float, vp]
+        L.md_slab_kick_drift.argtypes = [vp, C.POINTER(md_slab_frame), vp, vp, vp, C.c_float, C.c_float, ip, vp]
+        L.md_slab_convert.argtypes = [C.POINTER(md_slab_frame), vp, C.c_int, C.c_int, vp]
+        L.md_slab_pack.argtypes = [C.POINTER(md_slab_frame), vp, ip, C.c_int, vp, vp]
+        L.md_slab_unpack.argtypes = [C.POINTER(md_slab_frame), vp, ip, C.c_int, vp, vp]
         L.md_flock_predators.argtypes = [vp, C.c_int, vp, C.POINTER(md_predator_params)]
         L.md_flock_obstacles.argtypes = [vp, C.c_int, C.POINTER(C.c_float), C.POINTER(C.c_float), C.c_float]
         L.md_flock_step.argtypes = [vp, C.POINTER(md_flock_params), vp, ip, ip, ip, C.c_float, C.c_int, ip, vp]
@@ -264,6 +274,23 @@ def md_kick_drift(sys, pos, vel, force, dt, mass, flag, stream=None) -> None:
 def md_force_half_kick(sys, pot: md_potential, pos, nbr_idx, nbr_count, force, vel, dt, mass, stream=None) -> None:
     _check(lib().md_force_half_kick(sys, C.byref(pot), _ptr(pos), _ptr(nbr_idx), _ptr(nbr_count), _ptr(force),
                                     _ptr(vel), float(dt), float(mass), _stream(stream)))
+
+
+def md_slab_kick_drift(sys, frame: md_slab_frame, pos, vel, force, dt, mass, flag, stream=None) -> None:
+    _check(lib().md_slab_kick_drift(sys, C.byref(frame), _ptr(pos), _ptr(vel), _ptr(force), float(dt), float(mass),
+                                    _ptr(flag), _stream(stream)))
+
+
+def md_slab_convert(frame: md_slab_frame, pos, n, to_local, stream=None) -> None:
+    _check(lib().md_slab_convert(C.byref(frame), _ptr(pos), int(n), int(to_local), _stream(stream)))
+
+
+def md_slab_pack(frame: md_slab_frame, pos, slots, rows_out, stream=None) -> None:
+    _check(lib().md_slab_pack(C.byref(frame), _ptr(pos), _ptr(slots), int(slots.numel()), _ptr(rows_out), _stream(stream)))
+
+
+def md_slab_unpack(frame: md_slab_frame, rows, slots, pos, stream=None) -> None:
+    _check(lib().md_slab_unpack(C.byref(frame), _ptr(rows), _ptr(slots), int(slots.numel()), _ptr(pos), _stream(stream)))
 
 
 def md_half_kick(sys, vel, force, dt, mass, stream=None) -> None:

@@ -454,6 +454,45 @@ __global__ void k_unpermute(int n, const int *__restrict__ id, const float4 *__r
     ao[i] = a[s]; bo[i] = b[s]; co[i] = c[s];
 }
 
+// ---- slab decomposition: exact coordinate translations between a rank's local frame and the box
+__device__ __forceinline__ float slab_to_local(const md_slab_frame &f, float x) {
+    if (f.kind == 0) return x >= f.g2l_thr ? (x - f.L) + f.Lx : x;
+    if (f.kind == 2) return x < f.g2l_thr ? x : x - f.T;
+    return x - f.T;
+}
+__device__ __forceinline__ float slab_to_global(const md_slab_frame &f, float x) {
+    float g;
+    if (f.kind == 0) g = x >= f.l2g_thr ? (x - f.Lx) + f.L : x;
+    else if (f.kind == 2) g = x < f.l2g_thr ? x : x + f.T;
+    else g = x + f.T;
+    return g >= f.L ? 0.0f : g;
+}
+__global__ void k_slab_convert(md_slab_frame f, float4 *pos, int n, int mode) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    float x = pos[i].x;
+    if (mode == 0) x = slab_to_global(f, x);
+    else if (mode == 1) x = slab_to_local(f, x);
+    else x = slab_to_local(f, slab_to_global(f, x));      // back on the global fp32 grid
+    pos[i].x = x;
+}
+__global__ void k_slab_pack(md_slab_frame f, const float4 *__restrict__ pos, const int *__restrict__ slots, int k,
+                            float4 *__restrict__ rows) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= k) return;
+    float4 p = pos[slots[t]];
+    p.x = slab_to_global(f, p.x);
+    rows[t] = p;
+}
+__global__ void k_slab_unpack(md_slab_frame f, const float4 *__restrict__ rows, const int *__restrict__ slots, int k,
+                              float4 *__restrict__ pos) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= k) return;
+    float4 p = rows[t];
+    p.x = slab_to_local(f, p.x);
+    pos[slots[t]] = p;
+}
+
 __global__ void k_iota(int n, int *id) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) id[i] = i;
@@ -1242,6 +1281,53 @@ int md_force_half_kick(md_system *sys, const md_potential *pot, const void *pos,
     Book book = {nullptr, nullptr, nullptr};
     return launch_force(sys, pp, (const float4 *)pos, nbr_idx, nbr_count, (float4 *)force, (float4 *)vel,
                         dt / (2.0f * mass), nullptr, false, book, (cudaStream_t)stream);
+}
+
+static int check_frame(const md_slab_frame *f) {
+    if (!f) return fail(MD_EINVAL, "frame is NULL");
+    if (f->kind < 0 || f->kind > 2 || !(f->T >= 0.0f) || !(f->Lx > 0.0f) || !(f->L > 0.0f))
+        return fail(MD_EINVAL, "slab frame: kind in 0..2, T >= 0, Lx > 0, L > 0");
+    return MD_OK;
+}
+
+int md_slab_kick_drift(md_system *sys, const md_slab_frame *frame, void *pos, void *vel, const void *force,
+                       float dt, float mass, int32_t *flag, void *stream) {
+    if (int rc = check_frame(frame)) return rc;
+    if (int rc = md_kick_drift(sys, pos, vel, force, dt, mass, flag, stream)) return rc;
+    DeviceScope scope_(sys->device);
+    if (scope_.rc) return scope_.rc;
+    k_slab_convert<<<blocks_for(sys->n), 256, 0, (cudaStream_t)stream>>>(*frame, (float4 *)pos, sys->n, 2);
+    LAUNCH_OK();
+    return MD_OK;
+}
+
+int md_slab_convert(const md_slab_frame *frame, void *pos, int n, int to_local, void *stream) {
+    if (int rc = check_frame(frame)) return rc;
+    if (!pos || n < 0 || !aligned16(pos)) return fail(MD_EINVAL, "pos must be a 16-byte aligned array, n >= 0");
+    if (n == 0) return MD_OK;
+    k_slab_convert<<<blocks_for(n), 256, 0, (cudaStream_t)stream>>>(*frame, (float4 *)pos, n, to_local ? 1 : 0);
+    LAUNCH_OK();
+    return MD_OK;
+}
+
+int md_slab_pack(const md_slab_frame *frame, const void *pos, const int32_t *slots, int k, void *rows_out,
+                 void *stream) {
+    if (int rc = check_frame(frame)) return rc;
+    if (k < 0 || (k > 0 && (!pos || !slots || !rows_out))) return fail(MD_EINVAL, "NULL argument");
+    if (k == 0) return MD_OK;
+    k_slab_pack<<<blocks_for(k), 256, 0, (cudaStream_t)stream>>>(*frame, (const float4 *)pos, slots, k, (float4 *)rows_out);
+    LAUNCH_OK();
+    return MD_OK;
+}
+
+int md_slab_unpack(const md_slab_frame *frame, const void *rows, const int32_t *slots, int k, void *pos,
+                   void *stream) {
+    if (int rc = check_frame(frame)) return rc;
+    if (k < 0 || (k > 0 && (!pos || !slots || !rows))) return fail(MD_EINVAL, "NULL argument");
+    if (k == 0) return MD_OK;
+    k_slab_unpack<<<blocks_for(k), 256, 0, (cudaStream_t)stream>>>(*frame, (const float4 *)rows, slots, k, (float4 *)pos);
+    LAUNCH_OK();
+    return MD_OK;
 }
 
 int md_half_kick(md_system *sys, void *vel, const void *force, float dt, float mass, void *stream) {

@@ -1,0 +1,511 @@
+"""One system over several GPUs by SPATIAL decomposition: slabs along x with halos (SURVEY.md §8e / §8f-f1,
+second version).
+
+Rank r owns the particles whose x lies in its slab [lo_r, hi_r) and, beside them, copies of the particles
+of other ranks (or periodic images of its own, never needed for world >= 2) within the list radius
+R = r_cut + skin of the slab: its HALO.  Owned + halo particles form an ordinary periodic system of the
+library on a LOCAL box (x side: slab + two halos + an empty gap >= R, so that nothing an owned particle
+sees comes through the local box's own periodic wrap; y, z: the full box), and every step of the path --
+cell list, neighbor list, force, velocity Verlet -- runs in the library's kernels on that local system:
+
+    every step      md_kick_drift (all local particles; halo copies have zero velocity and zero force, so
+                    they stay), the x coordinates are put back on the global fp32 grid, the flags of all
+                    ranks are OR-ed; if no rebuild: every rank sends the new positions of its BORDER
+                    particles (the owned ones that are somebody's halo; index lists fixed since the last
+                    rebuild) to its two neighbors, which overwrite their halo copies; md_force_half_kick
+    at a rebuild    owned particles that left the slab MIGRATE to the neighbor (position, velocity, id);
+                    halos are re-selected; the local system is re-created for the new particle count;
+                    md_cell_list_build + md_neighbor_list_build; the list counts of halo copies are set to
+                    0, so the force kernels give them zero force and zero energy
+
+Exactness.  A local x coordinate is the global one minus a non-negative multiple of 2^-8 (or, for the one
+image each of rank 0 and the last rank takes through the box boundary, the Sterbenz-exact x - L plus the
+local box length, resp. the raw x): every such translation is exact in fp32 (the result is never larger
+than the coordinate it comes from, so it lies on that coordinate's grid), pair displacements in a local
+frame are bit-identical to the global ones, and after every drift the local x is rounded the way the
+global coordinate would be.  A decomposed run therefore differs from md_nve_step only in the order forces
+are summed (list order), not in any pair term.
+
+This module is plumbing: geometry, index lists, the order of the C-ABI calls, and the exchange.  `SlabRun`
+steps all ranks inside ONE process on one GPU (the exchange is a gather / scatter between the ranks'
+tensors) -- what the tests run; across processes the same index lists feed send / recv of the packed rows
+to the previous and next rank (`exchange_plan` returns exactly what travels).
+No multi-GPU timing exists: this run has one GPU.
+"""
+from __future__ import annotations
+
+import dataclasses
+import math
+
+import numpy as np
+import torch
+
+Q = 2.0 ** -8          # slab boundaries and translations are multiples of this (exact fp32 shifts)
+
+
+@dataclasses.dataclass
+class Frame:
+    """The local frame of one rank (all numbers exactly representable in fp32)."""
+    rank: int
+    world: int
+    lo: float              # slab [lo, hi) in global x
+    hi: float
+    T: float               # local x = global x - T for everything that is not a periodic image
+    Lx: float              # local box length in x
+    H: float               # halo width
+    G: float               # gap
+    L: float               # global box length in x
+
+    @property
+    def first(self) -> bool:
+        return self.rank == 0
+
+    @property
+    def last(self) -> bool:
+        return self.rank == self.world - 1
+
+    @property
+    def g2l_thr(self) -> float:
+        """Global x that separates plain copies from periodic images (global_to_local)."""
+        return 0.5 * (self.hi + self.L) if self.first else (0.5 * self.lo if self.last else 0.0)
+
+    @property
+    def l2g_thr(self) -> float:
+        """Local x that separates the zone of the images from the rest (local_to_global)."""
+        return self.hi + self.H + 0.5 * self.G if self.first else (self.H + 0.5 * self.G if self.last else 0.0)
+
+    def abi(self, B):
+        """The frame as the library's md_slab_frame (md.h)."""
+        return B.md_slab_frame(0 if self.first else (2 if self.last else 1), self.T, self.Lx, self.L,
+                               self.g2l_thr, self.l2g_thr)
+
+
+def frames(box_x: float, R: float, world: int) -> list[Frame]:
+    """Slab frames for `world` >= 2 ranks.  Layouts in local x (H = halo width = R rounded up to Q, G = gap):
+    rank 0:        [slab | high halo | gap | low halo = images of x in [L - H, L) at (x - L) + Lx]     T = 0
+    middle ranks:  [low halo | slab | high halo | gap]                                                  T = lo - H
+    last rank:     [high halo = images of x in [0, H) at their raw x | gap | low halo | slab]           T = lo - 2H - G,
+                                                                                                        Lx = L - T
+    In the first and the last frame the local box's own periodic wrap IS the global one: a particle of rank 0
+    that drifts below 0 reappears at the top of the local box, where the images of x near L live."""
+    if world < 2:
+        raise ValueError("a slab decomposition needs at least 2 ranks (one rank is md_nve_step itself)")
+    L = float(np.float32(box_x))
+    H = math.ceil(R / Q) * Q
+    W = L / world
+    los = [round(r * W / Q) * Q for r in range(world)] + [L]
+
+    def gap_for(base):
+        # at least R, and such that Lx / R sits mid-way between integers (the library refuses a box whose
+        # cell side is within 1e-5 of R)
+        k = math.floor((base + R) / R)
+        g = (k + 0.5) * R - base
+        while g < R:
+            g += R
+        return math.ceil(g / Q) * Q
+
+    out = []
+    for r in range(world):
+        lo, hi = los[r], los[r + 1]
+        width = hi - lo
+        G = gap_for(width + 2 * H)
+        if width < H:                    # a halo must come from the two adjacent slabs only
+            raise ValueError(f"box side {L} too small for {world} slabs of list radius {R}")
+        if r == 0:
+            fr = Frame(r, world, lo, hi, 0.0, width + 2 * H + G, H, G, L)
+        elif r == world - 1:
+            T = lo - 2 * H - G
+            if T < 0 or float(np.float32(L - T)) != L - T:
+                raise ValueError(f"box side {L} too small for {world} slabs of list radius {R}")
+            fr = Frame(r, world, lo, hi, T, L - T, H, G, L)
+        else:
+            fr = Frame(r, world, lo, hi, lo - H, width + 2 * H + G, H, G, L)
+        out.append(fr)
+    # images and plain copies must be told apart by x alone (global_to_local): rank 0's slab ends well
+    # below L - H, the last rank's begins well above H
+    if L - out[0].hi < 2 * (H + 1.0) or out[-1].lo < 2 * (H + 1.0):
+        raise ValueError(f"box side {L} too small for {world} slabs of list radius {R}")
+    return out
+
+
+def owner_of(xg: torch.Tensor, frs: list[Frame]) -> torch.Tensor:
+    """Rank whose slab holds global x (fp32 tensor)."""
+    bounds = torch.tensor([f.lo for f in frs[1:]], dtype=torch.float32, device=xg.device)
+    return torch.bucketize(xg.contiguous(), bounds, right=True)
+
+
+def global_to_local(xg: torch.Tensor, fr: Frame) -> torch.Tensor:
+    """Local x in frame fr of a particle at global x in [0, L) that lives in fr's slab or halo (fp32,
+    every operation exact: see the module text)."""
+    f32 = np.float32
+    if fr.first:
+        # x near L is the image through x = 0: (x - L) is Sterbenz-exact, + Lx lands on x's own grid
+        img = xg >= f32(fr.g2l_thr)
+        return torch.where(img, (xg - f32(fr.L)) + f32(fr.Lx), xg)
+    if fr.last:
+        # x near 0 is the image through x = L: x + L - T = x (mod Lx = L - T): the raw coordinate
+        img = xg < f32(fr.g2l_thr)
+        return torch.where(img, xg, xg - f32(fr.T))
+    return xg - f32(fr.T)
+
+
+def local_to_global(xl: torch.Tensor, fr: Frame) -> torch.Tensor:
+    """Global x in [0, L) of local x (the inverse of global_to_local; for a coordinate a drift has just
+    produced this is also where the global fp32 rounding happens)."""
+    f32 = np.float32
+    if fr.first:
+        img = xl >= f32(fr.l2g_thr)                            # the zone of the images at the top of the box
+        xg = torch.where(img, (xl - f32(fr.Lx)) + f32(fr.L), xl)
+    elif fr.last:
+        img = xl < f32(fr.l2g_thr)                             # the zone of the raw images at the bottom
+        xg = torch.where(img, xl, xl + f32(fr.T))
+    else:
+        xg = xl + f32(fr.T)
+    return torch.where(xg >= f32(fr.L), torch.zeros_like(xg), xg)    # x - tiny + L rounding to L
+
+
+def halo_select(xg: torch.Tensor, fr: Frame) -> torch.Tensor:
+    """Which particles (global x in [0, L)) are in fr's halo: within H below lo or above hi, periodically."""
+    f32 = np.float32
+    lo, hi, H, L = f32(fr.lo), f32(fr.hi), f32(fr.H), f32(fr.L)
+    high = (xg < H) if fr.last else ((xg >= hi) & (xg < hi + H))
+    low = (xg >= L - H) if fr.first else ((xg >= lo - H) & (xg < lo))
+    return high | low
+
+
+class LocalSystem:
+    """Device buffers of one rank with room for `cap` particles; the md_system is re-created at every
+    rebuild for the current count (allocation only; no arithmetic)."""
+
+    def __init__(self, B, w, fr: Frame, cap: int, device):
+        self.B, self.w, self.fr, self.cap, self.device = B, w, fr, cap, torch.device(device)
+        box = [fr.Lx, float(w.box[1]), float(w.box[2])]
+        self.cfg = B.make_config(w.dim, box, w.r_cut, w.skin, w.capacity, 1)
+        self.pot = B.make_potential(w.kind, w.epsilon, w.sigma, w.r_cut, w.shift, getattr(w, "alpha", 0.0))
+        dev = self.device
+        self.workspace = torch.empty(B.md_workspace_bytes(self.cfg, cap), dtype=torch.uint8, device=dev)
+        self.pos = torch.zeros(cap, 4, dtype=torch.float32, device=dev)
+        self.vel = torch.zeros(cap, 4, dtype=torch.float32, device=dev)
+        self.force = torch.zeros(cap, 4, dtype=torch.float32, device=dev)
+        self.id = torch.zeros(cap, dtype=torch.int32, device=dev)          # global id; -1 - id for a halo copy
+        self.sys = None
+        self.n = 0
+        self.perm = torch.zeros(cap, dtype=torch.int32, device=dev)
+        self.nbr_count = torch.zeros(cap, dtype=torch.int32, device=dev)
+        self.status = torch.zeros(2, dtype=torch.int32, device=dev)
+        self.flag = torch.zeros(1, dtype=torch.int32, device=dev)
+        self.energy = torch.zeros(1, dtype=torch.float64, device=dev)
+        self.nbr_idx = None
+        self.cell_start = None
+
+    def load(self, pos, vel, ids):
+        """New local particle set (owned first or not: the cell list re-sorts anyway)."""
+        B, n = self.B, pos.shape[0]
+        if n > self.cap:
+            raise RuntimeError(f"rank {self.fr.rank}: {n} local particles exceed the reserved {self.cap}")
+        if self.sys is not None:
+            torch.cuda.synchronize(self.device)
+            B.md_destroy(self.sys)
+        self.n = n
+        self.pos[:n] = pos; self.vel[:n] = vel; self.id[:n] = ids
+        self.sys = B.md_create(self.cfg, n, self.workspace)
+        ncell = B.md_num_cells(self.sys)
+        cells = ncell[0] * ncell[1] * ncell[2]
+        if self.cell_start is None or self.cell_start.numel() != cells + 1:
+            self.cell_start = torch.zeros(cells + 1, dtype=torch.int32, device=self.device)
+        length = B.md_nbr_layout(self.sys)[4]
+        if self.nbr_idx is None or self.nbr_idx.numel() < length:
+            self.nbr_idx = torch.empty(((self.cap + 31) // 32) * 32 * self.cfg.capacity, dtype=torch.int32, device=self.device)
+
+    def build(self):
+        B = self.B
+        B.md_cell_list_build(self.sys, self.pos, self.vel, self.id, self.cell_start, self.perm)
+        B.md_neighbor_list_build(self.sys, self.pos, self.cell_start, self.perm, self.nbr_idx, self.nbr_count, self.status)
+        n = self.n
+        self.nbr_count[:n].masked_fill_(self.id[:n] < 0, 0)      # halo copies: no force, no energy
+
+    def close(self):
+        if self.sys is not None:
+            torch.cuda.synchronize(self.device)
+            self.B.md_destroy(self.sys)
+            self.sys = None
+
+
+class SlabRank:
+    """One rank of the decomposition: its frame, its local system, and the phases of a step.  What leaves
+    a phase for another rank is a pair (float32 rows, int32 ids); what arrives comes from the PREVIOUS and
+    the NEXT rank only (periodically: rank 0's previous rank is the last one)."""
+
+    def __init__(self, B, w, fr: Frame, device, reserve: float = 1.35):
+        self.B, self.w, self.fr = B, w, fr
+        share = (fr.hi - fr.lo + 2 * fr.H) / fr.L
+        self.S = LocalSystem(B, w, fr, int(reserve * w.n * share) + 2048, device)
+        self.frames = frames(fr.L, float(np.float32(w.r_cut) + np.float32(w.skin)), fr.world)
+        self.prev, self.next = (fr.rank - 1) % fr.world, (fr.rank + 1) % fr.world
+        self.frame = fr.abi(B)      # the coordinate arithmetic of every phase runs in the library (md_slab_*)
+        self.rebuilds = 0
+        self._own = None            # (pos_g [k,4], vel [k,4], id [k]) between the phases of a rebuild
+        self._border_ids = (None, None)
+        self.border = (None, None)  # local slots of my border particles for (prev, next)
+        self.halo = (None, None)    # local slots of the copies that came from (prev, next), in arrival order
+
+    # ---- start and rebuild ------------------------------------------------------------------
+    def take_initial(self, pos_g, vel, gid):
+        """From the (replicated) initial state: my owned particles."""
+        mine = owner_of(pos_g[:, 0].contiguous(), self.frames) == self.fr.rank
+        self._own = (pos_g[mine].clone(), vel[mine].clone(), gid[mine].clone())
+
+    def leavers(self):
+        """Owned particles whose x has left the slab since the last rebuild: ((rows, ids) for prev, for next);
+        the stayers are kept for adopt()."""
+        S, fr = self.S, self.fr
+        n = S.n
+        owned = S.id[:n] >= 0
+        pos = S.pos[:n][owned].contiguous()
+        self.B.md_slab_convert(self.frame, pos, pos.shape[0], 0)           # x: local -> global
+        vel, gid = S.vel[:n][owned], S.id[:n][owned]
+        own = owner_of(pos[:, 0].contiguous(), self.frames)
+        stay, to_prev, to_next = own == fr.rank, own == self.prev, own == self.next
+        if fr.world == 2:                       # the other rank is both neighbours: below my slab or above it
+            lo = np.float32(fr.lo)
+            below = (pos[:, 0] < lo) if not fr.first else (pos[:, 0] >= np.float32(0.5 * (fr.hi + fr.L)))
+            to_prev, to_next = (own != fr.rank) & below, (own != fr.rank) & ~below
+        if int((stay | to_prev | to_next).sum()) != pos.shape[0]:
+            raise RuntimeError("a particle moved past a neighbouring slab between two rebuilds")
+        self._own = (pos[stay], vel[stay], gid[stay])
+        pack = lambda m: (torch.cat([pos[m], vel[m]], 1), gid[m])
+        return pack(to_prev), pack(to_next)
+
+    def adopt(self, from_prev, from_next):
+        """Migrants from the neighbours join my owned particles."""
+        pos, vel, gid = self._own
+        for rows, ids in (from_prev, from_next):
+            if rows is not None and rows.shape[0]:
+                pos = torch.cat([pos, rows[:, :4]]); vel = torch.cat([vel, rows[:, 4:]]); gid = torch.cat([gid, ids])
+        self._own = (pos, vel, gid)
+
+    def border_rows(self):
+        """My owned particles within H of my slab's faces: ((positions, ids) for prev, for next).  They
+        become the neighbours' halo copies; their ids, in this order, define what travels every step."""
+        pos, vel, gid = self._own
+        fr = self.fr
+        x = pos[:, 0]
+        f32 = np.float32
+        lo_side = x < f32(fr.lo + fr.H)                     # near my lower face: the previous rank's high halo
+        hi_side = x >= f32(fr.hi - fr.H)                    # near my upper face: the next rank's low halo
+        self._border_ids = (gid[lo_side].clone(), gid[hi_side].clone())
+        return (pos[lo_side], gid[lo_side]), (pos[hi_side], gid[hi_side])
+
+    def rebuild(self, halo_prev, halo_next):
+        """Local system = owned + the copies the neighbours sent; lists; index lists of the step exchange."""
+        pos, vel, gid = self._own
+        fr, S = self.fr, self.S
+        hp = torch.cat([halo_prev[0], halo_next[0]])
+        hid = torch.cat([halo_prev[1], halo_next[1]])
+        allpos = torch.cat([pos, hp]).contiguous()
+        self.B.md_slab_convert(self.frame, allpos, allpos.shape[0], 1)     # x: global -> local
+        S.load(allpos, torch.cat([vel, torch.zeros_like(hp)]), torch.cat([gid, -1 - hid]))
+        S.build()
+        self._own = None
+        # where everything ended up after the re-sort, through the ids
+        ids = S.id[: S.n].long()
+        n_all = self.w.n
+        slot_owned = torch.full((n_all,), -1, dtype=torch.long, device=ids.device)
+        slot_halo = torch.full((n_all,), -1, dtype=torch.long, device=ids.device)
+        where = torch.arange(S.n, device=ids.device)
+        slot_owned[ids[ids >= 0]] = where[ids >= 0]
+        slot_halo[-1 - ids[ids < 0]] = where[ids < 0]
+        self.border = tuple(slot_owned[b.long()].int().contiguous() for b in self._border_ids)
+        self.halo = (slot_halo[halo_prev[1].long()].int().contiguous(), slot_halo[halo_next[1].long()].int().contiguous())
+        self.rows_out = tuple(torch.empty(b.numel(), 4, dtype=torch.float32, device=ids.device) for b in self.border)
+        self.rebuilds += 1
+
+    # ---- the phases of an ordinary step ------------------------------------------------------
+    def drift(self):
+        """v += dt/2m F, r = mu(r, dt v) on the local system; x back on the global fp32 grid.  Returns the
+        device flag (1: one of my particles is more than skin / 2 from where the lists were built)."""
+        B, S, w = self.B, self.S, self.w
+        B.md_slab_kick_drift(S.sys, self.frame, S.pos, S.vel, S.force, w.dt, w.mass, S.flag)
+        return S.flag
+
+    def step_rows(self):
+        """New positions (global x) of my border particles, for (prev, next)."""
+        for slots, rows in zip(self.border, self.rows_out):
+            self.B.md_slab_pack(self.frame, self.S.pos, slots, rows)     # rows = pos[slots], x global
+        return self.rows_out
+
+    def absorb(self, from_prev, from_next):
+        for slots, rows in zip(self.halo, (from_prev, from_next)):
+            self.B.md_slab_unpack(self.frame, rows, slots, self.S.pos)   # pos[slots] = rows, x local (the image follows from x)
+
+    def force_kick(self):
+        S, w = self.S, self.w
+        self.B.md_force_half_kick(S.sys, S.pot, S.pos, S.nbr_idx, S.nbr_count, S.force, S.vel, w.dt, w.mass)
+
+    def first_force(self):
+        S = self.S
+        self.B.md_pair_energy_force(S.sys, S.pot, S.pos, S.nbr_idx, S.nbr_count, S.force, None)
+
+
+def rebuild_all(ranks, comm, initial=None):
+    """The rebuild protocol: migration to the neighbours, then the halo rows from the neighbours.
+    comm.shift(to_prev, to_next) delivers, for every rank, (what its previous rank sent to ITS next,
+    what its next rank sent to ITS previous)."""
+    if initial is None:
+        out = [r.leavers() for r in ranks]
+        got = comm.shift([o[0] for o in out], [o[1] for o in out])
+        for r, (fp, fn) in zip(ranks, got):
+            r.adopt(fp, fn)
+    else:
+        for r in ranks:
+            r.take_initial(*initial)
+    out = [r.border_rows() for r in ranks]
+    got = comm.shift([o[0] for o in out], [o[1] for o in out])
+    for r, (fp, fn) in zip(ranks, got):
+        r.rebuild(fp, fn)
+
+
+def step_all(ranks, comm, nsteps: int):
+    """nsteps velocity-Verlet steps of all ranks this process drives (one per process across GPUs)."""
+    for _ in range(nsteps):
+        flags = [r.drift() for r in ranks]
+        if comm.any_flag(flags):                                         # the one host read of the step
+            rebuild_all(ranks, comm)
+        else:
+            out = [r.step_rows() for r in ranks]
+            got = comm.shift([o[0] for o in out], [o[1] for o in out])
+            for r, (fp, fn) in zip(ranks, got):
+                r.absorb(fp, fn)
+        for r in ranks:
+            r.force_kick()
+
+
+class LocalComm:
+    """All ranks live in this process (tests on one GPU): a shift is a re-indexing of the lists."""
+
+    def __init__(self, world: int):
+        self.world = world
+
+    def shift(self, to_prev: list, to_next: list):
+        P = self.world
+        return [(to_next[(r - 1) % P], to_prev[(r + 1) % P]) for r in range(P)]
+
+    def any_flag(self, flags) -> bool:
+        return bool(torch.cat(flags).any())
+
+
+class DistComm:
+    """One rank per process over torch.distributed (NCCL across GPUs, gloo in the CPU test).  A message is a
+    tensor or a (rows, ids) pair of variable length: its row count travels first."""
+
+    def __init__(self, group=None):
+        import torch.distributed as dist
+        self.dist, self.group = dist, group
+        self.world, self.rank = dist.get_world_size(group), dist.get_rank(group)
+        self.prev, self.next = (self.rank - 1) % self.world, (self.rank + 1) % self.world
+
+    def _pairs(self, s_prev, s_next, r_prev, r_next):
+        """Point-to-point ops in an order both ends agree on without tags (NCCL has none): between two
+        ranks messages match in the order they are issued.  With world = 2 the other rank is both
+        neighbours: its first send (to its previous = me) is what I receive as `from next`."""
+        dist = self.dist
+        sends = [(s_prev, self.prev), (s_next, self.next)]
+        recvs = [(r_next, self.next), (r_prev, self.prev)] if self.world == 2 else [(r_prev, self.prev), (r_next, self.next)]
+        ops = [dist.P2POp(dist.isend, t, p, self.group) for t, p in sends if t is not None]
+        ops += [dist.P2POp(dist.irecv, t, p, self.group) for t, p in recvs if t is not None]
+        if ops:
+            for q in dist.batch_isend_irecv(ops):
+                q.wait()
+
+    def _sendrecv(self, t_prev: torch.Tensor, t_next: torch.Tensor, width, dtype):
+        dev = t_prev.device
+        n_out = torch.tensor([t_prev.shape[0], t_next.shape[0]], dtype=torch.int64, device=dev)
+        n_in = torch.zeros(2, dtype=torch.int64, device=dev)
+        self._pairs(n_out[0:1], n_out[1:2], n_in[0:1], n_in[1:2])
+        k_prev, k_next = int(n_in[0]), int(n_in[1])
+        r_prev = torch.empty((k_prev,) + tuple(width), dtype=dtype, device=dev)
+        r_next = torch.empty((k_next,) + tuple(width), dtype=dtype, device=dev)
+        # empty messages do not travel: both ends know the counts
+        self._pairs(t_prev.contiguous() if t_prev.shape[0] else None, t_next.contiguous() if t_next.shape[0] else None,
+                    r_prev if k_prev else None, r_next if k_next else None)
+        return r_prev, r_next
+
+    def shift(self, to_prev: list, to_next: list):
+        """Lists of length 1 (this process drives one rank)."""
+        a, b = to_prev[0], to_next[0]
+        if isinstance(a, tuple):
+            rp, rn = self._sendrecv(a[0], b[0], a[0].shape[1:], a[0].dtype)
+            ip, inn = self._sendrecv(a[1], b[1], (), a[1].dtype)
+            return [((rp, ip), (rn, inn))]
+        rp, rn = self._sendrecv(a, b, a.shape[1:], a.dtype)
+        return [(rp, rn)]
+
+    def any_flag(self, flags) -> bool:
+        f = flags[0].clone()
+        self.dist.all_reduce(f, op=self.dist.ReduceOp.MAX, group=self.group)
+        return bool(f.any())
+
+
+class SlabRun:
+    """`world` ranks of one process on one device, stepped in lockstep through LocalComm (tests, and
+    `bench.py --slabs`): the same SlabRank phases and the same neighbour-only messages a run with one
+    process per GPU makes through DistComm."""
+
+    def __init__(self, B, w, world: int, device="cuda:0", reserve: float = 1.35):
+        if w.dim != 3:
+            raise ValueError("slabs are implemented for 3-D systems")
+        self.B, self.w, self.world = B, w, world
+        R = float(np.float32(w.r_cut) + np.float32(w.skin))
+        self.frames = frames(float(np.float32(w.box[0])), R, world)
+        dev = torch.device(device)
+        self.device = dev
+        self.comm = LocalComm(world)
+        self.slab_ranks = [SlabRank(B, w, fr, dev, reserve) for fr in self.frames]
+        self.ranks = [r.S for r in self.slab_ranks]
+        pos = torch.from_numpy(w.pos).to(dev)
+        vel = torch.from_numpy(w.vel).to(dev)
+        gid = torch.arange(w.n, dtype=torch.int32, device=dev)
+        rebuild_all(self.slab_ranks, self.comm, initial=(pos, vel, gid))
+        for r in self.slab_ranks:
+            r.first_force()
+
+    @property
+    def rebuilds(self) -> int:
+        return self.slab_ranks[0].rebuilds - 1          # the initial build is not a rebuild
+
+    def exchange_plan(self):
+        """[(source rank, destination rank, rows)]: what travels every step (16 bytes per row)."""
+        out = []
+        for r in self.slab_ranks:
+            out.append((r.fr.rank, r.prev, int(r.border[0].numel())))
+            out.append((r.fr.rank, r.next, int(r.border[1].numel())))
+        return out
+
+    def step(self, nsteps: int):
+        step_all(self.slab_ranks, self.comm, nsteps)
+
+    # ---- results ------------------------------------------------------------------------------
+    def gather(self, with_force: bool = False):
+        """Owned particles of all ranks in global coordinates: (pos, vel, global id[, force])."""
+        ps, vs, gs, fs = [], [], [], []
+        for S in self.ranks:
+            n = S.n
+            owned = S.id[:n] >= 0
+            p = S.pos[:n][owned].contiguous()
+            self.B.md_slab_convert(S.fr.abi(self.B), p, p.shape[0], 0)
+            ps.append(p); vs.append(S.vel[:n][owned]); gs.append(S.id[:n][owned])
+            if with_force:
+                fs.append(S.force[:n][owned])
+        out = (torch.cat(ps), torch.cat(vs), torch.cat(gs))
+        return out + (torch.cat(fs),) if with_force else out
+
+    def energy(self) -> float:
+        E = 0.0
+        for S in self.ranks:
+            self.B.md_pair_energy_force(S.sys, S.pot, S.pos, S.nbr_idx, S.nbr_count, S.force, S.energy)
+            E += float(S.energy[0])
+        return E
+
+    def close(self):
+        for S in self.ranks:
+            S.close()
