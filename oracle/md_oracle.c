@@ -510,6 +510,7 @@ int orc_energy_force(int n, int dim, const double *pos, const double *diam,
     if ((kind == KIND_SOFT || kind == KIND_LJ_SPECIES || kind == KIND_BKS) && !diam) return ORC_EINVAL;
     if (kind == KIND_LJ_SPECIES && g_ns < 1) return ORC_EINVAL;
     if (kind == KIND_BKS && g_bks_ns < 1) return ORC_EINVAL;
+    if ((kind == KIND_MORSE || kind == KIND_BUCK) && !(g_morse_alpha == g_morse_alpha)) return ORC_EINVAL;   /* unset */
     double u_c = (kind == KIND_LJ && shift) ? lj_u_cut(eps, sigma, r_cut) : 0.0;
     if (kind == KIND_MORSE && shift) {
         double fr_unused;
@@ -919,6 +920,17 @@ int orc_langevin_run(int n, int dim, double *pos, double *vel, double *force, co
  * state = {xi_1..xi_M, v_1..v_M}. */
 #define ORC_MAX_NH_CHAIN 8
 static int g_nh_chain = 1;
+
+/* The parameters of kinds 2-5 and the chain length are process state set by the orc_set_* calls above.
+ * orc_reset_params puts all of it into the UNSET state, in which a call that needs one of them fails with
+ * ORC_EINVAL: the test suite calls it before every test, so no test can pass on what another one left. */
+void orc_reset_params(void)
+{
+    g_morse_alpha = NAN;
+    g_ns = 0;
+    g_bks_ns = 0;
+    g_nh_chain = 1;
+}
 int orc_set_nh_chain(int M)
 {
     if (M < 1 || M > ORC_MAX_NH_CHAIN) return ORC_EINVAL;

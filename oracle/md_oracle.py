@@ -128,6 +128,12 @@ def set_species_bks(A, B, Cc, q, coulomb_alpha, k_e=1.0):
                                      C.c_double(k_e)), "set_species_bks")
 
 
+def reset_params() -> None:
+    """Forget every orc_set_* parameter (Morse / Buckingham alpha, species tables, chain length): a later
+    call that needs one fails until it is set again.  tests/conftest.py does this before every test."""
+    lib().orc_reset_params()
+
+
 def set_morse_alpha(alpha: float) -> None:
     """alpha of kind 2 (Morse) for the following energy_force / nve_run calls."""
     lib().orc_set_morse_alpha(C.c_double(alpha))

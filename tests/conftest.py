@@ -20,6 +20,16 @@ def orc():
     return md_oracle
 
 
+@pytest.fixture(autouse=True)
+def _oracle_parameters_do_not_leak():
+    """The oracle keeps the parameters of kinds 2-5 (and the thermostat chain length) as process state:
+    every test starts from the UNSET state, so none can pass on what another left behind."""
+    from oracle import md_oracle
+    if os.path.exists(md_oracle._LIB):
+        md_oracle.reset_params()
+    yield
+
+
 @pytest.fixture(scope="session")
 def W():
     from paper_1912_04232_b200 import workloads
