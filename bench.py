@@ -234,31 +234,43 @@ def run_next_rows(args):
         torch.cuda.synchronize()
         return a.elapsed_time(b) * 1e3 / nsteps
 
-    # f2: potentials on the fp64 pair chain (LJ first, for scale: fp32 fast path, then fp64 chain)
+    # f2: the pair force of every potential on two states of the same particles, the lattice as generated
+    # and the liquid it melts into; LJ, Morse and Buckingham on the fp32 fast path with fp64 re-evaluation
+    # (their default) and on the fp64 pair chain ("fast32" = 0), species LJ and BKS on the chain only
     S = B.System(base)
-    emit("f2", "LJ force, fp32 fast path with fp64 re-evaluation (the headline kernel)", time_force(S))
-    B.md_set_option(S.sys, "fast32", 0)
-    emit("f2", "LJ force, fp64 pair chain", time_force(S))
+    S.build(); S.compute_force(); S.step(400)
+    torch.cuda.synchronize()
+    liquid = np.empty_like(base.pos)
+    liquid[S.id.cpu().numpy()] = S.pos.cpu().numpy()
     S.close()
-    w = dataclasses.replace(base, kind=W.KIND_MORSE, epsilon=1.0, sigma=1.12, alpha=5.0)
-    S = B.System(w); emit("f2", "Morse force (D=1, alpha=5, r0=1.12), fp64 pair chain", time_force(S)); S.close()
-    w = dataclasses.replace(base, kind=W.KIND_BUCKINGHAM, epsilon=float(np.float32(9.02e5)),
-                            sigma=float(np.float32(3.454)), alpha=12.5)
-    S = B.System(w); emit("f2", "Buckingham exp-6 force, fp64 pair chain", time_force(S)); S.close()
-    pos = base.pos.copy()
-    pos[:, 3] = (np.arange(n) % 5 == 0).astype(np.float32)
-    w = dataclasses.replace(base, kind=W.KIND_LJ_SPECIES, pos=pos)
-    S = B.System(w)
+    states = [("lattice as generated", base.pos), ("liquid, after 400 LJ steps", liquid)]
     eps = np.array([[1.0, 1.5], [1.5, 0.5]], np.float32)
     sig = np.array([[1.0, 0.8], [0.8, 0.88]], np.float32)
-    B.md_set_species_lj(S.sys, eps, sig, (2.5 * sig).astype(np.float32))
-    emit("f2", "species x species LJ force (80:20 binary mixture), fp64 pair chain", time_force(S)); S.close()
-
-    w = dataclasses.replace(base, kind=W.KIND_BKS, pos=pos, r_cut=2.5)
-    S = B.System(w)
     one = np.ones((2, 2), np.float32)
-    B.md_set_species_bks(S.sys, 9.02e5 * one, 12.5 * one, 3.454 * one, np.array([0.6, -0.6], np.float32), 0.3, 1.0)
-    emit("f2", "BKS-type force (exp-6 + damped shifted-force Coulomb, 2 species), fp64 pair chain", time_force(S)); S.close()
+    potentials = [
+        ("LJ (the headline kernel)", dict(), True, None),
+        ("Morse (D=1, alpha=5, r0=1.12)", dict(kind=W.KIND_MORSE, epsilon=1.0, sigma=1.12, alpha=5.0), True, None),
+        ("Buckingham exp-6", dict(kind=W.KIND_BUCKINGHAM, epsilon=float(np.float32(9.02e5)),
+                                  sigma=float(np.float32(3.454)), alpha=12.5), True, None),
+        ("species x species LJ (80:20 binary mixture)", dict(kind=W.KIND_LJ_SPECIES), False,
+         lambda S: B.md_set_species_lj(S.sys, eps, sig, (2.5 * sig).astype(np.float32))),
+        ("BKS-type (exp-6 + damped shifted-force Coulomb, 2 species)", dict(kind=W.KIND_BKS, r_cut=2.5), False,
+         lambda S: B.md_set_species_bks(S.sys, 9.02e5 * one, 12.5 * one, 3.454 * one,
+                                        np.array([0.6, -0.6], np.float32), 0.3, 1.0)),
+    ]
+    for what, over, fast, setup in potentials:
+        for sname, spos in states:
+            pos = spos.copy()
+            if setup is not None:
+                pos[:, 3] = (np.arange(n) % 5 == 0).astype(np.float32)
+            S = B.System(dataclasses.replace(base, pos=pos, **over))
+            if setup is not None:
+                setup(S)
+            if fast:
+                emit("f2", f"{what} force, fp32 fast path with fp64 re-evaluation", time_force(S), state=sname)
+                B.md_set_option(S.sys, "fast32", 0)
+            emit("f2", f"{what} force, fp64 pair chain", time_force(S), state=sname)
+            S.close()
 
     # f3: update rules, LJ fast path, 200 steps each
     steps = 200

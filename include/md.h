@@ -94,11 +94,14 @@ int md_create(const md_config *cfg, int n, void *workspace, size_t bytes, md_sys
 int md_destroy(md_system *sys);
 
 /* Tuning knobs (host call; drops the cached step graph):
- *   "fast32"               1 (default): 3-D LJ forces by the fp32 fast path with an error estimate
- *                          and fp64 re-evaluation of the particles that need it;
- *                          0: every pair in fp64 (the kernels selected by threads_per_particle)
- *   "est_thr"              the fast path re-evaluates particle i in fp64 when
- *                          sum_j |f_ij / r_ij| > est_thr * max(|F_i|, 1e-3); default 8
+ *   "fast32"               1 (default): 3-D LJ, Morse and Buckingham forces by the fp32 fast path with
+ *                          an error estimate and fp64 re-evaluation of the particles that need it
+ *                          (DESIGN.md §5); 0: every pair in fp64 (the kernels selected by
+ *                          threads_per_particle), as SOFT, LJ_SPECIES, BKS and every 2-D system always
+ *   "est_thr"              the fast path re-evaluates particle i in fp64 when S_i, the sum over j of
+ *                          the pair's error scale (LJ: |f_ij / r_ij|; Morse and Buckingham: the parts
+ *                          of f_ij / r_ij times the amplification of their exponentials, scaled to
+ *                          LJ's), exceeds est_thr * max(|F_i|, 1e-3); default 8
  *   "threads_per_particle" fp64 force kernel variant: 0 = streaming kernel (one lane per particle,
  *                          list rows staged through shared memory by TMA; default for
  *                          n >= 32768), or 1, 2, 4 lanes sharing one particle (default 4 below)
@@ -278,7 +281,7 @@ int md_needs_rebuild(md_system *sys, const void *pos, int32_t *flag, void *strea
  *   nbr_idx / nbr_count  any list in the md_nbr_layout layout whose rows hold every pair
  *                        within the potential's range (entries beyond it contribute nothing)
  * Precision: SOFT, 2-D and fast32 = 0: pair terms evaluated and accumulated in fp64
- * from exact displacements; 3-D LJ (default): fp32 pair terms with a per-particle error estimate,
+ * from exact displacements; 3-D LJ, Morse, Buckingham (default): fp32 pair terms with a per-particle error estimate,
  * fp64 re-evaluation of every particle whose estimate exceeds 1/3 of the 1e-5 force tolerance or
  * that has a pair within 1e-5 r_cut^2 of the truncation radius.  Rounded to fp32 once, on store.
  */

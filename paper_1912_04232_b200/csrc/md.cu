@@ -396,13 +396,20 @@ int launch_force_t(md_system *s, const Pair &pp, const float4 *pos, const int *n
     return MD_OK;
 }
 
+// The kinds md_force32.cuh serves (3-D only): fp32 pair math, error estimate, fp64 re-evaluation.
+static bool fast32_kind(const md_system *s, const Pair &pp) {
+    return s->fast32 && s->g.dim == 3 &&
+           (pp.kind == MD_KIND_LJ || pp.kind == MD_KIND_MORSE || pp.kind == MD_KIND_BUCKINGHAM);
+}
+
 // want_energy: also e_i into force.w (and the fp64 total when etot != NULL); the step loop
 // does not need it and skips those fp64 operations (force.w = 0 there).
 int launch_force(md_system *s, const Pair &pp, const float4 *pos, const int *nbr_idx,
                  const int *nbr_count, float4 *force, float4 *vel, float a, double *etot,
                  bool want_energy, Book book, cudaStream_t st, NextStep nx = NextStep()) {
-    if (s->fast32 && pp.kind == MD_KIND_LJ && s->g.dim == 3) {
+    if (fast32_kind(s, pp)) {
         Pair32 q;
+        memset(&q, 0, sizeof(q));
         q.rc2 = (float)pp.drc2;
         q.sig6x2 = (float)pp.dsig6x2;
         q.ucut4 = (float)pp.du_cut4;
@@ -410,14 +417,30 @@ int launch_force(md_system *s, const Pair &pp, const float4 *pos, const int *nbr
         q.escale = (float)(2.0 * pp.deps);
         q.near_band = 1e-5f * q.rc2;
         q.est_thr = s->est_thr;
+        if (pp.kind == MD_KIND_MORSE) {
+            const double k = -pp.dalpha * 1.4426950408889634;
+            q.k_hi = (float)k; q.k_lo = (float)(k - (double)q.k_hi); q.s_unit = 0.025f;
+            q.m_r0 = (float)pp.dr0; q.m_2a = (float)(2.0 * pp.dalpha); q.m_a = (float)pp.dalpha;
+            q.ucut4 = (float)pp.du_cutm; q.fscale = (float)pp.deps; q.escale = (float)(0.5 * pp.deps);
+        } else if (pp.kind == MD_KIND_BUCKINGHAM) {
+            const double k = -pp.dalpha * 1.4426950408889634;
+            q.k_hi = (float)k; q.k_lo = (float)(k - (double)q.k_hi); q.s_unit = 0.025f;
+            q.b_A = (float)pp.dA; q.b_B = (float)pp.dalpha; q.b_C = (float)pp.dC;
+            q.ucut4 = (float)pp.du_cutm; q.fscale = 1.0f; q.escale = 0.5f;
+        }
         Geom gr = s->g;
         gr.n = s->r1;                                  // md_set_range: lanes beyond r1 are idle
         const int nb = blocks_for(s->r1 - s->r0, F32_WARPS * 32);
         int *nfix = s->words + 8;
         int P = 0, grid = nb;
         if (s->remap > 0 && nb > 4 * s->remap) { P = s->remap; grid = P * ((nb + P - 1) / P); }
-        if (want_energy) k_force_lj32<true><<<grid, F32_WARPS * 32, 0, st>>>(gr, pp, q, pos, nbr_idx, nbr_count, force, vel, a, etot, book, nfix, nx, P, nb, s->r0);
-        else k_force_lj32<false><<<grid, F32_WARPS * 32, 0, st>>>(gr, pp, q, pos, nbr_idx, nbr_count, force, vel, a, etot, book, nfix, nx, P, nb, s->r0);
+#define MD_F32_CASE(K)                                                                                      \
+    case K:                                                                                                 \
+        if (want_energy) k_force32<K, true><<<grid, F32_WARPS * 32, 0, st>>>(gr, pp, q, pos, nbr_idx, nbr_count, force, vel, a, etot, book, nfix, nx, P, nb, s->r0); \
+        else k_force32<K, false><<<grid, F32_WARPS * 32, 0, st>>>(gr, pp, q, pos, nbr_idx, nbr_count, force, vel, a, etot, book, nfix, nx, P, nb, s->r0); \
+        break;
+        switch (pp.kind) { MD_F32_CASE(0) MD_F32_CASE(2) MD_F32_CASE(3) }
+#undef MD_F32_CASE
         LAUNCH_OK();
         return MD_OK;
     }
@@ -659,7 +682,7 @@ int capture(md_system *s, const Pair &pp, const StepKey &k, int reps, cudaGraphE
     if (!s->cap_stream) CU(cudaStreamCreateWithFlags(&s->cap_stream, cudaStreamNonBlocking));
     CU(cudaStreamBeginCapture(s->cap_stream, cudaStreamCaptureModeThreadLocal));
     int rc = MD_OK;
-    if (s->fast32 && s->fused && pp.kind == MD_KIND_LJ && s->g.dim == 3 && (reps & 1))
+    if (fast32_kind(s, pp) && s->fused && (reps & 1))
         rc = record_fused(s, pp, (float4 *)k.pos, (float4 *)k.vel, (float4 *)k.force, (int *)k.id,
                           (int *)k.nbr_idx, (int *)k.nbr_count, k.dt, k.mass, (int *)k.stats, reps,
                           s->cap_stream);
@@ -1133,7 +1156,7 @@ int md_nve_step(md_system *sys, const md_potential *pot, void *pos, void *vel, v
     LAUNCH_OK();
     if (!sys->use_graph) {
         int left = nsteps;
-        if (sys->fast32 && sys->fused && pp.kind == MD_KIND_LJ && sys->g.dim == 3 && left > 0) {
+        if (fast32_kind(sys, pp) && sys->fused && left > 0) {
             // fused loop over an odd number of steps; an even count takes its first step unfused
             if (!(left & 1)) {
                 rc = record_step(sys, pp, (float4 *)pos, (float4 *)vel, (float4 *)force, id, nbr_idx,

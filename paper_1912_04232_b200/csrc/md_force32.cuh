@@ -34,6 +34,11 @@ struct Pair32 {
     float escale;       // 2 eps   (= 1/2 * 4 eps)
     float near_band;    // |r2 - rc2| <= near_band -> exact re-evaluation
     float est_thr;      // re-evaluate when fscale * S_i > est_thr * max(|F_i|, 1e-3)
+    // the other kinds of the fast path (the estimate term of each is scaled so that one est_thr serves all)
+    float k_hi, k_lo;                 // MORSE: -alpha log2(e), BUCKINGHAM: -B log2(e), as a float and what it drops
+    float s_unit;                     // scale of the estimate term against Lennard-Jones's
+    float m_r0, m_2a, m_a;            // MORSE: r0, 2 alpha, alpha;  ucut4 = shift * u(r_cut) / D
+    float b_A, b_B, b_C;              // BUCKINGHAM: A, B, C;        ucut4 = shift * u(r_cut)
 };
 
 struct Acc32 { float fx, fy, fz, s, e, near; };
@@ -106,9 +111,92 @@ __device__ __forceinline__ void lj_pair32x2(const Pair32 &pp, float2 dx, float2 
     }
 }
 
+__device__ __forceinline__ float ex2_32(float x) {
+    float y;
+    asm("ex2.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+__device__ __forceinline__ float rsq32(float x) {
+    float y;
+    asm("rsqrt.approx.ftz.f32 %0, %1;" : "=f"(y) : "f"(x));
+    return y;
+}
+
+// The same for the other kinds of the fast path.  Each accumulates the force coefficient c (force = c d),
+// the energy term and S, the scale of the coefficient's fp32 error: |c| times the factor by which the pair's
+// functional form amplifies a relative error of r (normalised to Lennard-Jones, where it is ~10), with the
+// floor that keeps S honest where c changes sign.
+template <int KIND, bool ENERGY>
+__device__ __forceinline__ void pair32x2(const Pair32 &pp, float2 dx, float2 dy, float2 dz, Acc2s &a) {
+    if (KIND == 0) { lj_pair32x2<ENERGY>(pp, dx, dy, dz, a); return; }
+    const float2 r2 = __ffma2_rn(dz, dz, __ffma2_rn(dy, dy, __fmul2_rn(dx, dx)));
+    const float2 w = __fadd2_rn(r2, make_float2(-pp.rc2, -pp.rc2));
+    a.near = fminf(a.near, fminf(fabsf(w.x), fabsf(w.y)));
+    const float2 m = make_float2(w.x < 0.0f ? 1.0f : 0.0f, w.y < 0.0f ? 1.0f : 0.0f);
+    // r and 1/r to an ulp from the 2-ulp hardware rsqrt (one Newton step), and the part of r that fp32
+    // drops: an exponential amplifies the relative error of r by alpha r ~ 5..15
+    const float2 ir0 = make_float2(rsq32(r2.x), rsq32(r2.y));
+    const float2 h = __fmul2_rn(r2, ir0);
+    const float2 nr = __ffma2_rn(make_float2(-h.x, -h.y), ir0, make_float2(1.0f, 1.0f));        // 1 - r2 ir0^2
+    const float2 r = __ffma2_rn(__fmul2_rn(h, make_float2(0.5f, 0.5f)), nr, h);
+    const float2 hir = __ffma2_rn(__fmul2_rn(ir0, make_float2(0.25f, 0.25f)), nr, __fmul2_rn(ir0, make_float2(0.5f, 0.5f)));   // 1 / (2 r)
+    const float2 ir = __fadd2_rn(hir, hir);
+    const float2 r_lo = __fmul2_rn(__ffma2_rn(make_float2(-r.x, -r.y), r, r2), hir);            // (r2 - r^2) / (2 r)
+    if (KIND == 2) {
+        // u / D = (1 - x)^2 - 1, x = exp(-alpha (r - r0));  c = -u'(r) / r / D = -2 alpha x (1 - x) / r
+        // the exponent k (r - r0), k = -alpha log2(e) = k_hi + k_lo, as a rounded product plus its remainder
+        const float2 d = __fadd2_rn(r, make_float2(-pp.m_r0, -pp.m_r0));
+        const float2 khi = make_float2(pp.k_hi, pp.k_hi);
+        const float2 a_hi = __fmul2_rn(d, khi);
+        float2 a_lo = __ffma2_rn(d, khi, make_float2(-a_hi.x, -a_hi.y));
+        a_lo = __ffma2_rn(d, make_float2(pp.k_lo, pp.k_lo), a_lo);
+        a_lo = __ffma2_rn(r_lo, khi, a_lo);
+        float2 x = make_float2(ex2_32(a_hi.x), ex2_32(a_hi.y));
+        x = __ffma2_rn(__fmul2_rn(x, make_float2(0.69314718f, 0.69314718f)), a_lo, x);
+        x = __fmul2_rn(x, m);
+        const float2 om = __fadd2_rn(make_float2(1.0f, 1.0f), make_float2(-x.x, -x.y));
+        const float2 g2 = __fmul2_rn(__fmul2_rn(x, ir), make_float2(pp.m_2a, pp.m_2a));       // 2 alpha x / r
+        const float2 c = __fmul2_rn(g2, make_float2(-om.x, -om.y));
+        a.fx = __ffma2_rn(c, dx, a.fx); a.fy = __ffma2_rn(c, dy, a.fy); a.fz = __ffma2_rn(c, dz, a.fz);
+        // error of c: x and 1 - x both carry x alpha r eps_r, 1/r carries eps_r
+        const float2 aom = make_float2(pp.s_unit * fabsf(om.x), pp.s_unit * fabsf(om.y));
+        const float2 amp = __ffma2_rn(__ffma2_rn(x, make_float2(pp.s_unit, pp.s_unit), aom),
+                                      __fmul2_rn(r, make_float2(pp.m_a, pp.m_a)), aom);
+        a.s = __ffma2_rn(g2, amp, a.s);
+        if (ENERGY) {
+            float2 e = __ffma2_rn(om, om, make_float2(-1.0f - pp.ucut4, -1.0f - pp.ucut4));
+            a.e = __ffma2_rn(e, m, a.e);
+        }
+    } else {
+        // u = A exp(-B r) - C / r^6;  c = (A B exp(-B r) r - 6 C / r^6) / r^2
+        const float2 y = __fmul2_rn(__fmul2_rn(ir, ir), m);
+        const float2 y3 = __fmul2_rn(__fmul2_rn(y, y), y);
+        const float2 khi = make_float2(pp.k_hi, pp.k_hi);                                     // -B log2(e)
+        const float2 a_hi = __fmul2_rn(r, khi);
+        float2 a_lo = __ffma2_rn(r, khi, make_float2(-a_hi.x, -a_hi.y));
+        a_lo = __ffma2_rn(r, make_float2(pp.k_lo, pp.k_lo), a_lo);
+        a_lo = __ffma2_rn(r_lo, khi, a_lo);
+        float2 x = make_float2(ex2_32(a_hi.x), ex2_32(a_hi.y));
+        x = __ffma2_rn(__fmul2_rn(x, make_float2(0.69314718f, 0.69314718f)), a_lo, x);
+        x = __fmul2_rn(x, make_float2(pp.b_A, pp.b_A));
+        const float2 t1 = __fmul2_rn(__fmul2_rn(x, r), make_float2(pp.b_B, pp.b_B));
+        const float2 t2 = __fmul2_rn(y3, make_float2(6.0f * pp.b_C, 6.0f * pp.b_C));
+        const float2 c = __fmul2_rn(__fadd2_rn(t1, make_float2(-t2.x, -t2.y)), y);
+        a.fx = __ffma2_rn(c, dx, a.fx); a.fy = __ffma2_rn(c, dy, a.fy); a.fz = __ffma2_rn(c, dz, a.fz);
+        // error of c: the exponential amplifies by B r + 3, the power law by 8
+        const float2 k1 = __ffma2_rn(r, make_float2(pp.s_unit * pp.b_B, pp.s_unit * pp.b_B), make_float2(3.0f * pp.s_unit, 3.0f * pp.s_unit));
+        const float2 amp = __ffma2_rn(t1, k1, __fmul2_rn(t2, make_float2(8.0f * pp.s_unit, 8.0f * pp.s_unit)));
+        a.s = __ffma2_rn(amp, y, a.s);
+        if (ENERGY) {
+            float2 e = __ffma2_rn(y3, make_float2(-pp.b_C, -pp.b_C), __fadd2_rn(x, make_float2(-pp.ucut4, -pp.ucut4)));
+            a.e = __ffma2_rn(e, m, a.e);
+        }
+    }
+}
+
 // Exact re-evaluation of one particle by a group of G = 8, 16 or 32 lanes striding over its row
 // (32 / G particles per warp at a time); the sum is returned in every lane of the group.
-template <bool ENERGY, bool WRAP>
+template <int KIND, bool ENERGY, bool WRAP>
 __device__ __forceinline__ Acc64 lj_row64(const Geom &g, const Pair &pp,
                                           const float4 *__restrict__ pos, const int *col, int cnt,
                                           const float4 &pb, int sub, int G) {
@@ -120,8 +208,8 @@ __device__ __forceinline__ Acc64 lj_row64(const Geom &g, const Pair &pp,
         const int j2 = v2 ? col[(k + G) * TILE] : j1;
         MD_CHECK(j1 >= 0 && j1 < g.ntot && j2 >= 0 && j2 < g.ntot);
         const float4 q1 = pos[j1], q2 = pos[j2];
-        pair_any<0, 3, ENERGY, WRAP>(pp, me, q1, true, acc);
-        pair_any<0, 3, ENERGY, WRAP>(pp, me, q2, v2, acc);
+        pair_any<KIND, 3, ENERGY, WRAP>(pp, me, q1, true, acc);
+        pair_any<KIND, 3, ENERGY, WRAP>(pp, me, q2, v2, acc);
     }
     for (int o = G >> 1; o > 0; o >>= 1) {              // G is warp-uniform
         acc.fx += __shfl_xor_sync(FULL, acc.fx, o);
@@ -147,7 +235,7 @@ constexpr int F32_U = MD_F32_U;
 // The pair loop of one lane over its column of the tile: rows [0, kmin) are owned by every lane
 // of the warp (no validity test), rows [kmin, kmax) are the ragged tail.  WX / WY / WZ: the warp
 // is near a box face in that direction and takes the nearest image there (warp-uniform).
-template <bool ENERGY, bool WX, bool WY, bool WZ>
+template <int KIND, bool ENERGY, bool WX, bool WY, bool WZ>
 __device__ __forceinline__ void lj_rows32(const Geom &g, const Pair32 &p32,
                                           const float4 *__restrict__ pos, const int *col,
                                           const float4 &pi, int ii, int cnt, int kmin, int kmax,
@@ -171,7 +259,7 @@ __device__ __forceinline__ void lj_rows32(const Geom &g, const Pair32 &p32,
         float ax, ay, az, bx, by, bz;
         disp(qa, ax, ay, az);
         disp(qb, bx, by, bz);
-        lj_pair32x2<ENERGY>(p32, make_float2(ax, bx), make_float2(ay, by), make_float2(az, bz), a2);
+        pair32x2<KIND, ENERGY>(p32, make_float2(ax, bx), make_float2(ay, by), make_float2(az, bz), a2);
     };
     int k = 0;
     int jn[F32_U];
@@ -223,9 +311,9 @@ struct NextStep {
     cudaGraphConditionalHandle cond;
     int has_cond;
 };
-template <bool ENERGY>
+template <int KIND, bool ENERGY>
 __global__ void __launch_bounds__(F32_WARPS * 32, MD_F32_MINBLOCKS)
-k_force_lj32(Geom g, Pair pp, Pair32 p32, const float4 *__restrict__ pos,
+k_force32(Geom g, Pair pp, Pair32 p32, const float4 *__restrict__ pos,
              const int *__restrict__ nbr_idx, const int *__restrict__ nbr_count,
              float4 *__restrict__ force, float4 *__restrict__ vel, float a, double *energy_total,
              Book book, int *nfix, NextStep nx, int remap_p, int nblocks, int i0) {
@@ -253,11 +341,11 @@ k_force_lj32(Geom g, Pair pp, Pair32 p32, const float4 *__restrict__ pos,
     const bool wz = __any_sync(FULL, active && (pi.z < g.face || pi.z > g.L[2] - g.face));
     Acc32 acc = {0.0f, 0.0f, 0.0f, 0.0f, 0.0f, 1e30f};
 
-    if (!(wx || wy || wz)) lj_rows32<ENERGY, false, false, false>(g, p32, pos, col, pi, ii, cnt, kmin, kmax, active, acc);
-    else if (wx && !wy && !wz) lj_rows32<ENERGY, true, false, false>(g, p32, pos, col, pi, ii, cnt, kmin, kmax, active, acc);
-    else if (!wx && wy && !wz) lj_rows32<ENERGY, false, true, false>(g, p32, pos, col, pi, ii, cnt, kmin, kmax, active, acc);
-    else if (!wx && !wy && wz) lj_rows32<ENERGY, false, false, true>(g, p32, pos, col, pi, ii, cnt, kmin, kmax, active, acc);
-    else lj_rows32<ENERGY, true, true, true>(g, p32, pos, col, pi, ii, cnt, kmin, kmax, active, acc);
+    if (!(wx || wy || wz)) lj_rows32<KIND, ENERGY, false, false, false>(g, p32, pos, col, pi, ii, cnt, kmin, kmax, active, acc);
+    else if (wx && !wy && !wz) lj_rows32<KIND, ENERGY, true, false, false>(g, p32, pos, col, pi, ii, cnt, kmin, kmax, active, acc);
+    else if (!wx && wy && !wz) lj_rows32<KIND, ENERGY, false, true, false>(g, p32, pos, col, pi, ii, cnt, kmin, kmax, active, acc);
+    else if (!wx && !wy && wz) lj_rows32<KIND, ENERGY, false, false, true>(g, p32, pos, col, pi, ii, cnt, kmin, kmax, active, acc);
+    else lj_rows32<KIND, ENERGY, true, true, true>(g, p32, pos, col, pi, ii, cnt, kmin, kmax, active, acc);
 
     // ---- fp32 result, error estimate, exact re-evaluation of the lanes that need it
     float fx = p32.fscale * acc.fx, fy = p32.fscale * acc.fy, fz = p32.fscale * acc.fz;
@@ -289,8 +377,8 @@ k_force_lj32(Geom g, Pair pp, Pair32 p32, const float4 *__restrict__ pos,
         int cb = __shfl_sync(FULL, cnt, bb);              // every lane takes part in the shuffle
         if (b < 0) cb = 0;
         // away from every face the fp32 difference is exact for every pair inside the cutoff
-        const Acc64 r = (wx || wy || wz) ? lj_row64<ENERGY, true>(g, pp, pos, tile0 + bb, cb, pb, sub, G)
-                                         : lj_row64<ENERGY, false>(g, pp, pos, tile0 + bb, cb, pb, sub, G);
+        const Acc64 r = (wx || wy || wz) ? lj_row64<KIND, ENERGY, true>(g, pp, pos, tile0 + bb, cb, pb, sub, G)
+                                         : lj_row64<KIND, ENERGY, false>(g, pp, pos, tile0 + bb, cb, pb, sub, G);
         // deliver: the lane whose rank among the flagged lanes is q < ng reads group q
         const int rank = __popc(todo & ((1u << lane) - 1u));
         const bool mine = ((todo >> lane) & 1u) && rank < ng;
@@ -299,9 +387,11 @@ k_force_lj32(Geom g, Pair pp, Pair32 p32, const float4 *__restrict__ pos,
         const double rz = __shfl_sync(FULL, r.fz, src);
         const double re = ENERGY ? __shfl_sync(FULL, r.e, src) : 0.0;
         if (mine) {
-            const double fs = 12.0 * pp.deps * pp.dsig6x2;
+            // as force_epilogue: 24 eps sigma^6 | D | 1 and half of 4 eps | D | 1
+            const double fs = KIND == 0 ? 12.0 * pp.deps * pp.dsig6x2 : (KIND == 2 ? pp.deps : 1.0);
+            const double es = KIND == 0 ? 2.0 * pp.deps : (KIND == 2 ? 0.5 * pp.deps : 0.5);
             fx = (float)(fs * rx); fy = (float)(fs * ry); fz = (float)(fs * rz);
-            if (ENERGY) e64 = 2.0 * pp.deps * re;
+            if (ENERGY) e64 = es * re;
         }
         todo = t;
     }

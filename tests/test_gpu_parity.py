@@ -544,6 +544,7 @@ def test_bks_type_binary_crystal(B, orc, W):
     B.md_set_species_bks(S5.sys, f32(A0) * one, f32(B0) * one, f32(C0) * one, f32([0.0, 0.0]), alpha_c, ke)
     w3 = dataclasses.replace(w, kind=3, epsilon=float(np.float32(A0)), sigma=float(np.float32(C0)), alpha=float(np.float32(B0)))
     S3 = B.System(w3)
+    B.md_set_option(S3.sys, "fast32", 0)              # the fp64 Buckingham chain, term by term the same arithmetic
     for X in (S5, S3):
         X.build(); X.compute_force()
     torch.cuda.synchronize()
@@ -1200,6 +1201,10 @@ def test_other_potentials_at_full_size(B, orc, W, kind):
         B.md_set_species_bks(S.sys, Am, Bm, Cm, q, float(np.float32(0.3)), 1.0)
         orc.set_species_bks(d64(Am), d64(Bm), d64(Cm), d64(q), float(np.float32(0.3)), 1.0)
     S.build()
+    # Morse and Buckingham default to the fp32 fast path with fp64 re-evaluation (as LJ does);
+    # "fast32" = 0 puts them on the fp64 kernels, which species LJ and BKS always use
+    state_force_parity(S, orc, w, alpha=alpha, species=species)
+    B.md_set_option(S.sys, "fast32", 0)
     state_force_parity(S, orc, w, alpha=alpha, species=species)
     # and the small-system kernel variant on the same state gives the same forces to rounding
     f_stream = S.force.clone()
@@ -1325,6 +1330,40 @@ def test_fast32_estimator_away_from_its_calibration(B, orc, W, name, gen, steps,
     B.md_counters(S.sys, cnt, reset=True); S.compute_force(); B.md_counters(S.sys, cnt)
     torch.cuda.synchronize()
     print(f"fast32 [{name}]: worst error {worst:.3f} x 1e-5, re-evaluated {int(cnt[0])} of {w.n}")
+    S.close()
+
+
+F2_STATES = [
+    ("morse alpha 3, r0 1.0, rho 0.6 after 200 steps", "morse", dict(rho=0.6), 200, dict(epsilon=0.5, sigma=1.0, alpha=3.0, dt=0.002)),
+    ("morse alpha 8, r0 1.2, jittered lattice", "morse", dict(), 0, dict(epsilon=2.0, sigma=1.2, alpha=8.0)),
+    ("morse alpha 5, T = 3 after 200 steps", "morse", dict(temperature=3.0), 200, dict(epsilon=0.9, sigma=1.12, alpha=5.0, dt=0.002)),
+    ("buckingham B 10, rho 0.6 after 200 steps", "buckingham", dict(rho=0.6), 200, dict(epsilon=1.0e5, sigma=2.0, alpha=10.0, dt=0.002)),
+    ("buckingham B 15, rho 1.0, jittered lattice", "buckingham", dict(rho=1.0), 0, dict(epsilon=1.0e7, sigma=3.454, alpha=15.0)),
+    ("buckingham B 12.5, cold crystal", "buckingham", dict(jitter=0.01, temperature=0.01), 0, dict(epsilon=9.02e5, sigma=3.454, alpha=12.5)),
+]
+
+
+@pytest.mark.parametrize("name,kind,gen,steps,over", F2_STATES, ids=[s[0] for s in F2_STATES])
+def test_fast32_of_the_other_potentials_away_from_its_calibration(B, orc, W, name, kind, gen, steps, over):
+    """As the test above for the Morse and Buckingham fast paths, whose estimate terms were scaled on
+    config 3's positions with the parameters of test_other_potentials_at_full_size: other stiffnesses,
+    densities and temperatures, at N = 32,000."""
+    w = W.lj_fcc(2, 20, seed=78, **gen)
+    over = {k: (float(np.float32(v)) if k in ("epsilon", "sigma") else v) for k, v in over.items()}
+    kinds = {"morse": W.KIND_MORSE, "buckingham": W.KIND_BUCKINGHAM}
+    w = dataclasses.replace(w, kind=kinds[kind], **over)
+    S = B.System(w)
+    S.build(); S.compute_force()
+    if steps:
+        S.step(steps)
+        torch.cuda.synchronize()
+        assert int(S.stats[2]) == -1
+    worst = state_force_parity(S, orc, w, alpha=over.get("alpha"))
+    cnt = torch.zeros(8, dtype=torch.int32, device=S.pos.device)
+    B.md_counters(S.sys, cnt, reset=True); S.compute_force(); B.md_counters(S.sys, cnt)
+    torch.cuda.synchronize()
+    print(f"fast32 [{name}]: worst error {worst:.3f} x 1e-5, re-evaluated {int(cnt[0])} of {w.n}")
+    assert int(cnt[0]) > 0                            # the fast path is the one that ran (the cutoff band alone flags some)
     S.close()
 
 
