@@ -201,6 +201,48 @@ int md_slab_pack(const md_slab_frame *frame, const void *pos, const int32_t *slo
 int md_slab_unpack(const md_slab_frame *frame, const void *rows, const int32_t *slots, int k, void *pos,
                    void *stream);
 
+/*
+ * The rebuild of a slab rank in five device phases (migration folded into the rebuild); every
+ * array is DEVICE memory, positions float4 with x GLOBAL in the owned / row arrays and LOCAL in pos, ids int32
+ * global particle numbers.  The caller reads the small count arrays back to size its messages; nothing else of
+ * the rebuild passes through the host.  The order of the compacted outputs is not specified (one atomic per
+ * warp); the cell list's canonical order makes the local system independent of it.
+ *
+ * md_slab_split:  the owned particles (id >= 0) among the n local slots, x made global, split by the slab
+ *   [lo, hi): stayers to own_pos / own_vel / own_id (room for n), the others to the rows of the previous or the
+ *   next rank, whichever is nearer round the periodic box: rows float[.][8] = position | velocity, ids int32.
+ *   counts int32[4] = {stayers, to previous, to next, rows dropped because cap_rows was too small}.
+ * md_slab_append: m received migrants (rows, ids) join the owned arrays at [offset, offset + m); *errors is
+ *   incremented for each one outside [lo, hi) (it crossed more than one slab between two rebuilds).
+ * md_slab_border: the owned particles with x < lo_edge (copies for the previous rank) and x >= hi_edge (for the
+ *   next): rows float4 (x global), ids; map_prev / map_next (int32[number of particles of the whole system],
+ *   all -1 between rebuilds) receive each one's position in its message.  counts int32[3] = {for previous, for
+ *   next, dropped}.
+ * md_slab_load:   the local system in pos / vel / id: the n_own owned particles, then the h_prev copies received
+ *   from the previous rank, then the h_next from the next (velocity 0, id = -1 - global id), x made local;
+ *   map_halo[global id] = position of the copy among the received rows (previous first).
+ * md_slab_plan:   after md_cell_list_build and md_neighbor_list_build of that system: nbr_count = 0 for the
+ *   copies (they take no force and no energy); border_prev / border_next / halo_slots = the slot each border
+ *   particle / copy has now, in message order: what md_slab_pack and md_slab_unpack move every step.  The three
+ *   maps are -1 again afterwards.
+ * Errors: MD_EINVAL (NULL, negative sizes, bad frame), MD_ECUDA.
+ */
+int md_slab_split(const md_slab_frame *frame, float lo, float hi, const void *pos, const void *vel,
+                  const int32_t *id, int n, void *own_pos, void *own_vel, int32_t *own_id, void *prev_rows,
+                  int32_t *prev_ids, void *next_rows, int32_t *next_ids, int cap_rows, int32_t *counts,
+                  void *stream);
+int md_slab_append(const void *rows, const int32_t *ids, int m, float lo, float hi, void *own_pos, void *own_vel,
+                   int32_t *own_id, int offset, int32_t *errors, void *stream);
+int md_slab_border(float lo_edge, float hi_edge, const void *own_pos, const int32_t *own_id, int n_own,
+                   void *prev_rows, int32_t *prev_ids, void *next_rows, int32_t *next_ids, int cap_rows,
+                   int32_t *map_prev, int32_t *map_next, int32_t *counts, void *stream);
+int md_slab_load(const md_slab_frame *frame, const void *own_pos, const void *own_vel, const int32_t *own_id,
+                 int n_own, const void *halo_prev_rows, const int32_t *halo_prev_ids, int h_prev,
+                 const void *halo_next_rows, const int32_t *halo_next_ids, int h_next, void *pos, void *vel,
+                 int32_t *id, int32_t *map_halo, void *stream);
+int md_slab_plan(const int32_t *id, int n, int32_t *nbr_count, int32_t *map_prev, int32_t *map_next,
+                 int32_t *map_halo, int32_t *border_prev, int32_t *border_next, int32_t *halo_slots, void *stream);
+
 /* BKS-type potential (L104 "Buckingham / BKS" [71-73], named only; reading A27): per species
  * pair the exp-6 term A_ab exp(-B_ab r) - C_ab / r^6, plus the Coulomb interaction of the species' point
  * charges in its damped shifted-force form (energy and force both vanish at r_cut):

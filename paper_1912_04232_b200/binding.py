@@ -26,6 +26,7 @@ SYMBOLS = [
     "md_flock_step", "md_flock_obstacles", "md_set_species_bks", "md_flock_predators",
     "md_set_range", "md_kick_drift", "md_half_kick", "md_force_half_kick",
     "md_slab_kick_drift", "md_slab_convert", "md_slab_pack", "md_slab_unpack",
+    "md_slab_split", "md_slab_append", "md_slab_border", "md_slab_load", "md_slab_plan",
 ]
 
 
@@ -104,6 +105,13 @@ def lib():
         L.md_slab_convert.argtypes = [C.POINTER(md_slab_frame), vp, C.c_int, C.c_int, vp]
         L.md_slab_pack.argtypes = [C.POINTER(md_slab_frame), vp, ip, C.c_int, vp, vp]
         L.md_slab_unpack.argtypes = [C.POINTER(md_slab_frame), vp, ip, C.c_int, vp, vp]
+        L.md_slab_split.argtypes = [C.POINTER(md_slab_frame), C.c_float, C.c_float, vp, vp, ip, C.c_int, vp, vp, ip,
+                                    vp, ip, vp, ip, C.c_int, ip, vp]
+        L.md_slab_append.argtypes = [vp, ip, C.c_int, C.c_float, C.c_float, vp, vp, ip, C.c_int, ip, vp]
+        L.md_slab_border.argtypes = [C.c_float, C.c_float, vp, ip, C.c_int, vp, ip, vp, ip, C.c_int, ip, ip, ip, vp]
+        L.md_slab_load.argtypes = [C.POINTER(md_slab_frame), vp, vp, ip, C.c_int, vp, ip, C.c_int, vp, ip, C.c_int,
+                                   vp, vp, ip, ip, vp]
+        L.md_slab_plan.argtypes = [ip, C.c_int, ip, ip, ip, ip, ip, ip, ip, vp]
         L.md_flock_predators.argtypes = [vp, C.c_int, vp, C.POINTER(md_predator_params)]
         L.md_flock_obstacles.argtypes = [vp, C.c_int, C.POINTER(C.c_float), C.POINTER(C.c_float), C.c_float]
         L.md_flock_step.argtypes = [vp, C.POINTER(md_flock_params), vp, ip, ip, ip, C.c_float, C.c_int, ip, vp]
@@ -291,6 +299,38 @@ def md_slab_pack(frame: md_slab_frame, pos, slots, rows_out, stream=None) -> Non
 
 def md_slab_unpack(frame: md_slab_frame, rows, slots, pos, stream=None) -> None:
     _check(lib().md_slab_unpack(C.byref(frame), _ptr(rows), _ptr(slots), int(slots.numel()), _ptr(pos), _stream(stream)))
+
+
+def md_slab_split(frame: md_slab_frame, lo, hi, pos, vel, id, n, own_pos, own_vel, own_id, prev_rows, prev_ids,
+                  next_rows, next_ids, cap_rows, counts, stream=None) -> None:
+    _check(lib().md_slab_split(C.byref(frame), float(lo), float(hi), _ptr(pos), _ptr(vel), _ptr(id), int(n),
+                               _ptr(own_pos), _ptr(own_vel), _ptr(own_id), _ptr(prev_rows), _ptr(prev_ids),
+                               _ptr(next_rows), _ptr(next_ids), int(cap_rows), _ptr(counts), _stream(stream)))
+
+
+def md_slab_append(rows, ids, m, lo, hi, own_pos, own_vel, own_id, offset, errors, stream=None) -> None:
+    _check(lib().md_slab_append(_ptr(rows), _ptr(ids), int(m), float(lo), float(hi), _ptr(own_pos), _ptr(own_vel),
+                                _ptr(own_id), int(offset), _ptr(errors), _stream(stream)))
+
+
+def md_slab_border(lo_edge, hi_edge, own_pos, own_id, n_own, prev_rows, prev_ids, next_rows, next_ids, cap_rows,
+                   map_prev, map_next, counts, stream=None) -> None:
+    _check(lib().md_slab_border(float(lo_edge), float(hi_edge), _ptr(own_pos), _ptr(own_id), int(n_own),
+                                _ptr(prev_rows), _ptr(prev_ids), _ptr(next_rows), _ptr(next_ids), int(cap_rows),
+                                _ptr(map_prev), _ptr(map_next), _ptr(counts), _stream(stream)))
+
+
+def md_slab_load(frame: md_slab_frame, own_pos, own_vel, own_id, n_own, hp_rows, hp_ids, h_prev, hn_rows, hn_ids,
+                 h_next, pos, vel, id, map_halo, stream=None) -> None:
+    _check(lib().md_slab_load(C.byref(frame), _ptr(own_pos), _ptr(own_vel), _ptr(own_id), int(n_own), _ptr(hp_rows),
+                              _ptr(hp_ids), int(h_prev), _ptr(hn_rows), _ptr(hn_ids), int(h_next), _ptr(pos),
+                              _ptr(vel), _ptr(id), _ptr(map_halo), _stream(stream)))
+
+
+def md_slab_plan(id, n, nbr_count, map_prev, map_next, map_halo, border_prev, border_next, halo_slots,
+                 stream=None) -> None:
+    _check(lib().md_slab_plan(_ptr(id), int(n), _ptr(nbr_count), _ptr(map_prev), _ptr(map_next), _ptr(map_halo),
+                              _ptr(border_prev), _ptr(border_next), _ptr(halo_slots), _stream(stream)))
 
 
 def md_half_kick(sys, vel, force, dt, mass, stream=None) -> None:

@@ -516,6 +516,117 @@ __global__ void k_slab_unpack(md_slab_frame f, const float4 *__restrict__ rows, 
     pos[slots[t]] = p;
 }
 
+// ---- slab decomposition: the rebuild (migration, border selection, assembly of the local system, exchange plan)
+// Position in a compacted output: one atomic per warp, lanes in order behind it.
+__device__ __forceinline__ int slab_take(bool mine, int *counter) {
+    const unsigned m = __ballot_sync(FULL, mine);
+    const int lane = threadIdx.x & 31;
+    int base = 0;
+    if (m && lane == __ffs(m) - 1) base = atomicAdd(counter, __popc(m));
+    base = __shfl_sync(FULL, base, m ? __ffs(m) - 1 : 0);
+    return base + __popc(m & ((1u << lane) - 1u));
+}
+// counts: {stayers, to previous, to next, errors}
+__global__ void k_slab_split(md_slab_frame f, float lo, float hi, const float4 *__restrict__ pos,
+                             const float4 *__restrict__ vel, const int *__restrict__ id, int n,
+                             float4 *own_pos, float4 *own_vel, int *own_id, float4 *prev_rows, int *prev_ids,
+                             float4 *next_rows, int *next_ids, int cap_rows, int *counts) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    const bool owned = i < n && id[i] >= 0;
+    float4 p = make_float4(0.f, 0.f, 0.f, 0.f);
+    int kind = -1;                                      // 0 stays, 1 to the previous rank, 2 to the next
+    if (owned) {
+        p = pos[i];
+        p.x = slab_to_global(f, p.x);
+        if (p.x >= lo && p.x < hi) kind = 0;
+        else {
+            // the nearer way round the periodic box
+            const float up = p.x >= hi ? p.x - hi : (p.x + f.L) - hi;
+            const float down = p.x < lo ? lo - p.x : (lo + f.L) - p.x;
+            kind = up < down ? 2 : 1;
+        }
+    }
+    const int a = slab_take(kind == 0, counts + 0);
+    const int b = slab_take(kind == 1, counts + 1);
+    const int c = slab_take(kind == 2, counts + 2);
+    if (kind == 0) { own_pos[a] = p; own_vel[a] = vel[i]; own_id[a] = id[i]; }
+    else if (kind > 0) {
+        const int t = kind == 1 ? b : c;
+        if (t >= cap_rows) { atomicAdd(counts + 3, 1); return; }
+        float4 *rows = kind == 1 ? prev_rows : next_rows;
+        rows[2 * t] = p; rows[2 * t + 1] = vel[i];
+        (kind == 1 ? prev_ids : next_ids)[t] = id[i];
+    }
+}
+// migrants join the owned set at [offset, offset + m); one outside [lo, hi) skipped a whole slab: an error
+__global__ void k_slab_append(const float4 *__restrict__ rows, const int *__restrict__ ids, int m, float lo, float hi,
+                              float4 *own_pos, float4 *own_vel, int *own_id, int offset, int *errors) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= m) return;
+    const float4 p = rows[2 * t];
+    if (!(p.x >= lo && p.x < hi)) atomicAdd(errors, 1);
+    own_pos[offset + t] = p; own_vel[offset + t] = rows[2 * t + 1]; own_id[offset + t] = ids[t];
+}
+// owned particles within the halo width of a face: what the neighbours copy.  counts: {for previous, for next, errors}
+__global__ void k_slab_border(float lo_edge, float hi_edge, const float4 *__restrict__ own_pos,
+                              const int *__restrict__ own_id, int n_own, float4 *prev_rows, int *prev_ids,
+                              float4 *next_rows, int *next_ids, int cap_rows, int *map_prev, int *map_next,
+                              int *counts) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    float4 p = make_float4(0.f, 0.f, 0.f, 0.f);
+    bool lo_side = false, hi_side = false;
+    int gid = 0;
+    if (i < n_own) {
+        p = own_pos[i]; gid = own_id[i];
+        lo_side = p.x < lo_edge; hi_side = p.x >= hi_edge;
+    }
+    const int a = slab_take(lo_side, counts + 0);
+    const int b = slab_take(hi_side, counts + 1);
+    if (lo_side) {
+        if (a < cap_rows) { prev_rows[a] = p; prev_ids[a] = gid; map_prev[gid] = a; } else atomicAdd(counts + 2, 1);
+    }
+    if (hi_side) {
+        if (b < cap_rows) { next_rows[b] = p; next_ids[b] = gid; map_next[gid] = b; } else atomicAdd(counts + 2, 1);
+    }
+}
+// local system = owned, then the copies from the previous rank, then those from the next; x local
+__global__ void k_slab_load(md_slab_frame f, const float4 *__restrict__ own_pos, const float4 *__restrict__ own_vel,
+                            const int *__restrict__ own_id, int n_own, const float4 *__restrict__ hp_rows,
+                            const int *__restrict__ hp_ids, int h_prev, const float4 *__restrict__ hn_rows,
+                            const int *__restrict__ hn_ids, int h_next, float4 *pos, float4 *vel, int *id,
+                            int *map_halo) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n_own + h_prev + h_next) return;
+    float4 p, v = make_float4(0.f, 0.f, 0.f, 0.f);
+    int g;
+    if (i < n_own) { p = own_pos[i]; v = own_vel[i]; g = own_id[i]; }
+    else {
+        const int q = i - n_own;
+        if (q < h_prev) { p = hp_rows[q]; g = hp_ids[q]; } else { p = hn_rows[q - h_prev]; g = hn_ids[q - h_prev]; }
+        map_halo[g] = q;
+        g = -1 - g;
+    }
+    p.x = slab_to_local(f, p.x);
+    pos[i] = p; vel[i] = v; id[i] = g;
+}
+// after the lists are built: copies take no force (count 0); where every border particle and every copy sits now,
+// in the order of the messages; the maps go back to -1
+__global__ void k_slab_plan(const int *__restrict__ id, int n, int *nbr_count, int *map_prev, int *map_next,
+                            int *map_halo, int *border_prev, int *border_next, int *halo_slots) {
+    const int s = blockIdx.x * blockDim.x + threadIdx.x;
+    if (s >= n) return;
+    const int g = id[s];
+    if (g < 0) {
+        nbr_count[s] = 0;
+        const int q = map_halo[-1 - g];
+        if (q >= 0) { halo_slots[q] = s; map_halo[-1 - g] = -1; }
+    } else {
+        const int a = map_prev[g], b = map_next[g];
+        if (a >= 0) { border_prev[a] = s; map_prev[g] = -1; }
+        if (b >= 0) { border_next[b] = s; map_next[g] = -1; }
+    }
+}
+
 __global__ void k_iota(int n, int *id) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i < n) id[i] = i;
@@ -1349,6 +1460,84 @@ int md_slab_unpack(const md_slab_frame *frame, const void *rows, const int32_t *
     if (k < 0 || (k > 0 && (!pos || !slots || !rows))) return fail(MD_EINVAL, "NULL argument");
     if (k == 0) return MD_OK;
     k_slab_unpack<<<blocks_for(k), 256, 0, (cudaStream_t)stream>>>(*frame, (const float4 *)rows, slots, k, (float4 *)pos);
+    LAUNCH_OK();
+    return MD_OK;
+}
+
+int md_slab_split(const md_slab_frame *frame, float lo, float hi, const void *pos, const void *vel,
+                  const int32_t *id, int n, void *own_pos, void *own_vel, int32_t *own_id, void *prev_rows,
+                  int32_t *prev_ids, void *next_rows, int32_t *next_ids, int cap_rows, int32_t *counts,
+                  void *stream) {
+    if (int rc = check_frame(frame)) return rc;
+    if (n < 0 || cap_rows < 0 || !counts) return fail(MD_EINVAL, "n, cap_rows >= 0 and counts != NULL");
+    if (n > 0 && (!pos || !vel || !id || !own_pos || !own_vel || !own_id)) return fail(MD_EINVAL, "NULL argument");
+    if (cap_rows > 0 && (!prev_rows || !prev_ids || !next_rows || !next_ids)) return fail(MD_EINVAL, "NULL argument");
+    if (!(lo < hi)) return fail(MD_EINVAL, "slab [%g, %g) is empty", lo, hi);
+    cudaStream_t st = (cudaStream_t)stream;
+    CU(cudaMemsetAsync(counts, 0, 4 * sizeof(int), st));
+    if (n == 0) return MD_OK;
+    k_slab_split<<<blocks_for(n), 256, 0, st>>>(*frame, lo, hi, (const float4 *)pos, (const float4 *)vel, id, n,
+                                                (float4 *)own_pos, (float4 *)own_vel, own_id, (float4 *)prev_rows,
+                                                prev_ids, (float4 *)next_rows, next_ids, cap_rows, counts);
+    LAUNCH_OK();
+    return MD_OK;
+}
+
+int md_slab_append(const void *rows, const int32_t *ids, int m, float lo, float hi, void *own_pos, void *own_vel,
+                   int32_t *own_id, int offset, int32_t *errors, void *stream) {
+    if (m < 0 || offset < 0 || !errors) return fail(MD_EINVAL, "m, offset >= 0 and errors != NULL");
+    if (m == 0) return MD_OK;
+    if (!rows || !ids || !own_pos || !own_vel || !own_id) return fail(MD_EINVAL, "NULL argument");
+    k_slab_append<<<blocks_for(m), 256, 0, (cudaStream_t)stream>>>((const float4 *)rows, ids, m, lo, hi, (float4 *)own_pos,
+                                                                   (float4 *)own_vel, own_id, offset, errors);
+    LAUNCH_OK();
+    return MD_OK;
+}
+
+int md_slab_border(float lo_edge, float hi_edge, const void *own_pos, const int32_t *own_id, int n_own,
+                   void *prev_rows, int32_t *prev_ids, void *next_rows, int32_t *next_ids, int cap_rows,
+                   int32_t *map_prev, int32_t *map_next, int32_t *counts, void *stream) {
+    if (n_own < 0 || cap_rows < 0 || !counts) return fail(MD_EINVAL, "n_own, cap_rows >= 0 and counts != NULL");
+    cudaStream_t st = (cudaStream_t)stream;
+    CU(cudaMemsetAsync(counts, 0, 3 * sizeof(int), st));
+    if (n_own == 0) return MD_OK;
+    if (!own_pos || !own_id || !prev_rows || !prev_ids || !next_rows || !next_ids || !map_prev || !map_next)
+        return fail(MD_EINVAL, "NULL argument");
+    k_slab_border<<<blocks_for(n_own), 256, 0, st>>>(lo_edge, hi_edge, (const float4 *)own_pos, own_id, n_own,
+                                                     (float4 *)prev_rows, prev_ids, (float4 *)next_rows, next_ids,
+                                                     cap_rows, map_prev, map_next, counts);
+    LAUNCH_OK();
+    return MD_OK;
+}
+
+int md_slab_load(const md_slab_frame *frame, const void *own_pos, const void *own_vel, const int32_t *own_id,
+                 int n_own, const void *halo_prev_rows, const int32_t *halo_prev_ids, int h_prev,
+                 const void *halo_next_rows, const int32_t *halo_next_ids, int h_next, void *pos, void *vel,
+                 int32_t *id, int32_t *map_halo, void *stream) {
+    if (int rc = check_frame(frame)) return rc;
+    if (n_own < 0 || h_prev < 0 || h_next < 0) return fail(MD_EINVAL, "negative count");
+    const int n = n_own + h_prev + h_next;
+    if (n == 0) return MD_OK;
+    if (!pos || !vel || !id || !map_halo || (n_own > 0 && (!own_pos || !own_vel || !own_id)) ||
+        (h_prev > 0 && (!halo_prev_rows || !halo_prev_ids)) || (h_next > 0 && (!halo_next_rows || !halo_next_ids)))
+        return fail(MD_EINVAL, "NULL argument");
+    k_slab_load<<<blocks_for(n), 256, 0, (cudaStream_t)stream>>>(*frame, (const float4 *)own_pos, (const float4 *)own_vel,
+                                                                 own_id, n_own, (const float4 *)halo_prev_rows,
+                                                                 halo_prev_ids, h_prev, (const float4 *)halo_next_rows,
+                                                                 halo_next_ids, h_next, (float4 *)pos, (float4 *)vel,
+                                                                 id, map_halo);
+    LAUNCH_OK();
+    return MD_OK;
+}
+
+int md_slab_plan(const int32_t *id, int n, int32_t *nbr_count, int32_t *map_prev, int32_t *map_next,
+                 int32_t *map_halo, int32_t *border_prev, int32_t *border_next, int32_t *halo_slots, void *stream) {
+    if (n < 0) return fail(MD_EINVAL, "n >= 0");
+    if (n == 0) return MD_OK;
+    if (!id || !nbr_count || !map_prev || !map_next || !map_halo || !border_prev || !border_next || !halo_slots)
+        return fail(MD_EINVAL, "NULL argument");
+    k_slab_plan<<<blocks_for(n), 256, 0, (cudaStream_t)stream>>>(id, n, nbr_count, map_prev, map_next, map_halo,
+                                                                 border_prev, border_next, halo_slots);
     LAUNCH_OK();
     return MD_OK;
 }

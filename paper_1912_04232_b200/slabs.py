@@ -195,34 +195,27 @@ class LocalSystem:
         self.status = torch.zeros(2, dtype=torch.int32, device=dev)
         self.flag = torch.zeros(1, dtype=torch.int32, device=dev)
         self.energy = torch.zeros(1, dtype=torch.float64, device=dev)
-        self.nbr_idx = None
+        self.nbr_idx = torch.empty(((cap + 31) // 32) * 32 * self.cfg.capacity, dtype=torch.int32, device=dev)
         self.cell_start = None
 
-    def load(self, pos, vel, ids):
-        """New local particle set (owned first or not: the cell list re-sorts anyway)."""
-        B, n = self.B, pos.shape[0]
+    def resize(self, n: int):
+        """A system of n particles over the same buffers (pos / vel / id are filled by the caller)."""
+        B = self.B
         if n > self.cap:
             raise RuntimeError(f"rank {self.fr.rank}: {n} local particles exceed the reserved {self.cap}")
         if self.sys is not None:
-            torch.cuda.synchronize(self.device)
-            B.md_destroy(self.sys)
+            B.md_destroy(self.sys)          # its kernels have finished: the caller has just read this rebuild's counts
         self.n = n
-        self.pos[:n] = pos; self.vel[:n] = vel; self.id[:n] = ids
         self.sys = B.md_create(self.cfg, n, self.workspace)
         ncell = B.md_num_cells(self.sys)
         cells = ncell[0] * ncell[1] * ncell[2]
         if self.cell_start is None or self.cell_start.numel() != cells + 1:
             self.cell_start = torch.zeros(cells + 1, dtype=torch.int32, device=self.device)
-        length = B.md_nbr_layout(self.sys)[4]
-        if self.nbr_idx is None or self.nbr_idx.numel() < length:
-            self.nbr_idx = torch.empty(((self.cap + 31) // 32) * 32 * self.cfg.capacity, dtype=torch.int32, device=self.device)
 
     def build(self):
         B = self.B
         B.md_cell_list_build(self.sys, self.pos, self.vel, self.id, self.cell_start, self.perm)
         B.md_neighbor_list_build(self.sys, self.pos, self.cell_start, self.perm, self.nbr_idx, self.nbr_count, self.status)
-        n = self.n
-        self.nbr_count[:n].masked_fill_(self.id[:n] < 0, 0)      # halo copies: no force, no energy
 
     def close(self):
         if self.sys is not None:
@@ -232,92 +225,109 @@ class LocalSystem:
 
 
 class SlabRank:
-    """One rank of the decomposition: its frame, its local system, and the phases of a step.  What leaves
-    a phase for another rank is a pair (float32 rows, int32 ids); what arrives comes from the PREVIOUS and
-    the NEXT rank only (periodically: rank 0's previous rank is the last one)."""
+    """One rank of the decomposition: its frame, its local system, and the phases of a step and of a rebuild.
+    Every phase is a call into the library (md_slab_*): the host sizes messages from small count arrays and
+    moves no particle data.  What leaves a phase for another rank is a pair (float32 rows, int32 ids); what
+    arrives comes from the PREVIOUS and the NEXT rank only (periodically: rank 0's previous rank is the last)."""
 
     def __init__(self, B, w, fr: Frame, device, reserve: float = 1.35):
         self.B, self.w, self.fr = B, w, fr
         share = (fr.hi - fr.lo + 2 * fr.H) / fr.L
-        self.S = LocalSystem(B, w, fr, int(reserve * w.n * share) + 2048, device)
+        cap = int(reserve * w.n * share) + 2048
+        self.S = LocalSystem(B, w, fr, cap, device)
         self.frames = frames(fr.L, float(np.float32(w.r_cut) + np.float32(w.skin)), fr.world)
         self.prev, self.next = (fr.rank - 1) % fr.world, (fr.rank + 1) % fr.world
         self.frame = fr.abi(B)      # the coordinate arithmetic of every phase runs in the library (md_slab_*)
         self.rebuilds = 0
-        self._own = None            # (pos_g [k,4], vel [k,4], id [k]) between the phases of a rebuild
-        self._border_ids = (None, None)
+        dev = self.S.device
+        f32 = dict(dtype=torch.float32, device=dev)
+        i32 = dict(dtype=torch.int32, device=dev)
+        # owned particles between the phases of a rebuild (x global)
+        self.own_pos, self.own_vel = torch.zeros(cap, 4, **f32), torch.zeros(cap, 4, **f32)
+        self.own_id = torch.zeros(cap, **i32)
+        self.n_own = 0
+        # messages: migrants (position | velocity) and border rows (position), for (prev, next)
+        self.cap_rows = int(reserve * w.n * fr.H / fr.L) + 2048
+        self.mig_rows = tuple(torch.zeros(self.cap_rows, 8, **f32) for _ in range(2))
+        self.mig_ids = tuple(torch.zeros(self.cap_rows, **i32) for _ in range(2))
+        self.bor_rows = tuple(torch.zeros(self.cap_rows, 4, **f32) for _ in range(2))
+        self.bor_ids = tuple(torch.zeros(self.cap_rows, **i32) for _ in range(2))
+        self.step_rows_buf = tuple(torch.zeros(self.cap_rows, 4, **f32) for _ in range(2))
+        self.counts = torch.zeros(8, **i32)      # [0:4] split, [4:7] border, [7] errors of append
+        # global id -> position in a message, -1 between rebuilds
+        self.map_prev, self.map_next, self.map_halo = (torch.full((w.n,), -1, **i32) for _ in range(3))
+        self.border_slots = tuple(torch.zeros(self.cap_rows, **i32) for _ in range(2))
+        self.halo_slots = torch.zeros(2 * self.cap_rows, **i32)
         self.border = (None, None)  # local slots of my border particles for (prev, next)
         self.halo = (None, None)    # local slots of the copies that came from (prev, next), in arrival order
+
+    def _read_counts(self):
+        c = self.counts.tolist()                                # the host read of this phase
+        if c[3] or c[6]:
+            raise RuntimeError(f"rank {self.fr.rank}: message buffers of {self.cap_rows} rows are too small")
+        if c[7]:
+            raise RuntimeError("a particle moved past a neighbouring slab between two rebuilds")
+        return c
 
     # ---- start and rebuild ------------------------------------------------------------------
     def take_initial(self, pos_g, vel, gid):
         """From the (replicated) initial state: my owned particles."""
         mine = owner_of(pos_g[:, 0].contiguous(), self.frames) == self.fr.rank
-        self._own = (pos_g[mine].clone(), vel[mine].clone(), gid[mine].clone())
+        k = int(mine.sum())
+        self.own_pos[:k] = pos_g[mine]; self.own_vel[:k] = vel[mine]; self.own_id[:k] = gid[mine]
+        self.n_own = k
 
     def leavers(self):
         """Owned particles whose x has left the slab since the last rebuild: ((rows, ids) for prev, for next);
         the stayers are kept for adopt()."""
-        S, fr = self.S, self.fr
-        n = S.n
-        owned = S.id[:n] >= 0
-        pos = S.pos[:n][owned].contiguous()
-        self.B.md_slab_convert(self.frame, pos, pos.shape[0], 0)           # x: local -> global
-        vel, gid = S.vel[:n][owned], S.id[:n][owned]
-        own = owner_of(pos[:, 0].contiguous(), self.frames)
-        stay, to_prev, to_next = own == fr.rank, own == self.prev, own == self.next
-        if fr.world == 2:                       # the other rank is both neighbours: below my slab or above it
-            lo = np.float32(fr.lo)
-            below = (pos[:, 0] < lo) if not fr.first else (pos[:, 0] >= np.float32(0.5 * (fr.hi + fr.L)))
-            to_prev, to_next = (own != fr.rank) & below, (own != fr.rank) & ~below
-        if int((stay | to_prev | to_next).sum()) != pos.shape[0]:
-            raise RuntimeError("a particle moved past a neighbouring slab between two rebuilds")
-        self._own = (pos[stay], vel[stay], gid[stay])
-        pack = lambda m: (torch.cat([pos[m], vel[m]], 1), gid[m])
-        return pack(to_prev), pack(to_next)
+        S, fr, B = self.S, self.fr, self.B
+        B.md_slab_split(self.frame, np.float32(fr.lo), np.float32(fr.hi), S.pos, S.vel, S.id, S.n,
+                        self.own_pos, self.own_vel, self.own_id, self.mig_rows[0], self.mig_ids[0],
+                        self.mig_rows[1], self.mig_ids[1], self.cap_rows, self.counts)
+        c = self._read_counts()
+        self.n_own = c[0]
+        return (self.mig_rows[0][: c[1]], self.mig_ids[0][: c[1]]), (self.mig_rows[1][: c[2]], self.mig_ids[1][: c[2]])
 
     def adopt(self, from_prev, from_next):
         """Migrants from the neighbours join my owned particles."""
-        pos, vel, gid = self._own
+        fr = self.fr
         for rows, ids in (from_prev, from_next):
-            if rows is not None and rows.shape[0]:
-                pos = torch.cat([pos, rows[:, :4]]); vel = torch.cat([vel, rows[:, 4:]]); gid = torch.cat([gid, ids])
-        self._own = (pos, vel, gid)
+            m = 0 if rows is None else int(rows.shape[0])
+            if m:
+                if self.n_own + m > self.S.cap:
+                    raise RuntimeError(f"rank {fr.rank}: more than the reserved {self.S.cap} particles")
+                self.B.md_slab_append(rows, ids, m, np.float32(fr.lo), np.float32(fr.hi), self.own_pos, self.own_vel,
+                                      self.own_id, self.n_own, self.counts[7:])
+                self.n_own += m
 
     def border_rows(self):
         """My owned particles within H of my slab's faces: ((positions, ids) for prev, for next).  They
         become the neighbours' halo copies; their ids, in this order, define what travels every step."""
-        pos, vel, gid = self._own
-        fr = self.fr
-        x = pos[:, 0]
-        f32 = np.float32
-        lo_side = x < f32(fr.lo + fr.H)                     # near my lower face: the previous rank's high halo
-        hi_side = x >= f32(fr.hi - fr.H)                    # near my upper face: the next rank's low halo
-        self._border_ids = (gid[lo_side].clone(), gid[hi_side].clone())
-        return (pos[lo_side], gid[lo_side]), (pos[hi_side], gid[hi_side])
+        fr, f32 = self.fr, np.float32
+        self.B.md_slab_border(f32(fr.lo + fr.H), f32(fr.hi - fr.H), self.own_pos, self.own_id, self.n_own,
+                              self.bor_rows[0], self.bor_ids[0], self.bor_rows[1], self.bor_ids[1], self.cap_rows,
+                              self.map_prev, self.map_next, self.counts[4:])
+        c = self._read_counts()
+        self.n_border = (c[4], c[5])
+        return (self.bor_rows[0][: c[4]], self.bor_ids[0][: c[4]]), (self.bor_rows[1][: c[5]], self.bor_ids[1][: c[5]])
 
     def rebuild(self, halo_prev, halo_next):
         """Local system = owned + the copies the neighbours sent; lists; index lists of the step exchange."""
-        pos, vel, gid = self._own
-        fr, S = self.fr, self.S
-        hp = torch.cat([halo_prev[0], halo_next[0]])
-        hid = torch.cat([halo_prev[1], halo_next[1]])
-        allpos = torch.cat([pos, hp]).contiguous()
-        self.B.md_slab_convert(self.frame, allpos, allpos.shape[0], 1)     # x: global -> local
-        S.load(allpos, torch.cat([vel, torch.zeros_like(hp)]), torch.cat([gid, -1 - hid]))
+        S, B = self.S, self.B
+        hp, hn = int(halo_prev[0].shape[0]), int(halo_next[0].shape[0])
+        if hp + hn > self.halo_slots.numel():
+            raise RuntimeError(f"rank {self.fr.rank}: more halo copies than the reserved {self.halo_slots.numel()}")
+        n = self.n_own + hp + hn
+        S.resize(n)
+        B.md_slab_load(self.frame, self.own_pos, self.own_vel, self.own_id, self.n_own, halo_prev[0].contiguous(),
+                       halo_prev[1].contiguous(), hp, halo_next[0].contiguous(), halo_next[1].contiguous(), hn,
+                       S.pos, S.vel, S.id, self.map_halo)
         S.build()
-        self._own = None
-        # where everything ended up after the re-sort, through the ids
-        ids = S.id[: S.n].long()
-        n_all = self.w.n
-        slot_owned = torch.full((n_all,), -1, dtype=torch.long, device=ids.device)
-        slot_halo = torch.full((n_all,), -1, dtype=torch.long, device=ids.device)
-        where = torch.arange(S.n, device=ids.device)
-        slot_owned[ids[ids >= 0]] = where[ids >= 0]
-        slot_halo[-1 - ids[ids < 0]] = where[ids < 0]
-        self.border = tuple(slot_owned[b.long()].int().contiguous() for b in self._border_ids)
-        self.halo = (slot_halo[halo_prev[1].long()].int().contiguous(), slot_halo[halo_next[1].long()].int().contiguous())
-        self.rows_out = tuple(torch.empty(b.numel(), 4, dtype=torch.float32, device=ids.device) for b in self.border)
+        B.md_slab_plan(S.id, n, S.nbr_count, self.map_prev, self.map_next, self.map_halo, self.border_slots[0],
+                       self.border_slots[1], self.halo_slots)
+        self.border = tuple(self.border_slots[k][: self.n_border[k]] for k in range(2))
+        self.halo = (self.halo_slots[:hp], self.halo_slots[hp: hp + hn])
+        self.rows_out = tuple(self.step_rows_buf[k][: self.n_border[k]] for k in range(2))
         self.rebuilds += 1
 
     # ---- the phases of an ordinary step ------------------------------------------------------
