@@ -185,11 +185,23 @@ typedef struct md_slab_frame {
     float l2g_thr;    /* local x at which the image zone starts (kind 0) / ends (kind 2) */
 } md_slab_frame;
 
-/* md_kick_drift on the whole local system, then every x put back on the GLOBAL fp32 grid
- * (x = to_local(to_global(x))): the rounding the global coordinate would get, so that a decomposed run
- * differs from md_nve_step only in the order forces are summed. */
+/* The opening of a step (v += dt/2m F, r = mu(r, dt v)) on the whole local system with every x put back on the
+ * GLOBAL fp32 grid (x = to_local(to_global(x))): the rounding the global coordinate would get, so that a
+ * decomposed run differs from md_nve_step only in the order forces are summed.  *flag is RAISED (never
+ * cleared: several ranks of one process may share the word) when a particle is more than skin / 2 from where
+ * the lists were built.  Halo copies (id[i] < 0) are left alone: their positions arrive from their owners.
+ * stop (may be NULL): while *stop != 0 the call changes nothing.
+ *
+ * md_slab_force_half_kick: md_force_half_kick that changes nothing while *flag != 0 and then raises *stop;
+ * *done (may be NULL) counts the calls that did run.  With these two the host can enqueue several steps
+ * (drift, exchange, force) without waiting: from the first step whose drift meets a stale list on ANY rank
+ * (the ranks share *flag, or all-reduce it between the two calls) every later call is a no-op, and the host
+ * reads *done once per batch, rebuilds, and finishes the interrupted step with md_force_half_kick. */
 int md_slab_kick_drift(md_system *sys, const md_slab_frame *frame, void *pos, void *vel, const void *force,
-                       float dt, float mass, int32_t *flag, void *stream);
+                       const int32_t *id, float dt, float mass, int32_t *flag, const int32_t *stop, void *stream);
+int md_slab_force_half_kick(md_system *sys, const md_potential *pot, const void *pos, const int32_t *nbr_idx,
+                            const int32_t *nbr_count, void *force, void *vel, float dt, float mass,
+                            const int32_t *flag, int32_t *stop, int32_t *done, void *stream);
 
 /* In place on the x component of n float4 positions: to_local != 0: global -> local, else local -> global. */
 int md_slab_convert(const md_slab_frame *frame, void *pos, int n, int to_local, void *stream);
@@ -200,6 +212,20 @@ int md_slab_pack(const md_slab_frame *frame, const void *pos, const int32_t *slo
                  void *stream);
 int md_slab_unpack(const md_slab_frame *frame, const void *rows, const int32_t *slots, int k, void *pos,
                    void *stream);
+
+/* One step of a slab rank in two calls with the exchange between them.
+ * md_slab_step_open  = md_slab_kick_drift, then both messages packed as md_slab_pack does (one launch).
+ * md_slab_step_close = both received messages unpacked as md_slab_unpack does (one launch), then
+ *                      md_slab_force_half_kick. */
+int md_slab_step_open(md_system *sys, const md_slab_frame *frame, void *pos, void *vel, const void *force,
+                      const int32_t *id, float dt, float mass, int32_t *flag, const int32_t *stop,
+                      const int32_t *border_prev, int k_prev, void *rows_prev, const int32_t *border_next,
+                      int k_next, void *rows_next, void *stream);
+int md_slab_step_close(md_system *sys, const md_slab_frame *frame, const md_potential *pot, const void *rows_prev,
+                       const int32_t *halo_prev, int h_prev, const void *rows_next, const int32_t *halo_next,
+                       int h_next, void *pos, const int32_t *nbr_idx, const int32_t *nbr_count, void *force,
+                       void *vel, float dt, float mass, const int32_t *flag, int32_t *stop, int32_t *done,
+                       void *stream);
 
 /*
  * The rebuild of a slab rank in five device phases (migration folded into the rebuild); every

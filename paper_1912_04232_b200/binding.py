@@ -26,7 +26,7 @@ SYMBOLS = [
     "md_flock_step", "md_flock_obstacles", "md_set_species_bks", "md_flock_predators",
     "md_set_range", "md_kick_drift", "md_half_kick", "md_force_half_kick",
     "md_slab_kick_drift", "md_slab_convert", "md_slab_pack", "md_slab_unpack",
-    "md_slab_split", "md_slab_append", "md_slab_border", "md_slab_load", "md_slab_plan",
+    "md_slab_force_half_kick", "md_slab_step_open", "md_slab_step_close", "md_slab_split", "md_slab_append", "md_slab_border", "md_slab_load", "md_slab_plan",
 ]
 
 
@@ -101,10 +101,16 @@ def lib():
         L.md_kick_drift.argtypes = [vp, vp, vp, vp, C.c_float, C.c_float, ip, vp]
         L.md_force_half_kick.argtypes = [vp, C.POINTER(md_potential), vp, ip, ip, vp, vp, C.c_float, C.c_float, vp]
         L.md_half_kick.argtypes = [vp, vp, vp, C.c_float, C.c_float, vp]
-        L.md_slab_kick_drift.argtypes = [vp, C.POINTER(md_slab_frame), vp, vp, vp, C.c_float, C.c_float, ip, vp]
+        L.md_slab_kick_drift.argtypes = [vp, C.POINTER(md_slab_frame), vp, vp, vp, ip, C.c_float, C.c_float, ip, ip, vp]
+        L.md_slab_force_half_kick.argtypes = [vp, C.POINTER(md_potential), vp, ip, ip, vp, vp, C.c_float, C.c_float,
+                                              ip, ip, ip, vp]
         L.md_slab_convert.argtypes = [C.POINTER(md_slab_frame), vp, C.c_int, C.c_int, vp]
         L.md_slab_pack.argtypes = [C.POINTER(md_slab_frame), vp, ip, C.c_int, vp, vp]
         L.md_slab_unpack.argtypes = [C.POINTER(md_slab_frame), vp, ip, C.c_int, vp, vp]
+        L.md_slab_step_open.argtypes = [vp, C.POINTER(md_slab_frame), vp, vp, vp, ip, C.c_float, C.c_float, ip, ip,
+                                        ip, C.c_int, vp, ip, C.c_int, vp, vp]
+        L.md_slab_step_close.argtypes = [vp, C.POINTER(md_slab_frame), C.POINTER(md_potential), vp, ip, C.c_int, vp, ip,
+                                         C.c_int, vp, ip, ip, vp, vp, C.c_float, C.c_float, ip, ip, ip, vp]
         L.md_slab_split.argtypes = [C.POINTER(md_slab_frame), C.c_float, C.c_float, vp, vp, ip, C.c_int, vp, vp, ip,
                                     vp, ip, vp, ip, C.c_int, ip, vp]
         L.md_slab_append.argtypes = [vp, ip, C.c_int, C.c_float, C.c_float, vp, vp, ip, C.c_int, ip, vp]
@@ -284,9 +290,16 @@ def md_force_half_kick(sys, pot: md_potential, pos, nbr_idx, nbr_count, force, v
                                     _ptr(vel), float(dt), float(mass), _stream(stream)))
 
 
-def md_slab_kick_drift(sys, frame: md_slab_frame, pos, vel, force, dt, mass, flag, stream=None) -> None:
-    _check(lib().md_slab_kick_drift(sys, C.byref(frame), _ptr(pos), _ptr(vel), _ptr(force), float(dt), float(mass),
-                                    _ptr(flag), _stream(stream)))
+def md_slab_kick_drift(sys, frame: md_slab_frame, pos, vel, force, id, dt, mass, flag, stop=None, stream=None) -> None:
+    _check(lib().md_slab_kick_drift(sys, C.byref(frame), _ptr(pos), _ptr(vel), _ptr(force), _ptr(id), float(dt), float(mass),
+                                    _ptr(flag), _ptr(stop), _stream(stream)))
+
+
+def md_slab_force_half_kick(sys, pot, pos, nbr_idx, nbr_count, force, vel, dt, mass, flag, stop, done,
+                            stream=None) -> None:
+    _check(lib().md_slab_force_half_kick(sys, C.byref(pot), _ptr(pos), _ptr(nbr_idx), _ptr(nbr_count), _ptr(force),
+                                         _ptr(vel), float(dt), float(mass), _ptr(flag), _ptr(stop), _ptr(done),
+                                         _stream(stream)))
 
 
 def md_slab_convert(frame: md_slab_frame, pos, n, to_local, stream=None) -> None:
@@ -299,6 +312,22 @@ def md_slab_pack(frame: md_slab_frame, pos, slots, rows_out, stream=None) -> Non
 
 def md_slab_unpack(frame: md_slab_frame, rows, slots, pos, stream=None) -> None:
     _check(lib().md_slab_unpack(C.byref(frame), _ptr(rows), _ptr(slots), int(slots.numel()), _ptr(pos), _stream(stream)))
+
+
+def md_slab_step_open(sys, frame: md_slab_frame, pos, vel, force, id, dt, mass, flag, stop, border_prev, rows_prev,
+                      border_next, rows_next, stream=None) -> None:
+    _check(lib().md_slab_step_open(sys, C.byref(frame), _ptr(pos), _ptr(vel), _ptr(force), _ptr(id), float(dt),
+                                   float(mass), _ptr(flag), _ptr(stop), _ptr(border_prev), int(border_prev.numel()),
+                                   _ptr(rows_prev), _ptr(border_next), int(border_next.numel()), _ptr(rows_next),
+                                   _stream(stream)))
+
+
+def md_slab_step_close(sys, frame: md_slab_frame, pot, rows_prev, halo_prev, rows_next, halo_next, pos, nbr_idx,
+                       nbr_count, force, vel, dt, mass, flag, stop, done, stream=None) -> None:
+    _check(lib().md_slab_step_close(sys, C.byref(frame), C.byref(pot), _ptr(rows_prev), _ptr(halo_prev),
+                                    int(halo_prev.numel()), _ptr(rows_next), _ptr(halo_next), int(halo_next.numel()),
+                                    _ptr(pos), _ptr(nbr_idx), _ptr(nbr_count), _ptr(force), _ptr(vel), float(dt),
+                                    float(mass), _ptr(flag), _ptr(stop), _ptr(done), _stream(stream)))
 
 
 def md_slab_split(frame: md_slab_frame, lo, hi, pos, vel, id, n, own_pos, own_vel, own_id, prev_rows, prev_ids,

@@ -499,6 +499,37 @@ __global__ void k_slab_convert(md_slab_frame f, float4 *pos, int n, int mode) {
     else x = slab_to_local(f, slab_to_global(f, x));      // back on the global fp32 grid
     pos[i].x = x;
 }
+// The opening of a slab rank's step in one kernel: k_kick_drift, then x put back on the global fp32 grid, then
+// the half-skin test on that x (differences of local coordinates are differences of global ones).  Does
+// nothing while *stop != 0: the host enqueues steps ahead and a stale list has been met (Book::skip).  Halo
+// copies (id < 0) are left alone: their positions arrive from their owners, whose own test covers them (a copy
+// whose owner has stepped just outside the halo zone has a local x below 0 that must not be wrapped or tested).
+template <int DIM>
+__global__ void __launch_bounds__(256)
+k_slab_kick_drift(Geom g, md_slab_frame f, float4 *__restrict__ pos, float4 *__restrict__ vel,
+                  const float4 *__restrict__ force, const float4 *__restrict__ ref, const int *__restrict__ id,
+                  float a, float dt, int *flag, const int *stop) {
+    if (stop && ld_volatile(stop)) return;
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    bool moved = false;
+    if (i < g.n && id[i] >= 0) {
+        float4 p = pos[i], v = vel[i];
+        const float4 fo = force[i];
+        v.x = fmaf(a, fo.x, v.x);
+        v.y = fmaf(a, fo.y, v.y);
+        p.x = wrap(fmaf(dt, v.x, p.x), g.L[0], g.inv_L[0]);
+        p.y = wrap(fmaf(dt, v.y, p.y), g.L[1], g.inv_L[1]);
+        if (DIM == 3) {
+            v.z = fmaf(a, fo.z, v.z);
+            p.z = wrap(fmaf(dt, v.z, p.z), g.L[2], g.inv_L[2]);
+        }
+        p.x = slab_to_local(f, slab_to_global(f, p.x));
+        pos[i] = p; vel[i] = v;
+        moved = disp2_from_ref<DIM>(g, p, ref[i]) > g.half_skin2;
+    }
+    if (__any_sync(FULL, moved) && (threadIdx.x & 31) == 0) *flag = 1;
+}
+
 __global__ void k_slab_pack(md_slab_frame f, const float4 *__restrict__ pos, const int *__restrict__ slots, int k,
                             float4 *__restrict__ rows) {
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
@@ -625,6 +656,30 @@ __global__ void k_slab_plan(const int *__restrict__ id, int n, int *nbr_count, i
         if (a >= 0) { border_prev[a] = s; map_prev[g] = -1; }
         if (b >= 0) { border_next[b] = s; map_next[g] = -1; }
     }
+}
+
+// both messages of a step in one launch: threads [0, k0) serve the first list, [k0, k0 + k1) the second
+__global__ void k_slab_pack2(md_slab_frame f, const float4 *__restrict__ pos, const int *__restrict__ slots0, int k0,
+                             float4 *__restrict__ rows0, const int *__restrict__ slots1, int k1,
+                             float4 *__restrict__ rows1) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= k0 + k1) return;
+    const bool first = t < k0;
+    const int u = first ? t : t - k0;
+    float4 p = pos[(first ? slots0 : slots1)[u]];
+    p.x = slab_to_global(f, p.x);
+    (first ? rows0 : rows1)[u] = p;
+}
+__global__ void k_slab_unpack2(md_slab_frame f, const float4 *__restrict__ rows0, const int *__restrict__ slots0, int k0,
+                               const float4 *__restrict__ rows1, const int *__restrict__ slots1, int k1,
+                               float4 *__restrict__ pos) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= k0 + k1) return;
+    const bool first = t < k0;
+    const int u = first ? t : t - k0;
+    float4 p = (first ? rows0 : rows1)[u];
+    p.x = slab_to_local(f, p.x);
+    pos[(first ? slots0 : slots1)[u]] = p;
 }
 
 __global__ void k_iota(int n, int *id) {
@@ -1425,14 +1480,37 @@ static int check_frame(const md_slab_frame *f) {
 }
 
 int md_slab_kick_drift(md_system *sys, const md_slab_frame *frame, void *pos, void *vel, const void *force,
-                       float dt, float mass, int32_t *flag, void *stream) {
+                       const int32_t *id, float dt, float mass, int32_t *flag, const int32_t *stop, void *stream) {
     if (int rc = check_frame(frame)) return rc;
-    if (int rc = md_kick_drift(sys, pos, vel, force, dt, mass, flag, stream)) return rc;
+    if (!sys || !pos || !vel || !force || !id || !flag) return fail(MD_EINVAL, "NULL argument");
+    if (!aligned16(pos) || !aligned16(vel) || !aligned16(force)) return fail(MD_EINVAL, "pos/vel/force must be 16-byte aligned");
+    if (!(dt > 0.0f) || !(mass > 0.0f)) return fail(MD_EINVAL, "dt and mass must be positive");
+    if (sys->r0 != 0 || sys->r1 != sys->n) return fail(MD_EINVAL, "a slab rank steps its whole local system: md_set_range must cover it");
     DeviceScope scope_(sys->device);
     if (scope_.rc) return scope_.rc;
-    k_slab_convert<<<blocks_for(sys->n), 256, 0, (cudaStream_t)stream>>>(*frame, (float4 *)pos, sys->n, 2);
+    cudaStream_t st = (cudaStream_t)stream;
+    const Geom &g = sys->g;
+    const float a = dt / (2.0f * mass);
+    if (g.dim == 3) k_slab_kick_drift<3><<<blocks_for(g.n), 256, 0, st>>>(g, *frame, (float4 *)pos, (float4 *)vel, (const float4 *)force, sys->ref_pos, id, a, dt, flag, stop);
+    else k_slab_kick_drift<2><<<blocks_for(g.n), 256, 0, st>>>(g, *frame, (float4 *)pos, (float4 *)vel, (const float4 *)force, sys->ref_pos, id, a, dt, flag, stop);
     LAUNCH_OK();
     return MD_OK;
+}
+
+int md_slab_force_half_kick(md_system *sys, const md_potential *pot, const void *pos, const int32_t *nbr_idx,
+                            const int32_t *nbr_count, void *force, void *vel, float dt, float mass,
+                            const int32_t *flag, int32_t *stop, int32_t *done, void *stream) {
+    if (!sys || !pos || !nbr_idx || !nbr_count || !force || !vel) return fail(MD_EINVAL, "NULL argument");
+    if (!aligned16(pos) || !aligned16(force) || !aligned16(vel)) return fail(MD_EINVAL, "pos/force/vel must be 16-byte aligned");
+    if (!(dt > 0.0f) || !(mass > 0.0f)) return fail(MD_EINVAL, "dt and mass must be positive");
+    Pair pp;
+    int rc = make_pair(sys, pot, &pp);
+    if (rc) return rc;
+    DeviceScope scope_(sys->device);
+    if (scope_.rc) return scope_.rc;
+    Book book = {nullptr, nullptr, nullptr, flag, stop, done};
+    return launch_force(sys, pp, (const float4 *)pos, nbr_idx, nbr_count, (float4 *)force, (float4 *)vel,
+                        dt / (2.0f * mass), nullptr, false, book, (cudaStream_t)stream);
 }
 
 int md_slab_convert(const md_slab_frame *frame, void *pos, int n, int to_local, void *stream) {
@@ -1462,6 +1540,43 @@ int md_slab_unpack(const md_slab_frame *frame, const void *rows, const int32_t *
     k_slab_unpack<<<blocks_for(k), 256, 0, (cudaStream_t)stream>>>(*frame, (const float4 *)rows, slots, k, (float4 *)pos);
     LAUNCH_OK();
     return MD_OK;
+}
+
+int md_slab_step_open(md_system *sys, const md_slab_frame *frame, void *pos, void *vel, const void *force,
+                      const int32_t *id, float dt, float mass, int32_t *flag, const int32_t *stop,
+                      const int32_t *border_prev, int k_prev, void *rows_prev, const int32_t *border_next,
+                      int k_next, void *rows_next, void *stream) {
+    if (k_prev < 0 || k_next < 0 || (k_prev > 0 && (!border_prev || !rows_prev)) || (k_next > 0 && (!border_next || !rows_next)))
+        return fail(MD_EINVAL, "border lists: NULL argument or negative length");
+    if (int rc = md_slab_kick_drift(sys, frame, pos, vel, force, id, dt, mass, flag, stop, stream)) return rc;
+    if (k_prev + k_next == 0) return MD_OK;
+    DeviceScope scope_(sys->device);
+    if (scope_.rc) return scope_.rc;
+    k_slab_pack2<<<blocks_for(k_prev + k_next), 256, 0, (cudaStream_t)stream>>>(*frame, (const float4 *)pos, border_prev, k_prev,
+                                                                               (float4 *)rows_prev, border_next, k_next,
+                                                                               (float4 *)rows_next);
+    LAUNCH_OK();
+    return MD_OK;
+}
+
+int md_slab_step_close(md_system *sys, const md_slab_frame *frame, const md_potential *pot, const void *rows_prev,
+                       const int32_t *halo_prev, int h_prev, const void *rows_next, const int32_t *halo_next,
+                       int h_next, void *pos, const int32_t *nbr_idx, const int32_t *nbr_count, void *force,
+                       void *vel, float dt, float mass, const int32_t *flag, int32_t *stop, int32_t *done,
+                       void *stream) {
+    if (int rc = check_frame(frame)) return rc;
+    if (!sys || !pos) return fail(MD_EINVAL, "NULL argument");
+    if (h_prev < 0 || h_next < 0 || (h_prev > 0 && (!halo_prev || !rows_prev)) || (h_next > 0 && (!halo_next || !rows_next)))
+        return fail(MD_EINVAL, "halo lists: NULL argument or negative length");
+    if (h_prev + h_next > 0) {
+        DeviceScope scope_(sys->device);
+        if (scope_.rc) return scope_.rc;
+        k_slab_unpack2<<<blocks_for(h_prev + h_next), 256, 0, (cudaStream_t)stream>>>(*frame, (const float4 *)rows_prev, halo_prev,
+                                                                                   h_prev, (const float4 *)rows_next, halo_next,
+                                                                                   h_next, (float4 *)pos);
+        LAUNCH_OK();
+    }
+    return md_slab_force_half_kick(sys, pot, pos, nbr_idx, nbr_count, force, vel, dt, mass, flag, stop, done, stream);
 }
 
 int md_slab_split(const md_slab_frame *frame, float lo, float hi, const void *pos, const void *vel,

@@ -328,6 +328,7 @@ k_force32(Geom g, Pair pp, Pair32 p32, const float4 *__restrict__ pos,
         if (bid >= nblocks) return;
     }
     const int gid = i0 + bid * blockDim.x + threadIdx.x;      // i0: first particle of this context's range
+    if (book_skips(book, gid)) return;
     const int i = gid;
     const bool active = i < g.n;
     const int ii = active ? i : g.n - 1;
@@ -432,6 +433,7 @@ k_force32(Geom g, Pair pp, Pair32 p32, const float4 *__restrict__ pos,
             atomicAdd(energy_total, t);
         }
     }
+    if (book.done && gid == 0) *book.done += 1;
     if (book.stats && gid == 0) {
         if (ld_volatile(book.flag)) {
             book.stats[1] += 1;

@@ -54,14 +54,27 @@ struct Pair {
     double bks_a, bks_tsp, bks_ec, bks_fc, bks_rc;
 };
 
+__device__ __forceinline__ int ld_volatile(const int *p) { return *(const volatile int *)p; }
+
 // Device words md_nve_step keeps between kernels.
 struct Book {
     int *flag;      // rebuild needed (set by drift, cleared by the force kernel)
     int *status;    // {overflow, max count} of the last build
     int *stats;     // {steps, rebuilds, first overflow step | -1, max count}
+    // slab steps enqueued ahead of the host (md_slab_force_half_kick): while *skip != 0 the kernel does
+    // nothing but raise *stop, which the drift kernels of the steps behind it read; *done counts the
+    // force evaluations that did run
+    const int *skip;
+    int *stop;
+    int *done;
 };
+// true: this launch must not touch the state (a rank's list is stale and the host has not rebuilt yet)
+__device__ __forceinline__ bool book_skips(const Book &book, int gid) {
+    if (!book.skip || !ld_volatile(book.skip)) return false;
+    if (gid == 0 && book.stop) *book.stop = 1;
+    return true;
+}
 
-__device__ __forceinline__ int ld_volatile(const int *p) { return *(const volatile int *)p; }
 
 // What a drift kernel does when one of its particles has moved beyond skin/2: raise the device
 // flag and, when the step runs inside a CUDA graph, the condition of the rebuild's IF node.
@@ -1004,6 +1017,7 @@ __device__ __forceinline__ void force_epilogue(const Pair &pp, const Acc64 &acc,
             atomicAdd(energy_total, t);
         }
     }
+    if (book.done && gid == 0) *book.done += 1;
     if (book.stats && gid == 0) {
         if (ld_volatile(book.flag)) {
             book.stats[1] += 1;
@@ -1027,6 +1041,7 @@ k_force(Geom g, Pair pp, const float4 *__restrict__ pos, const int *__restrict__
     __shared__ double sp[KIND == 4 || KIND == 5 ? SP_TAB : 1];
     if (KIND == 4 || KIND == 5) species_tables_to_shared(pp, sp);
     const int gid = i0 * TPP + blockIdx.x * blockDim.x + threadIdx.x;     // i0: first particle of the range
+    if (book_skips(book, gid)) return;
     const int i = gid / TPP, sub = gid % TPP;
     const bool active = i < g.n;
     const int ii = active ? i : g.n - 1;
@@ -1099,6 +1114,7 @@ k_force_stream(Geom g, Pair pp, const float4 *__restrict__ pos, const int *__res
     if (KIND == 4 || KIND == 5) species_tables_to_shared(pp, sp);
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int gid = i0 + blockIdx.x * blockDim.x + threadIdx.x;
+    if (book_skips(book, gid)) return;
     const int i = gid;
     const bool active = i < g.n;
     const int ii = active ? i : g.n - 1;

@@ -8,15 +8,17 @@ library on a LOCAL box (x side: slab + two halos + an empty gap >= R, so that no
 sees comes through the local box's own periodic wrap; y, z: the full box), and every step of the path --
 cell list, neighbor list, force, velocity Verlet -- runs in the library's kernels on that local system:
 
-    every step      md_kick_drift (all local particles; halo copies have zero velocity and zero force, so
-                    they stay), the x coordinates are put back on the global fp32 grid, the flags of all
-                    ranks are OR-ed; if no rebuild: every rank sends the new positions of its BORDER
-                    particles (the owned ones that are somebody's halo; index lists fixed since the last
-                    rebuild) to its two neighbors, which overwrite their halo copies; md_force_half_kick
+    every step      md_slab_step_open: kick and drift of the owned particles, x put back on the global fp32
+                    grid, half-skin test (a device flag word), the new positions of the BORDER particles
+                    (the owned ones that are somebody's halo; index lists fixed since the last rebuild) packed
+                    for the two neighbors; the exchange; md_slab_step_close: the received rows over the halo
+                    copies, force and second half-kick.  The host enqueues batches of steps and reads one
+                    device word per batch: once a flag is up every later call of the batch is a no-op.
     at a rebuild    owned particles that left the slab MIGRATE to the neighbor (position, velocity, id);
                     halos are re-selected; the local system is re-created for the new particle count;
                     md_cell_list_build + md_neighbor_list_build; the list counts of halo copies are set to
-                    0, so the force kernels give them zero force and zero energy
+                    0, so the force kernels give them zero force and zero energy.  Five device phases
+                    (md_slab_split / append / border / load / plan); the host reads two count arrays.
 
 Exactness.  A local x coordinate is the global one minus a non-negative multiple of 2^-8 (or, for the one
 image each of rank 0 and the last rank takes through the box boundary, the Sterbenz-exact x - L plus the
@@ -260,6 +262,12 @@ class SlabRank:
         self.halo_slots = torch.zeros(2 * self.cap_rows, **i32)
         self.border = (None, None)  # local slots of my border particles for (prev, next)
         self.halo = (None, None)    # local slots of the copies that came from (prev, next), in arrival order
+        # {flag: a list is stale, stop: every step call is a no-op, done: steps completed}; the ranks of one
+        # process share the words (attach), ranks in different processes all-reduce the flag every step
+        self.words = torch.zeros(4, **i32)
+
+    def attach(self, words: torch.Tensor):
+        self.words = words
 
     def _read_counts(self):
         c = self.counts.tolist()                                # the host read of this phase
@@ -331,24 +339,26 @@ class SlabRank:
         self.rebuilds += 1
 
     # ---- the phases of an ordinary step ------------------------------------------------------
-    def drift(self):
-        """v += dt/2m F, r = mu(r, dt v) on the local system; x back on the global fp32 grid.  Returns the
-        device flag (1: one of my particles is more than skin / 2 from where the lists were built)."""
+    def open_step(self):
+        """v += dt/2m F, r = mu(r, dt v) on my owned particles, x back on the global fp32 grid; raises the flag
+        word when one of them is more than skin / 2 from where the lists were built; a no-op once the stop word
+        is up.  Returns the new positions (global x) of my border particles, for (prev, next)."""
         B, S, w = self.B, self.S, self.w
-        B.md_slab_kick_drift(S.sys, self.frame, S.pos, S.vel, S.force, w.dt, w.mass, S.flag)
-        return S.flag
-
-    def step_rows(self):
-        """New positions (global x) of my border particles, for (prev, next)."""
-        for slots, rows in zip(self.border, self.rows_out):
-            self.B.md_slab_pack(self.frame, self.S.pos, slots, rows)     # rows = pos[slots], x global
+        B.md_slab_step_open(S.sys, self.frame, S.pos, S.vel, S.force, S.id, w.dt, w.mass, self.words[0:1],
+                            self.words[1:2], self.border[0], self.rows_out[0], self.border[1], self.rows_out[1])
         return self.rows_out
 
-    def absorb(self, from_prev, from_next):
-        for slots, rows in zip(self.halo, (from_prev, from_next)):
-            self.B.md_slab_unpack(self.frame, rows, slots, self.S.pos)   # pos[slots] = rows, x local (the image follows from x)
+    def close_step(self, from_prev, from_next, count: bool = False):
+        """The neighbours' rows into my halo copies (the image follows from x), then F = F(r), v += dt/2m F:
+        a no-op that raises the stop word while the flag word is up.  count: this rank's call is the one that
+        counts the step in the done word."""
+        B, S, w = self.B, self.S, self.w
+        B.md_slab_step_close(S.sys, self.frame, S.pot, from_prev, self.halo[0], from_next, self.halo[1], S.pos,
+                             S.nbr_idx, S.nbr_count, S.force, S.vel, w.dt, w.mass, self.words[0:1], self.words[1:2],
+                             self.words[2:3] if count else None)
 
     def force_kick(self):
+        """F = F(r), v += dt/2m F on the lists just rebuilt (the second half of an interrupted step)."""
         S, w = self.S, self.w
         self.B.md_force_half_kick(S.sys, S.pot, S.pos, S.nbr_idx, S.nbr_count, S.force, S.vel, w.dt, w.mass)
 
@@ -375,19 +385,38 @@ def rebuild_all(ranks, comm, initial=None):
         r.rebuild(fp, fn)
 
 
-def step_all(ranks, comm, nsteps: int):
-    """nsteps velocity-Verlet steps of all ranks this process drives (one per process across GPUs)."""
-    for _ in range(nsteps):
-        flags = [r.drift() for r in ranks]
-        if comm.any_flag(flags):                                         # the one host read of the step
+def step_all(ranks, comm, nsteps: int, state=None):
+    """nsteps velocity-Verlet steps of the ranks this process drives (one per process across GPUs).  The host
+    runs ahead of the device: it enqueues a batch of steps (drift, flag, exchange, force) and reads the done
+    word once per batch.  From the step whose drift finds a stale list on any rank every later call of the
+    batch is a no-op on the device; the host then rebuilds, finishes that step and goes on.  state: dict that
+    carries the batch length from call to call (the last rebuild interval)."""
+    state = {} if state is None else state
+    words = ranks[0].words
+    left = nsteps
+    interval = state.get("interval", 8)                  # steps between the last two rebuilds
+    since = state.get("since", 0)                        # steps since the last rebuild
+    while left > 0:
+        # up to where the next rebuild is expected in one batch, short batches beyond it
+        k = min(left, max(1, interval - since) if since < interval else max(1, interval // 4))
+        words.zero_()
+        for _ in range(k):
+            out = [r.open_step() for r in ranks]
+            comm.share_flag(words)
+            got = comm.shift_rows([o[0] for o in out], [o[1] for o in out], [tuple(h.numel() for h in r.halo) for r in ranks])
+            for i, (r, (fp, fn)) in enumerate(zip(ranks, got)):
+                r.close_step(fp, fn, count=(i == 0))
+        done = int(words[2])                               # the one host read of the batch
+        left -= done
+        since += done
+        if done < k:                                       # step done + 1 has drifted and waits for its lists
             rebuild_all(ranks, comm)
-        else:
-            out = [r.step_rows() for r in ranks]
-            got = comm.shift([o[0] for o in out], [o[1] for o in out])
-            for r, (fp, fn) in zip(ranks, got):
-                r.absorb(fp, fn)
-        for r in ranks:
-            r.force_kick()
+            words.zero_()
+            for r in ranks:
+                r.force_kick()
+            left -= 1
+            interval, since = max(1, since), 0
+    state["interval"], state["since"] = interval, since
 
 
 class LocalComm:
@@ -400,8 +429,11 @@ class LocalComm:
         P = self.world
         return [(to_next[(r - 1) % P], to_prev[(r + 1) % P]) for r in range(P)]
 
-    def any_flag(self, flags) -> bool:
-        return bool(torch.cat(flags).any())
+    def shift_rows(self, to_prev: list, to_next: list, sizes):
+        return self.shift(to_prev, to_next)
+
+    def share_flag(self, words):
+        pass                                             # the ranks of one process share the words
 
 
 class DistComm:
@@ -450,10 +482,21 @@ class DistComm:
         rp, rn = self._sendrecv(a, b, a.shape[1:], a.dtype)
         return [(rp, rn)]
 
-    def any_flag(self, flags) -> bool:
-        f = flags[0].clone()
-        self.dist.all_reduce(f, op=self.dist.ReduceOp.MAX, group=self.group)
-        return bool(f.any())
+    def shift_rows(self, to_prev: list, to_next: list, sizes):
+        """The step exchange: both ends know the row counts from the rebuild, nothing passes through the host."""
+        a, b = to_prev[0], to_next[0]
+        k_prev, k_next = sizes[0]
+        key = (k_prev, k_next, a.device, a.dtype)
+        if getattr(self, "_rows_key", None) != key:
+            self._rows_key = key
+            self._rows = (torch.empty((k_prev,) + tuple(a.shape[1:]), dtype=a.dtype, device=a.device),
+                          torch.empty((k_next,) + tuple(a.shape[1:]), dtype=a.dtype, device=a.device))
+        r_prev, r_next = self._rows
+        self._pairs(a if a.shape[0] else None, b if b.shape[0] else None, r_prev if k_prev else None, r_next if k_next else None)
+        return [(r_prev, r_next)]
+
+    def share_flag(self, words):
+        self.dist.all_reduce(words[0:1], op=self.dist.ReduceOp.MAX, group=self.group)
 
 
 class SlabRun:
@@ -472,6 +515,9 @@ class SlabRun:
         self.comm = LocalComm(world)
         self.slab_ranks = [SlabRank(B, w, fr, dev, reserve) for fr in self.frames]
         self.ranks = [r.S for r in self.slab_ranks]
+        for r in self.slab_ranks[1:]:
+            r.attach(self.slab_ranks[0].words)
+        self._step_state = {}
         pos = torch.from_numpy(w.pos).to(dev)
         vel = torch.from_numpy(w.vel).to(dev)
         gid = torch.arange(w.n, dtype=torch.int32, device=dev)
@@ -492,7 +538,7 @@ class SlabRun:
         return out
 
     def step(self, nsteps: int):
-        step_all(self.slab_ranks, self.comm, nsteps)
+        step_all(self.slab_ranks, self.comm, nsteps, self._step_state)
 
     # ---- results ------------------------------------------------------------------------------
     def gather(self, with_force: bool = False):

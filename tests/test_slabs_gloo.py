@@ -36,8 +36,18 @@ def _worker(rank, world, port, q):
             # plain tensors (the per-step position rows)
             (tp, tn), = comm.shift([torch.full((rank + 1, 4), float(rank))], [torch.full((rank + 2, 4), -float(rank))])
             ok &= torch.equal(tp, torch.full((prev + 2, 4), -float(prev))) and torch.equal(tn, torch.full((nxt + 1, 4), float(nxt)))
-        flags = [comm.any_flag([torch.tensor([1 if rank == r else 0], dtype=torch.int32)]) for r in range(world)]
-        none = comm.any_flag([torch.zeros(1, dtype=torch.int32)])
+            # the step exchange: row counts known to both ends, the receive buffers reused from step to step
+            for _ in range(2):
+                (tp, tn), = comm.shift_rows([torch.full((rank + 1, 4), float(rank + rnd))], [torch.full((rank + 2, 4), -float(rank + rnd))],
+                                            [(prev + 2, nxt + 1)])
+                ok &= torch.equal(tp, torch.full((prev + 2, 4), -float(prev + rnd))) and torch.equal(tn, torch.full((nxt + 1, 4), float(nxt + rnd)))
+        flags = []
+        for r in list(range(world)) + [-1]:
+            words = torch.tensor([1 if rank == r else 0, 0, 5, 0], dtype=torch.int32)
+            comm.share_flag(words)                                   # only the flag word travels
+            ok &= words.tolist()[1:] == [0, 5, 0]
+            flags.append(bool(words[0]))
+        none = flags.pop()
         q.put((rank, bool(ok), flags, none))
     finally:
         dist.destroy_process_group()
