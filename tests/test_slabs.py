@@ -166,3 +166,64 @@ def test_slabs_against_the_oracle_and_one_gpu(B, orc, W, world):
     r1 = int(one.stats[1])
     assert abs(run.rebuilds - r1) <= max(2, r1 // 3), (run.rebuilds, r1)
     one.close(); run.close()
+
+
+@pytest.mark.gpu
+def test_rebuild_phases_against_the_reference_selection(B, W):
+    """md_slab_split / border / load / plan (the rebuild on the device) against the torch reference functions
+    of slabs.py that the CPU tests above pin: who stays, who migrates where, who is border, and that the
+    exchange plan pairs every border particle with its copy on the neighbour."""
+    w = W.config(2)
+    world = 4
+    run = SL.SlabRun(B, w, world)
+    run.step(37)
+    torch.cuda.synchronize()
+    f32 = np.float32
+    ranks = run.slab_ranks
+    migrants = 0
+    for r in ranks:
+        S, fr = r.S, r.fr
+        n = S.n
+        ids = S.id[:n]
+        owned = ids >= 0
+        gid = ids[owned]
+        xg = SL.local_to_global(S.pos[:n, 0][owned], fr)
+        own = SL.owner_of(xg, r.frames)
+        (pr, pi), (nr, ni) = r.leavers()
+        for rows, mids, rank in ((pr, pi, r.prev), (nr, ni, r.next)):
+            want = gid[own == rank]
+            assert sorted(mids.tolist()) == sorted(want.tolist())
+            migrants += int(mids.numel())
+            if mids.numel():
+                # a row is (position with global x | velocity) of that particle
+                slot = torch.full((w.n,), -1, dtype=torch.long, device=ids.device)
+                slot[gid.long()] = torch.arange(n, device=ids.device)[owned]
+                s = slot[mids.long()]
+                assert torch.equal(rows[:, 1:4], S.pos[s, 1:4]) and torch.equal(rows[:, 4:], S.vel[s])
+                assert torch.equal(rows[:, 0], SL.local_to_global(S.pos[s, 0], fr))
+        stay = r.own_id[: r.n_own]
+        assert sorted(stay.tolist()) == sorted(gid[own == fr.rank].tolist())
+        (bp, bpi), (bn, bni) = r.border_rows()
+        x_own, id_own = r.own_pos[: r.n_own, 0], r.own_id[: r.n_own]
+        assert sorted(bpi.tolist()) == sorted(id_own[x_own < f32(fr.lo + fr.H)].tolist())
+        assert sorted(bni.tolist()) == sorted(id_own[x_own >= f32(fr.hi - fr.H)].tolist())
+        assert int((r.map_prev >= 0).sum()) == bpi.numel() and int((r.map_next >= 0).sum()) == bni.numel()
+    assert migrants > 0
+    # the whole protocol, then the plan
+    SL.rebuild_all(ranks, run.comm)
+    torch.cuda.synchronize()
+    for r in ranks:
+        S = r.S
+        for m in (r.map_prev, r.map_next, r.map_halo):
+            assert int((m >= 0).sum()) == 0
+        ids = S.id[: S.n]
+        assert int(S.nbr_count[: S.n][ids < 0].abs().sum()) == 0 and int(S.nbr_count[: S.n][ids >= 0].min()) > 0
+        prev, nxt = ranks[r.prev], ranks[r.next]
+        # what my previous rank sends to ITS next lands on my `from prev` copies, row by row
+        sent_by_prev = S.id.new_tensor(prev.S.id[prev.border[1].long()].tolist())
+        sent_by_next = S.id.new_tensor(nxt.S.id[nxt.border[0].long()].tolist())
+        assert torch.equal(ids[r.halo[0].long()], -1 - sent_by_prev)
+        assert torch.equal(ids[r.halo[1].long()], -1 - sent_by_next)
+        assert torch.equal(S.id[r.border[0].long()], r.bor_ids[0][: r.n_border[0]])
+        assert torch.equal(S.id[r.border[1].long()], r.bor_ids[1][: r.n_border[1]])
+    run.close()
