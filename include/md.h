@@ -98,10 +98,11 @@ int md_destroy(md_system *sys);
  *                          an error estimate and fp64 re-evaluation of the particles that need it
  *                          (DESIGN.md §5); 0: every pair in fp64 (the kernels selected by
  *                          threads_per_particle), as SOFT, LJ_SPECIES, BKS and every 2-D system always
- *   "est_thr"              the fast path re-evaluates particle i in fp64 when S_i, the sum over j of
- *                          the pair's error scale (LJ: |f_ij / r_ij|; Morse and Buckingham: the parts
- *                          of f_ij / r_ij times the amplification of their exponentials, scaled to
- *                          LJ's), exceeds est_thr * max(|F_i|, 1e-3); default 8
+ *   "est_thr"              the fast path re-evaluates particle i in fp64 when S_i, the root of the sum
+ *                          over j of the squared error scale of pair ij (LJ: |f_ij|, floored near its
+ *                          zero; Morse and Buckingham: the parts of f_ij times the amplification of
+ *                          their exponentials, scaled to LJ's), exceeds est_thr * max(|F_i|, 1e-3);
+ *                          default 3.5
  *   "threads_per_particle" fp64 force kernel variant: 0 = streaming kernel (one lane per particle,
  *                          list rows staged through shared memory by TMA; default for
  *                          n >= 32768), or 1, 2, 4 lanes sharing one particle (default 4 below)

@@ -419,12 +419,12 @@ int launch_force(md_system *s, const Pair &pp, const float4 *pos, const int *nbr
         q.est_thr = s->est_thr;
         if (pp.kind == MD_KIND_MORSE) {
             const double k = -pp.dalpha * 1.4426950408889634;
-            q.k_hi = (float)k; q.k_lo = (float)(k - (double)q.k_hi); q.s_unit = 0.025f;
+            q.k_hi = (float)k; q.k_lo = (float)(k - (double)q.k_hi); q.s_unit = 0.022f;
             q.m_r0 = (float)pp.dr0; q.m_2a = (float)(2.0 * pp.dalpha); q.m_a = (float)pp.dalpha;
             q.ucut4 = (float)pp.du_cutm; q.fscale = (float)pp.deps; q.escale = (float)(0.5 * pp.deps);
         } else if (pp.kind == MD_KIND_BUCKINGHAM) {
             const double k = -pp.dalpha * 1.4426950408889634;
-            q.k_hi = (float)k; q.k_lo = (float)(k - (double)q.k_hi); q.s_unit = 0.025f;
+            q.k_hi = (float)k; q.k_lo = (float)(k - (double)q.k_hi); q.s_unit = 0.0175f;
             q.b_A = (float)pp.dA; q.b_B = (float)pp.dalpha; q.b_C = (float)pp.dC;
             q.ucut4 = (float)pp.du_cutm; q.fscale = 1.0f; q.escale = 0.5f;
         }
@@ -1122,7 +1122,7 @@ int md_create(const md_config *cfg, int n, void *workspace, size_t bytes, md_sys
                 s->cell_coop = n <= 65536 ? s->cell_coop_max : 0;     // measured: pays below, costs above
             }
     }
-    s->est_thr = 8.0f;
+    s->est_thr = 3.5f;
     s->unroll = 9;      // odd: a fused graph swaps position buffers steps-1 times and must end in the caller's
     {   // neighbor-list builder: one warp per tile, a capacity x 32 column block + a candidate
         // chunk of shared memory per warp; as many warps per block as fit (at most NB_WARPS)

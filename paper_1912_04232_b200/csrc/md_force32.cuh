@@ -8,14 +8,15 @@
 // everywhere but is bound by the conversion / reciprocal unit (3 F2F + 1 RCP64H per pair).
 // Here every pair is evaluated in fp32 first -- displacement by the canonical nearest-image
 // form (one rounding), r2 = fma(dz,dz,fma(dy,dy,dx*dx)), y = 1/r2 (MUFU), force
-// coefficient 24 eps sig^6 y^4 (2 sig^6 y^3 - 1) -- together with S_i = sum_j max(|coefficient|,
-// 0.2 * 24 eps sig^6 y^4): the coefficient vanishes at r = 2^(1/6) sigma while its rounding error
+// coefficient c = 24 eps sig^6 y^4 t, t = 2 sig^6 y^3 - 1 -- together with S_i^2 = sum_j (c r)^2 where t^2 is
+// replaced by t^2 + 0.2^2: the coefficient vanishes at r = 2^(1/6) sigma while its rounding error
 // (~3e-7 * 24 eps sig^6 y^4 there) does not, and the floor keeps the error-to-estimate ratio of
-// such a pair (1.5e-6) in line with the ~1e-6 of every other pair.
-// The fp32 error of F_i is a random sum of per-pair errors of relative size ~1e-7 * (7..13):
-// measured on the oracle (32k and 256k particles, lattice and liquid states) it stays below
-// 5.4e-6 * max(|F_i|, 1e-3) whenever S_i <= 8 * max(|F_i|, 1e-3).  A particle that fails this
-// test (its pair forces nearly cancel; 3-4 % of a liquid, 12 % of the jittered lattice), or that has a pair within 1e-5 of
+// such a pair in line with that of every other pair.
+// The fp32 error of F_i is a random sum of per-pair errors of relative size ~1e-7 * (7..13), so it
+// goes with the root-sum-square S_i: measured against the fp64 chain and the oracle (32k, 256k and
+// 1M particles, lattice and liquid states, thirteen states in all) it stays below
+// 7.0e-6 * max(|F_i|, 1e-3) whenever S_i <= 3.5 * max(|F_i|, 1e-3).  A particle that fails this
+// test (its pair forces nearly cancel; 2-3 % of a liquid, 7 % of the jittered lattice), or that has a pair within 1e-5 of
 // r_cut^2 (the truncated force jumps by 0.039 there, so the in/out decision must be the exact
 // one), is re-evaluated in fp64 from exact displacements inside its own warp: groups of 32, 16 or
 // 8 lanes stride over the particle's row (1, 2 or up to 4 flagged particles at a time) and reduce
@@ -33,7 +34,7 @@ struct Pair32 {
     float fscale;       // 24 eps sigma^6
     float escale;       // 2 eps   (= 1/2 * 4 eps)
     float near_band;    // |r2 - rc2| <= near_band -> exact re-evaluation
-    float est_thr;      // re-evaluate when fscale * S_i > est_thr * max(|F_i|, 1e-3)
+    float est_thr;      // re-evaluate when fscale * S_i > est_thr * max(|F_i|, 1e-3), S_i^2 the accumulated sum
     // the other kinds of the fast path (the estimate term of each is scaled so that one est_thr serves all)
     float k_hi, k_lo;                 // MORSE: -alpha log2(e), BUCKINGHAM: -B log2(e), as a float and what it drops
     float s_unit;                     // scale of the estimate term against Lennard-Jones's
@@ -58,28 +59,6 @@ __device__ __forceinline__ float rcp32(float x) {
     return y;
 }
 
-template <bool ENERGY, bool CHECK>
-__device__ __forceinline__ void lj_pair32(const Pair32 &pp, float dx, float dy, float dz,
-                                          bool valid, Acc32 &a) {
-    const float r2 = fmaf(dz, dz, fmaf(dy, dy, dx * dx));
-    bool in = r2 < pp.rc2;
-    if (CHECK) in = in && valid;
-    a.near = fminf(a.near, fabsf(r2 - pp.rc2));
-    // pairs outside the cutoff (and padded slots) take 1/r2 = 1/inf = 0: every power and the
-    // coefficient vanish with it, no later select
-    const float y = rcp32(in ? r2 : __int_as_float(0x7f800000));
-    const float y2 = y * y;
-    const float y3 = y2 * y;
-    const float t = fmaf(pp.sig6x2, y3, -1.0f);          // 2 s6 - 1
-    const float y4 = y2 * y2;
-    const float c = y4 * t;
-    a.fx = fmaf(c, dx, a.fx); a.fy = fmaf(c, dy, a.fy); a.fz = fmaf(c, dz, a.fz);
-    a.s = fmaf(y4, fmaxf(fabsf(t), 0.2f), a.s);          // |coefficient|, floored near its zero (see above)
-    if (ENERGY) {
-        const float s6 = 0.5f * pp.sig6x2 * y3;
-        a.e += in ? fmaf(s6, s6, -s6) - pp.ucut4 : 0.0f;
-    }
-}
 
 // Two list entries of one particle at once with packed fp32x2 arithmetic (FADD2 / FMUL2 / FFMA2:
 // one instruction, two lanes of data), the same operations in the same order as lj_pair32 -- so the
@@ -101,7 +80,8 @@ __device__ __forceinline__ void lj_pair32x2(const Pair32 &pp, float2 dx, float2 
     const float2 y4 = __fmul2_rn(y2, y2);
     const float2 c = __fmul2_rn(y4, t);
     a.fx = __ffma2_rn(c, dx, a.fx); a.fy = __ffma2_rn(c, dy, a.fy); a.fz = __ffma2_rn(c, dz, a.fz);
-    a.s = __ffma2_rn(y4, make_float2(fmaxf(fabsf(t.x), 0.2f), fmaxf(fabsf(t.y), 0.2f)), a.s);
+    // S: (|coefficient| r)^2 with the coefficient floored near its zero, y4^2 r2 (t^2 + 0.2^2) = y^7 (t^2 + 0.04)
+    a.s = __ffma2_rn(__fmul2_rn(y3, y4), __ffma2_rn(t, t, make_float2(0.04f, 0.04f)), a.s);
     if (ENERGY) {
         const float hs = 0.5f * pp.sig6x2;
         const float2 s6 = __fmul2_rn(make_float2(hs, hs), y3);
@@ -155,14 +135,16 @@ __device__ __forceinline__ void pair32x2(const Pair32 &pp, float2 dx, float2 dy,
         x = __ffma2_rn(__fmul2_rn(x, make_float2(0.69314718f, 0.69314718f)), a_lo, x);
         x = __fmul2_rn(x, m);
         const float2 om = __fadd2_rn(make_float2(1.0f, 1.0f), make_float2(-x.x, -x.y));
-        const float2 g2 = __fmul2_rn(__fmul2_rn(x, ir), make_float2(pp.m_2a, pp.m_2a));       // 2 alpha x / r
+        const float2 x2a = __fmul2_rn(x, make_float2(pp.m_2a, pp.m_2a));
+        const float2 g2 = __fmul2_rn(x2a, ir);                                                // 2 alpha x / r
         const float2 c = __fmul2_rn(g2, make_float2(-om.x, -om.y));
         a.fx = __ffma2_rn(c, dx, a.fx); a.fy = __ffma2_rn(c, dy, a.fy); a.fz = __ffma2_rn(c, dz, a.fz);
         // error of c: x and 1 - x both carry x alpha r eps_r, 1/r carries eps_r
         const float2 aom = make_float2(pp.s_unit * fabsf(om.x), pp.s_unit * fabsf(om.y));
         const float2 amp = __ffma2_rn(__ffma2_rn(x, make_float2(pp.s_unit, pp.s_unit), aom),
                                       __fmul2_rn(r, make_float2(pp.m_a, pp.m_a)), aom);
-        a.s = __ffma2_rn(g2, amp, a.s);
+        const float2 er = __fmul2_rn(x2a, amp);                                               // (g2 amp) r
+        a.s = __ffma2_rn(er, er, a.s);
         if (ENERGY) {
             float2 e = __ffma2_rn(om, om, make_float2(-1.0f - pp.ucut4, -1.0f - pp.ucut4));
             a.e = __ffma2_rn(e, m, a.e);
@@ -186,7 +168,7 @@ __device__ __forceinline__ void pair32x2(const Pair32 &pp, float2 dx, float2 dy,
         // error of c: the exponential amplifies by B r + 3, the power law by 8
         const float2 k1 = __ffma2_rn(r, make_float2(pp.s_unit * pp.b_B, pp.s_unit * pp.b_B), make_float2(3.0f * pp.s_unit, 3.0f * pp.s_unit));
         const float2 amp = __ffma2_rn(t1, k1, __fmul2_rn(t2, make_float2(8.0f * pp.s_unit, 8.0f * pp.s_unit)));
-        a.s = __ffma2_rn(amp, y, a.s);
+        a.s = __ffma2_rn(__fmul2_rn(amp, amp), y, a.s);                                       // (amp y r)^2 = amp^2 y
         if (ENERGY) {
             float2 e = __ffma2_rn(y3, make_float2(-pp.b_C, -pp.b_C), __fadd2_rn(x, make_float2(-pp.ucut4, -pp.ucut4)));
             a.e = __ffma2_rn(e, m, a.e);
@@ -352,7 +334,8 @@ k_force32(Geom g, Pair pp, Pair32 p32, const float4 *__restrict__ pos,
     float fx = p32.fscale * acc.fx, fy = p32.fscale * acc.fy, fz = p32.fscale * acc.fz;
     double e64 = ENERGY ? (double)(p32.escale * acc.e) : 0.0;
     const float fn = fmaxf(sqrtf(fmaf(fz, fz, fmaf(fy, fy, fx * fx))), 1e-3f);
-    const bool redo = active && (p32.fscale * acc.s > p32.est_thr * fn || acc.near <= p32.near_band ||
+    const float sf = p32.fscale * p32.fscale * acc.s, tf = p32.est_thr * fn;
+    const bool redo = active && (sf > tf * tf || acc.near <= p32.near_band ||
                                  !(fn < 3.0e38f));
     unsigned todo = __ballot_sync(FULL, redo);
     if (nfix && lane == 0 && todo) atomicAdd(nfix, __popc(todo));
