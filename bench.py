@@ -92,15 +92,19 @@ def peaks():
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons (B200_PROFILING.md).  Started before the warm-up so
-    that the tool is already printing when the timed region begins; stop(t0, t1) keeps only the
-    samples whose timestamp falls inside the timed region [t0, t1] (host wall clock)."""
+    """SM clocks and throttle reasons DURING the timed region (B200_PROFILING.md).  Two sources: the recipe's
+    `nvidia-smi --query-gpu=... -lms 20`, started before the warm-up (start() waits for its first line, so the
+    tool is already printing when the timed region begins), and the same counters read through NVML in this
+    process every 10 ms.  nvidia-smi can take hundreds of ms per query on a busy box, which leaves a 160 ms timed
+    region without a sample; the NVML samples then carry the numbers ("source" says which).  stop(t0, t1) keeps
+    the samples whose timestamp falls inside [t0, t1] (host wall clock)."""
     Q = ("timestamp,index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,"
          "clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index=0):
         self.index, self.proc, self.lines = index, None, []
+        self.nvml, self.nvml_samples, self._run = None, [], False
 
     def start(self):
         try:
@@ -110,22 +114,57 @@ class ClockSampler:
                 stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.t = threading.Thread(target=self._read, daemon=True)
             self.t.start()
+            t_end = time.time() + 3.0
+            while not self.lines and time.time() < t_end and self.proc.poll() is None:
+                time.sleep(0.01)
         except Exception:
             self.proc = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nvml = pynvml
+            self.handle = pynvml.nvmlDeviceGetHandleByIndex(self.index)
+            self._run = True
+            self.t2 = threading.Thread(target=self._poll, daemon=True)
+            self.t2.start()
+        except Exception:
+            self.nvml = None
 
     def _read(self):
         for line in self.proc.stdout:
             self.lines.append(line.strip())
 
+    def _poll(self):
+        N = self.nvml
+        bits = [("hw_slowdown", "nvmlClocksThrottleReasonHwSlowdown"),
+                ("hw_thermal_slowdown", "nvmlClocksThrottleReasonHwThermalSlowdown"),
+                ("sw_thermal_slowdown", "nvmlClocksThrottleReasonSwThermalSlowdown"),
+                ("sw_power_cap", "nvmlClocksThrottleReasonSwPowerCap")]
+        bits = [(n, getattr(N, a)) for n, a in bits if hasattr(N, a)]
+        try:
+            cmax = float(N.nvmlDeviceGetMaxClockInfo(self.handle, N.NVML_CLOCK_SM))
+        except Exception:
+            cmax = None
+        while self._run:
+            try:
+                clk = float(N.nvmlDeviceGetClockInfo(self.handle, N.NVML_CLOCK_SM))
+                mask = int(N.nvmlDeviceGetCurrentClocksThrottleReasons(self.handle))
+                self.nvml_samples.append((time.time(), clk, cmax, [n for n, b in bits if mask & b]))
+            except Exception:
+                pass
+            time.sleep(0.01)
+
     def stop(self, t0=None, t1=None):
         import datetime
-        if not self.proc:
+        self._run = False
+        if not self.proc and not self.nvml:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        self.proc.terminate()
-        try:
-            self.proc.wait(timeout=2)
-        except Exception:
-            self.proc.kill()
+        if self.proc:
+            self.proc.terminate()
+            try:
+                self.proc.wait(timeout=2)
+            except Exception:
+                self.proc.kill()
         sm, mx, reasons, allsm = [], [], set(), []
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
         for ln in self.lines:
@@ -144,9 +183,24 @@ class ClockSampler:
             for name, v in zip(names, f[6:10]):
                 if v.lower().startswith("active"):
                     reasons.add(name)
+        source = "nvidia-smi -lms 20"
+        inside = [q for q in self.nvml_samples if t0 is None or t0 <= q[0] <= t1]
+        if inside and len(inside) > len(sm):
+            # the in-process NVML samples cover the region better: they carry the numbers, reasons are merged
+            source = "NVML in process every 10 ms (nvidia-smi -lms 20 gave %d samples inside the region, %d in all)" % (len(sm), len(allsm))
+            sm = [q[1] for q in inside]
+            mx = [q[2] for q in inside if q[2] is not None] or mx
+            for q in inside:
+                reasons.update(q[3])
+            allsm = [q[1] for q in self.nvml_samples]
+        if self.nvml:
+            try:
+                self.nvml.nvmlShutdown()
+            except Exception:
+                pass
         return {"sm_mhz": statistics.median(sm) if sm else None,
                 "sm_max_mhz": max(mx) if mx else None, "samples": len(sm),
-                "samples_total": len(allsm), "reasons": sorted(reasons)}
+                "samples_total": len(allsm), "reasons": sorted(reasons), "source": source}
 
 
 def oracle_sample(w, md_steps):
