@@ -410,8 +410,6 @@ static void lj_pair(double r2, double eps, double sigma, double *u, double *fr)
 
 /* Morse u(r) = D (1 - exp(-alpha (r - r0)))^2 - D and -u'(r)/r (PAPER.md:L104 [75]; the paper
  * names the potential only: the standard form with well depth D at r0, reading A19). */
-static double g_morse_alpha = 5.0;
-void orc_set_morse_alpha(double alpha) { g_morse_alpha = alpha; }
 
 static void morse_pair(double r, double D, double r0, double alpha, double *u, double *fr)
 {
@@ -422,7 +420,7 @@ static void morse_pair(double r, double D, double r0, double alpha, double *u, d
 
 /* Buckingham-type u(r) = A exp(-B r) - C / r^6 and -u'(r)/r (PAPER.md:L104 [71-73]; the paper names
  * the family only: the exp-6 form without the Coulomb term of BKS, reading A24).
- * A = eps, B = the alpha of orc_set_morse_alpha, C = sigma. */
+ * A = eps, B = orc_params.morse_alpha, C = sigma. */
 static void buck_pair(double r, double A, double B, double Cc, double *u, double *fr)
 {
     double x = A * exp(-B * r), r2 = r * r, r6 = r2 * r2 * r2;
@@ -434,14 +432,36 @@ static void buck_pair(double r, double A, double B, double Cc, double *u, double
  * sigma matrix of L298-L305 App. A): kind 4 reads eps_ab, sigma_ab and the truncation radius rc_ab
  * from tables set here; the species of particle i is (int)diam[i] (the pos.w channel). */
 #define ORC_MAX_SPECIES 4
-static int g_ns = 0;
-static double g_sp_eps[ORC_MAX_SPECIES * ORC_MAX_SPECIES], g_sp_sig[ORC_MAX_SPECIES * ORC_MAX_SPECIES],
-              g_sp_rc[ORC_MAX_SPECIES * ORC_MAX_SPECIES];
-int orc_set_species_lj(int ns, const double *eps, const double *sigma, const double *rc)
+#define ORC_MAX_NH_CHAIN 8
+/* The parameters of kinds 2-5 and the Nose-Hoover chain length travel with every call as one struct (the
+ * Python wrapper owns it); nothing of them is process state.  Unset fields make the call that needs them
+ * fail with ORC_EINVAL: morse_alpha = NaN, ns = 0, bks_ns = 0. */
+typedef struct orc_params {
+    double morse_alpha;                                   /* kind 2: alpha; kind 3: B */
+    int32_t ns;                                           /* kind 4 */
+    int32_t bks_ns;                                       /* kind 5 */
+    int32_t nh_chain;                                     /* 1..ORC_MAX_NH_CHAIN */
+    int32_t pad_;
+    double sp_eps[ORC_MAX_SPECIES * ORC_MAX_SPECIES], sp_sig[ORC_MAX_SPECIES * ORC_MAX_SPECIES],
+           sp_rc[ORC_MAX_SPECIES * ORC_MAX_SPECIES];
+    double bks_A[ORC_MAX_SPECIES * ORC_MAX_SPECIES], bks_B[ORC_MAX_SPECIES * ORC_MAX_SPECIES],
+           bks_C[ORC_MAX_SPECIES * ORC_MAX_SPECIES], bks_q[ORC_MAX_SPECIES], bks_a, bks_k;
+} orc_params;
+
+void orc_params_reset(orc_params *p)
 {
-    if (ns < 1 || ns > ORC_MAX_SPECIES) return ORC_EINVAL;
-    g_ns = ns;
-    for (int k = 0; k < ns * ns; ++k) { g_sp_eps[k] = eps[k]; g_sp_sig[k] = sigma[k]; g_sp_rc[k] = rc[k]; }
+    memset(p, 0, sizeof(*p));
+    p->morse_alpha = NAN;
+    p->nh_chain = 1;
+    p->bks_k = 1.0;
+}
+int orc_params_size(void) { return (int)sizeof(orc_params); }
+
+int orc_params_species_lj(orc_params *p, int ns, const double *eps, const double *sigma, const double *rc)
+{
+    if (!p || ns < 1 || ns > ORC_MAX_SPECIES) return ORC_EINVAL;
+    p->ns = ns;
+    for (int k = 0; k < ns * ns; ++k) { p->sp_eps[k] = eps[k]; p->sp_sig[k] = sigma[k]; p->sp_rc[k] = rc[k]; }
     return ORC_OK;
 }
 
@@ -452,16 +472,13 @@ int orc_set_species_lj(int ns, const double *eps, const double *sigma, const dou
  *   u_C(r) = k q_a q_b [ erfc(a r)/r - erfc(a rc)/rc + (erfc(a rc)/rc^2 + 2a/sqrt(pi) exp(-a^2 rc^2)/rc)(r - rc) ]
  *   -u_C'(r) = k q_a q_b [ erfc(a r)/r^2 + 2a/sqrt(pi) exp(-a^2 r^2)/r - erfc(a rc)/rc^2 - 2a/sqrt(pi) exp(-a^2 rc^2)/rc ]
  * kind 5: species = (int)diam[i]; r_cut is the one truncation radius; shift applies to the exp-6 term. */
-static double g_bks_A[ORC_MAX_SPECIES * ORC_MAX_SPECIES], g_bks_B[ORC_MAX_SPECIES * ORC_MAX_SPECIES],
-              g_bks_C[ORC_MAX_SPECIES * ORC_MAX_SPECIES], g_bks_q[ORC_MAX_SPECIES], g_bks_a = 0.0, g_bks_k = 1.0;
-static int g_bks_ns = 0;
-int orc_set_species_bks(int ns, const double *A, const double *B, const double *Cc, const double *q,
-                        double coulomb_alpha, double k_e)
+int orc_params_species_bks(orc_params *p, int ns, const double *A, const double *B, const double *Cc, const double *q,
+                           double coulomb_alpha, double k_e)
 {
-    if (ns < 1 || ns > ORC_MAX_SPECIES || !(coulomb_alpha >= 0.0)) return ORC_EINVAL;
-    g_bks_ns = ns; g_bks_a = coulomb_alpha; g_bks_k = k_e;
-    for (int k = 0; k < ns * ns; ++k) { g_bks_A[k] = A[k]; g_bks_B[k] = B[k]; g_bks_C[k] = Cc[k]; }
-    for (int k = 0; k < ns; ++k) g_bks_q[k] = q[k];
+    if (!p || ns < 1 || ns > ORC_MAX_SPECIES || !(coulomb_alpha >= 0.0)) return ORC_EINVAL;
+    p->bks_ns = ns; p->bks_a = coulomb_alpha; p->bks_k = k_e;
+    for (int k = 0; k < ns * ns; ++k) { p->bks_A[k] = A[k]; p->bks_B[k] = B[k]; p->bks_C[k] = Cc[k]; }
+    for (int k = 0; k < ns; ++k) p->bks_q[k] = q[k];
     return ORC_OK;
 }
 
@@ -487,13 +504,13 @@ static double lj_u_cut(double eps, double sigma, double r_cut)
  *   kind 1 SOFT: u = eps/2 (1 - r/d_ij)^2 for r < d_ij, d_ij = (d_i + d_j)/2
  *                (PAPER.md:L301); r = 0 gives energy eps/2 and zero force
  *   kind 2 MORSE: u = eps (1 - exp(-alpha (r - sigma)))^2 - eps - shift*u(r_cut) for r < r_cut,
- *                alpha set by orc_set_morse_alpha (PAPER.md:L104 [75])
- *   kind 4 LJ_SPECIES: LJ with eps, sigma, r_cut taken per species pair from orc_set_species_lj,
+ *                alpha = par->morse_alpha (PAPER.md:L104 [75])
+ *   kind 4 LJ_SPECIES: LJ with eps, sigma, r_cut taken per species pair from the tables of par (orc_params_species_lj),
  *                species = (int)diam[i]; eps, sigma, r_cut arguments unused
  *   kind 3 BUCKINGHAM: u = eps exp(-alpha r) - sigma / r^6 - shift*u(r_cut) for r < r_cut
  *                (A = eps, B = alpha, C = sigma; PAPER.md:L104 [71-73])
  *   kind 5 BKS:  exp-6 with A, B, C per species pair plus damped shifted-force Coulomb between the
- *                species' charges (orc_set_species_bks); eps, sigma unused; one r_cut
+ *                species' charges (orc_params_species_bks); eps, sigma unused; one r_cut
  *   nbr_idx == NULL: all pairs j != i (the definition);
  *   else: over the list rows (L80 smap.neighbors), entries >= n are padding.
  *   force double[n*3] (z = 0 in 2-D), e_i double[n], *E double.
@@ -502,15 +519,21 @@ int orc_energy_force(int n, int dim, const double *pos, const double *diam,
                      const double *box, int kind, double eps, double sigma,
                      double r_cut, int shift, const int32_t *nbr_idx,
                      const int32_t *nbr_count, int capacity, double *force,
-                     double *e_i, double *E)
+                     double *e_i, double *E, const orc_params *par)
 {
     if (n <= 0 || (dim != 2 && dim != 3)) return ORC_EINVAL;
     if (kind != KIND_LJ && kind != KIND_SOFT && kind != KIND_MORSE && kind != KIND_BUCK &&
         kind != KIND_LJ_SPECIES && kind != KIND_BKS) return ORC_EINVAL;
     if ((kind == KIND_SOFT || kind == KIND_LJ_SPECIES || kind == KIND_BKS) && !diam) return ORC_EINVAL;
-    if (kind == KIND_LJ_SPECIES && g_ns < 1) return ORC_EINVAL;
-    if (kind == KIND_BKS && g_bks_ns < 1) return ORC_EINVAL;
-    if ((kind == KIND_MORSE || kind == KIND_BUCK) && !(g_morse_alpha == g_morse_alpha)) return ORC_EINVAL;   /* unset */
+    if (kind != KIND_LJ && kind != KIND_SOFT && !par) return ORC_EINVAL;
+    if (kind == KIND_LJ_SPECIES && par->ns < 1) return ORC_EINVAL;
+    if (kind == KIND_BKS && par->bks_ns < 1) return ORC_EINVAL;
+    if ((kind == KIND_MORSE || kind == KIND_BUCK) && !(par->morse_alpha == par->morse_alpha)) return ORC_EINVAL;   /* unset */
+    const double g_morse_alpha = par ? par->morse_alpha : NAN;
+    const int g_ns = par ? par->ns : 0, g_bks_ns = par ? par->bks_ns : 0;
+    const double *g_sp_eps = par ? par->sp_eps : NULL, *g_sp_sig = par ? par->sp_sig : NULL, *g_sp_rc = par ? par->sp_rc : NULL;
+    const double *g_bks_A = par ? par->bks_A : NULL, *g_bks_B = par ? par->bks_B : NULL, *g_bks_C = par ? par->bks_C : NULL;
+    const double *g_bks_q = par ? par->bks_q : NULL, g_bks_a = par ? par->bks_a : 0.0, g_bks_k = par ? par->bks_k : 1.0;
     double u_c = (kind == KIND_LJ && shift) ? lj_u_cut(eps, sigma, r_cut) : 0.0;
     if (kind == KIND_MORSE && shift) {
         double fr_unused;
@@ -644,7 +667,7 @@ int orc_nve_run(int n, int dim, double *pos, double *vel, double *force,
                 const double *diam, const double *box, int kind, double eps,
                 double sigma, double r_cut, int shift, double dt, double mass,
                 int nsteps, int use_list, float skin, int capacity,
-                double *energies, int32_t *stats)
+                double *energies, int32_t *stats, const orc_params *par)
 {
     if (n <= 0 || (dim != 2 && dim != 3) || dt <= 0.0 || mass <= 0.0) return ORC_EINVAL;
     int rc = ORC_OK;
@@ -668,7 +691,7 @@ int orc_nve_run(int n, int dim, double *pos, double *vel, double *force,
     if (energies) {
         double ke = 0.0;
         rc = orc_energy_force(n, dim, pos, diam, box, kind, eps, sigma, r_cut, shift,
-                              idx, cnt, capacity, force, e_i, &E);
+                              idx, cnt, capacity, force, e_i, &E, par);
         if (rc) goto done;
         for (int i = 0; i < n; ++i)
             for (int q = 0; q < dim; ++q) ke += vel[3 * (size_t)i + q] * vel[3 * (size_t)i + q];
@@ -693,7 +716,7 @@ int orc_nve_run(int n, int dim, double *pos, double *vel, double *force,
             }
         }
         rc = orc_energy_force(n, dim, pos, diam, box, kind, eps, sigma, r_cut, shift,
-                              idx, cnt, capacity, force, e_i, &E);
+                              idx, cnt, capacity, force, e_i, &E, par);
         if (rc) goto done;
         double ke = 0.0;
         for (int i = 0; i < n; ++i)
@@ -729,17 +752,17 @@ done:
  */
 int orc_fire_run(int n, int dim, double *pos, double *vel, double *force, const double *diam,
                  const double *box, int kind, double eps, double sigma, double r_cut, int shift,
-                 const double *par, double *state, int nsteps, double *energies)
+                 const double *fire, double *state, int nsteps, double *energies, const orc_params *par)
 {
-    if (n <= 0 || (dim != 2 && dim != 3) || !par || !state) return ORC_EINVAL;
+    if (n <= 0 || (dim != 2 && dim != 3) || !fire || !state) return ORC_EINVAL;
     double *e_i = (double *)malloc((size_t)n * sizeof(double));
     if (!e_i) return ORC_ENOMEM;
     double dt = state[0], alpha = state[1];
     int n_pos = (int)state[2];
-    if (dt <= 0.0) { dt = par[0]; alpha = par[5]; n_pos = 0; }
+    if (dt <= 0.0) { dt = fire[0]; alpha = fire[5]; n_pos = 0; }
     double E = 0.0;
     int rc = orc_energy_force(n, dim, pos, diam, box, kind, eps, sigma, r_cut, shift,
-                              NULL, NULL, 0, force, e_i, &E);
+                              NULL, NULL, 0, force, e_i, &E, par);
     if (rc) { free(e_i); return rc; }
     if (energies) energies[0] = E;
     for (int s = 0; s < nsteps; ++s) {
@@ -750,7 +773,7 @@ int orc_fire_run(int n, int dim, double *pos, double *vel, double *force, const 
                 pos[t] = wrap64(pos[t] + dt * vel[t], box[q]);
             }
         rc = orc_energy_force(n, dim, pos, diam, box, kind, eps, sigma, r_cut, shift,
-                              NULL, NULL, 0, force, e_i, &E);
+                              NULL, NULL, 0, force, e_i, &E, par);
         if (rc) break;
         double P = 0.0, FF = 0.0, VV = 0.0;
         for (int i = 0; i < n; ++i)
@@ -767,13 +790,13 @@ int orc_fire_run(int n, int dim, double *pos, double *vel, double *force, const 
                     vel[t] = (1.0 - alpha) * vel[t] + c2 * force[t];
                 }
             n_pos += 1;
-            if (n_pos > (int)par[2]) {
-                dt = dt * par[3] < par[1] ? dt * par[3] : par[1];
-                alpha = alpha * par[6];
+            if (n_pos > (int)fire[2]) {
+                dt = dt * fire[3] < fire[1] ? dt * fire[3] : fire[1];
+                alpha = alpha * fire[6];
             }
         } else {
             for (size_t t = 0; t < 3 * (size_t)n; ++t) vel[t] = 0.0;
-            n_pos = 0; dt = dt * par[4]; alpha = par[5];
+            n_pos = 0; dt = dt * fire[4]; alpha = fire[5];
         }
         if (energies) energies[s + 1] = E;
     }
@@ -823,13 +846,14 @@ void orc_normals(uint32_t seed, uint32_t step, int n, int dim, double *out /* n*
  */
 int orc_brownian_run(int n, int dim, double *pos, double *force, const double *diam, const double *box,
                      int kind, double eps, double sigma, double r_cut, int shift, double dt,
-                     double gamma, double kT, uint32_t seed, uint32_t step0, int nsteps, double *energies)
+                     double gamma, double kT, uint32_t seed, uint32_t step0, int nsteps, double *energies,
+                     const orc_params *par)
 {
     if (n <= 0 || (dim != 2 && dim != 3) || dt <= 0.0 || gamma <= 0.0 || kT < 0.0) return ORC_EINVAL;
     double *e_i = (double *)malloc((size_t)n * sizeof(double));
     if (!e_i) return ORC_ENOMEM;
     double E = 0.0;
-    int rc = orc_energy_force(n, dim, pos, diam, box, kind, eps, sigma, r_cut, shift, NULL, NULL, 0, force, e_i, &E);
+    int rc = orc_energy_force(n, dim, pos, diam, box, kind, eps, sigma, r_cut, shift, NULL, NULL, 0, force, e_i, &E, par);
     if (energies) energies[0] = E;
     const double mu = dt / gamma, amp = sqrt(2.0 * kT * dt / gamma);
     for (int s = 0; s < nsteps && !rc; ++s) {
@@ -842,7 +866,7 @@ int orc_brownian_run(int n, int dim, double *pos, double *force, const double *d
                 pos[t] = wrap64(pos[t] + mu * force[t] + amp * g[q], box[q]);
             }
         }
-        rc = orc_energy_force(n, dim, pos, diam, box, kind, eps, sigma, r_cut, shift, NULL, NULL, 0, force, e_i, &E);
+        rc = orc_energy_force(n, dim, pos, diam, box, kind, eps, sigma, r_cut, shift, NULL, NULL, 0, force, e_i, &E, par);
         if (energies) energies[s + 1] = E;
     }
     free(e_i);
@@ -863,7 +887,7 @@ int orc_brownian_run(int n, int dim, double *pos, double *force, const double *d
 int orc_langevin_run(int n, int dim, double *pos, double *vel, double *force, const double *diam,
                      const double *box, int kind, double eps, double sigma, double r_cut, int shift,
                      double dt, double mass, double gamma, double kT, uint32_t seed, uint32_t step0,
-                     int nsteps)
+                     int nsteps, const orc_params *par)
 {
     if (n <= 0 || (dim != 2 && dim != 3) || dt <= 0.0 || mass <= 0.0 || gamma < 0.0 || kT < 0.0) return ORC_EINVAL;
     double *e_i = (double *)malloc((size_t)n * sizeof(double));
@@ -885,7 +909,7 @@ int orc_langevin_run(int n, int dim, double *pos, double *vel, double *force, co
                 vel[t] = v;
             }
         }
-        rc = orc_energy_force(n, dim, pos, diam, box, kind, eps, sigma, r_cut, shift, NULL, NULL, 0, force, e_i, &E);
+        rc = orc_energy_force(n, dim, pos, diam, box, kind, eps, sigma, r_cut, shift, NULL, NULL, 0, force, e_i, &E, par);
         for (int i = 0; i < n; ++i)
             for (int q = 0; q < dim; ++q) {
                 size_t t = 3 * (size_t)i + q;
@@ -918,26 +942,6 @@ int orc_langevin_run(int n, int dim, double *pos, double *vel, double *force, co
  *   v_{j-1}, K2);  v_M += d/2 G_M
  * Conserved: H' = K + U + sum_j Q_j v_j^2 / 2 + dof kT xi_1 + kT sum_{j>=2} xi_j.
  * state = {xi_1..xi_M, v_1..v_M}. */
-#define ORC_MAX_NH_CHAIN 8
-static int g_nh_chain = 1;
-
-/* The parameters of kinds 2-5 and the chain length are process state set by the orc_set_* calls above.
- * orc_reset_params puts all of it into the UNSET state, in which a call that needs one of them fails with
- * ORC_EINVAL: the test suite calls it before every test, so no test can pass on what another one left. */
-void orc_reset_params(void)
-{
-    g_morse_alpha = NAN;
-    g_ns = 0;
-    g_bks_ns = 0;
-    g_nh_chain = 1;
-}
-int orc_set_nh_chain(int M)
-{
-    if (M < 1 || M > ORC_MAX_NH_CHAIN) return ORC_EINVAL;
-    g_nh_chain = M;
-    return ORC_OK;
-}
-
 static double nh_G(int j, int M, double K2, double dofkT, double kT, const double *Q, const double *v)
 {
     (void)M;
@@ -970,17 +974,18 @@ static void nh_half(int n, int dim, double *vel, double mass, double dofkT, doub
 int orc_nose_hoover_run(int n, int dim, double *pos, double *vel, double *force, const double *diam,
                         const double *box, int kind, double eps, double sigma, double r_cut, int shift,
                         double dt, double mass, double kT, double tau, double *state, int nsteps,
-                        double *conserved)
+                        double *conserved, const orc_params *par)
 {
-    if (n <= 0 || (dim != 2 && dim != 3) || dt <= 0.0 || mass <= 0.0 || kT <= 0.0 || tau <= 0.0 || !state)
+    if (n <= 0 || (dim != 2 && dim != 3) || dt <= 0.0 || mass <= 0.0 || kT <= 0.0 || tau <= 0.0 || !state || !par ||
+        par->nh_chain < 1 || par->nh_chain > ORC_MAX_NH_CHAIN)
         return ORC_EINVAL;
     double *e_i = (double *)malloc((size_t)n * sizeof(double));
     if (!e_i) return ORC_ENOMEM;
     const double dofkT = (double)dim * n * kT, a = dt / (2.0 * mass);
-    const int M = g_nh_chain;
+    const int M = par->nh_chain;
     double Q[ORC_MAX_NH_CHAIN], xi[ORC_MAX_NH_CHAIN], vxi[ORC_MAX_NH_CHAIN], E = 0.0;
     for (int j = 0; j < M; ++j) { Q[j] = (j == 0 ? dofkT : kT) * tau * tau; xi[j] = state[j]; vxi[j] = state[M + j]; }
-    int rc = orc_energy_force(n, dim, pos, diam, box, kind, eps, sigma, r_cut, shift, NULL, NULL, 0, force, e_i, &E);
+    int rc = orc_energy_force(n, dim, pos, diam, box, kind, eps, sigma, r_cut, shift, NULL, NULL, 0, force, e_i, &E, par);
     for (int s = 0; s <= nsteps && !rc; ++s) {
         if (conserved) {
             double K2 = 0.0;
@@ -998,7 +1003,7 @@ int orc_nose_hoover_run(int n, int dim, double *pos, double *vel, double *force,
                 vel[t] += a * force[t];
                 pos[t] = wrap64(pos[t] + dt * vel[t], box[q]);
             }
-        rc = orc_energy_force(n, dim, pos, diam, box, kind, eps, sigma, r_cut, shift, NULL, NULL, 0, force, e_i, &E);
+        rc = orc_energy_force(n, dim, pos, diam, box, kind, eps, sigma, r_cut, shift, NULL, NULL, 0, force, e_i, &E, par);
         for (int i = 0; i < n; ++i)
             for (int q = 0; q < dim; ++q) vel[3 * (size_t)i + q] += a * force[3 * (size_t)i + q];
         nh_half(n, dim, vel, mass, dofkT, kT, Q, M, dt, xi, vxi);

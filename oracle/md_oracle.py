@@ -111,38 +111,77 @@ def predicate_band(pos, box, dim, r_cut, skin, method=1):
     return int(nd.value), float(band.value), float(close.value)
 
 
+class Params(C.Structure):
+    """orc_params of md_oracle.c: the parameters of kinds 2-5 and the Nose-Hoover chain length.  They travel
+    with every call; the C library keeps no state.  A fresh object is in the UNSET state (alpha = NaN, no
+    species tables), in which a call that needs one of them fails."""
+    _fields_ = [("morse_alpha", C.c_double), ("ns", C.c_int32), ("bks_ns", C.c_int32), ("nh_chain", C.c_int32),
+                ("pad_", C.c_int32), ("sp_eps", C.c_double * 16), ("sp_sig", C.c_double * 16),
+                ("sp_rc", C.c_double * 16), ("bks_A", C.c_double * 16), ("bks_B", C.c_double * 16),
+                ("bks_C", C.c_double * 16), ("bks_q", C.c_double * 4), ("bks_a", C.c_double), ("bks_k", C.c_double)]
+
+    def __init__(self):
+        super().__init__()
+        assert C.sizeof(Params) == lib().orc_params_size()
+        self.reset()
+
+    def reset(self):
+        lib().orc_params_reset(C.byref(self))
+
+    def species_lj(self, eps, sigma, rc):
+        e = _d(eps); sg = _d(sigma); r = _d(rc)
+        _check(lib().orc_params_species_lj(C.byref(self), e.shape[0], _pd(e.reshape(-1).copy()),
+                                           _pd(sg.reshape(-1).copy()), _pd(r.reshape(-1).copy())), "species_lj")
+
+    def species_bks(self, A, B, Cc, q, coulomb_alpha, k_e=1.0):
+        A = _d(A); B = _d(B); Cc = _d(Cc); q = _d(q)
+        ns = q.shape[0]
+        assert A.shape == (ns, ns) and B.shape == (ns, ns) and Cc.shape == (ns, ns)
+        _check(lib().orc_params_species_bks(C.byref(self), ns, _pd(A), _pd(B), _pd(Cc), _pd(q),
+                                            C.c_double(coulomb_alpha), C.c_double(k_e)), "species_bks")
+
+
+_DEFAULT = None
+
+
+def default_params() -> Params:
+    """The Params object the functions below pass when the caller gives none (`params=None`); the set_*
+    functions write into it.  tests/conftest.py resets it before every test."""
+    global _DEFAULT
+    if _DEFAULT is None:
+        _DEFAULT = Params()
+    return _DEFAULT
+
+
+def _par(params):
+    return C.byref(default_params() if params is None else params)
+
+
 def set_species_lj(eps, sigma, rc) -> None:
     """Tables of kind 4 (species x species LJ): square arrays eps_ab, sigma_ab, rc_ab."""
-    e = _d(eps); sg = _d(sigma); r = _d(rc)
-    ns = e.shape[0]
-    _check(lib().orc_set_species_lj(ns, _pd(e.reshape(-1).copy()), _pd(sg.reshape(-1).copy()),
-                                    _pd(r.reshape(-1).copy())), "set_species_lj")
+    default_params().species_lj(eps, sigma, rc)
 
 
 def set_species_bks(A, B, Cc, q, coulomb_alpha, k_e=1.0):
     """Tables of kind 5 (BKS-type): square arrays A_ab, B_ab, C_ab, charges q_a, DSF damping, Coulomb constant."""
-    A = _d(A); B = _d(B); Cc = _d(Cc); q = _d(q)
-    ns = q.shape[0]
-    assert A.shape == (ns, ns) and B.shape == (ns, ns) and Cc.shape == (ns, ns)
-    _check(lib().orc_set_species_bks(ns, _pd(A), _pd(B), _pd(Cc), _pd(q), C.c_double(coulomb_alpha),
-                                     C.c_double(k_e)), "set_species_bks")
+    default_params().species_bks(A, B, Cc, q, coulomb_alpha, k_e)
 
 
 def reset_params() -> None:
-    """Forget every orc_set_* parameter (Morse / Buckingham alpha, species tables, chain length): a later
-    call that needs one fails until it is set again.  tests/conftest.py does this before every test."""
-    lib().orc_reset_params()
+    """Put the default Params back into the unset state (Morse / Buckingham alpha, species tables, chain length):
+    a later call that needs one fails until it is set again.  tests/conftest.py does this before every test."""
+    default_params().reset()
 
 
 def set_morse_alpha(alpha: float) -> None:
-    """alpha of kind 2 (Morse) for the following energy_force / nve_run calls."""
-    lib().orc_set_morse_alpha(C.c_double(alpha))
+    """alpha of kind 2 (Morse) / B of kind 3 for the following calls that pass the default Params."""
+    default_params().morse_alpha = float(alpha)
 
 
 def energy_force(pos, diam, box, dim, kind, eps, sigma, r_cut, shift,
-                 nbr_idx=None, nbr_count=None, alpha=None):
+                 nbr_idx=None, nbr_count=None, alpha=None, params=None):
     if alpha is not None:
-        set_morse_alpha(alpha)
+        (default_params() if params is None else params).morse_alpha = float(alpha)
     p = _d(pos3(pos)); b = _d(box)
     n = p.shape[0]
     dm = _d(diam) if diam is not None else None
@@ -156,7 +195,7 @@ def energy_force(pos, diam, box, dim, kind, eps, sigma, r_cut, shift,
         cap = nbr_idx.shape[1]
     _check(lib().orc_energy_force(n, dim, _pd(p), _pd(dm), _pd(b), kind, C.c_double(eps),
                                   C.c_double(sigma), C.c_double(r_cut), shift, _pi(nbr_idx),
-                                  _pi(nbr_count), cap, _pd(f), _pd(e_i), C.byref(E)),
+                                  _pi(nbr_count), cap, _pd(f), _pd(e_i), C.byref(E), _par(params)),
            "energy_force")
     return f, e_i, float(E.value)
 
@@ -170,10 +209,10 @@ def needs_rebuild(pos, ref, box, dim, skin):
 
 
 def nve_run(pos, vel, force, diam, box, dim, kind, eps, sigma, r_cut, shift, dt, mass,
-            nsteps, use_list=0, skin=0.0, capacity=128, want_energies=True, alpha=None):
+            nsteps, use_list=0, skin=0.0, capacity=128, want_energies=True, alpha=None, params=None):
     """Returns (pos, vel, force, energies[(nsteps+1),2] or None, stats[3])."""
     if alpha is not None:
-        set_morse_alpha(alpha)
+        (default_params() if params is None else params).morse_alpha = float(alpha)
     p = _d(pos3(pos)).copy(); v = _d(pos3(vel)).copy(); f = _d(pos3(force)).copy()
     b = _d(box)
     dm = _d(diam) if diam is not None else None
@@ -182,7 +221,7 @@ def nve_run(pos, vel, force, diam, box, dim, kind, eps, sigma, r_cut, shift, dt,
     _check(lib().orc_nve_run(p.shape[0], dim, _pd(p), _pd(v), _pd(f), _pd(dm), _pd(b), kind,
                              C.c_double(eps), C.c_double(sigma), C.c_double(r_cut), shift,
                              C.c_double(dt), C.c_double(mass), nsteps, use_list,
-                             C.c_float(skin), capacity, _pd(en), _pi(stats)), "nve_run")
+                             C.c_float(skin), capacity, _pd(en), _pi(stats), _par(params)), "nve_run")
     return p, v, f, en, stats
 
 
@@ -190,10 +229,10 @@ FIRE_DEFAULT = (0.01, 0.1, 5, 1.1, 0.5, 0.1, 0.99)   # dt_start, dt_max, n_min, 
 
 
 def fire_run(pos, vel, diam, box, dim, kind, eps, sigma, r_cut, shift, nsteps, par=FIRE_DEFAULT,
-             state=None, alpha_morse=None):
+             state=None, alpha_morse=None, params=None):
     """Returns (pos, vel, force, energies[nsteps+1], state[3] = (dt, alpha, n_pos))."""
     if alpha_morse is not None:
-        set_morse_alpha(alpha_morse)
+        (default_params() if params is None else params).morse_alpha = float(alpha_morse)
     p = _d(pos3(pos)).copy(); v = _d(pos3(vel)).copy(); f = np.zeros_like(p)
     b = _d(box)
     dm = _d(diam) if diam is not None else None
@@ -203,7 +242,7 @@ def fire_run(pos, vel, diam, box, dim, kind, eps, sigma, r_cut, shift, nsteps, p
     en = np.zeros(nsteps + 1, dtype=np.float64)
     _check(lib().orc_fire_run(p.shape[0], dim, _pd(p), _pd(v), _pd(f), _pd(dm), _pd(b), kind,
                               C.c_double(eps), C.c_double(sigma), C.c_double(r_cut), shift,
-                              _pd(pr), _pd(st), nsteps, _pd(en)), "fire_run")
+                              _pd(pr), _pd(st), nsteps, _pd(en), _par(params)), "fire_run")
     return p, v, f, en, st
 
 
@@ -215,10 +254,10 @@ def normals(seed, step, n, dim):
 
 
 def brownian_run(pos, diam, box, dim, kind, eps, sigma, r_cut, shift, dt, gamma, kT, seed, nsteps,
-                 step0=0, alpha_morse=None):
+                 step0=0, alpha_morse=None, params=None):
     """Returns (pos, force, energies[nsteps+1])."""
     if alpha_morse is not None:
-        set_morse_alpha(alpha_morse)
+        (default_params() if params is None else params).morse_alpha = float(alpha_morse)
     p = _d(pos3(pos)).copy(); f = np.zeros_like(p)
     b = _d(box)
     dm = _d(diam) if diam is not None else None
@@ -226,12 +265,12 @@ def brownian_run(pos, diam, box, dim, kind, eps, sigma, r_cut, shift, dt, gamma,
     _check(lib().orc_brownian_run(p.shape[0], dim, _pd(p), _pd(f), _pd(dm), _pd(b), kind, C.c_double(eps),
                                   C.c_double(sigma), C.c_double(r_cut), shift, C.c_double(dt),
                                   C.c_double(gamma), C.c_double(kT), C.c_uint32(seed), C.c_uint32(step0),
-                                  nsteps, _pd(en)), "brownian_run")
+                                  nsteps, _pd(en), _par(params)), "brownian_run")
     return p, f, en
 
 
 def langevin_run(pos, vel, force, diam, box, dim, kind, eps, sigma, r_cut, shift, dt, mass, gamma, kT,
-                 seed, nsteps, step0=0):
+                 seed, nsteps, step0=0, params=None):
     """BAOAB Langevin; returns (pos, vel, force)."""
     p = _d(pos3(pos)).copy(); v = _d(pos3(vel)).copy(); f = _d(pos3(force)).copy()
     b = _d(box)
@@ -239,12 +278,12 @@ def langevin_run(pos, vel, force, diam, box, dim, kind, eps, sigma, r_cut, shift
     _check(lib().orc_langevin_run(p.shape[0], dim, _pd(p), _pd(v), _pd(f), _pd(dm), _pd(b), kind,
                                   C.c_double(eps), C.c_double(sigma), C.c_double(r_cut), shift,
                                   C.c_double(dt), C.c_double(mass), C.c_double(gamma), C.c_double(kT),
-                                  C.c_uint32(seed), C.c_uint32(step0), nsteps), "langevin_run")
+                                  C.c_uint32(seed), C.c_uint32(step0), nsteps, _par(params)), "langevin_run")
     return p, v, f
 
 
 def nose_hoover_run(pos, vel, diam, box, dim, kind, eps, sigma, r_cut, shift, dt, mass, kT, tau, nsteps,
-                    state=None, chain=1):
+                    state=None, chain=1, params=None):
     """Returns (pos, vel, force, conserved[nsteps+1], state[2*chain] = (xi_1.., v_xi_1..))."""
     p = _d(pos3(pos)).copy(); v = _d(pos3(vel)).copy(); f = np.zeros_like(p)
     b = _d(box)
@@ -252,11 +291,11 @@ def nose_hoover_run(pos, vel, diam, box, dim, kind, eps, sigma, r_cut, shift, dt
     st = (_d(state) if state is not None else np.zeros(2 * chain, dtype=np.float64)).copy()
     assert st.shape == (2 * chain,)
     cons = np.zeros(nsteps + 1, dtype=np.float64)
-    _check(lib().orc_set_nh_chain(int(chain)), "set_nh_chain")
+    (default_params() if params is None else params).nh_chain = int(chain)
     _check(lib().orc_nose_hoover_run(p.shape[0], dim, _pd(p), _pd(v), _pd(f), _pd(dm), _pd(b), kind,
                                      C.c_double(eps), C.c_double(sigma), C.c_double(r_cut), shift,
                                      C.c_double(dt), C.c_double(mass), C.c_double(kT), C.c_double(tau),
-                                     _pd(st), nsteps, _pd(cons)), "nose_hoover_run")
+                                     _pd(st), nsteps, _pd(cons), _par(params)), "nose_hoover_run")
     return p, v, f, cons, st
 
 

@@ -22,8 +22,9 @@ def orc():
 
 @pytest.fixture(autouse=True)
 def _oracle_parameters_do_not_leak():
-    """The oracle keeps the parameters of kinds 2-5 (and the thermostat chain length) as process state:
-    every test starts from the UNSET state, so none can pass on what another left behind."""
+    """The oracle's C library takes the parameters of kinds 2-5 (and the thermostat chain length) as a call
+    argument; its Python wrapper passes a default Params object that the set_* functions fill.  Every test
+    starts with that object in the UNSET state, so none can pass on what another left behind."""
     from oracle import md_oracle
     if os.path.exists(md_oracle._LIB):
         md_oracle.reset_params()
