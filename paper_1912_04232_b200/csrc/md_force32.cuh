@@ -224,7 +224,13 @@ __device__ __forceinline__ void lj_rows32(const Geom &g, const Pair32 &p32,
                                           bool active, Acc32 &acc) {
     // an idle lane of a ragged last tile owns no column: it loads no index (its column may hold
     // anything) and gathers its stand-in particle ii
-    const int kload = active ? kmax : 0;
+    // List rows are prefetched one iteration ahead with ONE warp-uniform guard: capacity is a multiple of 4
+    // (md_create) and so is k, hence rows k + U .. k + 2U - 1 exist whenever k + 2U <= capacity, and when they do
+    // not the loop is over.  What a row holds beyond a lane's count is never used as an index (the tail selects).
+    // A lane without a particle reads lane 0's column of the tile (valid entries of a valid particle) instead of
+    // its own, which nobody wrote.
+    static_assert(F32_U == 2 || F32_U == 4, "the row prefetch relies on capacity % F32_U == 0");
+    const int *cs = active ? col : col - (threadIdx.x & 31);
     const float Lx = g.L[0], Ly = g.L[1], Lz = g.L[2];
     const float hx = g.h[0], hy = g.h[1], hz = g.h[2];
     const float pxL = pi.x - Lx, pyL = pi.y - Ly, pzL = pi.z - Lz;
@@ -246,15 +252,17 @@ __device__ __forceinline__ void lj_rows32(const Geom &g, const Pair32 &p32,
     int k = 0;
     int jn[F32_U];
 #pragma unroll
-    for (int u = 0; u < F32_U; ++u) jn[u] = u < kload ? col[u * TILE] : ii;
+    for (int u = 0; u < F32_U; ++u) jn[u] = kmax > 0 ? cs[u * TILE] : ii;
     for (; k < kmin; k += F32_U) {
         int j[F32_U]; float4 q[F32_U];
 #pragma unroll
         for (int u = 0; u < F32_U; ++u) j[u] = jn[u];
 #pragma unroll
         for (int u = 0; u < F32_U; ++u) { MD_CHECK(j[u] >= 0 && j[u] < g.ntot); q[u] = pos[j[u]]; }
+        if (k + 2 * F32_U <= g.capacity) {
 #pragma unroll
-        for (int u = 0; u < F32_U; ++u) jn[u] = k + F32_U + u < kload ? col[(k + F32_U + u) * TILE] : ii;
+            for (int u = 0; u < F32_U; ++u) jn[u] = cs[(k + F32_U + u) * TILE];
+        }
 #pragma unroll
         for (int u = 0; u < F32_U; u += 2) two(q[u], q[u + 1]);
     }
@@ -266,8 +274,10 @@ __device__ __forceinline__ void lj_rows32(const Geom &g, const Pair32 &p32,
         for (int u = 0; u < F32_U; ++u) j[u] = k + u < cnt ? jn[u] : ii;
 #pragma unroll
         for (int u = 0; u < F32_U; ++u) { MD_CHECK(j[u] >= 0 && j[u] < g.ntot); q[u] = pos[j[u]]; }
+        if (k + 2 * F32_U <= g.capacity) {
 #pragma unroll
-        for (int u = 0; u < F32_U; ++u) jn[u] = k + F32_U + u < kload ? col[(k + F32_U + u) * TILE] : ii;
+            for (int u = 0; u < F32_U; ++u) jn[u] = cs[(k + F32_U + u) * TILE];
+        }
 #pragma unroll
         for (int u = 0; u < F32_U; ++u) if (!(k + u < cnt)) q[u].x = 1e18f;
 #pragma unroll
