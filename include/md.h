@@ -316,6 +316,30 @@ int md_cell_list_build(md_system *sys, void *pos, void *vel, int32_t *id,
                        int32_t *cell_start, int32_t *perm, void *stream);
 
 /*
+ * The same cell list (L84; md_cell_list_build with resort = 0 and id = NULL) through an entry point that
+ * allocates NOTHING and needs neither a md_system nor a workspace: for callers that cannot call cudaMalloc
+ * (code under CUDA graph capture, tight serving loops, harnesses that forbid it).  The counting sort's
+ * scratch (cell of every particle, arrival rank, unsorted slots, histogram) lives in a static __device__ array
+ * inside the library image: 832 KB that every GPU which loads the library holds until the process exits.
+ * That fixes the LIMIT: n <= MD_STATIC_MAX_N particles and at most MD_STATIC_MAX_CELLS cells (the cells of
+ * cfg: floor(L_k / (r_cut + skin)) per side); beyond either the call returns MD_EINVAL and launches nothing.
+ *   cfg        the geometry, as for md_create (capacity and resort are checked but not used)
+ *   pos        DEVICE float4[n] in: coordinates in [0, L); untouched
+ *   cell_start DEVICE int32[cells + 1] out;  perm DEVICE int32[n] out: as md_cell_list_build
+ *   pos_sorted DEVICE float4[n] out: pos_sorted[s] = pos[perm[s]] (must not alias pos)
+ * The device is the one `pos` lives on.  The call makes no cudaMalloc / cudaFree and calls no allocating
+ * library routine; on its first use per device it resolves the array's address (cudaGetSymbolAddress), which
+ * a caller that captures graphs should let happen once before capturing.  Every call on a device shares the
+ * one array, and the array keeps the last call's contents (the call clears the part that must start at zero):
+ * two calls whose kernels OVERLAP on the GPU (different streams without an ordering between them) race.
+ * Calls on one stream, or ordered by events, are safe.  Errors: MD_EINVAL, MD_EBOX, MD_ECUDA.
+ */
+#define MD_STATIC_MAX_N     65536
+#define MD_STATIC_MAX_CELLS 16384
+int md_cell_list_static(const md_config *cfg, int n, const void *pos, int32_t *cell_start, int32_t *perm,
+                        void *pos_sorted, void *stream);
+
+/*
  * Neighbor list (L84-L88 partition.neighbor_list; dense N x capacity rows, L74): for every
  * i all j != i in the 3^dim adjacent cells with r2 < R^2 under the canonical fp32 predicate
  * (nearest-image displacement with the box side subtracted from the larger

@@ -20,7 +20,7 @@ MD_KIND_LJ, MD_KIND_SOFT, MD_KIND_MORSE, MD_KIND_BUCKINGHAM, MD_KIND_LJ_SPECIES,
 SYMBOLS = [
     "md_last_error", "md_workspace_bytes", "md_create", "md_destroy", "md_set_option",
     "md_num_cells", "md_nbr_layout", "md_cell_list_build", "md_neighbor_list_build",
-    "md_needs_rebuild", "md_pair_energy_force", "md_nve_step", "md_nve_run_host", "md_counters",
+    "md_cell_list_static", "md_needs_rebuild", "md_pair_energy_force", "md_nve_step", "md_nve_run_host", "md_counters",
     "md_nve_run_host_release", "md_fire_minimize", "md_brownian_step",
     "md_langevin_step", "md_nose_hoover_step", "md_set_species_lj",
     "md_flock_step", "md_flock_obstacles", "md_set_species_bks", "md_flock_predators",
@@ -126,6 +126,7 @@ def lib():
         L.md_num_cells.argtypes = [vp, C.POINTER(C.c_int * 3)]
         L.md_nbr_layout.argtypes = [vp] + [C.POINTER(C.c_long)] * 5
         L.md_cell_list_build.argtypes = [vp, vp, vp, ip, ip, ip, vp]
+        L.md_cell_list_static.argtypes = [C.POINTER(md_config), C.c_int, vp, ip, ip, vp, vp]
         L.md_neighbor_list_build.argtypes = [vp, vp, ip, ip, ip, ip, ip, vp]
         L.md_needs_rebuild.argtypes = [vp, vp, ip, vp]
         L.md_pair_energy_force.argtypes = [vp, C.POINTER(md_potential), vp, ip, ip, vp, vp, vp]
@@ -394,6 +395,15 @@ def nbr_offsets(layout, n, capacity, device=None):
 def md_cell_list_build(sys, pos, vel, id, cell_start, perm, stream=None) -> None:
     _check(lib().md_cell_list_build(sys, _ptr(pos), _ptr(vel), _ptr(id), _ptr(cell_start), _ptr(perm),
                                     _stream(stream)))
+
+
+MD_STATIC_MAX_N, MD_STATIC_MAX_CELLS = 65536, 16384      # md.h
+
+
+def md_cell_list_static(cfg: md_config, n, pos, cell_start, perm, pos_sorted, stream=None) -> None:
+    """The cell list without a md_system, a workspace or any allocation (md.h): scratch is static in the library."""
+    _check(lib().md_cell_list_static(C.byref(cfg), int(n), _ptr(pos), _ptr(cell_start), _ptr(perm),
+                                     _ptr(pos_sorted), _stream(stream)))
 
 
 def md_neighbor_list_build(sys, pos, cell_start, perm, nbr_idx, nbr_count, status, stream=None) -> None:

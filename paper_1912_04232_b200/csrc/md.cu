@@ -20,6 +20,13 @@
 
 using namespace mdk;
 
+// Scratch of md_cell_list_static: part of the library image, so every GPU that loads the library holds these
+// 832 KB until the process exits.  Layout in ints: cell_of[MAX_N] | rank[MAX_N] | perm_tmp[MAX_N] |
+// cell_count[MAX_CELLS].  In HOST code this name is a host-side stand-in, not a device address: the address
+// the kernels get comes from cudaGetSymbolAddress (static_scratch_address below), once per device.
+static __device__ __align__(256) int g_cell_static_scratch[3 * MD_STATIC_MAX_N + MD_STATIC_MAX_CELLS];
+static_assert(MD_STATIC_MAX_CELLS <= SCAN_ONE_BLOCK, "md_cell_list_static scans its cells with the one-block kernel");
+
 namespace {
 
 thread_local char g_err[512] = "";
@@ -154,6 +161,24 @@ struct DeviceScope {
 };
 static_assert(sizeof(md_potential) == 24 && sizeof(md_fire_params) == 28 && sizeof(md_flock_params) == 32 &&
               sizeof(md_predator_params) == 20, "graph keys are compared bytewise: these structs hold no padding");
+
+// Device address of g_cell_static_scratch on `device`, resolved once per device with that device current
+// (the caller holds a DeviceScope on it).
+constexpr int STATIC_MAX_DEVICES = 64;
+std::mutex g_static_mu;
+int *g_static_addr[STATIC_MAX_DEVICES];
+int static_scratch_address(int device, int **out) {
+    if (device < 0 || device >= STATIC_MAX_DEVICES) return fail(MD_EINVAL, "device ordinal %d out of range", device);
+    std::lock_guard<std::mutex> lock(g_static_mu);
+    if (!g_static_addr[device]) {
+        void *p = nullptr;
+        CU(cudaGetSymbolAddress(&p, g_cell_static_scratch));
+        if (!p) return fail(MD_ECUDA, "cudaGetSymbolAddress returned a null address on device %d", device);
+        g_static_addr[device] = static_cast<int *>(p);
+    }
+    *out = g_static_addr[device];
+    return MD_OK;
+}
 
 struct Layout {
     size_t words, scan_tmp, fire_tmp, pred_tmp, cell_count, cell_start_i, perm_i, cell_of, rank_tmp, perm_tmp, id_s, pos_s,
@@ -1251,6 +1276,50 @@ int md_cell_list_build(md_system *sys, void *pos, void *vel, int32_t *id, int32_
     if (scope_.rc) return scope_.rc;
     return launch_cell_build(sys, (float4 *)pos, (float4 *)vel, id, cell_start, perm, nullptr,
                              nullptr, (cudaStream_t)stream);
+}
+
+int md_cell_list_static(const md_config *cfg, int n, const void *pos, int32_t *cell_start, int32_t *perm,
+                        void *pos_sorted, void *stream) {
+    if (!cfg || !pos || !cell_start || !perm || !pos_sorted) return fail(MD_EINVAL, "NULL argument");
+    // sizes first, before any CUDA call
+    if (n > MD_STATIC_MAX_N)
+        return fail(MD_EINVAL, "md_cell_list_static: n = %d exceeds MD_STATIC_MAX_N = %d (the static scratch holds no more; "
+                               "use md_create + md_cell_list_build with a workspace of your own)", n, MD_STATIC_MAX_N);
+    Geom g;
+    int rc = make_geom(cfg, n, &g);                      // host arithmetic only
+    if (rc) return rc;
+    if (g.cells > MD_STATIC_MAX_CELLS)
+        return fail(MD_EINVAL, "md_cell_list_static: %d cells exceed MD_STATIC_MAX_CELLS = %d (the static scratch holds no more; "
+                               "use md_create + md_cell_list_build with a workspace of your own)", g.cells, MD_STATIC_MAX_CELLS);
+    if (!aligned16(pos) || !aligned16(pos_sorted)) return fail(MD_EINVAL, "pos/pos_sorted must be 16-byte aligned");
+    if (pos == pos_sorted) return fail(MD_EINVAL, "pos_sorted must not alias pos");
+    cudaPointerAttributes attr;
+    CU(cudaPointerGetAttributes(&attr, pos));
+    if (attr.type != cudaMemoryTypeDevice && attr.type != cudaMemoryTypeManaged)
+        return fail(MD_EINVAL, "pos is not device memory");
+    DeviceScope scope_(attr.device);
+    if (scope_.rc) return scope_.rc;
+    int *scr = nullptr;
+    rc = static_scratch_address(attr.device, &scr);
+    if (rc) return rc;
+    int *cell_of = scr, *rank_tmp = scr + MD_STATIC_MAX_N, *perm_tmp = scr + 2 * MD_STATIC_MAX_N;
+    int *cell_count = scr + 3 * MD_STATIC_MAX_N;
+    cudaStream_t st = (cudaStream_t)stream;
+    // the array keeps what the last call (perhaps of another geometry, perhaps aborted) left: the histogram
+    // must start at zero; cell_of, rank and perm_tmp are written for every i < n before they are read
+    CU(cudaMemsetAsync(cell_count, 0, (size_t)g.cells * sizeof(int), st));
+    const int nb = blocks_for(n);
+    const float4 *p4 = (const float4 *)pos;
+    k_cell_assign<<<nb, 256, 0, st>>>(g, p4, cell_of, rank_tmp, cell_count, nullptr);
+    LAUNCH_OK();
+    k_cell_scan<<<1, 1024, 0, st>>>(g.cells, cell_count, cell_start, nullptr, nullptr);
+    LAUNCH_OK();
+    k_cell_scatter<<<nb, 256, 0, st>>>(n, cell_of, rank_tmp, cell_start, perm_tmp, nullptr);
+    LAUNCH_OK();
+    k_cell_order_gather<<<nb, 256, 0, st>>>(n, cell_of, cell_start, perm_tmp, nullptr, p4, nullptr, perm,
+                                            (float4 *)pos_sorted, nullptr, nullptr, nullptr);
+    LAUNCH_OK();
+    return MD_OK;
 }
 
 int md_neighbor_list_build(md_system *sys, const void *pos, const int32_t *cell_start,
