@@ -707,6 +707,13 @@ def main():
                                 "nve_particle_steps_per_s": value,
                                 "what": "cell list + re-sort + neighbor list through the API (cold L2) / the loop's force kernel "
                                         "per launch (cold L2) / the whole loop incl. rebuilds"}
+        # the rebuild (cell list with re-sort + neighbor list) on its own algorithmic bytes, (4K + 116) N
+        rebuild_bytes = (4.0 * kbar + 116.0) * w.n
+        rb_achieved = rebuild_bytes / (build_ms * 1e-3) / 1e9
+        out["roofline_rebuild"] = {"bound": "alu (instruction issue; profiles/r2_profiles.md), reported against hbm",
+                                   "kernels": "k_cell_assign, k_cell_scan, k_cell_scatter, k_cell_order_gather, k_copy_back, k_nbr_build2",
+                                   "achieved": rb_achieved, "peak": peak, "unit": "GB/s", "frac": rb_achieved / peak,
+                                   "algorithmic_bytes": rebuild_bytes, "ms_per_rebuild_cold_l2": build_ms}
     if survey is not None:
         out["survey_timing"] = survey
     if e2e is not None:

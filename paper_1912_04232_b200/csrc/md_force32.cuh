@@ -224,9 +224,9 @@ __device__ __forceinline__ void lj_rows32(const Geom &g, const Pair32 &p32,
                                           bool active, Acc32 &acc) {
     // an idle lane of a ragged last tile owns no column: it loads no index (its column may hold
     // anything) and gathers its stand-in particle ii
-    // List rows are prefetched one iteration ahead with ONE warp-uniform guard: capacity is a multiple of 4
-    // (md_create) and so is k, hence rows k + U .. k + 2U - 1 exist whenever k + 2U <= capacity, and when they do
-    // not the loop is over.  What a row holds beyond a lane's count is never used as an index (the tail selects).
+    // List rows are prefetched one iteration ahead with ONE warp-uniform guard, k + U < kmax: some lane then
+    // needs row k + U, and since capacity is a multiple of 4 (md_create) and so is k, rows k + U .. k + 2U - 1
+    // all exist.  What a row holds beyond a lane's count is never used as an index (the tail selects).
     // A lane without a particle reads lane 0's column of the tile (valid entries of a valid particle) instead of
     // its own, which nobody wrote.
     static_assert(F32_U == 2 || F32_U == 4, "the row prefetch relies on capacity % F32_U == 0");
@@ -259,7 +259,7 @@ __device__ __forceinline__ void lj_rows32(const Geom &g, const Pair32 &p32,
         for (int u = 0; u < F32_U; ++u) j[u] = jn[u];
 #pragma unroll
         for (int u = 0; u < F32_U; ++u) { MD_CHECK(j[u] >= 0 && j[u] < g.ntot); q[u] = pos[j[u]]; }
-        if (k + 2 * F32_U <= g.capacity) {
+        if (k + F32_U < kmax) {
 #pragma unroll
             for (int u = 0; u < F32_U; ++u) jn[u] = cs[(k + F32_U + u) * TILE];
         }
@@ -274,7 +274,7 @@ __device__ __forceinline__ void lj_rows32(const Geom &g, const Pair32 &p32,
         for (int u = 0; u < F32_U; ++u) j[u] = k + u < cnt ? jn[u] : ii;
 #pragma unroll
         for (int u = 0; u < F32_U; ++u) { MD_CHECK(j[u] >= 0 && j[u] < g.ntot); q[u] = pos[j[u]]; }
-        if (k + 2 * F32_U <= g.capacity) {
+        if (k + F32_U < kmax) {
 #pragma unroll
             for (int u = 0; u < F32_U; ++u) jn[u] = cs[(k + F32_U + u) * TILE];
         }
