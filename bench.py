@@ -667,6 +667,7 @@ def main():
     peak, peak_src = peaks()
     traffic, traffic_src = measured_traffic(args.config)
     fused = (w.kind == W.KIND_LJ and w.dim == 3)      # the configs md_nve_step runs as fused graphs
+    flagged = B.md_get_option(S.sys, "rebuild_flagged") != 0.0
     algo_bytes = (4.0 * kbar + 68.0) * w.n          # list + count + pos + vel read, force + vel written
     achieved = algo_bytes / (force_ms_cold * 1e-3) / 1e9
     step_bytes = (4.0 * kbar + 164.0) * w.n
@@ -695,9 +696,12 @@ def main():
                      "launch_ms_cold_l2": force_ms_cold, "launch_ms_warm_l2": force_ms_warm},
         # per bench step: k_init_stats + one force kernel per MD step + one k_kick_drift per graph
         # launch (graphs of 9 fused steps, then single steps; unfused configs: one per MD step)
-        # + 6 kernels (4 cell list, copy back, neighbor list) per rebuild an IF node ran
+        # + the rebuild: two flagged launches (cooperative cell list, builder) in EVERY MD step, or
+        # 6 kernels (4 cell list, copy back, neighbor list) per rebuild an IF node ran
         "gpu_launches": args.steps * (1 + md_steps + (md_steps // 9 + md_steps % 9 if fused else md_steps))
-                        + 6 * rebuilds,
+                        + (2 * args.steps * md_steps if flagged else 6 * rebuilds),
+        "rebuild_in_graph": "two launches per MD step that return at once while the step's flag is 0" if flagged
+                            else "IF node around the rebuild's six kernels",
     }
     if build_ms is not None:
         out["build_ms_per_rebuild"] = build_ms

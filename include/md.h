@@ -121,8 +121,18 @@ int md_destroy(md_system *sys);
  *   "use_graph"            0: the step calls launch their kernels directly instead of CUDA graphs -- the same
  *                          kernels in the same order (so a profiler lists them one by one); the rebuild kernels
  *                          are then launched every step and return at once while the step's device flag is 0
+ *   "rebuild_flagged"      how the step loops (md_nve_step and the other rules) run the rebuild inside their CUDA
+ *                          graphs.  1: two launches, the cooperative cell list and the neighbor-list builder, that
+ *                          are part of every step and return at once while the step's device flag is 0 (2.7 us
+ *                          each on B200); 0: the rebuild's kernels inside an IF node, which costs 9 us per step
+ *                          whether or not it fires; -1 (default): 1 up to 600,000 particles (beyond that the
+ *                          cooperative cell list loses more per rebuild than the IF node costs).  Same results.
  *   "nh_chain"             thermostats in md_nose_hoover_step's chain, 1 (default) .. 8 */
 int md_set_option(md_system *sys, const char *name, double value);
+
+/* The value in effect: "rebuild_flagged" (1 or 0: what the step loops will do), "est_thr", "fast32",
+ * "use_graph", "threads_per_particle".  Errors: MD_EINVAL (NULL, unknown name). */
+int md_get_option(md_system *sys, const char *name, double *value);
 
 /* Species x species Lennard-Jones tables (L104 pair potentials with per-species parameters; the
  * sigma matrix of L298-L305): host float[nspecies * nspecies], row-major, 1 <= nspecies <= 4, every

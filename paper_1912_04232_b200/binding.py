@@ -20,7 +20,7 @@ MD_KIND_LJ, MD_KIND_SOFT, MD_KIND_MORSE, MD_KIND_BUCKINGHAM, MD_KIND_LJ_SPECIES,
 SYMBOLS = [
     "md_last_error", "md_workspace_bytes", "md_create", "md_destroy", "md_set_option",
     "md_num_cells", "md_nbr_layout", "md_cell_list_build", "md_neighbor_list_build",
-    "md_cell_list_static", "md_needs_rebuild", "md_pair_energy_force", "md_nve_step", "md_nve_run_host", "md_counters",
+    "md_cell_list_static", "md_get_option", "md_needs_rebuild", "md_pair_energy_force", "md_nve_step", "md_nve_run_host", "md_counters",
     "md_nve_run_host_release", "md_fire_minimize", "md_brownian_step",
     "md_langevin_step", "md_nose_hoover_step", "md_set_species_lj",
     "md_flock_step", "md_flock_obstacles", "md_set_species_bks", "md_flock_predators",
@@ -88,6 +88,7 @@ def lib():
         L.md_create.argtypes = [C.POINTER(md_config), C.c_int, vp, C.c_size_t, C.POINTER(vp)]
         L.md_destroy.argtypes = [vp]
         L.md_set_option.argtypes = [vp, C.c_char_p, C.c_double]
+        L.md_get_option.argtypes = [vp, C.c_char_p, C.POINTER(C.c_double)]
         L.md_counters.argtypes = [vp, ip, C.c_int, vp]
         L.md_set_species_lj.argtypes = [vp, C.c_int, C.POINTER(C.c_float), C.POINTER(C.c_float), C.POINTER(C.c_float)]
         L.md_brownian_step.argtypes = [vp, C.POINTER(md_potential), vp, vp, ip, ip, ip, C.c_float, C.c_float,
@@ -200,6 +201,12 @@ def md_destroy(sys) -> None:
 
 def md_set_option(sys, name: str, value: float) -> None:
     _check(lib().md_set_option(sys, name.encode(), float(value)))
+
+
+def md_get_option(sys, name: str) -> float:
+    v = C.c_double(0.0)
+    _check(lib().md_get_option(sys, name.encode(), C.byref(v)))
+    return float(v.value)
 
 
 def md_brownian_step(sys, pot: md_potential, pos, force, id, nbr_idx, nbr_count, dt, gamma, kT, seed, step0,

@@ -116,6 +116,7 @@ struct md_system {
     int fused;           // fused step: the force kernel also opens the next step (graph mode, fast32)
     int remap;           // force kernel: block -> tile remap period (the SM count), 0 = off
     int nb_parts;        // builder: warps per tile (0 = by system size, 1, 2, 4)
+    int flagged;         // the rebuild of the step loops as flagged launches instead of an IF node: -1 by size, 0, 1
     int cell_coop;       // cell list as one cooperative launch with this many blocks at most (0: five kernels)
     int cell_coop_max;   // what the device allows
     int ns;              // md_set_species_lj: number of species and the tables (row-major)
@@ -309,13 +310,14 @@ int make_pair(const md_system *sys, const md_potential *pot, Pair *pp) {
 // ------------------------------------------------------------------ launch helpers ------
 
 int launch_cell_build(md_system *s, float4 *pos, float4 *vel, int *id, int *cell_start,
-                      int *perm, int *status, const int *cond, cudaStream_t st) {
+                      int *perm, int *status, const int *cond, cudaStream_t st, bool cooperative = false) {
     const Geom &g = s->g;
     const int nb = blocks_for(g.n);
     const bool resort = s->cfg.resort != 0;
-    if (s->cell_coop > 0) {
+    const int coop = cooperative ? s->cell_coop_max : s->cell_coop;
+    if (coop > 0) {
         // one cooperative launch (grid-wide barriers between the phases); needs every block resident
-        const int grid = std::min(nb, s->cell_coop);
+        const int grid = std::min(nb, coop);
         Geom gg = g;
         float4 *velp = (resort && vel) ? vel : nullptr, *vel_s = (resort && vel) ? s->vel_s : nullptr;
         int *idp = id, *id_s = (resort && id) ? s->id_s : nullptr;
@@ -419,6 +421,30 @@ int launch_force_t(md_system *s, const Pair &pp, const float4 *pos, const int *n
 #undef MD_FORCE_CASE
     LAUNCH_OK();
     return MD_OK;
+}
+
+// ---- the rebuild inside a step loop
+// Captured in a graph, the rebuild is either the body of an IF node that the drift raises, or launches that
+// are part of every step and return at once while the step's device flag is 0.  Measured on B200 (a lattice at
+// rest, 256,000 particles, no rebuild ever fires): a step costs 39.6 us without any rebuild machinery, 48.7 us
+// with the IF node (9 us whether or not it fires), 42.3 us with one cooperative kernel that returns at once
+// and 2.7-3.0 us more per further kernel.  So where the cooperative cell list keeps up with its five kernels
+// (at 1M particles it is 24 us slower per rebuild, more than the launches save) the rebuild is TWO flagged
+// launches, cooperative cell list and builder, and no IF node.
+constexpr int FLAGGED_MAX_N = 600000;
+bool rebuild_is_flagged(const md_system *s) {
+    if (s->flagged == 0 || !(s->cell_coop_max > 0)) return false;
+    return s->flagged > 0 || s->g.n <= FLAGGED_MAX_N;
+}
+// flag: device word; the launches do nothing while it is 0
+int launch_rebuild_flagged(md_system *s, float4 *pos, float4 *vel, int *id, int *nbr_idx, int *nbr_count,
+                           const int *flag, cudaStream_t st) {
+    int *status = s->words + 1;
+    const bool resort = s->cfg.resort != 0;
+    int rc = launch_cell_build(s, pos, vel, id, s->cell_start_i, s->perm_i, status, flag, st, rebuild_is_flagged(s));
+    if (rc) return rc;
+    return launch_nbr_build(s, resort ? pos : s->pos_s, s->cell_start_i, resort ? nullptr : s->perm_i,
+                            nbr_idx, nbr_count, status, flag, 1, st);
 }
 
 // The kinds md_force32.cuh serves (3-D only): fp32 pair math, error estimate, fp64 re-evaluation.
@@ -757,17 +783,13 @@ int record_step(md_system *s, const Pair &pp, float4 *pos, float4 *vel, float4 *
     int *flag = s->words + 0;
     int *status = s->words + 1;
     const int nb = blocks_for(g.n);
-    const bool resort = s->cfg.resort != 0;
     int rc;
-    if (!in_graph) {
+    if (!in_graph || rebuild_is_flagged(s)) {
         cudaGraphConditionalHandle none = 0;
         if (g.dim == 3) k_kick_drift<3, false><<<nb, 256, 0, st>>>(g, pos, vel, force, s->ref_pos, a, dt, flag, none);
         else k_kick_drift<2, false><<<nb, 256, 0, st>>>(g, pos, vel, force, s->ref_pos, a, dt, flag, none);
         LAUNCH_OK();
-        rc = launch_cell_build(s, pos, vel, id, s->cell_start_i, s->perm_i, status, flag, st);
-        if (rc) return rc;
-        rc = launch_nbr_build(s, resort ? pos : s->pos_s, s->cell_start_i, resort ? nullptr : s->perm_i,
-                              nbr_idx, nbr_count, status, flag, 1, st);
+        rc = launch_rebuild_flagged(s, pos, vel, id, nbr_idx, nbr_count, flag, st);
         if (rc) return rc;
     } else {
         cudaStreamCaptureStatus cs;
@@ -786,12 +808,19 @@ int record_step(md_system *s, const Pair &pp, float4 *pos, float4 *vel, float4 *
     return launch_force(s, pp, pos, nbr_idx, nbr_count, force, vel, a, nullptr, false, book, st);
 }
 
+int run_fused_direct(md_system *s, const Pair &pp, float4 *pos, float4 *vel, float4 *force, int *id,
+                     int *nbr_idx, int *nbr_count, float dt, float mass, int *stats, int nsteps,
+                     cudaStream_t st);
+
 // `reps` fused steps on the capturing stream `st` (3-D LJ fast path): one k_kick_drift opens the
 // first step, every force kernel but the last also opens the next step and writes the drifted
 // positions to the other buffer (pos <-> pos_alt); reps is 1 or odd, so the state ends in `pos`.
 int record_fused(md_system *s, const Pair &pp, float4 *pos, float4 *vel, float4 *force, int *id,
                  int *nbr_idx, int *nbr_count, float dt, float mass, int *stats, int reps,
                  cudaStream_t st) {
+    // the rebuild as launches that return at once on a zero flag: no IF nodes, the plain loop is the graph
+    if (rebuild_is_flagged(s))
+        return run_fused_direct(s, pp, pos, vel, force, id, nbr_idx, nbr_count, dt, mass, stats, reps, st);
     const Geom &g = s->g;
     const float a = dt / (2.0f * mass);
     int *flags[2] = {s->words + 0, s->words + 3};
@@ -834,16 +863,13 @@ int run_fused_direct(md_system *s, const Pair &pp, float4 *pos, float4 *vel, flo
     const float a = dt / (2.0f * mass);
     int *flags[2] = {s->words + 0, s->words + 3};
     int *status = s->words + 1;
-    const bool resort = s->cfg.resort != 0;
     cudaGraphConditionalHandle none = 0;
     k_kick_drift<3, false><<<blocks_for(g.n), 256, 0, st>>>(g, pos, vel, force, s->ref_pos, a, dt, flags[0], none);
     LAUNCH_OK();
     float4 *cur = pos, *other = s->pos_alt;
     for (int r = 0; r < nsteps; ++r) {
         int *flag = flags[r & 1];
-        int rc = launch_cell_build(s, cur, vel, id, s->cell_start_i, s->perm_i, status, flag, st);
-        if (!rc) rc = launch_nbr_build(s, resort ? cur : s->pos_s, s->cell_start_i, resort ? nullptr : s->perm_i,
-                                       nbr_idx, nbr_count, status, flag, 1, st);
+        int rc = launch_rebuild_flagged(s, cur, vel, id, nbr_idx, nbr_count, flag, st);
         if (rc) return rc;
         Book book = {flag, status, stats};
         NextStep nx = NextStep();
@@ -898,11 +924,11 @@ int capture(md_system *s, const Pair &pp, const StepKey &k, int reps, cudaGraphE
 int record_rule_step(md_system *s, const Pair &pp, const RuleArgs &A, cudaStream_t st, bool in_graph) {
     const Geom &g = s->g;
     int *flag = s->words + 0, *status = s->words + 1;
-    const bool resort = s->cfg.resort != 0;
     const int nb = blocks_for(g.n);
     float4 *p4 = (float4 *)A.pos, *v4 = (float4 *)A.vel, *f4 = (float4 *)A.force;
     Raise rs = {flag, 0, 0};
-    if (in_graph) {
+    const bool use_if = in_graph && !rebuild_is_flagged(s);
+    if (use_if) {
         cudaStreamCaptureStatus cs;
         cudaGraph_t graph = nullptr;
         CU(cudaStreamGetCaptureInfo(st, &cs, nullptr, &graph, nullptr, nullptr));
@@ -988,14 +1014,11 @@ int record_rule_step(md_system *s, const Pair &pp, const RuleArgs &A, cudaStream
     LAUNCH_OK();
     float4 *sort_vel = (A.rule == RULE_BROWNIAN || A.rule == RULE_FLOCK) ? nullptr : v4;
     int rc;
-    if (in_graph) {
+    if (use_if) {
         rc = record_rebuild_if(s, st, rs.cond, p4, sort_vel, A.id, A.nbr_idx, A.nbr_count);
         if (rc) return rc;
     } else {
-        rc = launch_cell_build(s, p4, sort_vel, A.id, s->cell_start_i, s->perm_i, status, flag, st);
-        if (rc) return rc;
-        rc = launch_nbr_build(s, resort ? p4 : s->pos_s, s->cell_start_i, resort ? nullptr : s->perm_i,
-                              A.nbr_idx, A.nbr_count, status, flag, 1, st);
+        rc = launch_rebuild_flagged(s, p4, sort_vel, A.id, A.nbr_idx, A.nbr_count, flag, st);
         if (rc) return rc;
     }
     Book book = {flag, status, A.stats};
@@ -1131,6 +1154,7 @@ int md_create(const md_config *cfg, int n, void *workspace, size_t bytes, md_sys
     s->r0 = 0; s->r1 = n;
     s->fast32 = 1;
     s->builder = 2;
+    s->flagged = -1;
     {   // block -> tile remap period: a quarter of the SM count measured best (46.7 -> 44.9 us at N = 256k on 148 SMs)
         int sms = 0;
         cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, attr.device);
@@ -1250,6 +1274,11 @@ int md_set_option(md_system *sys, const char *name, double value) {
         if (value != 0.0 && value != 1.0 && value != 2.0 && value != 4.0) return fail(MD_EINVAL, "builder_parts must be 0, 1, 2 or 4");
         sys->nb_parts = (int)value;
     }
+    else if (!strcmp(name, "rebuild_flagged")) {
+        if (value != -1.0 && value != 0.0 && value != 1.0) return fail(MD_EINVAL, "rebuild_flagged must be -1 (by size), 0 or 1");
+        if (value == 1.0 && !(sys->cell_coop_max > 0)) return fail(MD_EINVAL, "the device offers no cooperative launch");
+        sys->flagged = (int)value;
+    }
     else if (!strcmp(name, "builder")) {
         if (value != 1.0 && value != 2.0) return fail(MD_EINVAL, "builder must be 1 or 2");
         sys->builder = (int)value;
@@ -1265,6 +1294,19 @@ int md_set_option(md_system *sys, const char *name, double value) {
     }
     else return fail(MD_EINVAL, "unknown option %s", name);
     drop_graphs(sys);
+    return MD_OK;
+}
+
+int md_get_option(md_system *sys, const char *name, double *value) {
+    if (!sys || !name || !value) return fail(MD_EINVAL, "NULL argument");
+    DeviceScope scope_(sys->device);
+    if (scope_.rc) return scope_.rc;
+    if (!strcmp(name, "rebuild_flagged")) *value = rebuild_is_flagged(sys) ? 1.0 : 0.0;   // what the step loops do
+    else if (!strcmp(name, "est_thr")) *value = sys->est_thr;
+    else if (!strcmp(name, "fast32")) *value = sys->fast32;
+    else if (!strcmp(name, "use_graph")) *value = sys->use_graph;
+    else if (!strcmp(name, "threads_per_particle")) *value = sys->tpp;
+    else return fail(MD_EINVAL, "unknown option %s", name);
     return MD_OK;
 }
 

@@ -1017,6 +1017,42 @@ def test_fused_step_same_bits(B, W, ci, steps, resort):
     assert int(out[0][4][0]) == steps and int(out[0][4][1]) >= 5
 
 
+@pytest.mark.parametrize("ci,steps,resort", [(0, 100, 1), (1, 60, 1), (2, 120, 1), (2, 61, 0)])
+def test_rebuild_as_flagged_launches_or_if_node_same_bits(B, W, ci, steps, resort):
+    """Inside the step graphs the rebuild is either two launches that return at once while the step's flag
+    is 0 (cooperative cell list + builder; the default at these sizes) or the body of an IF node
+    ("rebuild_flagged" = 0): same bits, same rebuild history, same lists -- for the fused 3-D LJ loop, the 2-D
+    soft-sphere loop, and without the physical re-sort; and for one of the update rules."""
+    w = W.config(ci)
+    out = []
+    for flagged in (1, 0):
+        S = B.System(w, resort=resort)
+        B.md_set_option(S.sys, "rebuild_flagged", flagged)
+        assert B.md_get_option(S.sys, "rebuild_flagged") == flagged
+        S.build(); S.compute_force(); S.step(steps)
+        torch.cuda.synchronize()
+        out.append((S.pos.clone(), S.vel.clone(), S.force.clone(), S.id.clone(), S.stats.clone(), S.nbr_rows().clone(),
+                    S.nbr_count.clone()))
+        S.close()
+    for x, y in zip(out[0], out[1]):
+        assert torch.equal(x, y)
+    assert int(out[0][4][0]) == steps and int(out[0][4][1]) >= 3
+    if ci == 0:                                   # a rule other than NVE: Langevin through its own graphs
+        res = []
+        for flagged in (1, 0):
+            S = B.System(w)
+            B.md_set_option(S.sys, "rebuild_flagged", flagged)
+            S.build(); S.compute_force()
+            B.md_langevin_step(S.sys, S.pot, S.pos, S.vel, S.force, S.id, S.nbr_idx, S.nbr_count, w.dt, w.mass, 1.0, 1.0,
+                               7, 0, 50, S.stats)
+            torch.cuda.synchronize()
+            res.append((S.pos.clone(), S.vel.clone(), S.id.clone(), S.stats.clone()))
+            S.close()
+        for x, y in zip(res[0], res[1]):
+            assert torch.equal(x, y)
+        assert int(res[0][3][1]) >= 2
+
+
 def test_nve_run_host_context_reuse(B, W):
     """md_nve_run_host keeps its device context between calls: a second call with the same
     (cfg, n) must give the same bits, a call with another system must replace the context, and
