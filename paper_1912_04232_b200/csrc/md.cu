@@ -942,10 +942,13 @@ int record_rule_step(md_system *s, const Pair &pp, const RuleArgs &A, cudaStream
     const int nbk = blocks_for(g.n, NH_BLOCK), nbf = blocks_for(g.n, FIRE_BLOCK);
     double *partial = s->fire_tmp;
     switch (A.rule) {
-    case RULE_FIRE:
-        if (g.dim == 3) k_fire_kick_drift<3><<<nb, 256, 0, st>>>(g, p4, v4, f4, s->ref_pos, (const float *)A.state, rs);
-        else k_fire_kick_drift<2><<<nb, 256, 0, st>>>(g, p4, v4, f4, s->ref_pos, (const float *)A.state, rs);
+    case RULE_FIRE: {
+        // the mixing of the previous step (coef, written by its k_fire_finalize) happens in this kernel
+        const float *coef = reinterpret_cast<const float *>(s->fire_tmp + (size_t)nbf * 3);
+        if (g.dim == 3) k_fire_kick_drift<3><<<nb, 256, 0, st>>>(g, p4, v4, f4, s->ref_pos, (const float *)A.state, coef, rs);
+        else k_fire_kick_drift<2><<<nb, 256, 0, st>>>(g, p4, v4, f4, s->ref_pos, (const float *)A.state, coef, rs);
         break;
+    }
     case RULE_BROWNIAN: {
         const float mu = A.dt / A.gamma, amp = std::sqrt(2.0f * A.kT * A.dt / A.gamma);
         if (g.dim == 3) k_brownian_drift<3><<<nb, 256, 0, st>>>(g, p4, f4, A.id, s->ref_pos, mu, amp, reinterpret_cast<const unsigned *>(s->words + 20), A.stats, rs);
@@ -962,12 +965,13 @@ int record_rule_step(md_system *s, const Pair &pp, const RuleArgs &A, cudaStream
     }
     case RULE_NH: {
         const double dofkT = (double)g.dim * g.n * (double)A.kT, tau2 = (double)A.tau * (double)A.tau;
+        // scale = {this half step's factor, the previous step's closing factor (still to be applied), 1}
         float *scale = reinterpret_cast<float *>(s->fire_tmp + nbk);
-        k_nh_ke<<<nbk, NH_BLOCK, 0, st>>>(g.n, g.dim, v4, partial);
+        k_nh_ke<<<nbk, NH_BLOCK, 0, st>>>(g.n, g.dim, v4, partial, scale + 1);
         k_nh_finalize<<<1, 256, 0, st>>>(nbk, partial, (double)A.mass, dofkT, (double)A.kT, tau2, A.nh_chain,
                                          (double)A.dt, (double *)A.state, scale);
-        if (g.dim == 3) k_nh_kick_drift<3><<<nb, 256, 0, st>>>(g, p4, v4, f4, s->ref_pos, a, A.dt, scale, rs);
-        else k_nh_kick_drift<2><<<nb, 256, 0, st>>>(g, p4, v4, f4, s->ref_pos, a, A.dt, scale, rs);
+        if (g.dim == 3) k_nh_kick_drift<3><<<nb, 256, 0, st>>>(g, p4, v4, f4, s->ref_pos, a, A.dt, scale, scale + 1, rs);
+        else k_nh_kick_drift<2><<<nb, 256, 0, st>>>(g, p4, v4, f4, s->ref_pos, a, A.dt, scale, scale + 1, rs);
         force_vel = v4; force_a = a;
         break;
     }
@@ -1035,16 +1039,14 @@ int record_rule_step(md_system *s, const Pair &pp, const RuleArgs &A, cudaStream
         float *coef = reinterpret_cast<float *>(s->fire_tmp + (size_t)nbf * 3);
         k_fire_kick_reduce<<<nbf, FIRE_BLOCK, 0, st>>>(g.n, g.dim, v4, f4, (const float *)A.state, partial);
         k_fire_finalize<<<1, 256, 0, st>>>(nbf, partial, fp, (float *)A.state, coef);
-        k_fire_mix<<<nb, 256, 0, st>>>(g.n, v4, f4, coef);
-        LAUNCH_OK();
+        LAUNCH_OK();      // the mixing v = c1 v + c2 F: in the next step's k_fire_kick_drift, or in run_rule when the call ends
     } else if (A.rule == RULE_NH) {
         const double dofkT = (double)g.dim * g.n * (double)A.kT, tau2 = (double)A.tau * (double)A.tau;
         float *scale = reinterpret_cast<float *>(s->fire_tmp + nbk);
-        k_nh_ke<<<nbk, NH_BLOCK, 0, st>>>(g.n, g.dim, v4, partial);
+        k_nh_ke<<<nbk, NH_BLOCK, 0, st>>>(g.n, g.dim, v4, partial, scale + 2);
         k_nh_finalize<<<1, 256, 0, st>>>(nbk, partial, (double)A.mass, dofkT, (double)A.kT, tau2, A.nh_chain,
-                                         (double)A.dt, (double *)A.state, scale);
-        k_nh_scale<<<nb, 256, 0, st>>>(g.n, v4, scale);
-        LAUNCH_OK();
+                                         (double)A.dt, (double *)A.state, scale + 1);
+        LAUNCH_OK();      // v *= scale[1]: in the next step's k_nh_ke / k_nh_kick_drift, or in run_rule when the call ends
     }
     return MD_OK;
 }
@@ -1065,6 +1067,22 @@ int capture_rule(md_system *s, const Pair &pp, const RuleArgs &A, int reps, cuda
 }
 
 // nsteps of an update rule: stats reset, then graphs of 8 steps and of 1 step (or direct launches).
+// What a rule leaves for the next step's opening kernel is applied here when the call ends, so that the
+// caller's velocities are final: FIRE's mixing, Nose-Hoover's closing scale factor.
+int finish_rule(md_system *s, const RuleArgs &A, cudaStream_t st) {
+    const int n = s->g.n, nb = blocks_for(n);
+    if (A.rule == RULE_FIRE) {
+        const float *coef = reinterpret_cast<const float *>(s->fire_tmp + (size_t)blocks_for(n, FIRE_BLOCK) * 3);
+        k_fire_mix<<<nb, 256, 0, st>>>(n, (float4 *)A.vel, (const float4 *)A.force, coef);
+        LAUNCH_OK();
+    } else if (A.rule == RULE_NH) {
+        const float *scale = reinterpret_cast<const float *>(s->fire_tmp + blocks_for(n, NH_BLOCK));
+        k_nh_scale<<<nb, 256, 0, st>>>(n, (float4 *)A.vel, scale + 1);
+        LAUNCH_OK();
+    }
+    return MD_OK;
+}
+
 int run_rule(md_system *s, const Pair &pp, RuleArgs &A, int nsteps, cudaStream_t st) {
     if (s->r0 != 0 || s->r1 != s->g.n) return fail(MD_EINVAL, "a range is set (md_set_range): drive the step with md_kick_drift / md_half_kick");
     A.fast32 = s->fast32; A.builder = s->builder; A.nb_parts = s->nb_parts; A.remap = s->remap; A.est_thr = s->est_thr;
@@ -1072,9 +1090,13 @@ int run_rule(md_system *s, const Pair &pp, RuleArgs &A, int nsteps, cudaStream_t
     k_set_noise<<<1, 1, 0, st>>>(s->words, A.seed, A.step0);
     LAUNCH_OK();
     A.seed = 0; A.step0 = 0;          // not part of what a captured graph depends on
+    if (A.rule == RULE_NH) {
+        k_nh_begin<<<1, 1, 0, st>>>(reinterpret_cast<float *>(s->fire_tmp + blocks_for(s->g.n, NH_BLOCK)));
+        LAUNCH_OK();
+    }
     if (!s->use_graph) {
         for (int k = 0; k < nsteps; ++k) { int rc = record_rule_step(s, pp, A, st, false); if (rc) return rc; }
-        return MD_OK;
+        return finish_rule(s, A, st);
     }
     if (!s->rule_key_valid || memcmp(&A, &s->rule_key, sizeof(A)) != 0) {
         if (s->rule_exec1) cudaGraphExecDestroy(s->rule_exec1);
@@ -1093,7 +1115,7 @@ int run_rule(md_system *s, const Pair &pp, RuleArgs &A, int nsteps, cudaStream_t
         if (!s->rule_exec1) { rc = capture_rule(s, pp, A, 1, &s->rule_exec1); if (rc) return rc; }
         for (; left > 0; --left) CU(cudaGraphLaunch(s->rule_exec1, st));
     }
-    return MD_OK;
+    return finish_rule(s, A, st);
 }
 
 } // namespace
@@ -1873,7 +1895,7 @@ int md_fire_minimize(md_system *sys, const md_potential *pot, const md_fire_para
     if (scope_.rc) return scope_.rc;
     cudaStream_t st = (cudaStream_t)stream;
     const FirePar fp = {par->dt_start, par->dt_max, par->n_min, par->f_inc, par->f_dec, par->alpha_start, par->f_alpha};
-    k_fire_init<<<1, 1, 0, st>>>(fp, fire_state);
+    k_fire_init<<<1, 1, 0, st>>>(fp, fire_state, reinterpret_cast<float *>(sys->fire_tmp + (size_t)blocks_for(sys->g.n, FIRE_BLOCK) * 3));
     LAUNCH_OK();
     RuleArgs A;
     memset(&A, 0, sizeof(A));

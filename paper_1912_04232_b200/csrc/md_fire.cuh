@@ -3,7 +3,8 @@
 // paper gives no formulas: algorithm of Bitzek et al. 2006, reading A20).  Unit mass.
 //   1. v += dt/2 F;  r = mu(r, dt v);  [rebuild];  F = F(r);  v += dt/2 F
 //   2. P = sum F.v, FF = sum F.F, VV = sum v.v                 (fp64 sums of fp32 products)
-//   3. P > 0: v = (1 - alpha) v + alpha sqrt(VV / FF) F; n_pos += 1;
+//   3. (applied at the start of the next step's kernel 1, or by k_fire_mix when the call ends)
+//      P > 0: v = (1 - alpha) v + alpha sqrt(VV / FF) F; n_pos += 1;
 //             n_pos > n_min: dt = min(dt f_inc, dt_max), alpha *= f_alpha
 //      else:  v = 0; n_pos = 0; dt *= f_dec; alpha = alpha_start
 // dt, alpha, n_pos live in a device float[4] (`state`), so the step size never leaves the device.
@@ -15,20 +16,25 @@ namespace mdk {
 struct FirePar { float dt_start, dt_max; int n_min; float f_inc, f_dec, alpha_start, f_alpha; };
 
 // state = {dt, alpha, n_pos, last P (sign only)}; a non-positive dt on entry means "start".
-__global__ void k_fire_init(FirePar p, float *state) {
+// coef: the mixing coefficients {c1, c2} the velocities have still to take; none at the start of a call
+__global__ void k_fire_init(FirePar p, float *state, float *coef) {
     if (!(state[0] > 0.0f)) { state[0] = p.dt_start; state[1] = p.alpha_start; state[2] = 0.0f; state[3] = 0.0f; }
+    coef[0] = 1.0f; coef[1] = 0.0f;
 }
 
 template <int DIM>
 __global__ void __launch_bounds__(256)
 k_fire_kick_drift(Geom g, float4 *__restrict__ pos, float4 *__restrict__ vel,
                   const float4 *__restrict__ force, const float4 *__restrict__ ref,
-                  const float *__restrict__ state, Raise rs) {
+                  const float *__restrict__ state, const float *__restrict__ coef, Raise rs) {
     const float dt = state[0], a = 0.5f * dt;
+    const float c1 = coef[0], c2 = coef[1];
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     bool moved = false;
     if (i < g.n) {
         float4 p = pos[i], v = vel[i], f = force[i];
+        // the mixing step 3 of the previous MD step (k_fire_mix's arithmetic; {1, 0} leaves v as it is)
+        v.x = fmaf(c2, f.x, c1 * v.x); v.y = fmaf(c2, f.y, c1 * v.y); v.z = fmaf(c2, f.z, c1 * v.z);
         v.x = fmaf(a, f.x, v.x);
         v.y = fmaf(a, f.y, v.y);
         p.x = wrap(fmaf(dt, v.x, p.x), g.L[0], g.inv_L[0]);

@@ -12,12 +12,15 @@ namespace mdk {
 constexpr int NH_BLOCK = 256;
 
 __global__ void __launch_bounds__(NH_BLOCK)
-k_nh_ke(int n, int dim, const float4 *__restrict__ vel, double *__restrict__ partial) {
+k_nh_ke(int n, int dim, const float4 *__restrict__ vel, double *__restrict__ partial,
+        const float *__restrict__ pending) {
     __shared__ double red[NH_BLOCK / 32];
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     double s = 0.0;
+    const float sp = *pending;        // a scale the stored velocities have still to take (1: none)
     if (i < n) {
-        const float4 v = vel[i];
+        float4 v = vel[i];
+        v.x *= sp; v.y *= sp; v.z *= sp;
         s = (double)v.x * v.x + (double)v.y * v.y + (dim == 3 ? (double)v.z * v.z : 0.0);
     }
 #pragma unroll
@@ -80,12 +83,13 @@ template <int DIM>
 __global__ void __launch_bounds__(256)
 k_nh_kick_drift(Geom g, float4 *__restrict__ pos, float4 *__restrict__ vel,
                 const float4 *__restrict__ force, const float4 *__restrict__ ref, float a, float dt,
-                const float *__restrict__ scale, Raise rs) {
-    const float sc = *scale;
+                const float *__restrict__ scale, const float *__restrict__ pending, Raise rs) {
+    const float sc = *scale, sp = *pending;
     int i = blockIdx.x * blockDim.x + threadIdx.x;
     bool moved = false;
     if (i < g.n) {
         float4 p = pos[i], v = vel[i], f = force[i];
+        v.x *= sp; v.y *= sp; v.z *= sp;     // the closing thermostat half step of the previous MD step (k_nh_scale)
         v.x = fmaf(a, f.x, sc * v.x);
         v.y = fmaf(a, f.y, sc * v.y);
         p.x = wrap(fmaf(dt, v.x, p.x), g.L[0], g.inv_L[0]);
@@ -100,6 +104,10 @@ k_nh_kick_drift(Geom g, float4 *__restrict__ pos, float4 *__restrict__ vel,
     if (__any_sync(FULL, moved) && (threadIdx.x & 31) == 0) raise_rebuild(rs);
 }
 
+// scale = {this half step's factor, the factor the stored velocities have still to take, 1}
+__global__ void k_nh_begin(float *scale) { scale[1] = 1.0f; scale[2] = 1.0f; }
+
+// the pending factor into the stored velocities (when a call ends)
 __global__ void __launch_bounds__(256)
 k_nh_scale(int n, float4 *__restrict__ vel, const float *__restrict__ scale) {
     int i = blockIdx.x * blockDim.x + threadIdx.x;
