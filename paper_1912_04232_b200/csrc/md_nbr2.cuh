@@ -8,8 +8,9 @@
 // per-lane column of capacity + 1 rows in shared memory (16.5 KB per warp at capacity 128:
 // 12 warps per SM) through a chain of predicated store / pointer bumps, 12.5 instructions per
 // candidate.  Here the sign bit of fl(r2 - R2) -- set exactly when r2 < R2 -- is shifted into a
-// per-lane bit mask, one funnel shift per candidate and no branch, 32 candidates per word; the
-// masks of up to NB2_WORDS words (5 KB per warp) are expanded afterwards, every lane pulling
+// per-lane bit mask, one funnel shift per candidate and no branch, 32 candidates per word; every
+// lane keeps its NON-ZERO words (and the slot each starts at) densely in its own shared-memory column,
+// up to NB2_WORDS of them (6 KB per warp), and they are expanded afterwards, every lane pulling
 // its next set bit per iteration, so row k of the tile leaves as one coalesced 128-byte store.
 #pragma once
 #include "md_kernels.cuh"
@@ -20,13 +21,12 @@ namespace mdk {
 #define MD_NB2_WARPS 4
 #endif
 constexpr int NB2_WARPS = MD_NB2_WARPS;   // tiles per block
-constexpr int NB2_WORDS = 40;         // mask words per lane per batch (1280 candidates)
+constexpr int NB2_WORDS = 24;         // NON-ZERO mask words a lane can hold per batch
 constexpr int NB2_CHUNK = 128;        // candidates staged per round (4 words)
-static_assert(NB2_WORDS <= 64, "two 32-bit masks of pending words per lane");
 
 struct Nb2Warp {                      // shared memory of one builder warp
-    unsigned mask[NB2_WORDS][TILE];   // [word][lane]
-    int wbase[NB2_WORDS];             // slot of bit 31 of each word
+    unsigned mask[NB2_WORDS][TILE];   // [k][lane]: the k-th non-zero mask word of the lane
+    int wb[NB2_WORDS][TILE];          // slot of bit 31 of that word
     float sx[NB2_CHUNK], sy[NB2_CHUNK], sz[NB2_CHUNK];
 };
 
@@ -143,48 +143,42 @@ k_nbr_build2(Geom g, const float4 *__restrict__ spos, const int *__restrict__ ce
             // start after the other parts' hits): part 0 then scans the whole segment alone
             bool solo = false;
             if (PARTS > 1) {
-                const int words = lane < 3 * ROWS ? ((t1 - t0 + 31) >> 5) + 1 : 0;
+                const int words = lane < 3 * ROWS ? (t1 - t0 + 31) >> 5 : 0;     // chunks split a piece at multiples of 128
 #pragma unroll
                 for (int q = 0; q < PARTS; ++q)
                     solo = solo || warp_sum_i(lane % PARTS == q ? words : 0) > NB2_WORDS;
             }
-            int nw = 0;                      // mask words of the current batch (warp-uniform)
-            unsigned nzlo = 0u, nzhi = 0u;   // which of them are non-zero for this lane (words 0-31, 32-)
+            int myw = 0;                     // non-zero mask words this lane holds in the current batch
             int nhit = 0;                    // hits of this lane in the current batch (self excluded)
-            // every lane pulls its next hit per iteration (taking its next non-zero mask word when
-            // the current one is used up): row k of the tile leaves as one 128-byte store.  The trip
-            // count is the largest number of hits any lane holds, so the loop needs no vote.
+            // every lane pulls its next hit per iteration (taking its next stored word when the current one
+            // is used up): row k of the tile leaves as one 128-byte store.  The trip count is the largest
+            // number of hits any lane holds, so the loop needs no vote.
             auto expand = [&]() {
                 __syncwarp();
-                unsigned plo = inseg ? nzlo : 0u, phi = inseg ? nzhi : 0u;   // words still to visit
-                const int nit = warp_max(inseg ? nhit : 0);
-                unsigned word = 0u;
+                const int nit = warp_max(nhit);
                 int w = 0;
+                unsigned word = myw > 0 ? W.mask[0][lane] : 0u;      // stored words are non-zero
+                int wbv = myw > 0 ? W.wb[0][lane] : 0;
                 int *optr = outp + (size_t)min(cnt, cap) * TILE;
-                // branch-free body: selects and predicated memory operations only
                 for (int it = 0; it < nit; ++it) {
-                    const bool need = word == 0u && (plo | phi) != 0u;
-                    const int wl = __ffs(plo) - 1, wh = 31 + __ffs(phi);
-                    const int wn = plo ? wl : wh;
-                    const unsigned nlo = plo & (plo - 1u), nhi = plo ? phi : (phi & (phi - 1u));
-                    w = need ? wn : w;
-                    plo = need ? nlo : plo;
-                    phi = need ? nhi : phi;
-                    MD_CHECK(w >= 0 && w < NB2_WORDS);
-                    const unsigned fresh = W.mask[w][lane];        // w is always a valid word index
-                    word = need ? fresh : word;
                     const bool has = word != 0u;
                     const int bit = __clz(word) & 31;
-                    const int slot = W.wbase[w] + bit;
+                    const int slot = wbv + bit;
                     word &= 0x7fffffffu >> bit;                    // drop that bit (all above it are 0)
                     MD_CHECK(!has || (slot >= 0 && slot < g.n && slot != s));
                     MD_CHECK(!(has && cnt < cap) || (optr >= outp && optr < outp + (size_t)cap * TILE));
                     if (has && cnt < cap) *optr = MAPPED ? map[slot] : slot;
                     optr += (has && cnt < cap) ? TILE : 0;
                     cnt += has ? 1 : 0;
+                    if (word == 0u && w + 1 < myw) {               // my next word
+                        ++w;
+                        MD_CHECK(w < NB2_WORDS);
+                        word = W.mask[w][lane];
+                        wbv = W.wb[w][lane];
+                    }
                 }
                 __syncwarp();
-                nw = 0; nzlo = 0u; nzhi = 0u; nhit = 0;
+                myw = 0; nhit = 0;
             };
 
             // ---- walk the pieces; the next chunk is loaded while the current one is tested
@@ -218,8 +212,9 @@ k_nbr_build2(Geom g, const float4 *__restrict__ spos, const int *__restrict__ ce
                 const float piy = rcy + dy >= ncy ? __fsub_rn(pi.y, Ly) : pi.y;
                 const float piz = (DIM == 3 && rcz + dz >= ncz) ? __fsub_rn(pi.z, Lz) : pi.z;
                 const int m = min(NB2_CHUNK, pt1 - base);
-                if (nw + ((m + 31) >> 5) > NB2_WORDS) expand();   // batch full (warp-uniform)
-                MD_CHECK(m > 0 && base >= 0 && pt1 <= g.n && nw + ((m + 31) >> 5) <= NB2_WORDS);
+                // a lane's column could overflow if every word of this chunk came out non-zero: flush first
+                if (__any_sync(FULL, myw + ((m + 31) >> 5) > NB2_WORDS)) expand();
+                MD_CHECK(m > 0 && base >= 0 && pt1 <= g.n && myw + ((m + 31) >> 5) <= NB2_WORDS);
                 // stage -(candidate - shift), structure of arrays; the tail of the last group of
                 // four is a far-away point
 #pragma unroll
@@ -234,7 +229,6 @@ k_nbr_build2(Geom g, const float4 *__restrict__ spos, const int *__restrict__ ce
                         if (DIM == 3) W.sz[c] = 0.0f;
                     }
                 }
-                if (lane < ((m + 31) >> 5)) W.wbase[nw + lane] = base + lane * 32;
                 __syncwarp();
                 // next chunk
                 int np = p, nbase = base + NB2_CHUNK, npt1 = pt1;
@@ -281,11 +275,13 @@ k_nbr_build2(Geom g, const float4 *__restrict__ spos, const int *__restrict__ ce
                         const unsigned self = (unsigned)(s - (base + c0));
                         if (self < 32u) hi &= ~(0x80000000u >> self);
                     }
+                    if (!inseg) hi = 0u;                           // other segments' lanes record nothing
                     nhit += __popc(hi);
-                    W.mask[nw][lane] = hi;
-                    if (nw < 32) nzlo |= (hi != 0u ? 1u : 0u) << nw;
-                    else nzhi |= (hi != 0u ? 1u : 0u) << (nw - 32);
-                    ++nw;
+                    if (hi != 0u) {
+                        W.mask[myw][lane] = hi;
+                        W.wb[myw][lane] = base + c0;
+                        ++myw;
+                    }
                 }
                 __syncwarp();
                 p = np; base = nbase; pt1 = npt1;
