@@ -14,6 +14,7 @@
 // its next set bit per iteration, so row k of the tile leaves as one coalesced 128-byte store.
 #pragma once
 #include "md_kernels.cuh"
+#include <cstddef>
 
 namespace mdk {
 
@@ -26,9 +27,10 @@ constexpr int NB2_CHUNK = 128;        // candidates staged per round (4 words)
 
 struct Nb2Warp {                      // shared memory of one builder warp
     unsigned mask[NB2_WORDS][TILE];   // [k][lane]: the k-th non-zero mask word of the lane
-    int wb[NB2_WORDS][TILE];          // slot of bit 31 of that word
+    int wb[NB2_WORDS][TILE];          // slot of bit 31 of that word (directly behind mask: expand() relies on it)
     float sx[NB2_CHUNK], sy[NB2_CHUNK], sz[NB2_CHUNK];
 };
+static_assert(offsetof(Nb2Warp, wb) == sizeof(unsigned) * NB2_WORDS * TILE, "wb directly behind mask");
 
 // Sign bits of four fl(r2 - R2) into the mask, oldest candidate in the highest bit.
 __device__ __forceinline__ unsigned push4(unsigned m, float2 a, float2 b) {
@@ -156,27 +158,30 @@ k_nbr_build2(Geom g, const float4 *__restrict__ spos, const int *__restrict__ ce
             auto expand = [&]() {
                 __syncwarp();
                 const int nit = warp_max(nhit);
-                int w = 0;
-                unsigned word = myw > 0 ? W.mask[0][lane] : 0u;      // stored words are non-zero
-                int wbv = myw > 0 ? W.wb[0][lane] : 0;
+                // a lane's hits are its first nhit iterations (its stored words are non-zero and taken in
+                // order), of which the first `room` fit its column
+                const int keep = min(nhit, max(cap - cnt, 0));
+                const unsigned *pm = &W.mask[0][lane];               // my current word; its slot base sits
+                constexpr int WB = (int)(sizeof(W.mask) / sizeof(unsigned));     // WB entries further on
+                const unsigned *pend = &W.mask[NB2_WORDS - 1][lane];
+                unsigned word = pm[0];
+                int wbv = (int)pm[WB];
                 int *optr = outp + (size_t)min(cnt, cap) * TILE;
                 for (int it = 0; it < nit; ++it) {
-                    const bool has = word != 0u;
                     const int bit = __clz(word) & 31;
                     const int slot = wbv + bit;
                     word &= 0x7fffffffu >> bit;                    // drop that bit (all above it are 0)
-                    MD_CHECK(!has || (slot >= 0 && slot < g.n && slot != s));
-                    MD_CHECK(!(has && cnt < cap) || (optr >= outp && optr < outp + (size_t)cap * TILE));
-                    if (has && cnt < cap) *optr = MAPPED ? map[slot] : slot;
-                    optr += (has && cnt < cap) ? TILE : 0;
-                    cnt += has ? 1 : 0;
-                    if (word == 0u && w + 1 < myw) {               // my next word
-                        ++w;
-                        MD_CHECK(w < NB2_WORDS);
-                        word = W.mask[w][lane];
-                        wbv = W.wb[w][lane];
+                    MD_CHECK(!(it < nhit) || (slot >= 0 && slot < g.n && slot != s));
+                    MD_CHECK(!(it < keep) || (optr >= outp && optr < outp + (size_t)cap * TILE));
+                    if (it < keep) *optr = MAPPED ? map[slot] : slot;
+                    optr += TILE;
+                    if (word == 0u) {                              // my next word (beyond my last one: anything)
+                        pm = pm < pend ? pm + TILE : pm;
+                        word = pm[0];
+                        wbv = (int)pm[WB];
                     }
                 }
+                cnt += nhit;
                 __syncwarp();
                 myw = 0; nhit = 0;
             };
