@@ -118,6 +118,7 @@ int md_destroy(md_system *sys);
  *                          1 appends them to per-lane shared-memory columns (first design)
  *   "cell_coop"            1: the cell list as ONE cooperative launch (grid barriers between its phases), 0: five
  *                          kernels; default 1 up to 65,536 particles (where it is faster), else 0.  Same results.
+ *                          (The step loops use the cooperative form on their own account, "rebuild_flagged".)
  *   "use_graph"            0: the step calls launch their kernels directly instead of CUDA graphs -- the same
  *                          kernels in the same order (so a profiler lists them one by one); the rebuild kernels
  *                          are then launched every step and return at once while the step's device flag is 0
