@@ -433,8 +433,9 @@ k_force32(Geom g, Pair pp, Pair32 p32, const float4 *__restrict__ pos,
             int mc = ld_volatile(book.status + 1);
             if (mc > book.stats[3]) book.stats[3] = mc;
             if (ld_volatile(book.status) && book.stats[2] < 0) book.stats[2] = book.stats[0];
-            *book.flag = 0;
+            if (!book.clear) *book.flag = 0;
         }
+        if (book.clear) *book.clear = 0;
         book.stats[0] += 1;
     }
 }

@@ -67,9 +67,17 @@ struct Book {
     const int *skip;
     int *stop;
     int *done;
+    // the two force launches of a forked step (md.cu run_fused_direct): the one on the main branch has
+    // skip = the step's flag, the one behind the rebuild on the side branch only_if = that flag, so exactly one
+    // of them runs; neither clears the flag the other may still have to read: they clear `clear`, the flag
+    // word of the step before, instead
+    const int *only_if;
+    int *clear;
 };
-// true: this launch must not touch the state (a rank's list is stale and the host has not rebuilt yet)
+// true: this launch must not touch the state (a rank's list is stale and the host has not rebuilt yet; or
+// the other force launch of a forked step is the one that runs)
 __device__ __forceinline__ bool book_skips(const Book &book, int gid) {
+    if (book.only_if && !ld_volatile(book.only_if)) return true;
     if (!book.skip || !ld_volatile(book.skip)) return false;
     if (gid == 0 && book.stop) *book.stop = 1;
     return true;
@@ -1024,8 +1032,9 @@ __device__ __forceinline__ void force_epilogue(const Pair &pp, const Acc64 &acc,
             int mc = ld_volatile(book.status + 1);
             if (mc > book.stats[3]) book.stats[3] = mc;
             if (ld_volatile(book.status) && book.stats[2] < 0) book.stats[2] = book.stats[0];
-            *book.flag = 0;
+            if (!book.clear) *book.flag = 0;
         }
+        if (book.clear) *book.clear = 0;
         book.stats[0] += 1;
     }
 }

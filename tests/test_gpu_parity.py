@@ -1037,6 +1037,26 @@ def test_rebuild_as_flagged_launches_or_if_node_same_bits(B, W, ci, steps, resor
     for x, y in zip(out[0], out[1]):
         assert torch.equal(x, y)
     assert int(out[0][4][0]) == steps and int(out[0][4][1]) >= 3
+    if w.dim == 3 and resort:
+        # the fused loop with the flagged rebuild beside the force kernel ("step_fork", the default) or in front
+        # of it, as graphs and as plain launches on two streams, over step counts that are and are not multiples
+        # of the graph's nine steps and of the three flag words: same bits
+        for nst in (steps, 9, 10, 13):
+            res = []
+            for fork, graph in ((1, 1), (0, 1), (1, 0)):
+                S = B.System(w)
+                B.md_set_option(S.sys, "step_fork", fork)
+                B.md_set_option(S.sys, "use_graph", graph)
+                S.build(); S.compute_force(); S.step(nst); S.step(nst)
+                torch.cuda.synchronize()
+                res.append((S.pos.clone(), S.vel.clone(), S.force.clone(), S.id.clone(), S.stats.clone(),
+                            S.nbr_rows().clone(), S.nbr_count.clone()))
+                S.close()
+            for o in res[1:]:
+                for x, y in zip(res[0], o):
+                    assert torch.equal(x, y)
+            if nst == steps:
+                assert int(res[0][4][0]) == nst and int(res[0][4][1]) >= 2      # stats are per call
     if ci == 0:                                   # a rule other than NVE: Langevin through its own graphs
         res = []
         for flagged in (1, 0):
