@@ -668,6 +668,7 @@ def main():
     traffic, traffic_src = measured_traffic(args.config)
     fused = (w.kind == W.KIND_LJ and w.dim == 3)      # the configs md_nve_step runs as fused graphs
     flagged = B.md_get_option(S.sys, "rebuild_flagged") != 0.0
+    forked = B.md_get_option(S.sys, "step_fork") != 0.0
     algo_bytes = (4.0 * kbar + 68.0) * w.n          # list + count + pos + vel read, force + vel written
     achieved = algo_bytes / (force_ms_cold * 1e-3) / 1e9
     step_bytes = (4.0 * kbar + 164.0) * w.n
@@ -698,9 +699,13 @@ def main():
         # launch (graphs of 9 fused steps, then single steps; unfused configs: one per MD step)
         # + the rebuild: two flagged launches (cooperative cell list, builder) in EVERY MD step, or
         # 6 kernels (4 cell list, copy back, neighbor list) per rebuild an IF node ran
+        # (in the fused loop the flagged rebuild sits on a side branch that ends in a second launch of the force
+        # kernel: of the step's two force launches the one whose turn it is not returns at once)
         "gpu_launches": args.steps * (1 + md_steps + (md_steps // 9 + md_steps % 9 if fused else md_steps))
-                        + (2 * args.steps * md_steps if flagged else 6 * rebuilds),
-        "rebuild_in_graph": "two launches per MD step that return at once while the step's flag is 0" if flagged
+                        + ((3 if fused and forked else 2) * args.steps * md_steps if flagged else 6 * rebuilds),
+        "rebuild_in_graph": ("two launches per MD step that return at once while the step's flag is 0"
+                             + (", on a branch beside the force kernel that ends in a second, conditional force launch"
+                                if fused and forked else "")) if flagged
                             else "IF node around the rebuild's six kernels",
     }
     if build_ms is not None:
